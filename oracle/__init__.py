@@ -1,0 +1,190 @@
+"""ctypes front-end of the CPU oracle (oracle/encore_oracle.c) — TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It never imports paper_2105_08722_b200 and shares nothing with it.
+The C file is compiled on first use with gcc (OpenMP) into oracle/libencore_oracle.so.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "encore_oracle.c")
+_LIB = os.path.join(_HERE, "libencore_oracle.so")
+_lib = None
+
+CFLAGS = ["-O2", "-std=gnu11", "-fopenmp", "-ffp-contract=off", "-fcx-limited-range",
+          "-shared", "-fPIC", "-Wall"]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (gcc).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.run(["gcc", *CFLAGS, "-o", tmp, _SRC, "-lm"], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = C.CDLL(build())
+    dp = C.POINTER(C.c_double)
+    ip = C.POINTER(C.c_int)
+    lib.oracle_wigner3j.restype = C.c_double
+    lib.oracle_wigner3j.argtypes = [C.c_int] * 6
+    lib.oracle_ylm.restype = None
+    lib.oracle_ylm.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, dp, dp]
+    lib.oracle_multiplets.restype = C.c_int
+    lib.oracle_multiplets.argtypes = [C.c_int, C.c_int, C.c_int, ip]
+    lib.oracle_coupling.restype = C.c_double
+    lib.oracle_coupling.argtypes = [C.c_int, ip, ip]
+    lib.oracle_count_terms.restype = C.c_int64
+    lib.oracle_count_terms.argtypes = [C.c_int] * 4
+    lib.oracle_bin_edges.restype = None
+    lib.oracle_bin_edges.argtypes = [C.c_double, C.c_double, C.c_int, dp]
+    lib.oracle_cell_ids.restype = C.c_int
+    lib.oracle_cell_ids.argtypes = [dp, C.c_int64, C.c_double, C.c_double, C.c_int,
+                                    C.POINTER(C.c_int32), ip]
+    lib.oracle_bin_tuples.restype = C.c_int64
+    lib.oracle_bin_tuples.argtypes = [C.c_int, C.c_int, ip]
+    lib.oracle_alm.restype = C.c_int
+    lib.oracle_alm.argtypes = [dp, dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int,
+                               C.c_int, C.c_int64, C.c_int, dp, dp, C.POINTER(C.c_uint32)]
+    lib.oracle_zeta.restype = C.c_int
+    lib.oracle_zeta.argtypes = [C.c_int, dp, dp, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                C.c_int, C.c_int, C.c_int, ip, C.c_int64, C.c_int64, C.c_int64,
+                                C.c_int, dp, dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), dp]
+    lib.oracle_num_threads.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ip(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int))
+
+
+def _pos(pos):
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    assert pos.ndim == 2 and pos.shape[0] == 3, "positions are SoA (3, n)"
+    return pos
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def wigner3j(j1, j2, j3, m1, m2, m3) -> float:
+    return float(_load().oracle_wigner3j(j1, j2, j3, m1, m2, m3))
+
+
+def ylm(lmax: int, v) -> np.ndarray:
+    """Y_lm of a unit vector, complex array indexed l*l+l+m."""
+    n = (lmax + 1) ** 2
+    re, im = np.empty(n), np.empty(n)
+    _load().oracle_ylm(lmax, float(v[0]), float(v[1]), float(v[2]), _dp(re), _dp(im))
+    return re + 1j * im
+
+
+def multiplets(order: int, lmax: int, allparity: bool = False) -> np.ndarray:
+    lib = _load()
+    n = lib.oracle_multiplets(order, lmax, int(allparity), None)
+    out = np.empty((n, 2 * order - 5), dtype=np.int32)
+    lib.oracle_multiplets(order, lmax, int(allparity), _ip(out))
+    return out
+
+
+def coupling(order: int, lam, m) -> float:
+    lam = np.ascontiguousarray(lam, dtype=np.int32)
+    m = np.ascontiguousarray(m, dtype=np.int32)
+    return float(_load().oracle_coupling(order, _ip(lam), _ip(m)))
+
+
+def count_terms(order: int, lmax: int, allparity: bool = False, half: bool = False) -> int:
+    return int(_load().oracle_count_terms(order, lmax, int(allparity), int(half)))
+
+
+def bin_edges(rmin: float, rmax: float, nbins: int) -> np.ndarray:
+    e = np.empty(nbins + 1)
+    _load().oracle_bin_edges(rmin, rmax, nbins, _dp(e))
+    return e
+
+
+def bin_tuples(order: int, nbins: int) -> np.ndarray:
+    lib = _load()
+    n = lib.oracle_bin_tuples(order, nbins, None)
+    out = np.empty((n, order - 1), dtype=np.int32)
+    lib.oracle_bin_tuples(order, nbins, _ip(out))
+    return out
+
+
+def cell_ids(pos, box: float, rmax: float, sub: int):
+    """(cid int32[n], nc[3]) by the formula of reading R11."""
+    pos = _pos(pos)
+    n = pos.shape[1]
+    cid = np.empty(n, dtype=np.int32)
+    nc = np.zeros(3, dtype=np.int32)
+    rc = _load().oracle_cell_ids(_dp(pos), n, box, rmax, sub,
+                                 cid.ctypes.data_as(C.POINTER(C.c_int32)), _ip(nc))
+    assert rc == 0
+    return cid, nc
+
+
+def alm(pos, w, box, rmin, rmax, nbins, lmax, i, force_allpairs=False):
+    """(a[nbins, (lmax+1)^2] complex, counts[nbins] uint32) of primary i (eq. 35)."""
+    pos = _pos(pos)
+    n = pos.shape[1]
+    nlm = (lmax + 1) ** 2
+    re, im = np.empty((nbins, nlm)), np.empty((nbins, nlm))
+    cnt = np.zeros(nbins, dtype=np.uint32)
+    wp = None if w is None else _dp(np.ascontiguousarray(w, dtype=np.float64))
+    rc = _load().oracle_alm(_dp(pos), wp, n, box, rmin, rmax, nbins, lmax, int(i),
+                            int(force_allpairs), _dp(re), _dp(im),
+                            cnt.ctypes.data_as(C.POINTER(C.c_uint32)))
+    assert rc == 0, rc
+    return re + 1j * im, cnt
+
+
+def zeta(order, pos, w, box, rmin, rmax, nbins, lmax, *, allparity=False, bins=None,
+         prim_offset=0, prim_stride=1, force_allpairs=False, want_prim_counts=False):
+    """zeta^B_Lambda by eq. 34/35 over primaries offset, offset+stride, ...
+
+    Returns dict(zeta[nLam,nB], zeta_im, bin_counts[nbins] uint64, prim_counts or None,
+    max_imag, multiplets, bins).
+    """
+    lib = _load()
+    pos = _pos(pos)
+    n = pos.shape[1]
+    lam = multiplets(order, lmax, allparity)
+    if bins is None:
+        bt = bin_tuples(order, nbins)
+        bptr, nB = None, bt.shape[0]
+    else:
+        bt = np.ascontiguousarray(bins, dtype=np.int32).reshape(-1, order - 1)
+        bptr, nB = _ip(bt), bt.shape[0]
+    z = np.zeros((lam.shape[0], nB))
+    zi = np.zeros((lam.shape[0], nB))
+    bc = np.zeros(nbins, dtype=np.uint64)
+    pc = np.zeros((n, nbins), dtype=np.uint32) if want_prim_counts else None
+    mi = C.c_double(0.0)
+    wa = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+    rc = lib.oracle_zeta(order, _dp(pos), None if wa is None else _dp(wa), n, float(box),
+                         float(rmin), float(rmax), nbins, lmax, int(allparity), bptr, nB,
+                         int(prim_offset), int(prim_stride), int(force_allpairs), _dp(z), _dp(zi),
+                         bc.ctypes.data_as(C.POINTER(C.c_uint64)),
+                         None if pc is None else pc.ctypes.data_as(C.POINTER(C.c_uint32)),
+                         C.byref(mi))
+    if rc != 0:
+        raise ValueError(f"oracle_zeta failed with status {rc}")
+    return dict(zeta=z, zeta_im=zi, bin_counts=bc, prim_counts=pc, max_imag=mi.value,
+                multiplets=lam, bins=bt)
