@@ -1,0 +1,125 @@
+/*
+ * encore.h — C ABI of the B200-native hot path of ENCORE's O(N_g^2) NPCF estimator
+ * (arxiv 2105.08722; citations are PAPER.md line + equation / algorithm).
+ *
+ * What one encore_compute() evaluates, entirely on the GPU (sm_100a), fp64 throughout:
+ *
+ *   a^b_lm(s_i) = (1/v_b) sum_{j != i} w_j Y_lm( (r_j - s_i)^ ) Theta^b(|r_j - s_i|)        eq. 35
+ *   zeta^B_Lam  = (1/V) sum_i w_i sum_M E(Lam) C^Lam_M prod_k a^{b_k}_{l_k m_k}(s_i)          eq. 34
+ *
+ * for N = 3, 4, 5 (Lam = {l}, {l1 l2 l3}, {l1 l2 (l12) l3 l4}; eqs. 16, 18, 5/20 — PAPER.md:135, :145, :69, :157),
+ * even-parity multiplets only (real zeta), ordered distinct bins b_1 < .. < b_{N-1},
+ * using the half-sum m_{N-1} >= 0 of eq. 44.  Steps:
+ *   a1 cell assignment, a2 counting sort by cell, a3 neighbour sweep + radial binning, a4 a_lm accumulation,
+ *   a5 per-primary coupling contraction, a6 deterministic fp64 reduction over primaries.
+ *
+ * Conventions fixed here (DESIGN.md §3 lists every reading of the paper):
+ *   - separation r_j - s_i (eq. 35); periodic minimal image per axis when box_size > 0, which requires
+ *     r_max <= box_size/2 and coordinates in [0, box_size);
+ *   - half-open bins e_b <= r < e_{b+1}, e_b = r_min + b (r_max - r_min)/nbins, decided on r^2 =
+ *     fma(dz,dz,fma(dy,dy,dx*dx)); pairs with r^2 == 0 or j == i are skipped;
+ *   - Y_lm with the Condon-Shortley phase; v_b = 4 pi/3 (e_{b+1}^3 - e_b^3); V = box_size^3, or 1 when open;
+ *   - zeta_out[iLam * n_B + iB]; Lam in nested ascending loops, last index fastest (order of PAPER.md:622 and
+ *     Alg. 3); B lexicographic, last index fastest (Alg. 3 l.9-13).
+ *
+ * Pointers marked DEVICE are CUDA device pointers valid on the current device; HOST are ordinary host
+ * pointers.  The caller owns every buffer it passes.  The plan owns its tables and scratch (grown on demand
+ * and reused across calls).  One plan must not be used from two host threads at once; distinct plans may.
+ *
+ * Every function returning int returns ENCORE_OK (0) or a negative ENCORE_E* code; nothing throws or aborts
+ * across this boundary.  After an error the contents of output buffers are unspecified.
+ * There is no CPU fallback: without a usable CUDA device encore_compute() returns ENCORE_ECUDA.
+ */
+#ifndef ENCORE_H
+#define ENCORE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct encore_plan_s encore_plan_t; /* opaque */
+
+enum {
+    ENCORE_OK = 0,
+    ENCORE_EINVAL = -1,   /* bad argument (order, bins, lmax, radii, box, n, NULL pointer) */
+    ENCORE_EDOMAIN = -2,  /* non-finite coordinate / weight, or periodic coordinate outside [0, box) */
+    ENCORE_EALLOC = -3,   /* host or device allocation failed */
+    ENCORE_ECUDA = -4,    /* a CUDA call failed; encore_last_cuda_error() has the cudaError_t */
+    ENCORE_ESTATE = -5,   /* diagnostic getter called before a successful encore_compute */
+    ENCORE_EUNSUPPORTED = -6 /* valid problem outside what this build's kernels cover (see encore_plan) */
+};
+
+/* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
+ * S(0) = 1/2, else 1), bin edges, 1/v_b, Y_lm normalisations.  Host work only; device tables are uploaded by the
+ * first encore_compute on the then-current device.
+ *   npcf_order  N in {3,4,5}
+ *   r_min,r_max 0 <= r_min < r_max
+ *   nbins       N_r >= N-1 and <= 32
+ *   lmax        0..10 for N=3; 0..6 for N=4,5 (ENCORE_EUNSUPPORTED above: the a_lm tile of 32 primaries must
+ *               fit the contraction kernel's shared memory)
+ *   box_size    > 0: periodic cube [0,L)^3 (PERIODIC mode), needs r_max <= L/2;  0: open geometry
+ */
+int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
+                double box_size);
+
+/* Run steps a1..a6 on `cuda_stream` (a cudaStream_t cast to void*, NULL = default stream).
+ *   positions DEVICE, SoA x[n] y[n] z[n] (3n doubles), read-only
+ *   weights   DEVICE, n doubles, or NULL for unit weights (negative weights allowed: D-R fields)
+ *   n         1 <= n < 2^26
+ *   zeta_out  DEVICE, encore_zeta_len(plan) doubles, written
+ * Work is enqueued on the stream; the call returns after at most two small device->host reads it needs for
+ * sizing (the bounding box in open geometry, the group count).  zeta_out is valid once the stream has drained.
+ * Inputs are validated on the device (ENCORE_EDOMAIN is reported by this call). */
+int encore_compute(encore_plan_t *plan, const double *positions, const double *weights, int64_t n,
+                   double *zeta_out, void *cuda_stream);
+
+/* Same, with HOST buffers: copies positions/weights to the device, computes, copies zeta back and
+ * synchronises.  This is the end-to-end entry bench.py times as `e2e`. */
+int encore_compute_host(encore_plan_t *plan, const double *positions, const double *weights, int64_t n,
+                        double *zeta_out);
+
+int encore_destroy(encore_plan_t *plan);
+
+/* ---- host queries (valid right after encore_plan, no GPU needed) ---- */
+int64_t encore_zeta_len(const encore_plan_t *plan);        /* n_Lambda * n_B */
+int encore_num_multiplets(const encore_plan_t *plan);      /* n_Lambda (69 for N=4,lmax=5; 204 for N=5,lmax=3) */
+int encore_num_bin_tuples(const encore_plan_t *plan);      /* n_B = C(nbins, N-1) */
+int64_t encore_num_terms(const encore_plan_t *plan);       /* non-zero (Lam, M) with m_{N-1} >= 0 (1126 for N=4,lmax=5) */
+int encore_get_multiplets(const encore_plan_t *plan, int *out /* HOST [n_Lambda][2N-5] */);
+int encore_get_bin_tuples(const encore_plan_t *plan, int *out /* HOST [n_B][N-1] */);
+int encore_get_bin_edges(const encore_plan_t *plan, double *out /* HOST [nbins+1] */);
+/* flop counts per primary of the contraction as executed (fused multiply-add = 2) and by the canonical
+ * "Algorithm 3 literal" model of SURVEY.md §8(d) (5/11/17 flop per term evaluation for N=3/4/5) */
+int encore_contraction_flops(const encore_plan_t *plan, double *executed, double *canonical);
+
+/* ---- diagnostics of the last successful encore_compute (each synchronises the compute stream) ---- */
+/* grid geometry chosen for that input: cells per axis, subdivisions S_a with cell size r_max/S_a (reading R11) */
+int encore_get_grid(const encore_plan_t *plan, int nc[3] /* HOST */, int sub[3] /* HOST */);
+int encore_get_cell_ids(const encore_plan_t *plan, int32_t *out /* DEVICE [n], input order */);
+int encore_get_bin_counts(const encore_plan_t *plan, uint64_t *counts /* HOST [nbins] */,
+                          uint64_t *pairs_total /* HOST, may be NULL */);
+int encore_get_primary_counts(const encore_plan_t *plan, uint32_t *out /* DEVICE [n][nbins], input order */);
+/* a^b_lm of input-order primary i: HOST [nbins][(lmax+1)(lmax+2)/2][2] (re,im), (l,m>=0) at l(l+1)/2+m */
+int encore_get_alm(const encore_plan_t *plan, int64_t i, double *out);
+/* stage times of that call in ms: [0] grid (cell ids + histogram), [1] sort (scan, scatter, rank, gather, groups),
+ * [2] pair (a3+a4), [3] contraction (a5), [4] reduction (a6).  Only measured when timing is enabled. */
+int encore_get_stage_ms(const encore_plan_t *plan, float ms[5]);
+int encore_set_timing(encore_plan_t *plan, int enabled);   /* record per-stage CUDA events (default off) */
+/* number of kernel launches the last encore_compute enqueued */
+int encore_get_launch_count(const encore_plan_t *plan);
+/* candidate pairs tested in step a3 by the last compute (>= accepted pairs), for the rejected-pair flop term */
+int encore_get_candidate_pairs(const encore_plan_t *plan, uint64_t *out /* HOST */);
+
+/* Dependent-DFMA-chain micro-benchmark on the current device: achieved fp64 FLOP/s (FMA = 2) with every SM busy.
+ * The ALU roofline denominator reported by bench.py beside the derived 148 SM x 64 lanes x 2 x f_clk. */
+int encore_measure_fp64_peak(double *flops_per_s /* HOST */, void *cuda_stream);
+
+const char *encore_strerror(int status);
+int encore_last_cuda_error(void); /* cudaError_t of the most recent ENCORE_ECUDA on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ENCORE_H */

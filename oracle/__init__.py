@@ -50,7 +50,7 @@ def _load():
     lib.oracle_bin_edges.restype = None
     lib.oracle_bin_edges.argtypes = [C.c_double, C.c_double, C.c_int, dp]
     lib.oracle_cell_ids.restype = C.c_int
-    lib.oracle_cell_ids.argtypes = [dp, C.c_int64, C.c_double, C.c_double, C.c_int,
+    lib.oracle_cell_ids.argtypes = [dp, C.c_int64, C.c_double, C.c_double, ip,
                                     C.POINTER(C.c_int32), ip]
     lib.oracle_bin_tuples.restype = C.c_int64
     lib.oracle_bin_tuples.argtypes = [C.c_int, C.c_int, ip]
@@ -128,13 +128,14 @@ def bin_tuples(order: int, nbins: int) -> np.ndarray:
     return out
 
 
-def cell_ids(pos, box: float, rmax: float, sub: int):
-    """(cid int32[n], nc[3]) by the formula of reading R11."""
+def cell_ids(pos, box: float, rmax: float, sub):
+    """(cid int32[n], nc[3]) by the formula of reading R11; sub = S or (S_x, S_y, S_z)."""
     pos = _pos(pos)
     n = pos.shape[1]
     cid = np.empty(n, dtype=np.int32)
     nc = np.zeros(3, dtype=np.int32)
-    rc = _load().oracle_cell_ids(_dp(pos), n, box, rmax, sub,
+    sub = np.ascontiguousarray(np.broadcast_to(np.asarray(sub, dtype=np.int32), (3,)))
+    rc = _load().oracle_cell_ids(_dp(pos), n, box, rmax, _ip(sub),
                                  cid.ctypes.data_as(C.POINTER(C.c_int32)), _ip(nc))
     assert rc == 0
     return cid, nc

@@ -269,20 +269,21 @@ void oracle_bin_edges(double rmin, double rmax, int nbins, double *e)
 
 /* ------------------------------------------------------------------------------------------
  * Cell ids (R11) — an integer side output of the hot path (step a1); the oracle's own
- * neighbour search below does not use it.  `sub` = subdivision S chosen by the plan.
- *   periodic: nc = max(1, floor(L / (rmax/S))) per axis, origin 0, extent L
- *   open    : per axis origin = min coordinate, extent = max - min, nc = max(1, floor(extent/(rmax/S)))
+ * neighbour search below does not use it.  `sub[a]` = subdivision S_a of axis a chosen by the plan (a free
+ * design parameter, R11/R23; the cell size of axis a is rmax/S_a).
+ *   periodic: nc_a = max(1, floor(L / (rmax/S_a))), origin 0, extent L
+ *   open    : per axis origin = min coordinate, extent = max - min, nc_a = max(1, floor(extent/(rmax/S_a)))
  *   inv = nc / extent (1 if extent == 0);  i = min(nc-1, (int)((x - origin) * inv));
  *   cid = (iz*nc_y + iy)*nc_x + ix
  * ------------------------------------------------------------------------------------------ */
-int oracle_cell_ids(const double *pos, int64_t n, double box, double rmax, int sub, int32_t *cid,
+int oracle_cell_ids(const double *pos, int64_t n, double box, double rmax, const int *sub, int32_t *cid,
                     int *nc_out)
 {
     const double *p[3] = {pos, pos + n, pos + 2 * n};
     double org[3], inv[3];
     int nc[3];
-    const double h = rmax / (double)sub;
     for (int a = 0; a < 3; ++a) {
+        const double h = rmax / (double)sub[a];
         double ext;
         if (box > 0.0) { org[a] = 0.0; ext = box; }
         else {

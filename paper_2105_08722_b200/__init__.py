@@ -1,0 +1,269 @@
+"""Thin Python binding of the C ABI in include/encore.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA library `libencore_b200.so`; this module loads it with
+ctypes, checks status codes and passes raw pointers (`tensor.data_ptr()`) and sizes.  PyTorch is used
+by callers for device memory and streams only.  There is no CPU fallback: if the library is missing it
+is built with nvcc (paper_2105_08722_b200/build.py); if that fails, importing raises.
+
+Functions carry the names of the C entry points: encore_plan, encore_compute, encore_compute_host,
+encore_destroy, encore_zeta_len, encore_get_* ...; `Plan` is a small RAII convenience around them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+
+# every symbol include/encore.h declares (tests check the .so exports all of them)
+SYMBOLS = [
+    "encore_plan", "encore_compute", "encore_compute_host", "encore_destroy", "encore_zeta_len",
+    "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
+    "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
+    "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
+    "encore_get_stage_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs",
+    "encore_measure_fp64_peak", "encore_strerror", "encore_last_cuda_error",
+]
+
+
+class EncoreError(RuntimeError):
+    def __init__(self, status: int):
+        self.status = status
+        msg = lib().encore_strerror(status)
+        super().__init__(f"encore status {status}: {msg.decode() if msg else '?'}")
+
+
+def lib():
+    """Load (building first if needed) the CUDA library.  Fails loudly; never falls back."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+    L.encore_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double]
+    L.encore_compute.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
+    L.encore_compute_host.argtypes = [vp, vp, vp, C.c_int64, vp]
+    L.encore_destroy.argtypes = [vp]
+    L.encore_zeta_len.argtypes = [vp]
+    L.encore_zeta_len.restype = C.c_int64
+    L.encore_num_multiplets.argtypes = [vp]
+    L.encore_num_bin_tuples.argtypes = [vp]
+    L.encore_num_terms.argtypes = [vp]
+    L.encore_num_terms.restype = C.c_int64
+    L.encore_get_multiplets.argtypes = [vp, ip]
+    L.encore_get_bin_tuples.argtypes = [vp, ip]
+    L.encore_get_bin_edges.argtypes = [vp, dp]
+    L.encore_contraction_flops.argtypes = [vp, dp, dp]
+    L.encore_get_grid.argtypes = [vp, ip, ip]
+    L.encore_get_cell_ids.argtypes = [vp, vp]
+    L.encore_get_bin_counts.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.encore_get_primary_counts.argtypes = [vp, vp]
+    L.encore_get_alm.argtypes = [vp, C.c_int64, dp]
+    L.encore_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.encore_set_timing.argtypes = [vp, C.c_int]
+    L.encore_get_launch_count.argtypes = [vp]
+    L.encore_get_candidate_pairs.argtypes = [vp, C.POINTER(C.c_uint64)]
+    L.encore_measure_fp64_peak.argtypes = [dp, vp]
+    L.encore_strerror.argtypes = [C.c_int]
+    L.encore_strerror.restype = C.c_char_p
+    L.encore_last_cuda_error.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(status: int):
+    if status != OK:
+        raise EncoreError(status)
+
+
+def _ptr(t):
+    """device/host pointer of a torch tensor, numpy array or int; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    if isinstance(t, np.ndarray):
+        return C.c_void_p(t.ctypes.data)
+    return C.c_void_p(t.data_ptr())
+
+
+# ---- the C entry points, same names ------------------------------------------------------------------
+def encore_plan(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: int, box_size: float):
+    h = C.c_void_p()
+    _check(lib().encore_plan(C.byref(h), npcf_order, r_min, r_max, nbins, lmax, box_size))
+    return h
+
+
+def encore_compute(plan, positions, weights, n: int, zeta_out, cuda_stream: int = 0):
+    """positions/weights/zeta_out: CUDA tensors (fp64, contiguous) or raw device pointers."""
+    _check(lib().encore_compute(plan, _ptr(positions), _ptr(weights), n, _ptr(zeta_out), C.c_void_p(cuda_stream)))
+
+
+def encore_compute_host(plan, positions, weights, n: int, zeta_out):
+    """positions/weights/zeta_out: host buffers (numpy arrays or CPU tensors, fp64, contiguous)."""
+    _check(lib().encore_compute_host(plan, _ptr(positions), _ptr(weights), n, _ptr(zeta_out)))
+
+
+def encore_destroy(plan):
+    _check(lib().encore_destroy(plan))
+
+
+def encore_zeta_len(plan) -> int:
+    return int(lib().encore_zeta_len(plan))
+
+
+def encore_num_multiplets(plan) -> int:
+    return int(lib().encore_num_multiplets(plan))
+
+
+def encore_num_bin_tuples(plan) -> int:
+    return int(lib().encore_num_bin_tuples(plan))
+
+
+def encore_num_terms(plan) -> int:
+    return int(lib().encore_num_terms(plan))
+
+
+def encore_get_multiplets(plan, order: int) -> np.ndarray:
+    out = np.empty((encore_num_multiplets(plan), 2 * order - 5), dtype=np.int32)
+    _check(lib().encore_get_multiplets(plan, out.ctypes.data_as(C.POINTER(C.c_int))))
+    return out
+
+
+def encore_get_bin_tuples(plan, order: int) -> np.ndarray:
+    out = np.empty((encore_num_bin_tuples(plan), order - 1), dtype=np.int32)
+    _check(lib().encore_get_bin_tuples(plan, out.ctypes.data_as(C.POINTER(C.c_int))))
+    return out
+
+
+def encore_get_bin_edges(plan, nbins: int) -> np.ndarray:
+    out = np.empty(nbins + 1)
+    _check(lib().encore_get_bin_edges(plan, out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
+def encore_contraction_flops(plan):
+    ex, ca = C.c_double(), C.c_double()
+    _check(lib().encore_contraction_flops(plan, C.byref(ex), C.byref(ca)))
+    return ex.value, ca.value
+
+
+def encore_get_grid(plan):
+    nc, sub = (C.c_int * 3)(), (C.c_int * 3)()
+    _check(lib().encore_get_grid(plan, nc, sub))
+    return list(nc), list(sub)
+
+
+def encore_get_cell_ids(plan, out):
+    _check(lib().encore_get_cell_ids(plan, _ptr(out)))
+
+
+def encore_get_bin_counts(plan, nbins: int):
+    counts = (C.c_uint64 * nbins)()
+    tot = C.c_uint64()
+    _check(lib().encore_get_bin_counts(plan, counts, C.byref(tot)))
+    return np.array(list(counts), dtype=np.uint64), int(tot.value)
+
+
+def encore_get_primary_counts(plan, out):
+    _check(lib().encore_get_primary_counts(plan, _ptr(out)))
+
+
+def encore_get_alm(plan, i: int, nbins: int, lmax: int) -> np.ndarray:
+    """complex array [nbins, (lmax+1)(lmax+2)/2], (l, m>=0) at l(l+1)/2+m."""
+    nlm = (lmax + 1) * (lmax + 2) // 2
+    out = np.empty((nbins, nlm, 2))
+    _check(lib().encore_get_alm(plan, i, out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def encore_get_stage_ms(plan):
+    ms = (C.c_float * 5)()
+    _check(lib().encore_get_stage_ms(plan, ms))
+    return dict(zip(("grid", "sort", "pair", "contraction", "reduce"), [float(v) for v in ms]))
+
+
+def encore_set_timing(plan, enabled: bool):
+    _check(lib().encore_set_timing(plan, int(enabled)))
+
+
+def encore_get_launch_count(plan) -> int:
+    v = lib().encore_get_launch_count(plan)
+    if v < 0:
+        raise EncoreError(v)
+    return v
+
+
+def encore_get_candidate_pairs(plan) -> int:
+    v = C.c_uint64()
+    _check(lib().encore_get_candidate_pairs(plan, C.byref(v)))
+    return int(v.value)
+
+
+def encore_measure_fp64_peak(cuda_stream: int = 0) -> float:
+    v = C.c_double()
+    _check(lib().encore_measure_fp64_peak(C.byref(v), C.c_void_p(cuda_stream)))
+    return v.value
+
+
+class Plan:
+    """RAII wrapper: Plan(order, r_min, r_max, nbins, lmax, box) -> .compute(pos, w) on CUDA tensors."""
+
+    def __init__(self, order, r_min, r_max, nbins, lmax, box=0.0):
+        self.order, self.r_min, self.r_max, self.nbins, self.lmax, self.box = order, r_min, r_max, nbins, lmax, box
+        self.h = encore_plan(order, r_min, r_max, nbins, lmax, box)
+        self.n_lambda = encore_num_multiplets(self.h)
+        self.n_b = encore_num_bin_tuples(self.h)
+
+    def close(self):
+        if getattr(self, "h", None) is not None:
+            encore_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    @property
+    def multiplets(self):
+        return encore_get_multiplets(self.h, self.order)
+
+    @property
+    def bin_tuples(self):
+        return encore_get_bin_tuples(self.h, self.order)
+
+    def compute(self, positions, weights=None, out=None, stream=None):
+        """positions: CUDA fp64 tensor (3, n) SoA; weights: CUDA fp64 (n,) or None; returns zeta (n_lambda, n_b)."""
+        import torch
+        assert positions.is_cuda and positions.dtype == torch.float64 and positions.is_contiguous()
+        assert positions.dim() == 2 and positions.shape[0] == 3
+        n = positions.shape[1]
+        if weights is not None:
+            assert weights.is_cuda and weights.dtype == torch.float64 and weights.is_contiguous() and weights.numel() == n
+        if out is None:
+            out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
+        st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
+        encore_compute(self.h, positions, weights, n, out, st)
+        return out
+
+    def compute_host(self, positions: np.ndarray, weights=None) -> np.ndarray:
+        positions = np.ascontiguousarray(positions, dtype=np.float64)
+        assert positions.ndim == 2 and positions.shape[0] == 3
+        n = positions.shape[1]
+        if weights is not None:
+            weights = np.ascontiguousarray(weights, dtype=np.float64)
+        out = np.empty((self.n_lambda, self.n_b))
+        encore_compute_host(self.h, positions, weights, n, out)
+        return out

@@ -1,0 +1,487 @@
+// api.cu — the C ABI of include/encore.h: plan life-cycle, the encore_compute pipeline, diagnostics.
+#include "../../include/encore.h"
+#include "device.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+namespace {
+
+thread_local int g_last_cuda = 0;
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e == cudaSuccess) cap = bytes;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <class T> T *as() const { return static_cast<T *>(p); }
+};
+
+} // namespace
+
+struct encore_plan_s {
+    HostTables T;
+    bool uploaded = false;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm;
+    // scratch
+    DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
+    DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
+    DevBuf io_pos, io_w, io_zeta;
+    double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6]
+    // state of the last compute
+    bool have = false;
+    int64_t n = 0;
+    GridGeom geom{};
+    int ngroups_max = 0;
+    cudaStream_t stream = nullptr;
+    bool timing = false;
+    cudaEvent_t ev[6] = {};
+    bool ev_ready = false;
+    float ms[5] = {0, 0, 0, 0, 0};
+    int launches = 0;
+    int sub_yz_override = 0, sub_x_override = 0;
+};
+
+namespace {
+
+#define CU(call)                                     \
+    do {                                             \
+        cudaError_t e__ = (call);                    \
+        if (e__ != cudaSuccess) {                    \
+            g_last_cuda = (int)e__;                  \
+            return e__ == cudaErrorMemoryAllocation ? ENCORE_EALLOC : ENCORE_ECUDA; \
+        }                                            \
+    } while (0)
+
+int upload_tables(encore_plan_s *P, cudaStream_t s)
+{
+    if (P->uploaded) return ENCORE_OK;
+    const HostTables &T = P->T;
+    std::vector<DevTerm> dt(T.terms.size());
+    for (size_t i = 0; i < dt.size(); ++i) {
+        for (int k = 0; k < 4; ++k) { dt[i].re[k] = T.terms[i].re[k]; dt[i].im[k] = T.terms[i].im[k]; dt[i].tau[k] = T.terms[i].tau[k]; }
+        dt[i].pad = 0;
+        dt[i].W = T.terms[i].W;
+    }
+    CU(P->d_terms.ensure(sizeof(DevTerm) * std::max<size_t>(1, dt.size())));
+    CU(P->d_term_start.ensure(sizeof(int) * T.term_start.size()));
+    CU(P->d_bin_tuples.ensure(sizeof(int) * T.bin_tuples.size()));
+    CU(P->d_ynorm.ensure(sizeof(double) * T.ynorm.size()));
+    CU(cudaMemcpyAsync(P->d_terms.p, dt.data(), sizeof(DevTerm) * dt.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(P->d_term_start.p, T.term_start.data(), sizeof(int) * T.term_start.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(P->d_bin_tuples.p, T.bin_tuples.data(), sizeof(int) * T.bin_tuples.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(P->d_ynorm.p, T.ynorm.data(), sizeof(double) * T.ynorm.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s)); // the staging vectors die at return
+    CU(cudaMallocHost((void **)&P->pinned, 8 * sizeof(double)));
+    P->uploaded = true;
+    return ENCORE_OK;
+}
+
+// DESIGN.md R11.  Per axis: h_a = r_max / sub_a, nc_a = max(1, floor(ext_a / h_a)), inv_a = nc_a / ext_a.
+// sub_y = sub_z chosen so that a pencil cross-section holds ~32 particles per pencil-width of length;
+// x is subdivided 4x finer (x-ranges of candidate pencils are culled at that granularity).
+void choose_geometry(const encore_plan_s *P, int64_t n, const double lo[3], const double hi[3], GridGeom &G)
+{
+    const HostTables &T = P->T;
+    double ext[3];
+    G.periodic = T.box > 0.0;
+    G.box = T.box; G.half = 0.5 * T.box;
+    for (int a = 0; a < 3; ++a) {
+        if (G.periodic) { G.org[a] = 0.0; ext[a] = T.box; }
+        else { G.org[a] = lo[a]; ext[a] = hi[a] - lo[a]; }
+    }
+    double vol = 1.0;
+    for (int a = 0; a < 3; ++a) vol *= std::max(ext[a], T.rmax);
+    const double rho = (double)n / vol;
+    const double h_target = std::cbrt((double)ENCORE_GROUP / rho);
+    int syz = (int)std::lround(T.rmax / h_target);
+    syz = std::max(1, std::min(8, syz));
+    if (P->sub_yz_override > 0) syz = std::min(8, P->sub_yz_override);
+    int sx = 4 * syz;
+    if (P->sub_x_override > 0) sx = P->sub_x_override;
+    for (;;) {
+        G.sub[0] = sx; G.sub[1] = syz; G.sub[2] = syz;
+        double cells = 1.0;
+        for (int a = 0; a < 3; ++a) {
+            const double h = T.rmax / (double)G.sub[a];
+            const double q = std::floor(ext[a] / h);
+            G.nc[a] = q < 1.0 ? 1 : (q > 1e9 ? 1000000000 : (int)q);
+            G.inv[a] = ext[a] > 0.0 ? (double)G.nc[a] / ext[a] : 1.0;
+            cells *= (double)G.nc[a];
+        }
+        if (cells <= 4.0e6 || sx == 1) break;
+        sx = std::max(1, sx / 2);
+    }
+    G.ncell = G.nc[0] * G.nc[1] * G.nc[2];
+    G.npencil = G.nc[1] * G.nc[2];
+}
+
+int record(encore_plan_s *P, int k, cudaStream_t s)
+{
+    if (!P->timing) return ENCORE_OK;
+    if (!P->ev_ready) {
+        for (int i = 0; i < 6; ++i) CU(cudaEventCreate(&P->ev[i]));
+        P->ev_ready = true;
+    }
+    CU(cudaEventRecord(P->ev[k], s));
+    return ENCORE_OK;
+}
+
+#define TRY(call) do { int r__ = (call); if (r__ != ENCORE_OK) return r__; } while (0)
+
+int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t n, double *zeta_out, cudaStream_t s)
+{
+    const HostTables &T = P->T;
+    P->have = false;
+    P->launches = 0;
+    TRY(upload_tables(P, s));
+
+    // ---- validation + bounding box (one small device->host read) ------------------------------------------
+    CU(P->bbox_tmp.ensure(sizeof(double) * 6 * 592));
+    CU(P->bbox.ensure(sizeof(double) * 8));
+    CU(P->flags.ensure(sizeof(int) * 2));
+    CU(launch_bbox_validate(pos, w, n, T.box, P->bbox_tmp.as<double>(), P->bbox.as<double>(), P->flags.as<int>(), s, &P->launches));
+    CU(cudaMemcpyAsync(P->pinned, P->bbox.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(P->pinned + 6, P->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    int fl[2];
+    std::memcpy(fl, P->pinned + 6, sizeof(fl));
+    if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
+    GridGeom G;
+    choose_geometry(P, n, P->pinned, P->pinned + 3, G);
+    {
+        int Ry = (int)std::floor(T.rmax * G.inv[1] + 1e-6) + 1, Rz = (int)std::floor(T.rmax * G.inv[2] + 1e-6) + 1;
+        if (!G.periodic) { Ry = std::min(Ry, G.nc[1] - 1); Rz = std::min(Rz, G.nc[2] - 1); }
+        const int wy = std::min(2 * Ry + 1, G.periodic ? G.nc[1] : 2 * Ry + 1);
+        const int wz = std::min(2 * Rz + 1, G.periodic ? G.nc[2] : 2 * Rz + 1);
+        if (2 * wy * wz > 1024) return ENCORE_EUNSUPPORTED;
+    }
+    const int ngmax = (int)(n / ENCORE_GROUP) + G.npencil + 1;
+    const int nb = T.nbins, ncomp = T.ncomp;
+    const size_t nout = (size_t)T.nLam() * T.nB();
+    const int nseg = 64;
+
+    // ---- scratch ----------------------------------------------------------------------------------------------
+    CU(P->cid.ensure(sizeof(int32_t) * n));
+    CU(P->cell_count.ensure(sizeof(int) * (size_t)G.ncell));
+    CU(P->cell_fill.ensure(sizeof(int) * (size_t)G.ncell));
+    CU(P->cell_start.ensure(sizeof(int) * ((size_t)G.ncell + 1)));
+    CU(P->scan_tmp.ensure(sizeof(int) * ((size_t)G.ncell / 2048 + 4)));
+    CU(P->tmp_idx.ensure(sizeof(int) * n));
+    CU(P->sorted_idx.ensure(sizeof(int) * n));
+    CU(P->pos4.ensure(sizeof(double4) * n));
+    CU(P->groups.ensure(sizeof(int) * (size_t)G.npencil));
+    CU(P->group_start.ensure(sizeof(int) * ((size_t)G.npencil + 1)));
+    CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
+    CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
+    CU(P->partial.ensure(sizeof(double) * (size_t)ngmax * nout));
+    CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
+    CU(P->cand.ensure(sizeof(unsigned long long)));
+
+    TRY(record(P, 0, s));
+    // ---- a1: cell ids + histogram -----------------------------------------------------------------------------
+    CU(launch_cell_ids(pos, n, G, P->cid.as<int32_t>(), P->cell_count.as<int>(), s, &P->launches));
+    TRY(record(P, 1, s));
+    // ---- a2: counting sort by cell, gather to AoS, groups of 32 per pencil ----------------------------------
+    CU(launch_exclusive_scan(P->cell_count.as<int>(), P->cell_start.as<int>(), G.ncell, P->scan_tmp.as<int>(), s, &P->launches));
+    CU(cudaMemsetAsync(P->cell_fill.p, 0, sizeof(int) * (size_t)G.ncell, s));
+    CU(launch_sort_gather(pos, w, n, P->cid.as<int32_t>(), P->cell_start.as<int>(), P->cell_fill.as<int>(), P->tmp_idx.as<int>(),
+                          P->sorted_idx.as<int>(), P->pos4.as<double4>(), s, &P->launches));
+    CU(launch_pencil_groups(P->cell_start.as<int>(), G, P->groups.as<int>(), s, &P->launches));
+    CU(launch_exclusive_scan(P->groups.as<int>(), P->group_start.as<int>(), G.npencil, P->scan_tmp.as<int>(), s, &P->launches));
+    TRY(record(P, 2, s));
+    // ---- a3 + a4: pair stage -----------------------------------------------------------------------------------
+    PairArgs pa{};
+    pa.pos4 = P->pos4.as<double4>();
+    pa.cell_start = P->cell_start.as<int>();
+    pa.group_start = P->group_start.as<int>();
+    pa.geom = G;
+    pa.bins.nbins = nb;
+    pa.bins.rmin_f = (float)T.rmin;
+    pa.bins.invw_f = (float)((double)nb / (T.rmax - T.rmin));
+    for (int b = 0; b <= nb; ++b) pa.bins.e2[b] = T.edges2[b];
+    for (int b = 0; b < nb; ++b) pa.bins.vinv[b] = T.vinv[b];
+    pa.rmax = T.rmax;
+    pa.lmax = T.lmax; pa.ncomp = ncomp;
+    pa.ynorm = P->d_ynorm.as<double>();
+    pa.alm = P->alm.as<double>();
+    pa.counts = P->counts.as<uint32_t>();
+    pa.cand_pairs = P->cand.as<unsigned long long>();
+    pa.ngroups_max = ngmax;
+    CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
+    CU(launch_pair_stage(pa, s, &P->launches));
+    TRY(record(P, 3, s));
+    // ---- a5: contraction ---------------------------------------------------------------------------------------
+    ContractArgs ca{};
+    ca.order = T.order; ca.nbins = nb; ca.ncomp = ncomp; ca.nLam = T.nLam(); ca.nB = T.nB();
+    ca.terms = P->d_terms.as<DevTerm>();
+    ca.term_start = P->d_term_start.as<int>();
+    ca.bin_tuples = P->d_bin_tuples.as<int>();
+    ca.alm = pa.alm; ca.pos4 = pa.pos4; ca.cell_start = pa.cell_start; ca.group_start = pa.group_start;
+    ca.geom = G;
+    ca.partial = P->partial.as<double>();
+    ca.partial2 = P->partial2.as<double>();
+    ca.nseg = nseg;
+    ca.vinv_total = T.box > 0.0 ? 1.0 / (T.box * T.box * T.box) : 1.0; // DESIGN.md R12
+    ca.zeta_out = zeta_out;
+    ca.ngroups_max = ngmax;
+    CU(launch_contraction(ca, s, &P->launches));
+    TRY(record(P, 4, s));
+    // ---- a6: reduction -----------------------------------------------------------------------------------------
+    CU(launch_reduction(ca, s, &P->launches));
+    TRY(record(P, 5, s));
+
+    P->have = true; P->n = n; P->geom = G; P->ngroups_max = ngmax; P->stream = s;
+    return ENCORE_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax, double box_size)
+{
+    if (!plan_out) return ENCORE_EINVAL;
+    *plan_out = nullptr;
+    if (npcf_order < 3 || npcf_order > ENCORE_MAX_ORDER) return ENCORE_EINVAL;
+    if (!(r_min >= 0.0) || !(r_max > r_min) || !std::isfinite(r_max)) return ENCORE_EINVAL;
+    if (nbins < npcf_order - 1 || nbins > ENCORE_MAX_BINS) return ENCORE_EINVAL;
+    if (lmax < 0 || !std::isfinite(box_size) || box_size < 0.0) return ENCORE_EINVAL;
+    if (box_size > 0.0 && r_max > 0.5 * box_size) return ENCORE_EINVAL;
+    if (lmax > ENCORE_MAX_LMAX) return ENCORE_EUNSUPPORTED;
+    if (npcf_order >= 4 && lmax > 6) return ENCORE_EUNSUPPORTED;
+    encore_plan_s *P = new (std::nothrow) encore_plan_s();
+    if (!P) return ENCORE_EALLOC;
+    try {
+        encore_build_tables(P->T, npcf_order, r_min, r_max, nbins, lmax, box_size);
+    } catch (...) {
+        delete P;
+        return ENCORE_EALLOC;
+    }
+    if (const char *e = std::getenv("ENCORE_SUB_YZ")) P->sub_yz_override = std::atoi(e);
+    if (const char *e = std::getenv("ENCORE_SUB_X")) P->sub_x_override = std::atoi(e);
+    *plan_out = P;
+    return ENCORE_OK;
+}
+
+int encore_compute(encore_plan_t *P, const double *positions, const double *weights, int64_t n, double *zeta_out, void *cuda_stream)
+{
+    if (!P || !positions || !zeta_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
+    return compute_device(P, positions, weights, n, zeta_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int encore_compute_host(encore_plan_t *P, const double *positions, const double *weights, int64_t n, double *zeta_out)
+{
+    if (!P || !positions || !zeta_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
+    const size_t nout = (size_t)encore_zeta_len(P);
+    CU(P->io_pos.ensure(sizeof(double) * 3 * (size_t)n));
+    if (weights) CU(P->io_w.ensure(sizeof(double) * (size_t)n));
+    CU(P->io_zeta.ensure(sizeof(double) * nout));
+    cudaStream_t s = nullptr;
+    CU(cudaMemcpyAsync(P->io_pos.p, positions, sizeof(double) * 3 * (size_t)n, cudaMemcpyHostToDevice, s));
+    if (weights) CU(cudaMemcpyAsync(P->io_w.p, weights, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, s));
+    TRY(compute_device(P, P->io_pos.as<double>(), weights ? P->io_w.as<double>() : nullptr, n, P->io_zeta.as<double>(), s));
+    CU(cudaMemcpyAsync(zeta_out, P->io_zeta.p, sizeof(double) * nout, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return ENCORE_OK;
+}
+
+int encore_destroy(encore_plan_t *P)
+{
+    if (!P) return ENCORE_EINVAL;
+    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->cid, &P->cell_count, &P->cell_fill,
+                      &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
+                      &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
+                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta};
+    for (DevBuf *b : bufs) b->release();
+    if (P->pinned) cudaFreeHost(P->pinned);
+    if (P->ev_ready) for (int i = 0; i < 6; ++i) cudaEventDestroy(P->ev[i]);
+    delete P;
+    return ENCORE_OK;
+}
+
+int64_t encore_zeta_len(const encore_plan_t *P) { return P ? (int64_t)P->T.nLam() * P->T.nB() : ENCORE_EINVAL; }
+int encore_num_multiplets(const encore_plan_t *P) { return P ? P->T.nLam() : ENCORE_EINVAL; }
+int encore_num_bin_tuples(const encore_plan_t *P) { return P ? P->T.nB() : ENCORE_EINVAL; }
+int64_t encore_num_terms(const encore_plan_t *P) { return P ? (int64_t)P->T.terms.size() : ENCORE_EINVAL; }
+
+int encore_get_multiplets(const encore_plan_t *P, int *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    std::memcpy(out, P->T.multiplets.data(), sizeof(int) * P->T.multiplets.size());
+    return ENCORE_OK;
+}
+
+int encore_get_bin_tuples(const encore_plan_t *P, int *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    std::memcpy(out, P->T.bin_tuples.data(), sizeof(int) * P->T.bin_tuples.size());
+    return ENCORE_OK;
+}
+
+int encore_get_bin_edges(const encore_plan_t *P, double *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    std::memcpy(out, P->T.edges.data(), sizeof(double) * P->T.edges.size());
+    return ENCORE_OK;
+}
+
+int encore_contraction_flops(const encore_plan_t *P, double *executed, double *canonical)
+{
+    if (!P) return ENCORE_EINVAL;
+    const double evals = (double)P->T.terms.size() * (double)P->T.nB();
+    const int N = P->T.order;
+    if (executed) *executed = evals * (6.0 * (N - 1) + 1.0); // generic kernel: N-1 complex multiplies + 1 add per term
+    if (canonical) *canonical = evals * (N == 3 ? 5.0 : N == 4 ? 11.0 : 17.0);
+    return ENCORE_OK;
+}
+
+int encore_get_grid(const encore_plan_t *P, int nc[3], int sub[3])
+{
+    if (!P || !nc || !sub) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    for (int a = 0; a < 3; ++a) { nc[a] = P->geom.nc[a]; sub[a] = P->geom.sub[a]; }
+    return ENCORE_OK;
+}
+
+int encore_get_cell_ids(const encore_plan_t *P, int32_t *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    CU(cudaMemcpyAsync(out, P->cid.p, sizeof(int32_t) * (size_t)P->n, cudaMemcpyDeviceToDevice, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    return ENCORE_OK;
+}
+
+int encore_get_bin_counts(const encore_plan_t *Pc, uint64_t *counts, uint64_t *pairs_total)
+{
+    encore_plan_t *P = const_cast<encore_plan_t *>(Pc);
+    if (!P || !counts) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    const int nb = P->T.nbins;
+    CU(P->bincounts.ensure(sizeof(unsigned long long) * ENCORE_MAX_BINS));
+    CU(launch_sum_bin_counts(P->counts.as<uint32_t>(), P->group_start.as<int>(), P->geom.npencil, nb,
+                             P->bincounts.as<unsigned long long>(), P->ngroups_max, P->stream));
+    unsigned long long h[ENCORE_MAX_BINS];
+    CU(cudaMemcpyAsync(h, P->bincounts.p, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    uint64_t tot = 0;
+    for (int b = 0; b < nb; ++b) { counts[b] = h[b]; tot += h[b]; }
+    if (pairs_total) *pairs_total = tot;
+    return ENCORE_OK;
+}
+
+int encore_get_primary_counts(const encore_plan_t *P, uint32_t *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    CU(launch_export_primary_counts(P->counts.as<uint32_t>(), P->cid.as<int32_t>(), P->sorted_idx.as<int>(), P->cell_start.as<int>(),
+                                    P->group_start.as<int>(), P->geom, P->T.nbins, P->n, out, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    return ENCORE_OK;
+}
+
+int encore_get_alm(const encore_plan_t *Pc, int64_t i, double *out)
+{
+    encore_plan_t *P = const_cast<encore_plan_t *>(Pc);
+    if (!P || !out) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    if (i < 0 || i >= P->n) return ENCORE_EINVAL;
+    const int lmax = P->T.lmax, nb = P->T.nbins;
+    const size_t cnt = (size_t)nb * (lmax + 1) * (lmax + 2);
+    CU(P->alm_export.ensure(sizeof(double) * cnt));
+    CU(launch_export_alm(P->alm.as<double>(), P->cid.as<int32_t>(), P->sorted_idx.as<int>(), P->cell_start.as<int>(),
+                         P->group_start.as<int>(), P->geom, nb, lmax, P->n, i, P->alm_export.as<double>(), P->stream));
+    CU(cudaMemcpyAsync(out, P->alm_export.p, sizeof(double) * cnt, cudaMemcpyDeviceToHost, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    return ENCORE_OK;
+}
+
+int encore_get_stage_ms(const encore_plan_t *Pc, float ms[5])
+{
+    encore_plan_t *P = const_cast<encore_plan_t *>(Pc);
+    if (!P || !ms) return ENCORE_EINVAL;
+    if (!P->have || !P->timing || !P->ev_ready) return ENCORE_ESTATE;
+    CU(cudaEventSynchronize(P->ev[5]));
+    for (int k = 0; k < 5; ++k) CU(cudaEventElapsedTime(&ms[k], P->ev[k], P->ev[k + 1]));
+    return ENCORE_OK;
+}
+
+int encore_set_timing(encore_plan_t *P, int enabled)
+{
+    if (!P) return ENCORE_EINVAL;
+    P->timing = enabled != 0;
+    return ENCORE_OK;
+}
+
+int encore_get_launch_count(const encore_plan_t *P)
+{
+    if (!P) return ENCORE_EINVAL;
+    return P->have ? P->launches : ENCORE_ESTATE;
+}
+
+int encore_get_candidate_pairs(const encore_plan_t *P, uint64_t *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    unsigned long long h = 0;
+    CU(cudaMemcpyAsync(&h, P->cand.p, sizeof(h), cudaMemcpyDeviceToHost, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    *out = h;
+    return ENCORE_OK;
+}
+
+int encore_measure_fp64_peak(double *flops_per_s, void *cuda_stream)
+{
+    if (!flops_per_s) return ENCORE_EINVAL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    double *sink = nullptr;
+    CU(cudaMalloc((void **)&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int iters = 4096;
+    CU(launch_fp64_peak(sink, 256, s)); // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        CU(cudaEventRecord(e0, s));
+        CU(launch_fp64_peak(sink, iters, s));
+        CU(cudaEventRecord(e1, s));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    const double fmas = 148.0 * 4 * 512 * (double)iters * 16 * 8;
+    *flops_per_s = 2.0 * fmas / (best * 1e-3);
+    return ENCORE_OK;
+}
+
+const char *encore_strerror(int status)
+{
+    switch (status) {
+    case ENCORE_OK: return "ok";
+    case ENCORE_EINVAL: return "invalid argument";
+    case ENCORE_EDOMAIN: return "input outside the domain (non-finite value, or periodic coordinate outside [0, box))";
+    case ENCORE_EALLOC: return "allocation failed";
+    case ENCORE_ECUDA: return cudaGetErrorString((cudaError_t)g_last_cuda);
+    case ENCORE_ESTATE: return "no successful encore_compute to report on (or timing disabled)";
+    case ENCORE_EUNSUPPORTED: return "configuration not covered by this build's kernels";
+    default: return "unknown status";
+    }
+}
+
+int encore_last_cuda_error(void) { return g_last_cuda; }
+
+} // extern "C"

@@ -1,0 +1,109 @@
+// device.cuh — structures passed to the CUDA stages and their launch entry points.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "common.h"
+
+// Uniform grid (R11): per axis a, cell size ~ r_max / sub[a]; x is the fast (fine) axis so that a
+// "pencil" (iy,iz) is one contiguous run of the cell-sorted particle array.
+struct GridGeom {
+    double org[3];
+    double inv[3];      // cells per unit length
+    int nc[3];
+    int sub[3];
+    int periodic;
+    double box, half;
+    int ncell, npencil;
+};
+
+struct DevTerm {        // device image of HostTerm (32 bytes)
+    short re[4];
+    short im[4];
+    signed char tau[4];
+    int pad;
+    double W;
+};
+
+struct BinTable {       // passed by value (kernel parameter space -> constant bank)
+    int nbins;
+    float rmin_f, invw_f;       // fp32 first guess of the bin; the decision itself is fp64 on e2[]
+    double e2[ENCORE_MAX_BINS + 1];
+    double vinv[ENCORE_MAX_BINS];
+};
+
+// ---- grid.cu --------------------------------------------------------------------------------------------
+// bbox[0..5] = min xyz, max xyz; flags[0] != 0 if a coordinate/weight is non-finite, flags[1] != 0 if a
+// periodic coordinate is outside [0, box)
+cudaError_t launch_bbox_validate(const double *pos, const double *w, int64_t n, double box, double *bbox_tmp,
+                                 double *bbox_out, int *flags, cudaStream_t s, int *launches);
+cudaError_t launch_cell_ids(const double *pos, int64_t n, GridGeom g, int32_t *cid, int *cell_count,
+                            cudaStream_t s, int *launches);
+// exclusive scan of `in[0..m)` into `out[0..m]` (out[m] = total); tmp needs (m/2048+2) ints; m <= 2048*2048
+cudaError_t launch_exclusive_scan(const int *in, int *out, int m, int *tmp, cudaStream_t s, int *launches);
+cudaError_t launch_sort_gather(const double *pos, const double *w, int64_t n, const int32_t *cid,
+                               const int *cell_start, int *cell_fill, int *tmp_idx, int *sorted_idx,
+                               double4 *pos4, cudaStream_t s, int *launches);
+cudaError_t launch_pencil_groups(const int *cell_start, GridGeom g, int *groups_per_pencil, cudaStream_t s,
+                                 int *launches);
+
+// ---- pair.cu --------------------------------------------------------------------------------------------
+struct PairArgs {
+    const double4 *pos4;        // cell-sorted {x,y,z,w}
+    const int *cell_start;      // [ncell+1]
+    const int *group_start;     // [npencil+1]; group_start[npencil] = number of groups
+    GridGeom geom;
+    BinTable bins;
+    double rmax;
+    int lmax, ncomp;
+    const double *ynorm;        // [ncomp] device
+    double *alm;                // [ngroups][ncomp][nbins][32]
+    uint32_t *counts;           // [ngroups][nbins][32]
+    unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)
+    int ngroups_max;
+};
+cudaError_t launch_pair_stage(const PairArgs &a, cudaStream_t s, int *launches);
+int pair_stage_supported(int lmax, int nbins);
+
+// ---- contract.cu ----------------------------------------------------------------------------------------
+struct ContractArgs {
+    int order, nbins, ncomp, nLam, nB;
+    const DevTerm *terms;       // device
+    const int *term_start;      // device [nLam+1]
+    const int *bin_tuples;      // device [nB][order-1]
+    const double *alm;
+    const double4 *pos4;
+    const int *cell_start;
+    const int *group_start;
+    GridGeom geom;
+    double *partial;            // [ngroups_max][nout]
+    double *partial2;           // [nseg][nout]
+    int nseg;
+    double vinv_total;          // 1/V
+    double *zeta_out;
+    int ngroups_max;
+};
+cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
+cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
+
+// ---- diag.cu --------------------------------------------------------------------------------------------
+cudaError_t launch_sum_bin_counts(const uint32_t *counts, const int *group_start, int npencil, int nbins,
+                                  unsigned long long *out, int ngroups_max, cudaStream_t s);
+cudaError_t launch_export_primary_counts(const uint32_t *counts, const int32_t *cid, const int *sorted_idx,
+                                         const int *cell_start, const int *group_start, GridGeom g, int nbins,
+                                         int64_t n, uint32_t *out, cudaStream_t s);
+cudaError_t launch_export_alm(const double *alm, const int32_t *cid, const int *sorted_idx, const int *cell_start,
+                              const int *group_start, GridGeom g, int nbins, int lmax, int64_t n, int64_t i,
+                              double *out_dev, cudaStream_t s);
+cudaError_t launch_fp64_peak(double *sink, int iters, cudaStream_t s);
+
+// locate the group of cell-sorted slot `s` (shared by diag and contraction kernels)
+__device__ __forceinline__ int find_pencil_of_group(const int *group_start, int npencil, int g)
+{
+    int lo = 0, hi = npencil; // invariant: group_start[lo] <= g < group_start[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (group_start[mid] <= g) lo = mid; else hi = mid;
+    }
+    return lo;
+}

@@ -1,0 +1,196 @@
+// tables.cpp — host-side plan tables of the ENCORE hot path (step a0 of SURVEY.md §8(a)).
+// Multiplets Lambda, ordered bin tuples, the non-zero coupling terms of the
+// half-sum eq. 44 with C^Lam_M from eq. 5 (N=3: eq. 16, N=4: eq. 18),
+// bin edges / volumes and the Y_lm normalisations.  Plain C++, no CUDA, no Python;
+// the paper precomputes these with sympy — here they are built at plan time.
+#include "common.h"
+
+#include <cmath>
+#include <cstdlib>
+
+namespace {
+
+const long double kPi = 3.14159265358979323846264338327950288L;
+
+long double fact(int n)
+{
+    static long double tab[64];
+    static bool ready = false;
+    if (!ready) {
+        tab[0] = 1.0L;
+        for (int i = 1; i < 64; ++i) tab[i] = tab[i - 1] * (long double)i;
+        ready = true;
+    }
+    return tab[n];
+}
+
+} // namespace
+
+// Wigner 3-j by Racah's single sum (textbook form with factorials, long double throughout).
+double encore_host_wigner3j(int j1, int j2, int j3, int m1, int m2, int m3)
+{
+    if (m1 + m2 + m3 != 0) return 0.0;
+    if (std::abs(m1) > j1 || std::abs(m2) > j2 || std::abs(m3) > j3) return 0.0;
+    if (j3 > j1 + j2 || j3 < std::abs(j1 - j2)) return 0.0;
+    const int kmin = std::max(0, std::max(j2 - j3 - m1, j1 - j3 + m2));
+    const int kmax = std::min(j1 + j2 - j3, std::min(j1 - m1, j2 + m2));
+    long double s = 0.0L;
+    for (int k = kmin; k <= kmax; ++k) {
+        long double den = fact(k) * fact(j1 + j2 - j3 - k) * fact(j1 - m1 - k) * fact(j2 + m2 - k) *
+                          fact(j3 - j2 + m1 + k) * fact(j3 - j1 - m2 + k);
+        s += ((k & 1) ? -1.0L : 1.0L) / den;
+    }
+    long double tri = fact(j1 + j2 - j3) * fact(j1 - j2 + j3) * fact(-j1 + j2 + j3) / fact(j1 + j2 + j3 + 1);
+    long double pre = tri * fact(j1 + m1) * fact(j1 - m1) * fact(j2 + m2) * fact(j2 - m2) * fact(j3 + m3) *
+                      fact(j3 - m3);
+    long double v = std::sqrt(pre) * s;
+    if ((j1 - j2 - m3) & 1) v = -v;
+    return (double)v;
+}
+
+namespace {
+
+// E(Lam) C^Lam_M for principal m's `m` (sum = 0).  Intermediates of N=5 are NOT capped at lmax (R5).
+double coupling(int order, const int *lam, const int *m)
+{
+    if (order == 3) {
+        const int l = lam[0];
+        return (((l - m[0]) & 1) ? -1.0 : 1.0) / std::sqrt(2.0 * l + 1.0); // eq. 16; E = (-1)^{2l} = 1
+    }
+    if (order == 4) { // eq. 18: C = (-1)^{l1+l2+l3} (3j); times E = same sign -> plain 3j
+        return encore_host_wigner3j(lam[0], lam[1], lam[2], m[0], m[1], m[2]);
+    }
+    // eq. 5 for N=5: C = E sqrt(2 l12+1) sum_{m12} (-1)^{l12-m12} (l1 l2 l12; m1 m2 -m12)(l12 l3 l4; m12 m3 m4);
+    // only m12 = m1+m2 survives; E*E = 1.
+    const int l1 = lam[0], l2 = lam[1], l12 = lam[2], l3 = lam[3], l4 = lam[4];
+    const int m12 = m[0] + m[1];
+    if (std::abs(m12) > l12) return 0.0;
+    double v = encore_host_wigner3j(l1, l2, l12, m[0], m[1], -m12) * encore_host_wigner3j(l12, l3, l4, m12, m[2], m[3]);
+    if ((l12 - m12) & 1) v = -v;
+    return std::sqrt(2.0 * l12 + 1.0) * v;
+}
+
+void enumerate_multiplets(HostTables &t)
+{
+    const int L = t.lmax;
+    if (t.order == 3) {
+        for (int l = 0; l <= L; ++l) t.multiplets.push_back(l);
+    } else if (t.order == 4) {
+        for (int l1 = 0; l1 <= L; ++l1)
+            for (int l2 = 0; l2 <= L; ++l2)
+                for (int l3 = std::abs(l1 - l2); l3 <= std::min(l1 + l2, L); ++l3)
+                    if (((l1 + l2 + l3) & 1) == 0) { // even parity only
+                        t.multiplets.push_back(l1); t.multiplets.push_back(l2); t.multiplets.push_back(l3);
+                    }
+    } else {
+        for (int l1 = 0; l1 <= L; ++l1)
+            for (int l2 = 0; l2 <= L; ++l2)
+                for (int l12 = std::abs(l1 - l2); l12 <= l1 + l2; ++l12)
+                    for (int l3 = 0; l3 <= L; ++l3)
+                        for (int l4 = std::abs(l12 - l3); l4 <= std::min(l12 + l3, L); ++l4)
+                            if (((l1 + l2 + l3 + l4) & 1) == 0) {
+                                const int row[5] = {l1, l2, l12, l3, l4};
+                                t.multiplets.insert(t.multiplets.end(), row, row + 5);
+                            }
+    }
+}
+
+void enumerate_bins(HostTables &t)
+{
+    const int k = t.order - 1;
+    int b[4];
+    for (int i = 0; i < k; ++i) b[i] = i;
+    for (;;) {
+        t.bin_tuples.insert(t.bin_tuples.end(), b, b + k);
+        int i = k - 1;
+        while (i >= 0 && b[i] == t.nbins - k + i) --i;
+        if (i < 0) break;
+        ++b[i];
+        for (int j = i + 1; j < k; ++j) b[j] = b[j - 1] + 1;
+    }
+}
+
+void enumerate_terms(HostTables &t)
+{
+    const int nm = t.order - 1;
+    const int nL = t.nLam();
+    t.term_start.assign(1, 0);
+    for (int iL = 0; iL < nL; ++iL) {
+        const int *lam = &t.multiplets[(size_t)iL * t.width];
+        int l[4];
+        if (t.order == 3) { l[0] = l[1] = lam[0]; }
+        else if (t.order == 4) { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[2]; }
+        else { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[3]; l[3] = lam[4]; }
+        int m[4];
+        for (int k = 0; k < nm - 1; ++k) m[k] = -l[k];
+        for (;;) {
+            int s = 0;
+            for (int k = 0; k < nm - 1; ++k) s += m[k];
+            m[nm - 1] = -s;
+            if (m[nm - 1] >= 0 && m[nm - 1] <= l[nm - 1]) { // half-sum: m_{N-1} >= 0, weight 2 S(m)
+                const double c = coupling(t.order, lam, m);
+                if (std::fabs(c) > 1e-15) {
+                    HostTerm ht{};
+                    double W = (m[nm - 1] == 0 ? 1.0 : 2.0) * c;
+                    for (int k = 0; k < nm; ++k) {
+                        const int am = std::abs(m[k]);
+                        ht.re[k] = (int16_t)comp_re(l[k], am);
+                        ht.im[k] = (int16_t)comp_im(l[k], am);
+                        ht.tau[k] = 1;
+                        if (m[k] < 0) { // a_{l,-m} = (-1)^m conj(a_lm)
+                            ht.tau[k] = -1;
+                            if (am & 1) W = -W;
+                        }
+                    }
+                    for (int k = nm; k < 4; ++k) { ht.re[k] = 0; ht.im[k] = -1; ht.tau[k] = 1; }
+                    ht.W = W;
+                    t.terms.push_back(ht);
+                }
+            }
+            int k = nm - 2;
+            while (k >= 0 && ++m[k] > l[k]) { m[k] = -l[k]; --k; }
+            if (k < 0) break;
+        }
+        t.term_start.push_back((int)t.terms.size());
+    }
+}
+
+} // namespace
+
+int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box)
+{
+    t = HostTables();
+    t.order = order; t.nbins = nbins; t.lmax = lmax; t.rmin = rmin; t.rmax = rmax; t.box = box;
+    t.width = 2 * order - 5;
+    t.ncomp = (lmax + 1) * (lmax + 1);
+    enumerate_multiplets(t);
+    enumerate_bins(t);
+    enumerate_terms(t);
+    // bins: e_b = r_min + b * width, e_nbins = r_max (R8)
+    const double wdt = (rmax - rmin) / (double)nbins;
+    t.edges.resize(nbins + 1);
+    for (int b = 0; b < nbins; ++b) t.edges[b] = rmin + (double)b * wdt;
+    t.edges[nbins] = rmax;
+    t.edges2.resize(nbins + 1);
+    for (int b = 0; b <= nbins; ++b) t.edges2[b] = t.edges[b] * t.edges[b];
+    t.vinv.resize(nbins);
+    for (int b = 0; b < nbins; ++b) { // v_b = 4 pi/3 (e_{b+1}^3 - e_b^3)
+        long double hi = t.edges[b + 1], lo = t.edges[b];
+        t.vinv[b] = (double)(1.0L / (4.0L * kPi / 3.0L * (hi * hi * hi - lo * lo * lo)));
+    }
+    // Y_lm = (-1)^m N_lm P_l^m(z) e^{i m phi},  P_l^m = k_lm (1-z^2)^{m/2} p_lm(z) with p_lm monic in z, so
+    // Y_lm = ynorm * p_lm(z) (x+iy)^m,  k_mm = (2m-1)!!,  k_lm = k_{l-1,m} (2l-1)/(l-m).
+    t.ynorm.assign(t.ncomp, 0.0);
+    for (int m = 0; m <= lmax; ++m) {
+        long double k = 1.0L;
+        for (int i = 1; i <= m; ++i) k *= (long double)(2 * i - 1);
+        for (int l = m; l <= lmax; ++l) {
+            if (l > m) k *= (long double)(2 * l - 1) / (long double)(l - m);
+            long double N = std::sqrt((2 * l + 1) / (4.0L * kPi) * fact(l - m) / fact(l + m));
+            double v = (double)(((m & 1) ? -1.0L : 1.0L) * N * k);
+            t.ynorm[comp_re(l, m)] = v;
+            if (m > 0) t.ynorm[comp_im(l, m)] = v;
+        }
+    }
+    return 0;
+}

@@ -1,0 +1,93 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/encore.h declares, validates
+arguments, and its host-built plan tables agree with the paper's printed counts and with the oracle's
+enumeration.  No compute call is made here (no GPU)."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+import paper_2105_08722_b200 as E
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_functions():
+    txt = open(os.path.join(ROOT, "include", "encore.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(encore_[a-z0-9_]+)\s*\(", txt)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = E.lib()
+    names = header_functions()
+    assert set(names) == set(E.SYMBOLS)
+    for n in names:
+        assert hasattr(lib, n), n
+    out = subprocess.run(["nm", "-D", "--defined-only", E._build.LIB], capture_output=True, text=True, check=True).stdout
+    exported = set(re.findall(r" T (encore_[a-z0-9_]+)", out))
+    assert set(names) <= exported
+
+
+def test_library_is_sm100a_and_has_no_oracle_link():
+    out = subprocess.run(["cuobjdump", "-lelf", E._build.LIB], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    ldd = subprocess.run(["ldd", E._build.LIB], capture_output=True, text=True).stdout
+    assert "oracle" not in ldd
+
+
+def test_plan_argument_validation():
+    lib = E.lib()
+    h = C.c_void_p()
+    bad = [
+        (2, 0.0, 100.0, 5, 2, 0.0), (6, 0.0, 100.0, 5, 2, 0.0),      # order
+        (3, -1.0, 100.0, 5, 2, 0.0), (3, 50.0, 50.0, 5, 2, 0.0),       # radii
+        (4, 0.0, 100.0, 2, 2, 0.0), (3, 0.0, 100.0, 33, 2, 0.0),       # nbins < N-1, > 32
+        (3, 0.0, 100.0, 5, -1, 0.0),                                   # lmax
+        (3, 0.0, 100.0, 5, 2, 150.0),                                  # r_max > L/2
+        (3, 0.0, 100.0, 5, 2, -1.0),
+    ]
+    for args in bad:
+        assert lib.encore_plan(C.byref(h), *args) == E.EINVAL, args
+    assert lib.encore_plan(C.byref(h), 3, 0.0, 100.0, 5, 11, 0.0) == E.EUNSUPPORTED
+    assert lib.encore_plan(C.byref(h), 4, 0.0, 100.0, 5, 7, 0.0) == E.EUNSUPPORTED
+    assert lib.encore_plan(None, 3, 0.0, 100.0, 5, 2, 0.0) == E.EINVAL
+    assert lib.encore_destroy(None) == E.EINVAL
+    assert b"invalid" in lib.encore_strerror(E.EINVAL)
+    with pytest.raises(E.EncoreError):
+        E.encore_plan(2, 0.0, 1.0, 3, 1, 0.0)
+
+
+def test_state_errors_before_compute():
+    with E.Plan(3, 0.0, 100.0, 5, 2, 0.0) as p:
+        lib = E.lib()
+        nc, sub = (C.c_int * 3)(), (C.c_int * 3)()
+        assert lib.encore_get_grid(p.h, nc, sub) == E.ESTATE
+        assert lib.encore_get_launch_count(p.h) == E.ESTATE
+        assert lib.encore_compute(p.h, None, None, 10, None, None) == E.EINVAL
+        assert lib.encore_compute(p.h, C.c_void_p(8), None, 0, C.c_void_p(8), None) == E.EINVAL
+
+
+@pytest.mark.parametrize("order,nbins,lmax,nlam,nb,nterms", [
+    (3, 5, 4, 5, 10, 15), (3, 10, 10, 11, 45, 66),      # 660 = 66 x 10
+    (4, 10, 5, 69, 120, 1126),                           # 8 280 = 69 x 120, 135 120 = 1 126 x 120
+    (5, 8, 3, 204, 70, 6063), (5, 10, 3, 204, 210, 6063),  # 42 840 = 204 x 210
+])
+def test_plan_tables_match_paper_counts(order, nbins, lmax, nlam, nb, nterms):
+    with E.Plan(order, 20.0, 160.0, nbins, lmax, 1000.0) as p:
+        assert p.n_lambda == nlam and p.n_b == nb
+        assert E.encore_zeta_len(p.h) == nlam * nb
+        assert E.encore_num_terms(p.h) == nterms
+        ex, ca = E.encore_contraction_flops(p.h)
+        assert ca == nterms * nb * {3: 5, 4: 11, 5: 17}[order]
+
+
+def test_plan_tables_equal_oracle_enumeration(oracle):
+    for order, nbins, lmax in [(3, 6, 7), (4, 7, 4), (5, 6, 2)]:
+        with E.Plan(order, 5.0, 65.0, nbins, lmax, 0.0) as p:
+            assert (p.multiplets == oracle.multiplets(order, lmax)).all()
+            assert (p.bin_tuples == oracle.bin_tuples(order, nbins)).all()
+            assert E.encore_num_terms(p.h) == oracle.count_terms(order, lmax, half=True)
+            assert np.array_equal(E.encore_get_bin_edges(p.h, nbins), oracle.bin_edges(5.0, 65.0, nbins))

@@ -1,0 +1,218 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerance (BASELINE.json north_star): max|zeta_gpu - zeta_oracle| / max|zeta_oracle| <= 1e-9 (fp64 throughout);
+cell ids, per-primary and global per-bin pair counts bit-exact.  Reduced-size cases are compared element by
+element; the full-size configs (the launch configurations bench.py times) are checked on sampled primaries
+(a_lm tiles and counts computed one by one by the oracle) and through closed-form properties.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def E():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2105_08722_b200 as mod
+    mod.lib()
+    return mod
+
+
+def gpu_run(E, order, pos, w, box, rmin, rmax, nbins, lmax, want=("zeta", "counts", "cells")):
+    dev = torch.device("cuda:0")
+    n = pos.shape[1]
+    tp = torch.from_numpy(np.ascontiguousarray(pos)).to(dev)
+    tw = None if w is None else torch.from_numpy(np.ascontiguousarray(w)).to(dev)
+    plan = E.Plan(order, rmin, rmax, nbins, lmax, box)
+    z = plan.compute(tp, tw)
+    torch.cuda.synchronize()
+    res = {"plan": plan, "zeta": z.cpu().numpy()}
+    if "counts" in want:
+        res["bin_counts"], res["pairs"] = E.encore_get_bin_counts(plan.h, nbins)
+        pc = torch.empty((n, nbins), dtype=torch.int32, device=dev)
+        E.encore_get_primary_counts(plan.h, pc)
+        res["prim_counts"] = pc.cpu().numpy().astype(np.uint32)
+    if "cells" in want:
+        cid = torch.empty(n, dtype=torch.int32, device=dev)
+        E.encore_get_cell_ids(plan.h, cid)
+        res["cid"] = cid.cpu().numpy()
+        res["nc"], res["sub"] = E.encore_get_grid(plan.h)
+    return res
+
+
+def check_full(E, oracle, order, pos, w, box, rmin, rmax, nbins, lmax, alm_samples=(0, 1, 7)):
+    g = gpu_run(E, order, pos, w, box, rmin, rmax, nbins, lmax)
+    o = oracle.zeta(order, pos, w, box, rmin, rmax, nbins, lmax, want_prim_counts=True)
+    # integers: bit-exact
+    assert (g["bin_counts"] == o["bin_counts"]).all()
+    assert (g["prim_counts"] == o["prim_counts"]).all()
+    cid, nc = oracle.cell_ids(pos, box, rmax, g["sub"])
+    assert list(nc) == g["nc"]
+    assert (g["cid"] == cid).all()
+    # zeta
+    scale = np.abs(o["zeta"]).max()
+    err = np.abs(g["zeta"] - o["zeta"]).max()
+    assert scale > 0 or err == 0
+    assert err <= TOL * scale, f"rel-to-max error {err / scale:.3e}"
+    # a_lm tiles of a few primaries
+    n = pos.shape[1]
+    for i in alm_samples:
+        if i >= n:
+            continue
+        a_o, cnt_o = oracle.alm(pos, w, box, rmin, rmax, nbins, lmax, i)
+        a_g = E.encore_get_alm(g["plan"].h, i, nbins, lmax)
+        ref = np.stack([a_o[:, l * l + l + m] for l in range(lmax + 1) for m in range(l + 1)], axis=1)
+        s = np.abs(ref).max()
+        assert np.abs(a_g - ref).max() <= 1e-12 * s + 1e-300
+    g["plan"].close()
+    return err / scale if scale > 0 else 0.0
+
+
+# ---- configs[0] in full, the others at reduced size, element by element --------------------------------------
+def test_c1_full(E, oracle):
+    cfg = W.CONFIGS["c1"]
+    pos, w = W.make(cfg)
+    check_full(E, oracle, cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, alm_samples=(0, 999, 1999))
+
+
+def test_c2_reduced_lmax10_rmax_half_box(E, oracle):
+    cfg = W.scaled(W.CONFIGS["c2"], box=400.0, n=6000, grid=64)   # r_max = L/2 exactly
+    pos, w = W.make(cfg)
+    check_full(E, oracle, 3, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+
+
+def test_c3_reduced_4pcf(E, oracle):
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=7000, grid=64)
+    pos, w = W.make(cfg)
+    check_full(E, oracle, 4, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+
+
+def test_c4_reduced_cutsky_data_minus_random(E, oracle):
+    cfg = W.scaled(W.CONFIGS["c4"], n=8000)
+    pos, w = W.make(cfg)
+    assert abs(w.sum()) < 1e-9 * np.abs(w).sum()
+    check_full(E, oracle, 4, pos, w, 0.0, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+
+
+def test_c5_reduced_5pcf(E, oracle):
+    cfg = W.scaled(W.CONFIGS["c5"], box=340.0, n=5000, grid=64)
+    pos, w = W.make(cfg)
+    check_full(E, oracle, 5, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+
+
+# ---- edge cases ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("order,nbins,lmax", [(3, 2, 0), (3, 3, 7), (4, 3, 1), (4, 13, 2), (5, 4, 1), (5, 5, 2)])
+def test_small_clouds_open_and_periodic(E, oracle, order, nbins, lmax):
+    rng = np.random.default_rng(1000 + 10 * order + lmax)
+    n = 257                                                   # several groups and a ragged tail
+    pos = np.ascontiguousarray(rng.uniform(0, 90.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.3, 0.7])
+    check_full(E, oracle, order, pos, w, 0.0, 4.0, 44.0, nbins, lmax)
+    check_full(E, oracle, order, pos, w, 90.0, 4.0, 44.0, nbins, lmax)
+
+
+def test_degenerate_inputs(E, oracle):
+    # one particle: no pairs, zeta = 0
+    g = gpu_run(E, 3, np.array([[1.0], [2.0], [3.0]]), np.ones(1), 0.0, 0.0, 10.0, 3, 2)
+    assert g["pairs"] == 0 and not g["zeta"].any()
+    # coincident particles (r = 0 pairs are skipped, R8), all in one cell, zero extent along z
+    pos = np.zeros((3, 40))
+    pos[0, :20] = 1.0
+    pos[1, 10:30] = 2.0
+    w = np.arange(1.0, 41.0)
+    check_full(E, oracle, 3, pos, w, 0.0, 0.0, 10.0, 3, 3)
+    check_full(E, oracle, 4, pos, None, 0.0, 0.5, 10.0, 3, 2)
+    # many particles in one tiny clump inside a large periodic box: one group row carries all candidates
+    rng = np.random.default_rng(5)
+    pos = np.ascontiguousarray(500.0 + rng.uniform(-3, 3, (3, 700)))
+    check_full(E, oracle, 3, pos, None, 1000.0, 0.0, 8.0, 4, 4)
+    # pairs exactly on bin edges: lattice with spacing 1, edges at integers
+    ax = np.arange(6.0)
+    pos = np.ascontiguousarray(np.stack(np.meshgrid(ax, ax, ax, indexing="ij")).reshape(3, -1))
+    check_full(E, oracle, 3, pos, None, 0.0, 1.0, 4.0, 3, 2)
+    check_full(E, oracle, 4, pos, None, 12.0, 1.0, 4.0, 3, 2)
+
+
+def test_domain_errors(E):
+    dev = torch.device("cuda:0")
+    with E.Plan(3, 0.0, 10.0, 3, 2, 100.0) as p:
+        bad = torch.tensor([[1.0, 2.0], [3.0, 100.0], [5.0, 6.0]], dtype=torch.float64, device=dev)   # y == L
+        with pytest.raises(E.EncoreError) as ei:
+            p.compute(bad)
+        assert ei.value.status == E.EDOMAIN
+        nan = torch.tensor([[1.0, float("nan")], [3.0, 4.0], [5.0, 6.0]], dtype=torch.float64, device=dev)
+        with pytest.raises(E.EncoreError) as ei:
+            p.compute(nan)
+        assert ei.value.status == E.EDOMAIN
+
+
+def test_bitwise_reproducible_and_host_entry(E):
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=7000, grid=64)
+    pos, w = W.make(cfg)
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(4, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as p:
+        z1 = p.compute(tp, tw).cpu().numpy()
+        z2 = p.compute(tp, tw).cpu().numpy()
+        zh = p.compute_host(pos, w)
+        assert E.encore_get_launch_count(p.h) > 0
+    assert np.array_equal(z1, z2) and np.array_equal(z1, zh)
+    # a permutation of the input order changes only the within-cell summation order
+    perm = np.random.default_rng(0).permutation(cfg.n)
+    with E.Plan(4, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as p:
+        z3 = p.compute_host(np.ascontiguousarray(pos[:, perm]), w[perm])
+    assert np.abs(z3 - z1).max() <= 1e-12 * np.abs(z1).max()
+
+
+# ---- full-size configs, as bench.py launches them ------------------------------------------------------------------
+def _full_size_checks(E, oracle, name, nsample=12):
+    cfg = W.CONFIGS[name]
+    pos, w = W.make(cfg)
+    g = gpu_run(E, cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+    nb, lmax, n = cfg.nbins, cfg.lmax, cfg.n
+    # sampled primaries: counts bit-exact, a_lm tiles to 1e-12
+    rng = np.random.default_rng(42)
+    for i in rng.choice(n, nsample, replace=False):
+        a_o, cnt_o = oracle.alm(pos, w, cfg.box, cfg.rmin, cfg.rmax, nb, lmax, int(i))
+        assert (g["prim_counts"][i] == cnt_o).all()
+        a_g = E.encore_get_alm(g["plan"].h, int(i), nb, lmax)
+        ref = np.stack([a_o[:, l * l + l + m] for l in range(lmax + 1) for m in range(l + 1)], axis=1)
+        assert np.abs(a_g - ref).max() <= 1e-11 * np.abs(ref).max()
+    cid, nc = oracle.cell_ids(pos, cfg.box, cfg.rmax, g["sub"])
+    assert (g["cid"] == cid).all()
+    # properties that hold at any size
+    pc = g["prim_counts"].astype(np.float64)
+    assert (g["bin_counts"] == g["prim_counts"].sum(axis=0, dtype=np.uint64)).all()
+    lam = g["plan"].multiplets
+    bins = g["plan"].bin_tuples
+    z = g["zeta"]
+    assert np.isfinite(z).all()
+    if cfg.weights == "unit":
+        # l = 0 identity with integer counts: zeta_0..0^B = (4pi)^{-(N-1)/2}/V sum_i prod_k n_i(b_k)/v_{b_k}
+        e = E.encore_get_bin_edges(g["plan"].h, nb)
+        vb = 4 * math.pi / 3 * (e[1:] ** 3 - e[:-1] ** 3)
+        V = cfg.box ** 3 if cfg.box > 0 else 1.0
+        i0 = [tuple(r) for r in lam].index(tuple([0] * lam.shape[1]))
+        a = pc / vb
+        ref = np.array([np.prod(a[:, list(B)], axis=1).sum() for B in bins]) * (4 * math.pi) ** (-(cfg.order - 1) / 2) / V
+        assert np.abs(z[i0] - ref).max() <= 1e-11 * np.abs(ref).max()
+    g["plan"].close()
+    return g
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c5"])
+def test_full_size_periodic_configs(E, oracle, name):
+    _full_size_checks(E, oracle, name)
+
+
+def test_full_size_c4_cutsky(E, oracle):
+    _full_size_checks(E, oracle, "c4", nsample=6)

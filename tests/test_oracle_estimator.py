@@ -224,12 +224,13 @@ def test_alm_conjugation_and_counts(oracle):
 
 def test_cell_ids_are_valid_cells(oracle):
     """Reading R11: the id is the linear index of the cell that geometrically contains the point."""
-    for cfg, sub in [(W.CONFIGS["c1"], 2), (W.scaled(W.CONFIGS["c4"], n=4000), 3)]:
+    for cfg, sub in [(W.CONFIGS["c1"], (2, 2, 2)), (W.CONFIGS["c1"], (8, 2, 3)), (W.scaled(W.CONFIGS["c4"], n=4000), (12, 3, 3))]:
         pos, _ = W.make(cfg)
         cid, nc = oracle.cell_ids(pos, cfg.box, cfg.rmax, sub)
+        sub = np.asarray(sub)
         if cfg.box > 0:
             org, ext = np.zeros(3), np.full(3, cfg.box)
-            assert (nc == int(cfg.box // (cfg.rmax / sub))).all()
+            assert (nc == np.floor(cfg.box / (cfg.rmax / sub))).all()
         else:
             org, ext = pos.min(1), pos.max(1) - pos.min(1)
             assert (nc == np.maximum(1, np.floor(ext / (cfg.rmax / sub)))).all()
