@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libencore_b200.so")
 SOURCES = ["tables.cpp", "grid.cu", "pair.cu", "contract.cu", "diag.cu", "api.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", INCLUDE]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", INCLUDE] + os.environ.get("ENCORE_NVCC_FLAGS", "").split()
 
 
 def _deps_mtime() -> float:

@@ -2,6 +2,7 @@
 #include "../../include/encore.h"
 #include "device.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -37,6 +38,11 @@ struct encore_plan_s {
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
     DevBuf io_pos, io_w, io_zeta;
+    DevBuf grows, gprefix, item_rows, item_off, list;
+    int *h_gprefix = nullptr;   // pinned
+    size_t h_gprefix_cap = 0;
+    size_t list_budget_bytes = (size_t)24 << 30;
+    int pair_steps = 0;
     double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6]
     // state of the last compute
     bool have = false;
@@ -176,7 +182,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->cell_count.ensure(sizeof(int) * (size_t)G.ncell));
     CU(P->cell_fill.ensure(sizeof(int) * (size_t)G.ncell));
     CU(P->cell_start.ensure(sizeof(int) * ((size_t)G.ncell + 1)));
-    CU(P->scan_tmp.ensure(sizeof(int) * ((size_t)G.ncell / 2048 + 4)));
+    CU(P->scan_tmp.ensure(sizeof(int) * (std::max<size_t>((size_t)G.ncell, 4000000) / 2048 + 8)));
     CU(P->tmp_idx.ensure(sizeof(int) * n));
     CU(P->sorted_idx.ensure(sizeof(int) * n));
     CU(P->pos4.ensure(sizeof(double4) * n));
@@ -211,15 +217,60 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.bins.invw_f = (float)((double)nb / (T.rmax - T.rmin));
     for (int b = 0; b <= nb; ++b) pa.bins.e2[b] = T.edges2[b];
     for (int b = 0; b < nb; ++b) pa.bins.vinv[b] = T.vinv[b];
+    for (int b = 0; b < nb; ++b) pa.bin_order[b] = b;
+    std::sort(pa.bin_order, pa.bin_order + nb, [&](int x, int y) { return T.vinv[x] != T.vinv[y] ? T.vinv[x] < T.vinv[y] : x < y; });
     pa.rmax = T.rmax;
     pa.lmax = T.lmax; pa.ncomp = ncomp;
     pa.ynorm = P->d_ynorm.as<double>();
     pa.alm = P->alm.as<double>();
     pa.counts = P->counts.as<uint32_t>();
     pa.cand_pairs = P->cand.as<unsigned long long>();
-    pa.ngroups_max = ngmax;
+    pa.ngroups = ngmax;
+    CU(P->grows.ensure(sizeof(int) * (size_t)ngmax));
+    CU(P->gprefix.ensure(sizeof(int) * ((size_t)ngmax + 2)));
+    pa.grows = P->grows.as<int>();
+    pa.gprefix = P->gprefix.as<int>();
+    pa.scan_tmp = P->scan_tmp.as<int>();
+    if (P->h_gprefix_cap < (size_t)ngmax + 2) {
+        if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
+        P->h_gprefix = nullptr; P->h_gprefix_cap = 0;
+        CU(cudaMallocHost((void **)&P->h_gprefix, sizeof(int) * ((size_t)ngmax + 2)));
+        P->h_gprefix_cap = (size_t)ngmax + 2;
+    }
     CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
-    CU(launch_pair_stage(pa, s, &P->launches));
+    CU(launch_pair_count(pa, s, &P->launches));
+    // second small device->host read: rows per group (prefix) and the number of groups -> super-steps
+    CU(cudaMemcpyAsync(P->h_gprefix, P->gprefix.p, sizeof(int) * ((size_t)ngmax + 1), cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(P->h_gprefix + ngmax + 1, P->group_start.as<int>() + G.npencil, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    {
+        const int ngroups = P->h_gprefix[ngmax + 1];
+        const int *gp = P->h_gprefix;
+        const size_t total_rows = (size_t)gp[ngroups];
+        const size_t budget_rows = std::max<size_t>(P->list_budget_bytes / 128, 1);
+        size_t max_group_rows = 0;
+        for (int g = 0; g < ngroups; ++g) max_group_rows = std::max(max_group_rows, (size_t)(gp[g + 1] - gp[g]));
+        const size_t cap_rows = std::max(std::min(total_rows, budget_rows), max_group_rows);
+        CU(P->list.ensure(std::max<size_t>(cap_rows, 1) * 128));
+        const int max_items = 4000000;
+        const int max_ng = std::max(1, max_items / nb);
+        CU(P->item_rows.ensure(sizeof(int) * (size_t)std::min(ngroups, max_ng) * nb + 64));
+        CU(P->item_off.ensure(sizeof(int) * (size_t)std::min(ngroups, max_ng) * nb + 64));
+        pa.item_rows = P->item_rows.as<int>();
+        pa.item_off = P->item_off.as<int>();
+        pa.list = P->list.as<unsigned>();
+        pa.list_rows_cap = cap_rows;
+        pa.ngroups = ngroups;
+        P->pair_steps = 0;
+        int g0 = 0;
+        while (g0 < ngroups) {
+            int g1 = g0 + 1;
+            while (g1 < ngroups && g1 - g0 < max_ng && (size_t)(gp[g1 + 1] - gp[g0]) <= cap_rows) ++g1;
+            CU(launch_pair_fill_harmonics(pa, g0, g1, s, &P->launches));
+            ++P->pair_steps;
+            g0 = g1;
+        }
+    }
     TRY(record(P, 3, s));
     // ---- a5: contraction ---------------------------------------------------------------------------------------
     ContractArgs ca{};
@@ -270,6 +321,7 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
     }
     if (const char *e = std::getenv("ENCORE_SUB_YZ")) P->sub_yz_override = std::atoi(e);
     if (const char *e = std::getenv("ENCORE_SUB_X")) P->sub_x_override = std::atoi(e);
+    if (const char *e = std::getenv("ENCORE_LIST_MB")) P->list_budget_bytes = (size_t)std::max(1, std::atoi(e)) << 20;
     *plan_out = P;
     return ENCORE_OK;
 }
@@ -302,9 +354,11 @@ int encore_destroy(encore_plan_t *P)
     DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
-                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta};
+                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->grows, &P->gprefix, &P->item_rows,
+                      &P->item_off, &P->list};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
+    if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
     if (P->ev_ready) for (int i = 0; i < 6; ++i) cudaEventDestroy(P->ev[i]);
     delete P;
     return ENCORE_OK;

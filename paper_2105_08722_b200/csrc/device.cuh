@@ -58,11 +58,23 @@ struct PairArgs {
     int lmax, ncomp;
     const double *ynorm;        // [ncomp] device
     double *alm;                // [ngroups][ncomp][nbins][32]
-    uint32_t *counts;           // [ngroups][nbins][32]
+    uint32_t *counts;           // [ngroups][nbins][32]  accepted pairs per (primary, bin): integer output of a3
     unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)
-    int ngroups_max;
+    int ngroups;                // upper bound n/32 + npencil + 1 for the count pass; exact afterwards
+    // candidate lists: item = (bin rank, group) of the current super-step; rows of 32 lanes
+    int *grows;                 // [ngroups]   rows needed by a group (sum over bins of max over lanes)
+    int *gprefix;               // [ngroups+1] exclusive scan of grows
+    int *item_rows;             // [nbins * ngroups]
+    int *item_off;              // [nbins * ngroups + 1]
+    int *scan_tmp;
+    unsigned *list;             // [list_rows_cap][32] entries: sorted index | image codes << 26; 0xffffffff = padding
+    size_t list_rows_cap;
+    int bin_order[ENCORE_MAX_BINS]; // bins by decreasing shell volume (work per item)
 };
-cudaError_t launch_pair_stage(const PairArgs &a, cudaStream_t s, int *launches);
+// count pass over all groups; fills counts, grows, gprefix (device).  The caller then reads gprefix back,
+// sizes `list`, and calls launch_pair_fill_harmonics once per super-step [g0, g1).
+cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches);
+cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches);
 int pair_stage_supported(int lmax, int nbins);
 
 // ---- contract.cu ----------------------------------------------------------------------------------------

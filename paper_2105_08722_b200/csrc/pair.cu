@@ -4,29 +4,40 @@
 //
 // The paper does this on the CPU, histogramming Cartesian monomials with AVX, eight secondaries at a time
 // (Alg. 2) and has no GPU version of it.  Design here:
-//   * one CTA per group of 32 consecutive cell-sorted primaries of one (iy,iz) pencil; lane = primary,
-//     warp = radial bin, so thread (i,b) owns the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS:
-//     no atomics, no cross-lane reductions, summation order fixed by the candidate order -> deterministic;
-//   * candidates = contiguous runs of the sorted array (one per neighbouring pencil, x-range culled against the
-//     group's cell range), streamed in chunks of one candidate per thread;
-//   * phase A: every thread tests its candidate against the 32 primaries in fp64 exactly as DESIGN.md R8-R10
-//     fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)), compare with e_b^2) and writes a one-byte bin code;
-//   * phase B: thread (i,b) scans row i of the code table for its bin, appends the hits to a private ring in
-//     shared memory and consumes them in lock-step with the other lanes of its warp (all lanes work on the same
-//     bin, so their queues fill at the same rate); per hit: unit vector, w (x+iy)^m by complex recurrence,
-//     monic associated-Legendre polynomials p_lm(z) = z p_{l-1,m} - gamma_lm p_{l-2,m}, one FMA per component.
-//   Normalisation (-1)^m N_lm k_lm / v_b is applied once per (primary, bin) in the epilogue.
+// the work is split by resource profile into three kernels around "groups" of 32 consecutive cell-sorted
+// primaries of one (iy,iz) pencil (lane = primary everywhere):
+//   k_bin<COUNT>  (a3, integer/fp32, few registers, high occupancy): candidates = contiguous runs of the sorted
+//     array (one per neighbouring pencil, x-range culled against the group's cell range); lane = candidate, loop
+//     over the 32 primaries.  A first fp32 evaluation on coordinates relative to the group decides every pair
+//     whose radius is farther than a proven error margin from all bin edges; the rest (~1e-4) is decided in fp64
+//     exactly as DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so counts are
+//     bit-exact.  __match_any_sync turns the 32 codes of a warp step into one hit mask per (primary, bin).
+//     Output: n_i(b), the per-(primary, bin) pair counts (an integer output of the path), which also size
+//   k_bin<FILL>   (a3 again, same tests): thread (i,b) pops the set bits of its masks, in candidate order, into
+//     the candidate list of item (group, b) in HBM: rows of 32 lanes, 4 bytes per accepted pair.
+//   k_harm        (a4, fp64, ~140 registers): one warp per item streams its rows (coalesced), gathers the
+//     candidates, and thread (i,b) keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
+//     atomics, no cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit
+//     vector, w (x+iy)^m by complex recurrence, monic associated-Legendre polynomials
+//     p_lm(z) = z p_{l-1,m} - gamma_lm p_{l-2,m}, one FMA per component; normalisation (-1)^m N_lm k_lm / v_b once
+//     per (primary, bin) in the epilogue.  Items are ordered heaviest bin first so the grid drains evenly.
 #include "device.cuh"
 
+#include <algorithm>
 #include <climits>
 
 namespace {
 
-constexpr int kCap = 64;          // ring slots per consumer thread
-constexpr int kMaxWarps = 12;     // bins handled per pass
+constexpr int kBinWarps = 8;        // k_bin: warps per CTA
+constexpr int kCandPerThread = 2;   // k_bin: candidates per thread and chunk
+constexpr int kNWord = kBinWarps * kCandPerThread;      // 32-candidate words per chunk
+constexpr int kChunk = kNWord * 32;
 constexpr int kMaxRanges = 1024;
-constexpr int kMinBatch = 4;      // do not start a lock-step consume for fewer entries than this
+constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
+constexpr unsigned kNoHit = 254u;
+constexpr unsigned kPadEntry = 0xffffffffu;
+constexpr unsigned kIdxMask = 0x3ffffffu;
 
 __host__ __device__ constexpr int ncomp_range(int lmax, int mlo, int mhi)
 {
@@ -88,53 +99,93 @@ __device__ __forceinline__ double sep(double xj, double xi, double box, double h
     return d;
 }
 
-struct Smem {
-    double *sp;           // [3][32] primary positions
-    double *e2;           // [40] squared bin edges
-    int *rng_start;       // [kMaxRanges]
-    int *rng_off;         // [kMaxRanges+1]
-    unsigned *jidx;       // [C]
-    unsigned char *codes; // [32][C+16]
-    unsigned *ring;       // [kCap][nthreads]
+// ---- the group of a CTA / warp ---------------------------------------------------------------------------
+struct Group {
+    int first, cnt;      // sorted index of primary 0, number of primaries (1..32)
+    int py, pz;          // pencil
+    int gx0, gx1;        // x-cell range of the members
+    double ext[3];       // bound on |x_i - x_primary0| per axis (cell geometry + 1 cell of slack)
+    bool fast;           // periodic only: the image of a candidate is the same for every member
 };
 
-template <int LMAX, int MLO, int MHI, bool PERIODIC>
-__global__ void __launch_bounds__(kMaxWarps * 32, 1) k_pair(PairArgs a, int bin0, int nw)
+template <bool PERIODIC>
+__device__ __forceinline__ Group locate_group(const PairArgs &a, int g)
 {
-    constexpr int NACC = ncomp_range(LMAX, MLO, MHI);
-    const int g = blockIdx.x;
     const GridGeom &G = a.geom;
-    if (g >= a.group_start[G.npencil]) return;
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nthreads = nw * 32, C = nthreads, rowlen = C + 16;
-    const int bin = bin0 + warp;
-
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    Smem S;
-    S.sp = reinterpret_cast<double *>(smem_raw);
-    S.e2 = S.sp + 96;
-    S.rng_start = reinterpret_cast<int *>(S.sp + 136);
-    S.rng_off = S.rng_start + kMaxRanges;
-    S.jidx = reinterpret_cast<unsigned *>(S.rng_off + kMaxRanges + 4);
-    S.codes = reinterpret_cast<unsigned char *>(S.jidx + C);
-    S.ring = reinterpret_cast<unsigned *>(S.codes + 32 * rowlen);
-
-    // ---- the group ------------------------------------------------------------------------------------
-    const int ncx = G.nc[0], ncy = G.nc[1], ncz = G.nc[2];
+    Group gr;
+    const int ncx = G.nc[0], ncy = G.nc[1];
     const int p = find_pencil_of_group(a.group_start, G.npencil, g);
     const int pstart = a.cell_start[p * ncx], pend = a.cell_start[(p + 1) * ncx];
-    const int first = pstart + ENCORE_GROUP * (g - a.group_start[p]);
-    const int cnt = min(ENCORE_GROUP, pend - first);
-    const bool active = lane < cnt;
-    const double4 me = a.pos4[first + (active ? lane : 0)];
-    if (warp == 0) { S.sp[lane] = me.x; S.sp[32 + lane] = me.y; S.sp[64 + lane] = me.z; }
-    if (tid <= a.bins.nbins) S.e2[tid] = a.bins.e2[tid];
-    const int gx0 = cell_coord(a.pos4[first].x, G.org[0], G.inv[0], ncx);
-    const int gx1 = cell_coord(a.pos4[first + cnt - 1].x, G.org[0], G.inv[0], ncx);
-    const int py = p % ncy, pz = p / ncy;
+    gr.first = pstart + ENCORE_GROUP * (g - a.group_start[p]);
+    gr.cnt = min(ENCORE_GROUP, pend - gr.first);
+    gr.py = p % ncy; gr.pz = p / ncy;
+    gr.gx0 = cell_coord(a.pos4[gr.first].x, G.org[0], G.inv[0], ncx);
+    gr.gx1 = cell_coord(a.pos4[gr.first + gr.cnt - 1].x, G.org[0], G.inv[0], ncx);
+    gr.ext[0] = (double)(gr.gx1 - gr.gx0 + 2) / G.inv[0];
+    gr.ext[1] = 2.0 / G.inv[1];
+    gr.ext[2] = 2.0 / G.inv[2];
+    // r_max + extent < L/2: an accepted pair's minimal image is then fixed by the candidate's image relative to
+    // primary 0, so it can travel with the list entry
+    gr.fast = !PERIODIC || (a.rmax + fmax(gr.ext[0], fmax(gr.ext[1], gr.ext[2])) < G.half * (1.0 - 1e-9));
+    return gr;
+}
+
+// ==========================================================================================================
+// k_bin: a3.  COUNT: counts[g][b][lane].  FILL: candidate lists.
+// ==========================================================================================================
+struct BinSmem {
+    double sp[96];                 // [3][32] primary positions (exact)
+    double e2[ENCORE_MAX_BINS + 2];
+    float spf[96];                 // relative to primary 0, fp32
+    int rng_start[kMaxRanges];
+    int rng_off[kMaxRanges + 4];
+    unsigned jidx[kChunk];         // sorted index | image codes << 26
+    int cnt[ENCORE_MAX_BINS * 32]; // COUNT: accepted pairs per (bin, primary)
+};
+
+// exact decision, the operations of DESIGN.md R8-R10 (the oracle's): returns the bin or kNoHit
+template <bool PERIODIC>
+__device__ __forceinline__ unsigned classify_exact(const double4 &cj, const double *sp, int i, const double *e2, int nb,
+                                                   double box, double half, float rmin_f, float invw_f)
+{
+    const double dx = sep<PERIODIC>(cj.x, sp[i], box, half);
+    const double dy = sep<PERIODIC>(cj.y, sp[32 + i], box, half);
+    const double dz = sep<PERIODIC>(cj.z, sp[64 + i], box, half);
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if (!(r2 > 0.0 && r2 >= e2[0] && r2 < e2[nb])) return kNoHit; // DESIGN.md R8
+    int b = (int)((sqrtf((float)r2) - rmin_f) * invw_f);
+    b = max(0, min(nb - 1, b));
+    while (r2 < e2[b]) --b;               // DESIGN.md R9: the decision is on squares, fp64
+    while (!(r2 < e2[b + 1])) ++b;
+    return (unsigned)b;
+}
+
+template <bool PERIODIC, bool FILL>
+__global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int g1)
+{
+    const int g = g0 + blockIdx.x;
+    const GridGeom &G = a.geom;
+    if (g >= g1 || g >= a.group_start[G.npencil]) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nb = a.bins.nbins;
+    constexpr int nthreads = kBinWarps * 32;
+
+    __shared__ BinSmem S;
+    extern __shared__ __align__(16) unsigned hm[]; // FILL: [nb][kNWord][32] hit masks of the current chunk
+
+    const Group gr = locate_group<PERIODIC>(a, g);
+    const int first = gr.first, cnt = gr.cnt;
+    const double4 ctr = a.pos4[first];
+    if (warp == 0) {
+        const double4 me = a.pos4[first + (lane < cnt ? lane : 0)];
+        S.sp[lane] = me.x; S.sp[32 + lane] = me.y; S.sp[64 + lane] = me.z;
+        S.spf[lane] = (float)(me.x - ctr.x); S.spf[32 + lane] = (float)(me.y - ctr.y); S.spf[64 + lane] = (float)(me.z - ctr.z);
+    }
+    if (tid <= nb) S.e2[tid] = a.bins.e2[tid];
+    if (!FILL) for (int k = tid; k < nb * 32; k += nthreads) S.cnt[k] = 0;
 
     // ---- candidate ranges: one or two runs of the sorted array per neighbouring pencil ------------------
+    const int ncx = G.nc[0], ncy = G.nc[1], ncz = G.nc[2];
     int Ry = (int)floor(a.rmax * G.inv[1] + 1e-6) + 1, Rz = (int)floor(a.rmax * G.inv[2] + 1e-6) + 1;
     if (!PERIODIC) { Ry = min(Ry, ncy - 1); Rz = min(Rz, ncz - 1); } // nothing beyond the grid
     const bool full_y = PERIODIC && (2 * Ry + 1 >= ncy), full_z = PERIODIC && (2 * Rz + 1 >= ncz);
@@ -145,14 +196,14 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) k_pair(PairArgs a, int bin0
         const int iy = r % wy, iz = r / wy;
         int cy, cz, dyc, dzc;
         bool ok = true;
-        if (full_y) { cy = iy; const int d = abs(cy - py); dyc = min(d, ncy - d); }
+        if (full_y) { cy = iy; const int d = abs(cy - gr.py); dyc = min(d, ncy - d); }
         else {
-            cy = py - Ry + iy; dyc = abs(iy - Ry);
+            cy = gr.py - Ry + iy; dyc = abs(iy - Ry);
             if (PERIODIC) cy = (cy + ncy) % ncy; else ok = ok && cy >= 0 && cy < ncy;
         }
-        if (full_z) { cz = iz; const int d = abs(cz - pz); dzc = min(d, ncz - d); }
+        if (full_z) { cz = iz; const int d = abs(cz - gr.pz); dzc = min(d, ncz - d); }
         else {
-            cz = pz - Rz + iz; dzc = abs(iz - Rz);
+            cz = gr.pz - Rz + iz; dzc = abs(iz - Rz);
             if (PERIODIC) cz = (cz + ncz) % ncz; else ok = ok && cz >= 0 && cz < ncz;
         }
         int s0 = 0, l0 = 0, s1 = 0, l1 = 0;
@@ -163,7 +214,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) k_pair(PairArgs a, int bin0
             const double t2 = ty * ty + tz * tz;
             if (t2 < rmax2) {
                 const int rx = (int)floor(sqrt(rmax2 - t2) * G.inv[0] + 1e-6) + 1;
-                int lo = gx0 - rx, hi = gx1 + rx; // inclusive x-cell range
+                int lo = gr.gx0 - rx, hi = gr.gx1 + rx; // inclusive x-cell range
                 const int row = (cz * ncy + cy) * ncx;
                 if (PERIODIC) {
                     if (hi - lo + 1 >= ncx) { lo = 0; hi = ncx - 1; }
@@ -201,158 +252,245 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) k_pair(PairArgs a, int bin0
     }
     __syncthreads();
     const int T = S.rng_off[nr];
-    const int nchunks = (T + C - 1) / C;
-    if (MLO == 0 && bin0 == 0 && tid == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
+    const int nchunks = (T + kChunk - 1) / kChunk;
+    if (!FILL && tid == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
 
-    // ---- stream the candidates -----------------------------------------------------------------------
-    double acc[NACC];
+    // fp32 screening constants: the bin coordinate u = (r - r_min)/width computed in fp32 is within
+    // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one, E^2 = sum of squared extents
+    const float rmin_f = a.bins.rmin_f, invw_f = a.bins.invw_f;
+    const float kA = 3.814697265625e-06f * invw_f;
+    const float kB = 1.9073486328125e-06f * invw_f *
+                     (float)(gr.ext[0] * gr.ext[0] + gr.ext[1] * gr.ext[1] + gr.ext[2] * gr.ext[2]);
+    const float nb_f = (float)nb;
+    const bool fast = gr.fast;
+
+    // FILL: list cursor of (primary lane, bin) for the bins this thread owns: b = warp, warp + 8, ...
+    constexpr int kOwn = (ENCORE_MAX_BINS + kBinWarps - 1) / kBinWarps;
+    int kk[kOwn];
+    size_t base[kOwn];
+    int rows[kOwn];
+    if (FILL) {
+        const int ng = g1 - g0;
 #pragma unroll
-    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    unsigned count = 0;
-    int head = 0, tail = 0;
-    const unsigned pat = 0x01010101u * (unsigned)bin;
-    const int nq = C / 16;
-    const uint4 *row = reinterpret_cast<const uint4 *>(S.codes + lane * rowlen);
-    const int nb = a.bins.nbins;
-    const double e2lo = a.bins.e2[0], e2hi = a.bins.e2[nb];
+        for (int sI = 0; sI < kOwn; ++sI) {
+            const int b = warp + sI * kBinWarps;
+            kk[sI] = 0; base[sI] = 0; rows[sI] = 0;
+            if (b < nb) {
+                int rank = 0;
+                for (int q = 0; q < nb; ++q) if (a.bin_order[q] == b) rank = q;
+                const int item = rank * ng + (g - g0);
+                base[sI] = (size_t)a.item_off[item] * 32 + lane;
+                rows[sI] = a.item_rows[item];
+            }
+        }
+    }
 
     for (int ch = 0; ch < nchunks; ++ch) {
-        // -- phase A: bin code of (primary i, this thread's candidate) for all i ---------------------------
-        {
-            const int s = ch * C + tid;
+        // -- phase A: lane = candidate; bin of (primary i, candidate) for all i ------------------------------
+#pragma unroll 1
+        for (int u = 0; u < kCandPerThread; ++u) {
+            const int wd = u * kBinWarps + warp;   // word of this chunk handled by this warp
+            const int slot = wd * 32 + lane;
+            const int s = ch * kChunk + slot;
             const bool valid = s < T;
             double4 cj = make_double4(0, 0, 0, 0);
-            unsigned j = 0;
+            float xf = 0.f, yf = 0.f, zf = 0.f;
+            unsigned j = kIdxMask;
             if (valid) {
                 int lo = 0, hi = nr; // rng_off[lo] <= s < rng_off[hi]
                 while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (S.rng_off[mid] <= s) lo = mid; else hi = mid; }
                 j = (unsigned)(S.rng_start[lo] + (s - S.rng_off[lo]));
                 cj = a.pos4[j];
-                S.jidx[tid] = j;
+                double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
+                unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer adds {+L, 0, -L}[code] to x_j
+                if (PERIODIC) {
+                    if (rx > G.half) { rx -= G.box; kx = 2; } else if (rx < -G.half) { rx += G.box; kx = 0; }
+                    if (ry > G.half) { ry -= G.box; ky = 2; } else if (ry < -G.half) { ry += G.box; ky = 0; }
+                    if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
+                }
+                xf = (float)rx; yf = (float)ry; zf = (float)rz;
+                if (FILL) S.jidx[slot] = j | (kx << 26) | (ky << 28) | (kz << 30);
             }
+            if (FILL) {
+                for (int b = 0; b < nb; ++b) hm[(b * kNWord + wd) * 32 + lane] = 0u;
+                __syncwarp();
+            }
+#pragma unroll 4
             for (int i = 0; i < cnt; ++i) {
-                unsigned char code = 255;
-                if (valid && j != (unsigned)(first + i)) {
-                    const double dx = sep<PERIODIC>(cj.x, S.sp[i], G.box, G.half);
-                    const double dy = sep<PERIODIC>(cj.y, S.sp[32 + i], G.box, G.half);
-                    const double dz = sep<PERIODIC>(cj.z, S.sp[64 + i], G.box, G.half);
-                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    if (r2 > 0.0 && r2 >= e2lo && r2 < e2hi) { // DESIGN.md R8
-                        int b = (int)((sqrtf((float)r2) - a.bins.rmin_f) * a.bins.invw_f);
-                        b = max(0, min(nb - 1, b));
-                        while (r2 < S.e2[b]) --b;               // DESIGN.md R9: the decision is on squares, fp64
-                        while (!(r2 < S.e2[b + 1])) ++b;
-                        code = (unsigned char)b;
+                unsigned code = kNoHit;
+                bool exact = valid && !fast;
+                if (valid && fast) {
+                    const float dx = xf - S.spf[i], dy = yf - S.spf[32 + i], dz = zf - S.spf[64 + i];
+                    const float t = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    const float rinv = rsqrtf(t);
+                    const float r = t * rinv;                       // NaN for t == 0: falls to the exact path
+                    const float uu = (r - rmin_f) * invw_f;
+                    const float du = fmaf(kA, r + rmin_f, fmaf(kB, rinv, 9.5367431640625e-07f * fabsf(uu)));
+                    if (!(uu < -du || uu >= nb_f + du)) {           // not surely outside [r_min, r_max)
+                        const float fl = floorf(uu);
+                        const float fr = uu - fl;
+                        if (fl >= 0.f && fl < nb_f && fr >= du && fr <= 1.f - du) code = (unsigned)(int)fl;
+                        else exact = true;
                     }
                 }
-                S.codes[i * rowlen + tid] = code;
+                if (exact)
+                    code = j == (unsigned)(first + i) ? kNoHit
+                                                      : classify_exact<PERIODIC>(cj, S.sp, i, S.e2, nb, G.box, G.half, rmin_f, invw_f);
+                const unsigned grp = __match_any_sync(kFull, code);
+                if (code != kNoHit && lane == __ffs(grp) - 1) {
+                    if (FILL) hm[(code * kNWord + wd) * 32 + i] = grp;
+                    else atomicAdd(&S.cnt[code * 32 + i], __popc(grp));
+                }
             }
         }
-        __syncthreads();
-
-        // -- phase B: gather my bin's hits into my ring, consume in lock-step with my warp -------------
-        const bool last = ch == nchunks - 1;
-        int q = 0;
-        for (;;) {
-            if (active) {
-                while (q < nq && tail - head <= kCap - 16) {
-                    const uint4 v = row[q];
-                    const unsigned wds[4] = {v.x, v.y, v.z, v.w};
+        if (FILL) {
+            __syncthreads();
+            // -- phase B: thread (lane = primary, bin) appends its hits, in candidate order, to its list -------
+            if (lane < cnt) {
 #pragma unroll
-                    for (int wi = 0; wi < 4; ++wi) {
-                        unsigned m = __vcmpeq4(wds[wi], pat);
-                        while (m) {
-                            const int byte = (__ffs(m) - 1) >> 3;
-                            S.ring[(tail & (kCap - 1)) * nthreads + tid] = S.jidx[q * 16 + wi * 4 + byte];
-                            ++tail;
-                            m &= ~(0xffu << (8 * byte));
+                for (int sI = 0; sI < kOwn; ++sI) {
+                    const int b = warp + sI * kBinWarps;
+                    if (b < nb) {
+                        for (int q = 0; q < kNWord; ++q) {
+                            unsigned m = hm[(b * kNWord + q) * 32 + lane];
+                            while (m) {
+                                const int c = __ffs(m) - 1;
+                                m &= m - 1;
+                                a.list[base[sI] + (size_t)kk[sI] * 32] = S.jidx[q * 32 + c];
+                                ++kk[sI];
+                            }
                         }
                     }
-                    ++q;
                 }
             }
-            const bool done = !active || q == nq;
-            const bool alldone = __all_sync(kFull, done);
-            const int avail = tail - head;
-            const int K = __reduce_min_sync(kFull, active ? avail : INT_MAX);
-            int n;
-            if (!active) n = 0;
-            else if (alldone) n = last ? avail : (K >= kMinBatch ? K : 0);
-            else n = max(K, avail - kCap / 2);
-            const int nmax = __reduce_max_sync(kFull, n);
-            if (nmax > 0) {
-                double4 nxt;
-                if (0 < n) nxt = a.pos4[S.ring[(head & (kCap - 1)) * nthreads + tid]];
-                else nxt = make_double4(me.x + 1.0, me.y, me.z, 0.0);
-                for (int k = 0; k < nmax; ++k) {
-                    const double4 cj = nxt;
-                    if (k + 1 < nmax) {
-                        if (k + 1 < n) nxt = a.pos4[S.ring[((head + k + 1) & (kCap - 1)) * nthreads + tid]];
-                        else nxt = make_double4(me.x + 1.0, me.y, me.z, 0.0); // padding entry: weight 0
-                    }
-                    const double dx = sep<PERIODIC>(cj.x, me.x, G.box, G.half);
-                    const double dy = sep<PERIODIC>(cj.y, me.y, G.box, G.half);
-                    const double dz = sep<PERIODIC>(cj.z, me.z, G.box, G.half);
-                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    const double rinv = rsqrt(r2);
-                    accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, cj.w);
-                }
-                head += n;
-                count += (unsigned)n;
-            }
-            if (alldone) break;
+            __syncthreads();
         }
-        __syncthreads();
     }
 
-    // ---- epilogue: normalise and store the tile column of (primary lane, bin) --------------------------
-    if (bin < nb) {
-        const double vinv = a.bins.vinv[bin];
-        double *out = a.alm + (size_t)g * a.ncomp * nb * 32 + (size_t)bin * 32 + lane;
-        int k = 0;
+    if (FILL) {
+        // pad the unused tail of every lane's column
 #pragma unroll
-        for (int m = MLO; m <= MHI; ++m) {
-#pragma unroll
-            for (int l = m; l <= LMAX; ++l) {
-                const int cre = m == 0 ? l * l : l * l + 2 * m - 1;
-                out[(size_t)cre * nb * 32] = active ? acc[k] * (a.ynorm[cre] * vinv) : 0.0;
-                if (m) out[(size_t)(cre + 1) * nb * 32] = active ? acc[k + 1] * (a.ynorm[cre + 1] * vinv) : 0.0;
-                k += m ? 2 : 1;
-            }
+        for (int sI = 0; sI < kOwn; ++sI) {
+            const int b = warp + sI * kBinWarps;
+            if (b < nb)
+                for (int k = (lane < cnt ? kk[sI] : 0); k < rows[sI]; ++k) a.list[base[sI] + (size_t)k * 32] = kPadEntry;
         }
-        if (MLO == 0) a.counts[((size_t)g * nb + bin) * 32 + lane] = active ? count : 0u;
+    } else {
+        __syncthreads();
+        for (int k = tid; k < nb * 32; k += nthreads) a.counts[(size_t)g * nb * 32 + k] = (uint32_t)S.cnt[k];
     }
 }
 
-size_t pair_smem_bytes(int nw)
+// rows needed by a group: sum over bins of the largest per-lane count
+__global__ void k_group_rows(PairArgs a)
 {
-    const int C = nw * 32;
-    return 136 * sizeof(double) + (2 * kMaxRanges + 4) * sizeof(int) + (size_t)C * 4 + 32 * (size_t)(C + 16) +
-           (size_t)kCap * C * 4;
+    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (g >= a.ngroups) return;
+    const int lane = threadIdx.x & 31, nb = a.bins.nbins;
+    int tot = 0;
+    if (g < a.group_start[a.geom.npencil])
+        for (int b = 0; b < nb; ++b) tot += (int)__reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]);
+    if (lane == 0) a.grows[g] = tot;
+}
+
+// rows of the items of super-step [g0,g1): item = rank(b) * (g1-g0) + (g-g0)
+__global__ void k_item_rows(PairArgs a, int g0, int g1)
+{
+    const int ng = g1 - g0, nb = a.bins.nbins;
+    const int item = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (item >= ng * nb) return;
+    const int lane = threadIdx.x & 31;
+    const int b = a.bin_order[item / ng], g = g0 + item % ng;
+    const unsigned m = __reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]);
+    if (lane == 0) a.item_rows[item] = (int)m;
+}
+
+// ==========================================================================================================
+// k_harm: a4.  One warp per item (group, bin): stream the rows, accumulate a_lm in registers.
+// ==========================================================================================================
+// MODE 0: open geometry; 1: periodic, image carried by the entry; 2: periodic, image decided per pair
+template <int MODE>
+__device__ __forceinline__ double4 fetch(const double4 *__restrict__ pos4, unsigned e, const double4 &pad, double box)
+{
+    if (e == kPadEntry) return pad;
+    const double2 *q = reinterpret_cast<const double2 *>(pos4 + (e & kIdxMask));
+    const double2 xy = __ldg(q), zw = __ldg(q + 1);
+    double4 p = make_double4(xy.x, xy.y, zw.x, zw.y);
+    if (MODE == 1) { // x_j + {+L, 0, -L}[code]
+        const unsigned kx = (e >> 26) & 3u, ky = (e >> 28) & 3u, kz = e >> 30;
+        p.x += kx == 1u ? 0.0 : (kx == 0u ? box : -box);
+        p.y += ky == 1u ? 0.0 : (ky == 0u ? box : -box);
+        p.z += kz == 1u ? 0.0 : (kz == 0u ? box : -box);
+    }
+    return p;
+}
+
+template <int LMAX, int MLO, int MHI, int MODE>
+__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ col,
+                                          int rows, const double4 *__restrict__ pos4, const double4 &me, double box, double half)
+{
+    const double4 pad = make_double4(me.x + 1.0, me.y, me.z, 0.0); // padding entry: unit separation, weight 0
+    unsigned e1 = rows > 1 ? __ldcs(col + 32) : kPadEntry;
+    double4 p0 = fetch<MODE>(pos4, rows > 0 ? __ldcs(col) : kPadEntry, pad, box);
+    for (int k = 0; k < rows; ++k) {
+        const unsigned e2 = k + 2 < rows ? __ldcs(col + (size_t)(k + 2) * 32) : kPadEntry;
+        const double4 p1 = fetch<MODE>(pos4, e1, pad, box);
+        const double dx = sep<MODE == 2>(p0.x, me.x, box, half);
+        const double dy = sep<MODE == 2>(p0.y, me.y, box, half);
+        const double dz = sep<MODE == 2>(p0.z, me.z, box, half);
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        const double rinv = rsqrt(r2);
+        accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, p0.w);
+        p0 = p1; e1 = e2;
+    }
+}
+
+template <int LMAX, int MLO, int MHI, bool PERIODIC>
+__global__ void __launch_bounds__(kHarmWarps * 32) k_harm(PairArgs a, int g0, int g1)
+{
+    constexpr int NACC = ncomp_range(LMAX, MLO, MHI);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ng = g1 - g0, nb = a.bins.nbins;
+    const int item = blockIdx.x * kHarmWarps + warp;
+    if (item >= ng * nb) return;
+    const int bin = a.bin_order[item / ng], g = g0 + item % ng;
+    const int rows = a.item_rows[item];
+    const unsigned *col = a.list + (size_t)a.item_off[item] * 32 + lane;
+    const Group gr = locate_group<PERIODIC>(a, g);
+    const bool active = lane < gr.cnt;
+    const double4 me = a.pos4[gr.first + (active ? lane : 0)];
+
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
+    else if (gr.fast) harm_rows<LMAX, MLO, MHI, 1>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
+    else harm_rows<LMAX, MLO, MHI, 2>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
+
+    const double vinv = a.bins.vinv[bin];
+    double *out = a.alm + (size_t)g * a.ncomp * nb * 32 + (size_t)bin * 32 + lane;
+    int k = 0;
+#pragma unroll
+    for (int m = MLO; m <= MHI; ++m) {
+#pragma unroll
+        for (int l = m; l <= LMAX; ++l) {
+            const int cre = m == 0 ? l * l : l * l + 2 * m - 1;
+            out[(size_t)cre * nb * 32] = active ? acc[k] * (a.ynorm[cre] * vinv) : 0.0;
+            if (m) out[(size_t)(cre + 1) * nb * 32] = active ? acc[k + 1] * (a.ynorm[cre + 1] * vinv) : 0.0;
+            k += m ? 2 : 1;
+        }
+    }
 }
 
 template <int LMAX, int MLO, int MHI>
-cudaError_t launch_one(const PairArgs &a, cudaStream_t s, int *launches)
+cudaError_t launch_harm(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches)
 {
-    const int nb = a.bins.nbins;
-    for (int bin0 = 0; bin0 < nb; bin0 += kMaxWarps) {
-        const int nw = min(kMaxWarps, nb - bin0);
-        const size_t smem = pair_smem_bytes(nw);
-        cudaError_t e;
-        if (a.geom.periodic) {
-            e = cudaFuncSetAttribute(k_pair<LMAX, MLO, MHI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            k_pair<LMAX, MLO, MHI, true><<<a.ngroups_max, nw * 32, smem, s>>>(a, bin0, nw);
-        } else {
-            e = cudaFuncSetAttribute(k_pair<LMAX, MLO, MHI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            k_pair<LMAX, MLO, MHI, false><<<a.ngroups_max, nw * 32, smem, s>>>(a, bin0, nw);
-        }
-        *launches += 1;
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
+    const int nitems = (g1 - g0) * a.bins.nbins;
+    const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
+    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1);
+    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1);
+    *launches += 1;
+    return cudaGetLastError();
 }
 
 } // namespace
@@ -362,27 +500,59 @@ int pair_stage_supported(int lmax, int nbins)
     return lmax >= 0 && lmax <= ENCORE_MAX_LMAX && nbins >= 1 && nbins <= ENCORE_MAX_BINS;
 }
 
-#define PAIR_PASS(L, A, B)                                              \
+cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches)
+{
+    if (a.ngroups <= 0) return cudaSuccess;
+    if (a.geom.periodic) k_bin<true, false><<<a.ngroups, kBinWarps * 32, 0, s>>>(a, 0, a.ngroups);
+    else k_bin<false, false><<<a.ngroups, kBinWarps * 32, 0, s>>>(a, 0, a.ngroups);
+    k_group_rows<<<(a.ngroups + 7) / 8, 256, 0, s>>>(a);
+    *launches += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return launch_exclusive_scan(a.grows, a.gprefix, a.ngroups, a.scan_tmp, s, launches);
+}
+
+#define HARM_PASS(L, A, B)                                              \
     {                                                                   \
-        cudaError_t e = launch_one<L, A, B>(a, s, launches);            \
+        cudaError_t e = launch_harm<L, A, B>(a, g0, g1, s, launches);   \
         if (e != cudaSuccess) return e;                                 \
     }
 
 // m-ranges per lmax keep the register-resident accumulators of one pass at <= 36 doubles
-cudaError_t launch_pair_stage(const PairArgs &a, cudaStream_t s, int *launches)
+cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches)
 {
+    const int ng = g1 - g0, nb = a.bins.nbins;
+    if (ng <= 0) return cudaSuccess;
+    const int nitems = ng * nb;
+    k_item_rows<<<(nitems + 7) / 8, 256, 0, s>>>(a, g0, g1);
+    *launches += 1;
+    cudaError_t e = launch_exclusive_scan(a.item_rows, a.item_off, nitems, a.scan_tmp, s, launches);
+    if (e != cudaSuccess) return e;
+    const size_t hm_bytes = (size_t)nb * kNWord * 32 * sizeof(unsigned);
+    if (a.geom.periodic) {
+        e = cudaFuncSetAttribute(k_bin<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hm_bytes);
+        if (e != cudaSuccess) return e;
+        k_bin<true, true><<<ng, kBinWarps * 32, hm_bytes, s>>>(a, g0, g1);
+    } else {
+        e = cudaFuncSetAttribute(k_bin<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hm_bytes);
+        if (e != cudaSuccess) return e;
+        k_bin<false, true><<<ng, kBinWarps * 32, hm_bytes, s>>>(a, g0, g1);
+    }
+    *launches += 1;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
     switch (a.lmax) {
-    case 0: PAIR_PASS(0, 0, 0) break;
-    case 1: PAIR_PASS(1, 0, 1) break;
-    case 2: PAIR_PASS(2, 0, 2) break;
-    case 3: PAIR_PASS(3, 0, 3) break;
-    case 4: PAIR_PASS(4, 0, 4) break;
-    case 5: PAIR_PASS(5, 0, 5) break;
-    case 6: PAIR_PASS(6, 0, 2) PAIR_PASS(6, 3, 6) break;
-    case 7: PAIR_PASS(7, 0, 1) PAIR_PASS(7, 2, 3) PAIR_PASS(7, 4, 7) break;
-    case 8: PAIR_PASS(8, 0, 1) PAIR_PASS(8, 2, 3) PAIR_PASS(8, 4, 8) break;
-    case 9: PAIR_PASS(9, 0, 1) PAIR_PASS(9, 2, 3) PAIR_PASS(9, 4, 5) PAIR_PASS(9, 6, 9) break;
-    case 10: PAIR_PASS(10, 0, 1) PAIR_PASS(10, 2, 3) PAIR_PASS(10, 4, 5) PAIR_PASS(10, 6, 10) break;
+    case 0: HARM_PASS(0, 0, 0) break;
+    case 1: HARM_PASS(1, 0, 1) break;
+    case 2: HARM_PASS(2, 0, 2) break;
+    case 3: HARM_PASS(3, 0, 3) break;
+    case 4: HARM_PASS(4, 0, 4) break;
+    case 5: HARM_PASS(5, 0, 5) break;
+    case 6: HARM_PASS(6, 0, 2) HARM_PASS(6, 3, 6) break;
+    case 7: HARM_PASS(7, 0, 1) HARM_PASS(7, 2, 3) HARM_PASS(7, 4, 7) break;
+    case 8: HARM_PASS(8, 0, 1) HARM_PASS(8, 2, 3) HARM_PASS(8, 4, 8) break;
+    case 9: HARM_PASS(9, 0, 1) HARM_PASS(9, 2, 3) HARM_PASS(9, 4, 5) HARM_PASS(9, 6, 9) break;
+    case 10: HARM_PASS(10, 0, 1) HARM_PASS(10, 2, 3) HARM_PASS(10, 4, 5) HARM_PASS(10, 6, 10) break;
     default: return cudaErrorInvalidValue;
     }
     return cudaSuccess;
