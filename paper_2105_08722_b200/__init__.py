@@ -228,7 +228,11 @@ class Plan:
             encore_destroy(self.h)
             self.h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     def __enter__(self):
         return self

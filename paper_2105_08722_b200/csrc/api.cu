@@ -33,7 +33,8 @@ struct DevBuf {
 struct encore_plan_s {
     HostTables T;
     bool uploaded = false;
-    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_tuple_index, gweights;
+    bool force_generic = false;
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
@@ -87,6 +88,28 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
     CU(cudaMemcpyAsync(P->d_term_start.p, T.term_start.data(), sizeof(int) * T.term_start.size(), cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(P->d_bin_tuples.p, T.bin_tuples.data(), sizeof(int) * T.bin_tuples.size(), cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(P->d_ynorm.p, T.ynorm.data(), sizeof(double) * T.ynorm.size(), cudaMemcpyHostToDevice, s));
+    {   // factorised-contraction tables
+        const int nm = T.order - 1, nb = T.nbins;
+        size_t cells = 1;
+        for (int k = 0; k < nm; ++k) cells *= (size_t)nb;
+        std::vector<int> tix(cells, -1);
+        for (int iB = 0; iB < T.nB(); ++iB) {
+            size_t key = 0;
+            for (int k = 0; k < nm; ++k) key = key * nb + (size_t)T.bin_tuples[(size_t)iB * nm + k];
+            tix[key] = iB;
+        }
+        CU(P->d_pair_terms.ensure(sizeof(PairTerm) * std::max<size_t>(1, T.pair_terms.size())));
+        CU(P->d_lam4.ensure(sizeof(Lam4) * std::max<size_t>(1, T.lam4.size())));
+        CU(P->d_lam5.ensure(sizeof(Lam5) * std::max<size_t>(1, T.lam5.size())));
+        CU(P->d_lam_order.ensure(sizeof(int) * std::max<size_t>(1, T.lam_order.size())));
+        CU(P->d_tuple_index.ensure(sizeof(int) * cells));
+        CU(cudaMemcpyAsync(P->d_pair_terms.p, T.pair_terms.data(), sizeof(PairTerm) * T.pair_terms.size(), cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(P->d_lam4.p, T.lam4.data(), sizeof(Lam4) * T.lam4.size(), cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(P->d_lam5.p, T.lam5.data(), sizeof(Lam5) * T.lam5.size(), cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(P->d_lam_order.p, T.lam_order.data(), sizeof(int) * T.lam_order.size(), cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(P->d_tuple_index.p, tix.data(), sizeof(int) * cells, cudaMemcpyHostToDevice, s));
+        CU(cudaStreamSynchronize(s));
+    }
     CU(cudaStreamSynchronize(s)); // the staging vectors die at return
     CU(cudaMallocHost((void **)&P->pinned, 8 * sizeof(double)));
     P->uploaded = true;
@@ -190,7 +213,10 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->group_start.ensure(sizeof(int) * ((size_t)G.npencil + 1)));
     CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
     CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
-    CU(P->partial.ensure(sizeof(double) * (size_t)ngmax * nout));
+    const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax);
+    const int nchunk = 32;
+    CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout));
+    CU(P->gweights.ensure(sizeof(double) * (size_t)ngmax * 32));
     CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
     CU(P->cand.ensure(sizeof(unsigned long long)));
 
@@ -225,6 +251,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.alm = P->alm.as<double>();
     pa.counts = P->counts.as<uint32_t>();
     pa.cand_pairs = P->cand.as<unsigned long long>();
+    pa.gweights = P->gweights.as<double>();
     pa.ngroups = ngmax;
     CU(P->grows.ensure(sizeof(int) * (size_t)ngmax));
     CU(P->gprefix.ensure(sizeof(int) * ((size_t)ngmax + 2)));
@@ -278,7 +305,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.terms = P->d_terms.as<DevTerm>();
     ca.term_start = P->d_term_start.as<int>();
     ca.bin_tuples = P->d_bin_tuples.as<int>();
-    ca.alm = pa.alm; ca.pos4 = pa.pos4; ca.cell_start = pa.cell_start; ca.group_start = pa.group_start;
+    ca.alm = pa.alm; ca.gweights = pa.gweights; ca.pos4 = pa.pos4; ca.cell_start = pa.cell_start; ca.group_start = pa.group_start;
     ca.geom = G;
     ca.partial = P->partial.as<double>();
     ca.partial2 = P->partial2.as<double>();
@@ -286,6 +313,14 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.vinv_total = T.box > 0.0 ? 1.0 / (T.box * T.box * T.box) : 1.0; // DESIGN.md R12
     ca.zeta_out = zeta_out;
     ca.ngroups_max = ngmax;
+    ca.pair_terms = P->d_pair_terms.as<PairTerm>();
+    ca.lam4 = P->d_lam4.as<Lam4>();
+    ca.lam5 = P->d_lam5.as<Lam5>();
+    ca.lam_order = P->d_lam_order.as<int>();
+    ca.tuple_index = P->d_tuple_index.as<int>();
+    ca.lmax = T.lmax;
+    ca.nchunk = nchunk;
+    ca.factorised = factorised ? 1 : 0;
     CU(launch_contraction(ca, s, &P->launches));
     TRY(record(P, 4, s));
     // ---- a6: reduction -----------------------------------------------------------------------------------------
@@ -321,6 +356,7 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
     }
     if (const char *e = std::getenv("ENCORE_SUB_YZ")) P->sub_yz_override = std::atoi(e);
     if (const char *e = std::getenv("ENCORE_SUB_X")) P->sub_x_override = std::atoi(e);
+    if (const char *e = std::getenv("ENCORE_GENERIC_CONTRACT")) P->force_generic = std::atoi(e) != 0;
     if (const char *e = std::getenv("ENCORE_LIST_MB")) P->list_budget_bytes = (size_t)std::max(1, std::atoi(e)) << 20;
     *plan_out = P;
     return ENCORE_OK;
@@ -351,7 +387,8 @@ int encore_compute_host(encore_plan_t *P, const double *positions, const double 
 int encore_destroy(encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
-    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->cid, &P->cell_count, &P->cell_fill,
+    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
+                      &P->d_lam_order, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
                       &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->grows, &P->gprefix, &P->item_rows,
@@ -393,9 +430,35 @@ int encore_get_bin_edges(const encore_plan_t *P, double *out)
 int encore_contraction_flops(const encore_plan_t *P, double *executed, double *canonical)
 {
     if (!P) return ENCORE_EINVAL;
-    const double evals = (double)P->T.terms.size() * (double)P->T.nB();
-    const int N = P->T.order;
-    if (executed) *executed = evals * (6.0 * (N - 1) + 1.0); // generic kernel: N-1 complex multiplies + 1 add per term
+    const HostTables &T = P->T;
+    const double evals = (double)T.terms.size() * (double)T.nB();
+    const int N = T.order, nb = T.nbins;
+    double ex = evals * (6.0 * (N - 1) + 1.0); // generic kernel: N-1 complex multiplies + 1 add per term
+    if (!P->force_generic && contraction_is_factorised(N, nb, T.lmax)) {
+        // executed by the factorised kernels, fused multiply-add = 2
+        ex = 0.0;
+        if (N == 4) {
+            for (const Lam4 &q : T.lam4)
+                for (int b1 = 0; b1 + 2 < nb; ++b1) {
+                    const int nb2 = nb - 1 - b1;
+                    ex += (double)q.nterms * (4.0 + 8.0 * (nb2 - 1));                        // G: 4 mul + 4 FMA per upper bin
+                    ex += (double)(q.l3 + 1) * (2.0 * (nb2 - 1) + 4.0 * nb2 * (nb2 - 1) / 2); // Re[G a3]: 2 FMA per triple
+                }
+        } else {
+            for (const Lam5 &q : T.lam5) {
+                const int nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0];
+                for (int b1 = 0; b1 + 3 < nb; ++b1) {
+                    const int nb2 = nb - 1 - b1;
+                    ex += (double)nl * (6.0 + 8.0 * (nb2 - 2));
+                    for (int k3 = 1; k3 < nb2 - 1; ++k3) {
+                        ex += (double)nr * (4.0 + 8.0 * (nb2 - 1 - k3));
+                        ex += (double)(q.l12 + 1) * 4.0 * (nb2 - 1 - k3) * k3;
+                    }
+                }
+            }
+        }
+    }
+    if (executed) *executed = ex;
     if (canonical) *canonical = evals * (N == 3 ? 5.0 : N == 4 ? 11.0 : 17.0);
     return ENCORE_OK;
 }

@@ -24,6 +24,33 @@ struct HostTerm {
     double W;
 };
 
+// One term of a coupled pair  Y = sum_{m_a, m_b} (3j) a~_{l_a m_a}(b_a) a~_{l_b m_b}(b_b)  with every sign, conjugation
+// and overall factor folded into four real weights:
+//   Re Y += wrr r_a r_b + wii i_a i_b,   Im Y += wri r_a i_b + wir i_a r_b.
+// ia_*, ib_* are component indices INSIDE the l-block of the factor: Re(l,m) at 2m-1 (m>0) or 0, Im(l,m) at 2m.
+struct PairTerm {
+    int ia_re, ia_im, ib_re, ib_im;
+    double wrr, wii, wri, wir;
+};
+
+// N=4 multiplet for the factorised contraction:
+//   H_i = sum_{m3>=0} Re[ G_{m3}(b1,b2) a_{l3 m3}(b3) ],  G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2
+struct Lam4 {
+    int l1, l2, l3;
+    int tbeg[9];        // terms of m3 are [tbeg[m3], tbeg[m3+1]) in pair_terms
+    int nterms;
+};
+
+// N=5 multiplet:  H_i = sum_{M>=0} Re[ Y12_M(b1,b2) R34_M(b3,b4) ]  with
+//   Y12_M = f_M sum_{m1+m2=M} (l1 l2 l12; m1 m2 -M) a~1 a~2,  f_M = sqrt(2 l12+1) (-1)^{l12-M} (2 - delta_M0),
+//   R34_M = sum_{m3+m4=-M} (l3 l4 l12; m3 m4 M) a~3 a~4.
+struct Lam5 {
+    int l1, l2, l12, l3, l4;
+    int lbeg[14];       // left terms of M: [lbeg[M], lbeg[M+1])   (M <= l12 <= 12)
+    int rbeg[14];       // right terms
+    int nterms;
+};
+
 struct HostTables {
     int order = 0, nbins = 0, lmax = 0, ncomp = 0, width = 0; // width = 2N-5 columns of a multiplet row
     double rmin = 0, rmax = 0, box = 0;
@@ -35,6 +62,10 @@ struct HostTables {
     std::vector<double> edges2;      // squared
     std::vector<double> vinv;        // 1/v_b
     std::vector<double> ynorm;       // [ncomp]: (-1)^m N_lm k_lm, turns sum w p_lm(z) (x+iy)^m into sum w Y_lm
+    std::vector<PairTerm> pair_terms; // factorised contraction (N=4,5)
+    std::vector<Lam4> lam4;
+    std::vector<Lam5> lam5;
+    std::vector<int> lam_order;      // multiplets by decreasing work (launch order)
     int nLam() const { return width ? (int)multiplets.size() / width : 0; }
     int nB() const { return order > 1 ? (int)bin_tuples.size() / (order - 1) : 0; }
 };

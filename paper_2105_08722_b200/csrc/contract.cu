@@ -63,7 +63,7 @@ __global__ void k_reduce_groups(ContractArgs a)
     const int nout = a.nLam * a.nB;
     const int o = blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= nout) return;
-    const int ngroups = a.group_start[a.geom.npencil];
+    const int ngroups = a.factorised ? a.nchunk : a.group_start[a.geom.npencil]; // rows of `partial`
     const int s = blockIdx.y;
     const int per = (ngroups + a.nseg - 1) / a.nseg;
     const int g0 = s * per, g1 = min(ngroups, g0 + per);
@@ -82,13 +82,316 @@ __global__ void k_reduce_segments(ContractArgs a)
     a.zeta_out[o] = sum * a.vinv_total;
 }
 
+
+// ==========================================================================================================
+// Factorised contraction.  lane = primary of a 32-group; the a_lm blocks a multiplet needs are
+// staged in shared memory as [component][bin][lane]; every warp owns a fixed set of bin tuples of one multiplet
+// and keeps their zeta partial sums in registers over all groups of its chunk.
+// ==========================================================================================================
+__host__ __device__ constexpr int c2(int n) { return n * (n - 1) / 2; }
+__host__ __device__ constexpr int c3(int n) { return n * (n - 1) * (n - 2) / 6; }
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(kFull, v, d);
+    return v;
+}
+
+__device__ __forceinline__ void stage_block(double *dst, const double *src, int ndoubles, int tid, int nthreads)
+{
+    const double2 *s2 = reinterpret_cast<const double2 *>(src);
+    double2 *d2 = reinterpret_cast<double2 *>(dst);
+    for (int k = tid; k < ndoubles / 2; k += nthreads) d2[k] = __ldg(s2 + k);
+}
+
+// ---- N = 4 ------------------------------------------------------------------------------------------------
+// bins b1 < b2 < b3 with b2 = b1+1+k, b3 = b1+1+kp (k < kp < NB2, NB2 = nbins-1-b1); acc[OFF + c2(kp) + k]
+template <int NB2, int OFF, int NTOT>
+__device__ __forceinline__ void task4(double (&acc)[NTOT], int b1, const Lam4 &L, const PairTerm *__restrict__ terms,
+                                      const double *s1, const double *s2, const double *s3, int nb, double wi)
+{
+    const int rs = nb * 32;
+    const double *p1 = s1 + b1 * 32, *p2 = s2 + (b1 + 1) * 32, *p3 = s3 + (b1 + 1) * 32;
+    for (int m3 = 0; m3 <= L.l3; ++m3) {
+        double gr[NB2 - 1], gi[NB2 - 1]; // G_{m3}(b1, b2)
+#pragma unroll
+        for (int k = 0; k < NB2 - 1; ++k) { gr[k] = 0.0; gi[k] = 0.0; }
+        const int t1 = L.tbeg[m3 + 1];
+        for (int t = L.tbeg[m3]; t < t1; ++t) {
+            const PairTerm T = terms[t];
+            const double r1 = p1[T.ia_re * rs], i1 = p1[T.ia_im * rs];
+            const double u = T.wrr * r1, v = T.wii * i1, sx = T.wri * r1, w = T.wir * i1;
+            const double *qr = p2 + T.ib_re * rs, *qi = p2 + T.ib_im * rs;
+#pragma unroll
+            for (int k = 0; k < NB2 - 1; ++k) {
+                const double r2 = qr[k * 32], i2 = qi[k * 32];
+                gr[k] = fma(u, r2, fma(v, i2, gr[k]));
+                gi[k] = fma(sx, i2, fma(w, r2, gi[k]));
+            }
+        }
+        const int cr = m3 == 0 ? 0 : 2 * m3 - 1;
+        const double *q3r = p3 + cr * rs, *q3i = p3 + (m3 == 0 ? cr : cr + 1) * rs;
+        const double wim = m3 == 0 ? 0.0 : -wi;
+#pragma unroll
+        for (int kp = 1; kp < NB2; ++kp) {
+            const double r3 = wi * q3r[kp * 32], i3 = wim * q3i[kp * 32]; // Re[G a3] = Gr r3 - Gi i3
+#pragma unroll
+            for (int k = 0; k < kp; ++k) acc[OFF + c2(kp) + k] = fma(gr[k], r3, fma(gi[k], i3, acc[OFF + c2(kp) + k]));
+        }
+    }
+}
+
+template <int NB2, int OFF, int NTOT>
+__device__ __forceinline__ void flush4(const double (&acc)[NTOT], int b1, int nb, const int *tuple_index, double *out, int lane)
+{
+#pragma unroll
+    for (int kp = 1; kp < NB2; ++kp)
+#pragma unroll
+        for (int k = 0; k < kp; ++k) {
+            const double v = warp_sum(acc[OFF + c2(kp) + k]);
+            if (lane == 0) out[tuple_index[(b1 * nb + (b1 + 1 + k)) * nb + (b1 + 1 + kp)]] = v;
+        }
+}
+
+// warp W of the CTA owns b1 = W (NB-1-W upper bins) and b1 = NB-3-W (W+2 upper bins): equal work per warp
+template <int NB, int W>
+__device__ __forceinline__ void warp4(const ContractArgs &a, const Lam4 &L, int iL, double *smem, int off1, int off2, int off3)
+{
+    constexpr int NBA = NB - 1 - W, WB = NB - 3 - W, NBB = WB > W ? NB - 1 - WB : 0;
+    constexpr int NTOT = c2(NBA) + (NBB ? c2(NBB) : 0);
+    const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x, nb = a.nbins;
+    const int ngroups = a.group_start[a.geom.npencil];
+    const size_t tile = (size_t)a.ncomp * nb * 32;
+    double acc[NTOT];
+#pragma unroll
+    for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
+    for (int g = blockIdx.y; g < ngroups; g += gridDim.y) {
+        __syncthreads();
+        const double *src = a.alm + (size_t)g * tile;
+        stage_block(smem + off1, src + (size_t)L.l1 * L.l1 * nb * 32, (2 * L.l1 + 1) * nb * 32, tid, nthreads);
+        if (off2 != off1) stage_block(smem + off2, src + (size_t)L.l2 * L.l2 * nb * 32, (2 * L.l2 + 1) * nb * 32, tid, nthreads);
+        if (off3 != off1 && off3 != off2) stage_block(smem + off3, src + (size_t)L.l3 * L.l3 * nb * 32, (2 * L.l3 + 1) * nb * 32, tid, nthreads);
+        __syncthreads();
+        const double wi = a.gweights[(size_t)g * 32 + lane];
+        task4<NBA, 0, NTOT>(acc, W, L, a.pair_terms, smem + off1 + lane, smem + off2 + lane, smem + off3 + lane, nb, wi);
+        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, a.pair_terms, smem + off1 + lane, smem + off2 + lane, smem + off3 + lane, nb, wi);
+    }
+    double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
+    flush4<NBA, 0, NTOT>(acc, W, nb, a.tuple_index, out, lane);
+    if constexpr (NBB > 0) flush4<NBB, c2(NBA), NTOT>(acc, WB, nb, a.tuple_index, out, lane);
+}
+
+template <int NB, int W>
+__device__ __forceinline__ void dispatch4(int warp, const ContractArgs &a, const Lam4 &L, int iL, double *smem, int o1, int o2, int o3)
+{
+    constexpr int NW = (NB - 2 + 1) / 2;
+    if (warp == W) warp4<NB, W>(a, L, iL, smem, o1, o2, o3);
+    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(warp, a, L, iL, smem, o1, o2, o3);
+}
+
+template <int NB>
+__global__ void __launch_bounds__(((NB - 2 + 1) / 2) * 32) k_contract4(ContractArgs a)
+{
+    extern __shared__ __align__(16) double smem_c[];
+    const int iL = a.lam_order[blockIdx.x];
+    const Lam4 L = a.lam4[iL];
+    const int nb = a.nbins;
+    const int n1 = (2 * L.l1 + 1) * nb * 32, n2 = (2 * L.l2 + 1) * nb * 32;
+    const int off1 = 0;
+    const int off2 = L.l2 == L.l1 ? off1 : n1;
+    const int off3 = L.l3 == L.l1 ? off1 : (L.l3 == L.l2 ? off2 : (L.l2 == L.l1 ? n1 : n1 + n2));
+    dispatch4<NB, 0>(threadIdx.x >> 5, a, L, iL, smem_c, off1, off2, off3);
+}
+
+// ---- N = 5 ------------------------------------------------------------------------------------------------
+// bins b1 < b2 < b3 < b4 with b_j = b1+1+k_j (k2 < k3 < k4 < NB2); acc[OFF + c3(k4) + c2(k3) + k2]
+template <int NB2, int OFF, int NTOT>
+__device__ __forceinline__ void task5(double (&acc)[NTOT], int b1, const Lam5 &L, const PairTerm *__restrict__ terms,
+                                      const double *sA, int nb, double wi)
+{
+    const int rs = nb * 32;
+    const double *p1 = sA + (size_t)L.l1 * L.l1 * rs + b1 * 32;
+    const double *p2 = sA + (size_t)L.l2 * L.l2 * rs + (b1 + 1) * 32;
+    const double *p3 = sA + (size_t)L.l3 * L.l3 * rs + (b1 + 1) * 32;
+    const double *p4 = sA + (size_t)L.l4 * L.l4 * rs + (b1 + 1) * 32;
+    for (int M = 0; M <= L.l12; ++M) {
+        double yr[NB2 - 2], yi[NB2 - 2]; // w_i Y12_M(b1, b2)
+#pragma unroll
+        for (int k = 0; k < NB2 - 2; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
+        for (int t = L.lbeg[M]; t < L.lbeg[M + 1]; ++t) {
+            const PairTerm T = terms[t];
+            const double r1 = wi * p1[T.ia_re * rs], i1 = wi * p1[T.ia_im * rs];
+            const double u = T.wrr * r1, v = T.wii * i1, sx = T.wri * r1, w = T.wir * i1;
+            const double *qr = p2 + T.ib_re * rs, *qi = p2 + T.ib_im * rs;
+#pragma unroll
+            for (int k = 0; k < NB2 - 2; ++k) {
+                const double r2 = qr[k * 32], i2 = qi[k * 32];
+                yr[k] = fma(u, r2, fma(v, i2, yr[k]));
+                yi[k] = fma(sx, i2, fma(w, r2, yi[k]));
+            }
+        }
+#pragma unroll
+        for (int k3 = 1; k3 < NB2 - 1; ++k3) {
+            double rr[NB2 - 2], ri[NB2 - 2]; // R34_M(b3, b4), b4 = b1+1+k3+1+q, q < NB2-1-k3
+#pragma unroll
+            for (int q = 0; q < NB2 - 1 - k3; ++q) { rr[q] = 0.0; ri[q] = 0.0; }
+            for (int t = L.rbeg[M]; t < L.rbeg[M + 1]; ++t) {
+                const PairTerm T = terms[t];
+                const double r3 = p3[T.ia_re * rs + k3 * 32], i3 = p3[T.ia_im * rs + k3 * 32];
+                const double u = T.wrr * r3, v = T.wii * i3, sx = T.wri * r3, w = T.wir * i3;
+                const double *qr = p4 + T.ib_re * rs + (k3 + 1) * 32, *qi = p4 + T.ib_im * rs + (k3 + 1) * 32;
+#pragma unroll
+                for (int q = 0; q < NB2 - 1 - k3; ++q) {
+                    const double r4 = qr[q * 32], i4 = qi[q * 32];
+                    rr[q] = fma(u, r4, fma(v, i4, rr[q]));
+                    ri[q] = fma(sx, i4, fma(w, r4, ri[q]));
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < NB2 - 1 - k3; ++q)
+#pragma unroll
+                for (int k2 = 0; k2 < k3; ++k2) { // Re[Y R] = Yr Rr - Yi Ri
+                    const int o = OFF + c3(k3 + 1 + q) + c2(k3) + k2;
+                    acc[o] = fma(yr[k2], rr[q], fma(-yi[k2], ri[q], acc[o]));
+                }
+        }
+    }
+}
+
+template <int NB2, int OFF, int NTOT>
+__device__ __forceinline__ void flush5(const double (&acc)[NTOT], int b1, int nb, const int *tuple_index, double *out, int lane)
+{
+#pragma unroll
+    for (int k4 = 2; k4 < NB2; ++k4)
+#pragma unroll
+        for (int k3 = 1; k3 < k4; ++k3)
+#pragma unroll
+            for (int k2 = 0; k2 < k3; ++k2) {
+                const double v = warp_sum(acc[OFF + c3(k4) + c2(k3) + k2]);
+                const int b2 = b1 + 1 + k2, b3 = b1 + 1 + k3, b4 = b1 + 1 + k4;
+                if (lane == 0) out[tuple_index[((b1 * nb + b2) * nb + b3) * nb + b4]] = v;
+            }
+}
+
+// second warp of a multiplet: b1 = 1 .. NB-4 one after the other (NB2 = NB-2 .. 3), all partial sums in registers
+template <int NB, int B1, int OFF, int NTOT>
+__device__ __forceinline__ void rest5(double (&acc)[NTOT], const Lam5 &L, const PairTerm *terms, const double *sA, int nb, double wi)
+{
+    if constexpr (NB - 1 - B1 >= 3) {
+        task5<NB - 1 - B1, OFF, NTOT>(acc, B1, L, terms, sA, nb, wi);
+        rest5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, L, terms, sA, nb, wi);
+    }
+}
+template <int NB, int B1, int OFF, int NTOT>
+__device__ __forceinline__ void restflush5(const double (&acc)[NTOT], int nb, const int *tuple_index, double *out, int lane)
+{
+    if constexpr (NB - 1 - B1 >= 3) {
+        flush5<NB - 1 - B1, OFF, NTOT>(acc, B1, nb, tuple_index, out, lane);
+        restflush5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, nb, tuple_index, out, lane);
+    }
+}
+__host__ __device__ constexpr int rest5_total(int nb) { int s = 0; for (int b1 = 1; nb - 1 - b1 >= 3; ++b1) s += c3(nb - 1 - b1); return s > 0 ? s : 1; }
+
+constexpr int kLamPerCta5 = 4;
+
+template <int NB>
+__global__ void __launch_bounds__(kLamPerCta5 * 64) k_contract5(ContractArgs a)
+{
+    extern __shared__ __align__(16) double smem_c[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nb = a.nbins;
+    const int slot = blockIdx.x * kLamPerCta5 + (warp >> 1);
+    const bool have = slot < a.nLam;
+    const int iL = a.lam_order[have ? slot : a.nLam - 1];
+    const Lam5 L = a.lam5[iL];
+    const bool second = warp & 1;
+    const int ngroups = a.group_start[a.geom.npencil];
+    const size_t tile = (size_t)a.ncomp * nb * 32;
+    constexpr int NA = c3(NB - 1), NR = rest5_total(NB);
+    constexpr int NTOT = NA > NR ? NA : NR;
+    double acc[NTOT];
+#pragma unroll
+    for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
+    for (int g = blockIdx.y; g < ngroups; g += gridDim.y) {
+        __syncthreads();
+        stage_block(smem_c, a.alm + (size_t)g * tile, (int)tile, tid, blockDim.x);
+        __syncthreads();
+        if (!have) continue;
+        const double wi = a.gweights[(size_t)g * 32 + lane];
+        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, a.pair_terms, smem_c + lane, nb, wi);
+        else rest5<NB, 1, 0, NTOT>(acc, L, a.pair_terms, smem_c + lane, nb, wi);
+    }
+    if (!have) return;
+    double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
+    if (!second) flush5<NB - 1, 0, NTOT>(acc, 0, nb, a.tuple_index, out, lane);
+    else restflush5<NB, 1, 0, NTOT>(acc, nb, a.tuple_index, out, lane);
+}
+
+template <int NB>
+cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
+{
+    const int lm = a.lmax;
+    const size_t smem = (size_t)3 * (2 * lm + 1) * a.nbins * 32 * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    k_contract4<NB><<<dim3(a.nLam, a.nchunk), ((NB - 2 + 1) / 2) * 32, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <int NB>
+cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
+{
+    const size_t smem = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    k_contract5<NB><<<dim3((a.nLam + kLamPerCta5 - 1) / kLamPerCta5, a.nchunk), kLamPerCta5 * 64, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
 } // namespace
+
+// Factorised kernels cover the bin counts whose per-warp partial sums fit in registers; anything else (and N = 3,
+// which is cheap) runs the generic kernel.
+int contraction_is_factorised(int order, int nbins, int lmax)
+{
+    if (order == 4) return nbins >= 3 && nbins <= 10 && lmax <= 6;
+    if (order == 5) return nbins >= 4 && nbins <= 8 && lmax <= 4;
+    return 0;
+}
 
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches)
 {
-    k_contract_generic<<<a.ngroups_max, kWarps * 32, 0, s>>>(a);
     *launches += 1;
-    return cudaGetLastError();
+    if (!a.factorised) {
+        k_contract_generic<<<a.ngroups_max, kWarps * 32, 0, s>>>(a);
+        return cudaGetLastError();
+    }
+    // every (multiplet, tuple) of a chunk row is written by exactly one warp; no initialisation needed
+    if (a.order == 4) {
+        switch (a.nbins) {
+        case 3: return launch4<3>(a, s);
+        case 4: return launch4<4>(a, s);
+        case 5: return launch4<5>(a, s);
+        case 6: return launch4<6>(a, s);
+        case 7: return launch4<7>(a, s);
+        case 8: return launch4<8>(a, s);
+        case 9: return launch4<9>(a, s);
+        case 10: return launch4<10>(a, s);
+        }
+    } else if (a.order == 5) {
+        switch (a.nbins) {
+        case 4: return launch5<4>(a, s);
+        case 5: return launch5<5>(a, s);
+        case 6: return launch5<6>(a, s);
+        case 7: return launch5<7>(a, s);
+        case 8: return launch5<8>(a, s);
+        }
+    }
+    return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches)

@@ -60,6 +60,7 @@ struct PairArgs {
     double *alm;                // [ngroups][ncomp][nbins][32]
     uint32_t *counts;           // [ngroups][nbins][32]  accepted pairs per (primary, bin): integer output of a3
     unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)
+    double *gweights;           // [ngroups][32] weight of (group, lane), 0 for empty lanes
     int ngroups;                // upper bound n/32 + npencil + 1 for the count pass; exact afterwards
     // candidate lists: item = (bin rank, group) of the current super-step; rows of 32 lanes
     int *grows;                 // [ngroups]   rows needed by a group (sum over bins of max over lanes)
@@ -84,6 +85,7 @@ struct ContractArgs {
     const int *term_start;      // device [nLam+1]
     const int *bin_tuples;      // device [nB][order-1]
     const double *alm;
+    const double *gweights;     // [ngroups][32]
     const double4 *pos4;
     const int *cell_start;
     const int *group_start;
@@ -94,7 +96,17 @@ struct ContractArgs {
     double vinv_total;          // 1/V
     double *zeta_out;
     int ngroups_max;
+    // factorised kernels (N = 4, 5)
+    const PairTerm *pair_terms; // device
+    const Lam4 *lam4;           // device [nLam]
+    const Lam5 *lam5;           // device [nLam]
+    const int *lam_order;       // device [nLam], heaviest first
+    const int *tuple_index;     // device [nbins^(N-1)]: index of the ordered tuple in bin_tuples, -1 if not ordered
+    int lmax;
+    int nchunk;                 // partial has nchunk rows when the factorised kernels ran (ngroups rows otherwise)
+    int factorised;             // set by launch_contraction
 };
+int contraction_is_factorised(int order, int nbins, int lmax);
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
 

@@ -180,6 +180,7 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
         const double4 me = a.pos4[first + (lane < cnt ? lane : 0)];
         S.sp[lane] = me.x; S.sp[32 + lane] = me.y; S.sp[64 + lane] = me.z;
         S.spf[lane] = (float)(me.x - ctr.x); S.spf[32 + lane] = (float)(me.y - ctr.y); S.spf[64 + lane] = (float)(me.z - ctr.z);
+        if (!FILL) a.gweights[(size_t)g * 32 + lane] = lane < cnt ? me.w : 0.0;
     }
     if (tid <= nb) S.e2[tid] = a.bins.e2[tid];
     if (!FILL) for (int k = tid; k < nb * 32; k += nthreads) S.cnt[k] = 0;

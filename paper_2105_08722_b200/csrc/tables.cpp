@@ -5,6 +5,7 @@
 // the paper precomputes these with sympy — here they are built at plan time.
 #include "common.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 
@@ -155,6 +156,79 @@ void enumerate_terms(HostTables &t)
     }
 }
 
+// Terms of sum_{ma+mb=msum} (la lb L; ma mb -msum) a~_{la ma} a~_{lb mb} times `factor`.
+void coupled_pair_terms(int la, int lb, int L, int msum, double factor, std::vector<PairTerm> &out)
+{
+    for (int ma = -la; ma <= la; ++ma) {
+        const int mb = msum - ma;
+        if (std::abs(mb) > lb) continue;
+        double w = factor * encore_host_wigner3j(la, lb, L, ma, mb, -msum);
+        if (std::fabs(w) < 1e-15) continue;
+        // a~ = sigma (re + i tau im): m >= 0: sigma = tau = 1; m < 0: sigma = (-1)^m, tau = -1
+        const int aa = std::abs(ma), ab = std::abs(mb);
+        const double ta = ma < 0 ? -1.0 : 1.0, tb = mb < 0 ? -1.0 : 1.0;
+        if (ma < 0 && (aa & 1)) w = -w;
+        if (mb < 0 && (ab & 1)) w = -w;
+        PairTerm t{};
+        t.ia_re = aa == 0 ? 0 : 2 * aa - 1;
+        t.ib_re = ab == 0 ? 0 : 2 * ab - 1;
+        t.ia_im = aa == 0 ? t.ia_re : 2 * aa;   // m = 0: no imaginary part; point at a valid row, zero the weights
+        t.ib_im = ab == 0 ? t.ib_re : 2 * ab;
+        t.wrr = w;
+        t.wii = (aa && ab) ? -w * ta * tb : 0.0;
+        t.wri = ab ? w * tb : 0.0;
+        t.wir = aa ? w * ta : 0.0;
+        out.push_back(t);
+    }
+}
+
+void build_factorised(HostTables &t)
+{
+    const int nL = t.nLam();
+    std::vector<double> cost(nL, 0.0);
+    if (t.order == 4) {
+        for (int iL = 0; iL < nL; ++iL) {
+            const int *lam = &t.multiplets[(size_t)iL * 3];
+            Lam4 q{};
+            q.l1 = lam[0]; q.l2 = lam[1]; q.l3 = lam[2];
+            for (int m3 = 0; m3 <= q.l3; ++m3) {
+                q.tbeg[m3] = (int)t.pair_terms.size();
+                // G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2   (eq. 44 with E C = plain 3-j, eq. 18)
+                coupled_pair_terms(q.l1, q.l2, q.l3, -m3, m3 == 0 ? 1.0 : 2.0, t.pair_terms);
+            }
+            for (int m3 = q.l3 + 1; m3 < 9; ++m3) q.tbeg[m3] = (int)t.pair_terms.size();
+            q.nterms = q.tbeg[q.l3 + 1] - q.tbeg[0];
+            cost[iL] = q.nterms + 0.3 * (q.l3 + 1);
+            t.lam4.push_back(q);
+        }
+    } else if (t.order == 5) {
+        for (int iL = 0; iL < nL; ++iL) {
+            const int *lam = &t.multiplets[(size_t)iL * 5];
+            Lam5 q{};
+            q.l1 = lam[0]; q.l2 = lam[1]; q.l12 = lam[2]; q.l3 = lam[3]; q.l4 = lam[4];
+            for (int M = 0; M <= q.l12; ++M) {
+                const double f = std::sqrt(2.0 * q.l12 + 1.0) * (((q.l12 - M) & 1) ? -1.0 : 1.0) * (M == 0 ? 1.0 : 2.0);
+                q.lbeg[M] = (int)t.pair_terms.size();
+                coupled_pair_terms(q.l1, q.l2, q.l12, M, f, t.pair_terms);   // (l1 l2 l12; m1 m2 -M)
+                q.lbeg[M + 1] = (int)t.pair_terms.size();
+            }
+            for (int M = q.l12 + 1; M < 13; ++M) q.lbeg[M + 1] = q.lbeg[q.l12 + 1];
+            for (int M = 0; M <= q.l12; ++M) {
+                q.rbeg[M] = (int)t.pair_terms.size();
+                coupled_pair_terms(q.l3, q.l4, q.l12, -M, 1.0, t.pair_terms); // (l3 l4 l12; m3 m4 M) = (l12 l3 l4; M m3 m4)
+                q.rbeg[M + 1] = (int)t.pair_terms.size();
+            }
+            for (int M = q.l12 + 1; M < 13; ++M) q.rbeg[M + 1] = q.rbeg[q.l12 + 1];
+            q.nterms = (q.lbeg[q.l12 + 1] - q.lbeg[0]) + (q.rbeg[q.l12 + 1] - q.rbeg[0]);
+            cost[iL] = (q.lbeg[q.l12 + 1] - q.lbeg[0]) + 3.0 * (q.rbeg[q.l12 + 1] - q.rbeg[0]) + (q.l12 + 1);
+            t.lam5.push_back(q);
+        }
+    }
+    t.lam_order.resize(nL);
+    for (int i = 0; i < nL; ++i) t.lam_order[i] = i;
+    std::stable_sort(t.lam_order.begin(), t.lam_order.end(), [&](int x, int y) { return cost[x] > cost[y]; });
+}
+
 } // namespace
 
 int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box)
@@ -192,5 +266,6 @@ int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int 
             if (m > 0) t.ynorm[comp_im(l, m)] = v;
         }
     }
+    build_factorised(t);
     return 0;
 }
