@@ -98,13 +98,6 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-__device__ __forceinline__ void stage_block(double *dst, const double *src, int ndoubles, int tid, int nthreads)
-{
-    const double2 *s2 = reinterpret_cast<const double2 *>(src);
-    double2 *d2 = reinterpret_cast<double2 *>(dst);
-    for (int k = tid; k < ndoubles / 2; k += nthreads) d2[k] = __ldg(s2 + k);
-}
-
 // ---- N = 4 ------------------------------------------------------------------------------------------------
 // bins b1 < b2 < b3 with b2 = b1+1+k, b3 = b1+1+kp (k < kp < NB2, NB2 = nbins-1-b1); acc[OFF + c2(kp) + k]
 template <int NB2, int OFF, int NTOT>
@@ -154,54 +147,131 @@ __device__ __forceinline__ void flush4(const double (&acc)[NTOT], int b1, int nb
         }
 }
 
-// warp W of the CTA owns b1 = W (NB-1-W upper bins) and b1 = NB-3-W (W+2 upper bins): equal work per warp
+// ---- tile pipeline: the a_lm tile of a group ([component][bin][lane], contiguous in HBM) is brought into shared
+// memory by one TMA bulk copy (cp.async.bulk + mbarrier complete_tx), double-buffered so that group k+1 streams in
+// while group k is contracted.  All warps of the CTA run the same loop (same number of barriers).
+constexpr int kCtaWarps = 12;
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void tile_load(double *dst, const double *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    // bulk copies are limited by the tx-count field (2^20-1 bytes); tiles are < 256 kB
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+struct TilePipe {
+    double *buf[2];
+    unsigned long long *bar; // [2]
+    unsigned bytes;
+    int nbuf;
+};
+
+// Calls body(tile_in_smem, g) for the groups g = blockIdx.y, blockIdx.y + gridDim.y, ...
+template <class Body>
+__device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const TilePipe &tp, Body body)
+{
+    const int ngroups = a.group_start[a.geom.npencil];
+    const size_t tile = (size_t)a.ncomp * a.nbins * 32;
+    const int stride = gridDim.y;
+    const bool issuer = threadIdx.x == 0;
+    int g = blockIdx.y;
+    if (issuer && g < ngroups) tile_load(tp.buf[0], a.alm + (size_t)g * tile, tp.bytes, &tp.bar[0]);
+    for (int k = 0; g < ngroups; ++k, g += stride) {
+        const int st = tp.nbuf == 2 ? (k & 1) : 0;
+        if (tp.nbuf == 2 && issuer && g + stride < ngroups)
+            tile_load(tp.buf[st ^ 1], a.alm + (size_t)(g + stride) * tile, tp.bytes, &tp.bar[st ^ 1]);
+        mbar_wait(&tp.bar[st], tp.nbuf == 2 ? (unsigned)((k >> 1) & 1) : (unsigned)(k & 1));
+        body(tp.buf[st], g);
+        __syncthreads(); // every warp is done with buf[st] before it is refilled
+        if (tp.nbuf == 1 && issuer && g + stride < ngroups)
+            tile_load(tp.buf[0], a.alm + (size_t)(g + stride) * tile, tp.bytes, &tp.bar[0]);
+    }
+}
+
+__device__ __forceinline__ TilePipe make_pipe(const ContractArgs &a, double *smem, int nbuf)
+{
+    TilePipe tp;
+    const size_t tile = (size_t)a.ncomp * a.nbins * 32;
+    tp.buf[0] = smem;
+    tp.buf[1] = smem + (nbuf == 2 ? tile : 0);
+    tp.bar = reinterpret_cast<unsigned long long *>(smem + (size_t)nbuf * tile);
+    tp.bytes = (unsigned)(tile * sizeof(double));
+    tp.nbuf = nbuf;
+    if (threadIdx.x == 0) {
+        mbar_init(&tp.bar[0], 1);
+        mbar_init(&tp.bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    return tp;
+}
+
+// warp W of a multiplet owns b1 = W (NB-1-W upper bins) and b1 = NB-3-W (W+2 upper bins): equal work per warp
 template <int NB, int W>
-__device__ __forceinline__ void warp4(const ContractArgs &a, const Lam4 &L, int iL, double *smem, int off1, int off2, int off3)
+__device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL)
 {
     constexpr int NBA = NB - 1 - W, WB = NB - 3 - W, NBB = WB > W ? NB - 1 - WB : 0;
     constexpr int NTOT = c2(NBA) + (NBB ? c2(NBB) : 0);
-    const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x, nb = a.nbins;
-    const int ngroups = a.group_start[a.geom.npencil];
-    const size_t tile = (size_t)a.ncomp * nb * 32;
+    const int lane = threadIdx.x & 31, nb = a.nbins;
+    const int o1 = L.l1 * L.l1 * nb * 32 + lane, o2 = L.l2 * L.l2 * nb * 32 + lane, o3 = L.l3 * L.l3 * nb * 32 + lane;
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for (int g = blockIdx.y; g < ngroups; g += gridDim.y) {
-        __syncthreads();
-        const double *src = a.alm + (size_t)g * tile;
-        stage_block(smem + off1, src + (size_t)L.l1 * L.l1 * nb * 32, (2 * L.l1 + 1) * nb * 32, tid, nthreads);
-        if (off2 != off1) stage_block(smem + off2, src + (size_t)L.l2 * L.l2 * nb * 32, (2 * L.l2 + 1) * nb * 32, tid, nthreads);
-        if (off3 != off1 && off3 != off2) stage_block(smem + off3, src + (size_t)L.l3 * L.l3 * nb * 32, (2 * L.l3 + 1) * nb * 32, tid, nthreads);
-        __syncthreads();
+    for_each_group_tile(a, tp, [&](const double *t, int g) {
+        if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        task4<NBA, 0, NTOT>(acc, W, L, a.pair_terms, smem + off1 + lane, smem + off2 + lane, smem + off3 + lane, nb, wi);
-        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, a.pair_terms, smem + off1 + lane, smem + off2 + lane, smem + off3 + lane, nb, wi);
-    }
+        task4<NBA, 0, NTOT>(acc, W, L, a.pair_terms, t + o1, t + o2, t + o3, nb, wi);
+        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, a.pair_terms, t + o1, t + o2, t + o3, nb, wi);
+    });
+    if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
     flush4<NBA, 0, NTOT>(acc, W, nb, a.tuple_index, out, lane);
     if constexpr (NBB > 0) flush4<NBB, c2(NBA), NTOT>(acc, WB, nb, a.tuple_index, out, lane);
 }
 
 template <int NB, int W>
-__device__ __forceinline__ void dispatch4(int warp, const ContractArgs &a, const Lam4 &L, int iL, double *smem, int o1, int o2, int o3)
+__device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL)
 {
     constexpr int NW = (NB - 2 + 1) / 2;
-    if (warp == W) warp4<NB, W>(a, L, iL, smem, o1, o2, o3);
-    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(warp, a, L, iL, smem, o1, o2, o3);
+    if (w == W) warp4<NB, W>(a, tp, have, L, iL);
+    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(w, a, tp, have, L, iL);
 }
 
+// 12 warps per CTA = 12/NW multiplets, each on NW = ceil((NB-2)/2) warps
 template <int NB>
-__global__ void __launch_bounds__(((NB - 2 + 1) / 2) * 32) k_contract4(ContractArgs a)
+__global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract4(ContractArgs a, int nbuf)
 {
-    extern __shared__ __align__(16) double smem_c[];
-    const int iL = a.lam_order[blockIdx.x];
+    extern __shared__ __align__(128) double smem_c[];
+    constexpr int NW = (NB - 2 + 1) / 2, LPC = kCtaWarps / NW;
+    const int warp = threadIdx.x >> 5;
+    const int slot = blockIdx.x * LPC + warp / NW;
+    const bool have = warp < LPC * NW && slot < a.nLam;
+    const int iL = a.lam_order[have ? slot : 0];
     const Lam4 L = a.lam4[iL];
-    const int nb = a.nbins;
-    const int n1 = (2 * L.l1 + 1) * nb * 32, n2 = (2 * L.l2 + 1) * nb * 32;
-    const int off1 = 0;
-    const int off2 = L.l2 == L.l1 ? off1 : n1;
-    const int off3 = L.l3 == L.l1 ? off1 : (L.l3 == L.l2 ? off2 : (L.l2 == L.l1 ? n1 : n1 + n2));
-    dispatch4<NB, 0>(threadIdx.x >> 5, a, L, iL, smem_c, off1, off2, off3);
+    const TilePipe tp = make_pipe(a, smem_c, nbuf);
+    dispatch4<NB, 0>(have ? warp % NW : 0, a, tp, have, L, iL);
 }
 
 // ---- N = 5 ------------------------------------------------------------------------------------------------
@@ -293,62 +363,66 @@ __device__ __forceinline__ void restflush5(const double (&acc)[NTOT], int nb, co
 }
 __host__ __device__ constexpr int rest5_total(int nb) { int s = 0; for (int b1 = 1; nb - 1 - b1 >= 3; ++b1) s += c3(nb - 1 - b1); return s > 0 ? s : 1; }
 
-constexpr int kLamPerCta5 = 4;
-
+// 12 warps per CTA = 6 multiplets; even warp: b1 = 0, odd warp: b1 = 1 .. NB-4
 template <int NB>
-__global__ void __launch_bounds__(kLamPerCta5 * 64) k_contract5(ContractArgs a)
+__global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a, int nbuf)
 {
-    extern __shared__ __align__(16) double smem_c[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nb = a.nbins;
-    const int slot = blockIdx.x * kLamPerCta5 + (warp >> 1);
+    extern __shared__ __align__(128) double smem_c[];
+    constexpr int LPC = kCtaWarps / 2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = a.nbins;
+    const int slot = blockIdx.x * LPC + (warp >> 1);
     const bool have = slot < a.nLam;
-    const int iL = a.lam_order[have ? slot : a.nLam - 1];
+    const int iL = a.lam_order[have ? slot : 0];
     const Lam5 L = a.lam5[iL];
     const bool second = warp & 1;
-    const int ngroups = a.group_start[a.geom.npencil];
-    const size_t tile = (size_t)a.ncomp * nb * 32;
     constexpr int NA = c3(NB - 1), NR = rest5_total(NB);
     constexpr int NTOT = NA > NR ? NA : NR;
+    const TilePipe tp = make_pipe(a, smem_c, nbuf);
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for (int g = blockIdx.y; g < ngroups; g += gridDim.y) {
-        __syncthreads();
-        stage_block(smem_c, a.alm + (size_t)g * tile, (int)tile, tid, blockDim.x);
-        __syncthreads();
-        if (!have) continue;
+    for_each_group_tile(a, tp, [&](const double *t, int g) {
+        if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, a.pair_terms, smem_c + lane, nb, wi);
-        else rest5<NB, 1, 0, NTOT>(acc, L, a.pair_terms, smem_c + lane, nb, wi);
-    }
+        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, a.pair_terms, t + lane, nb, wi);
+        else rest5<NB, 1, 0, NTOT>(acc, L, a.pair_terms, t + lane, nb, wi);
+    });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
     if (!second) flush5<NB - 1, 0, NTOT>(acc, 0, nb, a.tuple_index, out, lane);
     else restflush5<NB, 1, 0, NTOT>(acc, nb, a.tuple_index, out, lane);
 }
 
+// shared memory: nbuf tiles + 2 mbarriers; two buffers whenever they fit
+static int pipe_config(const ContractArgs &a, size_t *smem)
+{
+    const size_t tile = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
+    const int nbuf = 2 * tile + 64 <= 220 * 1024 ? 2 : 1;
+    *smem = nbuf * tile + 64;
+    return nbuf;
+}
+
 template <int NB>
 cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 {
-    const int lm = a.lmax;
-    const size_t smem = (size_t)3 * (2 * lm + 1) * a.nbins * 32 * sizeof(double);
+    size_t smem;
+    const int nbuf = pipe_config(a, &smem);
+    constexpr int LPC = kCtaWarps / ((NB - 2 + 1) / 2);
     cudaError_t e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    k_contract4<NB><<<dim3(a.nLam, a.nchunk), ((NB - 2 + 1) / 2) * 32, smem, s>>>(a);
+    k_contract4<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);
     return cudaGetLastError();
 }
 
 template <int NB>
 cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 {
-    const size_t smem = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
+    size_t smem;
+    const int nbuf = pipe_config(a, &smem);
+    constexpr int LPC = kCtaWarps / 2;
     cudaError_t e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    k_contract5<NB><<<dim3((a.nLam + kLamPerCta5 - 1) / kLamPerCta5, a.nchunk), kLamPerCta5 * 64, smem, s>>>(a);
+    k_contract5<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);
     return cudaGetLastError();
 }
 
