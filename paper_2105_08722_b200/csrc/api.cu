@@ -319,6 +319,9 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.lam_order = P->d_lam_order.as<int>();
     ca.tuple_index = P->d_tuple_index.as<int>();
     ca.lmax = T.lmax;
+    ca.max_terms = 1;
+    for (const Lam4 &q : T.lam4) ca.max_terms = std::max(ca.max_terms, q.nterms);
+    for (const Lam5 &q : T.lam5) ca.max_terms = std::max(ca.max_terms, q.nterms);
     ca.nchunk = nchunk;
     ca.factorised = factorised ? 1 : 0;
     CU(launch_contraction(ca, s, &P->launches));

@@ -88,6 +88,8 @@ __global__ void k_reduce_segments(ContractArgs a)
 // staged in shared memory as [component][bin][lane]; every warp owns a fixed set of bin tuples of one multiplet
 // and keeps their zeta partial sums in registers over all groups of its chunk.
 // ==========================================================================================================
+extern __shared__ __align__(128) double smem_c[]; // dynamic shared memory of the factorised kernels
+
 __host__ __device__ constexpr int c2(int n) { return n * (n - 1) / 2; }
 __host__ __device__ constexpr int c3(int n) { return n * (n - 1) * (n - 2) / 6; }
 
@@ -101,11 +103,13 @@ __device__ __forceinline__ double warp_sum(double v)
 // ---- N = 4 ------------------------------------------------------------------------------------------------
 // bins b1 < b2 < b3 with b2 = b1+1+k, b3 = b1+1+kp (k < kp < NB2, NB2 = nbins-1-b1); acc[OFF + c2(kp) + k]
 template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void task4(double (&acc)[NTOT], int b1, const Lam4 &L, const PairTerm *__restrict__ terms,
-                                      const double *s1, const double *s2, const double *s3, int nb, double wi)
+__device__ __forceinline__ void task4(double (&acc)[NTOT], int b1, const Lam4 &L, int toff, int s1, int s2, int s3,
+                                      int nb, double wi)
 {
+    // s1, s2, s3: offsets (in doubles, lane included) of the l1, l2, l3 blocks inside smem_c; toff: of the term list
     const int rs = nb * 32;
-    const double *p1 = s1 + b1 * 32, *p2 = s2 + (b1 + 1) * 32, *p3 = s3 + (b1 + 1) * 32;
+    const double *p1 = smem_c + s1 + b1 * 32, *p2 = smem_c + s2 + (b1 + 1) * 32, *p3 = smem_c + s3 + (b1 + 1) * 32;
+    const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.tbeg[0];
     for (int m3 = 0; m3 <= L.l3; ++m3) {
         double gr[NB2 - 1], gi[NB2 - 1]; // G_{m3}(b1, b2)
 #pragma unroll
@@ -182,8 +186,8 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
 }
 
 struct TilePipe {
-    double *buf[2];
-    unsigned long long *bar; // [2]
+    int buf[2];              // offsets into smem_c (doubles)
+    int bar;                 // offset of the two mbarriers
     unsigned bytes;
     int nbuf;
 };
@@ -197,40 +201,49 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
     const int stride = gridDim.y;
     const bool issuer = threadIdx.x == 0;
     int g = blockIdx.y;
-    if (issuer && g < ngroups) tile_load(tp.buf[0], a.alm + (size_t)g * tile, tp.bytes, &tp.bar[0]);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
+    if (issuer && g < ngroups) tile_load(smem_c + tp.buf[0], a.alm + (size_t)g * tile, tp.bytes, &bar[0]);
     for (int k = 0; g < ngroups; ++k, g += stride) {
         const int st = tp.nbuf == 2 ? (k & 1) : 0;
         if (tp.nbuf == 2 && issuer && g + stride < ngroups)
-            tile_load(tp.buf[st ^ 1], a.alm + (size_t)(g + stride) * tile, tp.bytes, &tp.bar[st ^ 1]);
-        mbar_wait(&tp.bar[st], tp.nbuf == 2 ? (unsigned)((k >> 1) & 1) : (unsigned)(k & 1));
+            tile_load(smem_c + tp.buf[st ^ 1], a.alm + (size_t)(g + stride) * tile, tp.bytes, &bar[st ^ 1]);
+        mbar_wait(&bar[st], tp.nbuf == 2 ? (unsigned)((k >> 1) & 1) : (unsigned)(k & 1));
         body(tp.buf[st], g);
         __syncthreads(); // every warp is done with buf[st] before it is refilled
         if (tp.nbuf == 1 && issuer && g + stride < ngroups)
-            tile_load(tp.buf[0], a.alm + (size_t)(g + stride) * tile, tp.bytes, &tp.bar[0]);
+            tile_load(smem_c + tp.buf[0], a.alm + (size_t)(g + stride) * tile, tp.bytes, &bar[0]);
     }
 }
 
-__device__ __forceinline__ TilePipe make_pipe(const ContractArgs &a, double *smem, int nbuf)
+// shared memory: [nbuf tiles][2 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
+__device__ __forceinline__ TilePipe make_pipe(const ContractArgs &a, int nbuf)
 {
     TilePipe tp;
-    const size_t tile = (size_t)a.ncomp * a.nbins * 32;
-    tp.buf[0] = smem;
-    tp.buf[1] = smem + (nbuf == 2 ? tile : 0);
-    tp.bar = reinterpret_cast<unsigned long long *>(smem + (size_t)nbuf * tile);
+    const int tile = a.ncomp * a.nbins * 32;
+    tp.buf[0] = 0;
+    tp.buf[1] = nbuf == 2 ? tile : 0;
+    tp.bar = nbuf * tile;
     tp.bytes = (unsigned)(tile * sizeof(double));
     tp.nbuf = nbuf;
     if (threadIdx.x == 0) {
-        mbar_init(&tp.bar[0], 1);
-        mbar_init(&tp.bar[1], 1);
+        unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
-    return tp;
+    return tp; // the caller's __syncthreads (after it has copied its term list) publishes the barriers
+}
+
+// copy `n` terms starting at `src` to smem_c + off (one warp), 6 doubles per term
+__device__ __forceinline__ void stage_terms(int off, const PairTerm *src, int n, int lane)
+{
+    const double *s = reinterpret_cast<const double *>(src);
+    for (int k = lane; k < 6 * n; k += 32) smem_c[off + k] = s[k];
 }
 
 // warp W of a multiplet owns b1 = W (NB-1-W upper bins) and b1 = NB-3-W (W+2 upper bins): equal work per warp
 template <int NB, int W>
-__device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL)
+__device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
     constexpr int NBA = NB - 1 - W, WB = NB - 3 - W, NBB = WB > W ? NB - 1 - WB : 0;
     constexpr int NTOT = c2(NBA) + (NBB ? c2(NBB) : 0);
@@ -239,11 +252,11 @@ __device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp,
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for_each_group_tile(a, tp, [&](const double *t, int g) {
+    for_each_group_tile(a, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        task4<NBA, 0, NTOT>(acc, W, L, a.pair_terms, t + o1, t + o2, t + o3, nb, wi);
-        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, a.pair_terms, t + o1, t + o2, t + o3, nb, wi);
+        task4<NBA, 0, NTOT>(acc, W, L, toff, t + o1, t + o2, t + o3, nb, wi);
+        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, toff, t + o1, t + o2, t + o3, nb, wi);
     });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
@@ -252,39 +265,41 @@ __device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp,
 }
 
 template <int NB, int W>
-__device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL)
+__device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
     constexpr int NW = (NB - 2 + 1) / 2;
-    if (w == W) warp4<NB, W>(a, tp, have, L, iL);
-    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(w, a, tp, have, L, iL);
+    if (w == W) warp4<NB, W>(a, tp, have, L, iL, toff);
+    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(w, a, tp, have, L, iL, toff);
 }
 
 // 12 warps per CTA = 12/NW multiplets, each on NW = ceil((NB-2)/2) warps
 template <int NB>
 __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract4(ContractArgs a, int nbuf)
 {
-    extern __shared__ __align__(128) double smem_c[];
     constexpr int NW = (NB - 2 + 1) / 2, LPC = kCtaWarps / NW;
     const int warp = threadIdx.x >> 5;
     const int slot = blockIdx.x * LPC + warp / NW;
     const bool have = warp < LPC * NW && slot < a.nLam;
     const int iL = a.lam_order[have ? slot : 0];
     const Lam4 L = a.lam4[iL];
-    const TilePipe tp = make_pipe(a, smem_c, nbuf);
-    dispatch4<NB, 0>(have ? warp % NW : 0, a, tp, have, L, iL);
+    const TilePipe tp = make_pipe(a, nbuf);
+    const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // this multiplet's term list in shared memory
+    if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.tbeg[0], L.nterms, threadIdx.x & 31);
+    __syncthreads();
+    dispatch4<NB, 0>(have ? warp % NW : 0, a, tp, have, L, iL, toff);
 }
 
 // ---- N = 5 ------------------------------------------------------------------------------------------------
 // bins b1 < b2 < b3 < b4 with b_j = b1+1+k_j (k2 < k3 < k4 < NB2); acc[OFF + c3(k4) + c2(k3) + k2]
 template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void task5(double (&acc)[NTOT], int b1, const Lam5 &L, const PairTerm *__restrict__ terms,
-                                      const double *sA, int nb, double wi)
+__device__ __forceinline__ void task5(double (&acc)[NTOT], int b1, const Lam5 &L, int toff, int sA, int nb, double wi)
 {
     const int rs = nb * 32;
-    const double *p1 = sA + (size_t)L.l1 * L.l1 * rs + b1 * 32;
-    const double *p2 = sA + (size_t)L.l2 * L.l2 * rs + (b1 + 1) * 32;
-    const double *p3 = sA + (size_t)L.l3 * L.l3 * rs + (b1 + 1) * 32;
-    const double *p4 = sA + (size_t)L.l4 * L.l4 * rs + (b1 + 1) * 32;
+    const double *p1 = smem_c + sA + L.l1 * L.l1 * rs + b1 * 32;
+    const double *p2 = smem_c + sA + L.l2 * L.l2 * rs + (b1 + 1) * 32;
+    const double *p3 = smem_c + sA + L.l3 * L.l3 * rs + (b1 + 1) * 32;
+    const double *p4 = smem_c + sA + L.l4 * L.l4 * rs + (b1 + 1) * 32;
+    const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
     for (int M = 0; M <= L.l12; ++M) {
         double yr[NB2 - 2], yi[NB2 - 2]; // w_i Y12_M(b1, b2)
 #pragma unroll
@@ -346,11 +361,11 @@ __device__ __forceinline__ void flush5(const double (&acc)[NTOT], int b1, int nb
 
 // second warp of a multiplet: b1 = 1 .. NB-4 one after the other (NB2 = NB-2 .. 3), all partial sums in registers
 template <int NB, int B1, int OFF, int NTOT>
-__device__ __forceinline__ void rest5(double (&acc)[NTOT], const Lam5 &L, const PairTerm *terms, const double *sA, int nb, double wi)
+__device__ __forceinline__ void rest5(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, int nb, double wi)
 {
     if constexpr (NB - 1 - B1 >= 3) {
-        task5<NB - 1 - B1, OFF, NTOT>(acc, B1, L, terms, sA, nb, wi);
-        rest5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, L, terms, sA, nb, wi);
+        task5<NB - 1 - B1, OFF, NTOT>(acc, B1, L, toff, sA, nb, wi);
+        rest5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, L, toff, sA, nb, wi);
     }
 }
 template <int NB, int B1, int OFF, int NTOT>
@@ -367,7 +382,6 @@ __host__ __device__ constexpr int rest5_total(int nb) { int s = 0; for (int b1 =
 template <int NB>
 __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a, int nbuf)
 {
-    extern __shared__ __align__(128) double smem_c[];
     constexpr int LPC = kCtaWarps / 2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = a.nbins;
     const int slot = blockIdx.x * LPC + (warp >> 1);
@@ -377,15 +391,18 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a,
     const bool second = warp & 1;
     constexpr int NA = c3(NB - 1), NR = rest5_total(NB);
     constexpr int NTOT = NA > NR ? NA : NR;
-    const TilePipe tp = make_pipe(a, smem_c, nbuf);
+    const TilePipe tp = make_pipe(a, nbuf);
+    const int toff = tp.bar + 8 + (warp >> 1) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
+    if (have && !second) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
+    __syncthreads();
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for_each_group_tile(a, tp, [&](const double *t, int g) {
+    for_each_group_tile(a, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, a.pair_terms, t + lane, nb, wi);
-        else rest5<NB, 1, 0, NTOT>(acc, L, a.pair_terms, t + lane, nb, wi);
+        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, toff, t + lane, nb, wi);
+        else rest5<NB, 1, 0, NTOT>(acc, L, toff, t + lane, nb, wi);
     });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
@@ -394,11 +411,12 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a,
 }
 
 // shared memory: nbuf tiles + 2 mbarriers; two buffers whenever they fit
-static int pipe_config(const ContractArgs &a, size_t *smem)
+static int pipe_config(const ContractArgs &a, int lam_per_cta, size_t *smem)
 {
     const size_t tile = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
-    const int nbuf = 2 * tile + 64 <= 220 * 1024 ? 2 : 1;
-    *smem = nbuf * tile + 64;
+    const size_t extra = 64 + (size_t)lam_per_cta * a.max_terms * sizeof(PairTerm);
+    const int nbuf = 2 * tile + extra <= 224 * 1024 ? 2 : 1;
+    *smem = nbuf * tile + extra;
     return nbuf;
 }
 
@@ -406,8 +424,8 @@ template <int NB>
 cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 {
     size_t smem;
-    const int nbuf = pipe_config(a, &smem);
     constexpr int LPC = kCtaWarps / ((NB - 2 + 1) / 2);
+    const int nbuf = pipe_config(a, LPC, &smem);
     cudaError_t e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_contract4<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);
@@ -418,8 +436,8 @@ template <int NB>
 cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 {
     size_t smem;
-    const int nbuf = pipe_config(a, &smem);
     constexpr int LPC = kCtaWarps / 2;
+    const int nbuf = pipe_config(a, LPC, &smem);
     cudaError_t e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_contract5<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);

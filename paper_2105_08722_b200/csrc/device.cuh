@@ -103,6 +103,7 @@ struct ContractArgs {
     const int *lam_order;       // device [nLam], heaviest first
     const int *tuple_index;     // device [nbins^(N-1)]: index of the ordered tuple in bin_tuples, -1 if not ordered
     int lmax;
+    int max_terms;              // largest number of coupled-pair terms of one multiplet
     int nchunk;                 // partial has nchunk rows when the factorised kernels ran (ngroups rows otherwise)
     int factorised;             // set by launch_contraction
 };
