@@ -136,16 +136,15 @@ __device__ __forceinline__ Group locate_group(const PairArgs &a, int g)
 struct BinSmem {
     double sp[96];                 // [3][32] primary positions (exact)
     double e2[ENCORE_MAX_BINS + 2];
-    float spf[96];                 // relative to primary 0, fp32
+    float4 cand4[kChunk];          // candidates of the chunk relative to primary 0, fp32
     int rng_start[kMaxRanges];
     int rng_off[kMaxRanges + 4];
     unsigned jidx[kChunk];         // sorted index | image codes << 26
-    int cnt[ENCORE_MAX_BINS * 32]; // COUNT: accepted pairs per (bin, primary)
 };
 
 // exact decision, the operations of DESIGN.md R8-R10 (the oracle's): returns the bin or kNoHit
 template <bool PERIODIC>
-__device__ __forceinline__ unsigned classify_exact(const double4 &cj, const double *sp, int i, const double *e2, int nb,
+__device__ __noinline__ unsigned classify_exact(const double4 &cj, const double *sp, int i, const double *e2, int nb,
                                                    double box, double half, float rmin_f, float invw_f)
 {
     const double dx = sep<PERIODIC>(cj.x, sp[i], box, half);
@@ -179,11 +178,15 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
     if (warp == 0) {
         const double4 me = a.pos4[first + (lane < cnt ? lane : 0)];
         S.sp[lane] = me.x; S.sp[32 + lane] = me.y; S.sp[64 + lane] = me.z;
-        S.spf[lane] = (float)(me.x - ctr.x); S.spf[32 + lane] = (float)(me.y - ctr.y); S.spf[64 + lane] = (float)(me.z - ctr.z);
         if (!FILL) a.gweights[(size_t)g * 32 + lane] = lane < cnt ? me.w : 0.0;
     }
     if (tid <= nb) S.e2[tid] = a.bins.e2[tid];
-    if (!FILL) for (int k = tid; k < nb * 32; k += nthreads) S.cnt[k] = 0;
+    // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
+    const double4 mine = a.pos4[first + (lane < cnt ? lane : 0)];
+    const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
+    // COUNT: per-warp private counters [warp][bin][lane] in dynamic shared memory
+    int *wcnt = reinterpret_cast<int *>(hm) + warp * nb * 32;
+    if (!FILL) for (int b = 0; b < nb; ++b) wcnt[b * 32 + lane] = 0;
 
     // ---- candidate ranges: one or two runs of the sorted array per neighbouring pencil ------------------
     const int ncx = G.nc[0], ncy = G.nc[1], ncz = G.nc[2];
@@ -257,19 +260,23 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
     if (!FILL && tid == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
 
     // fp32 screening constants: the bin coordinate u = (r - r_min)/width computed in fp32 is within
-    // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one, E^2 = sum of squared extents
+    // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one (E^2 = sum of squared group
+    // extents).  For r <= 2 r_max the r-dependent part is bounded by the constant duc; beyond, u - du >= N_r trivially.
     const float rmin_f = a.bins.rmin_f, invw_f = a.bins.invw_f;
-    const float kA = 3.814697265625e-06f * invw_f;
+    const float c0 = -rmin_f * invw_f;
+    const float nb_f = (float)nb;
+    const float duc = 3.814697265625e-06f * invw_f * (2.f * (float)a.rmax + rmin_f) + 9.5367431640625e-07f * (2.f * nb_f + 2.f);
     const float kB = 1.9073486328125e-06f * invw_f *
                      (float)(gr.ext[0] * gr.ext[0] + gr.ext[1] * gr.ext[1] + gr.ext[2] * gr.ext[2]);
-    const float nb_f = (float)nb;
     const bool fast = gr.fast;
 
     // FILL: list cursor of (primary lane, bin) for the bins this thread owns: b = warp, warp + 8, ...
+    // list layout of an item: blocks of 8 rows, [block][lane][8] (a lane's 8 entries are one 32-byte sector)
     constexpr int kOwn = (ENCORE_MAX_BINS + kBinWarps - 1) / kBinWarps;
     int kk[kOwn];
     size_t base[kOwn];
     int rows[kOwn];
+    unsigned *stg = hm + nb * kNWord * 32; // [nb][8][32] staging of the open block of every (bin, lane)
     if (FILL) {
         const int ng = g1 - g0;
 #pragma unroll
@@ -280,28 +287,36 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
                 int rank = 0;
                 for (int q = 0; q < nb; ++q) if (a.bin_order[q] == b) rank = q;
                 const int item = rank * ng + (g - g0);
-                base[sI] = (size_t)a.item_off[item] * 32 + lane;
+                base[sI] = (size_t)a.item_off[item] * 32 + (size_t)lane * 8;
                 rows[sI] = a.item_rows[item];
             }
         }
     }
+    auto flush_block = [&](int b, size_t dst) { // stg[b][0..7][lane] -> 32 bytes at list[dst]
+        const unsigned *sp = stg + (b * 8) * 32 + lane;
+        const uint4 v0 = make_uint4(sp[0], sp[32], sp[64], sp[96]);
+        const uint4 v1 = make_uint4(sp[128], sp[160], sp[192], sp[224]);
+        uint4 *d = reinterpret_cast<uint4 *>(a.list + dst);
+        __stcs(d, v0);
+        __stcs(d + 1, v1);
+    };
 
     for (int ch = 0; ch < nchunks; ++ch) {
-        // -- phase A: lane = candidate; bin of (primary i, candidate) for all i ------------------------------
+        // -- phase A: every warp stages two words of 32 candidates (fp32, relative to primary 0) and then walks
+        //    through them with lane = primary: the bin of (primary lane, candidate c) lands in lane-private state,
+        //    a hit mask per (bin, word) in FILL and a counter per bin in COUNT; no votes, no atomics -------------
 #pragma unroll 1
         for (int u = 0; u < kCandPerThread; ++u) {
             const int wd = u * kBinWarps + warp;   // word of this chunk handled by this warp
             const int slot = wd * 32 + lane;
             const int s = ch * kChunk + slot;
-            const bool valid = s < T;
-            double4 cj = make_double4(0, 0, 0, 0);
-            float xf = 0.f, yf = 0.f, zf = 0.f;
-            unsigned j = kIdxMask;
-            if (valid) {
+            float4 cf = make_float4(1e18f, 1e18f, 1e18f, 0.f); // beyond the candidate list: never a hit
+            unsigned packed = kPadEntry;
+            if (s < T) {
                 int lo = 0, hi = nr; // rng_off[lo] <= s < rng_off[hi]
                 while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (S.rng_off[mid] <= s) lo = mid; else hi = mid; }
-                j = (unsigned)(S.rng_start[lo] + (s - S.rng_off[lo]));
-                cj = a.pos4[j];
+                const unsigned j = (unsigned)(S.rng_start[lo] + (s - S.rng_off[lo]));
+                const double4 cj = a.pos4[j];
                 double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
                 unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer adds {+L, 0, -L}[code] to x_j
                 if (PERIODIC) {
@@ -309,38 +324,48 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
                     if (ry > G.half) { ry -= G.box; ky = 2; } else if (ry < -G.half) { ry += G.box; ky = 0; }
                     if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
                 }
-                xf = (float)rx; yf = (float)ry; zf = (float)rz;
-                if (FILL) S.jidx[slot] = j | (kx << 26) | (ky << 28) | (kz << 30);
+                cf = make_float4((float)rx, (float)ry, (float)rz, 0.f);
+                packed = j | (kx << 26) | (ky << 28) | (kz << 30);
             }
-            if (FILL) {
-                for (int b = 0; b < nb; ++b) hm[(b * kNWord + wd) * 32 + lane] = 0u;
-                __syncwarp();
-            }
-#pragma unroll 4
-            for (int i = 0; i < cnt; ++i) {
-                unsigned code = kNoHit;
-                bool exact = valid && !fast;
-                if (valid && fast) {
-                    const float dx = xf - S.spf[i], dy = yf - S.spf[32 + i], dz = zf - S.spf[64 + i];
-                    const float t = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    const float rinv = rsqrtf(t);
-                    const float r = t * rinv;                       // NaN for t == 0: falls to the exact path
-                    const float uu = (r - rmin_f) * invw_f;
-                    const float du = fmaf(kA, r + rmin_f, fmaf(kB, rinv, 9.5367431640625e-07f * fabsf(uu)));
-                    if (!(uu < -du || uu >= nb_f + du)) {           // not surely outside [r_min, r_max)
+            S.cand4[slot] = cf;
+            S.jidx[slot] = packed;
+            if (FILL) for (int b = 0; b < nb; ++b) hm[(b * kNWord + wd) * 32 + lane] = 0u;
+            __syncwarp();
+            const int nvalid = min(32, T - (ch * kChunk + wd * 32)); // candidates of this word (<= 0: none)
+            if (lane < cnt) {
+                unsigned amb = 0u; // candidates whose pair with this primary needs the exact fp64 decision
+                if (fast) {
+#pragma unroll 8
+                    for (int c = 0; c < 32; ++c) {
+                        const float4 q = S.cand4[wd * 32 + c];
+                        const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
+                        const float t = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        float rinv;
+                        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(t));
+                        const float uu = fmaf(t * rinv, invw_f, c0);    // NaN for t == 0 -> exact path
+                        const float du = fmaf(kB, rinv, duc);
                         const float fl = floorf(uu);
                         const float fr = uu - fl;
-                        if (fl >= 0.f && fl < nb_f && fr >= du && fr <= 1.f - du) code = (unsigned)(int)fl;
-                        else exact = true;
+                        const bool sure = fr >= du && fr <= 1.f - du;   // farther than du from every bin edge
+                        if (!sure && !(uu < -du) && !(uu >= nb_f + du)) amb |= 1u << c;
+                        if (sure && uu >= 0.f && uu < nb_f) {
+                            const int code = (int)fl;
+                            if (FILL) hm[(code * kNWord + wd) * 32 + lane] |= 1u << c;
+                            else wcnt[code * 32 + lane] += 1;
+                        }
                     }
-                }
-                if (exact)
-                    code = j == (unsigned)(first + i) ? kNoHit
-                                                      : classify_exact<PERIODIC>(cj, S.sp, i, S.e2, nb, G.box, G.half, rmin_f, invw_f);
-                const unsigned grp = __match_any_sync(kFull, code);
-                if (code != kNoHit && lane == __ffs(grp) - 1) {
-                    if (FILL) hm[(code * kNWord + wd) * 32 + i] = grp;
-                    else atomicAdd(&S.cnt[code * 32 + i], __popc(grp));
+                } else if (nvalid > 0) amb = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+                // near a bin edge (~1e-4 of the pairs), or a group too wide for a common image: exact decision
+                while (amb) {
+                    const int c = __ffs(amb) - 1;
+                    amb &= amb - 1;
+                    const unsigned j = S.jidx[wd * 32 + c] & kIdxMask;
+                    if (j == (unsigned)(first + lane)) continue;
+                    const unsigned code = classify_exact<PERIODIC>(a.pos4[j], S.sp, lane, S.e2, nb, G.box, G.half, rmin_f, invw_f);
+                    if (code != kNoHit) {
+                        if (FILL) hm[(code * kNWord + wd) * 32 + lane] |= 1u << c;
+                        else wcnt[code * 32 + lane] += 1;
+                    }
                 }
             }
         }
@@ -357,8 +382,9 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
                             while (m) {
                                 const int c = __ffs(m) - 1;
                                 m &= m - 1;
-                                a.list[base[sI] + (size_t)kk[sI] * 32] = S.jidx[q * 32 + c];
+                                stg[(b * 8 + (kk[sI] & 7)) * 32 + lane] = S.jidx[q * 32 + c];
                                 ++kk[sI];
+                                if ((kk[sI] & 7) == 0) flush_block(b, base[sI] + (size_t)(kk[sI] / 8 - 1) * 256);
                             }
                         }
                     }
@@ -369,16 +395,34 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
     }
 
     if (FILL) {
-        // pad the unused tail of every lane's column
+        // close the open block of every lane and pad the rest of its column
 #pragma unroll
         for (int sI = 0; sI < kOwn; ++sI) {
             const int b = warp + sI * kBinWarps;
-            if (b < nb)
-                for (int k = (lane < cnt ? kk[sI] : 0); k < rows[sI]; ++k) a.list[base[sI] + (size_t)k * 32] = kPadEntry;
+            if (b < nb) {
+                int k = lane < cnt ? kk[sI] : 0;
+                if (k & 7) {
+                    for (int q = k & 7; q < 8; ++q) stg[(b * 8 + q) * 32 + lane] = kPadEntry;
+                    flush_block(b, base[sI] + (size_t)(k / 8) * 256);
+                    k = (k + 7) & ~7;
+                }
+                const uint4 padv = make_uint4(kPadEntry, kPadEntry, kPadEntry, kPadEntry);
+                for (; k < rows[sI]; k += 8) {
+                    uint4 *d = reinterpret_cast<uint4 *>(a.list + base[sI] + (size_t)(k / 8) * 256);
+                    __stcs(d, padv);
+                    __stcs(d + 1, padv);
+                }
+            }
         }
     } else {
         __syncthreads();
-        for (int k = tid; k < nb * 32; k += nthreads) a.counts[(size_t)g * nb * 32 + k] = (uint32_t)S.cnt[k];
+        const int *all = reinterpret_cast<const int *>(hm);
+        for (int k = tid; k < nb * 32; k += nthreads) {
+            int tot = 0;
+#pragma unroll
+            for (int w = 0; w < kBinWarps; ++w) tot += all[w * nb * 32 + k];
+            a.counts[(size_t)g * nb * 32 + k] = (uint32_t)tot;
+        }
     }
 }
 
@@ -390,7 +434,7 @@ __global__ void k_group_rows(PairArgs a)
     const int lane = threadIdx.x & 31, nb = a.bins.nbins;
     int tot = 0;
     if (g < a.group_start[a.geom.npencil])
-        for (int b = 0; b < nb; ++b) tot += (int)__reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]);
+        for (int b = 0; b < nb; ++b) tot += ((int)__reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]) + 7) & ~7;
     if (lane == 0) a.grows[g] = tot;
 }
 
@@ -403,7 +447,7 @@ __global__ void k_item_rows(PairArgs a, int g0, int g1)
     const int lane = threadIdx.x & 31;
     const int b = a.bin_order[item / ng], g = g0 + item % ng;
     const unsigned m = __reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]);
-    if (lane == 0) a.item_rows[item] = (int)m;
+    if (lane == 0) a.item_rows[item] = ((int)m + 7) & ~7; // whole blocks of 8 rows
 }
 
 // ==========================================================================================================
@@ -427,22 +471,29 @@ __device__ __forceinline__ double4 fetch(const double4 *__restrict__ pos4, unsig
 }
 
 template <int LMAX, int MLO, int MHI, int MODE>
-__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ col,
-                                          int rows, const double4 *__restrict__ pos4, const double4 &me, double box, double half)
+__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const uint4 *__restrict__ col,
+                                          int nblk, const double4 *__restrict__ pos4, const double4 &me, double box, double half)
 {
+    // col: this lane's two uint4 of block 0; block kb is 64 uint4 further (32 lanes x 2)
     const double4 pad = make_double4(me.x + 1.0, me.y, me.z, 0.0); // padding entry: unit separation, weight 0
-    unsigned e1 = rows > 1 ? __ldcs(col + 32) : kPadEntry;
-    double4 p0 = fetch<MODE>(pos4, rows > 0 ? __ldcs(col) : kPadEntry, pad, box);
-    for (int k = 0; k < rows; ++k) {
-        const unsigned e2 = k + 2 < rows ? __ldcs(col + (size_t)(k + 2) * 32) : kPadEntry;
-        const double4 p1 = fetch<MODE>(pos4, e1, pad, box);
-        const double dx = sep<MODE == 2>(p0.x, me.x, box, half);
-        const double dy = sep<MODE == 2>(p0.y, me.y, box, half);
-        const double dz = sep<MODE == 2>(p0.z, me.z, box, half);
-        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        const double rinv = rsqrt(r2);
-        accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, p0.w);
-        p0 = p1; e1 = e2;
+    const uint4 padv = make_uint4(kPadEntry, kPadEntry, kPadEntry, kPadEntry);
+    uint4 q0 = nblk > 0 ? __ldcs(col) : padv, q1 = nblk > 0 ? __ldcs(col + 1) : padv;
+    double4 p0 = fetch<MODE>(pos4, q0.x, pad, box);
+    for (int kb = 0; kb < nblk; ++kb) {
+        const unsigned e[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+        if (kb + 1 < nblk) { q0 = __ldcs(col + (size_t)(kb + 1) * 64); q1 = __ldcs(col + (size_t)(kb + 1) * 64 + 1); }
+        else { q0 = padv; q1 = padv; }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const double4 p1 = fetch<MODE>(pos4, u < 7 ? e[u + 1] : q0.x, pad, box); // next candidate, one step ahead
+            const double dx = sep<MODE == 2>(p0.x, me.x, box, half);
+            const double dy = sep<MODE == 2>(p0.y, me.y, box, half);
+            const double dz = sep<MODE == 2>(p0.z, me.z, box, half);
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double rinv = rsqrt(r2);
+            accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, p0.w);
+            p0 = p1;
+        }
     }
 }
 
@@ -455,8 +506,8 @@ __global__ void __launch_bounds__(kHarmWarps * 32) k_harm(PairArgs a, int g0, in
     const int item = blockIdx.x * kHarmWarps + warp;
     if (item >= ng * nb) return;
     const int bin = a.bin_order[item / ng], g = g0 + item % ng;
-    const int rows = a.item_rows[item];
-    const unsigned *col = a.list + (size_t)a.item_off[item] * 32 + lane;
+    const int rows = a.item_rows[item] >> 3; // blocks of 8 rows
+    const uint4 *col = reinterpret_cast<const uint4 *>(a.list + (size_t)a.item_off[item] * 32) + lane * 2;
     const Group gr = locate_group<PERIODIC>(a, g);
     const bool active = lane < gr.cnt;
     const double4 me = a.pos4[gr.first + (active ? lane : 0)];
@@ -504,8 +555,9 @@ int pair_stage_supported(int lmax, int nbins)
 cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches)
 {
     if (a.ngroups <= 0) return cudaSuccess;
-    if (a.geom.periodic) k_bin<true, false><<<a.ngroups, kBinWarps * 32, 0, s>>>(a, 0, a.ngroups);
-    else k_bin<false, false><<<a.ngroups, kBinWarps * 32, 0, s>>>(a, 0, a.ngroups);
+    const size_t cnt_bytes = (size_t)kBinWarps * a.bins.nbins * 32 * sizeof(int);
+    if (a.geom.periodic) k_bin<true, false><<<a.ngroups, kBinWarps * 32, cnt_bytes, s>>>(a, 0, a.ngroups);
+    else k_bin<false, false><<<a.ngroups, kBinWarps * 32, cnt_bytes, s>>>(a, 0, a.ngroups);
     k_group_rows<<<(a.ngroups + 7) / 8, 256, 0, s>>>(a);
     *launches += 2;
     cudaError_t e = cudaGetLastError();
@@ -529,7 +581,7 @@ cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, cudaSt
     *launches += 1;
     cudaError_t e = launch_exclusive_scan(a.item_rows, a.item_off, nitems, a.scan_tmp, s, launches);
     if (e != cudaSuccess) return e;
-    const size_t hm_bytes = (size_t)nb * kNWord * 32 * sizeof(unsigned);
+    const size_t hm_bytes = (size_t)nb * (kNWord + 8) * 32 * sizeof(unsigned); // hit masks + staging blocks
     if (a.geom.periodic) {
         e = cudaFuncSetAttribute(k_bin<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hm_bytes);
         if (e != cudaSuccess) return e;
