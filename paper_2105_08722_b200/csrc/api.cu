@@ -39,10 +39,10 @@ struct encore_plan_s {
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
     DevBuf io_pos, io_w, io_zeta;
-    DevBuf grows, gprefix, item_rows, item_off, list;
+    DevBuf gbound, gprefix, pool, pool_cursor, page_next, first_page;
     int *h_gprefix = nullptr;   // pinned
     size_t h_gprefix_cap = 0;
-    size_t list_budget_bytes = (size_t)24 << 30;
+    size_t list_budget_bytes = (size_t)32 << 30;
     int pair_steps = 0;
     double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6]
     // state of the last compute
@@ -188,12 +188,14 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
     GridGeom G;
     choose_geometry(P, n, P->pinned, P->pinned + 3, G);
+    int nr_cap;
     {
         int Ry = (int)std::floor(T.rmax * G.inv[1] + 1e-6) + 1, Rz = (int)std::floor(T.rmax * G.inv[2] + 1e-6) + 1;
         if (!G.periodic) { Ry = std::min(Ry, G.nc[1] - 1); Rz = std::min(Rz, G.nc[2] - 1); }
         const int wy = std::min(2 * Ry + 1, G.periodic ? G.nc[1] : 2 * Ry + 1);
         const int wz = std::min(2 * Rz + 1, G.periodic ? G.nc[2] : 2 * Rz + 1);
-        if (2 * wy * wz > 1024) return ENCORE_EUNSUPPORTED;
+        nr_cap = 2 * wy * wz;   // candidate runs of a group (k_fill keeps their table in shared memory)
+        if (pair_fill_smem_bytes(T.nbins, nr_cap) > 200 * 1024) return ENCORE_EUNSUPPORTED;
     }
     const int ngmax = (int)(n / ENCORE_GROUP) + G.npencil + 1;
     const int nb = T.nbins, ncomp = T.ncomp;
@@ -253,11 +255,16 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.cand_pairs = P->cand.as<unsigned long long>();
     pa.gweights = P->gweights.as<double>();
     pa.ngroups = ngmax;
-    CU(P->grows.ensure(sizeof(int) * (size_t)ngmax));
+    CU(P->gbound.ensure(sizeof(int) * (size_t)ngmax));
     CU(P->gprefix.ensure(sizeof(int) * ((size_t)ngmax + 2)));
-    pa.grows = P->grows.as<int>();
+    CU(P->first_page.ensure(sizeof(int) * (size_t)ngmax * nb * 32));
+    CU(P->pool_cursor.ensure(sizeof(unsigned) * 2));
+    pa.gbound = P->gbound.as<int>();
     pa.gprefix = P->gprefix.as<int>();
     pa.scan_tmp = P->scan_tmp.as<int>();
+    pa.first_page = P->first_page.as<int>();
+    pa.pool_cursor = P->pool_cursor.as<unsigned>();
+    pa.err_flag = reinterpret_cast<int *>(P->pool_cursor.as<unsigned>() + 1);
     if (P->h_gprefix_cap < (size_t)ngmax + 2) {
         if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
         P->h_gprefix = nullptr; P->h_gprefix_cap = 0;
@@ -265,35 +272,35 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         P->h_gprefix_cap = (size_t)ngmax + 2;
     }
     CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
-    CU(launch_pair_count(pa, s, &P->launches));
-    // second small device->host read: rows per group (prefix) and the number of groups -> super-steps
+    CU(cudaMemsetAsync(P->pool_cursor.p, 0, 2 * sizeof(unsigned), s));
+    CU(launch_pair_bounds(pa, s, &P->launches));
+    // second small device->host read: slab bounds per group (prefix) and the number of groups -> super-steps
     CU(cudaMemcpyAsync(P->h_gprefix, P->gprefix.p, sizeof(int) * ((size_t)ngmax + 1), cudaMemcpyDeviceToHost, s));
     CU(cudaMemcpyAsync(P->h_gprefix + ngmax + 1, P->group_start.as<int>() + G.npencil, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     {
         const int ngroups = P->h_gprefix[ngmax + 1];
         const int *gp = P->h_gprefix;
-        const size_t total_rows = (size_t)gp[ngroups];
-        const size_t budget_rows = std::max<size_t>(P->list_budget_bytes / 128, 1);
-        size_t max_group_rows = 0;
-        for (int g = 0; g < ngroups; ++g) max_group_rows = std::max(max_group_rows, (size_t)(gp[g + 1] - gp[g]));
-        const size_t cap_rows = std::max(std::min(total_rows, budget_rows), max_group_rows);
-        CU(P->list.ensure(std::max<size_t>(cap_rows, 1) * 128));
-        const int max_items = 4000000;
-        const int max_ng = std::max(1, max_items / nb);
-        CU(P->item_rows.ensure(sizeof(int) * (size_t)std::min(ngroups, max_ng) * nb + 64));
-        CU(P->item_off.ensure(sizeof(int) * (size_t)std::min(ngroups, max_ng) * nb + 64));
-        pa.item_rows = P->item_rows.as<int>();
-        pa.item_off = P->item_off.as<int>();
-        pa.list = P->list.as<unsigned>();
-        pa.list_rows_cap = cap_rows;
+        const size_t slab_bytes = (size_t)ENCORE_SLAB_PAGES * ENCORE_PAGE_WORDS * sizeof(unsigned);
+        const size_t total_slabs = (size_t)gp[ngroups];
+        const size_t budget_slabs = std::max<size_t>(P->list_budget_bytes / slab_bytes, 1);
+        size_t max_group_slabs = 0;
+        for (int g = 0; g < ngroups; ++g) max_group_slabs = std::max(max_group_slabs, (size_t)(gp[g + 1] - gp[g]));
+        const size_t cap_slabs = std::max(std::min(total_slabs, budget_slabs), std::max<size_t>(max_group_slabs, 1));
+        const size_t cap_pages = cap_slabs * ENCORE_SLAB_PAGES;
+        if (cap_pages >= ((size_t)1 << 31)) return ENCORE_EUNSUPPORTED;
+        CU(P->pool.ensure(cap_slabs * slab_bytes));
+        CU(P->page_next.ensure(cap_pages * sizeof(int)));
+        pa.pool = P->pool.as<unsigned>();
+        pa.pool_pages = (unsigned)cap_pages;
+        pa.page_next = P->page_next.as<int>();
         pa.ngroups = ngroups;
         P->pair_steps = 0;
         int g0 = 0;
         while (g0 < ngroups) {
             int g1 = g0 + 1;
-            while (g1 < ngroups && g1 - g0 < max_ng && (size_t)(gp[g1 + 1] - gp[g0]) <= cap_rows) ++g1;
-            CU(launch_pair_fill_harmonics(pa, g0, g1, s, &P->launches));
+            while (g1 < ngroups && (size_t)(gp[g1 + 1] - gp[g0]) <= cap_slabs) ++g1;
+            CU(launch_pair_fill_harmonics(pa, g0, g1, nr_cap, s, &P->launches));
             ++P->pair_steps;
             g0 = g1;
         }
@@ -394,8 +401,8 @@ int encore_destroy(encore_plan_t *P)
                       &P->d_lam_order, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
-                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->grows, &P->gprefix, &P->item_rows,
-                      &P->item_off, &P->list};
+                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->pool,
+                      &P->pool_cursor, &P->page_next, &P->first_page};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);

@@ -8,6 +8,8 @@
 #define ENCORE_MAX_BINS 32
 #define ENCORE_MAX_LMAX 10
 #define ENCORE_GROUP 32              // primaries per group = lanes of a warp
+#define ENCORE_PAGE_WORDS 64         // candidate-list page: 64 entries (256 bytes) of one (primary, bin) list
+#define ENCORE_SLAB_PAGES 256        // pages a warp takes from the pool at a time (64 kB)
 
 // Real-component layout of one a_lm tile row (per radial bin): (lmax+1)^2 doubles,
 //   (l,0) at l*l;  Re(l,m) at l*l+2m-1;  Im(l,m) at l*l+2m   (m = 1..l).

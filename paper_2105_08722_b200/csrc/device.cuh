@@ -61,21 +61,24 @@ struct PairArgs {
     uint32_t *counts;           // [ngroups][nbins][32]  accepted pairs per (primary, bin): integer output of a3
     unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)
     double *gweights;           // [ngroups][32] weight of (group, lane), 0 for empty lanes
-    int ngroups;                // upper bound n/32 + npencil + 1 for the count pass; exact afterwards
-    // candidate lists: item = (bin rank, group) of the current super-step; rows of 32 lanes
-    int *grows;                 // [ngroups]   rows needed by a group (sum over bins of max over lanes)
-    int *gprefix;               // [ngroups+1] exclusive scan of grows
-    int *item_rows;             // [nbins * ngroups]
-    int *item_off;              // [nbins * ngroups + 1]
+    int ngroups;                // upper bound n/32 + npencil + 1 before the bounds are read back; exact afterwards
+    // candidate lists: one list per (group, bin, lane) = chain of 256-byte pages of `pool`
+    int *gbound;                // [ngroups]   upper bound on the pool slabs a group can take
+    int *gprefix;               // [ngroups+1] exclusive scan of gbound
     int *scan_tmp;
-    unsigned *list;             // [list_rows_cap][32] entries: sorted index | image codes << 26; 0xffffffff = padding
-    size_t list_rows_cap;
+    unsigned *pool;             // [pool_pages][64] entries: sorted index | image codes << 26; 0xffffffff = padding
+    unsigned pool_pages;
+    unsigned *pool_cursor;      // next free page (advanced a slab at a time)
+    int *page_next;             // [pool_pages] next page of the same list
+    int *first_page;            // [ngroups][nbins][32] first page of the list of (group, bin, lane)
+    int *err_flag;              // set if the pool overflowed (excluded by the step bounds)
     int bin_order[ENCORE_MAX_BINS]; // bins by decreasing shell volume (work per item)
 };
-// count pass over all groups; fills counts, grows, gprefix (device).  The caller then reads gprefix back,
-// sizes `list`, and calls launch_pair_fill_harmonics once per super-step [g0, g1).
-cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches);
-cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches);
+// per-group slab bounds -> gbound, gprefix (device).  The caller reads gprefix back, sizes the pool, and calls
+// launch_pair_fill_harmonics once per super-step [g0, g1); nr_cap >= number of candidate runs of a group.
+cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches);
+cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches);
+size_t pair_fill_smem_bytes(int nbins, int nr_cap);
 int pair_stage_supported(int lmax, int nbins);
 
 // ---- contract.cu ----------------------------------------------------------------------------------------

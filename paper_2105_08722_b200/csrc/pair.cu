@@ -4,19 +4,19 @@
 //
 // The paper does this on the CPU, histogramming Cartesian monomials with AVX, eight secondaries at a time
 // (Alg. 2) and has no GPU version of it.  Design here:
-// the work is split by resource profile into three kernels around "groups" of 32 consecutive cell-sorted
+// the work is split by resource profile into two kernels around "groups" of 32 consecutive cell-sorted
 // primaries of one (iy,iz) pencil (lane = primary everywhere):
-//   k_bin<COUNT>  (a3, integer/fp32, few registers, high occupancy): candidates = contiguous runs of the sorted
-//     array (one per neighbouring pencil, x-range culled against the group's cell range); lane = candidate, loop
-//     over the 32 primaries.  A first fp32 evaluation on coordinates relative to the group decides every pair
-//     whose radius is farther than a proven error margin from all bin edges; the rest (~1e-4) is decided in fp64
-//     exactly as DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so counts are
-//     bit-exact.  __match_any_sync turns the 32 codes of a warp step into one hit mask per (primary, bin).
-//     Output: n_i(b), the per-(primary, bin) pair counts (an integer output of the path), which also size
-//   k_bin<FILL>   (a3 again, same tests): thread (i,b) pops the set bits of its masks, in candidate order, into
-//     the candidate list of item (group, b) in HBM: rows of 32 lanes, 4 bytes per accepted pair.
-//   k_harm        (a4, fp64, ~140 registers): one warp per item streams its rows (coalesced), gathers the
-//     candidates, and thread (i,b) keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
+//   k_fill  (a3, integer/fp32, few registers): ONE WARP per group.  Candidates = contiguous runs of the sorted
+//     array (one or two per neighbouring pencil, x-range culled against the group's cell range), staged 32 at a
+//     time in shared memory relative to primary 0 in fp32 and broadcast to the lanes.  A first fp32 evaluation
+//     decides every pair whose radius is farther than a proven error margin from all bin edges; the rest (~1e-4)
+//     is decided in fp64 exactly as DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so
+//     counts are bit-exact.  An accepted pair is appended, in candidate order, to the list of (primary, bin):
+//     lane-private cursors and an 8-entry ring per (bin, lane) in shared memory, flushed 4 entries (16 bytes)
+//     at a time into 256-byte pages of a pool in HBM; pages of one list are chained through page_next[].
+//     The final cursors are n_i(b), the per-(primary, bin) pair counts (an integer output of the path).
+//   k_harm  (a4, fp64, ~130 registers): one warp per (group, bin); every lane streams its own list, gathers the
+//     candidates two rows ahead, and keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
 //     atomics, no cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit
 //     vector, w (x+iy)^m by complex recurrence, monic associated-Legendre polynomials
 //     p_lm(z) = z p_{l-1,m} - gamma_lm p_{l-2,m}, one FMA per component; normalisation (-1)^m N_lm k_lm / v_b once
@@ -28,16 +28,14 @@
 
 namespace {
 
-constexpr int kBinWarps = 8;        // k_bin: warps per CTA
-constexpr int kCandPerThread = 2;   // k_bin: candidates per thread and chunk
-constexpr int kNWord = kBinWarps * kCandPerThread;      // 32-candidate words per chunk
-constexpr int kChunk = kNWord * 32;
-constexpr int kMaxRanges = 1024;
+constexpr int kRing = 8;            // k_fill: ring entries per (bin, lane): a block of 4 is flushed while the other fills
 constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
 constexpr unsigned kPadEntry = 0xffffffffu;
 constexpr unsigned kIdxMask = 0x3ffffffu;
+constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: (x + kMagic) - kMagic = round-to-nearest-integer(x)
+constexpr int kMagicBits = 0x4B400000;
 
 __host__ __device__ constexpr int ncomp_range(int lmax, int mlo, int mhi)
 {
@@ -99,7 +97,7 @@ __device__ __forceinline__ double sep(double xj, double xi, double box, double h
     return d;
 }
 
-// ---- the group of a CTA / warp ---------------------------------------------------------------------------
+// ---- the group of a warp ---------------------------------------------------------------------------------
 struct Group {
     int first, cnt;      // sorted index of primary 0, number of primaries (1..32)
     int py, pz;          // pencil
@@ -130,73 +128,23 @@ __device__ __forceinline__ Group locate_group(const PairArgs &a, int g)
     return gr;
 }
 
-// ==========================================================================================================
-// k_bin: a3.  COUNT: counts[g][b][lane].  FILL: candidate lists.
-// ==========================================================================================================
-struct BinSmem {
-    double sp[96];                 // [3][32] primary positions (exact)
-    double e2[ENCORE_MAX_BINS + 2];
-    float4 cand4[kChunk];          // candidates of the chunk relative to primary 0, fp32
-    int rng_start[kMaxRanges];
-    int rng_off[kMaxRanges + 4];
-    unsigned jidx[kChunk];         // sorted index | image codes << 26
-};
-
-// exact decision, the operations of DESIGN.md R8-R10 (the oracle's): returns the bin or kNoHit
-template <bool PERIODIC>
-__device__ __noinline__ unsigned classify_exact(const double4 &cj, const double *sp, int i, const double *e2, int nb,
-                                                   double box, double half, float rmin_f, float invw_f)
+// ---- candidate ranges of a group (one warp): one or two runs of the sorted array per neighbouring pencil -----
+// STORE: rng_start[r] = first sorted index of run r, rng_off[r] = candidates before run r (rng_off[nr] = total).
+// Returns the number of candidates T of the group.
+template <bool PERIODIC, bool STORE>
+__device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, int lane, int *rng_start, int *rng_off,
+                                            int *nr_out)
 {
-    const double dx = sep<PERIODIC>(cj.x, sp[i], box, half);
-    const double dy = sep<PERIODIC>(cj.y, sp[32 + i], box, half);
-    const double dz = sep<PERIODIC>(cj.z, sp[64 + i], box, half);
-    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-    if (!(r2 > 0.0 && r2 >= e2[0] && r2 < e2[nb])) return kNoHit; // DESIGN.md R8
-    int b = (int)((sqrtf((float)r2) - rmin_f) * invw_f);
-    b = max(0, min(nb - 1, b));
-    while (r2 < e2[b]) --b;               // DESIGN.md R9: the decision is on squares, fp64
-    while (!(r2 < e2[b + 1])) ++b;
-    return (unsigned)b;
-}
-
-template <bool PERIODIC, bool FILL>
-__global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int g1)
-{
-    const int g = g0 + blockIdx.x;
     const GridGeom &G = a.geom;
-    if (g >= g1 || g >= a.group_start[G.npencil]) return;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nb = a.bins.nbins;
-    constexpr int nthreads = kBinWarps * 32;
-
-    __shared__ BinSmem S;
-    extern __shared__ __align__(16) unsigned hm[]; // FILL: [nb][kNWord][32] hit masks of the current chunk
-
-    const Group gr = locate_group<PERIODIC>(a, g);
-    const int first = gr.first, cnt = gr.cnt;
-    const double4 ctr = a.pos4[first];
-    if (warp == 0) {
-        const double4 me = a.pos4[first + (lane < cnt ? lane : 0)];
-        S.sp[lane] = me.x; S.sp[32 + lane] = me.y; S.sp[64 + lane] = me.z;
-        if (!FILL) a.gweights[(size_t)g * 32 + lane] = lane < cnt ? me.w : 0.0;
-    }
-    if (tid <= nb) S.e2[tid] = a.bins.e2[tid];
-    // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
-    const double4 mine = a.pos4[first + (lane < cnt ? lane : 0)];
-    const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
-    // COUNT: per-warp private counters [warp][bin][lane] in dynamic shared memory
-    int *wcnt = reinterpret_cast<int *>(hm) + warp * nb * 32;
-    if (!FILL) for (int b = 0; b < nb; ++b) wcnt[b * 32 + lane] = 0;
-
-    // ---- candidate ranges: one or two runs of the sorted array per neighbouring pencil ------------------
     const int ncx = G.nc[0], ncy = G.nc[1], ncz = G.nc[2];
     int Ry = (int)floor(a.rmax * G.inv[1] + 1e-6) + 1, Rz = (int)floor(a.rmax * G.inv[2] + 1e-6) + 1;
     if (!PERIODIC) { Ry = min(Ry, ncy - 1); Rz = min(Rz, ncz - 1); } // nothing beyond the grid
     const bool full_y = PERIODIC && (2 * Ry + 1 >= ncy), full_z = PERIODIC && (2 * Rz + 1 >= ncz);
     const int wy = full_y ? ncy : 2 * Ry + 1, wz = full_z ? ncz : 2 * Rz + 1;
-    const int nyz = wy * wz; // host guarantees 2*nyz <= kMaxRanges
+    const int nyz = wy * wz; // host guarantees 2*nyz <= nr_cap
     const double rmax2 = a.rmax * a.rmax;
-    for (int r = tid; r < nyz; r += nthreads) {
+    int mine = 0;
+    for (int r = lane; r < nyz; r += 32) {
         const int iy = r % wy, iz = r / wy;
         int cy, cz, dyc, dzc;
         bool ok = true;
@@ -237,263 +185,369 @@ __global__ void __launch_bounds__(kBinWarps * 32) k_bin(PairArgs a, int g0, int 
                 }
             }
         }
-        S.rng_start[2 * r] = s0; S.rng_off[2 * r + 1] = l0;       // lengths parked in rng_off[.+1], scanned below
-        S.rng_start[2 * r + 1] = s1; S.rng_off[2 * r + 2] = l1;
+        mine += l0 + l1;
+        if (STORE) {
+            rng_start[2 * r] = s0; rng_off[2 * r + 1] = l0;       // lengths parked in rng_off[.+1], scanned below
+            rng_start[2 * r + 1] = s1; rng_off[2 * r + 2] = l1;
+        }
     }
-    __syncthreads();
     const int nr = 2 * nyz;
-    if (warp == 0) { // inclusive scan of the lengths into offsets
+    *nr_out = nr;
+    if (!STORE) return __reduce_add_sync(kFull, mine);
+    __syncwarp();
+    { // inclusive scan of the lengths into offsets
         const int per = (nr + 31) / 32;
         const int b0 = lane * per, b1 = min(nr, b0 + per);
         int sum = 0;
-        for (int r = b0; r < b1; ++r) sum += S.rng_off[r + 1];
+        for (int r = b0; r < b1; ++r) sum += rng_off[r + 1];
         int x = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { int y = __shfl_up_sync(kFull, x, d); if (lane >= d) x += y; }
         int run = x - sum;
-        for (int r = b0; r < b1; ++r) { const int len = S.rng_off[r + 1]; run += len; S.rng_off[r + 1] = run; }
-        if (lane == 0) S.rng_off[0] = 0;
+        for (int r = b0; r < b1; ++r) { const int len = rng_off[r + 1]; run += len; rng_off[r + 1] = run; }
+        if (lane == 0) rng_off[0] = 0;
     }
-    __syncthreads();
-    const int T = S.rng_off[nr];
-    const int nchunks = (T + kChunk - 1) / kChunk;
-    if (!FILL && tid == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
+    __syncwarp();
+    return rng_off[nr];
+}
+
+// exact decision, the operations of DESIGN.md R8-R10 (the oracle's): returns the bin or kNoHit
+template <bool PERIODIC>
+__device__ __noinline__ unsigned classify_exact(const double4 &cj, const double *sp, int i, const double *e2, int nb,
+                                                   double box, double half, float rmin_f, float invw_f)
+{
+    const double dx = sep<PERIODIC>(cj.x, sp[i], box, half);
+    const double dy = sep<PERIODIC>(cj.y, sp[32 + i], box, half);
+    const double dz = sep<PERIODIC>(cj.z, sp[64 + i], box, half);
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if (!(r2 > 0.0 && r2 >= e2[0] && r2 < e2[nb])) return kNoHit; // DESIGN.md R8
+    int b = (int)((sqrtf((float)r2) - rmin_f) * invw_f);
+    b = max(0, min(nb - 1, b));
+    while (r2 < e2[b]) --b;               // DESIGN.md R9: the decision is on squares, fp64
+    while (!(r2 < e2[b + 1])) ++b;
+    return (unsigned)b;
+}
+
+// upper bound on the pool slabs a group can take (see k_fill: a slab yields >= kSlabPages-31 usable pages)
+__device__ __forceinline__ int slab_bound(long long cand, int cnt, int nb)
+{
+    const long long need = (cand * cnt) / ENCORE_PAGE_WORDS + (long long)cnt * nb;
+    const long long slabs = need / (ENCORE_SLAB_PAGES - 31) + 1;
+    return (int)(slabs > INT_MAX ? INT_MAX : slabs);
+}
+
+// per group: candidates T and the slab bound (sizes the super-steps on the host)
+template <bool PERIODIC>
+__global__ void __launch_bounds__(128) k_group_bound(PairArgs a)
+{
+    const int g = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (g >= a.ngroups) return;
+    if (g >= a.group_start[a.geom.npencil]) { if (lane == 0) a.gbound[g] = 0; return; }
+    const Group gr = locate_group<PERIODIC>(a, g);
+    int nr;
+    const int T = build_ranges<PERIODIC, false>(a, gr, lane, nullptr, nullptr, &nr);
+    if (lane == 0) a.gbound[g] = slab_bound(T, gr.cnt, a.bins.nbins);
+}
+
+// ==========================================================================================================
+// k_fill: a3.  One warp (= one CTA) per group.
+// ==========================================================================================================
+// dynamic shared memory: cand[2][32] float4 | sp[96] double | e2[nb+1] double | ring[nb][16][32] u32 |
+//                        cursor[nb][32] u32 | pagecur[nb][32] int | rng_start[nr_cap] | rng_off[nr_cap+1]
+__host__ __device__ inline size_t fill_smem_bytes(int nb, int nr_cap)
+{
+    return 2 * 32 * 16 + 96 * 8 + (size_t)((nb + 2) & ~1) * 8 + (size_t)nb * kRing * 32 * 4 + (size_t)nb * 32 * 4 * 2 +
+           (size_t)(2 * nr_cap + 4) * 4;
+}
+
+template <bool PERIODIC>
+__global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_cap)
+{
+    const int g = g0 + blockIdx.x;
+    const GridGeom &G = a.geom;
+    if (g >= g1 || g >= a.group_start[G.npencil]) return;
+    const int lane = threadIdx.x;
+    const int nb = a.bins.nbins;
+
+    extern __shared__ __align__(16) unsigned char fill_smem[];
+    float4 *cand = reinterpret_cast<float4 *>(fill_smem);
+    double *sp = reinterpret_cast<double *>(cand + 64);
+    double *e2 = sp + 96;
+    unsigned *ring = reinterpret_cast<unsigned *>(e2 + ((nb + 2) & ~1));
+    unsigned *cursor = ring + nb * kRing * 32;
+    int *pagecur = reinterpret_cast<int *>(cursor + nb * 32);
+    int *rng_start = pagecur + nb * 32;
+    int *rng_off = rng_start + nr_cap;
+
+    const Group gr = locate_group<PERIODIC>(a, g);
+    const int first = gr.first, cnt = gr.cnt;
+    const double4 ctr = a.pos4[first];
+    const double4 mine = a.pos4[first + (lane < cnt ? lane : 0)];
+    sp[lane] = mine.x; sp[32 + lane] = mine.y; sp[64 + lane] = mine.z;
+    a.gweights[(size_t)g * 32 + lane] = lane < cnt ? mine.w : 0.0;
+    if (lane <= nb) e2[lane] = a.bins.e2[lane];
+    for (int b = 0; b < nb; ++b) cursor[b * 32 + lane] = 0u;
+    // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
+    const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
+
+    int nr;
+    const int T = build_ranges<PERIODIC, true>(a, gr, lane, rng_start, rng_off, &nr);
+    if (lane == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
 
     // fp32 screening constants: the bin coordinate u = (r - r_min)/width computed in fp32 is within
     // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one (E^2 = sum of squared group
     // extents).  For r <= 2 r_max the r-dependent part is bounded by the constant duc; beyond, u - du >= N_r trivially.
+    // The loop works with uh = u - 1/2: round-to-nearest(uh) = floor(u) away from the edges, and the pair is surely
+    // inside bin floor(u) iff |uh - rn(uh)| <= 1/2 - du.
     const float rmin_f = a.bins.rmin_f, invw_f = a.bins.invw_f;
-    const float c0 = -rmin_f * invw_f;
+    const float c0h = -rmin_f * invw_f - 0.5f;
     const float nb_f = (float)nb;
     const float duc = 3.814697265625e-06f * invw_f * (2.f * (float)a.rmax + rmin_f) + 9.5367431640625e-07f * (2.f * nb_f + 2.f);
     const float kB = 1.9073486328125e-06f * invw_f *
                      (float)(gr.ext[0] * gr.ext[0] + gr.ext[1] * gr.ext[1] + gr.ext[2] * gr.ext[2]);
+    const float thr0 = 0.5f - duc;
+    const float uh_hi = nb_f - 0.5f;
     const bool fast = gr.fast;
 
-    // FILL: list cursor of (primary lane, bin) for the bins this thread owns: b = warp, warp + 8, ...
-    // list layout of an item: blocks of 8 rows, [block][lane][8] (a lane's 8 entries are one 32-byte sector)
-    constexpr int kOwn = (ENCORE_MAX_BINS + kBinWarps - 1) / kBinWarps;
-    int kk[kOwn];
-    size_t base[kOwn];
-    int rows[kOwn];
-    unsigned *stg = hm + nb * kNWord * 32; // [nb][8][32] staging of the open block of every (bin, lane)
-    if (FILL) {
-        const int ng = g1 - g0;
-#pragma unroll
-        for (int sI = 0; sI < kOwn; ++sI) {
-            const int b = warp + sI * kBinWarps;
-            kk[sI] = 0; base[sI] = 0; rows[sI] = 0;
-            if (b < nb) {
-                int rank = 0;
-                for (int q = 0; q < nb; ++q) if (a.bin_order[q] == b) rank = q;
-                const int item = rank * ng + (g - g0);
-                base[sI] = (size_t)a.item_off[item] * 32 + (size_t)lane * 8;
-                rows[sI] = a.item_rows[item];
+    // ---- list state -----------------------------------------------------------------------------------------
+    // blocks of 4 completed but not yet written: (block index << 5) | bin.  The tests run two candidates between
+    // flushes, a lane appends at most once per candidate, so two slots suffice.
+    int pendA = -1, pendB = -1;
+    int slab_next = 0, slab_end = 0; // pages of the pool owned by this warp (uniform)
+    const unsigned lt_mask = (1u << lane) - 1u;
+
+    // all lanes call; lanes with a pending block write it (4 entries, 16 bytes) to their page.
+    // ring layout [bin][half][lane][4]: the flush is one conflict-free 16-byte shared-memory load
+    auto flush_block = [&](int &pend) {
+        const bool act = pend >= 0;
+        const int b = pend & 31, kb = pend >> 5;
+        const bool newpage = act && (kb & 15) == 0;
+        const unsigned nm = __ballot_sync(kFull, newpage);
+        if (nm) {
+            const int nn = __popc(nm);
+            if (slab_next + nn > slab_end) { // the rest of the old slab (< 32 pages) is dropped: see slab_bound
+                unsigned base = 0;
+                if (lane == 0) base = atomicAdd(a.pool_cursor, (unsigned)ENCORE_SLAB_PAGES);
+                base = __shfl_sync(kFull, base, 0);
+                if (base + ENCORE_SLAB_PAGES > a.pool_pages) { // excluded by the host's step bounds; stay in bounds
+                    if (lane == 0) *a.err_flag = 1;
+                    base = 0;
+                }
+                slab_next = (int)base; slab_end = (int)base + ENCORE_SLAB_PAGES;
             }
+            if (newpage) {
+                const int pg = slab_next + __popc(nm & lt_mask);
+                if (kb == 0) a.first_page[((size_t)g * nb + b) * 32 + lane] = pg;
+                else a.page_next[pagecur[b * 32 + lane]] = pg;
+                pagecur[b * 32 + lane] = pg;
+            }
+            slab_next += nn;
         }
-    }
-    auto flush_block = [&](int b, size_t dst) { // stg[b][0..7][lane] -> 32 bytes at list[dst]
-        const unsigned *sp = stg + (b * 8) * 32 + lane;
-        const uint4 v0 = make_uint4(sp[0], sp[32], sp[64], sp[96]);
-        const uint4 v1 = make_uint4(sp[128], sp[160], sp[192], sp[224]);
-        uint4 *d = reinterpret_cast<uint4 *>(a.list + dst);
-        __stcs(d, v0);
-        __stcs(d + 1, v1);
+        if (act) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(ring + ((((b << 1) | (kb & 1)) << 5) + lane) * 4);
+            __stcs(reinterpret_cast<uint4 *>(a.pool + (size_t)pagecur[b * 32 + lane] * ENCORE_PAGE_WORDS + ((kb & 15) << 2)), v);
+        }
+        pend = -1;
+    };
+    auto flush_all = [&]() {
+        if (__any_sync(kFull, pendA >= 0)) {
+            flush_block(pendA);
+            if (__any_sync(kFull, pendB >= 0)) flush_block(pendB);
+        }
+    };
+    auto append = [&](unsigned code, unsigned entry) {
+        unsigned *cp = cursor + code * 32 + lane;
+        const unsigned pos = *cp;
+        *cp = pos + 1u;
+        ring[((((code << 1) | ((pos >> 2) & 1u)) << 5) + lane) * 4 + (pos & 3u)] = entry;
+        if ((pos & 3u) == 3u) {
+            const int v = (int)(((pos >> 2) << 5) | code);
+            if (pendA < 0) pendA = v; else pendB = v;
+        }
     };
 
-    for (int ch = 0; ch < nchunks; ++ch) {
-        // -- phase A: every warp stages two words of 32 candidates (fp32, relative to primary 0) and then walks
-        //    through them with lane = primary: the bin of (primary lane, candidate c) lands in lane-private state,
-        //    a hit mask per (bin, word) in FILL and a counter per bin in COUNT; no votes, no atomics -------------
+    // ---- staging of a word of 32 candidates (fp32, relative to primary 0; .w = list entry) ----------------------
+    auto load_cand = [&](int s, double4 &cj, unsigned &j) {
+        j = kPadEntry;
+        if (s < T) {
+            int lo = 0, hi = nr; // rng_off[lo] <= s < rng_off[hi]
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (rng_off[mid] <= s) lo = mid; else hi = mid; }
+            j = (unsigned)(rng_start[lo] + (s - rng_off[lo]));
+            cj = a.pos4[j];
+        }
+    };
+    auto stage = [&](int buf, const double4 &cj, unsigned j) {
+        float4 cf = make_float4(1e18f, 1e18f, 1e18f, __uint_as_float(kPadEntry)); // beyond the list: never a hit
+        if (j != kPadEntry) {
+            double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
+            unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer subtracts {-L, 0, +L}[code] from x_i
+            if (PERIODIC) {
+                if (rx > G.half) { rx -= G.box; kx = 2; } else if (rx < -G.half) { rx += G.box; kx = 0; }
+                if (ry > G.half) { ry -= G.box; ky = 2; } else if (ry < -G.half) { ry += G.box; ky = 0; }
+                if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
+            }
+            cf = make_float4((float)rx, (float)ry, (float)rz, __uint_as_float(j | (kx << 26) | (ky << 28) | (kz << 30)));
+        }
+        cand[buf * 32 + lane] = cf;
+    };
+
+    const int nwords = (T + 31) >> 5;
+    double4 cj = make_double4(0, 0, 0, 0);
+    unsigned cjx = kPadEntry;
+    load_cand(lane, cj, cjx);
+    stage(0, cj, cjx);
+    __syncwarp();
+    for (int wd = 0; wd < nwords; ++wd) {
+        const int buf = wd & 1;
+        load_cand((wd + 1) * 32 + lane, cj, cjx); // next word: in flight during the tests of this one
+        const float4 *cw = cand + buf * 32;
+        if (fast) {
 #pragma unroll 1
-        for (int u = 0; u < kCandPerThread; ++u) {
-            const int wd = u * kBinWarps + warp;   // word of this chunk handled by this warp
-            const int slot = wd * 32 + lane;
-            const int s = ch * kChunk + slot;
-            float4 cf = make_float4(1e18f, 1e18f, 1e18f, 0.f); // beyond the candidate list: never a hit
-            unsigned packed = kPadEntry;
-            if (s < T) {
-                int lo = 0, hi = nr; // rng_off[lo] <= s < rng_off[hi]
-                while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (S.rng_off[mid] <= s) lo = mid; else hi = mid; }
-                const unsigned j = (unsigned)(S.rng_start[lo] + (s - S.rng_off[lo]));
-                const double4 cj = a.pos4[j];
-                double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
-                unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer adds {+L, 0, -L}[code] to x_j
-                if (PERIODIC) {
-                    if (rx > G.half) { rx -= G.box; kx = 2; } else if (rx < -G.half) { rx += G.box; kx = 0; }
-                    if (ry > G.half) { ry -= G.box; ky = 2; } else if (ry < -G.half) { ry += G.box; ky = 0; }
-                    if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
-                }
-                cf = make_float4((float)rx, (float)ry, (float)rz, 0.f);
-                packed = j | (kx << 26) | (ky << 28) | (kz << 30);
-            }
-            S.cand4[slot] = cf;
-            S.jidx[slot] = packed;
-            if (FILL) for (int b = 0; b < nb; ++b) hm[(b * kNWord + wd) * 32 + lane] = 0u;
-            __syncwarp();
-            const int nvalid = min(32, T - (ch * kChunk + wd * 32)); // candidates of this word (<= 0: none)
-            if (lane < cnt) {
-                unsigned amb = 0u; // candidates whose pair with this primary needs the exact fp64 decision
-                if (fast) {
-#pragma unroll 8
-                    for (int c = 0; c < 32; ++c) {
-                        const float4 q = S.cand4[wd * 32 + c];
-                        const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
-                        const float t = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        float rinv;
-                        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(t));
-                        const float uu = fmaf(t * rinv, invw_f, c0);    // NaN for t == 0 -> exact path
-                        const float du = fmaf(kB, rinv, duc);
-                        const float fl = floorf(uu);
-                        const float fr = uu - fl;
-                        const bool sure = fr >= du && fr <= 1.f - du;   // farther than du from every bin edge
-                        if (!sure && !(uu < -du) && !(uu >= nb_f + du)) amb |= 1u << c;
-                        if (sure && uu >= 0.f && uu < nb_f) {
-                            const int code = (int)fl;
-                            if (FILL) hm[(code * kNWord + wd) * 32 + lane] |= 1u << c;
-                            else wcnt[code * 32 + lane] += 1;
-                        }
-                    }
-                } else if (nvalid > 0) amb = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
-                // near a bin edge (~1e-4 of the pairs), or a group too wide for a common image: exact decision
-                while (amb) {
-                    const int c = __ffs(amb) - 1;
-                    amb &= amb - 1;
-                    const unsigned j = S.jidx[wd * 32 + c] & kIdxMask;
-                    if (j == (unsigned)(first + lane)) continue;
-                    const unsigned code = classify_exact<PERIODIC>(a.pos4[j], S.sp, lane, S.e2, nb, G.box, G.half, rmin_f, invw_f);
-                    if (code != kNoHit) {
-                        if (FILL) hm[(code * kNWord + wd) * 32 + lane] |= 1u << c;
-                        else wcnt[code * 32 + lane] += 1;
-                    }
-                }
-            }
-        }
-        if (FILL) {
-            __syncthreads();
-            // -- phase B: thread (lane = primary, bin) appends its hits, in candidate order, to its list -------
-            if (lane < cnt) {
+            for (int c4 = 0; c4 < 32; c4 += 4) {
+                // four independent tests first (instruction-level parallelism), then the appends in candidate order
+                unsigned ent[4], code[4];
+                bool ok[4], am[4];
 #pragma unroll
-                for (int sI = 0; sI < kOwn; ++sI) {
-                    const int b = warp + sI * kBinWarps;
-                    if (b < nb) {
-                        for (int q = 0; q < kNWord; ++q) {
-                            unsigned m = hm[(b * kNWord + q) * 32 + lane];
-                            while (m) {
-                                const int c = __ffs(m) - 1;
-                                m &= m - 1;
-                                stg[(b * 8 + (kk[sI] & 7)) * 32 + lane] = S.jidx[q * 32 + c];
-                                ++kk[sI];
-                                if ((kk[sI] & 7) == 0) flush_block(b, base[sI] + (size_t)(kk[sI] / 8 - 1) * 256);
-                            }
+                for (int cc = 0; cc < 4; ++cc) {
+                    const float4 q = cw[c4 + cc];
+                    const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
+                    const float t = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), 1e-30f); // t = 0: r = 0 -> exact path
+                    float rinv;
+                    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(t));
+                    const float uh = fmaf(t * rinv, invw_f, c0h);
+                    const float thr = fmaf(-kB, rinv, thr0);
+                    const float v = uh + kMagic;
+                    const float fr = uh - (v - kMagic);
+                    const bool sure = fabsf(fr) <= thr;              // farther than du from every bin edge
+                    // v in [kMagic, kMagic + nb) <=> uh rounds into 0..nb-1 (float bits are monotonic)
+                    code[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
+                    ok[cc] = sure && code[cc] < (unsigned)nb;
+                    am[cc] = !sure && code[cc] + 1u < (unsigned)nb + 2u;
+                    ent[cc] = __float_as_uint(q.w);
+                }
+                if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
+                    if (ok[0]) append(code[0], ent[0]);
+                    if (ok[1]) append(code[1], ent[1]);
+                    flush_all();
+                    if (ok[2]) append(code[2], ent[2]);
+                    if (ok[3]) append(code[3], ent[3]);
+                    flush_all();
+                } else {
+                    // some pair is within the error margin of a bin edge (~1e-4 of the pairs): exact decision
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) {
+                        if (ok[cc]) append(code[cc], ent[cc]);
+                        else if (am[cc] && ent[cc] != kPadEntry) {
+                            const unsigned cx = classify_exact<PERIODIC>(a.pos4[ent[cc] & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
+                            if (cx != kNoHit) append(cx, ent[cc]);
                         }
+                        if (cc & 1) flush_all();
                     }
                 }
             }
-            __syncthreads();
+        } else {
+            // group too wide for a common image: every pair is decided exactly
+            const int nvalid = min(32, T - wd * 32);
+            for (int c = 0; c < nvalid; ++c) {
+                const unsigned e = __float_as_uint(cw[c].w);
+                if (lane < cnt) {
+                    const unsigned code = classify_exact<PERIODIC>(a.pos4[e & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
+                    if (code != kNoHit) append(code, e);
+                }
+                flush_all();
+            }
         }
+        stage(buf ^ 1, cj, cjx);
+        __syncwarp();
     }
 
-    if (FILL) {
-        // close the open block of every lane and pad the rest of its column
-#pragma unroll
-        for (int sI = 0; sI < kOwn; ++sI) {
-            const int b = warp + sI * kBinWarps;
-            if (b < nb) {
-                int k = lane < cnt ? kk[sI] : 0;
-                if (k & 7) {
-                    for (int q = k & 7; q < 8; ++q) stg[(b * 8 + q) * 32 + lane] = kPadEntry;
-                    flush_block(b, base[sI] + (size_t)(k / 8) * 256);
-                    k = (k + 7) & ~7;
-                }
-                const uint4 padv = make_uint4(kPadEntry, kPadEntry, kPadEntry, kPadEntry);
-                for (; k < rows[sI]; k += 8) {
-                    uint4 *d = reinterpret_cast<uint4 *>(a.list + base[sI] + (size_t)(k / 8) * 256);
-                    __stcs(d, padv);
-                    __stcs(d + 1, padv);
-                }
-            }
+    // close the open block of every (bin, lane): pad it to 4 entries, flush, and complete the last group of 8
+    // (k_harm reads 8 entries at a time); cursors are n_i(b)
+    for (int b = 0; b < nb; ++b) {
+        const unsigned k = cursor[b * 32 + lane];
+        a.counts[((size_t)g * nb + b) * 32 + lane] = k;
+        unsigned nblk4 = k >> 2;
+        if (k & 3u) {
+            for (unsigned q = k & 3u; q < 4u; ++q) ring[((((b << 1) | (nblk4 & 1u)) << 5) + lane) * 4 + q] = kPadEntry;
+            pendA = (int)((nblk4 << 5) | (unsigned)b);
+            ++nblk4;
         }
-    } else {
-        __syncthreads();
-        const int *all = reinterpret_cast<const int *>(hm);
-        for (int k = tid; k < nb * 32; k += nthreads) {
-            int tot = 0;
-#pragma unroll
-            for (int w = 0; w < kBinWarps; ++w) tot += all[w * nb * 32 + k];
-            a.counts[(size_t)g * nb * 32 + k] = (uint32_t)tot;
+        flush_all();
+        if (nblk4 & 1u) {
+            for (unsigned q = 0; q < 4u; ++q) ring[((((b << 1) | 1u) << 5) + lane) * 4 + q] = kPadEntry;
+            pendA = (int)((nblk4 << 5) | (unsigned)b);
         }
+        flush_all();
     }
 }
 
-// rows needed by a group: sum over bins of the largest per-lane count
-__global__ void k_group_rows(PairArgs a)
+// ==========================================================================================================
+// k_harm: a4.  One warp per item (group, bin): every lane streams its list, a_lm accumulates in registers.
+// ==========================================================================================================
+struct Raw { double2 xy, zw; };
+
+__device__ __forceinline__ Raw gather(const double4 *__restrict__ pos4, unsigned e)
 {
-    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (g >= a.ngroups) return;
-    const int lane = threadIdx.x & 31, nb = a.bins.nbins;
-    int tot = 0;
-    if (g < a.group_start[a.geom.npencil])
-        for (int b = 0; b < nb; ++b) tot += ((int)__reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]) + 7) & ~7;
-    if (lane == 0) a.grows[g] = tot;
+    Raw r;
+    // a padding entry reads particle 0 (always valid memory); its contribution is cancelled by weight 0 below
+    const double2 *q = reinterpret_cast<const double2 *>(pos4 + (e == kPadEntry ? 0u : (e & kIdxMask)));
+    r.xy = __ldg(q);
+    r.zw = __ldg(q + 1);
+    return r;
 }
 
-// rows of the items of super-step [g0,g1): item = rank(b) * (g1-g0) + (g-g0)
-__global__ void k_item_rows(PairArgs a, int g0, int g1)
-{
-    const int ng = g1 - g0, nb = a.bins.nbins;
-    const int item = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (item >= ng * nb) return;
-    const int lane = threadIdx.x & 31;
-    const int b = a.bin_order[item / ng], g = g0 + item % ng;
-    const unsigned m = __reduce_max_sync(kFull, a.counts[((size_t)g * nb + b) * 32 + lane]);
-    if (lane == 0) a.item_rows[item] = ((int)m + 7) & ~7; // whole blocks of 8 rows
-}
-
-// ==========================================================================================================
-// k_harm: a4.  One warp per item (group, bin): stream the rows, accumulate a_lm in registers.
-// ==========================================================================================================
 // MODE 0: open geometry; 1: periodic, image carried by the entry; 2: periodic, image decided per pair
-template <int MODE>
-__device__ __forceinline__ double4 fetch(const double4 *__restrict__ pos4, unsigned e, const double4 &pad, double box)
-{
-    if (e == kPadEntry) return pad;
-    const double2 *q = reinterpret_cast<const double2 *>(pos4 + (e & kIdxMask));
-    const double2 xy = __ldg(q), zw = __ldg(q + 1);
-    double4 p = make_double4(xy.x, xy.y, zw.x, zw.y);
-    if (MODE == 1) { // x_j + {+L, 0, -L}[code]
-        const unsigned kx = (e >> 26) & 3u, ky = (e >> 28) & 3u, kz = e >> 30;
-        p.x += kx == 1u ? 0.0 : (kx == 0u ? box : -box);
-        p.y += ky == 1u ? 0.0 : (ky == 0u ? box : -box);
-        p.z += kz == 1u ? 0.0 : (kz == 0u ? box : -box);
-    }
-    return p;
-}
-
+// mtab (MODE 1): shared memory [axis][image code][thread] = x_i + {-L, 0, +L}: x_j - (x_i -/+ L) is the minimal image
 template <int LMAX, int MLO, int MHI, int MODE>
-__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const uint4 *__restrict__ col,
-                                          int nblk, const double4 *__restrict__ pos4, const double4 &me, double box, double half)
+__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ pool,
+                                          const int *__restrict__ page_next, int page, int nblk_lane, int nblk,
+                                          const double4 *__restrict__ pos4, const double4 &me, const double *mtab,
+                                          double box, double half)
 {
-    // col: this lane's two uint4 of block 0; block kb is 64 uint4 further (32 lanes x 2)
-    const double4 pad = make_double4(me.x + 1.0, me.y, me.z, 0.0); // padding entry: unit separation, weight 0
     const uint4 padv = make_uint4(kPadEntry, kPadEntry, kPadEntry, kPadEntry);
-    uint4 q0 = nblk > 0 ? __ldcs(col) : padv, q1 = nblk > 0 ? __ldcs(col + 1) : padv;
-    double4 p0 = fetch<MODE>(pos4, q0.x, pad, box);
+    uint4 q0 = padv, q1 = padv;
+    int nextp = 0;
+    if (nblk_lane > 0) {
+        const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS);
+        q0 = __ldcs(p); q1 = __ldcs(p + 1);
+        if (nblk_lane > 8) nextp = page_next[page];
+    }
+    Raw r0 = gather(pos4, q0.x), r1 = gather(pos4, q0.y);
     for (int kb = 0; kb < nblk; ++kb) {
-        const unsigned e[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
-        if (kb + 1 < nblk) { q0 = __ldcs(col + (size_t)(kb + 1) * 64); q1 = __ldcs(col + (size_t)(kb + 1) * 64 + 1); }
-        else { q0 = padv; q1 = padv; }
+        uint4 n0 = padv, n1 = padv; // entries of block kb+1
+        if (kb + 1 < nblk_lane) {
+            const bool turn = ((kb + 1) & 7) == 0;
+            if (turn) page = nextp;
+            const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS + (((kb + 1) & 7) << 3));
+            n0 = __ldcs(p); n1 = __ldcs(p + 1);
+            if (turn && kb + 9 < nblk_lane) nextp = page_next[page];
+        }
+        const unsigned e[10] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, n0.x, n0.y};
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const double4 p1 = fetch<MODE>(pos4, u < 7 ? e[u + 1] : q0.x, pad, box); // next candidate, one step ahead
-            const double dx = sep<MODE == 2>(p0.x, me.x, box, half);
-            const double dy = sep<MODE == 2>(p0.y, me.y, box, half);
-            const double dz = sep<MODE == 2>(p0.z, me.z, box, half);
-            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-            const double rinv = rsqrt(r2);
-            accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, p0.w);
-            p0 = p1;
+            const Raw r2 = gather(pos4, e[u + 2]); // two candidates ahead
+            const unsigned en = e[u];
+            double dx, dy, dz;
+            if (MODE == 1) {
+                const unsigned kx = (en >> 26) & 3u, ky = (en >> 28) & 3u, kz = en >> 30;
+                dx = r0.xy.x - mtab[(0 * 3 + kx) * (kHarmWarps * 32)];
+                dy = r0.xy.y - mtab[(1 * 3 + ky) * (kHarmWarps * 32)];
+                dz = r0.zw.x - mtab[(2 * 3 + (kz > 2u ? 1u : kz)) * (kHarmWarps * 32)];
+            } else {
+                dx = sep<MODE == 2>(r0.xy.x, me.x, box, half);
+                dy = sep<MODE == 2>(r0.xy.y, me.y, box, half);
+                dz = sep<MODE == 2>(r0.zw.x, me.z, box, half);
+            }
+            const bool pad = en == kPadEntry;
+            if (pad) { dx = 1.0; dy = 0.0; dz = 0.0; }
+            const double wj = pad ? 0.0 : r0.zw.y;
+            const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double rinv = rsqrt(r2s);
+            accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
+            r0 = r1; r1 = r2;
         }
+        q0 = n0; q1 = n1;
     }
 }
 
@@ -501,23 +555,34 @@ template <int LMAX, int MLO, int MHI, bool PERIODIC>
 __global__ void __launch_bounds__(kHarmWarps * 32) k_harm(PairArgs a, int g0, int g1)
 {
     constexpr int NACC = ncomp_range(LMAX, MLO, MHI);
+    __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
     const int item = blockIdx.x * kHarmWarps + warp;
     if (item >= ng * nb) return;
     const int bin = a.bin_order[item / ng], g = g0 + item % ng;
-    const int rows = a.item_rows[item] >> 3; // blocks of 8 rows
-    const uint4 *col = reinterpret_cast<const uint4 *>(a.list + (size_t)a.item_off[item] * 32) + lane * 2;
     const Group gr = locate_group<PERIODIC>(a, g);
     const bool active = lane < gr.cnt;
     const double4 me = a.pos4[gr.first + (active ? lane : 0)];
+    const size_t col = ((size_t)g * nb + bin) * 32 + lane;
+    const unsigned n_mine = active ? a.counts[col] : 0u;
+    const int nblk_lane = (int)((n_mine + 7u) >> 3);
+    const int nblk = __reduce_max_sync(kFull, nblk_lane);
+    const int page = nblk_lane > 0 ? a.first_page[col] : 0;
 
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
-    else if (gr.fast) harm_rows<LMAX, MLO, MHI, 1>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
-    else harm_rows<LMAX, MLO, MHI, 2>(acc, col, rows, a.pos4, me, a.geom.box, a.geom.half);
+    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, 0.0, 0.0);
+    else if (gr.fast) {
+        double *mt = mtab + threadIdx.x;
+        const double L = a.geom.box;
+        mt[0 * kHarmWarps * 32] = me.x - L; mt[1 * kHarmWarps * 32] = me.x; mt[2 * kHarmWarps * 32] = me.x + L;
+        mt[3 * kHarmWarps * 32] = me.y - L; mt[4 * kHarmWarps * 32] = me.y; mt[5 * kHarmWarps * 32] = me.y + L;
+        mt[6 * kHarmWarps * 32] = me.z - L; mt[7 * kHarmWarps * 32] = me.z; mt[8 * kHarmWarps * 32] = me.z + L;
+        __syncwarp();
+        harm_rows<LMAX, MLO, MHI, 1>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, mt, L, a.geom.half);
+    } else harm_rows<LMAX, MLO, MHI, 2>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, a.geom.box, a.geom.half);
 
     const double vinv = a.bins.vinv[bin];
     double *out = a.alm + (size_t)g * a.ncomp * nb * 32 + (size_t)bin * 32 + lane;
@@ -552,17 +617,17 @@ int pair_stage_supported(int lmax, int nbins)
     return lmax >= 0 && lmax <= ENCORE_MAX_LMAX && nbins >= 1 && nbins <= ENCORE_MAX_BINS;
 }
 
-cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches)
+size_t pair_fill_smem_bytes(int nbins, int nr_cap) { return fill_smem_bytes(nbins, nr_cap); }
+
+cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches)
 {
     if (a.ngroups <= 0) return cudaSuccess;
-    const size_t cnt_bytes = (size_t)kBinWarps * a.bins.nbins * 32 * sizeof(int);
-    if (a.geom.periodic) k_bin<true, false><<<a.ngroups, kBinWarps * 32, cnt_bytes, s>>>(a, 0, a.ngroups);
-    else k_bin<false, false><<<a.ngroups, kBinWarps * 32, cnt_bytes, s>>>(a, 0, a.ngroups);
-    k_group_rows<<<(a.ngroups + 7) / 8, 256, 0, s>>>(a);
-    *launches += 2;
+    if (a.geom.periodic) k_group_bound<true><<<(a.ngroups + 3) / 4, 128, 0, s>>>(a);
+    else k_group_bound<false><<<(a.ngroups + 3) / 4, 128, 0, s>>>(a);
+    *launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    return launch_exclusive_scan(a.grows, a.gprefix, a.ngroups, a.scan_tmp, s, launches);
+    return launch_exclusive_scan(a.gbound, a.gprefix, a.ngroups, a.scan_tmp, s, launches);
 }
 
 #define HARM_PASS(L, A, B)                                              \
@@ -572,24 +637,21 @@ cudaError_t launch_pair_count(const PairArgs &a, cudaStream_t s, int *launches)
     }
 
 // m-ranges per lmax keep the register-resident accumulators of one pass at <= 36 doubles
-cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches)
+cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches)
 {
     const int ng = g1 - g0, nb = a.bins.nbins;
     if (ng <= 0) return cudaSuccess;
-    const int nitems = ng * nb;
-    k_item_rows<<<(nitems + 7) / 8, 256, 0, s>>>(a, g0, g1);
-    *launches += 1;
-    cudaError_t e = launch_exclusive_scan(a.item_rows, a.item_off, nitems, a.scan_tmp, s, launches);
+    cudaError_t e = cudaMemsetAsync(a.pool_cursor, 0, sizeof(unsigned), s);
     if (e != cudaSuccess) return e;
-    const size_t hm_bytes = (size_t)nb * (kNWord + 8) * 32 * sizeof(unsigned); // hit masks + staging blocks
+    const size_t smem = fill_smem_bytes(nb, nr_cap);
     if (a.geom.periodic) {
-        e = cudaFuncSetAttribute(k_bin<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hm_bytes);
+        e = cudaFuncSetAttribute(k_fill<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_bin<true, true><<<ng, kBinWarps * 32, hm_bytes, s>>>(a, g0, g1);
+        k_fill<true><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
     } else {
-        e = cudaFuncSetAttribute(k_bin<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hm_bytes);
+        e = cudaFuncSetAttribute(k_fill<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_bin<false, true><<<ng, kBinWarps * 32, hm_bytes, s>>>(a, g0, g1);
+        k_fill<false><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
     }
     *launches += 1;
     e = cudaGetLastError();
