@@ -33,7 +33,7 @@ struct DevBuf {
 struct encore_plan_s {
     HostTables T;
     bool uploaded = false;
-    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_tuple_index, gweights;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_tuple_index, gweights;
     bool force_generic = false;
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
@@ -84,10 +84,12 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
     CU(P->d_term_start.ensure(sizeof(int) * T.term_start.size()));
     CU(P->d_bin_tuples.ensure(sizeof(int) * T.bin_tuples.size()));
     CU(P->d_ynorm.ensure(sizeof(double) * T.ynorm.size()));
+    CU(P->d_ycoef.ensure(sizeof(double) * T.ycoef.size()));
     CU(cudaMemcpyAsync(P->d_terms.p, dt.data(), sizeof(DevTerm) * dt.size(), cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(P->d_term_start.p, T.term_start.data(), sizeof(int) * T.term_start.size(), cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(P->d_bin_tuples.p, T.bin_tuples.data(), sizeof(int) * T.bin_tuples.size(), cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(P->d_ynorm.p, T.ynorm.data(), sizeof(double) * T.ynorm.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(P->d_ycoef.p, T.ycoef.data(), sizeof(double) * T.ycoef.size(), cudaMemcpyHostToDevice, s));
     {   // factorised-contraction tables
         const int nm = T.order - 1, nb = T.nbins;
         size_t cells = 1;
@@ -250,6 +252,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.rmax = T.rmax;
     pa.lmax = T.lmax; pa.ncomp = ncomp;
     pa.ynorm = P->d_ynorm.as<double>();
+    pa.ycoef = P->d_ycoef.as<double>();
     pa.alm = P->alm.as<double>();
     pa.counts = P->counts.as<uint32_t>();
     pa.cand_pairs = P->cand.as<unsigned long long>();
@@ -397,7 +400,7 @@ int encore_compute_host(encore_plan_t *P, const double *positions, const double 
 int encore_destroy(encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
-    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
+    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_ycoef, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
                       &P->d_lam_order, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,

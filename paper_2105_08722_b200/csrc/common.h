@@ -64,6 +64,7 @@ struct HostTables {
     std::vector<double> edges2;      // squared
     std::vector<double> vinv;        // 1/v_b
     std::vector<double> ynorm;       // [ncomp]: (-1)^m N_lm k_lm, turns sum w p_lm(z) (x+iy)^m into sum w Y_lm
+    std::vector<double> ycoef;       // [ncomp][lmax+1]: ynorm * coefficient of z^k in the monic p_lm(z)
     std::vector<PairTerm> pair_terms; // factorised contraction (N=4,5)
     std::vector<Lam4> lam4;
     std::vector<Lam5> lam5;

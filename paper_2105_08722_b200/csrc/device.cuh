@@ -57,6 +57,7 @@ struct PairArgs {
     double rmax;
     int lmax, ncomp;
     const double *ynorm;        // [ncomp] device
+    const double *ycoef;        // [ncomp][lmax+1] device: Y_lm = sum_k ycoef[c][k] z^k (x+iy)^m
     double *alm;                // [ngroups][ncomp][nbins][32]
     uint32_t *counts;           // [ngroups][nbins][32]  accepted pairs per (primary, bin): integer output of a3
     unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)

@@ -18,9 +18,10 @@
 //   k_harm  (a4, fp64, ~130 registers): one warp per (group, bin); every lane streams its own list, gathers the
 //     candidates two rows ahead, and keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
 //     atomics, no cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit
-//     vector, w (x+iy)^m by complex recurrence, monic associated-Legendre polynomials
-//     p_lm(z) = z p_{l-1,m} - gamma_lm p_{l-2,m}, one FMA per component; normalisation (-1)^m N_lm k_lm / v_b once
-//     per (primary, bin) in the epilogue.  Items are ordered heaviest bin first so the grid drains evenly.
+//     vector (fp32 rsqrt seed + one third-order fp64 step), w (x+iy)^m by complex recurrence, powers of z, one FMA
+//     per component into S_{m,k} = sum w z^k (x+iy)^m; the monic associated-Legendre polynomials p_lm(z) and the
+//     normalisation (-1)^m N_lm k_lm / v_b are applied once per (primary, bin) in the epilogue (table ycoef).
+//     Items are ordered heaviest bin first so the grid drains evenly.
 #include "device.cuh"
 
 #include <algorithm>
@@ -50,11 +51,18 @@ __device__ __forceinline__ int cell_coord(double x, double org, double inv, int 
     return v > nc - 1 ? nc - 1 : v;
 }
 
-// acc[] order: m ascending, l ascending, (re, im)
+// acc[] order: m ascending, k ascending, (re, im): S_{m,k} = sum w z^k (x+iy)^m, k = 0..LMAX-m.
+// Same number of accumulators as the a_lm themselves ((LMAX+1)^2 reals over all m) and one FMA each per pair; the
+// Legendre polynomials p_lm(z) are applied once per (primary, bin) in the epilogue through the table ycoef
+// (tables.cpp): 4 multiplies for the powers of z replace the 2 operations per (l,m) of a recurrence in every pair.
 template <int LMAX, int MLO, int MHI>
 __device__ __forceinline__ void accumulate(double (&acc)[ncomp_range(LMAX, MLO, MHI)], double x, double y, double z,
                                            double w)
 {
+    double zp[LMAX + 1];
+    zp[0] = 1.0;
+#pragma unroll
+    for (int k = 1; k <= LMAX - MLO; ++k) zp[k] = k == 1 ? z : zp[k - 1] * z;
     double c = w, s = 0.0; // w (x + i y)^m
     int k = 0;
 #pragma unroll
@@ -66,24 +74,31 @@ __device__ __forceinline__ void accumulate(double (&acc)[ncomp_range(LMAX, MLO, 
             c = cn; s = sn;
         }
         if (m >= MLO) {
-            double pm2 = 1.0, pm1 = z;
 #pragma unroll
-            for (int l = m; l <= LMAX; ++l) {
-                double p;
-                if (l == m) p = 1.0;
-                else if (l == m + 1) p = z;
-                else {
-                    // monic recurrence: gamma_lm = ((l-1)^2 - m^2) / (4 (l-1)^2 - 1)
-                    const double gam = (double)((l - 1) * (l - 1) - m * m) / (double)(4 * (l - 1) * (l - 1) - 1);
-                    p = fma(z, pm1, -(gam * pm2));
-                    pm2 = pm1; pm1 = p;
-                }
-                if (l == m) { acc[k] += c; if (m) acc[k + 1] += s; }
-                else { acc[k] = fma(p, c, acc[k]); if (m) acc[k + 1] = fma(p, s, acc[k + 1]); }
+            for (int q = 0; q <= LMAX - m; ++q) {
+                if (q == 0) { acc[k] += c; if (m) acc[k + 1] += s; }
+                else { acc[k] = fma(zp[q], c, acc[k]); if (m) acc[k + 1] = fma(zp[q], s, acc[k + 1]); }
                 k += m ? 2 : 1;
             }
         }
     }
+}
+
+// 1/sqrt(a) to full double precision from the fp32 approximation y0 (relative error <= 2^-21.4 including the
+// rounding of a to fp32) and ONE third-order step: with e = 1 - a y0^2, a^-1/2 = y0 (1 - e)^-1/2 =
+// y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...), truncation 5/16 |e|^3 < 2^-62.  5 fp64 operations instead of the
+// library routine's ~10; arguments outside fp32's comfortable range take the library path.
+__device__ __forceinline__ double rsqrt_pair(double a)
+{
+    const float af = __double2float_rn(a);
+    if (!(af > 1e-30f && af < 1e30f)) return rsqrt(a);
+    float yf;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"(af));
+    const double y0 = (double)yf;
+    const double t = a * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(y0, e * p, y0);
 }
 
 template <bool PERIODIC>
@@ -293,7 +308,6 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 
     int nr;
     const int T = build_ranges<PERIODIC, true>(a, gr, lane, rng_start, rng_off, &nr);
-    if (lane == 0) atomicAdd(a.cand_pairs, (unsigned long long)T * (unsigned long long)cnt);
 
     // fp32 screening constants: the bin coordinate u = (r - r_min)/width computed in fp32 is within
     // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one (E^2 = sum of squared group
@@ -312,7 +326,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 
     // ---- list state -----------------------------------------------------------------------------------------
     // blocks of 4 completed but not yet written: (block index << 5) | bin.  The tests run two candidates between
-    // flushes, a lane appends at most once per candidate, so two slots suffice.
+    // flushes, a lane appends at most once per candidate (possibly to two different bins), so two slots suffice.
     int pendA = -1, pendB = -1;
     int slab_next = 0, slab_end = 0; // pages of the pool owned by this warp (uniform)
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -367,7 +381,11 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
         }
     };
 
-    // ---- staging of a word of 32 candidates (fp32, relative to primary 0; .w = list entry) ----------------------
+    // ---- candidate queue ------------------------------------------------------------------------------------------
+    // Candidates are read a word (32) at a time, lane = candidate: fp64 -> relative to primary 0 (periodic image) ->
+    // fp32, then culled against the group's bounding box (distance to the box > r_max: no primary of the group can
+    // accept it) and the survivors are compacted into a 64-entry ring in shared memory (.w = list entry).  The pair
+    // tests below always run on 32 queued candidates, so their cost follows the culled candidate count.
     auto load_cand = [&](int s, double4 &cj, unsigned &j) {
         j = kPadEntry;
         if (s < T) {
@@ -377,8 +395,30 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
             cj = a.pos4[j];
         }
     };
-    auto stage = [&](int buf, const double4 &cj, unsigned j) {
-        float4 cf = make_float4(1e18f, 1e18f, 1e18f, __uint_as_float(kPadEntry)); // beyond the list: never a hit
+    // bounding box of the group's primaries (same fp32 values the tests use) and the cull radius: r_max plus the
+    // fp32 rounding of the coordinates involved (<= 2^-23 (extent + r_max) per axis), with a safety factor
+    float blo[3], bhi[3];
+    {
+        const bool act = lane < cnt;
+        const float v[3] = {act ? pxf : 0.f, act ? pyf : 0.f, act ? pzf : 0.f}; // primary 0 sits at the origin
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+            float lo = v[ax], hi = v[ax];
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                lo = fminf(lo, __shfl_xor_sync(kFull, lo, d));
+                hi = fmaxf(hi, __shfl_xor_sync(kFull, hi, d));
+            }
+            blo[ax] = lo; bhi[ax] = hi;
+        }
+    }
+    const double rcut = (a.rmax + 9.5367431640625e-07 * (gr.ext[0] + gr.ext[1] + gr.ext[2] + a.rmax)) * (1.0 + 1e-6);
+    const float cut2 = (float)(rcut * rcut * (1.0 + 1e-6));
+    int qh = 0, qn = 0; // ring head and fill level (uniform)
+    unsigned long long kept = 0ull;
+    auto stage = [&](const double4 &cj, unsigned j) {
+        float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
+        bool keep = false;
         if (j != kPadEntry) {
             double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
             unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer subtracts {-L, 0, +L}[code] from x_i
@@ -388,20 +428,34 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                 if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
             }
             cf = make_float4((float)rx, (float)ry, (float)rz, __uint_as_float(j | (kx << 26) | (ky << 28) | (kz << 30)));
+            const float ex = fmaxf(fmaxf(blo[0] - cf.x, cf.x - bhi[0]), 0.f);
+            const float ey = fmaxf(fmaxf(blo[1] - cf.y, cf.y - bhi[1]), 0.f);
+            const float ez = fmaxf(fmaxf(blo[2] - cf.z, cf.z - bhi[2]), 0.f);
+            keep = !fast || fmaf(ez, ez, fmaf(ey, ey, ex * ex)) <= cut2; // wide groups (exact path) keep everything
         }
-        cand[buf * 32 + lane] = cf;
+        const unsigned km = __ballot_sync(kFull, keep);
+        if (keep) cand[(qh + qn + __popc(km & lt_mask)) & 63] = cf;
+        qn += __popc(km);
+        kept += (unsigned long long)__popc(km);
     };
 
     const int nwords = (T + 31) >> 5;
-    double4 cj = make_double4(0, 0, 0, 0);
-    unsigned cjx = kPadEntry;
-    load_cand(lane, cj, cjx);
-    stage(0, cj, cjx);
-    __syncwarp();
-    for (int wd = 0; wd < nwords; ++wd) {
-        const int buf = wd & 1;
-        load_cand((wd + 1) * 32 + lane, cj, cjx); // next word: in flight during the tests of this one
-        const float4 *cw = cand + buf * 32;
+    int wnext = 0; // next word to stage; cjA holds it, cjB the one after
+    double4 cjA = make_double4(0, 0, 0, 0), cjB = cjA;
+    unsigned jA = kPadEntry, jB = kPadEntry;
+    load_cand(lane, cjA, jA);
+    load_cand(32 + lane, cjB, jB);
+    for (;;) {
+        while (qn < 32 && wnext < nwords) {
+            stage(cjA, jA);
+            cjA = cjB; jA = jB;
+            ++wnext;
+            load_cand((wnext + 1) * 32 + lane, cjB, jB); // two words ahead: in flight during the tests below
+        }
+        if (qn == 0) break;
+        const int nvalid = min(qn, 32);
+        if (lane >= nvalid) cand[(qh + lane) & 63] = make_float4(1e18f, 1e18f, 1e18f, __uint_as_float(kPadEntry)); // never a hit
+        __syncwarp();
         if (fast) {
 #pragma unroll 1
             for (int c4 = 0; c4 < 32; c4 += 4) {
@@ -410,7 +464,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                 bool ok[4], am[4];
 #pragma unroll
                 for (int cc = 0; cc < 4; ++cc) {
-                    const float4 q = cw[c4 + cc];
+                    const float4 q = cand[(qh + c4 + cc) & 63];
                     const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
                     const float t = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), 1e-30f); // t = 0: r = 0 -> exact path
                     float rinv;
@@ -448,9 +502,8 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
             }
         } else {
             // group too wide for a common image: every pair is decided exactly
-            const int nvalid = min(32, T - wd * 32);
             for (int c = 0; c < nvalid; ++c) {
-                const unsigned e = __float_as_uint(cw[c].w);
+                const unsigned e = __float_as_uint(cand[(qh + c) & 63].w);
                 if (lane < cnt) {
                     const unsigned code = classify_exact<PERIODIC>(a.pos4[e & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
                     if (code != kNoHit) append(code, e);
@@ -458,9 +511,11 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                 flush_all();
             }
         }
-        stage(buf ^ 1, cj, cjx);
+        qh = (qh + 32) & 63;
+        qn -= nvalid;
         __syncwarp();
     }
+    if (lane == 0) atomicAdd(a.cand_pairs, kept * (unsigned long long)cnt);
 
     // close the open block of every (bin, lane): pad it to 4 entries, flush, and complete the last group of 8
     // (k_harm reads 8 entries at a time); cursors are n_i(b)
@@ -543,7 +598,7 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
             if (pad) { dx = 1.0; dy = 0.0; dz = 0.0; }
             const double wj = pad ? 0.0 : r0.zw.y;
             const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
-            const double rinv = rsqrt(r2s);
+            const double rinv = rsqrt_pair(r2s);
             accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
             r0 = r1; r1 = r2;
         }
@@ -584,18 +639,28 @@ __global__ void __launch_bounds__(kHarmWarps * 32) k_harm(PairArgs a, int g0, in
         harm_rows<LMAX, MLO, MHI, 1>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, mt, L, a.geom.half);
     } else harm_rows<LMAX, MLO, MHI, 2>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, a.geom.box, a.geom.half);
 
+    // epilogue: a_lm = (1/v_b) sum_k ycoef[c][k] S_{m,k}, k = l-m, l-m-2, ... (p_lm has the parity of l-m)
     const double vinv = a.bins.vinv[bin];
     double *out = a.alm + (size_t)g * a.ncomp * nb * 32 + (size_t)bin * 32 + lane;
-    int k = 0;
+    int base = 0;
 #pragma unroll
     for (int m = MLO; m <= MHI; ++m) {
+        const int st = m ? 2 : 1;
 #pragma unroll
         for (int l = m; l <= LMAX; ++l) {
             const int cre = m == 0 ? l * l : l * l + 2 * m - 1;
-            out[(size_t)cre * nb * 32] = active ? acc[k] * (a.ynorm[cre] * vinv) : 0.0;
-            if (m) out[(size_t)(cre + 1) * nb * 32] = active ? acc[k + 1] * (a.ynorm[cre + 1] * vinv) : 0.0;
-            k += m ? 2 : 1;
+            const double *yc = a.ycoef + (size_t)cre * (LMAX + 1);
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int q = (l - m) & 1; q <= l - m; q += 2) {
+                const double cf = __ldg(yc + q);
+                sr = fma(cf, acc[base + q * st], sr);
+                if (m) si = fma(cf, acc[base + q * st + 1], si);
+            }
+            out[(size_t)cre * nb * 32] = active ? sr * vinv : 0.0;
+            if (m) out[(size_t)(cre + 1) * nb * 32] = active ? si * vinv : 0.0;
         }
+        base += (LMAX - m + 1) * st;
     }
 }
 

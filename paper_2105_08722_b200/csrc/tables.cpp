@@ -266,6 +266,28 @@ int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int 
             if (m > 0) t.ynorm[comp_im(l, m)] = v;
         }
     }
+    // k_harm accumulates S_{m,k} = sum w z^k (x+iy)^m (one FMA per component, no Legendre recurrence per pair) and
+    // maps to a_lm once per (primary, bin): Y_lm = sum_k ycoef[c][k] z^k (x+iy)^m with ycoef = ynorm * (coefficient of
+    // z^k in the monic p_lm), p_mm = 1, p_{m+1,m} = z, p_lm = z p_{l-1,m} - gamma_lm p_{l-2,m},
+    // gamma_lm = ((l-1)^2 - m^2) / (4 (l-1)^2 - 1).
+    t.ycoef.assign((size_t)t.ncomp * (lmax + 1), 0.0);
+    for (int m = 0; m <= lmax; ++m) {
+        std::vector<long double> pm2(lmax + 1, 0.0L), pm1(lmax + 1, 0.0L), p(lmax + 1, 0.0L);
+        for (int l = m; l <= lmax; ++l) {
+            std::fill(p.begin(), p.end(), 0.0L);
+            if (l == m) p[0] = 1.0L;
+            else if (l == m + 1) p[1] = 1.0L;
+            else {
+                const long double gam = (long double)((l - 1) * (l - 1) - m * m) / (long double)(4 * (l - 1) * (l - 1) - 1);
+                for (int k = 0; k <= l - m; ++k) p[k] = (k > 0 ? pm1[k - 1] : 0.0L) - gam * pm2[k];
+            }
+            for (int k = 0; k <= lmax; ++k) {
+                t.ycoef[(size_t)comp_re(l, m) * (lmax + 1) + k] = (double)((long double)t.ynorm[comp_re(l, m)] * p[k]);
+                if (m > 0) t.ycoef[(size_t)comp_im(l, m) * (lmax + 1) + k] = t.ycoef[(size_t)comp_re(l, m) * (lmax + 1) + k];
+            }
+            pm2 = pm1; pm1 = p;
+        }
+    }
     build_factorised(t);
     return 0;
 }
