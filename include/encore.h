@@ -80,6 +80,20 @@ int encore_compute(encore_plan_t *plan, const double *positions, const double *w
 int encore_compute_host(encore_plan_t *plan, const double *positions, const double *weights, int64_t n,
                         double *zeta_out);
 
+/* Multi-GPU sharding over primaries (the paper's only parallel loop).
+ * Every rank holds the whole catalogue and calls this with the same inputs and its own `shard` in [0, nshards):
+ * the cell-sorted primaries are cut into nshards contiguous ranges of groups with equal pair-stage work bounds and
+ * the call evaluates eq. 34's sum over the primaries of range `shard` only, INCLUDING the 1/V factor, into
+ * zeta_partial_out (DEVICE, encore_zeta_len doubles).  The sum of the nshards partial vectors, taken in shard
+ * order, is the estimator; that sum is the caller's one collective (paper_2105_08722_b200.sharded does it with an
+ * all-gather and a fixed-order sum, bit-identical on every rank).  Diagnostics after this call (bin counts, primary
+ * counts, a_lm tiles) cover the shard's primaries only; counts of other primaries read 0.
+ * nshards = 1 is encore_compute.  Errors as encore_compute, plus ENCORE_EINVAL for shard outside [0, nshards). */
+int encore_compute_shard(encore_plan_t *plan, const double *positions, const double *weights, int64_t n, int shard,
+                         int nshards, double *zeta_partial_out, void *cuda_stream);
+/* groups of the last compute: out = {first group, one past the last group, number of groups} (HOST) */
+int encore_get_shard_groups(const encore_plan_t *plan, int out[3]);
+
 int encore_destroy(encore_plan_t *plan);
 
 /* ---- host queries (valid right after encore_plan, no GPU needed) ---- */

@@ -24,7 +24,8 @@ OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_compute", "encore_compute_host", "encore_destroy", "encore_zeta_len",
+    "encore_plan", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups",
+    "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
     "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
@@ -51,6 +52,8 @@ def lib():
     L.encore_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double]
     L.encore_compute.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
     L.encore_compute_host.argtypes = [vp, vp, vp, C.c_int64, vp]
+    L.encore_compute_shard.argtypes = [vp, vp, vp, C.c_int64, C.c_int, C.c_int, vp, vp]
+    L.encore_get_shard_groups.argtypes = [vp, ip]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
     L.encore_zeta_len.restype = C.c_int64
@@ -105,6 +108,17 @@ def encore_plan(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: i
 def encore_compute(plan, positions, weights, n: int, zeta_out, cuda_stream: int = 0):
     """positions/weights/zeta_out: CUDA tensors (fp64, contiguous) or raw device pointers."""
     _check(lib().encore_compute(plan, _ptr(positions), _ptr(weights), n, _ptr(zeta_out), C.c_void_p(cuda_stream)))
+
+
+def encore_compute_shard(plan, positions, weights, n: int, shard: int, nshards: int, zeta_partial_out, cuda_stream: int = 0):
+    _check(lib().encore_compute_shard(plan, _ptr(positions), _ptr(weights), n, shard, nshards, _ptr(zeta_partial_out),
+                                      C.c_void_p(cuda_stream)))
+
+
+def encore_get_shard_groups(plan):
+    out = (C.c_int * 3)()
+    _check(lib().encore_get_shard_groups(plan, out))
+    return int(out[0]), int(out[1]), int(out[2])
 
 
 def encore_compute_host(plan, positions, weights, n: int, zeta_out):
@@ -260,6 +274,20 @@ class Plan:
             out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
         st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
         encore_compute(self.h, positions, weights, n, out, st)
+        return out
+
+    def compute_shard(self, positions, weights, shard: int, nshards: int, out=None, stream=None):
+        """Partial zeta over the primaries of shard `shard` of `nshards` (encore_compute_shard); same arguments as compute."""
+        import torch
+        assert positions.is_cuda and positions.dtype == torch.float64 and positions.is_contiguous()
+        assert positions.dim() == 2 and positions.shape[0] == 3
+        n = positions.shape[1]
+        if weights is not None:
+            assert weights.is_cuda and weights.dtype == torch.float64 and weights.is_contiguous() and weights.numel() == n
+        if out is None:
+            out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
+        st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
+        encore_compute_shard(self.h, positions, weights, n, shard, nshards, out, st)
         return out
 
     def compute_host(self, positions: np.ndarray, weights=None) -> np.ndarray:

@@ -50,6 +50,7 @@ struct encore_plan_s {
     int64_t n = 0;
     GridGeom geom{};
     int ngroups_max = 0;
+    int g_begin = 0, g_end = 0, ngroups = 0;  // groups the last compute covered (a shard's range, or all) of how many
     cudaStream_t stream = nullptr;
     bool timing = false;
     cudaEvent_t ev[6] = {};
@@ -170,7 +171,10 @@ int record(encore_plan_s *P, int k, cudaStream_t s)
 
 #define TRY(call) do { int r__ = (call); if (r__ != ENCORE_OK) return r__; } while (0)
 
-int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t n, double *zeta_out, cudaStream_t s)
+// shard/nshards: the primaries are cut into nshards contiguous ranges of cell-sorted groups with equal pair-stage
+// work bounds; this call evaluates the sums over the primaries of range `shard` only (1 of 1 = everything).
+int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t n, double *zeta_out, cudaStream_t s,
+                   int shard = 0, int nshards = 1)
 {
     const HostTables &T = P->T;
     P->have = false;
@@ -274,6 +278,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         CU(cudaMallocHost((void **)&P->h_gprefix, sizeof(int) * ((size_t)ngmax + 2)));
         P->h_gprefix_cap = (size_t)ngmax + 2;
     }
+    int g_begin = 0, g_end = 0, ngroups_total = 0;
     CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
     CU(cudaMemsetAsync(P->pool_cursor.p, 0, 2 * sizeof(unsigned), s));
     CU(launch_pair_bounds(pa, s, &P->launches));
@@ -298,11 +303,21 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         pa.pool_pages = (unsigned)cap_pages;
         pa.page_next = P->page_next.as<int>();
         pa.ngroups = ngroups;
+        ngroups_total = ngroups;
         P->pair_steps = 0;
-        int g0 = 0;
-        while (g0 < ngroups) {
+        // shard k takes the groups [cut(k), cut(k+1)), cut(k) = first g with gp[g] >= total * k / nshards
+        auto cut = [&](int k) {
+            if (k <= 0) return 0;
+            if (k >= nshards) return ngroups;
+            const long long want = ((long long)total_slabs * k + nshards - 1) / nshards;
+            return (int)(std::lower_bound(gp, gp + ngroups + 1, want, [](int v, long long t) { return (long long)v < t; }) - gp);
+        };
+        g_begin = cut(shard); g_end = std::max(g_begin, std::min(ngroups, cut(shard + 1)));
+        if (nshards > 1) CU(cudaMemsetAsync(P->counts.p, 0, sizeof(uint32_t) * (size_t)ngroups * nb * 32, s));
+        int g0 = g_begin;
+        while (g0 < g_end) {
             int g1 = g0 + 1;
-            while (g1 < ngroups && (size_t)(gp[g1 + 1] - gp[g0]) <= cap_slabs) ++g1;
+            while (g1 < g_end && (size_t)(gp[g1 + 1] - gp[g0]) <= cap_slabs) ++g1;
             CU(launch_pair_fill_harmonics(pa, g0, g1, nr_cap, s, &P->launches));
             ++P->pair_steps;
             g0 = g1;
@@ -323,6 +338,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.vinv_total = T.box > 0.0 ? 1.0 / (T.box * T.box * T.box) : 1.0; // DESIGN.md R12
     ca.zeta_out = zeta_out;
     ca.ngroups_max = ngmax;
+    ca.g_begin = g_begin; ca.g_end = g_end;
     ca.pair_terms = P->d_pair_terms.as<PairTerm>();
     ca.lam4 = P->d_lam4.as<Lam4>();
     ca.lam5 = P->d_lam5.as<Lam5>();
@@ -341,6 +357,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     TRY(record(P, 5, s));
 
     P->have = true; P->n = n; P->geom = G; P->ngroups_max = ngmax; P->stream = s;
+    P->g_begin = g_begin; P->g_end = g_end; P->ngroups = ngroups_total;
     return ENCORE_OK;
 }
 
@@ -379,6 +396,22 @@ int encore_compute(encore_plan_t *P, const double *positions, const double *weig
 {
     if (!P || !positions || !zeta_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
     return compute_device(P, positions, weights, n, zeta_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int encore_compute_shard(encore_plan_t *P, const double *positions, const double *weights, int64_t n, int shard, int nshards,
+                         double *zeta_partial_out, void *cuda_stream)
+{
+    if (!P || !positions || !zeta_partial_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
+    if (nshards < 1 || shard < 0 || shard >= nshards) return ENCORE_EINVAL;
+    return compute_device(P, positions, weights, n, zeta_partial_out, static_cast<cudaStream_t>(cuda_stream), shard, nshards);
+}
+
+int encore_get_shard_groups(const encore_plan_t *P, int out[3])
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    out[0] = P->g_begin; out[1] = P->g_end; out[2] = P->ngroups;
+    return ENCORE_OK;
 }
 
 int encore_compute_host(encore_plan_t *P, const double *positions, const double *weights, int64_t n, double *zeta_out)

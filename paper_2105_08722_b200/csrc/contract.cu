@@ -18,9 +18,9 @@ constexpr unsigned kFull = 0xffffffffu;
 // Generic kernel, any N in {3,4,5}: one warp per output (Lam,B), terms looped, complex products in registers.
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
-    const int g = blockIdx.x;
+    const int g = a.g_begin + blockIdx.x;
     const GridGeom &G = a.geom;
-    if (g >= a.group_start[G.npencil]) return;
+    if (g >= a.g_end) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nb = a.nbins, nm = a.order - 1;
     const int p = find_pencil_of_group(a.group_start, G.npencil, g);
@@ -63,10 +63,11 @@ __global__ void k_reduce_groups(ContractArgs a)
     const int nout = a.nLam * a.nB;
     const int o = blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= nout) return;
-    const int ngroups = a.factorised ? a.nchunk : a.group_start[a.geom.npencil]; // rows of `partial`
+    // rows of `partial`: one per chunk (factorised kernels) or one per group of this call's range
+    const int r0 = a.factorised ? 0 : a.g_begin, r1 = a.factorised ? a.nchunk : a.g_end;
     const int s = blockIdx.y;
-    const int per = (ngroups + a.nseg - 1) / a.nseg;
-    const int g0 = s * per, g1 = min(ngroups, g0 + per);
+    const int per = (r1 - r0 + a.nseg - 1) / a.nseg;
+    const int g0 = r0 + s * per, g1 = min(r1, g0 + per);
     double sum = 0.0;
     for (int g = g0; g < g1; ++g) sum += a.partial[(size_t)g * nout + o];
     a.partial2[(size_t)s * nout + o] = sum;
@@ -192,15 +193,15 @@ struct TilePipe {
     int nbuf;
 };
 
-// Calls body(tile_in_smem, g) for the groups g = blockIdx.y, blockIdx.y + gridDim.y, ...
+// Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.y, + gridDim.y, ... < g_end
 template <class Body>
 __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const TilePipe &tp, Body body)
 {
-    const int ngroups = a.group_start[a.geom.npencil];
+    const int ngroups = a.g_end;
     const size_t tile = (size_t)a.ncomp * a.nbins * 32;
     const int stride = gridDim.y;
     const bool issuer = threadIdx.x == 0;
-    int g = blockIdx.y;
+    int g = a.g_begin + blockIdx.y;
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
     if (issuer && g < ngroups) tile_load(smem_c + tp.buf[0], a.alm + (size_t)g * tile, tp.bytes, &bar[0]);
     for (int k = 0; g < ngroups; ++k, g += stride) {
@@ -459,7 +460,8 @@ cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launc
 {
     *launches += 1;
     if (!a.factorised) {
-        k_contract_generic<<<a.ngroups_max, kWarps * 32, 0, s>>>(a);
+        if (a.g_end <= a.g_begin) return cudaSuccess;
+        k_contract_generic<<<a.g_end - a.g_begin, kWarps * 32, 0, s>>>(a);
         return cudaGetLastError();
     }
     // every (multiplet, tuple) of a chunk row is written by exactly one warp; no initialisation needed

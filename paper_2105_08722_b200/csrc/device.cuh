@@ -100,6 +100,7 @@ struct ContractArgs {
     double vinv_total;          // 1/V
     double *zeta_out;
     int ngroups_max;
+    int g_begin, g_end;         // groups of this call (all of them, or one shard's contiguous range)
     // factorised kernels (N = 4, 5)
     const PairTerm *pair_terms; // device
     const Lam4 *lam4;           // device [nLam]

@@ -542,13 +542,15 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 // ==========================================================================================================
 struct Raw { double2 xy, zw; };
 
+// One 256-bit load per candidate (LDG.E.256, sm_100): the gather is one 32-byte sector per lane, and the L1 tag stage
+// handles one sector per cycle, so two 128-bit loads of the same sector cost twice the L1 time (the v4 kernel sat at
+// 80 % L1 throughput with the FP64 pipe at 60 %).
 __device__ __forceinline__ Raw gather(const double4 *__restrict__ pos4, unsigned e)
 {
     Raw r;
     // a padding entry reads particle 0 (always valid memory); its contribution is cancelled by weight 0 below
-    const double2 *q = reinterpret_cast<const double2 *>(pos4 + (e == kPadEntry ? 0u : (e & kIdxMask)));
-    r.xy = __ldg(q);
-    r.zw = __ldg(q + 1);
+    const double4 *q = pos4 + (e == kPadEntry ? 0u : (e & kIdxMask));
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.xy.x), "=d"(r.xy.y), "=d"(r.zw.x), "=d"(r.zw.y) : "l"(q));
     return r;
 }
 

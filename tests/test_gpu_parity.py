@@ -226,3 +226,47 @@ def test_full_size_periodic_configs(E, oracle, name):
 
 def test_full_size_c4_cutsky(E, oracle):
     _full_size_checks(E, oracle, "c4", nsample=6)
+
+
+# ---- sharding over primaries: the shards' partial sums add up to the estimator ------------------
+@pytest.mark.parametrize("name,nshards", [("c3", 3), ("c4", 2), ("c2", 5), ("c5", 2)])
+def test_shards_add_up_to_the_oracle(E, oracle, name, nshards):
+    cfg = {"c2": W.scaled(W.CONFIGS["c2"], box=400.0, n=3000, grid=64), "c3": W.scaled(W.CONFIGS["c3"], box=360.0, n=5000, grid=64),
+           "c4": W.scaled(W.CONFIGS["c4"], n=6000), "c5": W.scaled(W.CONFIGS["c5"], box=340.0, n=3000, grid=64)}[name]
+    pos, w = W.make(cfg)
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(np.ascontiguousarray(pos)).to(dev), torch.from_numpy(np.ascontiguousarray(w)).to(dev)
+    o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, want_prim_counts=True)
+    with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+        total = np.zeros((plan.n_lambda, plan.n_b))
+        counts = np.zeros(cfg.nbins, dtype=np.uint64)
+        prim = np.zeros((cfg.n, cfg.nbins), dtype=np.uint32)
+        edge = 0
+        for k in range(nshards):                              # rank order, as sharded.combine_partials adds them
+            z = plan.compute_shard(tp, tw, k, nshards)
+            torch.cuda.synchronize()
+            total += z.cpu().numpy()
+            g0, g1, ng = E.encore_get_shard_groups(plan.h)
+            assert g0 == edge and g0 <= g1 <= ng                # contiguous ranges that cover every group once
+            edge = g1
+            c, _ = E.encore_get_bin_counts(plan.h, cfg.nbins)
+            counts += c
+            pc = torch.empty((cfg.n, cfg.nbins), dtype=torch.int32, device=dev)
+            E.encore_get_primary_counts(plan.h, pc)
+            pk = pc.cpu().numpy().astype(np.uint32)
+            assert not (prim.astype(bool) & pk.astype(bool)).any()   # a primary belongs to one shard
+            prim += pk
+        assert edge == ng
+    assert (counts == o["bin_counts"]).all()
+    assert (prim == o["prim_counts"]).all()
+    scale = np.abs(o["zeta"]).max()
+    assert np.abs(total.ravel() - o["zeta"].ravel()).max() <= TOL * scale
+
+
+def test_shard_argument_errors(E):
+    pos = torch.rand((3, 64), dtype=torch.float64, device="cuda:0") * 50.0
+    with E.Plan(3, 1.0, 20.0, 3, 2, 0.0) as plan:
+        for shard, nshards in [(-1, 2), (2, 2), (0, 0)]:
+            with pytest.raises(E.EncoreError) as ei:
+                plan.compute_shard(pos, None, shard, nshards)
+            assert ei.value.status == E.EINVAL
