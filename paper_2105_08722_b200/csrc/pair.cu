@@ -29,7 +29,7 @@
 
 namespace {
 
-constexpr int kRing = 8;            // k_fill: ring entries per (bin, lane): a block of 4 is flushed while the other fills
+constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes) per (bin, lane); see the append/flush notes
 constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(128) k_group_bound(PairArgs a)
 // ==========================================================================================================
 // k_fill: a3.  One warp (= one CTA) per group.
 // ==========================================================================================================
-// dynamic shared memory: cand[2][32] float4 | sp[96] double | e2[nb+1] double | ring[nb][16][32] u32 |
+// dynamic shared memory: cand[64] float4 | sp[96] double | e2[nb+1] double | ring[nb][32][4] u32 |
 //                        cursor[nb][32] u32 | pagecur[nb][32] int | rng_start[nr_cap] | rng_off[nr_cap+1]
 __host__ __device__ inline size_t fill_smem_bytes(int nb, int nr_cap)
 {
@@ -326,14 +326,19 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 
     // ---- list state -----------------------------------------------------------------------------------------
     // blocks of 4 completed but not yet written: (block index << 5) | bin.  The tests run two candidates between
-    // flushes, a lane appends at most once per candidate (possibly to two different bins), so two slots suffice.
+    // flushes and a lane appends at most once per candidate, so at most two blocks (of two different bins) complete
+    // in between: two slots.  If the first append completes a block and the second goes to the same bin, the entry
+    // waits in a register (ovf_entry) and becomes entry 0 of the block once that has been written: the ring is a
+    // single block per (bin, lane) - 5 kB for 10 bins instead of 10 kB, which is what sets the warps per SM.
     int pendA = -1, pendB = -1;
+    bool ovf = false;
+    unsigned ovf_entry = 0u;
     int slab_next = 0, slab_end = 0; // pages of the pool owned by this warp (uniform)
     const unsigned lt_mask = (1u << lane) - 1u;
 
     // all lanes call; lanes with a pending block write it (4 entries, 16 bytes) to their page.
-    // ring layout [bin][half][lane][4]: the flush is one conflict-free 16-byte shared-memory load
-    auto flush_block = [&](int &pend) {
+    // ring layout [bin][lane][4]: the flush is one conflict-free 16-byte shared-memory load
+    auto flush_block = [&](int &pend, bool with_ovf) {
         const bool act = pend >= 0;
         const int b = pend & 31, kb = pend >> 5;
         const bool newpage = act && (kb & 15) == 0;
@@ -359,25 +364,32 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
             slab_next += nn;
         }
         if (act) {
-            const uint4 v = *reinterpret_cast<const uint4 *>(ring + ((((b << 1) | (kb & 1)) << 5) + lane) * 4);
+            unsigned *blk = ring + ((b << 5) + lane) * 4;
+            const uint4 v = *reinterpret_cast<const uint4 *>(blk);
             __stcs(reinterpret_cast<uint4 *>(a.pool + (size_t)pagecur[b * 32 + lane] * ENCORE_PAGE_WORDS + ((kb & 15) << 2)), v);
+            if (with_ovf && ovf) blk[0] = ovf_entry;
         }
         pend = -1;
     };
     auto flush_all = [&]() {
         if (__any_sync(kFull, pendA >= 0)) {
-            flush_block(pendA);
-            if (__any_sync(kFull, pendB >= 0)) flush_block(pendB);
+            flush_block(pendA, true);
+            ovf = false;
+            if (__any_sync(kFull, pendB >= 0)) flush_block(pendB, false);
         }
     };
-    auto append = [&](unsigned code, unsigned entry) {
+    // `second`: an append may have happened since the last flush (then pendA may hold this bin's full block)
+    auto append = [&](unsigned code, unsigned entry, bool second) {
         unsigned *cp = cursor + code * 32 + lane;
         const unsigned pos = *cp;
         *cp = pos + 1u;
-        ring[((((code << 1) | ((pos >> 2) & 1u)) << 5) + lane) * 4 + (pos & 3u)] = entry;
-        if ((pos & 3u) == 3u) {
-            const int v = (int)(((pos >> 2) << 5) | code);
-            if (pendA < 0) pendA = v; else pendB = v;
+        if (second && pendA >= 0 && (unsigned)(pendA & 31) == code) { ovf = true; ovf_entry = entry; } // pos & 3 == 0
+        else {
+            ring[((code << 5) + lane) * 4 + (pos & 3u)] = entry;
+            if ((pos & 3u) == 3u) {
+                const int v = (int)(((pos >> 2) << 5) | code);
+                if (pendA < 0) pendA = v; else pendB = v;
+            }
         }
     };
 
@@ -481,20 +493,20 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                     ent[cc] = __float_as_uint(q.w);
                 }
                 if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
-                    if (ok[0]) append(code[0], ent[0]);
-                    if (ok[1]) append(code[1], ent[1]);
+                    if (ok[0]) append(code[0], ent[0], false);
+                    if (ok[1]) append(code[1], ent[1], true);
                     flush_all();
-                    if (ok[2]) append(code[2], ent[2]);
-                    if (ok[3]) append(code[3], ent[3]);
+                    if (ok[2]) append(code[2], ent[2], false);
+                    if (ok[3]) append(code[3], ent[3], true);
                     flush_all();
                 } else {
                     // some pair is within the error margin of a bin edge (~1e-4 of the pairs): exact decision
 #pragma unroll
                     for (int cc = 0; cc < 4; ++cc) {
-                        if (ok[cc]) append(code[cc], ent[cc]);
+                        if (ok[cc]) append(code[cc], ent[cc], cc & 1);
                         else if (am[cc] && ent[cc] != kPadEntry) {
                             const unsigned cx = classify_exact<PERIODIC>(a.pos4[ent[cc] & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
-                            if (cx != kNoHit) append(cx, ent[cc]);
+                            if (cx != kNoHit) append(cx, ent[cc], cc & 1);
                         }
                         if (cc & 1) flush_all();
                     }
@@ -506,7 +518,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                 const unsigned e = __float_as_uint(cand[(qh + c) & 63].w);
                 if (lane < cnt) {
                     const unsigned code = classify_exact<PERIODIC>(a.pos4[e & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
-                    if (code != kNoHit) append(code, e);
+                    if (code != kNoHit) append(code, e, false);
                 }
                 flush_all();
             }
@@ -522,15 +534,16 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     for (int b = 0; b < nb; ++b) {
         const unsigned k = cursor[b * 32 + lane];
         a.counts[((size_t)g * nb + b) * 32 + lane] = k;
+        unsigned *blk = ring + ((b << 5) + lane) * 4;
         unsigned nblk4 = k >> 2;
         if (k & 3u) {
-            for (unsigned q = k & 3u; q < 4u; ++q) ring[((((b << 1) | (nblk4 & 1u)) << 5) + lane) * 4 + q] = kPadEntry;
+            for (unsigned q = k & 3u; q < 4u; ++q) blk[q] = kPadEntry;
             pendA = (int)((nblk4 << 5) | (unsigned)b);
             ++nblk4;
         }
         flush_all();
         if (nblk4 & 1u) {
-            for (unsigned q = 0; q < 4u; ++q) ring[((((b << 1) | 1u) << 5) + lane) * 4 + q] = kPadEntry;
+            for (unsigned q = 0; q < 4u; ++q) blk[q] = kPadEntry;
             pendA = (int)((nblk4 << 5) | (unsigned)b);
         }
         flush_all();
