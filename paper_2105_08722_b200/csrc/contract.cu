@@ -10,6 +10,8 @@
 // shuffle tree per warp, a fixed-order sum over groups per segment and a fixed-order sum over segments: no atomics.
 #include "device.cuh"
 
+#include <type_traits>
+
 namespace {
 
 constexpr int kWarps = 8;
@@ -102,60 +104,128 @@ __device__ __forceinline__ double warp_sum(double v)
 }
 
 // ---- N = 4 ------------------------------------------------------------------------------------------------
-// bins b1 < b2 < b3 with b2 = b1+1+k, b3 = b1+1+kp (k < kp < NB2, NB2 = nbins-1-b1); acc[OFF + c2(kp) + k]
-template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void task4(double (&acc)[NTOT], int b1, const Lam4 &L, int toff, int s1, int s2, int s3,
-                                      int nb, double wi)
+// The first bins b1 = 0 .. NB-3 of a multiplet are dealt to its NW warps in snake order (0,1,..,NW-1,NW-1,..,1,0,0,1,..):
+// equal numbers of (b1,b2) pairs per warp.  A warp sweeps ALL its b1 together, so that an operand a~2(b2) or a3(b3)
+// read from shared memory is used for every b1 below it: the kernel is bound by shared-memory wavefronts, and this
+// cuts the operand loads per term from 2 + 2 (NB-2-b1) per b1 to 2 |set| + 2 (NB-2-min b1).
+// acc layout: for the j-th b1 of the set, offset aoff(j), then [c2(b3-b1-1) + (b2-b1-1)] for b1 < b2 < b3.
+struct Set4 {
+    int n;          // number of b1 in the set
+    int b1[8];      // ascending
+    int goff[9];    // prefix sums of (NB-2-b1): G_{m3}(b1, b2) slots
+    int aoff[9];    // prefix sums of c2(NB-1-b1): partial sums
+};
+__host__ __device__ constexpr Set4 make_set4(int nb, int nw, int w)
 {
+    Set4 s{};
+    s.n = 0;
+    s.goff[0] = 0; s.aoff[0] = 0;
+    for (int p = 0; p < nb - 2; ++p) {
+        const int r = p / nw, i = p % nw;
+        const int owner = (r & 1) ? nw - 1 - i : i;
+        if (owner == w) {
+            s.b1[s.n] = p;
+            s.goff[s.n + 1] = s.goff[s.n] + (nb - 2 - p);
+            s.aoff[s.n + 1] = s.aoff[s.n] + c2(nb - 1 - p);
+            ++s.n;
+        }
+    }
+    return s;
+}
+
+// compile-time loop: f(std::integral_constant<int, I>) for I = A .. B-1 (indices into Set4 must be constant expressions)
+template <int A, int B, class F>
+__device__ __forceinline__ void static_for(F &&f)
+{
+    if constexpr (A < B) {
+        f(std::integral_constant<int, A>{});
+        static_for<A + 1, B>(f);
+    }
+}
+
+template <int NB, int NW, int W>
+__device__ __forceinline__ void task4(double (&acc)[make_set4(NB, NW, W).aoff[make_set4(NB, NW, W).n]], const Lam4 &L,
+                                      int toff, int s1, int s2, int s3, double wi)
+{
+    constexpr Set4 S = make_set4(NB, NW, W);
+    constexpr int NS = S.n, NG = S.goff[S.n], BMIN = S.b1[0];
     // s1, s2, s3: offsets (in doubles, lane included) of the l1, l2, l3 blocks inside smem_c; toff: of the term list
-    const int rs = nb * 32;
-    const double *p1 = smem_c + s1 + b1 * 32, *p2 = smem_c + s2 + (b1 + 1) * 32, *p3 = smem_c + s3 + (b1 + 1) * 32;
+    constexpr int rs = NB * 32;
+    const double *p1 = smem_c + s1, *p2 = smem_c + s2, *p3 = smem_c + s3;
     const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.tbeg[0];
     for (int m3 = 0; m3 <= L.l3; ++m3) {
-        double gr[NB2 - 1], gi[NB2 - 1]; // G_{m3}(b1, b2)
+        double gr[NG], gi[NG]; // G_{m3}(b1, b2)
 #pragma unroll
-        for (int k = 0; k < NB2 - 1; ++k) { gr[k] = 0.0; gi[k] = 0.0; }
+        for (int k = 0; k < NG; ++k) { gr[k] = 0.0; gi[k] = 0.0; }
         const int t1 = L.tbeg[m3 + 1];
         for (int t = L.tbeg[m3]; t < t1; ++t) {
             const PairTerm T = terms[t];
-            const double r1 = p1[T.ia_re * rs], i1 = p1[T.ia_im * rs];
-            const double u = T.wrr * r1, v = T.wii * i1, sx = T.wri * r1, w = T.wir * i1;
+            double u[NS], v[NS], sx[NS], w[NS];
+            const double *ar = p1 + T.ia_re * rs, *ai = p1 + T.ia_im * rs;
+            static_for<0, NS>([&](auto J) {
+                constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                const double r1 = ar[b1 * 32], i1 = ai[b1 * 32];
+                u[j] = T.wrr * r1; v[j] = T.wii * i1; sx[j] = T.wri * r1; w[j] = T.wir * i1;
+            });
             const double *qr = p2 + T.ib_re * rs, *qi = p2 + T.ib_im * rs;
-#pragma unroll
-            for (int k = 0; k < NB2 - 1; ++k) {
-                const double r2 = qr[k * 32], i2 = qi[k * 32];
-                gr[k] = fma(u, r2, fma(v, i2, gr[k]));
-                gi[k] = fma(sx, i2, fma(w, r2, gi[k]));
-            }
+            static_for<BMIN + 1, NB - 1>([&](auto B2) {
+                constexpr int b2 = decltype(B2)::value;
+                const double r2 = qr[b2 * 32], i2 = qi[b2 * 32];
+                static_for<0, NS>([&](auto J) {
+                    constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                    if constexpr (b2 > b1) {
+                        constexpr int k = make_set4(NB, NW, W).goff[j] + b2 - b1 - 1;
+                        gr[k] = fma(u[j], r2, fma(v[j], i2, gr[k]));
+                        gi[k] = fma(sx[j], i2, fma(w[j], r2, gi[k]));
+                    }
+                });
+            });
         }
         const int cr = m3 == 0 ? 0 : 2 * m3 - 1;
         const double *q3r = p3 + cr * rs, *q3i = p3 + (m3 == 0 ? cr : cr + 1) * rs;
         const double wim = m3 == 0 ? 0.0 : -wi;
-#pragma unroll
-        for (int kp = 1; kp < NB2; ++kp) {
-            const double r3 = wi * q3r[kp * 32], i3 = wim * q3i[kp * 32]; // Re[G a3] = Gr r3 - Gi i3
-#pragma unroll
-            for (int k = 0; k < kp; ++k) acc[OFF + c2(kp) + k] = fma(gr[k], r3, fma(gi[k], i3, acc[OFF + c2(kp) + k]));
-        }
+        static_for<BMIN + 2, NB>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value;
+            const double r3 = wi * q3r[b3 * 32], i3 = wim * q3i[b3 * 32]; // Re[G a3] = Gr r3 - Gi i3
+            static_for<0, NS>([&](auto J) {
+                constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                static_for<b1 + 1, b3>([&](auto B2) {
+                    constexpr int b2 = decltype(B2)::value;
+                    constexpr int k = make_set4(NB, NW, W).goff[j] + b2 - b1 - 1;
+                    constexpr int o = make_set4(NB, NW, W).aoff[j] + c2(b3 - b1 - 1) + (b2 - b1 - 1);
+                    acc[o] = fma(gr[k], r3, fma(gi[k], i3, acc[o]));
+                });
+            });
+        });
     }
 }
 
-template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void flush4(const double (&acc)[NTOT], int b1, int nb, const int *tuple_index, double *out, int lane)
+template <int NB, int NW, int W>
+__device__ __forceinline__ void flush4(const double (&acc)[make_set4(NB, NW, W).aoff[make_set4(NB, NW, W).n]],
+                                       const int *tuple_index, double *out, int lane)
 {
-#pragma unroll
-    for (int kp = 1; kp < NB2; ++kp)
-#pragma unroll
-        for (int k = 0; k < kp; ++k) {
-            const double v = warp_sum(acc[OFF + c2(kp) + k]);
-            if (lane == 0) out[tuple_index[(b1 * nb + (b1 + 1 + k)) * nb + (b1 + 1 + kp)]] = v;
-        }
+    constexpr int NS = make_set4(NB, NW, W).n;
+    static_for<0, NS>([&](auto J) {
+        constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+        static_for<b1 + 2, NB>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value;
+            static_for<b1 + 1, b3>([&](auto B2) {
+                constexpr int b2 = decltype(B2)::value;
+                const double v = warp_sum(acc[make_set4(NB, NW, W).aoff[j] + c2(b3 - b1 - 1) + (b2 - b1 - 1)]);
+                if (lane == 0) out[tuple_index[(b1 * NB + b2) * NB + b3]] = v;
+            });
+        });
+    });
 }
 
 // ---- tile pipeline: the a_lm tile of a group ([component][bin][lane], contiguous in HBM) is brought into shared
 // memory by one TMA bulk copy (cp.async.bulk + mbarrier complete_tx), double-buffered so that group k+1 streams in
 // while group k is contracted.  All warps of the CTA run the same loop (same number of barriers).
 constexpr int kCtaWarps = 12;
+#ifndef ENCORE_NW4_WIDE
+#define ENCORE_NW4_WIDE 2     // N = 4, 9-10 bins: warps per multiplet (measured on c3: 4x3 19.4 ms, 3x3 15.0, 4x2 22.8, 2x4 10.9)
+#define ENCORE_LPC4_WIDE 4    //                   multiplets per CTA
+#endif
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -242,52 +312,54 @@ __device__ __forceinline__ void stage_terms(int off, const PairTerm *src, int n,
     for (int k = lane; k < 6 * n; k += 32) smem_c[off + k] = s[k];
 }
 
-// warp W of a multiplet owns b1 = W (NB-1-W upper bins) and b1 = NB-3-W (W+2 upper bins): equal work per warp
-template <int NB, int W>
+// warps per multiplet and multiplets per CTA for the N = 4 kernel
+__host__ __device__ constexpr int nw4(int nb) { return nb >= 9 ? ENCORE_NW4_WIDE : (nb - 2 + 1) / 2; }
+__host__ __device__ constexpr int lpc4(int nb) { return nb >= 9 ? ENCORE_LPC4_WIDE : kCtaWarps / nw4(nb); }
+
+template <int NB, int NW, int W>
 __device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
-    constexpr int NBA = NB - 1 - W, WB = NB - 3 - W, NBB = WB > W ? NB - 1 - WB : 0;
-    constexpr int NTOT = c2(NBA) + (NBB ? c2(NBB) : 0);
-    const int lane = threadIdx.x & 31, nb = a.nbins;
-    const int o1 = L.l1 * L.l1 * nb * 32 + lane, o2 = L.l2 * L.l2 * nb * 32 + lane, o3 = L.l3 * L.l3 * nb * 32 + lane;
+    constexpr Set4 S = make_set4(NB, NW, W);
+    constexpr int NTOT = S.aoff[S.n];
+    const int lane = threadIdx.x & 31;
+    const int o1 = L.l1 * L.l1 * NB * 32 + lane, o2 = L.l2 * L.l2 * NB * 32 + lane, o3 = L.l3 * L.l3 * NB * 32 + lane;
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
     for_each_group_tile(a, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        task4<NBA, 0, NTOT>(acc, W, L, toff, t + o1, t + o2, t + o3, nb, wi);
-        if constexpr (NBB > 0) task4<NBB, c2(NBA), NTOT>(acc, WB, L, toff, t + o1, t + o2, t + o3, nb, wi);
+        task4<NB, NW, W>(acc, L, toff, t + o1, t + o2, t + o3, wi);
     });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
-    flush4<NBA, 0, NTOT>(acc, W, nb, a.tuple_index, out, lane);
-    if constexpr (NBB > 0) flush4<NBB, c2(NBA), NTOT>(acc, WB, nb, a.tuple_index, out, lane);
+    flush4<NB, NW, W>(acc, a.tuple_index, out, lane);
 }
 
-template <int NB, int W>
+template <int NB, int NW, int W>
 __device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
-    constexpr int NW = (NB - 2 + 1) / 2;
-    if (w == W) warp4<NB, W>(a, tp, have, L, iL, toff);
-    else if constexpr (W + 1 < NW) dispatch4<NB, W + 1>(w, a, tp, have, L, iL, toff);
+    if (w == W) warp4<NB, NW, W>(a, tp, have, L, iL, toff);
+    else if constexpr (W + 1 < NW) dispatch4<NB, NW, W + 1>(w, a, tp, have, L, iL, toff);
 }
 
-// 12 warps per CTA = 12/NW multiplets, each on NW = ceil((NB-2)/2) warps
+// LPC multiplets per CTA, each on NW warps
+// registers: the file is split over the 4 SM sub-partitions (16384 each), so 9-12 warps cap a thread at 168 registers
+// and up to 8 warps allow 255
 template <int NB>
-__global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract4(ContractArgs a, int nbuf)
+__global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(ContractArgs a, int nbuf)
 {
-    constexpr int NW = (NB - 2 + 1) / 2, LPC = kCtaWarps / NW;
+    constexpr int NW = nw4(NB), LPC = lpc4(NB);
     const int warp = threadIdx.x >> 5;
     const int slot = blockIdx.x * LPC + warp / NW;
-    const bool have = warp < LPC * NW && slot < a.nLam;
+    const bool have = slot < a.nLam;
     const int iL = a.lam_order[have ? slot : 0];
     const Lam4 L = a.lam4[iL];
     const TilePipe tp = make_pipe(a, nbuf);
     const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // this multiplet's term list in shared memory
     if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.tbeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
-    dispatch4<NB, 0>(have ? warp % NW : 0, a, tp, have, L, iL, toff);
+    dispatch4<NB, NW, 0>(warp % NW, a, tp, have, L, iL, toff);
 }
 
 // ---- N = 5 ------------------------------------------------------------------------------------------------
@@ -425,11 +497,11 @@ template <int NB>
 cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 {
     size_t smem;
-    constexpr int LPC = kCtaWarps / ((NB - 2 + 1) / 2);
+    constexpr int LPC = lpc4(NB);
     const int nbuf = pipe_config(a, LPC, &smem);
     cudaError_t e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_contract4<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);
+    k_contract4<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), nw4(NB) * LPC * 32, smem, s>>>(a, nbuf);
     return cudaGetLastError();
 }
 
