@@ -363,106 +363,233 @@ __global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(Contra
 }
 
 // ---- N = 5 ------------------------------------------------------------------------------------------------
-// bins b1 < b2 < b3 < b4 with b_j = b1+1+k_j (k2 < k3 < k4 < NB2); acc[OFF + c3(k4) + c2(k3) + k2]
-template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void task5(double (&acc)[NTOT], int b1, const Lam5 &L, int toff, int sA, int nb, double wi)
+// H = sum_{M>=0} Re[ Y12_M(b1,b2) R34_M(b3,b4) ] over b1 < b2 < b3 < b4.  Two warps per multiplet split the tuples by
+// the second bin: warp A takes b2 <= T, warp B takes b2 > T (T = t5(NB) balances the coupled-pair sums per warp).
+//   warp A holds its few Y(b1,b2) (b2 <= T) and streams R(b3,.) one b3 at a time;
+//   warp B holds its few R(b3,b4) (b3 >= T+2) and streams Y(.,b2) one b2 at a time.
+// Every Y pair is computed once and an R pair at most twice (36 coupled-pair sums per M at 8 bins instead of the 50 of
+// a split by b1), and both warps keep 35 partial sums at 8 bins.
+__host__ __device__ constexpr int npairs_above(int nb, int b) { return c2(nb - 1 - b); } // pairs b < b3 < b4 <= nb-1
+__host__ __device__ constexpr int work5(int nb, int t, int second)
 {
-    const int rs = nb * 32;
-    const double *p1 = smem_c + sA + L.l1 * L.l1 * rs + b1 * 32;
-    const double *p2 = smem_c + sA + L.l2 * L.l2 * rs + (b1 + 1) * 32;
-    const double *p3 = smem_c + sA + L.l3 * L.l3 * rs + (b1 + 1) * 32;
-    const double *p4 = smem_c + sA + L.l4 * L.l4 * rs + (b1 + 1) * 32;
+    int y = 0;
+    if (!second) { for (int b2 = 1; b2 <= t; ++b2) y += b2; return y + npairs_above(nb, 1); }
+    for (int b2 = t + 1; b2 <= nb - 3; ++b2) y += b2;
+    return y + (t + 1 <= nb - 3 ? npairs_above(nb, t + 1) : 0);
+}
+__host__ __device__ constexpr int t5(int nb)
+{
+    int best = 1, cost = 1 << 30;
+    for (int t = 1; t <= nb - 3; ++t) {
+        const int a = work5(nb, t, 0), b = work5(nb, t, 1), m = a > b ? a : b;
+        if (m < cost) { cost = m; best = t; }
+    }
+    return best;
+}
+// partial sums of a warp whose second bins are lo..hi: [abase(b2) + pidx(b2; b3, b4) * b2 + b1]
+__host__ __device__ constexpr int abase5(int nb, int lo, int b2)
+{
+    int s = 0;
+    for (int b = lo; b < b2; ++b) s += b * npairs_above(nb, b);
+    return s;
+}
+__host__ __device__ constexpr int pidx5(int nb, int b2, int b3, int b4)
+{
+    int s = 0;
+    for (int b = b2 + 1; b < b3; ++b) s += nb - 1 - b;
+    return s + (b4 - b3 - 1);
+}
+__host__ __device__ constexpr int aidx5(int nb, int lo, int b1, int b2, int b3, int b4)
+{
+    return abase5(nb, lo, b2) + pidx5(nb, b2, b3, b4) * b2 + b1;
+}
+__host__ __device__ constexpr int ntot5(int nb, int lo, int hi) { const int n = hi >= lo ? abase5(nb, lo, hi + 1) : 0; return n > 0 ? n : 1; }
+
+// Coupled-pair sums  Z(x,y) += sum_t [wrr r_x r_y + wii i_x i_y] + i [wri r_x i_y + wir i_x r_y]  (PairTerm), first
+// factor from block pa at bin x, second from block pb at bin y, for the terms [t0, t1).
+// fixed first bin X, second bins Y0..Y1: zr[y - Y0]
+template <int NB, int X, int Y0, int Y1, int NZ>
+__device__ __forceinline__ void pairs_fixed_x(double (&zr)[NZ], double (&zi)[NZ], const PairTerm *terms, int t0, int t1,
+                                              const double *pa, const double *pb)
+{
+    constexpr int rs = NB * 32;
+    for (int t = t0; t < t1; ++t) {
+        const PairTerm T = terms[t];
+        const double rx = pa[T.ia_re * rs + X * 32], ix = pa[T.ia_im * rs + X * 32];
+        const double u = T.wrr * rx, v = T.wii * ix, sx = T.wri * rx, w = T.wir * ix;
+        const double *qr = pb + T.ib_re * rs, *qi = pb + T.ib_im * rs;
+        static_for<Y0, Y1 + 1>([&](auto Yc) {
+            constexpr int y = decltype(Yc)::value;
+            const double ry = qr[y * 32], iy = qi[y * 32];
+            zr[y - Y0] = fma(u, ry, fma(v, iy, zr[y - Y0]));
+            zi[y - Y0] = fma(sx, iy, fma(w, ry, zi[y - Y0]));
+        });
+    }
+}
+// fixed second bin Y, first bins X0..X1: zr[x - X0]
+template <int NB, int Y, int X0, int X1, int NZ>
+__device__ __forceinline__ void pairs_fixed_y(double (&zr)[NZ], double (&zi)[NZ], const PairTerm *terms, int t0, int t1,
+                                              const double *pa, const double *pb)
+{
+    constexpr int rs = NB * 32;
+    for (int t = t0; t < t1; ++t) {
+        const PairTerm T = terms[t];
+        const double ry = pb[T.ib_re * rs + Y * 32], iy = pb[T.ib_im * rs + Y * 32];
+        const double u = T.wrr * ry, v = T.wii * iy, sx = T.wri * iy, w = T.wir * ry;
+        const double *qr = pa + T.ia_re * rs, *qi = pa + T.ia_im * rs;
+        static_for<X0, X1 + 1>([&](auto Xc) {
+            constexpr int x = decltype(Xc)::value;
+            const double rx = qr[x * 32], ix = qi[x * 32];
+            zr[x - X0] = fma(u, rx, fma(v, ix, zr[x - X0]));
+            zi[x - X0] = fma(sx, rx, fma(w, ix, zi[x - X0]));
+        });
+    }
+}
+// block of pairs x in X0..X1, y in Y0..Y1, x < y, all swept together (each operand is read once per term);
+// KIND 0: slot = c2(y) - c2(Y0) + x (pairs (b1,b2) by b2);  KIND 1: slot = sum_{b=X0}^{x-1} (NB-1-b) + y-x-1 (pairs (b3,b4) by b3)
+template <int NB, int KIND, int X0, int Y0>
+__host__ __device__ constexpr int slot5(int x, int y)
+{
+    if (KIND == 0) return c2(y) - c2(Y0) + x;
+    int s = 0;
+    for (int b = X0; b < x; ++b) s += NB - 1 - b;
+    return s + (y - x - 1);
+}
+template <int NB, int KIND, int X0, int X1, int Y0, int Y1, int NZ>
+__device__ __forceinline__ void pairs_block(double (&zr)[NZ], double (&zi)[NZ], const PairTerm *terms, int t0, int t1,
+                                            const double *pa, const double *pb)
+{
+    constexpr int rs = NB * 32, NY = Y1 - Y0 + 1;
+    for (int t = t0; t < t1; ++t) {
+        const PairTerm T = terms[t];
+        double u[NY], v[NY], sx[NY], w[NY];
+        const double *br = pb + T.ib_re * rs, *bi = pb + T.ib_im * rs;
+        static_for<Y0, Y1 + 1>([&](auto Yc) {
+            constexpr int y = decltype(Yc)::value;
+            const double ry = br[y * 32], iy = bi[y * 32];
+            u[y - Y0] = T.wrr * ry; v[y - Y0] = T.wii * iy; sx[y - Y0] = T.wri * iy; w[y - Y0] = T.wir * ry;
+        });
+        const double *ar = pa + T.ia_re * rs, *ai = pa + T.ia_im * rs;
+        static_for<X0, X1 + 1>([&](auto Xc) {
+            constexpr int x = decltype(Xc)::value;
+            const double rx = ar[x * 32], ix = ai[x * 32];
+            static_for<(x + 1 > Y0 ? x + 1 : Y0), Y1 + 1>([&](auto Yc) {
+                constexpr int y = decltype(Yc)::value;
+                constexpr int k = slot5<NB, KIND, X0, Y0>(x, y);
+                zr[k] = fma(u[y - Y0], rx, fma(v[y - Y0], ix, zr[k]));
+                zi[k] = fma(sx[y - Y0], rx, fma(w[y - Y0], ix, zi[k]));
+            });
+        });
+    }
+}
+
+// warp A: second bins 1..T.  Y(b1,b2) of all its pairs held in registers, R(b3,.) streamed by b3.
+template <int NB, int T, int NTOT>
+__device__ __forceinline__ void task5a(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, double wi)
+{
+    constexpr int rs = NB * 32, NYH = c2(T + 1); // pairs b1 < b2 <= T
+    const double *p1 = smem_c + sA + L.l1 * L.l1 * rs, *p2 = smem_c + sA + L.l2 * L.l2 * rs;
+    const double *p3 = smem_c + sA + L.l3 * L.l3 * rs, *p4 = smem_c + sA + L.l4 * L.l4 * rs;
     const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
     for (int M = 0; M <= L.l12; ++M) {
-        double yr[NB2 - 2], yi[NB2 - 2]; // w_i Y12_M(b1, b2)
+        double yr[NYH], yi[NYH];
 #pragma unroll
-        for (int k = 0; k < NB2 - 2; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
-        for (int t = L.lbeg[M]; t < L.lbeg[M + 1]; ++t) {
-            const PairTerm T = terms[t];
-            const double r1 = wi * p1[T.ia_re * rs], i1 = wi * p1[T.ia_im * rs];
-            const double u = T.wrr * r1, v = T.wii * i1, sx = T.wri * r1, w = T.wir * i1;
-            const double *qr = p2 + T.ib_re * rs, *qi = p2 + T.ib_im * rs;
+        for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
+        pairs_block<NB, 0, 0, T - 1, 1, T, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
 #pragma unroll
-            for (int k = 0; k < NB2 - 2; ++k) {
-                const double r2 = qr[k * 32], i2 = qi[k * 32];
-                yr[k] = fma(u, r2, fma(v, i2, yr[k]));
-                yi[k] = fma(sx, i2, fma(w, r2, yi[k]));
-            }
+        for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
+        static_for<2, NB - 1>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value, NR = NB - 1 - b3;
+            double rr[NR], ri[NR];
+#pragma unroll
+            for (int q = 0; q < NR; ++q) { rr[q] = 0.0; ri[q] = 0.0; }
+            pairs_fixed_x<NB, b3, b3 + 1, NB - 1, NR>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+            static_for<b3 + 1, NB>([&](auto B4) {
+                constexpr int b4 = decltype(B4)::value;
+                static_for<1, (T < b3 - 1 ? T : b3 - 1) + 1>([&](auto B2) {
+                    constexpr int b2 = decltype(B2)::value;
+                    static_for<0, b2>([&](auto B1) {
+                        constexpr int b1 = decltype(B1)::value;
+                        constexpr int o = aidx5(NB, 1, b1, b2, b3, b4), k = c2(b2) + b1;
+                        acc[o] = fma(yr[k], rr[b4 - b3 - 1], fma(yi[k], ri[b4 - b3 - 1], acc[o]));
+                    });
+                });
+            });
+        });
+    }
+}
+
+// warp B: second bins T+1..NB-3.  R(b3,b4) of all its pairs (b3 >= T+2) held in registers, Y(.,b2) streamed by b2.
+template <int NB, int T, int NTOT>
+__device__ __forceinline__ void task5b(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, double wi)
+{
+    if constexpr (T + 1 <= NB - 3) {
+        constexpr int rs = NB * 32, NRH = c2(NB - 2 - T); // pairs T+2 <= b3 < b4 <= NB-1
+        const double *p1 = smem_c + sA + L.l1 * L.l1 * rs, *p2 = smem_c + sA + L.l2 * L.l2 * rs;
+        const double *p3 = smem_c + sA + L.l3 * L.l3 * rs, *p4 = smem_c + sA + L.l4 * L.l4 * rs;
+        const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
+        for (int M = 0; M <= L.l12; ++M) {
+            double rr[NRH], ri[NRH];
+#pragma unroll
+            for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
+            pairs_block<NB, 1, T + 2, NB - 2, T + 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+            static_for<T + 1, NB - 2>([&](auto B2) {
+                constexpr int b2 = decltype(B2)::value;
+                double yr[b2], yi[b2];
+#pragma unroll
+                for (int k = 0; k < b2; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
+                pairs_fixed_y<NB, b2, 0, b2 - 1, b2>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
+#pragma unroll
+                for (int k = 0; k < b2; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
+                static_for<b2 + 1, NB - 1>([&](auto B3) {
+                    constexpr int b3 = decltype(B3)::value;
+                    static_for<b3 + 1, NB>([&](auto B4) {
+                        constexpr int b4 = decltype(B4)::value;
+                        constexpr int k = slot5<NB, 1, T + 2, T + 3>(b3, b4);
+                        static_for<0, b2>([&](auto B1) {
+                            constexpr int b1 = decltype(B1)::value;
+                            constexpr int o = aidx5(NB, T + 1, b1, b2, b3, b4);
+                            acc[o] = fma(yr[b1], rr[k], fma(yi[b1], ri[k], acc[o]));
+                        });
+                    });
+                });
+            });
         }
-#pragma unroll
-        for (int k3 = 1; k3 < NB2 - 1; ++k3) {
-            double rr[NB2 - 2], ri[NB2 - 2]; // R34_M(b3, b4), b4 = b1+1+k3+1+q, q < NB2-1-k3
-#pragma unroll
-            for (int q = 0; q < NB2 - 1 - k3; ++q) { rr[q] = 0.0; ri[q] = 0.0; }
-            for (int t = L.rbeg[M]; t < L.rbeg[M + 1]; ++t) {
-                const PairTerm T = terms[t];
-                const double r3 = p3[T.ia_re * rs + k3 * 32], i3 = p3[T.ia_im * rs + k3 * 32];
-                const double u = T.wrr * r3, v = T.wii * i3, sx = T.wri * r3, w = T.wir * i3;
-                const double *qr = p4 + T.ib_re * rs + (k3 + 1) * 32, *qi = p4 + T.ib_im * rs + (k3 + 1) * 32;
-#pragma unroll
-                for (int q = 0; q < NB2 - 1 - k3; ++q) {
-                    const double r4 = qr[q * 32], i4 = qi[q * 32];
-                    rr[q] = fma(u, r4, fma(v, i4, rr[q]));
-                    ri[q] = fma(sx, i4, fma(w, r4, ri[q]));
-                }
-            }
-#pragma unroll
-            for (int q = 0; q < NB2 - 1 - k3; ++q)
-#pragma unroll
-                for (int k2 = 0; k2 < k3; ++k2) { // Re[Y R] = Yr Rr - Yi Ri
-                    const int o = OFF + c3(k3 + 1 + q) + c2(k3) + k2;
-                    acc[o] = fma(yr[k2], rr[q], fma(-yi[k2], ri[q], acc[o]));
-                }
-        }
     }
 }
 
-template <int NB2, int OFF, int NTOT>
-__device__ __forceinline__ void flush5(const double (&acc)[NTOT], int b1, int nb, const int *tuple_index, double *out, int lane)
+// one shuffle tree per tuple of a warp whose second bins are LO..HI
+template <int NB, int LO, int HI, int NTOT>
+__device__ __forceinline__ void flush5(const double (&acc)[NTOT], const int *tuple_index, double *out, int lane)
 {
-#pragma unroll
-    for (int k4 = 2; k4 < NB2; ++k4)
-#pragma unroll
-        for (int k3 = 1; k3 < k4; ++k3)
-#pragma unroll
-            for (int k2 = 0; k2 < k3; ++k2) {
-                const double v = warp_sum(acc[OFF + c3(k4) + c2(k3) + k2]);
-                const int b2 = b1 + 1 + k2, b3 = b1 + 1 + k3, b4 = b1 + 1 + k4;
-                if (lane == 0) out[tuple_index[((b1 * nb + b2) * nb + b3) * nb + b4]] = v;
-            }
+    static_for<LO, HI + 1>([&](auto B2) {
+        constexpr int b2 = decltype(B2)::value;
+        static_for<b2 + 1, NB - 1>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value;
+            static_for<b3 + 1, NB>([&](auto B4) {
+                constexpr int b4 = decltype(B4)::value;
+                static_for<0, b2>([&](auto B1) {
+                    constexpr int b1 = decltype(B1)::value;
+                    const double v = warp_sum(acc[aidx5(NB, LO, b1, b2, b3, b4)]);
+                    if (lane == 0) out[tuple_index[((b1 * NB + b2) * NB + b3) * NB + b4]] = v;
+                });
+            });
+        });
+    });
 }
 
-// second warp of a multiplet: b1 = 1 .. NB-4 one after the other (NB2 = NB-2 .. 3), all partial sums in registers
-template <int NB, int B1, int OFF, int NTOT>
-__device__ __forceinline__ void rest5(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, int nb, double wi)
-{
-    if constexpr (NB - 1 - B1 >= 3) {
-        task5<NB - 1 - B1, OFF, NTOT>(acc, B1, L, toff, sA, nb, wi);
-        rest5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, L, toff, sA, nb, wi);
-    }
-}
-template <int NB, int B1, int OFF, int NTOT>
-__device__ __forceinline__ void restflush5(const double (&acc)[NTOT], int nb, const int *tuple_index, double *out, int lane)
-{
-    if constexpr (NB - 1 - B1 >= 3) {
-        flush5<NB - 1 - B1, OFF, NTOT>(acc, B1, nb, tuple_index, out, lane);
-        restflush5<NB, B1 + 1, OFF + c3(NB - 1 - B1), NTOT>(acc, nb, tuple_index, out, lane);
-    }
-}
-__host__ __device__ constexpr int rest5_total(int nb) { int s = 0; for (int b1 = 1; nb - 1 - b1 >= 3; ++b1) s += c3(nb - 1 - b1); return s > 0 ? s : 1; }
-
-// 12 warps per CTA = 6 multiplets; even warp: b1 = 0, odd warp: b1 = 1 .. NB-4
+// 12 warps per CTA = 6 multiplets; even warp: b2 <= T, odd warp: b2 > T
 template <int NB>
 __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a, int nbuf)
 {
-    constexpr int LPC = kCtaWarps / 2;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = a.nbins;
+    constexpr int LPC = kCtaWarps / 2, T = t5(NB);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int slot = blockIdx.x * LPC + (warp >> 1);
     const bool have = slot < a.nLam;
     const int iL = a.lam_order[have ? slot : 0];
     const Lam5 L = a.lam5[iL];
     const bool second = warp & 1;
-    constexpr int NA = c3(NB - 1), NR = rest5_total(NB);
+    constexpr int NA = ntot5(NB, 1, T), NR = ntot5(NB, T + 1, NB - 3);
     constexpr int NTOT = NA > NR ? NA : NR;
     const TilePipe tp = make_pipe(a, nbuf);
     const int toff = tp.bar + 8 + (warp >> 1) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
@@ -474,13 +601,13 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a,
     for_each_group_tile(a, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        if (!second) task5<NB - 1, 0, NTOT>(acc, 0, L, toff, t + lane, nb, wi);
-        else rest5<NB, 1, 0, NTOT>(acc, L, toff, t + lane, nb, wi);
+        if (!second) task5a<NB, T, NTOT>(acc, L, toff, t + lane, wi);
+        else task5b<NB, T, NTOT>(acc, L, toff, t + lane, wi);
     });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
-    if (!second) flush5<NB - 1, 0, NTOT>(acc, 0, nb, a.tuple_index, out, lane);
-    else restflush5<NB, 1, 0, NTOT>(acc, nb, a.tuple_index, out, lane);
+    if (!second) flush5<NB, 1, T, NTOT>(acc, a.tuple_index, out, lane);
+    else flush5<NB, T + 1, NB - 3, NTOT>(acc, a.tuple_index, out, lane);
 }
 
 // shared memory: nbuf tiles + 2 mbarriers; two buffers whenever they fit
