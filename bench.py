@@ -37,6 +37,9 @@ if ROOT not in sys.path:
 import workloads as W  # noqa: E402
 
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
+# dram__bytes_read.sum + dram__bytes_write.sum of k_fill + k_harm per step, from the committed `ncu --set full` capture
+# profiles/r1_v5_ncu_full_c3.txt (an ALU-bound stage: the traffic is the candidate lists written and read back once)
+NCU_PAIR_STAGE_DRAM_BYTES = {"c3": 19.59e9}
 
 
 def peaks():
@@ -281,7 +284,8 @@ def main():
             "contraction_frac_fp64_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / peak_derived,
         },
         "roofline": {"bound": "alu", "kernel": "k_pair (a3+a4)", "achieved": pair_tflops, "peak": peak_derived / 1e12,
-                     "unit": "TFLOP/s", "frac": pair_tflops * 1e12 / peak_derived, "traffic": None,
+                     "unit": "TFLOP/s", "frac": pair_tflops * 1e12 / peak_derived,
+                     "traffic": NCU_PAIR_STAGE_DRAM_BYTES.get(cfg.name),
                      "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} fp64 FMA lanes x 2 x {sm_max_mhz:g} MHz ({peak_src} clock)",
                      "peak_measured_dfma_chain": fp64_measured / 1e12,
                      "flops_model": "4.5 (lmax+1)^2 + 25 per accepted pair + 12 per rejected candidate (DESIGN.md §7)"},

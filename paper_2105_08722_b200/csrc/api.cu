@@ -491,15 +491,21 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
                     ex += (double)(q.l3 + 1) * (2.0 * (nb2 - 1) + 4.0 * nb2 * (nb2 - 1) / 2); // Re[G a3]: 2 FMA per triple
                 }
         } else {
+            // two warps per multiplet split by the second bin at t (contract.cu): A holds Y(b1,b2<=t) and streams
+            // R(b3,.), B holds R(b3>=t+2,b4) and streams Y(.,b2>t); 4 multiplies per pre-weighted operand, 4 FMA per pair
+            const int t = contraction_split5(nb);
+            auto c2 = [](int n) { return n * (n - 1) / 2; };
+            double tupA = 0, tupB = 0;
+            for (int b2 = 1; b2 <= nb - 3; ++b2) (b2 <= t ? tupA : tupB) += (double)b2 * c2(nb - 1 - b2);
             for (const Lam5 &q : T.lam5) {
-                const int nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0];
-                for (int b1 = 0; b1 + 3 < nb; ++b1) {
-                    const int nb2 = nb - 1 - b1;
-                    ex += (double)nl * (6.0 + 8.0 * (nb2 - 2));
-                    for (int k3 = 1; k3 < nb2 - 1; ++k3) {
-                        ex += (double)nr * (4.0 + 8.0 * (nb2 - 1 - k3));
-                        ex += (double)(q.l12 + 1) * 4.0 * (nb2 - 1 - k3) * k3;
-                    }
+                const double nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0], nM = q.l12 + 1;
+                ex += nl * (4.0 * t + 8.0 * c2(t + 1)) + nM * 2.0 * c2(t + 1);                 // A: Y block, times w_i
+                for (int b3 = 2; b3 <= nb - 2; ++b3) ex += nr * (4.0 + 8.0 * (nb - 1 - b3));   // A: R(b3,.)
+                ex += nM * 4.0 * tupA;                                                         // A: Re[Y R]
+                if (t + 1 <= nb - 3) {
+                    ex += nr * (4.0 * (nb - 3 - t) + 8.0 * c2(nb - 2 - t));                    // B: R block
+                    for (int b2 = t + 1; b2 <= nb - 3; ++b2) ex += nl * (4.0 + 8.0 * b2) + nM * 2.0 * b2; // B: Y(.,b2)
+                    ex += nM * 4.0 * tupB;                                                     // B: Re[Y R]
                 }
             }
         }

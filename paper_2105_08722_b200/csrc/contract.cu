@@ -648,6 +648,8 @@ cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 
 // Factorised kernels cover the bin counts whose per-warp partial sums fit in registers; anything else (and N = 3,
 // which is cheap) runs the generic kernel.
+int contraction_split5(int nbins) { return t5(nbins); }
+
 int contraction_is_factorised(int order, int nbins, int lmax)
 {
     if (order == 4) return nbins >= 3 && nbins <= 10 && lmax <= 6;

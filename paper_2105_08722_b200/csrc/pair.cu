@@ -580,7 +580,7 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
     int nextp = 0;
     if (nblk_lane > 0) {
         const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS);
-        q0 = __ldcs(p); q1 = __ldcs(p + 1);
+        q0 = __ldcg(p); q1 = __ldcg(p + 1);
         if (nblk_lane > 8) nextp = page_next[page];
     }
     Raw r0 = gather(pos4, q0.x), r1 = gather(pos4, q0.y);
@@ -590,7 +590,7 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
             const bool turn = ((kb + 1) & 7) == 0;
             if (turn) page = nextp;
             const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS + (((kb + 1) & 7) << 3));
-            n0 = __ldcs(p); n1 = __ldcs(p + 1);
+            n0 = __ldcg(p); n1 = __ldcg(p + 1);
             if (turn && kb + 9 < nblk_lane) nextp = page_next[page];
         }
         const unsigned e[10] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, n0.x, n0.y};
