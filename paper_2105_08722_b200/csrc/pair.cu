@@ -7,15 +7,16 @@
 // the work is split by resource profile into two kernels around "groups" of 32 consecutive cell-sorted
 // primaries of one (iy,iz) pencil (lane = primary everywhere):
 //   k_fill  (a3, integer/fp32, few registers): ONE WARP per group.  Candidates = contiguous runs of the sorted
-//     array (one or two per neighbouring pencil, x-range culled against the group's cell range), staged 32 at a
-//     time in shared memory relative to primary 0 in fp32 and broadcast to the lanes.  A first fp32 evaluation
+//     array (one or two per neighbouring pencil, x-range culled against the group's cell range), read 32 at a time,
+//     made relative to primary 0 in fp32, culled against the bounding box of the group's primaries and compacted
+//     into a ring in shared memory, from where they are broadcast to the lanes.  A first fp32 evaluation
 //     decides every pair whose radius is farther than a proven error margin from all bin edges; the rest (~1e-4)
 //     is decided in fp64 exactly as DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so
 //     counts are bit-exact.  An accepted pair is appended, in candidate order, to the list of (primary, bin):
-//     lane-private cursors and an 8-entry ring per (bin, lane) in shared memory, flushed 4 entries (16 bytes)
-//     at a time into 256-byte pages of a pool in HBM; pages of one list are chained through page_next[].
+//     lane-private cursors and one 4-entry block per (bin, lane) in shared memory, written 16 bytes at a time
+//     into 256-byte pages of a pool in HBM; pages of one list are chained through page_next[].
 //     The final cursors are n_i(b), the per-(primary, bin) pair counts (an integer output of the path).
-//   k_harm  (a4, fp64, ~130 registers): one warp per (group, bin); every lane streams its own list, gathers the
+//   k_harm  (a4, fp64, ~166 registers): one warp per (group, bin); every lane streams its own list, gathers the
 //     candidates two rows ahead, and keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
 //     atomics, no cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit
 //     vector (fp32 rsqrt seed + one third-order fp64 step), w (x+iy)^m by complex recurrence, powers of z, one FMA
