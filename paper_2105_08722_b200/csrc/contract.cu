@@ -158,6 +158,7 @@ __device__ __forceinline__ void task4(double (&acc)[make_set4(NB, NW, W).aoff[ma
 #pragma unroll
         for (int k = 0; k < NG; ++k) { gr[k] = 0.0; gi[k] = 0.0; }
         const int t1 = L.tbeg[m3 + 1];
+#pragma unroll 1
         for (int t = L.tbeg[m3]; t < t1; ++t) {
             const PairTerm T = terms[t];
             double u[NS], v[NS], sx[NS], w[NS];
@@ -413,6 +414,7 @@ __device__ __forceinline__ void pairs_fixed_x(double (&zr)[NZ], double (&zi)[NZ]
                                               const double *pa, const double *pb)
 {
     constexpr int rs = NB * 32;
+#pragma unroll 1
     for (int t = t0; t < t1; ++t) {
         const PairTerm T = terms[t];
         const double rx = pa[T.ia_re * rs + X * 32], ix = pa[T.ia_im * rs + X * 32];
@@ -432,6 +434,7 @@ __device__ __forceinline__ void pairs_fixed_y(double (&zr)[NZ], double (&zi)[NZ]
                                               const double *pa, const double *pb)
 {
     constexpr int rs = NB * 32;
+#pragma unroll 1
     for (int t = t0; t < t1; ++t) {
         const PairTerm T = terms[t];
         const double ry = pb[T.ib_re * rs + Y * 32], iy = pb[T.ib_im * rs + Y * 32];
@@ -460,6 +463,7 @@ __device__ __forceinline__ void pairs_block(double (&zr)[NZ], double (&zi)[NZ], 
                                             const double *pa, const double *pb)
 {
     constexpr int rs = NB * 32, NY = Y1 - Y0 + 1;
+#pragma unroll 1
     for (int t = t0; t < t1; ++t) {
         const PairTerm T = terms[t];
         double u[NY], v[NY], sx[NY], w[NY];
