@@ -222,7 +222,19 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
     CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
     const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax);
-    const int nchunk = 32;
+    // chunks of groups per multiplet slot: the grid (slots x chunks CTAs, one per SM) should fill whole waves
+    int nchunk = 32;
+    if (factorised) {
+        int sms = 148, dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const int slots = contraction_grid_x(T.order, nb, T.nLam());
+        double best = 0.0;
+        for (int c = 28; c <= 40; ++c) {
+            const int ctas = slots * c, waves = (ctas + sms - 1) / sms;
+            const double eff = (double)ctas / ((double)waves * sms) - 1e-4 * std::abs(c - 32);
+            if (eff > best) { best = eff; nchunk = c; }
+        }
+    }
     CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout));
     CU(P->gweights.ensure(sizeof(double) * (size_t)ngmax * 32));
     CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
@@ -491,8 +503,8 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
                     ex += (double)(q.l3 + 1) * (2.0 * (nb2 - 1) + 4.0 * nb2 * (nb2 - 1) / 2); // Re[G a3]: 2 FMA per triple
                 }
         } else {
-            // two warps per multiplet split by the second bin at t (contract.cu): A holds Y(b1,b2<=t) and streams
-            // R(b3,.), B holds R(b3>=t+2,b4) and streams Y(.,b2>t); 4 multiplies per pre-weighted operand, 4 FMA per pair
+            // two warps per multiplet split by the second bin at t (contract.cu): A takes Y(b1,b2<=t) and R(b3>=2,b4),
+            // B takes Y(b1,b2>t) and R(b3>=t+2,b4); 4 multiplies per pre-weighted operand, 4 FMA per pair and term
             const int t = contraction_split5(nb);
             auto c2 = [](int n) { return n * (n - 1) / 2; };
             double tupA = 0, tupB = 0;
@@ -500,11 +512,12 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
             for (const Lam5 &q : T.lam5) {
                 const double nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0], nM = q.l12 + 1;
                 ex += nl * (4.0 * t + 8.0 * c2(t + 1)) + nM * 2.0 * c2(t + 1);                 // A: Y block, times w_i
-                for (int b3 = 2; b3 <= nb - 2; ++b3) ex += nr * (4.0 + 8.0 * (nb - 1 - b3));   // A: R(b3,.)
+                ex += nr * (4.0 * (nb - 3) + 8.0 * c2(nb - 2));                                // A: R block (all b3 >= 2)
                 ex += nM * 4.0 * tupA;                                                         // A: Re[Y R]
                 if (t + 1 <= nb - 3) {
-                    ex += nr * (4.0 * (nb - 3 - t) + 8.0 * c2(nb - 2 - t));                    // B: R block
-                    for (int b2 = t + 1; b2 <= nb - 3; ++b2) ex += nl * (4.0 + 8.0 * b2) + nM * 2.0 * b2; // B: Y(.,b2)
+                    const double nyb = c2(nb - 2) - c2(t + 1);
+                    ex += nr * (4.0 * (nb - 3 - t) + 8.0 * c2(nb - 2 - t));                    // B: R block (b3 >= t+2)
+                    ex += nl * (4.0 * (nb - 3 - t) + 8.0 * nyb) + nM * 2.0 * nyb;              // B: Y block, times w_i
                     ex += nM * 4.0 * tupB;                                                     // B: Re[Y R]
                 }
             }

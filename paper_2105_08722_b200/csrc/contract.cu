@@ -502,20 +502,22 @@ __device__ __forceinline__ void task5a(double (&acc)[NTOT], const Lam5 &L, int t
         pairs_block<NB, 0, 0, T - 1, 1, T, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
 #pragma unroll
         for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
-        static_for<2, NB - 1>([&](auto B3) {
-            constexpr int b3 = decltype(B3)::value, NR = NB - 1 - b3;
-            double rr[NR], ri[NR];
+        constexpr int NRH = c2(NB - 2); // pairs 2 <= b3 < b4 <= NB-1
+        double rr[NRH], ri[NRH];
 #pragma unroll
-            for (int q = 0; q < NR; ++q) { rr[q] = 0.0; ri[q] = 0.0; }
-            pairs_fixed_x<NB, b3, b3 + 1, NB - 1, NR>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+        for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
+        pairs_block<NB, 1, 2, NB - 2, 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+        static_for<2, NB - 1>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value;
             static_for<b3 + 1, NB>([&](auto B4) {
                 constexpr int b4 = decltype(B4)::value;
+                constexpr int q = slot5<NB, 1, 2, 3>(b3, b4);
                 static_for<1, (T < b3 - 1 ? T : b3 - 1) + 1>([&](auto B2) {
                     constexpr int b2 = decltype(B2)::value;
                     static_for<0, b2>([&](auto B1) {
                         constexpr int b1 = decltype(B1)::value;
                         constexpr int o = aidx5(NB, 1, b1, b2, b3, b4), k = c2(b2) + b1;
-                        acc[o] = fma(yr[k], rr[b4 - b3 - 1], fma(yi[k], ri[b4 - b3 - 1], acc[o]));
+                        acc[o] = fma(yr[k], rr[q], fma(yi[k], ri[q], acc[o]));
                     });
                 });
             });
@@ -537,14 +539,15 @@ __device__ __forceinline__ void task5b(double (&acc)[NTOT], const Lam5 &L, int t
 #pragma unroll
             for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
             pairs_block<NB, 1, T + 2, NB - 2, T + 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+            constexpr int NYH = c2(NB - 2) - c2(T + 1); // pairs b1 < b2, T+1 <= b2 <= NB-3
+            double yr[NYH], yi[NYH];
+#pragma unroll
+            for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
+            pairs_block<NB, 0, 0, NB - 4, T + 1, NB - 3, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
+#pragma unroll
+            for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
             static_for<T + 1, NB - 2>([&](auto B2) {
                 constexpr int b2 = decltype(B2)::value;
-                double yr[b2], yi[b2];
-#pragma unroll
-                for (int k = 0; k < b2; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
-                pairs_fixed_y<NB, b2, 0, b2 - 1, b2>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
-#pragma unroll
-                for (int k = 0; k < b2; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
                 static_for<b2 + 1, NB - 1>([&](auto B3) {
                     constexpr int b3 = decltype(B3)::value;
                     static_for<b3 + 1, NB>([&](auto B4) {
@@ -552,8 +555,8 @@ __device__ __forceinline__ void task5b(double (&acc)[NTOT], const Lam5 &L, int t
                         constexpr int k = slot5<NB, 1, T + 2, T + 3>(b3, b4);
                         static_for<0, b2>([&](auto B1) {
                             constexpr int b1 = decltype(B1)::value;
-                            constexpr int o = aidx5(NB, T + 1, b1, b2, b3, b4);
-                            acc[o] = fma(yr[b1], rr[k], fma(yi[b1], ri[k], acc[o]));
+                            constexpr int o = aidx5(NB, T + 1, b1, b2, b3, b4), q = slot5<NB, 0, 0, T + 1>(b1, b2);
+                            acc[o] = fma(yr[q], rr[k], fma(yi[q], ri[k], acc[o]));
                         });
                     });
                 });
@@ -582,11 +585,12 @@ __device__ __forceinline__ void flush5(const double (&acc)[NTOT], const int *tup
     });
 }
 
-// 12 warps per CTA = 6 multiplets; even warp: b2 <= T, odd warp: b2 > T
+// 8 warps per CTA (255 registers) = 4 multiplets; even warp: b2 <= T, odd warp: b2 > T
+constexpr int kCtaWarps5 = 8;
 template <int NB>
-__global__ void __launch_bounds__(kCtaWarps * 32, 1) k_contract5(ContractArgs a, int nbuf)
+__global__ void __launch_bounds__(kCtaWarps5 * 32, 1) k_contract5(ContractArgs a, int nbuf)
 {
-    constexpr int LPC = kCtaWarps / 2, T = t5(NB);
+    constexpr int LPC = kCtaWarps5 / 2, T = t5(NB);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int slot = blockIdx.x * LPC + (warp >> 1);
     const bool have = slot < a.nLam;
@@ -640,11 +644,11 @@ template <int NB>
 cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 {
     size_t smem;
-    constexpr int LPC = kCtaWarps / 2;
+    constexpr int LPC = kCtaWarps5 / 2;
     const int nbuf = pipe_config(a, LPC, &smem);
     cudaError_t e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_contract5<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps * 32, smem, s>>>(a, nbuf);
+    k_contract5<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps5 * 32, smem, s>>>(a, nbuf);
     return cudaGetLastError();
 }
 
@@ -653,6 +657,13 @@ cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 // Factorised kernels cover the bin counts whose per-warp partial sums fit in registers; anything else (and N = 3,
 // which is cheap) runs the generic kernel.
 int contraction_split5(int nbins) { return t5(nbins); }
+
+// CTAs along x of the factorised kernels (multiplet slots)
+int contraction_grid_x(int order, int nbins, int nlam)
+{
+    const int lpc = order == 4 ? lpc4(nbins) : kCtaWarps5 / 2;
+    return (nlam + lpc - 1) / lpc;
+}
 
 int contraction_is_factorised(int order, int nbins, int lmax)
 {

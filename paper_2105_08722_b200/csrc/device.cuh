@@ -113,6 +113,7 @@ struct ContractArgs {
     int factorised;             // set by launch_contraction
 };
 int contraction_is_factorised(int order, int nbins, int lmax);
+int contraction_grid_x(int order, int nbins, int nlam);
 int contraction_split5(int nbins);   // N = 5: second bins <= this go to the first warp of a multiplet
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
