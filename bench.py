@@ -144,7 +144,7 @@ def run_reference(args, cfg):
 
 
 def workload_config(cfg, args):
-    return {"workload": f"{cfg.name}: {cfg.order}PCF, n={cfg.n} {cfg.kind} points, "
+    return {"workload": f"{cfg.name}{' ALLPARITY' if getattr(args, 'allparity', False) else ''}: {cfg.order}PCF, n={cfg.n} {cfg.kind} points, "
                         f"{'periodic L=%g' % cfg.box if cfg.box > 0 else 'open cut-sky shell'}, weights {cfg.weights}, "
                         f"{cfg.nbins} bins in [{cfg.rmin:g},{cfg.rmax:g}], lmax={cfg.lmax}",
             "l2": "256 MiB device memset between steps inside the timed bracket; per-step intermediates (a_lm tiles, "
@@ -152,11 +152,11 @@ def workload_config(cfg, args):
             "sharding": "one independent catalogue per rank (seed + 100 rank), no collective"}
 
 
-def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True):
+def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False):
     pos, w = make_catalogue(cfg, rank)
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    plan = E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box)
+    plan = E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box, allparity=allparity)
     E.encore_set_timing(plan.h, True)
     out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream(dev)
@@ -230,6 +230,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--all-configs", action="store_true", help="also measure c1..c5 (2 steps each) into per_config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--allparity", action="store_true", help="ALLPARITY plan: parity-odd multiplets too (not the headline config)")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]
     if args.impl == "reference":
@@ -253,7 +254,7 @@ def main():
     steps, warmup = args.steps, max(3, args.warmup)
 
     with ClockSampler(local) as clocks:
-        res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev)
+        res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev, allparity=args.allparity)
     ms_total = max_over_ranks(torch, res["ms_total"], dev)
     e2e_ms = max_over_ranks(torch, res["e2e_ms_total"], dev)
     ms_per_step = ms_total / steps
@@ -311,6 +312,14 @@ def main():
                          "pair_frac_fp64": pair_flops(c.lmax, r["pairs"], r["candidates"]) / (s["pair"] * 1e-3) / peak_derived,
                          "contraction_gflops_canonical": c.n * ca / (s["contraction"] * 1e-3) / 1e9,
                          "contraction_frac_fp64_executed": c.n * ex / (s["contraction"] * 1e-3) / peak_derived}
+        # the same c3 catalogue with the parity-odd multiplets too (111 instead of 69 multiplets)
+        r, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, allparity=True)
+        ex, ca = r["flops_contraction"]
+        per["c3_allparity"] = {"order": 4, "n": W.CONFIGS["c3"].n, "ms_per_step": r["ms_total"] / 2,
+                               "primaries_per_s": W.CONFIGS["c3"].n / (r["ms_total"] / 2 * 1e-3), "stage_ms": r["stages"],
+                               "n_multiplets": r["nout"] // 120,
+                               "contraction_gflops_canonical": W.CONFIGS["c3"].n * ca / (r["stages"]["contraction"] * 1e-3) / 1e9,
+                               "contraction_frac_fp64_executed": W.CONFIGS["c3"].n * ex / (r["stages"]["contraction"] * 1e-3) / peak_derived}
         line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))

@@ -64,6 +64,15 @@ enum {
 int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
                 double box_size);
 
+/* encore_plan with mode flags.  ENCORE_ALLPARITY (the paper's ALLPARITY mode): the multiplet list
+ * also holds the parity-odd multiplets (odd sum of the principal l's; 111 instead of 69 for N=4, lmax=5).
+ * Their zeta is purely imaginary (eq. 8): zeta_out holds Re zeta for even and Im zeta for odd multiplets,
+ *   Im zeta = (1/V) sum_i w_i sum_{M, m_{N-1} >= 0} 2 S(m_{N-1}) E(Lam) C^Lam_M Im[prod_k a~]   (App. B),
+ * with separations r_j - s_i as in eq. 35 (the sign of odd multiplets depends on it).  Unknown flags: ENCORE_EINVAL. */
+#define ENCORE_ALLPARITY 1u
+int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
+                      double box_size, unsigned flags);
+
 /* Run steps a1..a6 on `cuda_stream` (a cudaStream_t cast to void*, NULL = default stream).
  *   positions DEVICE, SoA x[n] y[n] z[n] (3n doubles), read-only
  *   weights   DEVICE, n doubles, or NULL for unit weights (negative weights allowed: D-R fields)
@@ -103,6 +112,7 @@ int encore_num_bin_tuples(const encore_plan_t *plan);      /* n_B = C(nbins, N-1
 int64_t encore_num_terms(const encore_plan_t *plan);       /* non-zero (Lam, M) with m_{N-1} >= 0 (1126 for N=4,lmax=5) */
 int encore_get_multiplets(const encore_plan_t *plan, int *out /* HOST [n_Lambda][2N-5] */);
 int encore_get_bin_tuples(const encore_plan_t *plan, int *out /* HOST [n_B][N-1] */);
+int encore_get_multiplet_parity(const encore_plan_t *plan, int *out /* HOST [n_Lambda]: 0 even (Re zeta stored), 1 odd (Im zeta) */);
 int encore_get_bin_edges(const encore_plan_t *plan, double *out /* HOST [nbins+1] */);
 /* flop counts per primary of the contraction as executed (fused multiply-add = 2) and by the canonical
  * "Algorithm 3 literal" model of SURVEY.md §8(d) (5/11/17 flop per term evaluation for N=3/4/5) */

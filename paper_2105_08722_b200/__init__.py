@@ -24,7 +24,7 @@ OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -50,6 +50,8 @@ def lib():
     L = C.CDLL(path)
     vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
     L.encore_plan.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double]
+    L.encore_plan_flags.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_uint]
+    L.encore_get_multiplet_parity.argtypes = [vp, ip]
     L.encore_compute.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
     L.encore_compute_host.argtypes = [vp, vp, vp, C.c_int64, vp]
     L.encore_compute_shard.argtypes = [vp, vp, vp, C.c_int64, C.c_int, C.c_int, vp, vp]
@@ -103,6 +105,21 @@ def encore_plan(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: i
     h = C.c_void_p()
     _check(lib().encore_plan(C.byref(h), npcf_order, r_min, r_max, nbins, lmax, box_size))
     return h
+
+
+ALLPARITY = 1
+
+
+def encore_plan_flags(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: int, box_size: float, flags: int):
+    h = C.c_void_p()
+    _check(lib().encore_plan_flags(C.byref(h), npcf_order, r_min, r_max, nbins, lmax, box_size, flags))
+    return h
+
+
+def encore_get_multiplet_parity(plan) -> np.ndarray:
+    out = np.zeros(encore_num_multiplets(plan), dtype=np.int32)
+    _check(lib().encore_get_multiplet_parity(plan, out.ctypes.data_as(C.POINTER(C.c_int))))
+    return out
 
 
 def encore_compute(plan, positions, weights, n: int, zeta_out, cuda_stream: int = 0):
@@ -231,9 +248,10 @@ def encore_measure_fp64_peak(cuda_stream: int = 0) -> float:
 class Plan:
     """RAII wrapper: Plan(order, r_min, r_max, nbins, lmax, box) -> .compute(pos, w) on CUDA tensors."""
 
-    def __init__(self, order, r_min, r_max, nbins, lmax, box=0.0):
+    def __init__(self, order, r_min, r_max, nbins, lmax, box=0.0, allparity=False):
         self.order, self.r_min, self.r_max, self.nbins, self.lmax, self.box = order, r_min, r_max, nbins, lmax, box
-        self.h = encore_plan(order, r_min, r_max, nbins, lmax, box)
+        self.h = (encore_plan_flags(order, r_min, r_max, nbins, lmax, box, ALLPARITY) if allparity
+                  else encore_plan(order, r_min, r_max, nbins, lmax, box))
         self.n_lambda = encore_num_multiplets(self.h)
         self.n_b = encore_num_bin_tuples(self.h)
 

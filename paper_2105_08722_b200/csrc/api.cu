@@ -33,7 +33,7 @@ struct DevBuf {
 struct encore_plan_s {
     HostTables T;
     bool uploaded = false;
-    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_tuple_index, gweights;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_lam_parity, d_tuple_index, gweights;
     bool force_generic = false;
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
@@ -105,6 +105,8 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
         CU(P->d_lam4.ensure(sizeof(Lam4) * std::max<size_t>(1, T.lam4.size())));
         CU(P->d_lam5.ensure(sizeof(Lam5) * std::max<size_t>(1, T.lam5.size())));
         CU(P->d_lam_order.ensure(sizeof(int) * std::max<size_t>(1, T.lam_order.size())));
+        CU(P->d_lam_parity.ensure(sizeof(int) * std::max<size_t>(1, T.parity.size())));
+        CU(cudaMemcpyAsync(P->d_lam_parity.p, T.parity.data(), sizeof(int) * T.parity.size(), cudaMemcpyHostToDevice, s));
         CU(P->d_tuple_index.ensure(sizeof(int) * cells));
         CU(cudaMemcpyAsync(P->d_pair_terms.p, T.pair_terms.data(), sizeof(PairTerm) * T.pair_terms.size(), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(P->d_lam4.p, T.lam4.data(), sizeof(Lam4) * T.lam4.size(), cudaMemcpyHostToDevice, s));
@@ -355,6 +357,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.lam4 = P->d_lam4.as<Lam4>();
     ca.lam5 = P->d_lam5.as<Lam5>();
     ca.lam_order = P->d_lam_order.as<int>();
+    ca.lam_parity = P->d_lam_parity.as<int>();
     ca.tuple_index = P->d_tuple_index.as<int>();
     ca.lmax = T.lmax;
     ca.max_terms = 1;
@@ -379,6 +382,13 @@ extern "C" {
 
 int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax, double box_size)
 {
+    return encore_plan_flags(plan_out, npcf_order, r_min, r_max, nbins, lmax, box_size, 0u);
+}
+
+int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax, double box_size,
+                      unsigned flags)
+{
+    if (flags & ~(unsigned)ENCORE_ALLPARITY) return plan_out ? (*plan_out = nullptr, ENCORE_EINVAL) : ENCORE_EINVAL;
     if (!plan_out) return ENCORE_EINVAL;
     *plan_out = nullptr;
     if (npcf_order < 3 || npcf_order > ENCORE_MAX_ORDER) return ENCORE_EINVAL;
@@ -391,7 +401,7 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
     encore_plan_s *P = new (std::nothrow) encore_plan_s();
     if (!P) return ENCORE_EALLOC;
     try {
-        encore_build_tables(P->T, npcf_order, r_min, r_max, nbins, lmax, box_size);
+        encore_build_tables(P->T, npcf_order, r_min, r_max, nbins, lmax, box_size, (flags & ENCORE_ALLPARITY) ? 1 : 0);
     } catch (...) {
         delete P;
         return ENCORE_EALLOC;
@@ -416,6 +426,13 @@ int encore_compute_shard(encore_plan_t *P, const double *positions, const double
     if (!P || !positions || !zeta_partial_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
     if (nshards < 1 || shard < 0 || shard >= nshards) return ENCORE_EINVAL;
     return compute_device(P, positions, weights, n, zeta_partial_out, static_cast<cudaStream_t>(cuda_stream), shard, nshards);
+}
+
+int encore_get_multiplet_parity(const encore_plan_t *P, int *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    for (size_t i = 0; i < P->T.parity.size(); ++i) out[i] = P->T.parity[i];
+    return ENCORE_OK;
 }
 
 int encore_get_shard_groups(const encore_plan_t *P, int out[3])
@@ -446,7 +463,7 @@ int encore_destroy(encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
     DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_ycoef, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
-                      &P->d_lam_order, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
+                      &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
                       &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->pool,

@@ -39,6 +39,7 @@ struct PairTerm {
 //   H_i = sum_{m3>=0} Re[ G_{m3}(b1,b2) a_{l3 m3}(b3) ],  G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2
 struct Lam4 {
     int l1, l2, l3;
+    int odd;            // parity-odd multiplet: the stored result is Im instead of Re (App. B)
     int tbeg[9];        // terms of m3 are [tbeg[m3], tbeg[m3+1]) in pair_terms
     int nterms;
 };
@@ -48,6 +49,7 @@ struct Lam4 {
 //   R34_M = sum_{m3+m4=-M} (l3 l4 l12; m3 m4 M) a~3 a~4.
 struct Lam5 {
     int l1, l2, l12, l3, l4;
+    int odd;
     int lbeg[14];       // left terms of M: [lbeg[M], lbeg[M+1])   (M <= l12 <= 12)
     int rbeg[14];       // right terms
     int nterms;
@@ -55,6 +57,8 @@ struct Lam5 {
 
 struct HostTables {
     int order = 0, nbins = 0, lmax = 0, ncomp = 0, width = 0; // width = 2N-5 columns of a multiplet row
+    int allparity = 0;               // 1: odd-parity multiplets too (ALLPARITY mode)
+    std::vector<int> parity;         // [nLam] 0 even (zeta real), 1 odd (zeta = i * stored value)
     double rmin = 0, rmax = 0, box = 0;
     std::vector<int> multiplets;     // [nLam][width]
     std::vector<int> bin_tuples;     // [nB][N-1]
@@ -75,4 +79,4 @@ struct HostTables {
 
 // Host side (tables.cpp)
 double encore_host_wigner3j(int j1, int j2, int j3, int m1, int m2, int m3);
-int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box);
+int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box, int allparity = 0);

@@ -39,6 +39,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a
         int boff[4];
         for (int k = 0; k < nm; ++k) boff[k] = a.bin_tuples[iB * nm + k] * 32;
         double acc = 0.0;
+        const bool odd = a.lam_parity[iL] != 0; // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)
         const int t1 = a.term_start[iL + 1];
         for (int t = a.term_start[iL]; t < t1; ++t) {
             const DevTerm tm = a.terms[t];
@@ -50,7 +51,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a
                 const double ni = pr * im + pi * re;
                 pr = nr; pi = ni;
             }
-            acc += pr;
+            acc += odd ? pi : pr;
         }
         acc *= wi;
 #pragma unroll
@@ -184,10 +185,12 @@ __device__ __forceinline__ void task4(double (&acc)[make_set4(NB, NW, W).aoff[ma
         }
         const int cr = m3 == 0 ? 0 : 2 * m3 - 1;
         const double *q3r = p3 + cr * rs, *q3i = p3 + (m3 == 0 ? cr : cr + 1) * rs;
-        const double wim = m3 == 0 ? 0.0 : -wi;
+        // even parity: Re[G a3] = Gr Re a3 - Gi Im a3;  odd parity: Im[G a3] = Gr Im a3 + Gi Re a3  (Im a3 = 0 at m3 = 0)
+        const double *pA = L.odd ? q3i : q3r, *pB = L.odd ? q3r : q3i;
+        const double cA = L.odd ? (m3 == 0 ? 0.0 : wi) : wi, cB = L.odd ? wi : (m3 == 0 ? 0.0 : -wi);
         static_for<BMIN + 2, NB>([&](auto B3) {
             constexpr int b3 = decltype(B3)::value;
-            const double r3 = wi * q3r[b3 * 32], i3 = wim * q3i[b3 * 32]; // Re[G a3] = Gr r3 - Gi i3
+            const double r3 = cA * pA[b3 * 32], i3 = cB * pB[b3 * 32];
             static_for<0, NS>([&](auto J) {
                 constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
                 static_for<b1 + 1, b3>([&](auto B2) {
@@ -500,13 +503,18 @@ __device__ __forceinline__ void task5a(double (&acc)[NTOT], const Lam5 &L, int t
 #pragma unroll
         for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
         pairs_block<NB, 0, 0, T - 1, 1, T, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
+        const double wyi = L.odd ? wi : -wi;
 #pragma unroll
-        for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
+        for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= wyi; } // even: Re[Y R] = Yr Rr - Yi Ri; odd: Im[Y R] = Yr Ri + Yi Rr
         constexpr int NRH = c2(NB - 2); // pairs 2 <= b3 < b4 <= NB-1
         double rr[NRH], ri[NRH];
 #pragma unroll
         for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
         pairs_block<NB, 1, 2, NB - 2, 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
+        if (L.odd) {
+#pragma unroll
+            for (int k = 0; k < NRH; ++k) { const double x = rr[k]; rr[k] = ri[k]; ri[k] = x; }
+        }
         static_for<2, NB - 1>([&](auto B3) {
             constexpr int b3 = decltype(B3)::value;
             static_for<b3 + 1, NB>([&](auto B4) {
@@ -544,8 +552,13 @@ __device__ __forceinline__ void task5b(double (&acc)[NTOT], const Lam5 &L, int t
 #pragma unroll
             for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
             pairs_block<NB, 0, 0, NB - 4, T + 1, NB - 3, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
+            const double wyi = L.odd ? wi : -wi;
 #pragma unroll
-            for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= -wi; } // Re[Y R] = Yr Rr - Yi Ri
+            for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= wyi; } // even: Yr Rr - Yi Ri; odd: Yr Ri + Yi Rr
+            if (L.odd) {
+#pragma unroll
+                for (int k = 0; k < NRH; ++k) { const double x = rr[k]; rr[k] = ri[k]; ri[k] = x; }
+            }
             static_for<T + 1, NB - 2>([&](auto B2) {
                 constexpr int b2 = decltype(B2)::value;
                 static_for<b2 + 1, NB - 1>([&](auto B3) {

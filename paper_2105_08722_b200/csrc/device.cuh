@@ -106,6 +106,7 @@ struct ContractArgs {
     const Lam4 *lam4;           // device [nLam]
     const Lam5 *lam5;           // device [nLam]
     const int *lam_order;       // device [nLam], heaviest first
+    const int *lam_parity;      // device [nLam]: 1 = parity-odd multiplet (the stored value is Im zeta)
     const int *tuple_index;     // device [nbins^(N-1)]: index of the ordered tuple in bin_tuples, -1 if not ordered
     int lmax;
     int max_terms;              // largest number of coupled-pair terms of one multiplet

@@ -80,7 +80,7 @@ void enumerate_multiplets(HostTables &t)
         for (int l1 = 0; l1 <= L; ++l1)
             for (int l2 = 0; l2 <= L; ++l2)
                 for (int l3 = std::abs(l1 - l2); l3 <= std::min(l1 + l2, L); ++l3)
-                    if (((l1 + l2 + l3) & 1) == 0) { // even parity only
+                    if (t.allparity || ((l1 + l2 + l3) & 1) == 0) { // even parity unless ALLPARITY
                         t.multiplets.push_back(l1); t.multiplets.push_back(l2); t.multiplets.push_back(l3);
                     }
     } else {
@@ -89,10 +89,24 @@ void enumerate_multiplets(HostTables &t)
                 for (int l12 = std::abs(l1 - l2); l12 <= l1 + l2; ++l12)
                     for (int l3 = 0; l3 <= L; ++l3)
                         for (int l4 = std::abs(l12 - l3); l4 <= std::min(l12 + l3, L); ++l4)
-                            if (((l1 + l2 + l3 + l4) & 1) == 0) {
+                            if (t.allparity || ((l1 + l2 + l3 + l4) & 1) == 0) {
                                 const int row[5] = {l1, l2, l12, l3, l4};
                                 t.multiplets.insert(t.multiplets.end(), row, row + 5);
                             }
+    }
+}
+
+// E(Lam) = (-1)^{sum of principal l}: 0 = parity-even (zeta real), 1 = parity-odd (zeta imaginary)
+void fill_parity(HostTables &t)
+{
+    const int nL = t.nLam();
+    t.parity.assign(nL, 0);
+    for (int iL = 0; iL < nL; ++iL) {
+        const int *lam = &t.multiplets[(size_t)iL * t.width];
+        int s = 0;
+        if (t.order == 4) s = lam[0] + lam[1] + lam[2];
+        else if (t.order == 5) s = lam[0] + lam[1] + lam[3] + lam[4];
+        t.parity[iL] = s & 1;
     }
 }
 
@@ -190,7 +204,7 @@ void build_factorised(HostTables &t)
         for (int iL = 0; iL < nL; ++iL) {
             const int *lam = &t.multiplets[(size_t)iL * 3];
             Lam4 q{};
-            q.l1 = lam[0]; q.l2 = lam[1]; q.l3 = lam[2];
+            q.l1 = lam[0]; q.l2 = lam[1]; q.l3 = lam[2]; q.odd = t.parity[iL];
             for (int m3 = 0; m3 <= q.l3; ++m3) {
                 q.tbeg[m3] = (int)t.pair_terms.size();
                 // G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2   (eq. 44 with E C = plain 3-j, eq. 18)
@@ -205,7 +219,7 @@ void build_factorised(HostTables &t)
         for (int iL = 0; iL < nL; ++iL) {
             const int *lam = &t.multiplets[(size_t)iL * 5];
             Lam5 q{};
-            q.l1 = lam[0]; q.l2 = lam[1]; q.l12 = lam[2]; q.l3 = lam[3]; q.l4 = lam[4];
+            q.l1 = lam[0]; q.l2 = lam[1]; q.l12 = lam[2]; q.l3 = lam[3]; q.l4 = lam[4]; q.odd = t.parity[iL];
             for (int M = 0; M <= q.l12; ++M) {
                 const double f = std::sqrt(2.0 * q.l12 + 1.0) * (((q.l12 - M) & 1) ? -1.0 : 1.0) * (M == 0 ? 1.0 : 2.0);
                 q.lbeg[M] = (int)t.pair_terms.size();
@@ -231,13 +245,15 @@ void build_factorised(HostTables &t)
 
 } // namespace
 
-int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box)
+int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box, int allparity)
 {
     t = HostTables();
+    t.allparity = allparity;
     t.order = order; t.nbins = nbins; t.lmax = lmax; t.rmin = rmin; t.rmax = rmax; t.box = box;
     t.width = 2 * order - 5;
     t.ncomp = (lmax + 1) * (lmax + 1);
     enumerate_multiplets(t);
+    fill_parity(t);
     enumerate_bins(t);
     enumerate_terms(t);
     // bins: e_b = r_min + b * width, e_nbins = r_max (R8)

@@ -91,3 +91,26 @@ def test_plan_tables_equal_oracle_enumeration(oracle):
             assert (p.bin_tuples == oracle.bin_tuples(order, nbins)).all()
             assert E.encore_num_terms(p.h) == oracle.count_terms(order, lmax, half=True)
             assert np.array_equal(E.encore_get_bin_edges(p.h, nbins), oracle.bin_edges(5.0, 65.0, nbins))
+
+
+def test_allparity_tables_on_the_host():
+    """ALLPARITY plan (host tables only): the multiplet counts of PAPER.md:602 and the oracle's enumeration"""
+    import oracle
+    import paper_2105_08722_b200 as E
+    for order, lmax, expect in [(4, 5, 111), (4, 3, None), (5, 2, None), (3, 4, 5)]:
+        h = E.encore_plan_flags(order, 1.0, 20.0, 6, lmax, 0.0, E.ALLPARITY)
+        try:
+            lam = E.encore_get_multiplets(h, order)
+            ref = oracle.multiplets(order, lmax, allparity=True)
+            assert (lam == ref).all()
+            if expect is not None:
+                assert len(lam) == expect
+            assert E.encore_num_terms(h) == oracle.count_terms(order, lmax, allparity=True, half=True)
+            par = E.encore_get_multiplet_parity(h)
+            principal = ref[:, [0, 1, 3, 4]] if order == 5 else ref
+            assert (par == principal.sum(axis=1) % 2).all() if order > 3 else not par.any()
+        finally:
+            E.encore_destroy(h)
+    import pytest
+    with pytest.raises(E.EncoreError):
+        E.encore_plan_flags(4, 1.0, 20.0, 6, 2, 0.0, 2)      # unknown flag

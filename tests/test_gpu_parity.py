@@ -270,3 +270,31 @@ def test_shard_argument_errors(E):
             with pytest.raises(E.EncoreError) as ei:
                 plan.compute_shard(pos, None, shard, nshards)
             assert ei.value.status == E.EINVAL
+
+
+# ---- ALLPARITY: parity-odd multiplets, zeta imaginary ----------------
+@pytest.mark.parametrize("order,nbins,lmax,box", [(4, 10, 3, 0.0), (4, 6, 4, 90.0), (4, 11, 2, 0.0), (5, 8, 2, 0.0),
+                                                  (5, 5, 2, 90.0), (5, 9, 1, 0.0), (3, 4, 3, 0.0)])
+def test_allparity_matches_the_oracle(E, oracle, order, nbins, lmax, box):
+    rng = np.random.default_rng(4200 + 10 * order + nbins)
+    n = 300 if order == 4 else 180
+    pos = np.ascontiguousarray(rng.uniform(0, 90.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.2, 0.8])
+    o = oracle.zeta(order, pos, w, box, 4.0, 44.0, nbins, lmax, allparity=True)
+    dev = torch.device("cuda:0")
+    with E.Plan(order, 4.0, 44.0, nbins, lmax, box, allparity=True) as plan:
+        assert (plan.multiplets == o["multiplets"]).all()
+        par = E.encore_get_multiplet_parity(plan.h).astype(bool)
+        z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev))
+        torch.cuda.synchronize()
+        z = z.cpu().numpy()
+    principal = o["multiplets"][:, [0, 1, 3, 4]] if order == 5 else o["multiplets"]
+    assert (par == (principal.sum(axis=1) % 2 == 1)).all() if order > 3 else not par.any()
+    if order > 3:
+        assert par.any()
+    expect = np.where(par[:, None], o["zeta_im"], o["zeta"])      # Re zeta for even, Im zeta for odd multiplets
+    scale = max(np.abs(o["zeta"]).max(), np.abs(o["zeta_im"]).max())
+    # the oracle's other component vanishes: even multiplets are real, odd ones imaginary (eq. 8)
+    assert np.abs(np.where(par[:, None], o["zeta"], o["zeta_im"])).max() <= 1e-12 * scale
+    assert np.abs(z - expect).max() <= TOL * scale
+    assert np.abs(expect[par]).max() > 1e-6 * scale if order > 3 else True   # the odd part is not trivially zero
