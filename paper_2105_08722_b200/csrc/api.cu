@@ -512,7 +512,9 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
     if (!P->force_generic && contraction_is_factorised(N, nb, T.lmax)) {
         // executed by the factorised kernels, fused multiply-add = 2
         ex = 0.0;
-        if (N == 4) {
+        if (N == 3) { // per real component: nb scalings + one FMA per bin pair
+            ex = (double)T.ncomp * (nb + 2.0 * (nb * (nb - 1) / 2));
+        } else if (N == 4) {
             for (const Lam4 &q : T.lam4)
                 for (int b1 = 0; b1 + 2 < nb; ++b1) {
                     const int nb2 = nb - 1 - b1;

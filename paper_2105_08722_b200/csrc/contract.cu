@@ -104,6 +104,60 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// ---- N = 3 ------------------------------------------------------------------------------------------------
+// eq. 16 with a_{l,-m} = (-1)^m a*_lm:
+//   H_l(b1,b2) = (-1)^l / sqrt(2l+1) [ a_l0(b1) a_l0(b2) + 2 sum_{m>0} Re(a_lm(b1) conj a_lm(b2)) ]
+// i.e. a real dot product over the 2l+1 real components of the l-block.  One CTA per (l, chunk of groups), a warp per
+// group in turn, lane = primary; the c2(NB) partial sums of the block stay in registers over the warp's groups.  The
+// kernel reads every a_lm element exactly once (coalesced 256-byte rows): it is bound by HBM, not by arithmetic.
+template <int NB>
+__global__ void __launch_bounds__(128) k_contract3(ContractArgs a)
+{
+    constexpr int NP = c2(NB);
+    __shared__ double red[4][NP];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int l = a.nLam - 1 - (int)blockIdx.x; // heaviest block first
+    const int chunk = blockIdx.y;
+    double acc[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) acc[p] = 0.0;
+    for (int g = a.g_begin + chunk * 4 + warp; g < a.g_end; g += 4 * (int)gridDim.y) {
+        const double wi = a.gweights[(size_t)g * 32 + lane];
+        const double *tile = a.alm + ((size_t)g * a.ncomp + (size_t)l * l) * NB * 32 + lane;
+        for (int c = 0; c <= 2 * l; ++c) {
+            const double s = c == 0 ? wi : 2.0 * wi;
+            double v[NB], sv[NB];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) { v[b] = tile[((size_t)c * NB + b) * 32]; sv[b] = s * v[b]; }
+#pragma unroll
+            for (int b2 = 1; b2 < NB; ++b2)
+#pragma unroll
+                for (int b1 = 0; b1 < b2; ++b1) acc[c2(b2) + b1] = fma(sv[b1], v[b2], acc[c2(b2) + b1]);
+        }
+    }
+    const double cl = ((l & 1) ? -1.0 : 1.0) / sqrt(2.0 * l + 1.0);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const double t = warp_sum(acc[p]);
+        if (lane == 0) red[warp][p] = t;
+    }
+    __syncthreads();
+    double *out = a.partial + ((size_t)chunk * a.nLam + l) * a.nB;
+    for (int p = threadIdx.x; p < NP; p += 128) {
+        int b2 = 1;
+        while (c2(b2 + 1) <= p) ++b2;
+        const int b1 = p - c2(b2);
+        out[a.tuple_index[b1 * NB + b2]] = cl * (((red[0][p] + red[1][p]) + red[2][p]) + red[3][p]); // fixed order
+    }
+}
+
+template <int NB>
+cudaError_t launch3(const ContractArgs &a, cudaStream_t s)
+{
+    k_contract3<NB><<<dim3(a.nLam, a.nchunk), 128, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
 // ---- N = 4 ------------------------------------------------------------------------------------------------
 // The first bins b1 = 0 .. NB-3 of a multiplet are dealt to its NW warps in snake order (0,1,..,NW-1,NW-1,..,1,0,0,1,..):
 // equal numbers of (b1,b2) pairs per warp.  A warp sweeps ALL its b1 together, so that an operand a~2(b2) or a3(b3)
@@ -674,12 +728,14 @@ int contraction_split5(int nbins) { return t5(nbins); }
 // CTAs along x of the factorised kernels (multiplet slots)
 int contraction_grid_x(int order, int nbins, int nlam)
 {
+    if (order == 3) return nlam;
     const int lpc = order == 4 ? lpc4(nbins) : kCtaWarps5 / 2;
     return (nlam + lpc - 1) / lpc;
 }
 
 int contraction_is_factorised(int order, int nbins, int lmax)
 {
+    if (order == 3) return nbins >= 2 && nbins <= 10;
     if (order == 4) return nbins >= 3 && nbins <= 10 && lmax <= 6;
     if (order == 5) return nbins >= 4 && nbins <= 8 && lmax <= 4;
     return 0;
@@ -694,7 +750,19 @@ cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launc
         return cudaGetLastError();
     }
     // every (multiplet, tuple) of a chunk row is written by exactly one warp; no initialisation needed
-    if (a.order == 4) {
+    if (a.order == 3) {
+        switch (a.nbins) {
+        case 2: return launch3<2>(a, s);
+        case 3: return launch3<3>(a, s);
+        case 4: return launch3<4>(a, s);
+        case 5: return launch3<5>(a, s);
+        case 6: return launch3<6>(a, s);
+        case 7: return launch3<7>(a, s);
+        case 8: return launch3<8>(a, s);
+        case 9: return launch3<9>(a, s);
+        case 10: return launch3<10>(a, s);
+        }
+    } else if (a.order == 4) {
         switch (a.nbins) {
         case 3: return launch4<3>(a, s);
         case 4: return launch4<4>(a, s);
