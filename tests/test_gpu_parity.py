@@ -110,7 +110,8 @@ def test_c5_reduced_5pcf(E, oracle):
 
 
 # ---- edge cases ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("order,nbins,lmax", [(3, 2, 0), (3, 3, 7), (4, 3, 1), (4, 13, 2), (5, 4, 1), (5, 5, 2)])
+@pytest.mark.parametrize("order,nbins,lmax", [(3, 2, 0), (3, 3, 7), (3, 4, 6), (3, 3, 8), (3, 5, 9), (4, 3, 1), (4, 13, 2),
+                                              (5, 4, 1), (5, 5, 2)])
 def test_small_clouds_open_and_periodic(E, oracle, order, nbins, lmax):
     rng = np.random.default_rng(1000 + 10 * order + lmax)
     n = 257                                                   # several groups and a ragged tail
