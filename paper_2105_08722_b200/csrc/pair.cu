@@ -623,7 +623,7 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
 }
 
 template <int LMAX, int MLO, int MHI, bool PERIODIC>
-__global__ void __launch_bounds__(kHarmWarps * 32, 3) k_harm(PairArgs a, int g0, int g1)
+__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > 44 ? 2 : 3) k_harm(PairArgs a, int g0, int g1)
 {
     constexpr int NACC = ncomp_range(LMAX, MLO, MHI);
     __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
@@ -717,8 +717,9 @@ cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches)
         if (e != cudaSuccess) return e;                                 \
     }
 
-// m-ranges per lmax keep the register-resident accumulators of one pass at <= 49 doubles (168 registers, 12 warps/SM);
-// every pass re-reads the lists and gathers the candidates again (the L1 data pipe is ~70 % busy), so fewer is better
+// m-ranges per lmax.  Every pass re-reads the lists and gathers the candidates again (the L1 data pipe is ~70 % busy),
+// so fewer, fatter passes win: up to 44 accumulators run at 168 registers and 12 warps/SM, 45-65 at 255 registers and
+// 8 warps/SM (c2, lmax 10: four passes 46.3 ms, three 40.1 ms, two 37.1 ms for the pair stage).
 cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches)
 {
     const int ng = g1 - g0, nb = a.bins.nbins;
@@ -745,11 +746,11 @@ cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr
     case 3: HARM_PASS(3, 0, 3) break;
     case 4: HARM_PASS(4, 0, 4) break;
     case 5: HARM_PASS(5, 0, 5) break;
-    case 6: HARM_PASS(6, 0, 2) HARM_PASS(6, 3, 6) break;
-    case 7: HARM_PASS(7, 0, 2) HARM_PASS(7, 3, 7) break;
+    case 6: HARM_PASS(6, 0, 6) break;
+    case 7: HARM_PASS(7, 0, 7) break;
     case 8: HARM_PASS(8, 0, 2) HARM_PASS(8, 3, 8) break;
-    case 9: HARM_PASS(9, 0, 2) HARM_PASS(9, 3, 5) HARM_PASS(9, 6, 9) break;
-    case 10: HARM_PASS(10, 0, 1) HARM_PASS(10, 2, 4) HARM_PASS(10, 5, 10) break;
+    case 9: HARM_PASS(9, 0, 3) HARM_PASS(9, 4, 9) break;
+    case 10: HARM_PASS(10, 0, 3) HARM_PASS(10, 4, 10) break;
     default: return cudaErrorInvalidValue;
     }
     return cudaSuccess;
