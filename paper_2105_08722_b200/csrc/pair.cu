@@ -31,6 +31,9 @@
 namespace {
 
 constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes) per (bin, lane); see the append/flush notes
+#ifndef ENCORE_HARM_DEPTH
+#define ENCORE_HARM_DEPTH 2
+#endif
 constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
@@ -570,7 +573,8 @@ __device__ __forceinline__ Raw gather(const double4 *__restrict__ pos4, unsigned
 
 // MODE 0: open geometry; 1: periodic, image carried by the entry; 2: periodic, image decided per pair
 // mtab (MODE 1): shared memory [axis][image code][thread] = x_i + {-L, 0, +L}: x_j - (x_i -/+ L) is the minimal image
-template <int LMAX, int MLO, int MHI, int MODE>
+// D: candidates gathered ahead of the one being accumulated (2 at 12 warps/SM, 4 in the fat passes at 8 warps/SM)
+template <int LMAX, int MLO, int MHI, int MODE, int D>
 __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ pool,
                                           const int *__restrict__ page_next, int page, int nblk_lane, int nblk,
                                           const double4 *__restrict__ pos4, const double4 &me, const double *mtab,
@@ -584,7 +588,12 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
         q0 = __ldcg(p); q1 = __ldcg(p + 1);
         if (nblk_lane > 8) nextp = page_next[page];
     }
-    Raw r0 = gather(pos4, q0.x), r1 = gather(pos4, q0.y);
+    Raw r[D];
+    {
+        const unsigned e0[4] = {q0.x, q0.y, q0.z, q0.w};
+#pragma unroll
+        for (int d = 0; d < D; ++d) r[d] = gather(pos4, e0[d]);
+    }
     for (int kb = 0; kb < nblk; ++kb) {
         uint4 n0 = padv, n1 = padv; // entries of block kb+1
         if (kb + 1 < nblk_lane) {
@@ -594,10 +603,11 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
             n0 = __ldcg(p); n1 = __ldcg(p + 1);
             if (turn && kb + 9 < nblk_lane) nextp = page_next[page];
         }
-        const unsigned e[10] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, n0.x, n0.y};
+        const unsigned e[12] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, n0.x, n0.y, n0.z, n0.w};
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const Raw r2 = gather(pos4, e[u + 2]); // two candidates ahead
+            const Raw r0 = r[u % D];
+            r[u % D] = gather(pos4, e[u + D]); // D candidates ahead
             const unsigned en = e[u];
             double dx, dy, dz;
             if (MODE == 1) {
@@ -616,7 +626,6 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
             const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
             const double rinv = rsqrt_pair(r2s);
             accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
-            r0 = r1; r1 = r2;
         }
         q0 = n0; q1 = n1;
     }
@@ -625,7 +634,7 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
 template <int LMAX, int MLO, int MHI, bool PERIODIC>
 __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > 44 ? 2 : 3) k_harm(PairArgs a, int g0, int g1)
 {
-    constexpr int NACC = ncomp_range(LMAX, MLO, MHI);
+    constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > 44 ? 4 : ENCORE_HARM_DEPTH;
     __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
@@ -644,7 +653,7 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, 0.0, 0.0);
+    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, 0.0, 0.0);
     else if (gr.fast) {
         double *mt = mtab + threadIdx.x;
         const double L = a.geom.box;
@@ -652,8 +661,8 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
         mt[3 * kHarmWarps * 32] = me.y - L; mt[4 * kHarmWarps * 32] = me.y; mt[5 * kHarmWarps * 32] = me.y + L;
         mt[6 * kHarmWarps * 32] = me.z - L; mt[7 * kHarmWarps * 32] = me.z; mt[8 * kHarmWarps * 32] = me.z + L;
         __syncwarp();
-        harm_rows<LMAX, MLO, MHI, 1>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, mt, L, a.geom.half);
-    } else harm_rows<LMAX, MLO, MHI, 2>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, a.geom.box, a.geom.half);
+        harm_rows<LMAX, MLO, MHI, 1, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, mt, L, a.geom.half);
+    } else harm_rows<LMAX, MLO, MHI, 2, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, a.geom.box, a.geom.half);
 
     // epilogue: a_lm = (1/v_b) sum_k ycoef[c][k] S_{m,k}, k = l-m, l-m-2, ... (p_lm has the parity of l-m)
     const double vinv = a.bins.vinv[bin];
