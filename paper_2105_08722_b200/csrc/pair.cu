@@ -32,7 +32,13 @@ namespace {
 
 constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes) per (bin, lane); see the append/flush notes
 #ifndef ENCORE_HARM_DEPTH
-#define ENCORE_HARM_DEPTH 2
+#define ENCORE_HARM_DEPTH 4
+#endif
+#ifndef ENCORE_HARM_DEPTH_FAT
+#define ENCORE_HARM_DEPTH_FAT 4
+#endif
+#ifndef ENCORE_HARM_FAT
+#define ENCORE_HARM_FAT 44      // passes with more accumulators run at 8 warps/SM and 255 registers
 #endif
 constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
@@ -632,9 +638,9 @@ __device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, M
 }
 
 template <int LMAX, int MLO, int MHI, bool PERIODIC>
-__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > 44 ? 2 : 3) k_harm(PairArgs a, int g0, int g1)
+__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3) k_harm(PairArgs a, int g0, int g1)
 {
-    constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > 44 ? 4 : ENCORE_HARM_DEPTH;
+    constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH;
     __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
