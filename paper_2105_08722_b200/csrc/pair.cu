@@ -408,12 +408,13 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     // fp32, then culled against the group's bounding box (distance to the box > r_max: no primary of the group can
     // accept it) and the survivors are compacted into a 64-entry ring in shared memory (.w = list entry).  The pair
     // tests below always run on 32 queued candidates, so their cost follows the culled candidate count.
+    // a lane asks for s = lane, 32 + lane, 64 + lane, ...: its run index only moves forward
+    int run_lo = 0; // rng_off[run_lo] <= s < rng_off[run_lo + 1] once advanced (empty runs are stepped over)
     auto load_cand = [&](int s, double4 &cj, unsigned &j) {
         j = kPadEntry;
         if (s < T) {
-            int lo = 0, hi = nr; // rng_off[lo] <= s < rng_off[hi]
-            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (rng_off[mid] <= s) lo = mid; else hi = mid; }
-            j = (unsigned)(rng_start[lo] + (s - rng_off[lo]));
+            while (rng_off[run_lo + 1] <= s) ++run_lo; // s < T = rng_off[nr] bounds the walk
+            j = (unsigned)(rng_start[run_lo] + (s - rng_off[run_lo]));
             cj = a.pos4[j];
         }
     };
@@ -499,7 +500,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                     // v in [kMagic, kMagic + nb) <=> uh rounds into 0..nb-1 (float bits are monotonic)
                     code[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
                     ok[cc] = sure && code[cc] < (unsigned)nb;
-                    am[cc] = !sure && code[cc] + 1u < (unsigned)nb + 2u;
+                    am[cc] = !sure;                                  // ~2 du of all pairs, in range or not
                     ent[cc] = __float_as_uint(q.w);
                 }
                 if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
@@ -514,7 +515,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 #pragma unroll
                     for (int cc = 0; cc < 4; ++cc) {
                         if (ok[cc]) append(code[cc], ent[cc], cc & 1);
-                        else if (am[cc] && ent[cc] != kPadEntry) {
+                        else if (am[cc] && code[cc] + 1u < (unsigned)nb + 2u && ent[cc] != kPadEntry) {
                             const unsigned cx = classify_exact<PERIODIC>(a.pos4[ent[cc] & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
                             if (cx != kNoHit) append(cx, ent[cc], cc & 1);
                         }
