@@ -38,8 +38,8 @@ import workloads as W  # noqa: E402
 
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of k_fill + k_harm per step, from the committed `ncu --set full` capture
-# profiles/r1_v6_ncu_full.txt (an ALU-bound stage: the traffic is the candidate lists written and read back once)
-NCU_PAIR_STAGE_DRAM_BYTES = {"c3": 19.59e9}
+# profiles/r1_v7_ncu_full.txt (an ALU-bound stage: the traffic is the candidate lists written and read back once)
+NCU_PAIR_STAGE_DRAM_BYTES = {"c3": 19.65e9}
 
 
 def peaks():
