@@ -24,7 +24,7 @@ OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -56,6 +56,7 @@ def lib():
     L.encore_compute_host.argtypes = [vp, vp, vp, C.c_int64, vp]
     L.encore_compute_shard.argtypes = [vp, vp, vp, C.c_int64, C.c_int, C.c_int, vp, vp]
     L.encore_get_shard_groups.argtypes = [vp, ip]
+    L.encore_get_pair_steps.argtypes = [vp]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
     L.encore_zeta_len.restype = C.c_int64
@@ -136,6 +137,13 @@ def encore_get_shard_groups(plan):
     out = (C.c_int * 3)()
     _check(lib().encore_get_shard_groups(plan, out))
     return int(out[0]), int(out[1]), int(out[2])
+
+
+def encore_get_pair_steps(plan) -> int:
+    v = lib().encore_get_pair_steps(plan)
+    if v < 0:
+        _check(v)
+    return int(v)
 
 
 def encore_compute_host(plan, positions, weights, n: int, zeta_out):

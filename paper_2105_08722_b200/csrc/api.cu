@@ -428,6 +428,13 @@ int encore_compute_shard(encore_plan_t *P, const double *positions, const double
     return compute_device(P, positions, weights, n, zeta_partial_out, static_cast<cudaStream_t>(cuda_stream), shard, nshards);
 }
 
+int encore_get_pair_steps(const encore_plan_t *P)
+{
+    if (!P) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    return P->pair_steps;
+}
+
 int encore_get_multiplet_parity(const encore_plan_t *P, int *out)
 {
     if (!P || !out) return ENCORE_EINVAL;

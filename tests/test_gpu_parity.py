@@ -299,3 +299,28 @@ def test_allparity_matches_the_oracle(E, oracle, order, nbins, lmax, box):
     assert np.abs(np.where(par[:, None], o["zeta"], o["zeta_im"])).max() <= 1e-12 * scale
     assert np.abs(z - expect).max() <= TOL * scale
     assert np.abs(expect[par]).max() > 1e-6 * scale if order > 3 else True   # the odd part is not trivially zero
+
+
+def test_list_budget_super_steps(E, oracle, monkeypatch):
+    """a 1 MB list budget forces the pair stage through many super-steps: same bits as the single-step run"""
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=7000, grid=64)
+    pos, w = W.make(cfg)
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    out = {}
+    for tag, mb in [("one", None), ("many", "1")]:
+        if mb is None:
+            monkeypatch.delenv("ENCORE_LIST_MB", raising=False)
+        else:
+            monkeypatch.setenv("ENCORE_LIST_MB", mb)
+        with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+            z = plan.compute(tp, tw)
+            torch.cuda.synchronize()
+            counts, pairs = E.encore_get_bin_counts(plan.h, cfg.nbins)
+            out[tag] = (z.cpu().numpy(), counts, E.encore_get_pair_steps(plan.h))
+    assert out["one"][2] == 1 and out["many"][2] > 3
+    assert out["one"][0].tobytes() == out["many"][0].tobytes()
+    assert (out["one"][1] == out["many"][1]).all()
+    o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+    assert (out["many"][1] == o["bin_counts"]).all()
+    assert np.abs(out["many"][0] - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
