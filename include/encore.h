@@ -101,7 +101,8 @@ int encore_compute_host(encore_plan_t *plan, const double *positions, const doub
 int encore_compute_shard(encore_plan_t *plan, const double *positions, const double *weights, int64_t n, int shard,
                          int nshards, double *zeta_partial_out, void *cuda_stream);
 /* super-steps the pair stage of the last compute took: the candidate lists of a step stay under the byte budget
- * ENCORE_LIST_MB (environment, read by encore_plan; default 32768), whole groups per step.  >= 1, or a status < 0. */
+ * ENCORE_LIST_MB (environment, read by encore_plan; default: half of the free device memory, 4-96 GB), whole groups
+ * per step, steps of equal size.  >= 1, or a status < 0. */
 int encore_get_pair_steps(const encore_plan_t *plan);
 /* groups of the last compute: out = {first group, one past the last group, number of groups} (HOST) */
 int encore_get_shard_groups(const encore_plan_t *plan, int out[3]);
