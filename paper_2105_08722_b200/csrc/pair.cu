@@ -40,7 +40,10 @@ constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes)
 #ifndef ENCORE_HARM_FAT
 #define ENCORE_HARM_FAT 44      // passes with more accumulators run at 8 warps/SM and 255 registers
 #endif
-constexpr int kHarmWarps = 4;       // k_harm: independent warps (items) per CTA
+#ifndef ENCORE_HARM_WARPS
+#define ENCORE_HARM_WARPS 4
+#endif
+constexpr int kHarmWarps = ENCORE_HARM_WARPS;       // k_harm: independent warps (items) per CTA
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
 constexpr unsigned kPadEntry = 0xffffffffu;
