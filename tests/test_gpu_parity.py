@@ -121,14 +121,15 @@ def test_small_clouds_open_and_periodic(E, oracle, order, nbins, lmax):
     check_full(E, oracle, order, pos, w, 90.0, 4.0, 44.0, nbins, lmax)
 
 
-@pytest.mark.parametrize("order,nbins", [(4, 4), (4, 5), (4, 6), (4, 7), (4, 8), (4, 9), (4, 11), (5, 6), (5, 7), (5, 9)])
+@pytest.mark.parametrize("order,nbins", [(3, 6), (3, 7), (3, 8), (3, 9), (3, 12), (4, 4), (4, 5), (4, 6), (4, 7), (4, 8), (4, 9), (4, 11),
+                                         (5, 6), (5, 7), (5, 9)])
 def test_every_bin_count_of_the_factorised_contraction(E, oracle, order, nbins):
-    """one case per template instantiation of the N=4 / N=5 contraction kernels (and the generic fallback above them)"""
+    """one case per template instantiation of the N=3 / N=4 / N=5 contraction kernels (and the generic fallback above them)"""
     rng = np.random.default_rng(7000 + 20 * order + nbins)
     n = 150
     pos = np.ascontiguousarray(rng.uniform(0, 60.0, (3, n)))
     w = rng.uniform(0.5, 1.5, n)
-    check_full(E, oracle, order, pos, w, 0.0, 3.0, 40.0, nbins, 2 if order == 4 else 1, alm_samples=(3,))
+    check_full(E, oracle, order, pos, w, 0.0, 3.0, 40.0, nbins, {3: 3, 4: 2, 5: 1}[order], alm_samples=(3,))
 
 
 def test_degenerate_inputs(E, oracle):
