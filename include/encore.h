@@ -48,7 +48,8 @@ enum {
     ENCORE_EALLOC = -3,   /* host or device allocation failed */
     ENCORE_ECUDA = -4,    /* a CUDA call failed; encore_last_cuda_error() has the cudaError_t */
     ENCORE_ESTATE = -5,   /* diagnostic getter called before a successful encore_compute */
-    ENCORE_EUNSUPPORTED = -6 /* valid problem outside what this build's kernels cover (see encore_plan) */
+    ENCORE_EUNSUPPORTED = -6, /* valid problem outside what this build's kernels cover (see encore_plan) */
+    ENCORE_EINTERNAL = -7  /* a device-side consistency check failed; results must not be used (encore_get_status) */
 };
 
 /* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
@@ -100,9 +101,21 @@ int encore_compute_host(encore_plan_t *plan, const double *positions, const doub
  * nshards = 1 is encore_compute.  Errors as encore_compute, plus ENCORE_EINVAL for shard outside [0, nshards). */
 int encore_compute_shard(encore_plan_t *plan, const double *positions, const double *weights, int64_t n, int shard,
                          int nshards, double *zeta_partial_out, void *cuda_stream);
-/* super-steps the pair stage of the last compute took: the candidate lists of a step stay under the byte budget
- * ENCORE_LIST_MB (environment, read by encore_plan; default: half of the free device memory, 4-96 GB), whole groups
- * per step, steps of equal size.  >= 1, or a status < 0. */
+/* Plan options (host call, takes effect at the next encore_compute).  No behaviour is read from the environment.
+ *   "list_mb"          byte budget, in MiB, of the pair stage's acceptance-mask rows per super-step (0 = default:
+ *                      32 GiB, or half of the free device memory within 4-96 GiB when the rows need more)
+ *   "sub_yz", "sub_x"  grid subdivisions S_y = S_z and S_x of reading R11 (cell size r_max / S; 0 = automatic:
+ *                      S_y = clamp(round(r_max / (32 / density)^(1/3)), 1, 8), S_x = 4 S_y halved until <= 4e6 cells)
+ *   "generic_contract" 1: contract with the literal eq. 44 kernel (one warp per (Lambda, B)) instead of the
+ *                      factorised kernels
+ * Unknown key or value out of range: ENCORE_EINVAL. */
+int encore_set_option(encore_plan_t *plan, const char *key, long long value);
+/* Synchronises the last compute's stream and reports its device-side status: ENCORE_OK, or ENCORE_EINTERNAL if the
+ * pair stage's consistency check (one periodic image per candidate word) failed.  encore_compute_host
+ * returns this status itself. */
+int encore_get_status(const encore_plan_t *plan);
+/* super-steps the pair stage of the last compute took: the acceptance-mask rows of a step stay under the byte budget
+ * (option "list_mb"), whole groups per step, steps of equal size.  >= 1, or a status < 0. */
 int encore_get_pair_steps(const encore_plan_t *plan);
 /* groups of the last compute: out = {first group, one past the last group, number of groups} (HOST) */
 int encore_get_shard_groups(const encore_plan_t *plan, int out[3]);

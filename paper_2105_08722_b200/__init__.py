@@ -20,11 +20,11 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
-OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL = 0, -1, -2, -3, -4, -5, -6, -7
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -57,6 +57,8 @@ def lib():
     L.encore_compute_shard.argtypes = [vp, vp, vp, C.c_int64, C.c_int, C.c_int, vp, vp]
     L.encore_get_shard_groups.argtypes = [vp, ip]
     L.encore_get_pair_steps.argtypes = [vp]
+    L.encore_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
+    L.encore_get_status.argtypes = [vp]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
     L.encore_zeta_len.restype = C.c_int64
@@ -144,6 +146,14 @@ def encore_get_pair_steps(plan) -> int:
     if v < 0:
         _check(v)
     return int(v)
+
+
+def encore_set_option(plan, key: str, value: int):
+    _check(lib().encore_set_option(plan, key.encode(), int(value)))
+
+
+def encore_get_status(plan) -> int:
+    return int(lib().encore_get_status(plan))
 
 
 def encore_compute_host(plan, positions, weights, n: int, zeta_out):

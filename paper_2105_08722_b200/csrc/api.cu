@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 
 namespace {
 
@@ -39,13 +40,13 @@ struct encore_plan_s {
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
     DevBuf io_pos, io_w, io_zeta;
-    DevBuf gbound, gprefix, pool, pool_cursor, page_next, first_page;
+    DevBuf gbound, gprefix, gwide, rows, rowdesc, rowcnt, errflag;
     int *h_gprefix = nullptr;   // pinned
     size_t h_gprefix_cap = 0;
     size_t list_budget_bytes = (size_t)32 << 30;
-    bool list_budget_env = false;   // ENCORE_LIST_MB given: use it as is
+    bool list_budget_set = false;   // option "list_mb" given: use it as is
     int pair_steps = 0;
-    double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6]
+    double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6], internal-error flag as int in [7]
     // state of the last compute
     bool have = false;
     int64_t n = 0;
@@ -125,7 +126,7 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
 // DESIGN.md R11.  Per axis: h_a = r_max / sub_a, nc_a = max(1, floor(ext_a / h_a)), inv_a = nc_a / ext_a.
 // sub_y = sub_z chosen so that a pencil cross-section holds ~32 particles per pencil-width of length;
 // x is subdivided 4x finer (x-ranges of candidate pencils are culled at that granularity).
-void choose_geometry(const encore_plan_s *P, int64_t n, const double lo[3], const double hi[3], GridGeom &G)
+bool choose_geometry(const encore_plan_s *P, int64_t n, const double lo[3], const double hi[3], GridGeom &G)
 {
     const HostTables &T = P->T;
     double ext[3];
@@ -144,21 +145,27 @@ void choose_geometry(const encore_plan_s *P, int64_t n, const double lo[3], cons
     if (P->sub_yz_override > 0) syz = std::min(8, P->sub_yz_override);
     int sx = 4 * syz;
     if (P->sub_x_override > 0) sx = P->sub_x_override;
+    double cells = 0.0;
     for (;;) {
         G.sub[0] = sx; G.sub[1] = syz; G.sub[2] = syz;
-        double cells = 1.0;
+        cells = 1.0;
         for (int a = 0; a < 3; ++a) {
             const double h = T.rmax / (double)G.sub[a];
             const double q = std::floor(ext[a] / h);
             G.nc[a] = q < 1.0 ? 1 : (q > 1e9 ? 1000000000 : (int)q);
             G.inv[a] = ext[a] > 0.0 ? (double)G.nc[a] / ext[a] : 1.0;
+            // an axis thinner than one cell (nc = 1, e.g. a planar catalogue with noise in z): every particle is in
+            // cell 0 whatever inv is; keep inv <= 1/h so that r_max * inv stays a small number of cells
+            if (G.nc[a] == 1 && G.inv[a] > 1.0 / h) G.inv[a] = 1.0 / h;
             cells *= (double)G.nc[a];
         }
         if (cells <= 4.0e6 || sx == 1) break;
         sx = std::max(1, sx / 2);
     }
+    if (cells > 4.0e6) return false;    // box / r_max beyond what the cell tables are sized for
     G.ncell = G.nc[0] * G.nc[1] * G.nc[2];
     G.npencil = G.nc[1] * G.nc[2];
+    return true;
 }
 
 int record(encore_plan_s *P, int k, cudaStream_t s)
@@ -196,10 +203,11 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     std::memcpy(fl, P->pinned + 6, sizeof(fl));
     if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
     GridGeom G;
-    choose_geometry(P, n, P->pinned, P->pinned + 3, G);
+    if (!choose_geometry(P, n, P->pinned, P->pinned + 3, G)) return ENCORE_EUNSUPPORTED;
     int nr_cap;
     {
-        int Ry = (int)std::floor(T.rmax * G.inv[1] + 1e-6) + 1, Rz = (int)std::floor(T.rmax * G.inv[2] + 1e-6) + 1;
+        // inv <= sub / r_max (choose_geometry), so these are at most sub + 1 cells
+        int Ry = (int)std::floor(std::min(T.rmax * G.inv[1], 1e6) + 1e-6) + 1, Rz = (int)std::floor(std::min(T.rmax * G.inv[2], 1e6) + 1e-6) + 1;
         if (!G.periodic) { Ry = std::min(Ry, G.nc[1] - 1); Rz = std::min(Rz, G.nc[2] - 1); }
         const int wy = std::min(2 * Ry + 1, G.periodic ? G.nc[1] : 2 * Ry + 1);
         const int wz = std::min(2 * Rz + 1, G.periodic ? G.nc[2] : 2 * Rz + 1);
@@ -216,7 +224,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->cell_count.ensure(sizeof(int) * (size_t)G.ncell));
     CU(P->cell_fill.ensure(sizeof(int) * (size_t)G.ncell));
     CU(P->cell_start.ensure(sizeof(int) * ((size_t)G.ncell + 1)));
-    CU(P->scan_tmp.ensure(sizeof(int) * (std::max<size_t>((size_t)G.ncell, 4000000) / 2048 + 8)));
+    CU(P->scan_tmp.ensure(sizeof(int) * (std::max<size_t>(std::max<size_t>((size_t)G.ncell, (size_t)ngmax), 4000000) / 2048 + 8)));
     CU(P->tmp_idx.ensure(sizeof(int) * n));
     CU(P->sorted_idx.ensure(sizeof(int) * n));
     CU(P->pos4.ensure(sizeof(double4) * n));
@@ -279,14 +287,15 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.ngroups = ngmax;
     CU(P->gbound.ensure(sizeof(int) * (size_t)ngmax));
     CU(P->gprefix.ensure(sizeof(int) * ((size_t)ngmax + 2)));
-    CU(P->first_page.ensure(sizeof(int) * (size_t)ngmax * nb * 32));
-    CU(P->pool_cursor.ensure(sizeof(unsigned) * 2));
+    CU(P->gwide.ensure(sizeof(int) * (size_t)ngmax));
+    CU(P->rowcnt.ensure(sizeof(int) * (size_t)ngmax * nb));
+    CU(P->errflag.ensure(sizeof(int)));
     pa.gbound = P->gbound.as<int>();
     pa.gprefix = P->gprefix.as<int>();
+    pa.gwide = P->gwide.as<int>();
     pa.scan_tmp = P->scan_tmp.as<int>();
-    pa.first_page = P->first_page.as<int>();
-    pa.pool_cursor = P->pool_cursor.as<unsigned>();
-    pa.err_flag = reinterpret_cast<int *>(P->pool_cursor.as<unsigned>() + 1);
+    pa.rowcnt = P->rowcnt.as<int>();
+    pa.err_flag = P->errflag.as<int>();
     if (P->h_gprefix_cap < (size_t)ngmax + 2) {
         if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
         P->h_gprefix = nullptr; P->h_gprefix_cap = 0;
@@ -295,39 +304,37 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     }
     int g_begin = 0, g_end = 0, ngroups_total = 0;
     CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
-    CU(cudaMemsetAsync(P->pool_cursor.p, 0, 2 * sizeof(unsigned), s));
+    CU(cudaMemsetAsync(P->errflag.p, 0, sizeof(int), s));
     CU(launch_pair_bounds(pa, s, &P->launches));
-    // second small device->host read: slab bounds per group (prefix) and the number of groups -> super-steps
+    // second small device->host read: candidate words per group (prefix) and the number of groups -> super-steps
     CU(cudaMemcpyAsync(P->h_gprefix, P->gprefix.p, sizeof(int) * ((size_t)ngmax + 1), cudaMemcpyDeviceToHost, s));
     CU(cudaMemcpyAsync(P->h_gprefix + ngmax + 1, P->group_start.as<int>() + G.npencil, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     {
         const int ngroups = P->h_gprefix[ngmax + 1];
         const int *gp = P->h_gprefix;
-        const size_t slab_bytes = (size_t)ENCORE_SLAB_PAGES * ENCORE_PAGE_WORDS * sizeof(unsigned);
-        const size_t total_slabs = (size_t)gp[ngroups];
-        // byte budget of the candidate lists of one super-step: ENCORE_LIST_MB if set, else half of what the device
-        // has free (counting the pool this plan already owns), between 4 GB and 96 GB: fewer, longer steps are
-        // faster (every step ends with a partly filled last wave; c4: 8 steps 370 ms, 4 steps 351 ms, 2 steps 342 ms)
+        // a word of a group owns one 128-byte row and one descriptor in each of the nb bin streams
+        const size_t word_bytes = (size_t)nb * (32 + 1) * sizeof(unsigned);
+        const size_t total_words = (size_t)gp[ngroups];
+        // byte budget of the rows of one super-step: option "list_mb" if set, else 32 GB, or - when the rows do not fit
+        // that - half of what the device has free (counting the buffer this plan already owns), between 4 GB and
+        // 96 GB: fewer, longer steps are faster (every step ends with a partly filled last wave)
         size_t budget_bytes = P->list_budget_bytes;
-        if (!P->list_budget_env && total_slabs * (slab_bytes + ENCORE_SLAB_PAGES * sizeof(int)) > budget_bytes) {
-            size_t free_b = 0, total_b = 0; // (asked only when the lists do not fit the 32 GB default)
+        if (!P->list_budget_set && total_words * word_bytes > budget_bytes) {
+            size_t free_b = 0, total_b = 0;
             if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
-                const size_t avail = free_b + P->pool.cap + P->page_next.cap;
+                const size_t avail = free_b + P->rows.cap + P->rowdesc.cap;
                 budget_bytes = std::min<size_t>(std::max<size_t>(avail / 2, (size_t)4 << 30), (size_t)96 << 30);
             }
         }
-        const size_t budget_slabs = std::max<size_t>(budget_bytes / (slab_bytes + ENCORE_SLAB_PAGES * sizeof(int)), 1);
-        size_t max_group_slabs = 0;
-        for (int g = 0; g < ngroups; ++g) max_group_slabs = std::max(max_group_slabs, (size_t)(gp[g + 1] - gp[g]));
-        const size_t cap_slabs = std::max(std::min(total_slabs, budget_slabs), std::max<size_t>(max_group_slabs, 1));
-        const size_t cap_pages = cap_slabs * ENCORE_SLAB_PAGES;
-        if (cap_pages >= ((size_t)1 << 31)) return ENCORE_EUNSUPPORTED;
-        CU(P->pool.ensure(cap_slabs * slab_bytes));
-        CU(P->page_next.ensure(cap_pages * sizeof(int)));
-        pa.pool = P->pool.as<unsigned>();
-        pa.pool_pages = (unsigned)cap_pages;
-        pa.page_next = P->page_next.as<int>();
+        const size_t budget_words = std::max<size_t>(budget_bytes / word_bytes, 1);
+        size_t max_group_words = 0;
+        for (int g = 0; g < ngroups; ++g) max_group_words = std::max(max_group_words, (size_t)(gp[g + 1] - gp[g]));
+        const size_t cap_words = std::max(std::min(total_words, budget_words), std::max<size_t>(max_group_words, 1));
+        CU(P->rows.ensure(cap_words * nb * 32 * sizeof(unsigned)));
+        CU(P->rowdesc.ensure(cap_words * nb * sizeof(unsigned)));
+        pa.rows = P->rows.as<unsigned>();
+        pa.rowdesc = P->rowdesc.as<unsigned>();
         pa.ngroups = ngroups;
         ngroups_total = ngroups;
         P->pair_steps = 0;
@@ -335,24 +342,26 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         auto cut = [&](int k) {
             if (k <= 0) return 0;
             if (k >= nshards) return ngroups;
-            const long long want = ((long long)total_slabs * k + nshards - 1) / nshards;
+            const long long want = ((long long)total_words * k + nshards - 1) / nshards;
             return (int)(std::lower_bound(gp, gp + ngroups + 1, want, [](int v, long long t) { return (long long)v < t; }) - gp);
         };
         g_begin = cut(shard); g_end = std::max(g_begin, std::min(ngroups, cut(shard + 1)));
         if (nshards > 1) CU(cudaMemsetAsync(P->counts.p, 0, sizeof(uint32_t) * (size_t)ngroups * nb * 32, s));
         // super-steps of whole groups, evenly sized (a short last step would run at a few percent occupancy)
-        const size_t range_slabs = (size_t)(gp[g_end] - gp[g_begin]);
-        const size_t nsteps = std::max<size_t>((range_slabs + cap_slabs - 1) / cap_slabs, 1);
-        const size_t step_slabs = std::min(cap_slabs, std::max((range_slabs + nsteps - 1) / nsteps, std::max<size_t>(max_group_slabs, 1)));
+        const size_t range_words = (size_t)(gp[g_end] - gp[g_begin]);
+        const size_t nsteps = std::max<size_t>((range_words + cap_words - 1) / cap_words, 1);
+        const size_t step_words = std::min(cap_words, std::max((range_words + nsteps - 1) / nsteps, std::max<size_t>(max_group_words, 1)));
         int g0 = g_begin;
         while (g0 < g_end) {
             int g1 = g0 + 1;
-            while (g1 < g_end && (size_t)(gp[g1 + 1] - gp[g0]) <= step_slabs) ++g1;
+            while (g1 < g_end && (size_t)(gp[g1 + 1] - gp[g0]) <= step_words) ++g1;
             CU(launch_pair_fill_harmonics(pa, g0, g1, nr_cap, s, &P->launches));
             ++P->pair_steps;
             g0 = g1;
         }
     }
+    // internal-consistency flag of the pair stage, read by whoever synchronises next (encore_get_status, the getters)
+    CU(cudaMemcpyAsync(reinterpret_cast<int *>(P->pinned + 7), P->errflag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
     TRY(record(P, 3, s));
     // ---- a5: contraction ---------------------------------------------------------------------------------------
     ContractArgs ca{};
@@ -422,10 +431,6 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
         delete P;
         return ENCORE_EALLOC;
     }
-    if (const char *e = std::getenv("ENCORE_SUB_YZ")) P->sub_yz_override = std::atoi(e);
-    if (const char *e = std::getenv("ENCORE_SUB_X")) P->sub_x_override = std::atoi(e);
-    if (const char *e = std::getenv("ENCORE_GENERIC_CONTRACT")) P->force_generic = std::atoi(e) != 0;
-    if (const char *e = std::getenv("ENCORE_LIST_MB")) { P->list_budget_bytes = (size_t)std::max(1, std::atoi(e)) << 20; P->list_budget_env = true; }
     *plan_out = P;
     return ENCORE_OK;
 }
@@ -442,6 +447,37 @@ int encore_compute_shard(encore_plan_t *P, const double *positions, const double
     if (!P || !positions || !zeta_partial_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
     if (nshards < 1 || shard < 0 || shard >= nshards) return ENCORE_EINVAL;
     return compute_device(P, positions, weights, n, zeta_partial_out, static_cast<cudaStream_t>(cuda_stream), shard, nshards);
+}
+
+int encore_set_option(encore_plan_t *P, const char *key, long long value)
+{
+    if (!P || !key) return ENCORE_EINVAL;
+    const std::string k(key);
+    if (k == "list_mb") {           // byte budget of the acceptance-mask rows of one pair-stage super-step, in MiB; 0: default
+        if (value < 0) return ENCORE_EINVAL;
+        P->list_budget_set = value > 0;
+        P->list_budget_bytes = value > 0 ? (size_t)value << 20 : (size_t)32 << 30;
+    } else if (k == "sub_yz") {     // grid subdivision S_y = S_z (cell size r_max / S); 0: automatic
+        if (value < 0 || value > 8) return ENCORE_EINVAL;
+        P->sub_yz_override = (int)value;
+    } else if (k == "sub_x") {      // grid subdivision S_x; 0: 4 S_y
+        if (value < 0 || value > 32) return ENCORE_EINVAL;
+        P->sub_x_override = (int)value;
+    } else if (k == "generic_contract") { // 1: run the literal eq. 44 kernel instead of the factorised ones
+        if (value < 0 || value > 1) return ENCORE_EINVAL;
+        P->force_generic = value != 0;
+    } else return ENCORE_EINVAL;
+    return ENCORE_OK;
+}
+
+int encore_get_status(const encore_plan_t *P)
+{
+    if (!P) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    CU(cudaStreamSynchronize(P->stream));
+    int f = 0;
+    std::memcpy(&f, P->pinned + 7, sizeof(int));
+    return f ? ENCORE_EINTERNAL : ENCORE_OK;
 }
 
 int encore_get_pair_steps(const encore_plan_t *P)
@@ -479,7 +515,7 @@ int encore_compute_host(encore_plan_t *P, const double *positions, const double 
     TRY(compute_device(P, P->io_pos.as<double>(), weights ? P->io_w.as<double>() : nullptr, n, P->io_zeta.as<double>(), s));
     CU(cudaMemcpyAsync(zeta_out, P->io_zeta.p, sizeof(double) * nout, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
-    return ENCORE_OK;
+    return encore_get_status(P);
 }
 
 int encore_destroy(encore_plan_t *P)
@@ -489,8 +525,8 @@ int encore_destroy(encore_plan_t *P)
                       &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
-                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->pool,
-                      &P->pool_cursor, &P->page_next, &P->first_page};
+                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->gwide,
+                      &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
@@ -702,6 +738,7 @@ const char *encore_strerror(int status)
     case ENCORE_ECUDA: return cudaGetErrorString((cudaError_t)g_last_cuda);
     case ENCORE_ESTATE: return "no successful encore_compute to report on (or timing disabled)";
     case ENCORE_EUNSUPPORTED: return "configuration not covered by this build's kernels";
+    case ENCORE_EINTERNAL: return "internal consistency check of the pair stage failed (please report)";
     default: return "unknown status";
     }
 }

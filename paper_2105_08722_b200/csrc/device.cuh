@@ -63,20 +63,20 @@ struct PairArgs {
     unsigned long long *cand_pairs; // candidate pairs tested (diagnostic)
     double *gweights;           // [ngroups][32] weight of (group, lane), 0 for empty lanes
     int ngroups;                // upper bound n/32 + npencil + 1 before the bounds are read back; exact afterwards
-    // candidate lists: one list per (group, bin, lane) = chain of 256-byte pages of `pool`
-    int *gbound;                // [ngroups]   upper bound on the pool slabs a group can take
+    // acceptance-mask rows: per (group, bin) a stream of 128-byte rows, one 32-bit mask per primary,
+    // each row covering one word of 32 consecutive sorted candidates named by its descriptor
+    int *gbound;                // [ngroups]   candidate words of a group = row capacity of each of its bins
     int *gprefix;               // [ngroups+1] exclusive scan of gbound
+    int *gwide;                 // [ngroups]   1: a candidate run covers a whole periodic axis (exact path, no common image)
     int *scan_tmp;
-    unsigned *pool;             // [pool_pages][64] entries: sorted index | image codes << 26; 0xffffffff = padding
-    unsigned pool_pages;
-    unsigned *pool_cursor;      // next free page (advanced a slab at a time)
-    int *page_next;             // [pool_pages] next page of the same list
-    int *first_page;            // [ngroups][nbins][32] first page of the list of (group, bin, lane)
-    int *err_flag;              // set if the pool overflowed (excluded by the step bounds)
+    unsigned *rows;             // [(gprefix[g]-gprefix[g0]) * nbins + bin * words(g) + k][32] masks, lane = primary
+    unsigned *rowdesc;          // same index: first sorted index of the word | image codes << 26
+    int *rowcnt;                // [ngroups][nbins] rows written
+    int *err_flag;              // set if a word's candidates disagreed on the periodic image (excluded by DESIGN.md §5.3)
     int bin_order[ENCORE_MAX_BINS]; // bins by decreasing shell volume (work per item)
 };
-// per-group slab bounds -> gbound, gprefix (device).  The caller reads gprefix back, sizes the pool, and calls
-// launch_pair_fill_harmonics once per super-step [g0, g1); nr_cap >= number of candidate runs of a group.
+// per-group word counts -> gbound, gprefix, gwide (device).  The caller reads gprefix back, sizes the row buffer, and
+// calls launch_pair_fill_harmonics once per super-step [g0, g1); nr_cap >= number of candidate runs of a group.
 cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches);
 cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches);
 size_t pair_fill_smem_bytes(int nbins, int nr_cap);

@@ -7,30 +7,34 @@
 // the work is split by resource profile into two kernels around "groups" of 32 consecutive cell-sorted
 // primaries of one (iy,iz) pencil (lane = primary everywhere):
 //   k_fill  (a3, integer/fp32, few registers): ONE WARP per group.  Candidates = contiguous runs of the sorted
-//     array (one or two per neighbouring pencil, x-range culled against the group's cell range), read 32 at a time,
-//     made relative to primary 0 in fp32, culled against the bounding box of the group's primaries and compacted
-//     into a ring in shared memory, from where they are broadcast to the lanes.  A first fp32 evaluation
-//     decides every pair whose radius is farther than a proven error margin from all bin edges; the rest (~1e-4)
-//     is decided in fp64 exactly as DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so
-//     counts are bit-exact.  An accepted pair is appended, in candidate order, to the list of (primary, bin):
-//     lane-private cursors and one 4-entry block per (bin, lane) in shared memory, written 16 bytes at a time
-//     into 256-byte pages of a pool in HBM; pages of one list are chained through page_next[].
-//     The final cursors are n_i(b), the per-(primary, bin) pair counts (an integer output of the path).
-//   k_harm  (a4, fp64, ~166 registers): one warp per (group, bin); every lane streams its own list, gathers the
-//     candidates two rows ahead, and keeps the (lmax+1)^2 real accumulators of a^b_lm(s_i) in REGISTERS: no
-//     atomics, no cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit
-//     vector (fp32 rsqrt seed + one third-order fp64 step), w (x+iy)^m by complex recurrence, powers of z, one FMA
-//     per component into S_{m,k} = sum w z^k (x+iy)^m; the monic associated-Legendre polynomials p_lm(z) and the
-//     normalisation (-1)^m N_lm k_lm / v_b are applied once per (primary, bin) in the epilogue (table ycoef).
+//     array (one or two per neighbouring pencil, x-range culled against the group's cell range), cut into WORDS of
+//     32 consecutive sorted particles.  A word is read lane = candidate, made relative to primary 0 (periodic image)
+//     in fp32 and culled against the bounding box of the group's primaries; the survivors are broadcast from shared
+//     memory and every lane (= primary) tests them.  A first fp32 evaluation decides every pair whose radius is
+//     farther than a proven error margin from all bin edges; the rest (~1e-4) is decided in fp64 exactly as
+//     DESIGN.md R8-R10 fix it (r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) against e_b^2), so the binning is bit-exact.  The
+//     result of a word is one 32-bit acceptance mask per (bin, primary); for every bin with any bit set the warp
+//     writes ONE coalesced 128-byte ROW (32 masks, lane = primary) plus a one-word descriptor (first sorted index |
+//     image codes << 26) to the row stream of (group, bin), which sits at a fixed place (capacity = words of the
+//     group): no allocation, no lane-private list state, no atomics.
+//   k_harm  (a4, fp64, ~166 registers): one warp per (group, bin).  The rows are staged into shared memory with
+//     cp.async (two chunks of 16 rows in flight); every lane pushes its non-empty masks into a lane-private queue of
+//     (mask, descriptor) records in shared memory and walks their set bits, gathering the candidate four pairs ahead
+//     with one 256-bit load.  The (lmax+1)^2 real accumulators of a^b_lm(s_i) stay in REGISTERS: no atomics, no
+//     cross-lane reductions, summation order = candidate order -> deterministic.  Per pair: unit vector (fp32 rsqrt
+//     seed + one third-order fp64 step), w (x+iy)^m by complex recurrence, powers of z, one FMA per component into
+//     S_{m,k} = sum w z^k (x+iy)^m; the monic associated-Legendre polynomials p_lm(z) and the normalisation
+//     (-1)^m N_lm k_lm / v_b are applied once per (primary, bin) in the epilogue (table ycoef).  The number of set
+//     bits a lane walked is n_i(b), the per-(primary, bin) pair count (an integer output of the path).
 //     Items are ordered heaviest bin first so the grid drains evenly.
 #include "device.cuh"
 
 #include <algorithm>
 #include <climits>
+#include <mutex>
 
 namespace {
 
-constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes) per (bin, lane); see the append/flush notes
 #ifndef ENCORE_HARM_DEPTH
 #define ENCORE_HARM_DEPTH 4
 #endif
@@ -44,9 +48,10 @@ constexpr int kRing = 4;            // k_fill: one block of 4 entries (16 bytes)
 #define ENCORE_HARM_WARPS 4
 #endif
 constexpr int kHarmWarps = ENCORE_HARM_WARPS;       // k_harm: independent warps (items) per CTA
+constexpr int kQueue = 16;                          // k_harm: (mask, descriptor) records queued per lane
+constexpr int kStageRows = 16;                      // k_harm: rows per cp.async chunk (two chunks in flight)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
-constexpr unsigned kPadEntry = 0xffffffffu;
 constexpr unsigned kIdxMask = 0x3ffffffu;
 constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: (x + kMagic) - kMagic = round-to-nearest-integer(x)
 constexpr int kMagicBits = 0x4B400000;
@@ -157,11 +162,13 @@ __device__ __forceinline__ Group locate_group(const PairArgs &a, int g)
 }
 
 // ---- candidate ranges of a group (one warp): one or two runs of the sorted array per neighbouring pencil -----
-// STORE: rng_start[r] = first sorted index of run r, rng_off[r] = candidates before run r (rng_off[nr] = total).
-// Returns the number of candidates T of the group.
+// A run is cut into words of 32 consecutive sorted particles (the last word of a run may be partial).
+// STORE: rng_start[r] = first sorted index of run r, rng_len[r] = its length, rng_woff[r] = words before run r
+// (rng_woff[nr] = words of the group).  Returns the number of words W of the group.  *wide is set when a candidate
+// x-range covers the whole periodic axis (then no image is common to a run and the group takes the exact path).
 template <bool PERIODIC, bool STORE>
-__device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, int lane, int *rng_start, int *rng_off,
-                                            int *nr_out)
+__device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, int lane, int *rng_start, int *rng_len,
+                                            int *rng_woff, int *nr_out, bool *wide)
 {
     const GridGeom &G = a.geom;
     const int ncx = G.nc[0], ncy = G.nc[1], ncz = G.nc[2];
@@ -172,6 +179,7 @@ __device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, 
     const int nyz = wy * wz; // host guarantees 2*nyz <= nr_cap
     const double rmax2 = a.rmax * a.rmax;
     int mine = 0;
+    bool covers = full_y || full_z;
     for (int r = lane; r < nyz; r += 32) {
         const int iy = r % wy, iz = r / wy;
         int cy, cz, dyc, dzc;
@@ -197,7 +205,7 @@ __device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, 
                 int lo = gr.gx0 - rx, hi = gr.gx1 + rx; // inclusive x-cell range
                 const int row = (cz * ncy + cy) * ncx;
                 if (PERIODIC) {
-                    if (hi - lo + 1 >= ncx) { lo = 0; hi = ncx - 1; }
+                    if (hi - lo + 1 >= ncx) { lo = 0; hi = ncx - 1; covers = true; }
                     if (lo < 0) {
                         s0 = a.cell_start[row + lo + ncx]; l0 = a.cell_start[row + ncx] - s0;
                         s1 = a.cell_start[row]; l1 = a.cell_start[row + hi + 1] - s1;
@@ -213,30 +221,31 @@ __device__ __forceinline__ int build_ranges(const PairArgs &a, const Group &gr, 
                 }
             }
         }
-        mine += l0 + l1;
+        mine += ((l0 + 31) >> 5) + ((l1 + 31) >> 5);
         if (STORE) {
-            rng_start[2 * r] = s0; rng_off[2 * r + 1] = l0;       // lengths parked in rng_off[.+1], scanned below
-            rng_start[2 * r + 1] = s1; rng_off[2 * r + 2] = l1;
+            rng_start[2 * r] = s0; rng_len[2 * r] = l0; rng_woff[2 * r + 1] = (l0 + 31) >> 5; // words parked in [.+1], scanned below
+            rng_start[2 * r + 1] = s1; rng_len[2 * r + 1] = l1; rng_woff[2 * r + 2] = (l1 + 31) >> 5;
         }
     }
     const int nr = 2 * nyz;
     *nr_out = nr;
+    *wide = __any_sync(kFull, covers);
     if (!STORE) return __reduce_add_sync(kFull, mine);
     __syncwarp();
-    { // inclusive scan of the lengths into offsets
+    { // inclusive scan of the word counts into offsets
         const int per = (nr + 31) / 32;
         const int b0 = lane * per, b1 = min(nr, b0 + per);
         int sum = 0;
-        for (int r = b0; r < b1; ++r) sum += rng_off[r + 1];
+        for (int r = b0; r < b1; ++r) sum += rng_woff[r + 1];
         int x = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { int y = __shfl_up_sync(kFull, x, d); if (lane >= d) x += y; }
         int run = x - sum;
-        for (int r = b0; r < b1; ++r) { const int len = rng_off[r + 1]; run += len; rng_off[r + 1] = run; }
-        if (lane == 0) rng_off[0] = 0;
+        for (int r = b0; r < b1; ++r) { const int len = rng_woff[r + 1]; run += len; rng_woff[r + 1] = run; }
+        if (lane == 0) rng_woff[0] = 0;
     }
     __syncwarp();
-    return rng_off[nr];
+    return rng_woff[nr];
 }
 
 // exact decision, the operations of DESIGN.md R8-R10 (the oracle's): returns the bin or kNoHit
@@ -256,37 +265,29 @@ __device__ __noinline__ unsigned classify_exact(const double4 &cj, const double 
     return (unsigned)b;
 }
 
-// upper bound on the pool slabs a group can take (see k_fill: a slab yields >= kSlabPages-31 usable pages)
-__device__ __forceinline__ int slab_bound(long long cand, int cnt, int nb)
-{
-    const long long need = (cand * cnt) / ENCORE_PAGE_WORDS + (long long)cnt * nb;
-    const long long slabs = need / (ENCORE_SLAB_PAGES - 31) + 1;
-    return (int)(slabs > INT_MAX ? INT_MAX : slabs);
-}
-
-// per group: candidates T and the slab bound (sizes the super-steps on the host)
+// per group: number of candidate words (row capacity of each of its bins; sizes the super-steps on the host)
 template <bool PERIODIC>
 __global__ void __launch_bounds__(128) k_group_bound(PairArgs a)
 {
     const int g = blockIdx.x * 4 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (g >= a.ngroups) return;
-    if (g >= a.group_start[a.geom.npencil]) { if (lane == 0) a.gbound[g] = 0; return; }
+    if (g >= a.group_start[a.geom.npencil]) { if (lane == 0) { a.gbound[g] = 0; a.gwide[g] = 0; } return; }
     const Group gr = locate_group<PERIODIC>(a, g);
     int nr;
-    const int T = build_ranges<PERIODIC, false>(a, gr, lane, nullptr, nullptr, &nr);
-    if (lane == 0) a.gbound[g] = slab_bound(T, gr.cnt, a.bins.nbins);
+    bool wide;
+    const int W = build_ranges<PERIODIC, false>(a, gr, lane, nullptr, nullptr, nullptr, &nr, &wide);
+    if (lane == 0) { a.gbound[g] = W; a.gwide[g] = wide ? 1 : 0; }
 }
 
 // ==========================================================================================================
 // k_fill: a3.  One warp (= one CTA) per group.
 // ==========================================================================================================
-// dynamic shared memory: cand[64] float4 | sp[96] double | e2[nb+1] double | ring[nb][32][4] u32 |
-//                        cursor[nb][32] u32 | pagecur[nb][32] int | rng_start[nr_cap] | rng_off[nr_cap+1]
+// dynamic shared memory: cand[34] float4 | sp[96] double | e2[nb+1] double | masks[nb][32] u32 |
+//                        rng_start[nr_cap] | rng_len[nr_cap] | rng_woff[nr_cap+1]
 __host__ __device__ inline size_t fill_smem_bytes(int nb, int nr_cap)
 {
-    return 2 * 32 * 16 + 96 * 8 + (size_t)((nb + 2) & ~1) * 8 + (size_t)nb * kRing * 32 * 4 + (size_t)nb * 32 * 4 * 2 +
-           (size_t)(2 * nr_cap + 4) * 4;
+    return 34 * 16 + 96 * 8 + (size_t)((nb + 2) & ~1) * 8 + (size_t)nb * 32 * 4 + (size_t)(3 * nr_cap + 4) * 4;
 }
 
 template <bool PERIODIC>
@@ -300,13 +301,12 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 
     extern __shared__ __align__(16) unsigned char fill_smem[];
     float4 *cand = reinterpret_cast<float4 *>(fill_smem);
-    double *sp = reinterpret_cast<double *>(cand + 64);
+    double *sp = reinterpret_cast<double *>(cand + 34);
     double *e2 = sp + 96;
-    unsigned *ring = reinterpret_cast<unsigned *>(e2 + ((nb + 2) & ~1));
-    unsigned *cursor = ring + nb * kRing * 32;
-    int *pagecur = reinterpret_cast<int *>(cursor + nb * 32);
-    int *rng_start = pagecur + nb * 32;
-    int *rng_off = rng_start + nr_cap;
+    unsigned *masks = reinterpret_cast<unsigned *>(e2 + ((nb + 2) & ~1));
+    int *rng_start = reinterpret_cast<int *>(masks + nb * 32);
+    int *rng_len = rng_start + nr_cap;
+    int *rng_woff = rng_len + nr_cap;
 
     const Group gr = locate_group<PERIODIC>(a, g);
     const int first = gr.first, cnt = gr.cnt;
@@ -315,12 +315,14 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     sp[lane] = mine.x; sp[32 + lane] = mine.y; sp[64 + lane] = mine.z;
     a.gweights[(size_t)g * 32 + lane] = lane < cnt ? mine.w : 0.0;
     if (lane <= nb) e2[lane] = a.bins.e2[lane];
-    for (int b = 0; b < nb; ++b) cursor[b * 32 + lane] = 0u;
+    for (int b = 0; b < nb; ++b) masks[b * 32 + lane] = 0u;
+    if (lane == 0) cand[32] = make_float4(1e18f, 1e18f, 1e18f, 0.f); // filler of the 4-wide test blocks: never a hit
     // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
     const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
 
     int nr;
-    const int T = build_ranges<PERIODIC, true>(a, gr, lane, rng_start, rng_off, &nr);
+    bool wide;
+    const int nwords = build_ranges<PERIODIC, true>(a, gr, lane, rng_start, rng_len, rng_woff, &nr, &wide);
 
     // fp32 screening constants: the bin coordinate u = (r - r_min)/width computed in fp32 is within
     // du = [2^-18 (r + r_min) + 2^-19 E^2 / r] / width + 2^-20 |u| of the exact one (E^2 = sum of squared group
@@ -334,93 +336,9 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     const float kB = 1.9073486328125e-06f * invw_f *
                      (float)(gr.ext[0] * gr.ext[0] + gr.ext[1] * gr.ext[1] + gr.ext[2] * gr.ext[2]);
     const float thr0 = 0.5f - duc;
-    const float uh_hi = nb_f - 0.5f;
-    const bool fast = gr.fast;
+    // a common periodic image per run needs r_max + extent < L/2 and no run covering a whole axis
+    const bool fast = gr.fast && !wide;
 
-    // ---- list state -----------------------------------------------------------------------------------------
-    // blocks of 4 completed but not yet written: (block index << 5) | bin.  The tests run two candidates between
-    // flushes and a lane appends at most once per candidate, so at most two blocks (of two different bins) complete
-    // in between: two slots.  If the first append completes a block and the second goes to the same bin, the entry
-    // waits in a register (ovf_entry) and becomes entry 0 of the block once that has been written: the ring is a
-    // single block per (bin, lane) - 5 kB for 10 bins instead of 10 kB, which is what sets the warps per SM.
-    int pendA = -1, pendB = -1;
-    bool ovf = false;
-    unsigned ovf_entry = 0u;
-    int slab_next = 0, slab_end = 0; // pages of the pool owned by this warp (uniform)
-    const unsigned lt_mask = (1u << lane) - 1u;
-
-    // all lanes call; lanes with a pending block write it (4 entries, 16 bytes) to their page.
-    // ring layout [bin][lane][4]: the flush is one conflict-free 16-byte shared-memory load
-    auto flush_block = [&](int &pend, bool with_ovf) {
-        const bool act = pend >= 0;
-        const int b = pend & 31, kb = pend >> 5;
-        const bool newpage = act && (kb & 15) == 0;
-        const unsigned nm = __ballot_sync(kFull, newpage);
-        if (nm) {
-            const int nn = __popc(nm);
-            if (slab_next + nn > slab_end) { // the rest of the old slab (< 32 pages) is dropped: see slab_bound
-                unsigned base = 0;
-                if (lane == 0) base = atomicAdd(a.pool_cursor, (unsigned)ENCORE_SLAB_PAGES);
-                base = __shfl_sync(kFull, base, 0);
-                if (base + ENCORE_SLAB_PAGES > a.pool_pages) { // excluded by the host's step bounds; stay in bounds
-                    if (lane == 0) *a.err_flag = 1;
-                    base = 0;
-                }
-                slab_next = (int)base; slab_end = (int)base + ENCORE_SLAB_PAGES;
-            }
-            if (newpage) {
-                const int pg = slab_next + __popc(nm & lt_mask);
-                if (kb == 0) a.first_page[((size_t)g * nb + b) * 32 + lane] = pg;
-                else a.page_next[pagecur[b * 32 + lane]] = pg;
-                pagecur[b * 32 + lane] = pg;
-            }
-            slab_next += nn;
-        }
-        if (act) {
-            unsigned *blk = ring + ((b << 5) + lane) * 4;
-            const uint4 v = *reinterpret_cast<const uint4 *>(blk);
-            __stcs(reinterpret_cast<uint4 *>(a.pool + (size_t)pagecur[b * 32 + lane] * ENCORE_PAGE_WORDS + ((kb & 15) << 2)), v);
-            if (with_ovf && ovf) blk[0] = ovf_entry;
-        }
-        pend = -1;
-    };
-    auto flush_all = [&]() {
-        if (__any_sync(kFull, pendA >= 0)) {
-            flush_block(pendA, true);
-            ovf = false;
-            if (__any_sync(kFull, pendB >= 0)) flush_block(pendB, false);
-        }
-    };
-    // `second`: an append may have happened since the last flush (then pendA may hold this bin's full block)
-    auto append = [&](unsigned code, unsigned entry, bool second) {
-        unsigned *cp = cursor + code * 32 + lane;
-        const unsigned pos = *cp;
-        *cp = pos + 1u;
-        if (second && pendA >= 0 && (unsigned)(pendA & 31) == code) { ovf = true; ovf_entry = entry; } // pos & 3 == 0
-        else {
-            ring[((code << 5) + lane) * 4 + (pos & 3u)] = entry;
-            if ((pos & 3u) == 3u) {
-                const int v = (int)(((pos >> 2) << 5) | code);
-                if (pendA < 0) pendA = v; else pendB = v;
-            }
-        }
-    };
-
-    // ---- candidate queue ------------------------------------------------------------------------------------------
-    // Candidates are read a word (32) at a time, lane = candidate: fp64 -> relative to primary 0 (periodic image) ->
-    // fp32, then culled against the group's bounding box (distance to the box > r_max: no primary of the group can
-    // accept it) and the survivors are compacted into a 64-entry ring in shared memory (.w = list entry).  The pair
-    // tests below always run on 32 queued candidates, so their cost follows the culled candidate count.
-    // a lane asks for s = lane, 32 + lane, 64 + lane, ...: its run index only moves forward
-    int run_lo = 0; // rng_off[run_lo] <= s < rng_off[run_lo + 1] once advanced (empty runs are stepped over)
-    auto load_cand = [&](int s, double4 &cj, unsigned &j) {
-        j = kPadEntry;
-        if (s < T) {
-            while (rng_off[run_lo + 1] <= s) ++run_lo; // s < T = rng_off[nr] bounds the walk
-            j = (unsigned)(rng_start[run_lo] + (s - rng_off[run_lo]));
-            cj = a.pos4[j];
-        }
-    };
     // bounding box of the group's primaries (same fp32 values the tests use) and the cull radius: r_max plus the
     // fp32 rounding of the coordinates involved (<= 2^-23 (extent + r_max) per axis), with a safety factor
     float blo[3], bhi[3];
@@ -440,57 +358,75 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     }
     const double rcut = (a.rmax + 9.5367431640625e-07 * (gr.ext[0] + gr.ext[1] + gr.ext[2] + a.rmax)) * (1.0 + 1e-6);
     const float cut2 = (float)(rcut * rcut * (1.0 + 1e-6));
-    int qh = 0, qn = 0; // ring head and fill level (uniform)
+
+    // row streams of this group: bin b owns rows [b * nwords, (b+1) * nwords) behind the group's base
+    const size_t wbase = (size_t)(a.gprefix[g] - a.gprefix[g0]) * (size_t)nb;
+    unsigned *rows_g = a.rows + wbase * 32;
+    unsigned *desc_g = a.rowdesc + wbase;
+    int rowcnt = 0;                     // lane b holds the number of rows written for bin b
     unsigned long long kept = 0ull;
-    auto stage = [&](const double4 &cj, unsigned j) {
-        float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    // words are read one ahead: lane = candidate
+    int run = 0; // rng_woff[run] <= w < rng_woff[run + 1] once advanced (runs without words are stepped over)
+    auto load_word = [&](int w, double4 &cj, int &jbase, bool &valid) {
+        valid = false; jbase = 0;
+        if (w < nwords) {
+            while (rng_woff[run + 1] <= w) ++run; // w < nwords = rng_woff[nr] bounds the walk
+            const int k0 = (w - rng_woff[run]) << 5;
+            jbase = rng_start[run] + k0;
+            valid = k0 + lane < rng_len[run];
+            if (valid) cj = a.pos4[jbase + lane];
+        }
+    };
+    double4 cjA = make_double4(0, 0, 0, 0), cjB = cjA;
+    int jbA = 0, jbB = 0;
+    bool vA = false, vB = false;
+    load_word(0, cjA, jbA, vA);
+    for (int w = 0; w < nwords; ++w) {
+        load_word(w + 1, cjB, jbB, vB); // in flight during the tests below
+        // ---- stage the word: fp64 -> relative to primary 0 (periodic image) -> fp32, bounding-box cull ----
+        float4 cf = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+        unsigned code = 0x15u; // image codes (1,1,1): the consumer subtracts {-L, 0, +L}[code] per axis from x_i
         bool keep = false;
-        if (j != kPadEntry) {
-            double rx = cj.x - ctr.x, ry = cj.y - ctr.y, rz = cj.z - ctr.z;
-            unsigned kx = 1, ky = 1, kz = 1;  // image code: the list consumer subtracts {-L, 0, +L}[code] from x_i
+        if (vA) {
+            double rx = cjA.x - ctr.x, ry = cjA.y - ctr.y, rz = cjA.z - ctr.z;
+            unsigned kx = 1, ky = 1, kz = 1;
             if (PERIODIC) {
                 if (rx > G.half) { rx -= G.box; kx = 2; } else if (rx < -G.half) { rx += G.box; kx = 0; }
                 if (ry > G.half) { ry -= G.box; ky = 2; } else if (ry < -G.half) { ry += G.box; ky = 0; }
                 if (rz > G.half) { rz -= G.box; kz = 2; } else if (rz < -G.half) { rz += G.box; kz = 0; }
             }
-            cf = make_float4((float)rx, (float)ry, (float)rz, __uint_as_float(j | (kx << 26) | (ky << 28) | (kz << 30)));
+            code = kx | (ky << 2) | (kz << 4);
+            cf = make_float4((float)rx, (float)ry, (float)rz, 0.f);
             const float ex = fmaxf(fmaxf(blo[0] - cf.x, cf.x - bhi[0]), 0.f);
             const float ey = fmaxf(fmaxf(blo[1] - cf.y, cf.y - bhi[1]), 0.f);
             const float ez = fmaxf(fmaxf(blo[2] - cf.z, cf.z - bhi[2]), 0.f);
             keep = !fast || fmaf(ez, ez, fmaf(ey, ey, ex * ex)) <= cut2; // wide groups (exact path) keep everything
         }
         const unsigned km = __ballot_sync(kFull, keep);
-        if (keep) cand[(qh + qn + __popc(km & lt_mask)) & 63] = cf;
-        qn += __popc(km);
-        kept += (unsigned long long)__popc(km);
-    };
-
-    const int nwords = (T + 31) >> 5;
-    int wnext = 0; // next word to stage; cjA holds it, cjB the one after
-    double4 cjA = make_double4(0, 0, 0, 0), cjB = cjA;
-    unsigned jA = kPadEntry, jB = kPadEntry;
-    load_cand(lane, cjA, jA);
-    load_cand(32 + lane, cjB, jB);
-    for (;;) {
-        while (qn < 32 && wnext < nwords) {
-            stage(cjA, jA);
-            cjA = cjB; jA = jB;
-            ++wnext;
-            load_cand((wnext + 1) * 32 + lane, cjB, jB); // two words ahead: in flight during the tests below
+        const int jbase = jbA;
+        cjA = cjB; jbA = jbB; vA = vB;
+        if (km == 0u) continue;         // no candidate of the word is within reach of the group
+        const unsigned wcode = __shfl_sync(kFull, code, 0); // lane 0 of a word is always a candidate
+        if (PERIODIC && fast && __any_sync(kFull, keep && code != wcode)) { // excluded by DESIGN.md §5.3
+            if (lane == 0) *a.err_flag = 1;
         }
-        if (qn == 0) break;
-        const int nvalid = min(qn, 32);
-        if (lane >= nvalid) cand[(qh + lane) & 63] = make_float4(1e18f, 1e18f, 1e18f, __uint_as_float(kPadEntry)); // never a hit
+        cand[lane] = cf;
         __syncwarp();
+        kept += (unsigned long long)__popc(km);
         if (fast) {
+            unsigned rem = km;
 #pragma unroll 1
-            for (int c4 = 0; c4 < 32; c4 += 4) {
-                // four independent tests first (instruction-level parallelism), then the appends in candidate order
-                unsigned ent[4], code[4];
+            while (rem) {
+                // four independent tests (instruction-level parallelism) on the next four surviving candidates
+                int cpos[4];
+                unsigned codeb[4];
                 bool ok[4], am[4];
 #pragma unroll
                 for (int cc = 0; cc < 4; ++cc) {
-                    const float4 q = cand[(qh + c4 + cc) & 63];
+                    cpos[cc] = rem ? __ffs(rem) - 1 : 32;
+                    rem &= rem - 1u;
+                    const float4 q = cand[cpos[cc]];
                     const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
                     const float t = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), 1e-30f); // t = 0: r = 0 -> exact path
                     float rinv;
@@ -501,151 +437,210 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                     const float fr = uh - (v - kMagic);
                     const bool sure = fabsf(fr) <= thr;              // farther than du from every bin edge
                     // v in [kMagic, kMagic + nb) <=> uh rounds into 0..nb-1 (float bits are monotonic)
-                    code[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
-                    ok[cc] = sure && code[cc] < (unsigned)nb;
+                    codeb[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
+                    ok[cc] = sure && codeb[cc] < (unsigned)nb;
                     am[cc] = !sure;                                  // ~2 du of all pairs, in range or not
-                    ent[cc] = __float_as_uint(q.w);
                 }
                 if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
-                    if (ok[0]) append(code[0], ent[0], false);
-                    if (ok[1]) append(code[1], ent[1], true);
-                    flush_all();
-                    if (ok[2]) append(code[2], ent[2], false);
-                    if (ok[3]) append(code[3], ent[3], true);
-                    flush_all();
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc)
+                        if (ok[cc]) atomicOr(&masks[codeb[cc] * 32 + lane], 1u << cpos[cc]);
                 } else {
                     // some pair is within the error margin of a bin edge (~1e-4 of the pairs): exact decision
 #pragma unroll
                     for (int cc = 0; cc < 4; ++cc) {
-                        if (ok[cc]) append(code[cc], ent[cc], cc & 1);
-                        else if (am[cc] && code[cc] + 1u < (unsigned)nb + 2u && ent[cc] != kPadEntry) {
-                            const unsigned cx = classify_exact<PERIODIC>(a.pos4[ent[cc] & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
-                            if (cx != kNoHit) append(cx, ent[cc], cc & 1);
+                        if (ok[cc]) atomicOr(&masks[codeb[cc] * 32 + lane], 1u << cpos[cc]);
+                        else if (am[cc] && codeb[cc] + 1u < (unsigned)nb + 2u && cpos[cc] < 32) {
+                            const unsigned cx = classify_exact<PERIODIC>(a.pos4[jbase + cpos[cc]], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
+                            if (cx != kNoHit) atomicOr(&masks[cx * 32 + lane], 1u << cpos[cc]);
                         }
-                        if (cc & 1) flush_all();
                     }
                 }
             }
         } else {
             // group too wide for a common image: every pair is decided exactly
-            for (int c = 0; c < nvalid; ++c) {
-                const unsigned e = __float_as_uint(cand[(qh + c) & 63].w);
+            unsigned rem = km;
+            while (rem) {
+                const int c = __ffs(rem) - 1;
+                rem &= rem - 1u;
                 if (lane < cnt) {
-                    const unsigned code = classify_exact<PERIODIC>(a.pos4[e & kIdxMask], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
-                    if (code != kNoHit) append(code, e, false);
+                    const unsigned cx = classify_exact<PERIODIC>(a.pos4[jbase + c], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
+                    if (cx != kNoHit) masks[cx * 32 + lane] |= 1u << c;
                 }
-                flush_all();
             }
         }
-        qh = (qh + 32) & 63;
-        qn -= nvalid;
-        __syncwarp();
+        // ---- one coalesced row per bin that has any bit set --------------------------------------------------------
+        const unsigned desc = (unsigned)jbase | (wcode << 26);
+        for (int b = 0; b < nb; ++b) {
+            const unsigned m = masks[b * 32 + lane];
+            if (__any_sync(kFull, m != 0u)) {
+                const int k = __shfl_sync(kFull, rowcnt, b);
+                const size_t ro = (size_t)b * nwords + k;
+                __stcs(rows_g + ro * 32 + lane, m);
+                if (lane == 0) __stcs(desc_g + ro, desc);
+                if (lane == b) ++rowcnt;
+                masks[b * 32 + lane] = 0u;
+            }
+        }
+        __syncwarp(); // every lane is done with cand[] before the next word overwrites it
     }
+    if (lane < nb) a.rowcnt[(size_t)g * nb + lane] = rowcnt;
     if (lane == 0) atomicAdd(a.cand_pairs, kept * (unsigned long long)cnt);
-
-    // close the open block of every (bin, lane): pad it to 4 entries, flush, and complete the last group of 8
-    // (k_harm reads 8 entries at a time); cursors are n_i(b)
-    for (int b = 0; b < nb; ++b) {
-        const unsigned k = cursor[b * 32 + lane];
-        a.counts[((size_t)g * nb + b) * 32 + lane] = k;
-        unsigned *blk = ring + ((b << 5) + lane) * 4;
-        unsigned nblk4 = k >> 2;
-        if (k & 3u) {
-            for (unsigned q = k & 3u; q < 4u; ++q) blk[q] = kPadEntry;
-            pendA = (int)((nblk4 << 5) | (unsigned)b);
-            ++nblk4;
-        }
-        flush_all();
-        if (nblk4 & 1u) {
-            for (unsigned q = 0; q < 4u; ++q) blk[q] = kPadEntry;
-            pendA = (int)((nblk4 << 5) | (unsigned)b);
-        }
-        flush_all();
-    }
 }
 
 // ==========================================================================================================
-// k_harm: a4.  One warp per item (group, bin): every lane streams its list, a_lm accumulates in registers.
+// k_harm: a4.  One warp per item (group, bin): every lane walks the set bits of its column of the item's rows,
+// a_lm accumulates in registers.
 // ==========================================================================================================
 struct Raw { double2 xy, zw; };
 
 // One 256-bit load per candidate (LDG.E.256, sm_100): the gather is one 32-byte sector per lane, and the L1 tag stage
-// handles one sector per cycle, so two 128-bit loads of the same sector cost twice the L1 time (the v4 kernel sat at
-// 80 % L1 throughput with the FP64 pipe at 60 %).
-__device__ __forceinline__ Raw gather(const double4 *__restrict__ pos4, unsigned e)
+// handles one sector per cycle, so two 128-bit loads of the same sector cost twice the L1 time.
+__device__ __forceinline__ Raw gather(const double4 *__restrict__ pos4, unsigned idx)
 {
     Raw r;
-    // a padding entry reads particle 0 (always valid memory); its contribution is cancelled by weight 0 below
-    const double4 *q = pos4 + (e == kPadEntry ? 0u : (e & kIdxMask));
+    const double4 *q = pos4 + idx;
     asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.xy.x), "=d"(r.xy.y), "=d"(r.zw.x), "=d"(r.zw.y) : "l"(q));
     return r;
 }
 
-// MODE 0: open geometry; 1: periodic, image carried by the entry; 2: periodic, image decided per pair
-// mtab (MODE 1): shared memory [axis][image code][thread] = x_i + {-L, 0, +L}: x_j - (x_i -/+ L) is the minimal image
-// D: candidates gathered ahead of the one being accumulated (2 at 12 warps/SM, 4 in the fat passes at 8 warps/SM)
-template <int LMAX, int MLO, int MHI, int MODE, int D>
-__device__ __forceinline__ void harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ pool,
-                                          const int *__restrict__ page_next, int page, int nblk_lane, int nblk,
-                                          const double4 *__restrict__ pos4, const double4 &me, const double *mtab,
-                                          double box, double half)
+__device__ __forceinline__ void cp_async4(unsigned *smem_dst, const unsigned *gsrc)
 {
-    const uint4 padv = make_uint4(kPadEntry, kPadEntry, kPadEntry, kPadEntry);
-    uint4 q0 = padv, q1 = padv;
-    int nextp = 0;
-    if (nblk_lane > 0) {
-        const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS);
-        q0 = __ldcg(p); q1 = __ldcg(p + 1);
-        if (nblk_lane > 8) nextp = page_next[page];
-    }
-    Raw r[D];
-    {
-        const unsigned e0[4] = {q0.x, q0.y, q0.z, q0.w};
-#pragma unroll
-        for (int d = 0; d < D; ++d) r[d] = gather(pos4, e0[d]);
-    }
-    for (int kb = 0; kb < nblk; ++kb) {
-        uint4 n0 = padv, n1 = padv; // entries of block kb+1
-        if (kb + 1 < nblk_lane) {
-            const bool turn = ((kb + 1) & 7) == 0;
-            if (turn) page = nextp;
-            const uint4 *p = reinterpret_cast<const uint4 *>(pool + (size_t)page * ENCORE_PAGE_WORDS + (((kb + 1) & 7) << 3));
-            n0 = __ldcg(p); n1 = __ldcg(p + 1);
-            if (turn && kb + 9 < nblk_lane) nextp = page_next[page];
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// MODE 0: open geometry; 1: periodic, image carried by the row descriptor; 2: periodic, image decided per pair
+// mtab (MODE 1): shared memory [axis][image code][thread] = x_i + {-L, 0, +L}: x_j - (x_i -/+ L) is the minimal image
+// D: candidates gathered ahead of the one being accumulated.  Returns the number of pairs this lane accumulated.
+// qm/qd: this warp's record queue [kQueue][32]; stm: row staging [2][kStageRows][32]; std_: descriptors [2][32].
+template <int LMAX, int MLO, int MHI, int MODE, int D>
+__device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ rows,
+                                              const unsigned *__restrict__ rdesc, int nrows, bool active, unsigned *qm,
+                                              unsigned *qd, unsigned *stm, unsigned *std_, const double4 *__restrict__ pos4,
+                                              const double4 &me, const double *mtab, double box, double half, int lane)
+{
+    static_assert(D >= 1 && D <= 4, "the image-code fifo holds four bytes");
+    // ---- rows -> shared memory, two chunks in flight (every chunk slot commits one cp.async group, empty or not) ----
+    auto issue_chunk = [&](int c) {
+        const int r0 = c * kStageRows;
+        if (r0 < nrows) {
+            const int nr = min(kStageRows, nrows - r0);
+            unsigned *dst = stm + (c & 1) * kStageRows * 32 + lane;
+            const unsigned *src = rows + (size_t)r0 * 32 + lane;
+            for (int k = 0; k < nr; ++k) cp_async4(dst + k * 32, src + (size_t)k * 32);
+            if (lane < nr) cp_async4(std_ + (c & 1) * 32 + lane, rdesc + r0 + lane);
         }
-        const unsigned e[12] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, n0.x, n0.y, n0.z, n0.w};
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const Raw r0 = r[u % D];
-            r[u % D] = gather(pos4, e[u + D]); // D candidates ahead
-            const unsigned en = e[u];
-            double dx, dy, dz;
-            if (MODE == 1) {
-                const unsigned kx = (en >> 26) & 3u, ky = (en >> 28) & 3u, kz = en >> 30;
-                dx = r0.xy.x - mtab[(0 * 3 + kx) * (kHarmWarps * 32)];
-                dy = r0.xy.y - mtab[(1 * 3 + ky) * (kHarmWarps * 32)];
-                dz = r0.zw.x - mtab[(2 * 3 + (kz > 2u ? 1u : kz)) * (kHarmWarps * 32)];
-            } else {
-                dx = sep<MODE == 2>(r0.xy.x, me.x, box, half);
-                dy = sep<MODE == 2>(r0.xy.y, me.y, box, half);
-                dz = sep<MODE == 2>(r0.zw.x, me.z, box, half);
+        cp_async_commit();
+    };
+    issue_chunk(0);
+    issue_chunk(1);
+    int rows_done = 0;
+    unsigned head = 0u, tail = 0u;      // lane-private queue cursors
+    int avail = 0;                      // pairs queued and not yet generated (bits of cur + bits of the queued masks)
+    unsigned npairs = 0u;
+    unsigned cur = 0u, base = 0u, img = 0u;
+    bool drained = false;
+    // push rows while every lane has room for one more record; returns the number of steps to run next (0: finished)
+    auto refill = [&]() -> int {
+        int room = kQueue - __reduce_max_sync(kFull, (int)(tail - head));
+        while (room > 0 && rows_done < nrows) {
+            const int k = rows_done % kStageRows, buf = (rows_done / kStageRows) & 1;
+            if (k == 0) { cp_async_wait<1>(); __syncwarp(); }
+            const unsigned m = stm[(buf * kStageRows + k) * 32 + lane];
+            const unsigned d = std_[buf * 32 + k];
+            if (m) {
+                const unsigned slot = (tail & (kQueue - 1)) * 32 + lane;
+                qm[slot] = m; qd[slot] = d;
+                ++tail;
+                const int pc = __popc(m);
+                avail += pc; npairs += (unsigned)pc;
             }
-            const bool pad = en == kPadEntry;
-            if (pad) { dx = 1.0; dy = 0.0; dz = 0.0; }
-            const double wj = pad ? 0.0 : r0.zw.y;
-            const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
-            const double rinv = rsqrt_pair(r2s);
-            accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
+            ++rows_done; --room;
+            if (rows_done % kStageRows == 0) { __syncwarp(); issue_chunk(rows_done / kStageRows + 1); }
         }
-        q0 = n0; q1 = n1;
+        if (rows_done < nrows) { // a starving lane waits for rows: run while every active lane has pairs (at least 4 steps)
+            const int s = __reduce_min_sync(kFull, active ? avail : INT_MAX);
+            return s >= 4 ? (s & ~3) : 4;
+        }
+        const int s = __reduce_max_sync(kFull, avail);
+        if (s > 0) return (s + 3) & ~3;
+        if (drained) return 0;
+        drained = true;                 // the last D gathers are still in flight
+        return 4;
+    };
+    // next pair of this lane: sorted index + image code (0x80: padding, nothing left)
+    auto gen = [&](unsigned &idx, unsigned &code) {
+        if (cur == 0u && head != tail) {
+            const unsigned slot = (head & (kQueue - 1)) * 32 + lane;
+            cur = qm[slot];
+            const unsigned d = qd[slot];
+            ++head;
+            base = d & kIdxMask; img = d >> 26;
+        }
+        const bool pad = cur == 0u;
+        const unsigned bit = (unsigned)(__ffs((int)cur) - 1);
+        cur &= cur - 1u;
+        idx = pad ? 0u : base + bit;    // padding reads particle 0 (always valid memory); its weight is forced to 0
+        code = pad ? 0x80u : img;
+        avail -= pad ? 0 : 1;
+    };
+
+    int S = refill();
+    if (S == 0 || (drained && S == 4)) { cp_async_wait<0>(); return 0u; } // no pair in this item
+    Raw r[D];
+    unsigned fifo = 0u;                 // image codes of the D gathers in flight, newest in the low byte
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+        unsigned idx, code;
+        gen(idx, code);
+        r[d] = gather(pos4, idx);
+        fifo = (fifo << 8) | code;
     }
+    do {
+        for (int s = 0; s < S; s += 4) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const Raw r0 = r[u % D];
+                const unsigned c0 = (fifo >> (8 * (D - 1))) & 0xffu;
+                unsigned idx, code;
+                gen(idx, code);
+                r[u % D] = gather(pos4, idx); // D candidates ahead
+                fifo = (fifo << 8) | code;
+                double dx, dy, dz;
+                if (MODE == 1) {
+                    const unsigned kx = c0 & 3u, ky = (c0 >> 2) & 3u, kz = (c0 >> 4) & 3u;
+                    dx = r0.xy.x - mtab[(0 * 3 + kx) * (kHarmWarps * 32)];
+                    dy = r0.xy.y - mtab[(1 * 3 + ky) * (kHarmWarps * 32)];
+                    dz = r0.zw.x - mtab[(2 * 3 + kz) * (kHarmWarps * 32)];
+                } else {
+                    dx = sep<MODE == 2>(r0.xy.x, me.x, box, half);
+                    dy = sep<MODE == 2>(r0.xy.y, me.y, box, half);
+                    dz = sep<MODE == 2>(r0.zw.x, me.z, box, half);
+                }
+                const bool pad = (c0 & 0x80u) != 0u;
+                if (pad) { dx = 1.0; dy = 0.0; dz = 0.0; }
+                const double wj = pad ? 0.0 : r0.zw.y;
+                const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
+                const double rinv = rsqrt_pair(r2s);
+                accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
+            }
+        }
+        S = refill();
+    } while (S > 0);
+    cp_async_wait<0>();
+    return npairs;
 }
 
 template <int LMAX, int MLO, int MHI, bool PERIODIC>
-__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3) k_harm(PairArgs a, int g0, int g1)
+__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3) k_harm(PairArgs a, int g0, int g1, int write_counts)
 {
     constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH;
     __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
+    __shared__ unsigned s_qm[kHarmWarps][kQueue * 32], s_qd[kHarmWarps][kQueue * 32];
+    __shared__ unsigned s_stm[kHarmWarps][2 * kStageRows * 32], s_std[kHarmWarps][2 * 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
     const int item = blockIdx.x * kHarmWarps + warp;
@@ -655,24 +650,31 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     const bool active = lane < gr.cnt;
     const double4 me = a.pos4[gr.first + (active ? lane : 0)];
     const size_t col = ((size_t)g * nb + bin) * 32 + lane;
-    const unsigned n_mine = active ? a.counts[col] : 0u;
-    const int nblk_lane = (int)((n_mine + 7u) >> 3);
-    const int nblk = __reduce_max_sync(kFull, nblk_lane);
-    const int page = nblk_lane > 0 ? a.first_page[col] : 0;
+    // the row stream of (g, bin): see k_fill
+    const int nwords = a.gprefix[g + 1] - a.gprefix[g];
+    const size_t ro = (size_t)(a.gprefix[g] - a.gprefix[g0]) * (size_t)nb + (size_t)bin * nwords;
+    const unsigned *rows = a.rows + ro * 32;
+    const unsigned *rdesc = a.rowdesc + ro;
+    const int nrows = a.rowcnt[(size_t)g * nb + bin];
+    // the exact path of k_fill (no common image per run) is taken under the same condition there
+    bool fast = gr.fast;
+    if (PERIODIC && fast) fast = !a.gwide[g];
 
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    if (!PERIODIC) harm_rows<LMAX, MLO, MHI, 0, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, 0.0, 0.0);
-    else if (gr.fast) {
+    unsigned np;
+    if (!PERIODIC) np = harm_rows<LMAX, MLO, MHI, 0, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, nullptr, 0.0, 0.0, lane);
+    else if (fast) {
         double *mt = mtab + threadIdx.x;
         const double L = a.geom.box;
         mt[0 * kHarmWarps * 32] = me.x - L; mt[1 * kHarmWarps * 32] = me.x; mt[2 * kHarmWarps * 32] = me.x + L;
         mt[3 * kHarmWarps * 32] = me.y - L; mt[4 * kHarmWarps * 32] = me.y; mt[5 * kHarmWarps * 32] = me.y + L;
         mt[6 * kHarmWarps * 32] = me.z - L; mt[7 * kHarmWarps * 32] = me.z; mt[8 * kHarmWarps * 32] = me.z + L;
         __syncwarp();
-        harm_rows<LMAX, MLO, MHI, 1, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, mt, L, a.geom.half);
-    } else harm_rows<LMAX, MLO, MHI, 2, D>(acc, a.pool, a.page_next, page, nblk_lane, nblk, a.pos4, me, nullptr, a.geom.box, a.geom.half);
+        np = harm_rows<LMAX, MLO, MHI, 1, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, mt, L, a.geom.half, lane);
+    } else np = harm_rows<LMAX, MLO, MHI, 2, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, nullptr, a.geom.box, a.geom.half, lane);
+    if (write_counts) a.counts[col] = np;   // n_i(b); every m-range pass walks the same bits, the first one reports
 
     // epilogue: a_lm = (1/v_b) sum_k ycoef[c][k] S_{m,k}, k = l-m, l-m-2, ... (p_lm has the parity of l-m)
     const double vinv = a.bins.vinv[bin];
@@ -700,12 +702,12 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
 }
 
 template <int LMAX, int MLO, int MHI>
-cudaError_t launch_harm(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches)
+cudaError_t launch_harm(const PairArgs &a, int g0, int g1, int write_counts, cudaStream_t s, int *launches)
 {
     const int nitems = (g1 - g0) * a.bins.nbins;
     const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
-    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1);
-    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1);
+    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1, write_counts);
+    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1, write_counts);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -730,33 +732,32 @@ cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches)
     return launch_exclusive_scan(a.gbound, a.gprefix, a.ngroups, a.scan_tmp, s, launches);
 }
 
-#define HARM_PASS(L, A, B)                                              \
-    {                                                                   \
-        cudaError_t e = launch_harm<L, A, B>(a, g0, g1, s, launches);   \
-        if (e != cudaSuccess) return e;                                 \
+#define HARM_PASS(L, A, B)                                                      \
+    {                                                                           \
+        cudaError_t e = launch_harm<L, A, B>(a, g0, g1, (A) == 0, s, launches); \
+        if (e != cudaSuccess) return e;                                         \
     }
 
-// m-ranges per lmax.  Every pass re-reads the lists and gathers the candidates again (the L1 data pipe is ~70 % busy),
+// m-ranges per lmax.  Every pass walks the rows and gathers the candidates again (the L1 data pipe is ~70 % busy),
 // so fewer, fatter passes win: up to 44 accumulators run at 168 registers and 12 warps/SM, 45-65 at 255 registers and
 // 8 warps/SM (c2, lmax 10: four passes 46.3 ms, three 40.1 ms, two 37.1 ms for the pair stage).
 cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches)
 {
     const int ng = g1 - g0, nb = a.bins.nbins;
     if (ng <= 0) return cudaSuccess;
-    cudaError_t e = cudaMemsetAsync(a.pool_cursor, 0, sizeof(unsigned), s);
-    if (e != cudaSuccess) return e;
+    // the opt-in shared-memory limit is a per-kernel, process-wide attribute: set it once, to the most any plan asks for
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(k_fill<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (attr_err == cudaSuccess) attr_err = cudaFuncSetAttribute(k_fill<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    });
+    if (attr_err != cudaSuccess) return attr_err;
     const size_t smem = fill_smem_bytes(nb, nr_cap);
-    if (a.geom.periodic) {
-        e = cudaFuncSetAttribute(k_fill<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_fill<true><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
-    } else {
-        e = cudaFuncSetAttribute(k_fill<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_fill<false><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
-    }
+    if (a.geom.periodic) k_fill<true><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
+    else k_fill<false><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
     *launches += 1;
-    e = cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     switch (a.lmax) {
     case 0: HARM_PASS(0, 0, 0) break;

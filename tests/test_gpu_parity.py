@@ -6,6 +6,7 @@ element; the full-size configs (the launch configurations bench.py times) are ch
 (a_lm tiles and counts computed one by one by the oracle) and through closed-form properties.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -186,48 +187,134 @@ def test_bitwise_reproducible_and_host_entry(E):
 
 
 # ---- full-size configs, as bench.py launches them ------------------------------------------------------------------
-def _full_size_checks(E, oracle, name, nsample=12):
-    cfg = W.CONFIGS[name]
-    pos, w = W.make(cfg)
-    g = gpu_run(E, cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
-    nb, lmax, n = cfg.nbins, cfg.lmax, cfg.n
-    # sampled primaries: counts bit-exact, a_lm tiles to 1e-12
+# north_star: "GPU zeta matching the oracle within the stated tolerance on all five configs"; the paper's own standard
+# is agreement "to machine precision for all Lambda considered" (§5.2).  c1 is test_c1_full above.
+# c2, c3, c5: the oracle runs inside the test (about a minute each on the box's host cores); c4 (1.6e6 particles,
+# 2.5e10 pairs, ~20 oracle-minutes) compares with tests/golden/c4_oracle.npz, written by tests/golden/make_golden.py
+# from oracle/ + workloads/ only and guarded by the sha256 of the regenerated input.
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+_FULL = {}
+
+
+def full_oracle(oracle, name):
+    """oracle.zeta of a full-size config, computed once per test session"""
+    if name not in _FULL:
+        cfg = W.CONFIGS[name]
+        pos, w = W.make(cfg)
+        _FULL[name] = (pos, w, oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, want_prim_counts=True))
+    return _FULL[name]
+
+
+def _l0_identity(E, plan, cfg, z, wcounts):
+    """zeta_{0..0}^B = (4 pi)^{-(N-1)/2} / V  sum_i w_i prod_k n^w_i(b_k) / v_{b_k},  n^w_i(b) = sum_{j in b(i)} w_j
+    (Y_00 = (4 pi)^{-1/2}, C = 1).  wcounts = (w_i, n^w_i(b)) from a source other than zeta."""
+    wi, nw = wcounts
+    e = E.encore_get_bin_edges(plan.h, cfg.nbins)
+    vb = 4 * math.pi / 3 * (e[1:] ** 3 - e[:-1] ** 3)
+    V = cfg.box ** 3 if cfg.box > 0 else 1.0
+    lam, bins = plan.multiplets, plan.bin_tuples
+    i0 = [tuple(r) for r in lam].index(tuple([0] * lam.shape[1]))
+    a = nw / vb
+    ref = np.array([(wi * np.prod(a[:, list(B)], axis=1)).sum() for B in bins]) * (4 * math.pi) ** (-(cfg.order - 1) / 2) / V
+    assert np.abs(z[i0] - ref).max() <= 1e-10 * max(np.abs(ref).max(), np.abs(z).max())
+
+
+def _sampled_alm(E, oracle, g, cfg, pos, w, nsample):
     rng = np.random.default_rng(42)
-    for i in rng.choice(n, nsample, replace=False):
+    nb, lmax = cfg.nbins, cfg.lmax
+    for i in rng.choice(cfg.n, nsample, replace=False):
         a_o, cnt_o = oracle.alm(pos, w, cfg.box, cfg.rmin, cfg.rmax, nb, lmax, int(i))
         assert (g["prim_counts"][i] == cnt_o).all()
         a_g = E.encore_get_alm(g["plan"].h, int(i), nb, lmax)
         ref = np.stack([a_o[:, l * l + l + m] for l in range(lmax + 1) for m in range(l + 1)], axis=1)
         assert np.abs(a_g - ref).max() <= 1e-11 * np.abs(ref).max()
-    cid, nc = oracle.cell_ids(pos, cfg.box, cfg.rmax, g["sub"])
-    assert (g["cid"] == cid).all()
-    # properties that hold at any size
-    pc = g["prim_counts"].astype(np.float64)
-    assert (g["bin_counts"] == g["prim_counts"].sum(axis=0, dtype=np.uint64)).all()
-    lam = g["plan"].multiplets
-    bins = g["plan"].bin_tuples
-    z = g["zeta"]
-    assert np.isfinite(z).all()
-    if cfg.weights == "unit":
-        # l = 0 identity with integer counts: zeta_0..0^B = (4pi)^{-(N-1)/2}/V sum_i prod_k n_i(b_k)/v_{b_k}
-        e = E.encore_get_bin_edges(g["plan"].h, nb)
-        vb = 4 * math.pi / 3 * (e[1:] ** 3 - e[:-1] ** 3)
-        V = cfg.box ** 3 if cfg.box > 0 else 1.0
-        i0 = [tuple(r) for r in lam].index(tuple([0] * lam.shape[1]))
-        a = pc / vb
-        ref = np.array([np.prod(a[:, list(B)], axis=1).sum() for B in bins]) * (4 * math.pi) ** (-(cfg.order - 1) / 2) / V
-        assert np.abs(z[i0] - ref).max() <= 1e-11 * np.abs(ref).max()
-    g["plan"].close()
-    return g
 
 
+@pytest.mark.slow
 @pytest.mark.parametrize("name", ["c2", "c3", "c5"])
-def test_full_size_periodic_configs(E, oracle, name):
-    _full_size_checks(E, oracle, name)
+def test_full_size_zeta_matches_the_oracle(E, oracle, name):
+    """every element of zeta, every per-primary and global pair count and every cell id at the benchmarked size"""
+    cfg = W.CONFIGS[name]
+    pos, w, o = full_oracle(oracle, name)
+    g = gpu_run(E, cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+    assert (g["bin_counts"] == o["bin_counts"]).all()
+    assert (g["prim_counts"] == o["prim_counts"]).all()
+    cid, nc = oracle.cell_ids(pos, cfg.box, cfg.rmax, g["sub"])
+    assert list(nc) == g["nc"] and (g["cid"] == cid).all()
+    scale = np.abs(o["zeta"]).max()
+    err = np.abs(g["zeta"] - o["zeta"]).max() / scale
+    print(f"{name}: full-size zeta rel-to-max error {err:.3e} over {o['zeta'].size} elements, pairs {g['pairs']}")
+    assert err <= TOL
+    assert o["max_imag"] <= 1e-12 * scale
+    _sampled_alm(E, oracle, g, cfg, pos, w, 8)
+    if cfg.weights == "unit":   # l = 0 identity from the GPU's own integer counts
+        _l0_identity(E, g["plan"], cfg, g["zeta"], (np.ones(cfg.n), g["prim_counts"].astype(np.float64)))
+    g["plan"].close()
 
 
-def test_full_size_c4_cutsky(E, oracle):
-    _full_size_checks(E, oracle, "c4", nsample=6)
+@pytest.mark.slow
+def test_full_size_c4_cutsky_against_the_golden_oracle_run(E, oracle):
+    cfg = W.CONFIGS["c4"]
+    pos, w = W.make(cfg)
+    gold = np.load(os.path.join(GOLDEN, "c4_oracle.npz"))
+    assert str(gold["digest"]) == W.digest(pos, w), "tests/golden/c4_oracle.npz was written for other input bytes"
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+        E.encore_set_option(plan.h, "list_mb", 8192)          # several pair-stage super-steps, as on a fuller device
+        z = plan.compute(tp, tw)
+        torch.cuda.synchronize()
+        z = z.cpu().numpy()
+        assert E.encore_get_pair_steps(plan.h) >= 2
+        counts, pairs = E.encore_get_bin_counts(plan.h, cfg.nbins)
+        pc = torch.empty((cfg.n, cfg.nbins), dtype=torch.int32, device=dev)
+        E.encore_get_primary_counts(plan.h, pc)
+        g = {"plan": plan, "prim_counts": pc.cpu().numpy().astype(np.uint32)}
+        assert (counts == gold["bin_counts"]).all()
+        assert (counts == g["prim_counts"].sum(axis=0, dtype=np.uint64)).all()
+        scale = np.abs(gold["zeta"]).max()
+        err = np.abs(z - gold["zeta"]).max() / scale
+        print(f"c4: full-size zeta rel-to-max error {err:.3e} over {z.size} elements, pairs {pairs}")
+        assert err <= TOL
+        _sampled_alm(E, oracle, g, cfg, pos, w, 4)
+
+
+@pytest.mark.slow
+def test_full_size_c3_sharded_over_primaries(E, oracle):
+    """encore_compute_shard at the benchmarked size: three shards, added in rank order, against the full oracle run"""
+    cfg = W.CONFIGS["c3"]
+    pos, w, o = full_oracle(oracle, "c3")
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+        total = np.zeros((plan.n_lambda, plan.n_b))
+        counts = np.zeros(cfg.nbins, dtype=np.uint64)
+        for k in range(3):
+            total += plan.compute_shard(tp, tw, k, 3).cpu().numpy()
+            counts += E.encore_get_bin_counts(plan.h, cfg.nbins)[0]
+    assert (counts == o["bin_counts"]).all()
+    assert np.abs(total - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+
+
+def test_weighted_l0_identity_reduced_c3_c4(E, oracle):
+    """the l = 0 identity WITH weights (c3's w in [0.8,1.2], c4's data-minus-random): weighted neighbour counts from a
+    numpy all-pairs histogram, nothing from zeta's own path"""
+    for cfg in (W.scaled(W.CONFIGS["c3"], box=360.0, n=4000, grid=64), W.scaled(W.CONFIGS["c4"], n=4000)):
+        pos, w = W.make(cfg)
+        e = np.linspace(cfg.rmin, cfg.rmax, cfg.nbins + 1)
+        nw = np.zeros((cfg.n, cfg.nbins))
+        for i0 in range(0, cfg.n, 500):
+            d = pos[:, None, :] - pos[:, i0:i0 + 500, None]
+            if cfg.box > 0:
+                d -= cfg.box * np.round(d / cfg.box)
+            r = np.sqrt((d ** 2).sum(axis=0))
+            b = np.floor((r - cfg.rmin) / (cfg.rmax - cfg.rmin) * cfg.nbins).astype(int)
+            ok = (r > 0) & (r >= cfg.rmin) & (r < cfg.rmax)
+            for k in range(cfg.nbins):
+                nw[i0:i0 + 500, k] = ((ok & (b == k)) * w[None, :]).sum(axis=1)
+        g = gpu_run(E, cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, want=("zeta",))
+        _l0_identity(E, g["plan"], cfg, g["zeta"], (w, nw))
+        g["plan"].close()
 
 
 # ---- sharding over primaries (SURVEY.md §8(e)): the shards' partial sums add up to the estimator ------------------
@@ -302,21 +389,19 @@ def test_allparity_matches_the_oracle(E, oracle, order, nbins, lmax, box):
     assert np.abs(expect[par]).max() > 1e-6 * scale if order > 3 else True   # the odd part is not trivially zero
 
 
-def test_list_budget_super_steps(E, oracle, monkeypatch):
-    """a 1 MB list budget forces the pair stage through many super-steps: same bits as the single-step run"""
+def test_list_budget_super_steps(E, oracle):
+    """a 1 MiB row budget forces the pair stage through many super-steps: same bits as the single-step run"""
     cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=7000, grid=64)
     pos, w = W.make(cfg)
     dev = torch.device("cuda:0")
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     out = {}
-    for tag, mb in [("one", None), ("many", "1")]:
-        if mb is None:
-            monkeypatch.delenv("ENCORE_LIST_MB", raising=False)
-        else:
-            monkeypatch.setenv("ENCORE_LIST_MB", mb)
+    for tag, mb in [("one", 0), ("many", 1)]:
         with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+            E.encore_set_option(plan.h, "list_mb", mb)
             z = plan.compute(tp, tw)
             torch.cuda.synchronize()
+            assert E.encore_get_status(plan.h) == E.OK
             counts, pairs = E.encore_get_bin_counts(plan.h, cfg.nbins)
             out[tag] = (z.cpu().numpy(), counts, E.encore_get_pair_steps(plan.h))
     assert out["one"][2] == 1 and out["many"][2] > 3
@@ -325,3 +410,35 @@ def test_list_budget_super_steps(E, oracle, monkeypatch):
     o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
     assert (out["many"][1] == o["bin_counts"]).all()
     assert np.abs(out["many"][0] - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+
+
+def test_options_and_thin_axis(E, oracle):
+    """encore_set_option validation; a planar catalogue with 1e-12 noise along z (r_max * inv overflowed)"""
+    with E.Plan(3, 1.0, 20.0, 3, 2, 0.0) as plan:
+        for key, val in [("nope", 1), ("sub_yz", 9), ("sub_x", -1), ("list_mb", -5), ("generic_contract", 2)]:
+            with pytest.raises(E.EncoreError) as ei:
+                E.encore_set_option(plan.h, key, val)
+            assert ei.value.status == E.EINVAL
+    rng = np.random.default_rng(77)
+    n = 500
+    pos = np.ascontiguousarray(np.stack([rng.uniform(0, 80, n), rng.uniform(0, 80, n), 5.0 + 1e-12 * rng.uniform(-1, 1, n)]))
+    w = rng.uniform(0.5, 1.5, n)
+    check_full(E, oracle, 3, pos, w, 0.0, 2.0, 30.0, 4, 3)
+    pos2 = np.ascontiguousarray(pos[[2, 0, 1]])          # thin along x, the fine axis
+    check_full(E, oracle, 4, pos2, w, 0.0, 2.0, 30.0, 4, 2)
+    # the generic contraction through the option, and explicit grid subdivisions
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=3000, grid=64)
+    pos, w = W.make(cfg)
+    o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+    dev = torch.device("cuda:0")
+    for opts in [{"generic_contract": 1}, {"sub_yz": 2, "sub_x": 5}, {"sub_yz": 5}]:
+        with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+            for k, v in opts.items():
+                E.encore_set_option(plan.h, k, v)
+            z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+            assert E.encore_get_status(plan.h) == E.OK
+            if "sub_yz" in opts:
+                assert E.encore_get_grid(plan.h)[1][1] == opts["sub_yz"]
+            counts, _ = E.encore_get_bin_counts(plan.h, cfg.nbins)
+        assert (counts == o["bin_counts"]).all()
+        assert np.abs(z - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
