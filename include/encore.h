@@ -153,6 +153,12 @@ int encore_get_launch_count(const encore_plan_t *plan);
 /* candidate pairs tested in step a3 by the last compute (>= accepted pairs), for the rejected-pair flop term */
 int encore_get_candidate_pairs(const encore_plan_t *plan, uint64_t *out /* HOST */);
 
+/* lane utilisation of step a4 in the last compute: k_harm walks the pairs of 32 primaries in lock step, one warp per
+ * (group of 32 primaries, bin); `executed` = lock-step pair steps summed over warps, `ideal` = sum over warps of the
+ * largest pair count among the warp's primaries (what a perfectly packed schedule would execute).  Both read 0 unless
+ * the library was built with -DENCORE_HARM_STATS (the counters cost a few percent of k_harm). */
+int encore_get_harm_steps(const encore_plan_t *plan, uint64_t *executed /* HOST */, uint64_t *ideal /* HOST */);
+
 /* Dependent-DFMA-chain micro-benchmark on the current device: achieved fp64 FLOP/s (FMA = 2) with every SM busy.
  * The ALU roofline denominator reported by bench.py beside the derived 148 SM x 64 lanes x 2 x f_clk. */
 int encore_measure_fp64_peak(double *flops_per_s /* HOST */, void *cuda_stream);

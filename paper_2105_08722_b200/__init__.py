@@ -29,7 +29,7 @@ SYMBOLS = [
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
     "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
-    "encore_get_stage_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs",
+    "encore_get_stage_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs", "encore_get_harm_steps",
     "encore_measure_fp64_peak", "encore_strerror", "encore_last_cuda_error",
 ]
 
@@ -80,6 +80,7 @@ def lib():
     L.encore_get_launch_count.argtypes = [vp]
     L.encore_get_candidate_pairs.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.encore_measure_fp64_peak.argtypes = [dp, vp]
+    L.encore_get_harm_steps.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.encore_strerror.argtypes = [C.c_int]
     L.encore_strerror.restype = C.c_char_p
     L.encore_last_cuda_error.argtypes = []
@@ -255,6 +256,12 @@ def encore_get_candidate_pairs(plan) -> int:
     v = C.c_uint64()
     _check(lib().encore_get_candidate_pairs(plan, C.byref(v)))
     return int(v.value)
+
+
+def encore_get_harm_steps(plan):
+    ex, ideal = C.c_uint64(), C.c_uint64()
+    _check(lib().encore_get_harm_steps(plan, C.byref(ex), C.byref(ideal)))
+    return int(ex.value), int(ideal.value)
 
 
 def encore_measure_fp64_peak(cuda_stream: int = 0) -> float:

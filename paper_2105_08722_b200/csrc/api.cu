@@ -46,7 +46,7 @@ struct encore_plan_s {
     size_t list_budget_bytes = (size_t)32 << 30;
     bool list_budget_set = false;   // option "list_mb" given: use it as is
     int pair_steps = 0;
-    double *pinned = nullptr; // 8 doubles: bbox[6], flags as 2 ints in [6], internal-error flag as int in [7]
+    double *pinned = nullptr; // 16 doubles: bbox[6], flags as 2 ints in [6], internal-error flag as int in [7], padding particle [8..11]
     // state of the last compute
     bool have = false;
     int64_t n = 0;
@@ -118,7 +118,7 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
         CU(cudaStreamSynchronize(s));
     }
     CU(cudaStreamSynchronize(s)); // the staging vectors die at return
-    CU(cudaMallocHost((void **)&P->pinned, 8 * sizeof(double)));
+    CU(cudaMallocHost((void **)&P->pinned, 16 * sizeof(double)));
     P->uploaded = true;
     return ENCORE_OK;
 }
@@ -227,7 +227,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->scan_tmp.ensure(sizeof(int) * (std::max<size_t>(std::max<size_t>((size_t)G.ncell, (size_t)ngmax), 4000000) / 2048 + 8)));
     CU(P->tmp_idx.ensure(sizeof(int) * n));
     CU(P->sorted_idx.ensure(sizeof(int) * n));
-    CU(P->pos4.ensure(sizeof(double4) * n));
+    CU(P->pos4.ensure(sizeof(double4) * ((size_t)n + 1)));   // + the padding particle
     CU(P->groups.ensure(sizeof(int) * (size_t)G.npencil));
     CU(P->group_start.ensure(sizeof(int) * ((size_t)G.npencil + 1)));
     CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
@@ -249,7 +249,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout));
     CU(P->gweights.ensure(sizeof(double) * (size_t)ngmax * 32));
     CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
-    CU(P->cand.ensure(sizeof(unsigned long long)));
+    CU(P->cand.ensure(3 * sizeof(unsigned long long)));   // candidate pairs, k_harm steps, k_harm ideal steps
 
     TRY(record(P, 0, s));
     // ---- a1: cell ids + histogram -----------------------------------------------------------------------------
@@ -266,6 +266,24 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     // ---- a3 + a4: pair stage -----------------------------------------------------------------------------------
     PairArgs pa{};
     pa.pos4 = P->pos4.as<double4>();
+    pa.npart = (int)n;
+    {   // padding particle pos4[n]: weight 0, a few box sizes away from everything (k_harm's idle lanes add exact zeros)
+        double far[3], r2 = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            if (G.periodic) { far[a] = 3.0 * T.box; r2 += 9.0 * T.box * T.box; }
+            else {
+                const double ext = P->pinned[3 + a] - P->pinned[a];
+                const double emax = std::max(std::max(P->pinned[3] - P->pinned[0], P->pinned[4] - P->pinned[1]), P->pinned[5] - P->pinned[2]);
+                const double off = 2.0 * (emax + T.rmax);
+                far[a] = P->pinned[3 + a] + off;
+                r2 += (ext + off) * (ext + off);
+            }
+        }
+        // (the bounding box in pinned[0..5] was read above; the slots 8..11 are only written here, after that synchronise)
+        P->pinned[8] = far[0]; P->pinned[9] = far[1]; P->pinned[10] = far[2]; P->pinned[11] = 0.0;
+        pa.pad_r2max = r2;
+        CU(cudaMemcpyAsync(P->pos4.as<double4>() + n, P->pinned + 8, sizeof(double4), cudaMemcpyHostToDevice, s));
+    }
     pa.cell_start = P->cell_start.as<int>();
     pa.group_start = P->group_start.as<int>();
     pa.geom = G;
@@ -303,7 +321,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         P->h_gprefix_cap = (size_t)ngmax + 2;
     }
     int g_begin = 0, g_end = 0, ngroups_total = 0;
-    CU(cudaMemsetAsync(P->cand.p, 0, sizeof(unsigned long long), s));
+    CU(cudaMemsetAsync(P->cand.p, 0, 3 * sizeof(unsigned long long), s));
     CU(cudaMemsetAsync(P->errflag.p, 0, sizeof(int), s));
     CU(launch_pair_bounds(pa, s, &P->launches));
     // second small device->host read: candidate words per group (prefix) and the number of groups -> super-steps
@@ -698,6 +716,17 @@ int encore_get_candidate_pairs(const encore_plan_t *P, uint64_t *out)
     CU(cudaMemcpyAsync(&h, P->cand.p, sizeof(h), cudaMemcpyDeviceToHost, P->stream));
     CU(cudaStreamSynchronize(P->stream));
     *out = h;
+    return ENCORE_OK;
+}
+
+int encore_get_harm_steps(const encore_plan_t *P, uint64_t *executed, uint64_t *ideal)
+{
+    if (!P || !executed || !ideal) return ENCORE_EINVAL;
+    if (!P->have) return ENCORE_ESTATE;
+    unsigned long long h[3] = {0, 0, 0};
+    CU(cudaMemcpyAsync(h, P->cand.p, sizeof(h), cudaMemcpyDeviceToHost, P->stream));
+    CU(cudaStreamSynchronize(P->stream));
+    *executed = h[1]; *ideal = h[2];
     return ENCORE_OK;
 }
 

@@ -49,7 +49,9 @@ cudaError_t launch_pencil_groups(const int *cell_start, GridGeom g, int *groups_
 
 // ---- pair.cu --------------------------------------------------------------------------------------------
 struct PairArgs {
-    const double4 *pos4;        // cell-sorted {x,y,z,w}
+    const double4 *pos4;        // cell-sorted {x,y,z,w}; entry [npart] is the padding particle (weight 0, far away)
+    int npart;
+    double pad_r2max;           // bound on the squared distance of the padding particle from any particle
     const int *cell_start;      // [ncell+1]
     const int *group_start;     // [npencil+1]; group_start[npencil] = number of groups
     GridGeom geom;

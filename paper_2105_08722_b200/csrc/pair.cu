@@ -48,8 +48,11 @@ namespace {
 #define ENCORE_HARM_WARPS 4
 #endif
 constexpr int kHarmWarps = ENCORE_HARM_WARPS;       // k_harm: independent warps (items) per CTA
-constexpr int kQueue = 16;                          // k_harm: (mask, descriptor) records queued per lane
-constexpr int kStageRows = 16;                      // k_harm: rows per cp.async chunk (two chunks in flight)
+#ifndef ENCORE_HARM_QUEUE
+#define ENCORE_HARM_QUEUE 32
+#endif
+constexpr int kQueue = ENCORE_HARM_QUEUE;           // k_harm: (mask, descriptor) records queued per lane (power of two)
+constexpr int kStageRows = 8;                       // k_harm: rows per cp.async chunk (two chunks in flight)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
 constexpr unsigned kIdxMask = 0x3ffffffu;
@@ -102,17 +105,16 @@ __device__ __forceinline__ void accumulate(double (&acc)[ncomp_range(LMAX, MLO, 
     }
 }
 
-// 1/sqrt(a) to full double precision from the fp32 approximation y0 (relative error <= 2^-21.4 including the
-// rounding of a to fp32) and ONE third-order step: with e = 1 - a y0^2, a^-1/2 = y0 (1 - e)^-1/2 =
-// y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...), truncation 5/16 |e|^3 < 2^-62.  5 fp64 operations instead of the
-// library routine's ~10; arguments outside fp32's comfortable range take the library path.
+// 1/sqrt(a) to full double precision from the hardware seed y0 = rsqrt.approx.f64 (MUFU.RSQ64H: works on the upper
+// word of the double, relative error below 2^-20) and ONE third-order step: with e = 1 - a y0^2,
+// a^-1/2 = y0 (1 - e)^-1/2 = y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...), truncation 5/16 |e|^3 < 2^-58.
+// 5 fp64 operations and no conversions.  The seed flushes subnormals and has no special cases: k_harm checks the
+// edges of the item's bin once (every pair of the item has its r^2 between them) and takes the library routine for
+// bins that reach down to 0 or beyond 1e290.
 __device__ __forceinline__ double rsqrt_pair(double a)
 {
-    const float af = __double2float_rn(a);
-    if (!(af > 1e-30f && af < 1e30f)) return rsqrt(a);
-    float yf;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"(af));
-    const double y0 = (double)yf;
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(a));
     const double t = a * y0;
     const double e = fma(-t, y0, 1.0);
     const double p = fma(0.375, e, 0.5);
@@ -283,11 +285,11 @@ __global__ void __launch_bounds__(128) k_group_bound(PairArgs a)
 // ==========================================================================================================
 // k_fill: a3.  One warp (= one CTA) per group.
 // ==========================================================================================================
-// dynamic shared memory: cand[34] float4 | sp[96] double | e2[nb+1] double | masks[nb][32] u32 |
+// dynamic shared memory: cand[36] float4 | sp[96] double | e2[nb+1] double | masks[nb+1][32] u32 |
 //                        rng_start[nr_cap] | rng_len[nr_cap] | rng_woff[nr_cap+1]
 __host__ __device__ inline size_t fill_smem_bytes(int nb, int nr_cap)
 {
-    return 34 * 16 + 96 * 8 + (size_t)((nb + 2) & ~1) * 8 + (size_t)nb * 32 * 4 + (size_t)(3 * nr_cap + 4) * 4;
+    return 36 * 16 + 96 * 8 + (size_t)((nb + 2) & ~1) * 8 + (size_t)(nb + 1) * 32 * 4 + (size_t)(3 * nr_cap + 4) * 4;
 }
 
 template <bool PERIODIC>
@@ -301,10 +303,10 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
 
     extern __shared__ __align__(16) unsigned char fill_smem[];
     float4 *cand = reinterpret_cast<float4 *>(fill_smem);
-    double *sp = reinterpret_cast<double *>(cand + 34);
+    double *sp = reinterpret_cast<double *>(cand + 36);
     double *e2 = sp + 96;
-    unsigned *masks = reinterpret_cast<unsigned *>(e2 + ((nb + 2) & ~1));
-    int *rng_start = reinterpret_cast<int *>(masks + nb * 32);
+    unsigned *masks = reinterpret_cast<unsigned *>(e2 + ((nb + 2) & ~1)); // row nb takes the bits of rejected candidates
+    int *rng_start = reinterpret_cast<int *>(masks + (nb + 1) * 32);
     int *rng_len = rng_start + nr_cap;
     int *rng_woff = rng_len + nr_cap;
 
@@ -316,7 +318,6 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     a.gweights[(size_t)g * 32 + lane] = lane < cnt ? mine.w : 0.0;
     if (lane <= nb) e2[lane] = a.bins.e2[lane];
     for (int b = 0; b < nb; ++b) masks[b * 32 + lane] = 0u;
-    if (lane == 0) cand[32] = make_float4(1e18f, 1e18f, 1e18f, 0.f); // filler of the 4-wide test blocks: never a hit
     // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
     const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
 
@@ -364,6 +365,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     unsigned *rows_g = a.rows + wbase * 32;
     unsigned *desc_g = a.rowdesc + wbase;
     int rowcnt = 0;                     // lane b holds the number of rows written for bin b
+    const unsigned lt_mask = (1u << lane) - 1u;
     unsigned long long kept = 0ull;
 
     // words are read one ahead: lane = candidate
@@ -411,22 +413,22 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
         if (PERIODIC && fast && __any_sync(kFull, keep && code != wcode)) { // excluded by DESIGN.md §5.3
             if (lane == 0) *a.err_flag = 1;
         }
-        cand[lane] = cf;
+        // survivors compacted to the front of cand[] (.w = position in the word), padded to a multiple of four
+        const int nk = __popc(km);
+        if (keep) cand[__popc(km & lt_mask)] = make_float4(cf.x, cf.y, cf.z, __int_as_float(lane));
+        if (lane < 4) cand[nk + lane] = make_float4(1e18f, 1e18f, 1e18f, __int_as_float(0)); // never a hit
         __syncwarp();
-        kept += (unsigned long long)__popc(km);
+        kept += (unsigned long long)nk;
         if (fast) {
-            unsigned rem = km;
 #pragma unroll 1
-            while (rem) {
-                // four independent tests (instruction-level parallelism) on the next four surviving candidates
+            for (int q0 = 0; q0 < nk; q0 += 4) {
+                // four independent tests (instruction-level parallelism)
+                unsigned codeb[4], bitv[4];
                 int cpos[4];
-                unsigned codeb[4];
                 bool ok[4], am[4];
 #pragma unroll
                 for (int cc = 0; cc < 4; ++cc) {
-                    cpos[cc] = rem ? __ffs(rem) - 1 : 32;
-                    rem &= rem - 1u;
-                    const float4 q = cand[cpos[cc]];
+                    const float4 q = cand[q0 + cc];
                     const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
                     const float t = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), 1e-30f); // t = 0: r = 0 -> exact path
                     float rinv;
@@ -440,19 +442,21 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
                     codeb[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
                     ok[cc] = sure && codeb[cc] < (unsigned)nb;
                     am[cc] = !sure;                                  // ~2 du of all pairs, in range or not
+                    cpos[cc] = __float_as_int(q.w);
+                    bitv[cc] = 1u << cpos[cc];
                 }
                 if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
+                    // branch-free: a rejected candidate sets its bit in the spare row nb
 #pragma unroll
-                    for (int cc = 0; cc < 4; ++cc)
-                        if (ok[cc]) atomicOr(&masks[codeb[cc] * 32 + lane], 1u << cpos[cc]);
+                    for (int cc = 0; cc < 4; ++cc) atomicOr(&masks[(ok[cc] ? codeb[cc] : (unsigned)nb) * 32 + lane], bitv[cc]);
                 } else {
                     // some pair is within the error margin of a bin edge (~1e-4 of the pairs): exact decision
 #pragma unroll
                     for (int cc = 0; cc < 4; ++cc) {
-                        if (ok[cc]) atomicOr(&masks[codeb[cc] * 32 + lane], 1u << cpos[cc]);
-                        else if (am[cc] && codeb[cc] + 1u < (unsigned)nb + 2u && cpos[cc] < 32) {
+                        if (ok[cc]) atomicOr(&masks[codeb[cc] * 32 + lane], bitv[cc]);
+                        else if (am[cc] && codeb[cc] + 1u < (unsigned)nb + 2u && q0 + cc < nk) {
                             const unsigned cx = classify_exact<PERIODIC>(a.pos4[jbase + cpos[cc]], sp, lane, e2, nb, G.box, G.half, rmin_f, invw_f);
-                            if (cx != kNoHit) atomicOr(&masks[cx * 32 + lane], 1u << cpos[cc]);
+                            if (cx != kNoHit) atomicOr(&masks[cx * 32 + lane], bitv[cc]);
                         }
                     }
                 }
@@ -508,6 +512,10 @@ __device__ __forceinline__ void cp_async4(unsigned *smem_dst, const unsigned *gs
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void cp_async16(unsigned *smem_dst, const unsigned *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -515,116 +523,142 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // MODE 0: open geometry; 1: periodic, image carried by the row descriptor; 2: periodic, image decided per pair
 // mtab (MODE 1): shared memory [axis][image code][thread] = x_i + {-L, 0, +L}: x_j - (x_i -/+ L) is the minimal image
 // D: candidates gathered ahead of the one being accumulated.  Returns the number of pairs this lane accumulated.
-// qm/qd: this warp's record queue [kQueue][32]; stm: row staging [2][kStageRows][32]; std_: descriptors [2][32].
-template <int LMAX, int MLO, int MHI, int MODE, int D>
+// q: this warp's record queue [kQueue][32] of (mask, descriptor); stm: row staging [2][kStageRows][32];
+// std_: descriptors [2][kStageRows].
+// padent: entry of the padding particle pos4[n] (weight 0, far from everything): a lane with nothing left adds exact zeros.
+// CAREFUL: the bin reaches outside fp32's comfortable range for r^2 (r_min = 0, or extreme units): library rsqrt.
+struct HarmStats { unsigned steps; };
+
+template <int LMAX, int MLO, int MHI, int MODE, int D, bool CAREFUL>
 __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ rows,
-                                              const unsigned *__restrict__ rdesc, int nrows, bool active, unsigned *qm,
-                                              unsigned *qd, unsigned *stm, unsigned *std_, const double4 *__restrict__ pos4,
-                                              const double4 &me, const double *mtab, double box, double half, int lane)
+                                              const unsigned *__restrict__ rdesc, int nrows, bool active, uint2 *q,
+                                              unsigned *stm, unsigned *std_, const double4 *__restrict__ pos4,
+                                              const double4 &me, const double *mtab, double box, double half, int lane,
+                                              unsigned padent, HarmStats &st)
 {
-    static_assert(D >= 1 && D <= 4, "the image-code fifo holds four bytes");
-    // ---- rows -> shared memory, two chunks in flight (every chunk slot commits one cp.async group, empty or not) ----
+    static_assert(D >= 1 && D <= 4 && 4 % D == 0, "four steps per loop trip use the D gather slots in turn");
+    // ---- rows -> shared memory: a ring of 2 chunks of kStageRows rows, both in flight (every chunk slot commits one
+    // cp.async group, empty or not).  A chunk is kStageRows * 128 contiguous bytes: 16 bytes per lane and copy.
     auto issue_chunk = [&](int c) {
         const int r0 = c * kStageRows;
         if (r0 < nrows) {
             const int nr = min(kStageRows, nrows - r0);
-            unsigned *dst = stm + (c & 1) * kStageRows * 32 + lane;
-            const unsigned *src = rows + (size_t)r0 * 32 + lane;
-            for (int k = 0; k < nr; ++k) cp_async4(dst + k * 32, src + (size_t)k * 32);
-            if (lane < nr) cp_async4(std_ + (c & 1) * 32 + lane, rdesc + r0 + lane);
+            unsigned *dst = stm + (c & 1) * kStageRows * 32;
+            const unsigned *src = rows + (size_t)r0 * 32;
+#pragma unroll
+            for (int j = 0; j < kStageRows / 4; ++j) {
+                const int w = j * 128 + lane * 4;              // word offset inside the chunk; row = w / 32
+                if ((w >> 5) < nr) cp_async16(dst + w, src + w);
+            }
+            if (lane < nr) cp_async4(std_ + (c & 1) * kStageRows + lane, rdesc + r0 + lane);
         }
         cp_async_commit();
     };
     issue_chunk(0);
     issue_chunk(1);
     int rows_done = 0;
-    unsigned head = 0u, tail = 0u;      // lane-private queue cursors
+    // lane-private queue cursors as byte offsets into the lane's column of q (stride 256 bytes per record)
+    constexpr unsigned kQBytes = kQueue * 256u;
+    unsigned head = 0u, tail = 0u, level = 0u;
+    char *const qcol = reinterpret_cast<char *>(q + lane);
     int avail = 0;                      // pairs queued and not yet generated (bits of cur + bits of the queued masks)
     unsigned npairs = 0u;
-    unsigned cur = 0u, base = 0u, img = 0u;
+    unsigned cur = 0u, dsc = 0u;        // record being walked: remaining bits, descriptor
     bool drained = false;
     // push rows while every lane has room for one more record; returns the number of steps to run next (0: finished)
     auto refill = [&]() -> int {
-        int room = kQueue - __reduce_max_sync(kFull, (int)(tail - head));
+        int room = kQueue - __reduce_max_sync(kFull, (int)level);
         while (room > 0 && rows_done < nrows) {
-            const int k = rows_done % kStageRows, buf = (rows_done / kStageRows) & 1;
-            if (k == 0) { cp_async_wait<1>(); __syncwarp(); }
-            const unsigned m = stm[(buf * kStageRows + k) * 32 + lane];
-            const unsigned d = std_[buf * 32 + k];
-            if (m) {
-                const unsigned slot = (tail & (kQueue - 1)) * 32 + lane;
-                qm[slot] = m; qd[slot] = d;
-                ++tail;
-                const int pc = __popc(m);
-                avail += pc; npairs += (unsigned)pc;
+            const int k0 = rows_done & (kStageRows - 1);
+            if (k0 == 0) { cp_async_wait<1>(); __syncwarp(); }
+            const int nr = min(min(room, nrows - rows_done), kStageRows - k0);
+            const unsigned *ps = stm + (rows_done & (2 * kStageRows - 1)) * 32 + lane;
+            const unsigned *pd = std_ + (rows_done & (2 * kStageRows - 1));
+            for (int i = 0; i < nr; ++i) {
+                const unsigned m = ps[i * 32];
+                const unsigned d = pd[i];
+                if (m) {
+                    *reinterpret_cast<uint2 *>(qcol + tail) = make_uint2(m, d);
+                    tail = (tail + 256u) & (kQBytes - 1u);
+                    ++level;
+                    const int pc = __popc(m);
+                    avail += pc; npairs += (unsigned)pc;
+                }
             }
-            ++rows_done; --room;
-            if (rows_done % kStageRows == 0) { __syncwarp(); issue_chunk(rows_done / kStageRows + 1); }
+            rows_done += nr; room -= nr;
+            if ((rows_done & (kStageRows - 1)) == 0) { __syncwarp(); issue_chunk(rows_done / kStageRows + 1); }
         }
+        int s;
         if (rows_done < nrows) { // a starving lane waits for rows: run while every active lane has pairs (at least 4 steps)
-            const int s = __reduce_min_sync(kFull, active ? avail : INT_MAX);
-            return s >= 4 ? (s & ~3) : 4;
+            s = __reduce_min_sync(kFull, active ? avail : INT_MAX);
+            s = s >= 4 ? (s & ~3) : 4;
+        } else {
+            s = __reduce_max_sync(kFull, avail);
+            if (s > 0) s = (s + 3) & ~3;
+            else if (drained) s = 0;
+            else { drained = true; s = 4; } // the last D gathers are still in flight
         }
-        const int s = __reduce_max_sync(kFull, avail);
-        if (s > 0) return (s + 3) & ~3;
-        if (drained) return 0;
-        drained = true;                 // the last D gathers are still in flight
-        return 4;
+#ifdef ENCORE_HARM_STATS
+        st.steps += (unsigned)s;
+#endif
+        return s;
     };
-    // next pair of this lane: sorted index + image code (0x80: padding, nothing left)
-    auto gen = [&](unsigned &idx, unsigned &code) {
-        if (cur == 0u && head != tail) {
-            const unsigned slot = (head & (kQueue - 1)) * 32 + lane;
-            cur = qm[slot];
-            const unsigned d = qd[slot];
-            ++head;
-            base = d & kIdxMask; img = d >> 26;
+    // next pair of this lane as an entry: sorted index | image codes << 26 (padent: nothing left)
+    auto gen = [&]() -> unsigned {
+        if (cur == 0u && level != 0u) {
+            const uint2 rec = *reinterpret_cast<const uint2 *>(qcol + head);
+            cur = rec.x; dsc = rec.y;
+            head = (head + 256u) & (kQBytes - 1u);
+            --level;
         }
         const bool pad = cur == 0u;
         const unsigned bit = (unsigned)(__ffs((int)cur) - 1);
         cur &= cur - 1u;
-        idx = pad ? 0u : base + bit;    // padding reads particle 0 (always valid memory); its weight is forced to 0
-        code = pad ? 0x80u : img;
-        avail -= pad ? 0 : 1;
+        if (!pad) --avail;
+        return pad ? padent : dsc + bit; // the word's first index + bit stays below 2^26
     };
 
     int S = refill();
-    if (S == 0 || (drained && S == 4)) { cp_async_wait<0>(); return 0u; } // no pair in this item
+    if (S == 0 || (drained && S == 4)) { // no pair in this item
+        cp_async_wait<0>();
+#ifdef ENCORE_HARM_STATS
+        st.steps = 0u;
+#endif
+        return 0u;
+    }
     Raw r[D];
-    unsigned fifo = 0u;                 // image codes of the D gathers in flight, newest in the low byte
+    unsigned ent[D];
 #pragma unroll
     for (int d = 0; d < D; ++d) {
-        unsigned idx, code;
-        gen(idx, code);
-        r[d] = gather(pos4, idx);
-        fifo = (fifo << 8) | code;
+        ent[d] = gen();
+        r[d] = gather(pos4, ent[d] & kIdxMask);
     }
+    // MODE 1: byte address of this thread's column of mtab; the image code of an axis selects one of three rows
+    const char *const mcol = reinterpret_cast<const char *>(mtab);
+    constexpr unsigned kRowB = kHarmWarps * 32 * 8;   // bytes per mtab row (power of two: 1024 at 4 warps)
+    static_assert((kRowB & (kRowB - 1)) == 0, "mtab rows are selected by or-ing the code into the address");
     do {
         for (int s = 0; s < S; s += 4) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const Raw r0 = r[u % D];
-                const unsigned c0 = (fifo >> (8 * (D - 1))) & 0xffu;
-                unsigned idx, code;
-                gen(idx, code);
-                r[u % D] = gather(pos4, idx); // D candidates ahead
-                fifo = (fifo << 8) | code;
+                // everything that reads slot u first, so that the next gather can land in the same registers
                 double dx, dy, dz;
                 if (MODE == 1) {
-                    const unsigned kx = c0 & 3u, ky = (c0 >> 2) & 3u, kz = (c0 >> 4) & 3u;
-                    dx = r0.xy.x - mtab[(0 * 3 + kx) * (kHarmWarps * 32)];
-                    dy = r0.xy.y - mtab[(1 * 3 + ky) * (kHarmWarps * 32)];
-                    dz = r0.zw.x - mtab[(2 * 3 + kz) * (kHarmWarps * 32)];
+                    const unsigned c0 = ent[u % D];
+                    // rows 0..2 = x, 4..6 = y, 8..10 = z (a fourth, unused row per axis keeps the stride a power of two)
+                    dx = r[u % D].xy.x - *reinterpret_cast<const double *>(mcol + (((c0 >> 26) & 3u) * kRowB));
+                    dy = r[u % D].xy.y - *reinterpret_cast<const double *>(mcol + 4 * kRowB + (((c0 >> 28) & 3u) * kRowB));
+                    dz = r[u % D].zw.x - *reinterpret_cast<const double *>(mcol + 8 * kRowB + ((c0 >> 30) * kRowB));
                 } else {
-                    dx = sep<MODE == 2>(r0.xy.x, me.x, box, half);
-                    dy = sep<MODE == 2>(r0.xy.y, me.y, box, half);
-                    dz = sep<MODE == 2>(r0.zw.x, me.z, box, half);
+                    dx = sep<MODE == 2>(r[u % D].xy.x, me.x, box, half);
+                    dy = sep<MODE == 2>(r[u % D].xy.y, me.y, box, half);
+                    dz = sep<MODE == 2>(r[u % D].zw.x, me.z, box, half);
                 }
-                const bool pad = (c0 & 0x80u) != 0u;
-                if (pad) { dx = 1.0; dy = 0.0; dz = 0.0; }
-                const double wj = pad ? 0.0 : r0.zw.y;
+                const double wj = r[u % D].zw.y;
+                ent[u % D] = gen();
+                r[u % D] = gather(pos4, ent[u % D] & kIdxMask); // D candidates ahead
                 const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
-                const double rinv = rsqrt_pair(r2s);
+                const double rinv = CAREFUL ? rsqrt(r2s) : rsqrt_pair(r2s);
                 accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
             }
         }
@@ -634,13 +668,23 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
     return npairs;
 }
 
+// dynamic shared memory of k_harm per CTA: mtab[12][threads] double | queue[warps][kQueue][32] uint2 |
+//                                          stage[warps][2][kStageRows][32] u32 | stage descriptors[warps][2][kStageRows] u32
+constexpr size_t harm_smem_bytes(bool periodic)
+{
+    return (periodic ? (size_t)12 * kHarmWarps * 32 * 8 : 0) + (size_t)kHarmWarps * kQueue * 32 * 8 +
+           (size_t)kHarmWarps * 2 * kStageRows * 32 * 4 + (size_t)kHarmWarps * 2 * kStageRows * 4;
+}
+
 template <int LMAX, int MLO, int MHI, bool PERIODIC>
 __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3) k_harm(PairArgs a, int g0, int g1, int write_counts)
 {
     constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH;
-    __shared__ double mtab[PERIODIC ? 9 * kHarmWarps * 32 : 1];
-    __shared__ unsigned s_qm[kHarmWarps][kQueue * 32], s_qd[kHarmWarps][kQueue * 32];
-    __shared__ unsigned s_stm[kHarmWarps][2 * kStageRows * 32], s_std[kHarmWarps][2 * 32];
+    extern __shared__ __align__(16) unsigned char harm_smem[];
+    double *mtab = reinterpret_cast<double *>(harm_smem);
+    uint2 *s_q = reinterpret_cast<uint2 *>(harm_smem + (PERIODIC ? (size_t)12 * kHarmWarps * 32 * 8 : 0));
+    unsigned *s_stm = reinterpret_cast<unsigned *>(s_q + kHarmWarps * kQueue * 32);
+    unsigned *s_std = s_stm + kHarmWarps * 2 * kStageRows * 32;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
     const int item = blockIdx.x * kHarmWarps + warp;
@@ -659,22 +703,41 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     // the exact path of k_fill (no common image per run) is taken under the same condition there
     bool fast = gr.fast;
     if (PERIODIC && fast) fast = !a.gwide[g];
+    // padding entry: particle n of pos4 (weight 0, far away), image codes (1,1,1) = no shift
+    const unsigned padent = (unsigned)a.npart | (0x15u << 26);
+    // r^2 of every pair of this item lies in [e2[bin], e2[bin+1]) up to rounding; the padding particle is a few box sizes away
+    const bool careful = !(a.bins.e2[bin] > 1e-290 && a.bins.e2[bin + 1] < 1e290 && a.pad_r2max < 1e290);
+    uint2 *q = s_q + warp * kQueue * 32;
+    unsigned *stm = s_stm + warp * 2 * kStageRows * 32, *std_ = s_std + warp * 2 * kStageRows;
 
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned np;
-    if (!PERIODIC) np = harm_rows<LMAX, MLO, MHI, 0, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, nullptr, 0.0, 0.0, lane);
-    else if (fast) {
+    HarmStats st{0u};
+    if (!PERIODIC) {
+        if (careful) np = harm_rows<LMAX, MLO, MHI, 0, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
+        else np = harm_rows<LMAX, MLO, MHI, 0, D, false>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
+    } else if (fast) {
         double *mt = mtab + threadIdx.x;
         const double L = a.geom.box;
-        mt[0 * kHarmWarps * 32] = me.x - L; mt[1 * kHarmWarps * 32] = me.x; mt[2 * kHarmWarps * 32] = me.x + L;
-        mt[3 * kHarmWarps * 32] = me.y - L; mt[4 * kHarmWarps * 32] = me.y; mt[5 * kHarmWarps * 32] = me.y + L;
-        mt[6 * kHarmWarps * 32] = me.z - L; mt[7 * kHarmWarps * 32] = me.z; mt[8 * kHarmWarps * 32] = me.z + L;
+        constexpr int R = kHarmWarps * 32;
+        mt[0 * R] = me.x - L; mt[1 * R] = me.x; mt[2 * R] = me.x + L;
+        mt[4 * R] = me.y - L; mt[5 * R] = me.y; mt[6 * R] = me.y + L;
+        mt[8 * R] = me.z - L; mt[9 * R] = me.z; mt[10 * R] = me.z + L;
         __syncwarp();
-        np = harm_rows<LMAX, MLO, MHI, 1, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, mt, L, a.geom.half, lane);
-    } else np = harm_rows<LMAX, MLO, MHI, 2, D>(acc, rows, rdesc, nrows, active, s_qm[warp], s_qd[warp], s_stm[warp], s_std[warp], a.pos4, me, nullptr, a.geom.box, a.geom.half, lane);
-    if (write_counts) a.counts[col] = np;   // n_i(b); every m-range pass walks the same bits, the first one reports
+        if (careful) np = harm_rows<LMAX, MLO, MHI, 1, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
+        else np = harm_rows<LMAX, MLO, MHI, 1, D, false>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
+    } else np = harm_rows<LMAX, MLO, MHI, 2, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st);
+    if (write_counts) {
+        a.counts[col] = np;     // n_i(b); every m-range pass walks the same bits, the first one reports
+#ifdef ENCORE_HARM_STATS
+        // diagnostics (build with -DENCORE_HARM_STATS): lock-step pair steps executed and the most pairs any lane of the
+        // item had; their ratio is the lane utilisation of this kernel
+        const unsigned mx = __reduce_max_sync(kFull, np);
+        if (lane == 0) { atomicAdd(a.cand_pairs + 1, (unsigned long long)st.steps); atomicAdd(a.cand_pairs + 2, (unsigned long long)mx); }
+#endif
+    }
 
     // epilogue: a_lm = (1/v_b) sum_k ycoef[c][k] S_{m,k}, k = l-m, l-m-2, ... (p_lm has the parity of l-m)
     const double vinv = a.bins.vinv[bin];
@@ -682,22 +745,22 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     int base = 0;
 #pragma unroll
     for (int m = MLO; m <= MHI; ++m) {
-        const int st = m ? 2 : 1;
+        const int st2 = m ? 2 : 1;
 #pragma unroll
         for (int l = m; l <= LMAX; ++l) {
             const int cre = m == 0 ? l * l : l * l + 2 * m - 1;
             const double *yc = a.ycoef + (size_t)cre * (LMAX + 1);
             double sr = 0.0, si = 0.0;
 #pragma unroll
-            for (int q = (l - m) & 1; q <= l - m; q += 2) {
-                const double cf = __ldg(yc + q);
-                sr = fma(cf, acc[base + q * st], sr);
-                if (m) si = fma(cf, acc[base + q * st + 1], si);
+            for (int qq = (l - m) & 1; qq <= l - m; qq += 2) {
+                const double cf = __ldg(yc + qq);
+                sr = fma(cf, acc[base + qq * st2], sr);
+                if (m) si = fma(cf, acc[base + qq * st2 + 1], si);
             }
             out[(size_t)cre * nb * 32] = active ? sr * vinv : 0.0;
             if (m) out[(size_t)(cre + 1) * nb * 32] = active ? si * vinv : 0.0;
         }
-        base += (LMAX - m + 1) * st;
+        base += (LMAX - m + 1) * st2;
     }
 }
 
@@ -706,8 +769,17 @@ cudaError_t launch_harm(const PairArgs &a, int g0, int g1, int write_counts, cud
 {
     const int nitems = (g1 - g0) * a.bins.nbins;
     const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
-    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1, write_counts);
-    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, 0, s>>>(a, g0, g1, write_counts);
+    // the opt-in shared-memory limit is a per-kernel, process-wide attribute: set once per instantiation
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(true));
+        if (attr_err == cudaSuccess)
+            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(false));
+    });
+    if (attr_err != cudaSuccess) return attr_err;
+    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, harm_smem_bytes(true), s>>>(a, g0, g1, write_counts);
+    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, harm_smem_bytes(false), s>>>(a, g0, g1, write_counts);
     *launches += 1;
     return cudaGetLastError();
 }
