@@ -413,37 +413,62 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
         if (PERIODIC && fast && __any_sync(kFull, keep && code != wcode)) { // excluded by DESIGN.md §5.3
             if (lane == 0) *a.err_flag = 1;
         }
-        // survivors compacted to the front of cand[] (.w = position in the word), padded to a multiple of four
+        // survivors compacted to the front of cand[], two per 32-byte slot as {x0,x1,y0,y1 | z0,z1,pos0,pos1} (pos =
+        // position in the word) so that a pair of candidates feeds the packed fp32x2 instructions of sm_100; padded
+        // with never-hit fillers to a multiple of four
         const int nk = __popc(km);
-        if (keep) cand[__popc(km & lt_mask)] = make_float4(cf.x, cf.y, cf.z, __int_as_float(lane));
-        if (lane < 4) cand[nk + lane] = make_float4(1e18f, 1e18f, 1e18f, __int_as_float(0)); // never a hit
+        float *candf = reinterpret_cast<float *>(cand);
+        if (keep) {
+            const int k = __popc(km & lt_mask);
+            float *slot = candf + (k >> 1) * 8 + (k & 1);
+            slot[0] = cf.x; slot[2] = cf.y; slot[4] = cf.z; slot[6] = __int_as_float(lane);
+        }
+        if (lane < 4) {
+            const int k = nk + lane;
+            float *slot = candf + (k >> 1) * 8 + (k & 1);
+            slot[0] = 1e18f; slot[2] = 1e18f; slot[4] = 1e18f; slot[6] = __int_as_float(0);
+        }
         __syncwarp();
         kept += (unsigned long long)nk;
         if (fast) {
+            const float2 npx = make_float2(-pxf, -pxf), npy = make_float2(-pyf, -pyf), npz = make_float2(-pzf, -pzf);
+            const float2 invw2 = make_float2(invw_f, invw_f), c0h2 = make_float2(c0h, c0h), nkB2 = make_float2(-kB, -kB);
+            const float2 thr02 = make_float2(thr0, thr0), mag2 = make_float2(kMagic, kMagic), nmag2 = make_float2(-kMagic, -kMagic);
+            const float2 neg1 = make_float2(-1.f, -1.f);
 #pragma unroll 1
             for (int q0 = 0; q0 < nk; q0 += 4) {
-                // four independent tests (instruction-level parallelism)
+                // two packed pairs = four independent tests (instruction-level parallelism); every operation is the
+                // IEEE round-to-nearest fp32 operation of the scalar formulation, two lanes at a time
                 unsigned codeb[4], bitv[4];
                 int cpos[4];
                 bool ok[4], am[4];
 #pragma unroll
-                for (int cc = 0; cc < 4; ++cc) {
-                    const float4 q = cand[q0 + cc];
-                    const float dx = q.x - pxf, dy = q.y - pyf, dz = q.z - pzf;
-                    const float t = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), 1e-30f); // t = 0: r = 0 -> exact path
-                    float rinv;
-                    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(t));
-                    const float uh = fmaf(t * rinv, invw_f, c0h);
-                    const float thr = fmaf(-kB, rinv, thr0);
-                    const float v = uh + kMagic;
-                    const float fr = uh - (v - kMagic);
-                    const bool sure = fabsf(fr) <= thr;              // farther than du from every bin edge
-                    // v in [kMagic, kMagic + nb) <=> uh rounds into 0..nb-1 (float bits are monotonic)
-                    codeb[cc] = (unsigned)(__float_as_int(v) - kMagicBits);
-                    ok[cc] = sure && codeb[cc] < (unsigned)nb;
-                    am[cc] = !sure;                                  // ~2 du of all pairs, in range or not
-                    cpos[cc] = __float_as_int(q.w);
-                    bitv[cc] = 1u << cpos[cc];
+                for (int pp = 0; pp < 2; ++pp) {
+                    const float4 qa = cand[(q0 >> 1) * 2 + pp * 2], qb = cand[(q0 >> 1) * 2 + pp * 2 + 1];
+                    const float2 dx = __fadd2_rn(make_float2(qa.x, qa.y), npx), dy = __fadd2_rn(make_float2(qa.z, qa.w), npy);
+                    const float2 dz = __fadd2_rn(make_float2(qb.x, qb.y), npz);
+                    float2 t = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                    t.x = fmaxf(t.x, 1e-30f); t.y = fmaxf(t.y, 1e-30f); // t = 0: r = 0 -> exact path
+                    float2 rinv;
+                    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv.x) : "f"(t.x));
+                    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv.y) : "f"(t.y));
+                    const float2 uh = __ffma2_rn(__fmul2_rn(t, rinv), invw2, c0h2);
+                    const float2 thr = __ffma2_rn(nkB2, rinv, thr02);
+                    const float2 v = __fadd2_rn(uh, mag2);
+                    const float2 fr = __ffma2_rn(__fadd2_rn(v, nmag2), neg1, uh); // uh - (v - kMagic), exact products
+                    const float vv[2] = {v.x, v.y}, ff[2] = {fr.x, fr.y}, tt[2] = {thr.x, thr.y};
+                    const float ww[2] = {qb.z, qb.w};
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int cc = pp * 2 + e;
+                        const bool sure = fabsf(ff[e]) <= tt[e];         // farther than du from every bin edge
+                        // v in [kMagic, kMagic + nb) <=> uh rounds into 0..nb-1 (float bits are monotonic)
+                        codeb[cc] = (unsigned)(__float_as_int(vv[e]) - kMagicBits);
+                        ok[cc] = sure && codeb[cc] < (unsigned)nb;
+                        am[cc] = !sure;                                  // ~2 du of all pairs, in range or not
+                        cpos[cc] = __float_as_int(ww[e]);
+                        bitv[cc] = 1u << cpos[cc];
+                    }
                 }
                 if (!__any_sync(kFull, am[0] | am[1] | am[2] | am[3])) {
                     // branch-free: a rejected candidate sets its bit in the spare row nb
