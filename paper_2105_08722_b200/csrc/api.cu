@@ -34,7 +34,9 @@ struct DevBuf {
 struct encore_plan_s {
     HostTables T;
     bool uploaded = false;
-    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_lam_parity, d_tuple_index, gweights;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_lam_parity, d_tuple_index, d_ctas, gweights;
+    std::vector<CtaPlan> ctas;      // factorised N = 4, 5 kernels: multiplets and staged l-blocks per CTA
+    size_t cta_smem = 0;
     bool force_generic = false;
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
@@ -110,6 +112,8 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
         CU(P->d_lam_parity.ensure(sizeof(int) * std::max<size_t>(1, T.parity.size())));
         CU(cudaMemcpyAsync(P->d_lam_parity.p, T.parity.data(), sizeof(int) * T.parity.size(), cudaMemcpyHostToDevice, s));
         CU(P->d_tuple_index.ensure(sizeof(int) * cells));
+        CU(P->d_ctas.ensure(sizeof(CtaPlan) * std::max<size_t>(1, P->ctas.size())));
+        CU(cudaMemcpyAsync(P->d_ctas.p, P->ctas.data(), sizeof(CtaPlan) * P->ctas.size(), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(P->d_pair_terms.p, T.pair_terms.data(), sizeof(PairTerm) * T.pair_terms.size(), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(P->d_lam4.p, T.lam4.data(), sizeof(Lam4) * T.lam4.size(), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(P->d_lam5.p, T.lam5.data(), sizeof(Lam5) * T.lam5.size(), cudaMemcpyHostToDevice, s));
@@ -232,13 +236,13 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->group_start.ensure(sizeof(int) * ((size_t)G.npencil + 1)));
     CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
     CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
-    const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax);
+    const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax) && (T.order == 3 || P->cta_smem > 0);
     // chunks of groups per multiplet slot: the grid (slots x chunks CTAs, one per SM) should fill whole waves
     int nchunk = 32;
     if (factorised) {
         int sms = 148, dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        const int slots = contraction_grid_x(T.order, nb, T.nLam());
+        const int slots = T.order == 3 ? T.nLam() : (int)P->ctas.size();
         double best = 0.0;
         for (int c = 28; c <= 40; ++c) {
             const int ctas = slots * c, waves = (ctas + sms - 1) / sms;
@@ -406,6 +410,9 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.max_terms = 1;
     for (const Lam4 &q : T.lam4) ca.max_terms = std::max(ca.max_terms, q.nterms);
     for (const Lam5 &q : T.lam5) ca.max_terms = std::max(ca.max_terms, q.nterms);
+    ca.ctas = P->d_ctas.as<CtaPlan>();
+    ca.ncta = (int)P->ctas.size();
+    ca.cta_smem = P->cta_smem;
     ca.nchunk = nchunk;
     ca.factorised = factorised ? 1 : 0;
     CU(launch_contraction(ca, s, &P->launches));
@@ -440,7 +447,6 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
     if (lmax < 0 || !std::isfinite(box_size) || box_size < 0.0) return ENCORE_EINVAL;
     if (box_size > 0.0 && r_max > 0.5 * box_size) return ENCORE_EINVAL;
     if (lmax > ENCORE_MAX_LMAX) return ENCORE_EUNSUPPORTED;
-    if (npcf_order >= 4 && lmax > 6) return ENCORE_EUNSUPPORTED;
     encore_plan_s *P = new (std::nothrow) encore_plan_s();
     if (!P) return ENCORE_EALLOC;
     try {
@@ -449,6 +455,7 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
         delete P;
         return ENCORE_EALLOC;
     }
+    if (npcf_order >= 4 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
     *plan_out = P;
     return ENCORE_OK;
 }
@@ -540,7 +547,7 @@ int encore_destroy(encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
     DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_ycoef, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
-                      &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
+                      &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->d_ctas, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
                       &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->gwide,
@@ -586,35 +593,38 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
     const double evals = (double)T.terms.size() * (double)T.nB();
     const int N = T.order, nb = T.nbins;
     double ex = evals * (6.0 * (N - 1) + 1.0); // generic kernel: N-1 complex multiplies + 1 add per term
-    if (!P->force_generic && contraction_is_factorised(N, nb, T.lmax)) {
+    if (!P->force_generic && contraction_is_factorised(N, nb, T.lmax) && (N == 3 || P->cta_smem > 0)) {
         // executed by the factorised kernels, fused multiply-add = 2
         ex = 0.0;
+        auto c2 = [](int n) { return n * (n - 1) / 2; };
         if (N == 3) { // per real component: nb scalings + one FMA per bin pair
             ex = (double)T.ncomp * (nb + 2.0 * (nb * (nb - 1) / 2));
         } else if (N == 4) {
             for (const Lam4 &q : T.lam4)
                 for (int b1 = 0; b1 + 2 < nb; ++b1) {
                     const int nb2 = nb - 1 - b1;
-                    ex += (double)q.nterms * (4.0 + 8.0 * (nb2 - 1));                        // G: 4 mul + 4 FMA per upper bin
-                    ex += (double)(q.l3 + 1) * (2.0 * (nb2 - 1) + 4.0 * nb2 * (nb2 - 1) / 2); // Re[G a3]: 2 FMA per triple
+                    const double n0 = q.tbeg[1] - q.tbeg[0], nr = q.tbeg[q.l3 + 1] - q.tbeg[1];
+                    ex += n0 * (2.0 + 4.0 * (nb2 - 1));                                       // G_0: 2 mul + 2 FMA per upper bin
+                    ex += nr * (4.0 + 8.0 * (nb2 - 1));                                       // G_{m3>0}: 4 mul + 4 FMA per upper bin
+                    ex += 1.0 * (nb2 - 1) + 2.0 * nb2 * (nb2 - 1) / 2;                        // G_0 a3: 1 FMA per triple
+                    ex += (double)q.l3 * (2.0 * (nb2 - 1) + 4.0 * nb2 * (nb2 - 1) / 2);       // Re[G a3]: 2 FMA per triple
                 }
         } else {
-            // two warps per multiplet split by the second bin at t (contract.cu): A takes Y(b1,b2<=t) and R(b3>=2,b4),
-            // B takes Y(b1,b2>t) and R(b3>=t+2,b4); 4 multiplies per pre-weighted operand, 4 FMA per pair and term
-            const int t = contraction_split5(nb);
-            auto c2 = [](int n) { return n * (n - 1) / 2; };
-            double tupA = 0, tupB = 0;
-            for (int b2 = 1; b2 <= nb - 3; ++b2) (b2 <= t ? tupA : tupB) += (double)b2 * c2(nb - 1 - b2);
-            for (const Lam5 &q : T.lam5) {
-                const double nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0], nM = q.l12 + 1;
-                ex += nl * (4.0 * t + 8.0 * c2(t + 1)) + nM * 2.0 * c2(t + 1);                 // A: Y block, times w_i
-                ex += nr * (4.0 * (nb - 3) + 8.0 * c2(nb - 2));                                // A: R block (all b3 >= 2)
-                ex += nM * 4.0 * tupA;                                                         // A: Re[Y R]
-                if (t + 1 <= nb - 3) {
-                    const double nyb = c2(nb - 2) - c2(t + 1);
-                    ex += nr * (4.0 * (nb - 3 - t) + 8.0 * c2(nb - 2 - t));                    // B: R block (b3 >= t+2)
-                    ex += nl * (4.0 * (nb - 3 - t) + 8.0 * nyb) + nM * 2.0 * nyb;              // B: Y block, times w_i
-                    ex += nM * 4.0 * tupB;                                                     // B: Re[Y R]
+            // warp w of a multiplet takes the second bins lo..hi (contract.cu): Y(b1, b2 in lo..hi) and R(b3 > lo, b4);
+            // 4 multiplies per pre-weighted operand, 4 FMA per pair and term, 2 FMA per tuple and M
+            const int nw = contraction_warps5(nb);
+            for (int w = 0; w < nw; ++w) {
+                int lo, hi;
+                contraction_range5(nb, w, &lo, &hi);
+                if (lo > hi || hi > nb - 3) continue;
+                const double nyh = c2(hi + 1) - c2(lo), nrh = c2(nb - 1 - lo);
+                double tup = 0;
+                for (int b2 = lo; b2 <= hi; ++b2) tup += (double)b2 * c2(nb - 1 - b2);
+                for (const Lam5 &q : T.lam5) {
+                    const double nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0], nM = q.l12 + 1;
+                    ex += nl * (4.0 * (hi - lo + 1) + 8.0 * nyh) + nM * 2.0 * nyh;   // Y block, times w_i
+                    ex += nr * (4.0 * (nb - 2 - lo) + 8.0 * nrh);                    // R block
+                    ex += nM * 4.0 * tup;                                            // Re[Y R]
                 }
             }
         }

@@ -8,8 +8,6 @@
 #define ENCORE_MAX_BINS 32
 #define ENCORE_MAX_LMAX 10
 #define ENCORE_GROUP 32              // primaries per group = lanes of a warp
-#define ENCORE_PAGE_WORDS 64         // candidate-list page: 64 entries (256 bytes) of one (primary, bin) list
-#define ENCORE_SLAB_PAGES 256        // pages a warp takes from the pool at a time (64 kB)
 
 // Real-component layout of one a_lm tile row (per radial bin): (lmax+1)^2 doubles,
 //   (l,0) at l*l;  Re(l,m) at l*l+2m-1;  Im(l,m) at l*l+2m   (m = 1..l).
@@ -37,10 +35,13 @@ struct PairTerm {
 
 // N=4 multiplet for the factorised contraction:
 //   H_i = sum_{m3>=0} Re[ G_{m3}(b1,b2) a_{l3 m3}(b3) ],  G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2
+// m3 = 0: the terms (m1, -m1) and (-m1, m1) are complex conjugates of each other up to the sign (-1)^{l1+l2+l3}
+// (3-j column symmetry and a_{l,-m} = (-1)^m a*_lm), so G_0 is real for even and imaginary for odd multiplets and only
+// m1 >= 0 is kept: the m3 = 0 terms are "half terms" G_0 += wrr A[ia_re] B[ib_re] + wii A[ia_im] B[ib_im] (two FMAs).
 struct Lam4 {
     int l1, l2, l3;
     int odd;            // parity-odd multiplet: the stored result is Im instead of Re (App. B)
-    int tbeg[9];        // terms of m3 are [tbeg[m3], tbeg[m3+1]) in pair_terms
+    int tbeg[ENCORE_MAX_LMAX + 2]; // terms of m3 are [tbeg[m3], tbeg[m3+1]) in pair_terms; m3 = 0: half terms
     int nterms;
 };
 
@@ -53,6 +54,17 @@ struct Lam5 {
     int lbeg[14];       // left terms of M: [lbeg[M], lbeg[M+1])   (M <= l12 <= 12)
     int rbeg[14];       // right terms
     int nterms;
+};
+
+// One CTA of the factorised N = 4, 5 kernels: its multiplets and the l-blocks of the a_lm tile they need (only those
+// are brought into shared memory; a block l is the (2l+1) x nbins x 32 doubles starting at component l^2).
+struct CtaPlan {
+    int lam[8];                     // multiplet per slot, -1: empty
+    int nblk;
+    int bl[ENCORE_MAX_LMAX + 1];    // l of block j
+    int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged
+    int tile;                       // doubles per tile buffer
+    int nbuf;                       // 2: double-buffered, 1: single
 };
 
 struct HostTables {

@@ -10,7 +10,10 @@
 // shuffle tree per warp, a fixed-order sum over groups per segment and a fixed-order sum over segments: no atomics.
 #include "device.cuh"
 
+#include <algorithm>
+#include <mutex>
 #include <type_traits>
+#include <vector>
 
 namespace {
 
@@ -208,7 +211,48 @@ __device__ __forceinline__ void task4(double (&acc)[make_set4(NB, NW, W).aoff[ma
     constexpr int rs = NB * 32;
     const double *p1 = smem_c + s1, *p2 = smem_c + s2, *p3 = smem_c + s3;
     const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.tbeg[0];
-    for (int m3 = 0; m3 <= L.l3; ++m3) {
+    {   // m3 = 0: G_0 is real (even) or imaginary (odd) and a_{l3 0} is real: half terms, one real G, one FMA per triple
+        double g0[NG];
+#pragma unroll
+        for (int k = 0; k < NG; ++k) g0[k] = 0.0;
+        const int t1 = L.tbeg[1];
+#pragma unroll 1
+        for (int t = L.tbeg[0]; t < t1; ++t) {
+            const PairTerm T = terms[t];
+            double u[NS], v[NS];
+            const double *ar = p1 + T.ia_re * rs, *ai = p1 + T.ia_im * rs;
+            static_for<0, NS>([&](auto J) {
+                constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                u[j] = T.wrr * ar[b1 * 32]; v[j] = T.wii * ai[b1 * 32];
+            });
+            const double *qr = p2 + T.ib_re * rs, *qi = p2 + T.ib_im * rs;
+            static_for<BMIN + 1, NB - 1>([&](auto B2) {
+                constexpr int b2 = decltype(B2)::value;
+                const double r2 = qr[b2 * 32], i2 = qi[b2 * 32];
+                static_for<0, NS>([&](auto J) {
+                    constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                    if constexpr (b2 > b1) {
+                        constexpr int k = make_set4(NB, NW, W).goff[j] + b2 - b1 - 1;
+                        g0[k] = fma(u[j], r2, fma(v[j], i2, g0[k]));
+                    }
+                });
+            });
+        }
+        static_for<BMIN + 2, NB>([&](auto B3) {
+            constexpr int b3 = decltype(B3)::value;
+            const double r3 = wi * p3[b3 * 32];
+            static_for<0, NS>([&](auto J) {
+                constexpr int j = decltype(J)::value, b1 = make_set4(NB, NW, W).b1[j];
+                static_for<b1 + 1, b3>([&](auto B2) {
+                    constexpr int b2 = decltype(B2)::value;
+                    constexpr int k = make_set4(NB, NW, W).goff[j] + b2 - b1 - 1;
+                    constexpr int o = make_set4(NB, NW, W).aoff[j] + c2(b3 - b1 - 1) + (b2 - b1 - 1);
+                    acc[o] = fma(g0[k], r3, acc[o]);
+                });
+            });
+        });
+    }
+    for (int m3 = 1; m3 <= L.l3; ++m3) {
         double gr[NG], gi[NG]; // G_{m3}(b1, b2)
 #pragma unroll
         for (int k = 0; k < NG; ++k) { gr[k] = 0.0; gi[k] = 0.0; }
@@ -237,11 +281,11 @@ __device__ __forceinline__ void task4(double (&acc)[make_set4(NB, NW, W).aoff[ma
                 });
             });
         }
-        const int cr = m3 == 0 ? 0 : 2 * m3 - 1;
-        const double *q3r = p3 + cr * rs, *q3i = p3 + (m3 == 0 ? cr : cr + 1) * rs;
-        // even parity: Re[G a3] = Gr Re a3 - Gi Im a3;  odd parity: Im[G a3] = Gr Im a3 + Gi Re a3  (Im a3 = 0 at m3 = 0)
+        const int cr = 2 * m3 - 1;
+        const double *q3r = p3 + cr * rs, *q3i = p3 + (cr + 1) * rs;
+        // even parity: Re[G a3] = Gr Re a3 - Gi Im a3;  odd parity: Im[G a3] = Gr Im a3 + Gi Re a3
         const double *pA = L.odd ? q3i : q3r, *pB = L.odd ? q3r : q3i;
-        const double cA = L.odd ? (m3 == 0 ? 0.0 : wi) : wi, cB = L.odd ? wi : (m3 == 0 ? 0.0 : -wi);
+        const double cA = wi, cB = L.odd ? wi : -wi;
         static_for<BMIN + 2, NB>([&](auto B3) {
             constexpr int b3 = decltype(B3)::value;
             const double r3 = cA * pA[b3 * 32], i3 = cB * pB[b3 * 32];
@@ -291,10 +335,9 @@ __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned coun
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-__device__ __forceinline__ void tile_load(double *dst, const double *src, unsigned bytes, unsigned long long *bar)
+__device__ __forceinline__ void bulk_copy(double *dst, const double *src, unsigned bytes, unsigned long long *bar)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-    // bulk copies are limited by the tx-count field (2^20-1 bytes); tiles are < 256 kB
+    // (the tx-count field of an mbarrier holds 2^20-1 bytes; the staged blocks of a group are < 256 kB)
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
@@ -317,43 +360,50 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
 struct TilePipe {
     int buf[2];              // offsets into smem_c (doubles)
     int bar;                 // offset of the two mbarriers
-    unsigned bytes;
+    unsigned bytes;          // bytes of the staged l-blocks of one group
     int nbuf;
 };
 
-// Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.y, + gridDim.y, ... < g_end
+// Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.y, + gridDim.y, ... < g_end.  Only the l-blocks the
+// CTA's multiplets need (CtaPlan) are copied: one bulk copy per block, all completing on the buffer's mbarrier.
 template <class Body>
-__device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const TilePipe &tp, Body body)
+__device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, Body body)
 {
     const int ngroups = a.g_end;
     const size_t tile = (size_t)a.ncomp * a.nbins * 32;
     const int stride = gridDim.y;
     const bool issuer = threadIdx.x == 0;
+    const int rs = a.nbins * 32;
     int g = a.g_begin + blockIdx.y;
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
-    if (issuer && g < ngroups) tile_load(smem_c + tp.buf[0], a.alm + (size_t)g * tile, tp.bytes, &bar[0]);
+    auto load = [&](int buf, int gg) {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bar[buf])), "r"(tp.bytes) : "memory");
+        const double *src = a.alm + (size_t)gg * tile;
+        for (int j = 0; j < C.nblk; ++j) {
+            const int l = C.bl[j];
+            bulk_copy(smem_c + tp.buf[buf] + C.off[l], src + (size_t)l * l * rs, (unsigned)((2 * l + 1) * rs * sizeof(double)), &bar[buf]);
+        }
+    };
+    if (issuer && g < ngroups) load(0, g);
     for (int k = 0; g < ngroups; ++k, g += stride) {
         const int st = tp.nbuf == 2 ? (k & 1) : 0;
-        if (tp.nbuf == 2 && issuer && g + stride < ngroups)
-            tile_load(smem_c + tp.buf[st ^ 1], a.alm + (size_t)(g + stride) * tile, tp.bytes, &bar[st ^ 1]);
+        if (tp.nbuf == 2 && issuer && g + stride < ngroups) load(st ^ 1, g + stride);
         mbar_wait(&bar[st], tp.nbuf == 2 ? (unsigned)((k >> 1) & 1) : (unsigned)(k & 1));
         body(tp.buf[st], g);
         __syncthreads(); // every warp is done with buf[st] before it is refilled
-        if (tp.nbuf == 1 && issuer && g + stride < ngroups)
-            tile_load(smem_c + tp.buf[0], a.alm + (size_t)(g + stride) * tile, tp.bytes, &bar[0]);
+        if (tp.nbuf == 1 && issuer && g + stride < ngroups) load(0, g + stride);
     }
 }
 
-// shared memory: [nbuf tiles][2 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
-__device__ __forceinline__ TilePipe make_pipe(const ContractArgs &a, int nbuf)
+// shared memory: [nbuf tile buffers][2 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
+__device__ __forceinline__ TilePipe make_pipe(const CtaPlan &C)
 {
     TilePipe tp;
-    const int tile = a.ncomp * a.nbins * 32;
     tp.buf[0] = 0;
-    tp.buf[1] = nbuf == 2 ? tile : 0;
-    tp.bar = nbuf * tile;
-    tp.bytes = (unsigned)(tile * sizeof(double));
-    tp.nbuf = nbuf;
+    tp.buf[1] = C.nbuf == 2 ? C.tile : 0;
+    tp.bar = C.nbuf * C.tile;
+    tp.bytes = (unsigned)(C.tile * sizeof(double));
+    tp.nbuf = C.nbuf;
     if (threadIdx.x == 0) {
         unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
         mbar_init(&bar[0], 1);
@@ -375,16 +425,16 @@ __host__ __device__ constexpr int nw4(int nb) { return nb >= 9 ? ENCORE_NW4_WIDE
 __host__ __device__ constexpr int lpc4(int nb) { return nb >= 9 ? ENCORE_LPC4_WIDE : kCtaWarps / nw4(nb); }
 
 template <int NB, int NW, int W>
-__device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
+__device__ __forceinline__ void warp4(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
     constexpr Set4 S = make_set4(NB, NW, W);
     constexpr int NTOT = S.aoff[S.n];
     const int lane = threadIdx.x & 31;
-    const int o1 = L.l1 * L.l1 * NB * 32 + lane, o2 = L.l2 * L.l2 * NB * 32 + lane, o3 = L.l3 * L.l3 * NB * 32 + lane;
+    const int o1 = C.off[L.l1] + lane, o2 = C.off[L.l2] + lane, o3 = C.off[L.l3] + lane;
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for_each_group_tile(a, tp, [&](int t, int g) {
+    for_each_group_tile(a, C, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
         task4<NB, NW, W>(acc, L, toff, t + o1, t + o2, t + o3, wi);
@@ -395,29 +445,32 @@ __device__ __forceinline__ void warp4(const ContractArgs &a, const TilePipe &tp,
 }
 
 template <int NB, int NW, int W>
-__device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
+__device__ __forceinline__ void dispatch4(int w, const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, bool have, const Lam4 &L, int iL, int toff)
 {
-    if (w == W) warp4<NB, NW, W>(a, tp, have, L, iL, toff);
-    else if constexpr (W + 1 < NW) dispatch4<NB, NW, W + 1>(w, a, tp, have, L, iL, toff);
+    if (w == W) warp4<NB, NW, W>(a, C, tp, have, L, iL, toff);
+    else if constexpr (W + 1 < NW) dispatch4<NB, NW, W + 1>(w, a, C, tp, have, L, iL, toff);
 }
 
 // LPC multiplets per CTA, each on NW warps
 // registers: the file is split over the 4 SM sub-partitions (16384 each), so 9-12 warps cap a thread at 168 registers
 // and up to 8 warps allow 255
 template <int NB>
-__global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(ContractArgs a, int nbuf)
+__global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(ContractArgs a)
 {
-    constexpr int NW = nw4(NB), LPC = lpc4(NB);
+    constexpr int NW = nw4(NB);
+    __shared__ CtaPlan C;
+    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.x)[threadIdx.x];
+    __syncthreads();
     const int warp = threadIdx.x >> 5;
-    const int slot = blockIdx.x * LPC + warp / NW;
-    const bool have = slot < a.nLam;
-    const int iL = a.lam_order[have ? slot : 0];
+    const int iLs = C.lam[warp / NW];
+    const bool have = iLs >= 0;
+    const int iL = have ? iLs : 0;
     const Lam4 L = a.lam4[iL];
-    const TilePipe tp = make_pipe(a, nbuf);
+    const TilePipe tp = make_pipe(C);
     const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // this multiplet's term list in shared memory
     if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.tbeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
-    dispatch4<NB, NW, 0>(warp % NW, a, tp, have, L, iL, toff);
+    dispatch4<NB, NW, 0>(warp % NW, a, C, tp, have, L, iL, toff);
 }
 
 // ---- N = 5 ------------------------------------------------------------------------------------------------
@@ -544,85 +597,73 @@ __device__ __forceinline__ void pairs_block(double (&zr)[NZ], double (&zi)[NZ], 
     }
 }
 
-// warp A: second bins 1..T.  Y(b1,b2) of all its pairs held in registers, R(b3,.) streamed by b3.
-template <int NB, int T, int NTOT>
-__device__ __forceinline__ void task5a(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, double wi)
+// ---- how the second bins 1 .. NB-3 of a multiplet are dealt to its warps -----------------------------------
+// Up to 8 bins: two warps, b2 <= T and b2 > T (T = t5(NB), measured on c5).  9 and 10 bins: consecutive ranges grown
+// greedily while partial sums + held coupled pairs stay under 105 doubles (3 and 5 warps).
+__host__ __device__ constexpr int regs5(int nb, int lo, int hi)
 {
-    constexpr int rs = NB * 32, NYH = c2(T + 1); // pairs b1 < b2 <= T
-    const double *p1 = smem_c + sA + L.l1 * L.l1 * rs, *p2 = smem_c + sA + L.l2 * L.l2 * rs;
-    const double *p3 = smem_c + sA + L.l3 * L.l3 * rs, *p4 = smem_c + sA + L.l4 * L.l4 * rs;
-    const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
-    for (int M = 0; M <= L.l12; ++M) {
-        double yr[NYH], yi[NYH];
-#pragma unroll
-        for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
-        pairs_block<NB, 0, 0, T - 1, 1, T, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
-        const double wyi = L.odd ? wi : -wi;
-#pragma unroll
-        for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= wyi; } // even: Re[Y R] = Yr Rr - Yi Ri; odd: Im[Y R] = Yr Ri + Yi Rr
-        constexpr int NRH = c2(NB - 2); // pairs 2 <= b3 < b4 <= NB-1
-        double rr[NRH], ri[NRH];
-#pragma unroll
-        for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
-        pairs_block<NB, 1, 2, NB - 2, 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
-        if (L.odd) {
-#pragma unroll
-            for (int k = 0; k < NRH; ++k) { const double x = rr[k]; rr[k] = ri[k]; ri[k] = x; }
-        }
-        static_for<2, NB - 1>([&](auto B3) {
-            constexpr int b3 = decltype(B3)::value;
-            static_for<b3 + 1, NB>([&](auto B4) {
-                constexpr int b4 = decltype(B4)::value;
-                constexpr int q = slot5<NB, 1, 2, 3>(b3, b4);
-                static_for<1, (T < b3 - 1 ? T : b3 - 1) + 1>([&](auto B2) {
-                    constexpr int b2 = decltype(B2)::value;
-                    static_for<0, b2>([&](auto B1) {
-                        constexpr int b1 = decltype(B1)::value;
-                        constexpr int o = aidx5(NB, 1, b1, b2, b3, b4), k = c2(b2) + b1;
-                        acc[o] = fma(yr[k], rr[q], fma(yi[k], ri[q], acc[o]));
-                    });
-                });
-            });
-        });
-    }
+    return ntot5(nb, lo, hi) + 2 * c2(nb - 1 - lo) + 2 * (c2(hi + 1) - c2(lo));
 }
-
-// warp B: second bins T+1..NB-3.  R(b3,b4) of all its pairs (b3 >= T+2) held in registers, Y(.,b2) streamed by b2.
-template <int NB, int T, int NTOT>
-__device__ __forceinline__ void task5b(double (&acc)[NTOT], const Lam5 &L, int toff, int sA, double wi)
+__host__ __device__ constexpr int hi5(int nb, int w);
+__host__ __device__ constexpr int lo5(int nb, int w)
 {
-    if constexpr (T + 1 <= NB - 3) {
-        constexpr int rs = NB * 32, NRH = c2(NB - 2 - T); // pairs T+2 <= b3 < b4 <= NB-1
-        const double *p1 = smem_c + sA + L.l1 * L.l1 * rs, *p2 = smem_c + sA + L.l2 * L.l2 * rs;
-        const double *p3 = smem_c + sA + L.l3 * L.l3 * rs, *p4 = smem_c + sA + L.l4 * L.l4 * rs;
+    if (nb <= 8) return w == 0 ? 1 : t5(nb) + 1;
+    return w == 0 ? 1 : hi5(nb, w - 1) + 1;
+}
+__host__ __device__ constexpr int hi5(int nb, int w)
+{
+    if (nb <= 8) return w == 0 ? t5(nb) : nb - 3;
+    const int lo = lo5(nb, w);
+    int hi = lo;
+    while (hi + 1 <= nb - 3 && regs5(nb, lo, hi + 1) <= 105) ++hi;
+    return hi;
+}
+__host__ __device__ constexpr int nw5(int nb)
+{
+    if (nb <= 8) return 2;
+    int w = 0;
+    while (hi5(nb, w) < nb - 3) ++w;
+    return w + 1;
+}
+__host__ __device__ constexpr int lpc5(int nb) { return 8 / nw5(nb); } // multiplets per CTA: at most 8 warps, so that a thread may hold 255 registers
+
+// A warp whose second bins are LO..HI: Y(b1,b2) of its pairs (b2 in LO..HI) and R(b3,b4) of the pairs above LO
+// (b3 >= LO+1) are swept whole (every operand and every term read once per M) and held in registers, then the
+// products of the warp's tuples are added.
+template <int NB, int LO, int HI, int NTOT>
+__device__ __forceinline__ void task5(double (&acc)[NTOT], const Lam5 &L, int toff, const double *p1, const double *p2,
+                                      const double *p3, const double *p4, double wi)
+{
+    if constexpr (LO <= HI && HI <= NB - 3) {
+        constexpr int NYH = c2(HI + 1) - c2(LO);   // pairs b1 < b2, LO <= b2 <= HI
+        constexpr int NRH = c2(NB - 1 - LO);       // pairs LO+1 <= b3 < b4 <= NB-1
         const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
         for (int M = 0; M <= L.l12; ++M) {
-            double rr[NRH], ri[NRH];
-#pragma unroll
-            for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
-            pairs_block<NB, 1, T + 2, NB - 2, T + 3, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
-            constexpr int NYH = c2(NB - 2) - c2(T + 1); // pairs b1 < b2, T+1 <= b2 <= NB-3
             double yr[NYH], yi[NYH];
 #pragma unroll
             for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }
-            pairs_block<NB, 0, 0, NB - 4, T + 1, NB - 3, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
+            pairs_block<NB, 0, 0, HI - 1, LO, HI, NYH>(yr, yi, terms, L.lbeg[M], L.lbeg[M + 1], p1, p2);
             const double wyi = L.odd ? wi : -wi;
 #pragma unroll
-            for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= wyi; } // even: Yr Rr - Yi Ri; odd: Yr Ri + Yi Rr
+            for (int k = 0; k < NYH; ++k) { yr[k] *= wi; yi[k] *= wyi; } // even: Re[Y R] = Yr Rr - Yi Ri; odd: Im[Y R] = Yr Ri + Yi Rr
+            double rr[NRH], ri[NRH];
+#pragma unroll
+            for (int k = 0; k < NRH; ++k) { rr[k] = 0.0; ri[k] = 0.0; }
+            pairs_block<NB, 1, LO + 1, NB - 2, LO + 2, NB - 1, NRH>(rr, ri, terms, L.rbeg[M], L.rbeg[M + 1], p3, p4);
             if (L.odd) {
 #pragma unroll
                 for (int k = 0; k < NRH; ++k) { const double x = rr[k]; rr[k] = ri[k]; ri[k] = x; }
             }
-            static_for<T + 1, NB - 2>([&](auto B2) {
+            static_for<LO, HI + 1>([&](auto B2) {
                 constexpr int b2 = decltype(B2)::value;
                 static_for<b2 + 1, NB - 1>([&](auto B3) {
                     constexpr int b3 = decltype(B3)::value;
                     static_for<b3 + 1, NB>([&](auto B4) {
                         constexpr int b4 = decltype(B4)::value;
-                        constexpr int k = slot5<NB, 1, T + 2, T + 3>(b3, b4);
+                        constexpr int k = slot5<NB, 1, LO + 1, LO + 2>(b3, b4);
                         static_for<0, b2>([&](auto B1) {
                             constexpr int b1 = decltype(B1)::value;
-                            constexpr int o = aidx5(NB, T + 1, b1, b2, b3, b4), q = slot5<NB, 0, 0, T + 1>(b1, b2);
+                            constexpr int o = aidx5(NB, LO, b1, b2, b3, b4), q = slot5<NB, 0, 0, LO>(b1, b2);
                             acc[o] = fma(yr[q], rr[k], fma(yi[q], ri[k], acc[o]));
                         });
                     });
@@ -652,93 +693,150 @@ __device__ __forceinline__ void flush5(const double (&acc)[NTOT], const int *tup
     });
 }
 
-// 8 warps per CTA (255 registers) = 4 multiplets; even warp: b2 <= T, odd warp: b2 > T
-constexpr int kCtaWarps5 = 8;
-template <int NB>
-__global__ void __launch_bounds__(kCtaWarps5 * 32, 1) k_contract5(ContractArgs a, int nbuf)
+template <int NB, int W>
+__device__ __forceinline__ void warp5(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, bool have, const Lam5 &L, int iL, int toff)
 {
-    constexpr int LPC = kCtaWarps5 / 2, T = t5(NB);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int slot = blockIdx.x * LPC + (warp >> 1);
-    const bool have = slot < a.nLam;
-    const int iL = a.lam_order[have ? slot : 0];
-    const Lam5 L = a.lam5[iL];
-    const bool second = warp & 1;
-    constexpr int NA = ntot5(NB, 1, T), NR = ntot5(NB, T + 1, NB - 3);
-    constexpr int NTOT = NA > NR ? NA : NR;
-    const TilePipe tp = make_pipe(a, nbuf);
-    const int toff = tp.bar + 8 + (warp >> 1) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
-    if (have && !second) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
-    __syncthreads();
+    constexpr int LO = lo5(NB, W), HI = hi5(NB, W), NTOT = ntot5(NB, LO, HI);
+    const int lane = threadIdx.x & 31;
+    const int o1 = C.off[L.l1] + lane, o2 = C.off[L.l2] + lane, o3 = C.off[L.l3] + lane, o4 = C.off[L.l4] + lane;
     double acc[NTOT];
 #pragma unroll
     for (int k = 0; k < NTOT; ++k) acc[k] = 0.0;
-    for_each_group_tile(a, tp, [&](int t, int g) {
+    for_each_group_tile(a, C, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        if (!second) task5a<NB, T, NTOT>(acc, L, toff, t + lane, wi);
-        else task5b<NB, T, NTOT>(acc, L, toff, t + lane, wi);
+        task5<NB, LO, HI, NTOT>(acc, L, toff, smem_c + t + o1, smem_c + t + o2, smem_c + t + o3, smem_c + t + o4, wi);
     });
     if (!have) return;
     double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
-    if (!second) flush5<NB, 1, T, NTOT>(acc, a.tuple_index, out, lane);
-    else flush5<NB, T + 1, NB - 3, NTOT>(acc, a.tuple_index, out, lane);
+    if constexpr (LO <= HI) flush5<NB, LO, HI, NTOT>(acc, a.tuple_index, out, lane);
 }
 
-// shared memory: nbuf tiles + 2 mbarriers; two buffers whenever they fit
-static int pipe_config(const ContractArgs &a, int lam_per_cta, size_t *smem)
+template <int NB, int W>
+__device__ __forceinline__ void dispatch5(int w, const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, bool have, const Lam5 &L, int iL, int toff)
 {
-    const size_t tile = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
-    const size_t extra = 64 + (size_t)lam_per_cta * a.max_terms * sizeof(PairTerm);
-    const int nbuf = 2 * tile + extra <= 224 * 1024 ? 2 : 1;
-    *smem = nbuf * tile + extra;
-    return nbuf;
+    if (w == W) warp5<NB, W>(a, C, tp, have, L, iL, toff);
+    else if constexpr (W + 1 < nw5(NB)) dispatch5<NB, W + 1>(w, a, C, tp, have, L, iL, toff);
 }
+
+// lpc5 multiplets per CTA on nw5 warps each (8 warps at up to 8 bins: 255 registers)
+template <int NB>
+__global__ void __launch_bounds__(nw5(NB) * lpc5(NB) * 32, 1) k_contract5(ContractArgs a)
+{
+    constexpr int NW = nw5(NB);
+    __shared__ CtaPlan C;
+    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.x)[threadIdx.x];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int iLs = C.lam[warp / NW];
+    const bool have = iLs >= 0;
+    const int iL = have ? iLs : 0;
+    const Lam5 L = a.lam5[iL];
+    const TilePipe tp = make_pipe(C);
+    const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
+    if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
+    __syncthreads();
+    dispatch5<NB, 0>(warp % NW, a, C, tp, have, L, iL, toff);
+}
+
+// ---- host side: multiplets -> CTAs, l-blocks per CTA, shared memory ----------------------------------------------
+static int lpc_of(int order, int nb) { return order == 4 ? lpc4(nb) : lpc5(nb); }
+static constexpr size_t kSmemLimit = 224 * 1024;
 
 template <int NB>
 cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 {
-    size_t smem;
-    constexpr int LPC = lpc4(NB);
-    const int nbuf = pipe_config(a, LPC, &smem);
-    cudaError_t e = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_contract4<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), nw4(NB) * LPC * 32, smem, s>>>(a, nbuf);
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
+    if (attr_err != cudaSuccess) return attr_err;
+    k_contract4<NB><<<dim3(a.ncta, a.nchunk), nw4(NB) * lpc4(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();
 }
 
 template <int NB>
 cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 {
-    size_t smem;
-    constexpr int LPC = kCtaWarps5 / 2;
-    const int nbuf = pipe_config(a, LPC, &smem);
-    cudaError_t e = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_contract5<NB><<<dim3((a.nLam + LPC - 1) / LPC, a.nchunk), kCtaWarps5 * 32, smem, s>>>(a, nbuf);
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
+    if (attr_err != cudaSuccess) return attr_err;
+    k_contract5<NB><<<dim3(a.ncta, a.nchunk), nw5(NB) * lpc5(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();
 }
 
 } // namespace
 
-// Factorised kernels cover the bin counts whose per-warp partial sums fit in registers; anything else (and N = 3,
-// which is cheap) runs the generic kernel.
+// Factorised kernels cover the bin counts whose per-warp partial sums fit in registers; anything else runs the generic
+// kernel (one warp per (Lambda, B), literal eq. 44).
 int contraction_split5(int nbins) { return t5(nbins); }
-
-// CTAs along x of the factorised kernels (multiplet slots)
-int contraction_grid_x(int order, int nbins, int nlam)
-{
-    if (order == 3) return nlam;
-    const int lpc = order == 4 ? lpc4(nbins) : kCtaWarps5 / 2;
-    return (nlam + lpc - 1) / lpc;
-}
+int contraction_warps5(int nbins) { return nw5(nbins); }
+void contraction_range5(int nbins, int w, int *lo, int *hi) { *lo = lo5(nbins, w); *hi = hi5(nbins, w); }
 
 int contraction_is_factorised(int order, int nbins, int lmax)
 {
     if (order == 3) return nbins >= 2 && nbins <= 10;
-    if (order == 4) return nbins >= 3 && nbins <= 10 && lmax <= 6;
-    if (order == 5) return nbins >= 4 && nbins <= 8 && lmax <= 4;
+    if (order == 4) return nbins >= 3 && nbins <= 10 && lmax <= ENCORE_MAX_LMAX;
+    if (order == 5) return nbins >= 4 && nbins <= 10 && lmax <= 5;
     return 0;
+}
+
+// Deal the multiplets (heaviest first) to CTAs of lpc slots: a CTA takes the next multiplet while the l-blocks of all
+// its multiplets still fit one tile buffer; two buffers whenever they fit.  Returns the dynamic shared memory the
+// launch needs (0: a single multiplet does not fit).
+size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas)
+{
+    ctas.clear();
+    if (T.order < 4) return 0;
+    const int lpc = lpc_of(T.order, T.nbins), nL = T.nLam();
+    size_t max_terms = 1;
+    for (const Lam4 &q : T.lam4) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
+    for (const Lam5 &q : T.lam5) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
+    const size_t extra = 64 + sizeof(CtaPlan) + (size_t)lpc * max_terms * sizeof(PairTerm);
+    const size_t blk = (size_t)T.nbins * 32 * sizeof(double); // bytes of one component of a tile
+    auto ls_of = [&](int iL, int *l) {
+        if (T.order == 4) { const Lam4 &q = T.lam4[iL]; l[0] = q.l1; l[1] = q.l2; l[2] = q.l3; return 3; }
+        const Lam5 &q = T.lam5[iL]; l[0] = q.l1; l[1] = q.l2; l[2] = q.l3; l[3] = q.l4; return 4;
+    };
+    auto tile_bytes = [&](unsigned mask) {
+        size_t b = 0;
+        for (int l = 0; l <= T.lmax; ++l) if (mask >> l & 1u) b += (size_t)(2 * l + 1) * blk;
+        return b;
+    };
+    std::vector<unsigned> masks;
+    int fill = lpc;
+    for (int k = 0; k < nL; ++k) {
+        const int iL = T.lam_order[k];
+        int l[4];
+        const int nl = ls_of(iL, l);
+        unsigned m = 0;
+        for (int j = 0; j < nl; ++j) m |= 1u << l[j];
+        if (tile_bytes(m) + extra > kSmemLimit) return 0;
+        if (fill == lpc || tile_bytes(masks.back() | m) + extra > kSmemLimit) {
+            CtaPlan c{};
+            for (int j = 0; j < 8; ++j) c.lam[j] = -1;
+            ctas.push_back(c);
+            masks.push_back(0u);
+            fill = 0;
+        }
+        ctas.back().lam[fill++] = iL;
+        masks.back() |= m;
+    }
+    size_t smem = 0;
+    for (size_t i = 0; i < ctas.size(); ++i) {
+        CtaPlan &c = ctas[i];
+        int off = 0;
+        c.nblk = 0;
+        for (int l = 0; l <= ENCORE_MAX_LMAX; ++l) {
+            c.off[l] = -1;
+            if (l <= T.lmax && (masks[i] >> l & 1u)) { c.bl[c.nblk++] = l; c.off[l] = off; off += (2 * l + 1) * T.nbins * 32; }
+        }
+        c.tile = off;
+        const size_t tb = (size_t)off * sizeof(double);
+        c.nbuf = 2 * tb + extra <= kSmemLimit ? 2 : 1;
+        smem = std::max(smem, c.nbuf * tb + extra);
+    }
+    return smem;
 }
 
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches)
@@ -780,6 +878,8 @@ cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launc
         case 6: return launch5<6>(a, s);
         case 7: return launch5<7>(a, s);
         case 8: return launch5<8>(a, s);
+        case 9: return launch5<9>(a, s);
+        case 10: return launch5<10>(a, s);
         }
     }
     return cudaErrorInvalidValue;

@@ -112,12 +112,18 @@ struct ContractArgs {
     const int *tuple_index;     // device [nbins^(N-1)]: index of the ordered tuple in bin_tuples, -1 if not ordered
     int lmax;
     int max_terms;              // largest number of coupled-pair terms of one multiplet
+    const CtaPlan *ctas;        // device [ncta]: multiplets and staged l-blocks of every CTA of the factorised N = 4, 5 kernels
+    int ncta;
+    size_t cta_smem;            // dynamic shared memory of that launch
     int nchunk;                 // partial has nchunk rows when the factorised kernels ran (ngroups rows otherwise)
     int factorised;             // set by launch_contraction
 };
 int contraction_is_factorised(int order, int nbins, int lmax);
-int contraction_grid_x(int order, int nbins, int nlam);
-int contraction_split5(int nbins);   // N = 5: second bins <= this go to the first warp of a multiplet
+int contraction_split5(int nbins);   // N = 5, up to 8 bins: second bins <= this go to the first warp of a multiplet
+int contraction_warps5(int nbins);   // N = 5: warps per multiplet
+void contraction_range5(int nbins, int w, int *lo, int *hi); // N = 5: second bins lo..hi of warp w
+// multiplets -> CTAs of the factorised N = 4, 5 kernels; returns the dynamic shared memory of the launch (0: does not fit)
+size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas);
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
 

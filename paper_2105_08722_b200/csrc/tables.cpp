@@ -13,16 +13,19 @@ namespace {
 
 const long double kPi = 3.14159265358979323846264338327950288L;
 
+struct FactTable {
+    long double v[64];
+    FactTable()
+    {
+        v[0] = 1.0L;
+        for (int i = 1; i < 64; ++i) v[i] = v[i - 1] * (long double)i;
+    }
+};
+
 long double fact(int n)
 {
-    static long double tab[64];
-    static bool ready = false;
-    if (!ready) {
-        tab[0] = 1.0L;
-        for (int i = 1; i < 64; ++i) tab[i] = tab[i - 1] * (long double)i;
-        ready = true;
-    }
-    return tab[n];
+    static const FactTable tab; // function-local static: initialised once, thread-safe (C++11)
+    return tab.v[n];
 }
 
 } // namespace
@@ -205,14 +208,30 @@ void build_factorised(HostTables &t)
             const int *lam = &t.multiplets[(size_t)iL * 3];
             Lam4 q{};
             q.l1 = lam[0]; q.l2 = lam[1]; q.l3 = lam[2]; q.odd = t.parity[iL];
-            for (int m3 = 0; m3 <= q.l3; ++m3) {
+            // m3 = 0 half terms, m1 = 0 .. min(l1,l2):  with c = (l1 l2 l3; m1 -m1 0), s = (-1)^{m1},
+            //   T = c s a1_{m1} conj(a2_{m1}),  G_0 = T(m1=0) + sum_{m1>0} [T + sigma conj T],  sigma = (-1)^{l1+l2+l3}
+            //   even: G_0 = c0 r1 r2 + sum 2 c s (r1 r2 + i1 i2)          (real)
+            //   odd : G_0 = i sum 2 c s (i1 r2 - r1 i2)                   (imaginary; (l1 l2 l3; 0 0 0) = 0)
+            q.tbeg[0] = (int)t.pair_terms.size();
+            for (int m1 = 0; m1 <= std::min(q.l1, q.l2); ++m1) {
+                const double c = encore_host_wigner3j(q.l1, q.l2, q.l3, m1, -m1, 0);
+                if (std::fabs(c) < 1e-15) continue;
+                const double w = (m1 == 0 ? 1.0 : 2.0) * ((m1 & 1) ? -c : c);
+                const int re = m1 == 0 ? 0 : 2 * m1 - 1, im = m1 == 0 ? 0 : 2 * m1;
+                PairTerm pt{};
+                if (!q.odd) { pt.ia_re = re; pt.ib_re = re; pt.ia_im = im; pt.ib_im = im; pt.wrr = w; pt.wii = m1 ? w : 0.0; }
+                else if (m1 > 0) { pt.ia_re = im; pt.ib_re = re; pt.ia_im = re; pt.ib_im = im; pt.wrr = w; pt.wii = -w; }
+                else continue;
+                t.pair_terms.push_back(pt);
+            }
+            for (int m3 = 1; m3 <= q.l3; ++m3) {
                 q.tbeg[m3] = (int)t.pair_terms.size();
                 // G_{m3} = 2 S(m3) sum_{m1+m2=-m3} (l1 l2 l3; m1 m2 m3) a~1 a~2   (eq. 44 with E C = plain 3-j, eq. 18)
-                coupled_pair_terms(q.l1, q.l2, q.l3, -m3, m3 == 0 ? 1.0 : 2.0, t.pair_terms);
+                coupled_pair_terms(q.l1, q.l2, q.l3, -m3, 2.0, t.pair_terms);
             }
-            for (int m3 = q.l3 + 1; m3 < 9; ++m3) q.tbeg[m3] = (int)t.pair_terms.size();
+            for (int m3 = q.l3 + 1; m3 < ENCORE_MAX_LMAX + 2; ++m3) q.tbeg[m3] = (int)t.pair_terms.size();
             q.nterms = q.tbeg[q.l3 + 1] - q.tbeg[0];
-            cost[iL] = q.nterms + 0.3 * (q.l3 + 1);
+            cost[iL] = (q.tbeg[q.l3 + 1] - q.tbeg[1]) + 0.5 * (q.tbeg[1] - q.tbeg[0]) + 0.3 * (q.l3 + 1);
             t.lam4.push_back(q);
         }
     } else if (t.order == 5) {

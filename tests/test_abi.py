@@ -52,7 +52,13 @@ def test_plan_argument_validation():
     for args in bad:
         assert lib.encore_plan(C.byref(h), *args) == E.EINVAL, args
     assert lib.encore_plan(C.byref(h), 3, 0.0, 100.0, 5, 11, 0.0) == E.EUNSUPPORTED
-    assert lib.encore_plan(C.byref(h), 4, 0.0, 100.0, 5, 7, 0.0) == E.EUNSUPPORTED
+    assert lib.encore_plan(C.byref(h), 4, 0.0, 100.0, 5, 11, 0.0) == E.EUNSUPPORTED
+    # the paper's own GPU test shape: 4PCF at lmax = 10 has 381 multiplets and 45 720 outputs
+    with E.Plan(4, 0.0, 200.0, 10, 10, 1500.0) as p4:
+        assert (p4.n_lambda, p4.n_b, p4.n_lambda * p4.n_b) == (381, 120, 45720)
+    # 5PCF at lmax = 5, N_r = 10: 1406 x 210 = 295 260 outputs
+    with E.Plan(5, 0.0, 200.0, 10, 5, 1500.0) as p5:
+        assert (p5.n_lambda, p5.n_b, p5.n_lambda * p5.n_b) == (1406, 210, 295260)
     assert lib.encore_plan(None, 3, 0.0, 100.0, 5, 2, 0.0) == E.EINVAL
     assert lib.encore_destroy(None) == E.EINVAL
     assert b"invalid" in lib.encore_strerror(E.EINVAL)

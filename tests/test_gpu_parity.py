@@ -123,7 +123,7 @@ def test_small_clouds_open_and_periodic(E, oracle, order, nbins, lmax):
 
 
 @pytest.mark.parametrize("order,nbins", [(3, 6), (3, 7), (3, 8), (3, 9), (3, 12), (4, 4), (4, 5), (4, 6), (4, 7), (4, 8), (4, 9), (4, 11),
-                                         (5, 6), (5, 7), (5, 9)])
+                                         (5, 6), (5, 7), (5, 9), (5, 10), (5, 11)])
 def test_every_bin_count_of_the_factorised_contraction(E, oracle, order, nbins):
     """one case per template instantiation of the N=3 / N=4 / N=5 contraction kernels (and the generic fallback above them)"""
     rng = np.random.default_rng(7000 + 20 * order + nbins)
@@ -131,6 +131,32 @@ def test_every_bin_count_of_the_factorised_contraction(E, oracle, order, nbins):
     pos = np.ascontiguousarray(rng.uniform(0, 60.0, (3, n)))
     w = rng.uniform(0.5, 1.5, n)
     check_full(E, oracle, order, pos, w, 0.0, 3.0, 40.0, nbins, {3: 3, 4: 2, 5: 1}[order], alm_samples=(3,))
+
+
+@pytest.mark.parametrize("order,nbins,lmax,n", [(4, 10, 10, 260), (4, 10, 7, 260), (4, 9, 6, 200), (4, 10, 6, 200), (4, 6, 9, 200),
+                                                (5, 10, 5, 90), (5, 9, 3, 120), (5, 8, 4, 120), (5, 8, 5, 100)])
+def test_paper_gpu_shapes_and_largest_factorised_shapes(E, oracle, order, nbins, lmax, n):
+    """the paper's own GPU test shapes on the factorised kernels - 4PCF at lmax = 10 (381 multiplets, 45 720 outputs;
+    PAPER.md:537, :586) and 5PCF at lmax = 5, N_r = 10 (1406 x 210 = 295 260 outputs) - and the largest
+    template shapes (single-buffered tile pipeline, 255-register kernels), at reduced particle counts"""
+    rng = np.random.default_rng(9000 + 100 * order + 10 * nbins + lmax)
+    pos = np.ascontiguousarray(rng.uniform(0, 70.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n)
+    dev = torch.device("cuda:0")
+    o = oracle.zeta(order, pos, w, 0.0, 3.0, 45.0, nbins, lmax)
+    with E.Plan(order, 3.0, 45.0, nbins, lmax, 0.0) as plan:
+        if (order, nbins, lmax) == (4, 10, 10):
+            assert (plan.n_lambda, plan.n_lambda * plan.n_b) == (381, 45720)
+        if (order, nbins, lmax) == (5, 10, 5):
+            assert (plan.n_lambda, plan.n_lambda * plan.n_b) == (1406, 295260)
+        ex, ca = E.encore_contraction_flops(plan.h)
+        assert ex < ca                                  # the factorised kernels ran (the generic one executes more than the canonical model)
+        z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+        assert E.encore_get_status(plan.h) == E.OK
+        counts, _ = E.encore_get_bin_counts(plan.h, nbins)
+    assert (counts == o["bin_counts"]).all()
+    scale = np.abs(o["zeta"]).max()
+    assert np.abs(z - o["zeta"]).max() <= TOL * scale
 
 
 def test_degenerate_inputs(E, oracle):
@@ -363,7 +389,8 @@ def test_shard_argument_errors(E):
 
 # ---- ALLPARITY: parity-odd multiplets, zeta imaginary ----------------
 @pytest.mark.parametrize("order,nbins,lmax,box", [(4, 10, 3, 0.0), (4, 6, 4, 90.0), (4, 11, 2, 0.0), (5, 8, 2, 0.0),
-                                                  (5, 5, 2, 90.0), (5, 9, 1, 0.0), (3, 4, 3, 0.0)])
+                                                  (5, 5, 2, 90.0), (5, 9, 1, 0.0), (3, 4, 3, 0.0), (4, 10, 6, 0.0), (4, 9, 7, 90.0),
+                                                  (5, 10, 2, 0.0)])
 def test_allparity_matches_the_oracle(E, oracle, order, nbins, lmax, box):
     rng = np.random.default_rng(4200 + 10 * order + nbins)
     n = 300 if order == 4 else 180
