@@ -59,7 +59,7 @@ struct Lam5 {
 // One CTA of the factorised N = 4, 5 kernels: its multiplets and the l-blocks of the a_lm tile they need (only those
 // are brought into shared memory; a block l is the (2l+1) x nbins x 32 doubles starting at component l^2).
 struct CtaPlan {
-    int lam[8];                     // multiplet per slot, -1: empty
+    int lam[12];                    // multiplet per slot (at most 12: one warp per multiplet), -1: empty
     int nblk;
     int bl[ENCORE_MAX_LMAX + 1];    // l of block j
     int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged

@@ -741,6 +741,7 @@ __global__ void __launch_bounds__(nw5(NB) * lpc5(NB) * 32, 1) k_contract5(Contra
 
 // ---- host side: multiplets -> CTAs, l-blocks per CTA, shared memory ----------------------------------------------
 static int lpc_of(int order, int nb) { return order == 4 ? lpc4(nb) : lpc5(nb); }
+static_assert(kCtaWarps <= 12, "CtaPlan::lam has 12 slots");
 static constexpr size_t kSmemLimit = 224 * 1024;
 
 template <int NB>
@@ -814,7 +815,7 @@ size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas)
         if (tile_bytes(m) + extra > kSmemLimit) return 0;
         if (fill == lpc || tile_bytes(masks.back() | m) + extra > kSmemLimit) {
             CtaPlan c{};
-            for (int j = 0; j < 8; ++j) c.lam[j] = -1;
+            for (int j = 0; j < 12; ++j) c.lam[j] = -1;
             ctas.push_back(c);
             masks.push_back(0u);
             fill = 0;
