@@ -1,19 +1,22 @@
 #!/usr/bin/env python
 """bench.py — throughput of the ENCORE hot path (steps a1..a6) on B200, one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--impl ours|reference] [--all-configs]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--impl ours|reference] [--no-per-config]
 
 A "step" is one encore_compute over one synthetic catalogue (all of a1..a6).  The default workload is c3, the
 4PCF configuration BASELINE.json's target is stated on (300 000 lognormal-clustered points, 10 bins in [20,160],
-lmax=5); `--all-configs` adds one measured line per config c1..c5 under "per_config".
+lmax=5); the default line also carries one measured entry per config c1..c5 under "per_config" (2 steps each).
   value  = primaries/s with the catalogue already resident in HBM (CUDA events over K steps, max over ranks);
   e2e    = the same through encore_compute_host with pinned HOST buffers (H2D of positions+weights and D2H of
            zeta inside the timed region);
-  roofline = dominant kernel (the a_lm pair stage), plain FP64 ALU bound, timed live with the library's CUDA events
-           on the compute stream; algorithmic flops per DESIGN.md §7;
-  cpu_baseline = the oracle as it stands on this box's host cores on a strided subset of primaries.
-N > 1: every rank runs an independent catalogue of the same recipe (seed + rank) — separate mocks / D-R splits are
-how the paper spends extra nodes — no data-path collective; "scaling": "weak".
+  roofline = the kernel that takes the largest share of the step, `roofline_kernels` = one entry per real kernel
+           (k_fill, k_harm<..>, k_contract*), each timed live with the library's CUDA events on the compute stream;
+           algorithmic flops per DESIGN.md §7; plain FP64 / FP32 ALU bounds;
+  cpu_baseline = the oracle as it stands on this box's host cores on a strided subset of primaries, with its own
+           split into a_lm-stage and contraction seconds.
+N > 1 (torchrun): ONE catalogue sharded over primaries (encore_compute_shard + the NCCL all-gather of
+paper_2105_08722_b200.sharded inside the timed region), "scaling": "strong";
+the independent-catalogue arm (one mock per rank, no collective) is reported beside it under "replicas".
 `--impl reference` times the CPU oracle (test infrastructure) on the same config and metric.
 """
 from __future__ import annotations
@@ -22,6 +25,7 @@ import argparse
 import dataclasses
 import json
 import os
+import platform
 import statistics
 import subprocess
 import sys
@@ -36,10 +40,11 @@ if ROOT not in sys.path:
 
 import workloads as W  # noqa: E402
 
-SM_COUNT, FP64_LANES_PER_SM = 148, 64
-# dram__bytes_read.sum + dram__bytes_write.sum of k_fill + k_harm per step, from the committed `ncu --set full` capture
-# profiles/r1_v7_ncu_full.txt (an ALU-bound stage: the traffic is the candidate lists written and read back once)
-NCU_PAIR_STAGE_DRAM_BYTES = {"c3": 19.65e9}
+SM_COUNT, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this
+# round's kernels on c3 (profiles/r2_ncu_full_c3.txt names the command); None for workloads that were not captured
+NCU_DRAM_BYTES = {"c3": {"k_fill": 1.95e9, "k_harm": 2.96e9, "k_contract": None}}
+NCU_PROFILE = "profiles/r2_ncu_full_c3.txt"
 
 
 def peaks():
@@ -52,8 +57,18 @@ def peaks():
 
 # ---- algorithmic work models ------------------------------------------------
 def pair_flops(lmax: int, accepted: int, candidates: int) -> float:
-    """per accepted pair 4.5 (lmax+1)^2 + 25 flop, per rejected candidate 12 flop."""
+    """stage model: per accepted pair 4.5 (lmax+1)^2 + 25 flop, per rejected candidate 12 flop."""
     return accepted * (4.5 * (lmax + 1) ** 2 + 25.0) + max(0, candidates - accepted) * 12.0
+
+
+def fill_flops(candidates: int) -> float:
+    """k_fill's share of the stage model: separation + r^2 + bin of every candidate that reaches the pair test."""
+    return 12.0 * candidates
+
+
+def harm_flops(lmax: int, accepted: int) -> float:
+    """k_harm's share: everything of an accepted pair but the 12 flop already charged to k_fill."""
+    return accepted * (4.5 * (lmax + 1) ** 2 + 13.0)
 
 
 class ClockSampler:
@@ -100,8 +115,20 @@ def make_catalogue(cfg: W.Config, rank: int):
     return W.make(cfg)
 
 
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return platform.processor() or "unknown"
+
+
 def oracle_sample(cfg: W.Config, pos, w, target_s: float = 15.0):
-    """Oracle (as it stands) on primaries 0, stride, 2 stride, ...; returns (primaries/s, description, cores, seconds)."""
+    """Oracle (as it stands) on primaries 0, stride, 2 stride, ... against the full catalogue.
+
+    Returns dict(value primaries/s, sample, cores, seconds, pair_stage_seconds, contraction_seconds)."""
     import oracle
     oracle.build()
     cores = oracle.num_threads()
@@ -115,9 +142,16 @@ def oracle_sample(cfg: W.Config, pos, w, target_s: float = 15.0):
     stride = max(1, n // want)
     cnt = len(range(0, n, stride))
     t0 = time.perf_counter()
-    oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, prim_stride=stride)
+    o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, prim_stride=stride)
     dt = time.perf_counter() - t0
-    return cnt / dt, f"{cnt} of {n} primaries (every {stride}th) against the full catalogue, {dt:.1f} s", cores, dt
+    return {"value": cnt / dt, "sample": f"{cnt} of {n} primaries (every {stride}th) against the full catalogue, {dt:.1f} s",
+            "cores": cores, "seconds": dt, "pair_stage_seconds": o["stage_seconds"][0], "contraction_seconds": o["stage_seconds"][1]}
+
+
+def cpu_baseline_entry(s):
+    return {"value": s["value"], "unit": "primaries/s", "cores": s["cores"], "kind": "oracle", "sample": s["sample"],
+            "pair_stage_seconds": s["pair_stage_seconds"], "contraction_seconds": s["contraction_seconds"],
+            "nproc": os.cpu_count(), "cpu_model": cpu_model()}
 
 
 def run_reference(args, cfg):
@@ -128,61 +162,72 @@ def run_reference(args, cfg):
     vals = []
     per = max(2.0, 60.0 / max(1, args.steps + args.warmup))
     for it in range(args.warmup + args.steps):
-        v, desc, cores, dt = oracle_sample(cfg, pos, w, target_s=per)
+        s = oracle_sample(cfg, pos, w, target_s=per)
         if it >= args.warmup:
-            vals.append((v, dt, desc))
-    value = statistics.mean(v for v, _, _ in vals)
+            vals.append(s)
+    value = statistics.mean(s["value"] for s in vals)
     line = {
         "impl": "reference", "metric": "primaries_per_s", "value": value, "unit": "primaries/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * statistics.mean(d for _, d, _ in vals),
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, args),
-        "cpu_baseline": {"value": value, "unit": "primaries/s", "cores": cores, "kind": "oracle", "sample": vals[-1][2]},
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * statistics.mean(s["seconds"] for s in vals),
+        "higher_is_better": True, "scaling": "strong" if args.gpus > 1 else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args.gpus),
+        "cpu_baseline": dict(cpu_baseline_entry(vals[-1]), value=value),
         "e2e": {"value": value, "unit": "primaries/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
 
 
-def workload_config(cfg, args):
-    return {"workload": f"{cfg.name}{' ALLPARITY' if getattr(args, 'allparity', False) else ''}: {cfg.order}PCF, n={cfg.n} {cfg.kind} points, "
+def workload_config(cfg, world, allparity=False):
+    return {"workload": f"{cfg.name}{' ALLPARITY' if allparity else ''}: {cfg.order}PCF, n={cfg.n} {cfg.kind} points, "
                         f"{'periodic L=%g' % cfg.box if cfg.box > 0 else 'open cut-sky shell'}, weights {cfg.weights}, "
                         f"{cfg.nbins} bins in [{cfg.rmin:g},{cfg.rmax:g}], lmax={cfg.lmax}",
-            "l2": "256 MiB device memset between steps inside the timed bracket; per-step intermediates (a_lm tiles, "
-                  "per-group zeta partials) exceed the 126 MB L2",
-            "sharding": "one independent catalogue per rank (seed + 100 rank), no collective"}
+            "l2": "256 MiB device memset between steps inside the timed bracket; per-step intermediates (acceptance-mask rows, "
+                  "a_lm tiles) exceed the 126 MB L2",
+            "sharding": ("one catalogue, primaries sharded over the ranks (encore_compute_shard), one NCCL all-gather of the "
+                         "partial zeta per step" if world > 1 else "single GPU")}
 
 
-def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False):
-    pos, w = make_catalogue(cfg, rank)
+def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False, shard=None):
+    """shard = (rank, world): time sharded.compute_sharded (one catalogue, all-gather inside); None: the whole catalogue."""
+    from paper_2105_08722_b200 import sharded
+    pos, w = make_catalogue(cfg, rank if shard is None else 0)
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     plan = E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box, allparity=allparity)
     E.encore_set_timing(plan.h, True)
     out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream(dev)
-    for _ in range(warmup):
+
+    def one_step():
         flush.zero_()
-        plan.compute(tp, tw, out=out)
+        if shard is None:
+            plan.compute(tp, tw, out=out)
+        else:
+            sharded.compute_sharded(plan, tp, tw)
+
+    for _ in range(warmup):
+        one_step()
     torch.cuda.synchronize(dev)
-    stages = []
+    kern = []
     barrier()
     torch.cuda.synchronize(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(steps):
-        flush.zero_()
-        plan.compute(tp, tw, out=out)
-        stages.append(E.encore_get_stage_ms(plan.h))   # events of the library's own stream records; syncs that step
+        one_step()
+        kern.append(E.encore_get_kernel_ms(plan.h))   # events of the library's own stream records; syncs that step
     e1.record(stream)
     torch.cuda.synchronize(dev)
     barrier()
     ms = e0.elapsed_time(e1)
+    assert E.encore_get_status(plan.h) == E.OK
     launches = E.encore_get_launch_count(plan.h)
     counts, pairs = E.encore_get_bin_counts(plan.h, cfg.nbins)
     cand = E.encore_get_candidate_pairs(plan.h)
-    res = {"ms_total": ms, "stages": {k: statistics.mean(s[k] for s in stages) for k in stages[0]}, "launches": launches,
-           "pairs": pairs, "candidates": cand, "flops_contraction": E.encore_contraction_flops(plan.h),
-           "nout": plan.n_lambda * plan.n_b, "grid": E.encore_get_grid(plan.h)}
+    km = {k: statistics.mean(s[k] for s in kern) for k in kern[0]}
+    res = {"ms_total": ms, "kernel_ms": km, "launches": launches, "pairs": pairs, "candidates": cand,
+           "flops_contraction": E.encore_contraction_flops(plan.h), "nout": plan.n_lambda * plan.n_b,
+           "grid": E.encore_get_grid(plan.h), "pair_steps": E.encore_get_pair_steps(plan.h)}
     if want_e2e:
         hp = torch.from_numpy(pos).pin_memory()
         hw = torch.from_numpy(w).pin_memory()
@@ -201,6 +246,62 @@ def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allpa
         res["d2h"] = hz.numel() * 8
     plan.close()
     return res, (pos, w)
+
+
+def stage_ms(km):
+    return {"grid": km["grid"], "sort": km["sort"], "pair": km["bounds"] + km["k_fill"] + km["k_harm"],
+            "contraction": km["k_contract"], "reduce": km["reduce"]}
+
+
+def kernel_rooflines(cfg, res, fp64_peak, fp32_peak):
+    """one entry per real kernel of the step, the one with the largest share of the step first"""
+    km = res["kernel_ms"]
+    ex, ca = res["flops_contraction"]
+    hname = f"k_harm<{cfg.lmax}, 0, {cfg.lmax if cfg.lmax <= 7 else (2 if cfg.lmax == 8 else 3)}, {1 if cfg.box > 0 else 0}>"
+    if cfg.lmax > 7:
+        hname += f" + k_harm<{cfg.lmax}, {3 if cfg.lmax == 8 else 4}, {cfg.lmax}, {1 if cfg.box > 0 else 0}>"
+    cname = {3: f"k_contract3<{cfg.nbins}>", 4: f"k_contract4<{cfg.nbins}>", 5: f"k_contract5<{cfg.nbins}>"}[cfg.order]
+    traffic = NCU_DRAM_BYTES.get(cfg.name, {})
+    ents = []
+
+    def ent(kernel, ms, flops, peak, bound, unit_peak, **extra):
+        ach = flops / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        e = {"kernel": kernel, "bound": bound, "ms": ms, "achieved": ach, "peak": peak / 1e12, "unit": "TFLOP/s",
+             "frac": ach * 1e12 / peak, "share_of_step": None, "peak_kind": unit_peak}
+        e.update(extra)
+        return e
+    ents.append(ent(f"k_fill<{1 if cfg.box > 0 else 0}>", km["k_fill"], fill_flops(res["candidates"]), fp32_peak, "alu", "fp32 FMA lanes",
+                    model="12 flop per candidate pair that reaches the pair test (fp32 screening, exact fp64 fallback); the kernel is "
+                          "bound by instruction issue (integer + fp32 mix), not by the fp32 pipe",
+                    traffic=traffic.get("k_fill")))
+    ents.append(ent(hname, km["k_harm"], harm_flops(cfg.lmax, res["pairs"]), fp64_peak, "alu", "fp64 FMA lanes",
+                    model="4.5 (lmax+1)^2 + 13 flop per accepted pair", traffic=traffic.get("k_harm")))
+    ents.append(ent(cname, km["k_contract"], cfg.n * ex, fp64_peak, "alu" if cfg.order > 3 else "hbm", "fp64 FMA lanes",
+                    model="executed flops of the factorised kernel (FMA = 2), encore_contraction_flops",
+                    canonical_model_tflops=cfg.n * ca / (km["k_contract"] * 1e-3) / 1e12 if km["k_contract"] > 0 else 0.0,
+                    traffic=traffic.get("k_contract")))
+    tot = sum(km.values())
+    for e in ents:
+        e["share_of_step"] = e["ms"] / tot if tot > 0 else 0.0
+    ents.sort(key=lambda e: -e["ms"])
+    return ents
+
+
+def config_entry(cfg, res, steps, fp64_peak, fp32_peak):
+    ms1 = res["ms_total"] / steps
+    km = res["kernel_ms"]
+    st = stage_ms(km)
+    ex, ca = res["flops_contraction"]
+    pf = pair_flops(cfg.lmax, res["pairs"], res["candidates"])
+    return {"order": cfg.order, "n": cfg.n, "ms_per_step": ms1, "primaries_per_s": cfg.n / (ms1 * 1e-3),
+            "pairs_per_s": res["pairs"] / (ms1 * 1e-3), "accepted_pairs": res["pairs"], "candidate_pairs": res["candidates"],
+            "pair_steps": res["pair_steps"], "stage_ms": st, "kernel_ms": km,
+            "pair_frac_fp64": pf / (st["pair"] * 1e-3) / fp64_peak,
+            "pair_frac_fp64_accepted_only": res["pairs"] * (4.5 * (cfg.lmax + 1) ** 2 + 25.0) / (st["pair"] * 1e-3) / fp64_peak,
+            "k_harm_frac_fp64": harm_flops(cfg.lmax, res["pairs"]) / (km["k_harm"] * 1e-3) / fp64_peak if km["k_harm"] > 0 else 0.0,
+            "contraction_gflops_canonical": cfg.n * ca / (st["contraction"] * 1e-3) / 1e9,
+            "contraction_gflops_executed": cfg.n * ex / (st["contraction"] * 1e-3) / 1e9,
+            "contraction_frac_fp64_executed": cfg.n * ex / (st["contraction"] * 1e-3) / fp64_peak}
 
 
 _DIST = {"on": False}
@@ -228,7 +329,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c3", choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--all-configs", action="store_true", help="also measure c1..c5 (2 steps each) into per_config")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the c1..c5 entries (2 steps each) of per_config")
+    ap.add_argument("--all-configs", action="store_true", help="(default now) kept for compatibility")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--allparity", action="store_true", help="ALLPARITY plan: parity-odd multiplets too (not the headline config)")
     args = ap.parse_args()
@@ -252,74 +354,73 @@ def main():
         _DIST["on"] = True
     hbm_gbs, sm_max_mhz, peak_src = peaks()
     steps, warmup = args.steps, max(3, args.warmup)
+    fp64_peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6
+    fp32_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6
 
     with ClockSampler(local) as clocks:
-        res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev, allparity=args.allparity)
+        res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev, allparity=args.allparity,
+                                       shard=(rank, world) if world > 1 else None)
     ms_total = max_over_ranks(torch, res["ms_total"], dev)
     e2e_ms = max_over_ranks(torch, res["e2e_ms_total"], dev)
     ms_per_step = ms_total / steps
-    value = world * cfg.n / (ms_per_step * 1e-3)
-    st = res["stages"]
+    value = cfg.n / (ms_per_step * 1e-3)          # world > 1: ONE catalogue, sharded (strong scaling)
+    km = res["kernel_ms"]
+    st = stage_ms(km)
 
     fp64_measured = E.encore_measure_fp64_peak()
-    peak_derived = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6
+    ents = kernel_rooflines(cfg, res, fp64_peak, fp32_peak)
+    top = ents[0]
     pf = pair_flops(cfg.lmax, res["pairs"], res["candidates"])
-    pair_tflops = pf / (st["pair"] * 1e-3) / 1e12
     ex_flops, ca_flops = res["flops_contraction"]
     grid_bytes = cfg.n * (24 + 4)                        # a1: read x,y,z, write cell id
     sort_bytes = cfg.n * (4 + 4 + 4 + 4 + 4 + 32 + 32)   # a2: cid re-read, scatter idx w+r, rank idx, pos+w gather r+w
     line = {
         "metric": "primaries_per_s", "value": value, "unit": "primaries/s", "n_gpus": world, "steps": steps, "warmup": warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": workload_config(cfg, args),
-        "pairs_per_s": world * res["pairs"] / (ms_per_step * 1e-3),
-        "pairs_per_s_pair_stage": res["pairs"] / (st["pair"] * 1e-3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, args.allparity),
+        "pairs_per_s": res["pairs"] / (ms_per_step * 1e-3) if world == 1 else None,   # (a shard only counts its own pairs)
         "accepted_pairs": res["pairs"], "candidate_pairs": res["candidates"],
-        "contraction_gflops_canonical": cfg.n * ca_flops / (st["contraction"] * 1e-3) / 1e9,
-        "contraction_gflops_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / 1e9,
-        "stage_ms": st,
+        "contraction_gflops_canonical": cfg.n * ca_flops / (st["contraction"] * 1e-3) / 1e9 if world == 1 else None,
+        "contraction_gflops_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / 1e9 if world == 1 else None,
+        "stage_ms": st, "kernel_ms": km,
         "stage_rooflines": {
             "grid_GBps": grid_bytes / (st["grid"] * 1e-3) / 1e9, "sort_GBps": sort_bytes / (st["sort"] * 1e-3) / 1e9,
             "hbm_peak_GBps": hbm_gbs,
-            "pair_frac_fp64": pair_tflops * 1e12 / peak_derived,
-            "contraction_frac_fp64_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / peak_derived,
+            "pair_frac_fp64": pf / (st["pair"] * 1e-3) / fp64_peak,
+            "pair_frac_fp64_accepted_only": res["pairs"] * (4.5 * (cfg.lmax + 1) ** 2 + 25.0) / (st["pair"] * 1e-3) / fp64_peak,
+            "contraction_frac_fp64_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / fp64_peak,
         },
-        "roofline": {"bound": "alu", "kernel": "k_pair (a3+a4)", "achieved": pair_tflops, "peak": peak_derived / 1e12,
-                     "unit": "TFLOP/s", "frac": pair_tflops * 1e12 / peak_derived,
-                     "traffic": NCU_PAIR_STAGE_DRAM_BYTES.get(cfg.name),
-                     "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} fp64 FMA lanes x 2 x {sm_max_mhz:g} MHz ({peak_src} clock)",
-                     "peak_measured_dfma_chain": fp64_measured / 1e12,
-                     "flops_model": "4.5 (lmax+1)^2 + 25 per accepted pair + 12 per rejected candidate (DESIGN.md §7)"},
-        "e2e": {"value": world * cfg.n / (e2e_ms / steps * 1e-3), "unit": "primaries/s",
-                "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
+        "roofline": {"bound": top["bound"], "kernel": top["kernel"], "achieved": top["achieved"], "peak": top["peak"],
+                     "unit": "TFLOP/s", "frac": top["frac"], "traffic": top.get("traffic"), "traffic_source": NCU_PROFILE,
+                     "ms": top["ms"], "share_of_step": top["share_of_step"], "model": top["model"],
+                     "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} fp64 (x {FP32_LANES_PER_SM} fp32) FMA lanes x 2 x "
+                                    f"{sm_max_mhz:g} MHz ({peak_src} clock); MEASURED_PEAKS.json has no fp64 entry",
+                     "peak_measured_dfma_chain": fp64_measured / 1e12},
+        "roofline_kernels": ents,
+        "e2e": {"value": cfg.n / (e2e_ms / steps * 1e-3), "unit": "primaries/s",
+                "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"],
+                "note": "encore_compute_host on this rank's GPU (whole catalogue)" if world > 1 else "encore_compute_host"},
         "gpu_launches": res["launches"] * steps,
         "clocks": clocks.summary(),
         "grid": {"nc": res["grid"][0], "sub": res["grid"][1]},
     }
+    if world > 1:
+        # the independent-catalogue arm: one mock per rank, no data-path collective, weak scaling
+        r2, _ = measure_config(E, torch, cfg, rank, max(2, steps // 2), 3, dev, want_e2e=False)
+        ms_rep = max_over_ranks(torch, r2["ms_total"], dev) / max(2, steps // 2)
+        line["replicas"] = {"value": world * cfg.n / (ms_rep * 1e-3), "unit": "primaries/s", "scaling": "weak", "ms_per_step": ms_rep,
+                            "sharding": "one independent catalogue per rank (seed + 100 rank), no collective"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, cores, _ = oracle_sample(cfg, pos, w, target_s=15.0)
-        line["cpu_baseline"] = {"value": v, "unit": "primaries/s", "cores": cores, "kind": "oracle", "sample": desc}
-    if args.all_configs and world == 1:
+        line["cpu_baseline"] = cpu_baseline_entry(oracle_sample(cfg, pos, w, target_s=15.0))
+    if world == 1 and not args.no_per_config:
         per = {}
         for name in sorted(W.CONFIGS):
             c = W.CONFIGS[name]
             r, _ = measure_config(E, torch, c, 0, 2, 3, dev, want_e2e=False)
-            s = r["stages"]
-            ex, ca = r["flops_contraction"]
-            ms1 = r["ms_total"] / 2
-            per[name] = {"order": c.order, "n": c.n, "ms_per_step": ms1, "primaries_per_s": c.n / (ms1 * 1e-3),
-                         "pairs_per_s": r["pairs"] / (ms1 * 1e-3), "accepted_pairs": r["pairs"], "stage_ms": s,
-                         "pair_frac_fp64": pair_flops(c.lmax, r["pairs"], r["candidates"]) / (s["pair"] * 1e-3) / peak_derived,
-                         "contraction_gflops_canonical": c.n * ca / (s["contraction"] * 1e-3) / 1e9,
-                         "contraction_frac_fp64_executed": c.n * ex / (s["contraction"] * 1e-3) / peak_derived}
+            per[name] = config_entry(c, r, 2, fp64_peak, fp32_peak)
         # the same c3 catalogue with the parity-odd multiplets too (111 instead of 69 multiplets)
         r, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, allparity=True)
-        ex, ca = r["flops_contraction"]
-        per["c3_allparity"] = {"order": 4, "n": W.CONFIGS["c3"].n, "ms_per_step": r["ms_total"] / 2,
-                               "primaries_per_s": W.CONFIGS["c3"].n / (r["ms_total"] / 2 * 1e-3), "stage_ms": r["stages"],
-                               "n_multiplets": r["nout"] // 120,
-                               "contraction_gflops_canonical": W.CONFIGS["c3"].n * ca / (r["stages"]["contraction"] * 1e-3) / 1e9,
-                               "contraction_frac_fp64_executed": W.CONFIGS["c3"].n * ex / (r["stages"]["contraction"] * 1e-3) / peak_derived}
+        per["c3_allparity"] = dict(config_entry(W.CONFIGS["c3"], r, 2, fp64_peak, fp32_peak), n_multiplets=r["nout"] // 120)
         line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))

@@ -147,6 +147,10 @@ int encore_get_alm(const encore_plan_t *plan, int64_t i, double *out);
 /* stage times of that call in ms: [0] grid (cell ids + histogram), [1] sort (scan, scatter, rank, gather, groups),
  * [2] pair (a3+a4), [3] contraction (a5), [4] reduction (a6).  Only measured when timing is enabled. */
 int encore_get_stage_ms(const encore_plan_t *plan, float ms[5]);
+/* per-kernel times of that call in ms, summed over the pair-stage super-steps: [0] grid (bounding box, cell ids),
+ * [1] sort, [2] k_group_bound + scan + the host read of the word counts, [3] k_fill, [4] k_harm (all passes),
+ * [5] contraction kernel, [6] reduction.  Only measured when timing is enabled. */
+int encore_get_kernel_ms(const encore_plan_t *plan, float ms[7]);
 int encore_set_timing(encore_plan_t *plan, int enabled);   /* record per-stage CUDA events (default off) */
 /* number of kernel launches the last encore_compute enqueued */
 int encore_get_launch_count(const encore_plan_t *plan);

@@ -60,7 +60,7 @@ def _load():
     lib.oracle_zeta.restype = C.c_int
     lib.oracle_zeta.argtypes = [C.c_int, dp, dp, C.c_int64, C.c_double, C.c_double, C.c_double,
                                 C.c_int, C.c_int, C.c_int, ip, C.c_int64, C.c_int64, C.c_int64,
-                                C.c_int, dp, dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), dp]
+                                C.c_int, dp, dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), dp, dp]
     lib.oracle_num_threads.restype = C.c_int
     _lib = lib
     return lib
@@ -161,7 +161,7 @@ def zeta(order, pos, w, box, rmin, rmax, nbins, lmax, *, allparity=False, bins=N
     """zeta^B_Lambda by eq. 34/35 over primaries offset, offset+stride, ...
 
     Returns dict(zeta[nLam,nB], zeta_im, bin_counts[nbins] uint64, prim_counts or None,
-    max_imag, multiplets, bins).
+    max_imag, multiplets, bins, stage_seconds=(a_lm stage, contraction) wall seconds).
     """
     lib = _load()
     pos = _pos(pos)
@@ -178,14 +178,15 @@ def zeta(order, pos, w, box, rmin, rmax, nbins, lmax, *, allparity=False, bins=N
     bc = np.zeros(nbins, dtype=np.uint64)
     pc = np.zeros((n, nbins), dtype=np.uint32) if want_prim_counts else None
     mi = C.c_double(0.0)
+    secs = np.zeros(2)
     wa = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
     rc = lib.oracle_zeta(order, _dp(pos), None if wa is None else _dp(wa), n, float(box),
                          float(rmin), float(rmax), nbins, lmax, int(allparity), bptr, nB,
                          int(prim_offset), int(prim_stride), int(force_allpairs), _dp(z), _dp(zi),
                          bc.ctypes.data_as(C.POINTER(C.c_uint64)),
                          None if pc is None else pc.ctypes.data_as(C.POINTER(C.c_uint32)),
-                         C.byref(mi))
+                         C.byref(mi), _dp(secs))
     if rc != 0:
         raise ValueError(f"oracle_zeta failed with status {rc}")
     return dict(zeta=z, zeta_im=zi, bin_counts=bc, prim_counts=pc, max_imag=mi.value,
-                multiplets=lam, bins=bt)
+                multiplets=lam, bins=bt, stage_seconds=(float(secs[0]), float(secs[1])))

@@ -488,6 +488,8 @@ int oracle_alm(const double *pos, const double *w, int64_t n, double box, double
  *   zeta_im  : optional [nLam][nB] imaginary part (odd parity) or NULL
  *   bin_counts: [nbins] accepted ordered pairs over the processed primaries
  *   prim_counts: optional [n][nbins] (rows of unprocessed primaries untouched)
+ *   stage_seconds: optional [2]: wall-clock seconds spent in step (i) (a_lm of every primary) and in steps
+ *              (ii)+(iii) (contraction and sum), each averaged over the OpenMP threads (timing only)
  * ------------------------------------------------------------------------------------------ */
 static int64_t n_choose(int n, int k)
 {
@@ -515,12 +517,22 @@ int64_t oracle_bin_tuples(int order, int nbins, int *out)
     return cnt;
 }
 
+static double wall_seconds(void)
+{
+#ifdef _OPENMP
+    return omp_get_wtime();
+#else
+    return 0.0;
+#endif
+}
+
 typedef struct { int idx[4]; double c; } term_t; /* idx[k] = l_k*l_k + l_k + m_k; c = E(Lam) C^Lam_M */
 
 int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double box, double rmin,
                 double rmax, int nbins, int lmax, int allparity, const int *bins, int64_t nB,
                 int64_t prim_offset, int64_t prim_stride, int force_allpairs, double *zeta,
-                double *zeta_im, uint64_t *bin_counts, uint32_t *prim_counts, double *max_imag)
+                double *zeta_im, uint64_t *bin_counts, uint32_t *prim_counts, double *max_imag,
+                double *stage_seconds)
 {
     if (order < 3 || order > ORACLE_MAX_ORDER || lmax > ORACLE_MAX_L || nbins > 255 || n < 1) return -1;
     if (box > 0.0 && rmax > 0.5 * box) return -2;
@@ -583,6 +595,7 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
     long double *part = (long double *)calloc(nout * 2 * (size_t)nthreads, sizeof(long double));
     uint64_t *cpart = (uint64_t *)calloc((size_t)nbins * nthreads, sizeof(uint64_t));
     double *imax = (double *)calloc((size_t)nthreads, sizeof(double));
+    double *tsec = (double *)calloc((size_t)nthreads * 2, sizeof(double));
     const int64_t nprim = prim_offset < n ? (n - prim_offset + prim_stride - 1) / prim_stride : 0;
 
 #pragma omp parallel
@@ -599,7 +612,9 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
 #pragma omp for schedule(dynamic, 8)
         for (int64_t ip = 0; ip < nprim; ++ip) {
             const int64_t i = prim_offset + ip * prim_stride;
+            const double t0 = wall_seconds();
             alm_primary(&c, &cl, i, alm, cnt, acc, acc + tile);      /* step (i) */
+            const double t1 = wall_seconds();
             for (int b = 0; b < nbins; ++b) {
                 cc[b] += cnt[b];
                 if (prim_counts) prim_counts[(size_t)i * nbins + b] = cnt[b];
@@ -617,6 +632,8 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
                     zr[(size_t)iL * nB + iB] += (long double)(wi * creal(H)); /* step (iii) */
                     zi[(size_t)iL * nB + iB] += (long double)(wi * cimag(H));
                 }
+            tsec[2 * tid] += t1 - t0;
+            tsec[2 * tid + 1] += wall_seconds() - t1;
         }
         free(alm); free(acc);
     }
@@ -631,13 +648,17 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
         if (fabs(im) > mi) mi = fabs(im);
     }
     if (max_imag) *max_imag = mi;
+    if (stage_seconds) {
+        stage_seconds[0] = stage_seconds[1] = 0.0;
+        for (int t = 0; t < nthreads; ++t) { stage_seconds[0] += tsec[2 * t] / nthreads; stage_seconds[1] += tsec[2 * t + 1] / nthreads; }
+    }
     if (bin_counts)
         for (int b = 0; b < nbins; ++b) {
             uint64_t s = 0;
             for (int t = 0; t < nthreads; ++t) s += cpart[(size_t)t * nbins + b];
             bin_counts[b] = s;
         }
-    free(part); free(cpart); free(imax); free(terms); free(tstart); free(Lam); free(own_bins);
+    free(part); free(cpart); free(imax); free(tsec); free(terms); free(tstart); free(Lam); free(own_bins);
     cl_free(&cl);
     return 0;
 }

@@ -29,7 +29,7 @@ SYMBOLS = [
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
     "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
-    "encore_get_stage_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs", "encore_get_harm_steps",
+    "encore_get_stage_ms", "encore_get_kernel_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs", "encore_get_harm_steps",
     "encore_measure_fp64_peak", "encore_strerror", "encore_last_cuda_error",
 ]
 
@@ -77,6 +77,7 @@ def lib():
     L.encore_get_alm.argtypes = [vp, C.c_int64, dp]
     L.encore_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.encore_set_timing.argtypes = [vp, C.c_int]
+    L.encore_get_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.encore_get_launch_count.argtypes = [vp]
     L.encore_get_candidate_pairs.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.encore_measure_fp64_peak.argtypes = [dp, vp]
@@ -239,6 +240,12 @@ def encore_get_stage_ms(plan):
     ms = (C.c_float * 5)()
     _check(lib().encore_get_stage_ms(plan, ms))
     return dict(zip(("grid", "sort", "pair", "contraction", "reduce"), [float(v) for v in ms]))
+
+
+def encore_get_kernel_ms(plan):
+    ms = (C.c_float * 7)()
+    _check(lib().encore_get_kernel_ms(plan, ms))
+    return dict(zip(("grid", "sort", "bounds", "k_fill", "k_harm", "k_contract", "reduce"), [float(v) for v in ms]))
 
 
 def encore_set_timing(plan, enabled: bool):

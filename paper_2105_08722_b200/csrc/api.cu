@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 namespace {
 
@@ -57,8 +58,9 @@ struct encore_plan_s {
     int g_begin = 0, g_end = 0, ngroups = 0;  // groups the last compute covered (a shard's range, or all) of how many
     cudaStream_t stream = nullptr;
     bool timing = false;
-    cudaEvent_t ev[6] = {};
-    bool ev_ready = false;
+    std::vector<cudaEvent_t> ev;    // event pool (timing only); ev[i] closes an interval of kind ev_kind[i]
+    std::vector<int> ev_kind;
+    size_t ev_used = 0;
     float ms[5] = {0, 0, 0, 0, 0};
     int launches = 0;
     int sub_yz_override = 0, sub_x_override = 0;
@@ -172,14 +174,22 @@ bool choose_geometry(const encore_plan_s *P, int64_t n, const double lo[3], cons
     return true;
 }
 
-int record(encore_plan_s *P, int k, cudaStream_t s)
+// interval kinds of encore_get_kernel_ms
+enum { K_GRID = 0, K_SORT, K_BOUNDS, K_FILL, K_HARM, K_CONTRACT, K_REDUCE, K_COUNT, K_START = -1 };
+
+// timing only: record an event that closes an interval of kind `kind` (K_START opens the first one)
+int mark(encore_plan_s *P, int kind, cudaStream_t s)
 {
     if (!P->timing) return ENCORE_OK;
-    if (!P->ev_ready) {
-        for (int i = 0; i < 6; ++i) CU(cudaEventCreate(&P->ev[i]));
-        P->ev_ready = true;
+    if (kind == K_START) P->ev_used = 0;
+    if (P->ev_used == P->ev.size()) {
+        cudaEvent_t e;
+        CU(cudaEventCreate(&e));
+        P->ev.push_back(e);
+        P->ev_kind.push_back(0);
     }
-    CU(cudaEventRecord(P->ev[k], s));
+    P->ev_kind[P->ev_used] = kind;
+    CU(cudaEventRecord(P->ev[P->ev_used++], s));
     return ENCORE_OK;
 }
 
@@ -255,10 +265,10 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
     CU(P->cand.ensure(3 * sizeof(unsigned long long)));   // candidate pairs, k_harm steps, k_harm ideal steps
 
-    TRY(record(P, 0, s));
+    TRY(mark(P, K_START, s));
     // ---- a1: cell ids + histogram -----------------------------------------------------------------------------
     CU(launch_cell_ids(pos, n, G, P->cid.as<int32_t>(), P->cell_count.as<int>(), s, &P->launches));
-    TRY(record(P, 1, s));
+    TRY(mark(P, K_GRID, s));
     // ---- a2: counting sort by cell, gather to AoS, groups of 32 per pencil ----------------------------------
     CU(launch_exclusive_scan(P->cell_count.as<int>(), P->cell_start.as<int>(), G.ncell, P->scan_tmp.as<int>(), s, &P->launches));
     CU(cudaMemsetAsync(P->cell_fill.p, 0, sizeof(int) * (size_t)G.ncell, s));
@@ -266,7 +276,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
                           P->sorted_idx.as<int>(), P->pos4.as<double4>(), s, &P->launches));
     CU(launch_pencil_groups(P->cell_start.as<int>(), G, P->groups.as<int>(), s, &P->launches));
     CU(launch_exclusive_scan(P->groups.as<int>(), P->group_start.as<int>(), G.npencil, P->scan_tmp.as<int>(), s, &P->launches));
-    TRY(record(P, 2, s));
+    TRY(mark(P, K_SORT, s));
     // ---- a3 + a4: pair stage -----------------------------------------------------------------------------------
     PairArgs pa{};
     pa.pos4 = P->pos4.as<double4>();
@@ -332,6 +342,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(cudaMemcpyAsync(P->h_gprefix, P->gprefix.p, sizeof(int) * ((size_t)ngmax + 1), cudaMemcpyDeviceToHost, s));
     CU(cudaMemcpyAsync(P->h_gprefix + ngmax + 1, P->group_start.as<int>() + G.npencil, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
+    TRY(mark(P, K_BOUNDS, s));
     {
         const int ngroups = P->h_gprefix[ngmax + 1];
         const int *gp = P->h_gprefix;
@@ -377,14 +388,16 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         while (g0 < g_end) {
             int g1 = g0 + 1;
             while (g1 < g_end && (size_t)(gp[g1 + 1] - gp[g0]) <= step_words) ++g1;
-            CU(launch_pair_fill_harmonics(pa, g0, g1, nr_cap, s, &P->launches));
+            CU(launch_pair_fill(pa, g0, g1, nr_cap, s, &P->launches));
+            TRY(mark(P, K_FILL, s));
+            CU(launch_pair_harmonics(pa, g0, g1, s, &P->launches));
+            TRY(mark(P, K_HARM, s));
             ++P->pair_steps;
             g0 = g1;
         }
     }
     // internal-consistency flag of the pair stage, read by whoever synchronises next (encore_get_status, the getters)
     CU(cudaMemcpyAsync(reinterpret_cast<int *>(P->pinned + 7), P->errflag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
-    TRY(record(P, 3, s));
     // ---- a5: contraction ---------------------------------------------------------------------------------------
     ContractArgs ca{};
     ca.order = T.order; ca.nbins = nb; ca.ncomp = ncomp; ca.nLam = T.nLam(); ca.nB = T.nB();
@@ -416,10 +429,10 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     ca.nchunk = nchunk;
     ca.factorised = factorised ? 1 : 0;
     CU(launch_contraction(ca, s, &P->launches));
-    TRY(record(P, 4, s));
+    TRY(mark(P, K_CONTRACT, s));
     // ---- a6: reduction -----------------------------------------------------------------------------------------
     CU(launch_reduction(ca, s, &P->launches));
-    TRY(record(P, 5, s));
+    TRY(mark(P, K_REDUCE, s));
 
     P->have = true; P->n = n; P->geom = G; P->ngroups_max = ngmax; P->stream = s;
     P->g_begin = g_begin; P->g_end = g_end; P->ngroups = ngroups_total;
@@ -555,7 +568,7 @@ int encore_destroy(encore_plan_t *P)
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
-    if (P->ev_ready) for (int i = 0; i < 6; ++i) cudaEventDestroy(P->ev[i]);
+    for (cudaEvent_t e : P->ev) cudaEventDestroy(e);
     delete P;
     return ENCORE_OK;
 }
@@ -695,13 +708,27 @@ int encore_get_alm(const encore_plan_t *Pc, int64_t i, double *out)
     return ENCORE_OK;
 }
 
-int encore_get_stage_ms(const encore_plan_t *Pc, float ms[5])
+int encore_get_kernel_ms(const encore_plan_t *Pc, float ms[7])
 {
     encore_plan_t *P = const_cast<encore_plan_t *>(Pc);
     if (!P || !ms) return ENCORE_EINVAL;
-    if (!P->have || !P->timing || !P->ev_ready) return ENCORE_ESTATE;
-    CU(cudaEventSynchronize(P->ev[5]));
-    for (int k = 0; k < 5; ++k) CU(cudaEventElapsedTime(&ms[k], P->ev[k], P->ev[k + 1]));
+    if (!P->have || !P->timing || P->ev_used < 2) return ENCORE_ESTATE;
+    CU(cudaEventSynchronize(P->ev[P->ev_used - 1]));
+    for (int k = 0; k < K_COUNT; ++k) ms[k] = 0.f;
+    for (size_t i = 1; i < P->ev_used; ++i) {
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, P->ev[i - 1], P->ev[i]));
+        ms[P->ev_kind[i]] += t;
+    }
+    return ENCORE_OK;
+}
+
+int encore_get_stage_ms(const encore_plan_t *Pc, float ms[5])
+{
+    float k[K_COUNT];
+    const int rc = encore_get_kernel_ms(Pc, k);
+    if (rc != ENCORE_OK) return rc;
+    ms[0] = k[K_GRID]; ms[1] = k[K_SORT]; ms[2] = k[K_BOUNDS] + k[K_FILL] + k[K_HARM]; ms[3] = k[K_CONTRACT]; ms[4] = k[K_REDUCE];
     return ENCORE_OK;
 }
 

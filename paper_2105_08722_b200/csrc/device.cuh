@@ -78,9 +78,10 @@ struct PairArgs {
     int bin_order[ENCORE_MAX_BINS]; // bins by decreasing shell volume (work per item)
 };
 // per-group word counts -> gbound, gprefix, gwide (device).  The caller reads gprefix back, sizes the row buffer, and
-// calls launch_pair_fill_harmonics once per super-step [g0, g1); nr_cap >= number of candidate runs of a group.
+// calls launch_pair_fill then launch_pair_harmonics once per super-step [g0, g1); nr_cap >= number of candidate runs of a group.
 cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches);
-cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches);
+cudaError_t launch_pair_fill(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches);
+cudaError_t launch_pair_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches);
 size_t pair_fill_smem_bytes(int nbins, int nr_cap);
 int pair_stage_supported(int lmax, int nbins);
 

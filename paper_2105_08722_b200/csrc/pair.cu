@@ -838,7 +838,7 @@ cudaError_t launch_pair_bounds(const PairArgs &a, cudaStream_t s, int *launches)
 // m-ranges per lmax.  Every pass walks the rows and gathers the candidates again (the L1 data pipe is ~70 % busy),
 // so fewer, fatter passes win: up to 44 accumulators run at 168 registers and 12 warps/SM, 45-65 at 255 registers and
 // 8 warps/SM (c2, lmax 10: four passes 46.3 ms, three 40.1 ms, two 37.1 ms for the pair stage).
-cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches)
+cudaError_t launch_pair_fill(const PairArgs &a, int g0, int g1, int nr_cap, cudaStream_t s, int *launches)
 {
     const int ng = g1 - g0, nb = a.bins.nbins;
     if (ng <= 0) return cudaSuccess;
@@ -854,8 +854,12 @@ cudaError_t launch_pair_fill_harmonics(const PairArgs &a, int g0, int g1, int nr
     if (a.geom.periodic) k_fill<true><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
     else k_fill<false><<<ng, 32, smem, s>>>(a, g0, g1, nr_cap);
     *launches += 1;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pair_harmonics(const PairArgs &a, int g0, int g1, cudaStream_t s, int *launches)
+{
+    if (g1 - g0 <= 0) return cudaSuccess;
     switch (a.lmax) {
     case 0: HARM_PASS(0, 0, 0) break;
     case 1: HARM_PASS(1, 0, 1) break;

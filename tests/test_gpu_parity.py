@@ -378,6 +378,36 @@ def test_shards_add_up_to_the_oracle(E, oracle, name, nshards):
     assert np.abs(total.ravel() - o["zeta"].ravel()).max() <= TOL * scale
 
 
+def test_compute_sharded_under_a_one_rank_nccl_group(E, oracle):
+    """sharded.compute_sharded end to end (encore_compute_shard + the NCCL all-gather and rank-order sum) with one
+    process per device; this box has one GPU, so world_size is 1 (the 2-rank collective runs on gloo in
+    tests/test_sharded_gloo.py)"""
+    import socket
+
+    import torch.distributed as dist
+    from paper_2105_08722_b200 import sharded
+    if dist.is_initialized():
+        pytest.skip("a process group already exists")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=5000, grid=64)
+    pos, w = W.make(cfg)
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1, device_id=dev)
+    try:
+        with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+            z = sharded.compute_sharded(plan, torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev))
+            torch.cuda.synchronize()
+            z = z.cpu().numpy()
+            assert E.encore_get_shard_groups(plan.h)[0] == 0
+    finally:
+        dist.destroy_process_group()
+    o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+    assert np.abs(z - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+
+
 def test_shard_argument_errors(E):
     pos = torch.rand((3, 64), dtype=torch.float64, device="cuda:0") * 50.0
     with E.Plan(3, 1.0, 20.0, 3, 2, 0.0) as plan:

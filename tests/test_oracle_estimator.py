@@ -241,3 +241,32 @@ def test_cell_ids_are_valid_cells(oracle):
             lo, hi = org[a] + idx * h, org[a] + (idx + 1) * h
             tol = 1e-9 * h
             assert ((pos[a] >= lo - tol) & (pos[a] <= hi + tol)).all()
+
+
+def test_strided_primary_subsets_add_up_to_the_full_sum(oracle):
+    """prim_offset / prim_stride (what bench.py's cpu_baseline and --impl reference time): the s shards offset = 0..s-1
+    with stride s partition the primaries, so their zeta and counts add up to the stride-1 result, and each shard
+    holds exactly the primaries offset, offset+s, ... (checked through the per-primary counts it fills)"""
+    rng = np.random.default_rng(31)
+    n = 157                                              # not a multiple of the strides
+    pos = np.ascontiguousarray(rng.uniform(0, 60.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n)
+    full = oracle.zeta(4, pos, w, 0.0, 3.0, 30.0, 4, 2, want_prim_counts=True)
+    for stride in (2, 3, 7):
+        z = np.zeros_like(full["zeta"])
+        bc = np.zeros_like(full["bin_counts"])
+        for off in range(stride):
+            part = oracle.zeta(4, pos, w, 0.0, 3.0, 30.0, 4, 2, prim_offset=off, prim_stride=stride, want_prim_counts=True)
+            z += part["zeta"]
+            bc += part["bin_counts"]
+            mine = np.zeros(n, dtype=bool)
+            mine[off::stride] = True
+            assert (part["prim_counts"][mine] == full["prim_counts"][mine]).all()
+            assert not part["prim_counts"][~mine].any()          # rows of other primaries stay untouched (zero-initialised)
+            assert part["bin_counts"].sum() == full["prim_counts"][mine].sum()
+        assert (bc == full["bin_counts"]).all()
+        assert np.abs(z - full["zeta"]).max() <= 1e-13 * np.abs(full["zeta"]).max()
+    # an offset beyond n processes nothing
+    none = oracle.zeta(4, pos, w, 0.0, 3.0, 30.0, 4, 2, prim_offset=n, prim_stride=5)
+    assert not none["zeta"].any() and not none["bin_counts"].any()
+    assert full["stage_seconds"][0] >= 0.0 and full["stage_seconds"][1] >= 0.0
