@@ -47,7 +47,7 @@
 #include <omp.h>
 #endif
 
-#define ORACLE_MAX_ORDER 5
+#define ORACLE_MAX_ORDER 6
 #define ORACLE_MAX_L 16
 #define PI_L 3.14159265358979323846264338327950288L
 
@@ -147,7 +147,8 @@ void oracle_ylm(int lmax, double x, double y, double z, double *out_re, double *
 /* ------------------------------------------------------------------------------------------
  * Multiplets Lambda in the order of Alg. 3 / Fig. 4:
  * nested ascending loops, last index fastest.  Width of a row: 2N-5 (N=3: {l}; N=4: {l1,l2,l3};
- * N=5: {l1,l2,l12,l3,l4}).  allparity=0 keeps E(Lam)=+1 only (even sum of PRINCIPAL l's).
+ * N=5: {l1,l2,l12,l3,l4}; N=6: {l1,l2,l12,l3,l123,l4,l5}).  Intermediates run over their whole
+ * triangle range (R5); principal l's up to lmax.  allparity=0 keeps E(Lam)=+1 only (even sum of PRINCIPAL l's).
  * Returns the number of multiplets; writes them if out != NULL.
  * ------------------------------------------------------------------------------------------ */
 int oracle_multiplets(int order, int lmax, int allparity, int *out)
@@ -179,6 +180,21 @@ int oracle_multiplets(int order, int lmax, int allparity, int *out)
                             }
                             ++n;
                         }
+    } else if (order == 6) {
+        for (int l1 = 0; l1 <= lmax; ++l1)
+            for (int l2 = 0; l2 <= lmax; ++l2)
+                for (int l12 = abs(l1 - l2); l12 <= l1 + l2; ++l12)          /* R5: not capped */
+                    for (int l3 = 0; l3 <= lmax; ++l3)
+                        for (int l123 = abs(l12 - l3); l123 <= l12 + l3; ++l123) /* R5: not capped */
+                            for (int l4 = 0; l4 <= lmax; ++l4)
+                                for (int l5 = abs(l123 - l4); l5 <= l123 + l4 && l5 <= lmax; ++l5) {
+                                    if (!allparity && ((l1 + l2 + l3 + l4 + l5) & 1)) continue;
+                                    if (out) {
+                                        int *o = out + 7 * n;
+                                        o[0] = l1; o[1] = l2; o[2] = l12; o[3] = l3; o[4] = l123; o[5] = l4; o[6] = l5;
+                                    }
+                                    ++n;
+                                }
     } else {
         return -1;
     }
@@ -190,7 +206,8 @@ static void principal_ls(int order, const int *Lam, int *l)
 {
     if (order == 3) { l[0] = Lam[0]; l[1] = Lam[0]; }
     else if (order == 4) { l[0] = Lam[0]; l[1] = Lam[1]; l[2] = Lam[2]; }
-    else { l[0] = Lam[0]; l[1] = Lam[1]; l[2] = Lam[3]; l[3] = Lam[4]; }
+    else if (order == 5) { l[0] = Lam[0]; l[1] = Lam[1]; l[2] = Lam[3]; l[3] = Lam[4]; }
+    else { l[0] = Lam[0]; l[1] = Lam[1]; l[2] = Lam[3]; l[3] = Lam[5]; l[4] = Lam[6]; }
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -198,6 +215,8 @@ static void principal_ls(int order, const int *Lam, int *l)
  *   N=3: eq. 16   (-1)^{l-m1}/sqrt(2l+1) delta_{m1,-m2}
  *   N=4: eq. 18   (-1)^{l1+l2+l3} (l1 l2 l3; m1 m2 m3)
  *   N=5: eq. 5    E sqrt(2 l12+1) sum_{m12} (-1)^{l12-m12} (l1 l2 l12; m1 m2 -m12)(l12 l3 l4; m12 m3 m4)
+ *   N=6: eq. 5    E sqrt(2 l12+1) sqrt(2 l123+1) sum_{m12,m123} (-1)^{l12-m12+l123-m123}
+ *                 (l1 l2 l12; m1 m2 -m12)(l12 l3 l123; m12 m3 -m123)(l123 l4 l5; m123 m4 m5)
  * (R2: the sqrt(2 l12+1) of eq. 5 is kept although eq. 20 as printed drops it.)
  * ------------------------------------------------------------------------------------------ */
 double oracle_coupling(int order, const int *Lam, const int *m)
@@ -222,6 +241,19 @@ double oracle_coupling(int order, const int *Lam, const int *m)
         }
         return ((s & 1) ? -1.0 : 1.0) * sqrt(2.0 * l12 + 1.0) * sum;
     }
+    if (order == 6) {
+        int l1 = Lam[0], l2 = Lam[1], l12 = Lam[2], l3 = Lam[3], l123 = Lam[4], l4 = Lam[5], l5 = Lam[6];
+        int s = l1 + l2 + l3 + l4 + l5;
+        double sum = 0.0;
+        for (int m12 = -l12; m12 <= l12; ++m12)
+            for (int m123 = -l123; m123 <= l123; ++m123) {
+                double t = oracle_wigner3j(l1, l2, l12, m[0], m[1], -m12) *
+                           oracle_wigner3j(l12, l3, l123, m12, m[2], -m123) *
+                           oracle_wigner3j(l123, l4, l5, m123, m[3], m[4]);
+                sum += (((l12 - m12 + l123 - m123) & 1) ? -1.0 : 1.0) * t;
+            }
+        return ((s & 1) ? -1.0 : 1.0) * sqrt(2.0 * l12 + 1.0) * sqrt(2.0 * l123 + 1.0) * sum;
+    }
     return 0.0;
 }
 
@@ -235,7 +267,7 @@ int64_t oracle_count_terms(int order, int lmax, int allparity, int half)
     oracle_multiplets(order, lmax, allparity, Lam);
     int64_t cnt = 0;
     for (int iL = 0; iL < nL; ++iL) {
-        int l[4], m[4];
+        int l[5], m[5];
         principal_ls(order, Lam + iL * width, l);
         int nm = order - 1;
         /* odometer over m_1..m_{N-2}; m_{N-1} = -(sum) */
@@ -501,7 +533,7 @@ static int64_t n_choose(int n, int k)
 
 int64_t oracle_bin_tuples(int order, int nbins, int *out)
 {
-    int k = order - 1, b[4];
+    int k = order - 1, b[5];
     int64_t cnt = 0;
     if (k > nbins) return 0;
     for (int i = 0; i < k; ++i) b[i] = i;
@@ -526,7 +558,7 @@ static double wall_seconds(void)
 #endif
 }
 
-typedef struct { int idx[4]; double c; } term_t; /* idx[k] = l_k*l_k + l_k + m_k; c = E(Lam) C^Lam_M */
+typedef struct { int idx[5]; double c; } term_t; /* idx[k] = l_k*l_k + l_k + m_k; c = E(Lam) C^Lam_M */
 
 int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double box, double rmin,
                 double rmax, int nbins, int lmax, int allparity, const int *bins, int64_t nB,
@@ -558,7 +590,7 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
     size_t tcap = 1024, tn = 0;
     term_t *terms = (term_t *)malloc(sizeof(term_t) * tcap);
     for (int iL = 0; iL < nL; ++iL) {
-        int l[4], m[4], sl = 0;
+        int l[5], m[5], sl = 0;
         principal_ls(order, Lam + iL * width, l);
         for (int k = 0; k < nm; ++k) sl += l[k];
         const double E = (sl & 1) ? -1.0 : 1.0;

@@ -91,6 +91,35 @@ def test_5pcf_bruteforce(oracle):
     assert res["max_imag"] <= 1e-12 * scale
 
 
+def test_6pcf_bruteforce(oracle):
+    """N = 6 (two intermediates): eq. 34/35 through the oracle against explicit 6-tuple sums of
+    the basis functions of eq. 4/5 (scipy Y_lm, sympy 3-j), every multiplet of lmax = 1 incl. intermediates above lmax"""
+    pos, w = cloud(14, 66)
+    rmin, rmax, nb, lmax = 2.0, 62.0, 5, 1
+    res = oracle.zeta(6, pos, w, 0.0, rmin, rmax, nb, lmax)
+    bins = [tuple(b) for b in res["bins"]]
+    assert bins == [(0, 1, 2, 3, 4)]
+    scale = np.abs(res["zeta"]).max()
+    assert scale > 0
+    lams = [tuple(r) for r in res["multiplets"]]
+    assert (1, 1, 2, 1, 1, 1, 0) in lams and (1, 1, 2, 1, 3, 1, 0) not in lams and (1, 1, 2, 0, 2, 1, 1) in lams   # R5
+    for il, lam in enumerate(lams):
+        ref = tier0.tuple_sum(pos, w, 0.0, rmin, rmax, nb, bins, tier0.basis_eq4(6, lam))
+        assert np.abs(res["zeta"][il] - ref.real).max() <= 1e-12 * scale, lam
+    ref = tier0.tuple_sum(pos, w, 0.0, rmin, rmax, nb, bins,
+                          lambda v: FOURPI ** -0.5 * 3 / FOURPI ** 2 * tier0.dot(v[0], v[1]) * tier0.dot(v[3], v[4]) + 0 * v[2][0])
+    assert np.abs(res["zeta"][lams.index((1, 1, 0, 0, 0, 1, 1))] - ref.real).max() <= 1e-12 * scale
+    assert res["max_imag"] <= 1e-12 * scale
+    # odd-parity multiplets are imaginary, and equal the tuple sums too (ALLPARITY, PAPER.md:335)
+    res = oracle.zeta(6, pos, w, 0.0, rmin, rmax, nb, lmax, allparity=True)
+    lams = [tuple(r) for r in res["multiplets"]]
+    odd = [il for il, lam in enumerate(lams) if (lam[0] + lam[1] + lam[3] + lam[5] + lam[6]) % 2]
+    assert odd
+    for il in odd[:6]:
+        ref = tier0.tuple_sum(pos, w, 0.0, rmin, rmax, nb, bins, tier0.basis_eq4(6, lams[il]))
+        assert abs(res["zeta_im"][il, 0] - ref.imag[0]) <= 1e-12 * scale and abs(res["zeta"][il, 0]) <= 1e-12 * scale
+
+
 # ---- (ii) l = 0 identity --------------------------------------------------------------------
 @pytest.mark.parametrize("order", [3, 4, 5])
 def test_l0_identity_c1(oracle, order):
@@ -134,7 +163,7 @@ def _random_rotation(seed):
     return q
 
 
-@pytest.mark.parametrize("order,lmax,n", [(3, 6, 300), (4, 3, 200), (5, 2, 60)])
+@pytest.mark.parametrize("order,lmax,n", [(3, 6, 300), (4, 3, 200), (5, 2, 60), (6, 2, 24)])
 def test_rotation_invariance(oracle, order, lmax, n):
     pos, w = cloud(n, 100 + order, scale=100.0)
     args = (0.0, 10.0, 70.0, 5, lmax)

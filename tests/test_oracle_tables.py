@@ -109,6 +109,82 @@ def test_multiplet_counts_and_order(oracle):
         assert max(l1, l2, l3, l4) <= 3 and (l1 + l2 + l3 + l4) % 2 == 0
 
 
+def _enumerate6(lmax, cap):
+    """6PCF multiplets {l1,l2,(l12),l3,(l123),l4,l5} written out here from the triangle rules of eq. 5,
+    even parity; cap: intermediates limited to lmax as well (the counting behind PAPER.md:537)"""
+    rows = []
+    top = lmax if cap else 10 ** 9
+    for l1 in range(lmax + 1):
+        for l2 in range(lmax + 1):
+            for l12 in range(abs(l1 - l2), min(l1 + l2, top) + 1):
+                for l3 in range(lmax + 1):
+                    for l123 in range(abs(l12 - l3), min(l12 + l3, top) + 1):
+                        for l4 in range(lmax + 1):
+                            for l5 in range(abs(l123 - l4), min(l123 + l4, lmax) + 1):
+                                if (l1 + l2 + l3 + l4 + l5) % 2 == 0:
+                                    rows.append([l1, l2, l12, l3, l123, l4, l5])
+    return rows
+
+
+def test_6pcf_multiplet_counts(oracle):
+    """PAPER.md:537 prints 1 558 six-point multiplets at lmax = 3: that is the count with the intermediates capped at
+    lmax; reading R5 leaves them uncapped as for the 5PCF (204 / 1 406 of PAPER.md:606, :594), which gives
+    2 212.  Both enumerations are written out above; the oracle's is the uncapped one, in nested-loop order."""
+    assert len(_enumerate6(3, cap=True)) == 1558
+    assert len(_enumerate6(3, cap=False)) == 2212
+    assert oracle.multiplets(6, 3).tolist() == _enumerate6(3, cap=False)
+    assert oracle.multiplets(6, 2).tolist() == _enumerate6(2, cap=False)
+    assert len(oracle.multiplets(6, 1, allparity=True)) > len(oracle.multiplets(6, 1))
+    assert len(oracle.bin_tuples(6, 10)) == 252                  # C(10,5), PAPER.md:537 (R6)
+    assert oracle.bin_tuples(6, 6).tolist() == [list(c) for c in itertools.combinations(range(6), 5)]
+
+
+def test_6pcf_coupling(oracle):
+    """eq. 5 for N = 6: orthonormality (eq. 9), orthogonality across intermediates, eq. 6, against sympy, and the
+    closed form P_{11(0)0(0)11} = (4 pi)^{-1/2} 3 (4 pi)^{-2} (r1.r2)(r4.r5) (two eq.-17 functions times Y_00)."""
+    lams = oracle.multiplets(6, 1, allparity=True)
+    for lam in lams:
+        ls = (lam[0], lam[1], lam[3], lam[5], lam[6])
+        assert sum(oracle.coupling(6, lam, M) ** 2 for M in _all_M(ls)) == pytest.approx(1.0, abs=1e-13), lam
+    for lam in ([2, 1, 3, 2, 1, 1, 2], [1, 2, 2, 2, 4, 2, 2], [2, 2, 4, 2, 6, 2, 2 + 2]):   # intermediates above the principal l's
+        ls = (lam[0], lam[1], lam[3], lam[5], lam[6])
+        assert sum(oracle.coupling(6, lam, M) ** 2 for M in _all_M(ls)) == pytest.approx(1.0, abs=1e-12), lam
+    ls = (1, 1, 1, 1, 1, )
+    fam = [r for r in lams.tolist() if (r[0], r[1], r[3], r[5], r[6]) == (1, 1, 1, 1, 1) or False]
+    same = [r for r in oracle.multiplets(6, 1, allparity=True).tolist() if [r[0], r[1], r[3], r[5], r[6]] == [1, 1, 1, 1, 0]]
+    assert len(same) >= 2
+    for a in same:
+        for b in same:
+            s = sum(oracle.coupling(6, a, M) * oracle.coupling(6, b, M) for M in _all_M((1, 1, 1, 1, 0)))
+            assert s == pytest.approx(1.0 if a == b else 0.0, abs=1e-13)
+    rng = np.random.default_rng(66)
+    for lam in ([1, 1, 2, 1, 1, 1, 0], [1, 2, 1, 1, 2, 2, 1], [2, 1, 3, 1, 2, 1, 1]):
+        E = (-1) ** (lam[0] + lam[1] + lam[3] + lam[5] + lam[6])
+        l1, l2, l12, l3, l123, l4, l5 = lam
+        for M in _all_M((l1, l2, l3, l4, l5)):
+            c = oracle.coupling(6, lam, M)
+            assert oracle.coupling(6, lam, [-m for m in M]) == pytest.approx(E * c, abs=1e-15)      # eq. 6
+            m12, m123 = M[0] + M[1], M[0] + M[1] + M[2]
+            ref = 0.0
+            if abs(m12) <= l12 and abs(m123) <= l123:
+                ref = (E * math.sqrt((2 * l12 + 1) * (2 * l123 + 1)) * (-1) ** (l12 - m12 + l123 - m123)
+                       * float(wigner_3j(l1, l2, l12, M[0], M[1], -m12)) * float(wigner_3j(l12, l3, l123, m12, M[2], -m123))
+                       * float(wigner_3j(l123, l4, l5, m123, M[3], M[4])))
+            assert c == pytest.approx(ref, abs=1e-14)
+    u = rng.standard_normal((5, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    Y = [oracle.ylm(2, v) for v in u]
+    lam, ls = [1, 1, 0, 0, 0, 1, 1], (1, 1, 0, 1, 1)
+    tot = 0.0
+    for M in _all_M(ls):
+        pr = oracle.coupling(6, lam, M)
+        for k, (l, m) in enumerate(zip(ls, M)):
+            pr = pr * Y[k][l * l + l + m]
+        tot += pr
+    fourpi = 4 * math.pi
+    assert abs(tot - fourpi ** -0.5 * 3 / fourpi ** 2 * (u[0] @ u[1]) * (u[3] @ u[4])) < 1e-15
+
+
 def test_bin_tuple_counts_and_order(oracle):
     assert len(oracle.bin_tuples(3, 10)) == 45
     assert len(oracle.bin_tuples(4, 10)) == 120                # PAPER.md:606

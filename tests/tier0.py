@@ -104,6 +104,21 @@ def basis_eq4(order, lam):
                  * float(wigner_3j(l1, l2, l12, m1, m2, -m12)) * float(wigner_3j(l12, l3, l4, m12, m3, m4)))
             if c != 0.0:
                 terms.append(((m1, m2, m3, m4), c))
+    elif order == 6:
+        # eq. 5 with two intermediates: kappa = l12 - m12 + l123 - m123
+        l1, l2, l12, l3, l123, l4, l5 = lam
+        ls = (l1, l2, l3, l4, l5)
+        terms = []
+        for m1, m2, m3, m4 in itertools.product(range(-l1, l1 + 1), range(-l2, l2 + 1), range(-l3, l3 + 1), range(-l4, l4 + 1)):
+            m5 = -m1 - m2 - m3 - m4
+            m12, m123 = m1 + m2, m1 + m2 + m3
+            if abs(m5) > l5 or abs(m12) > l12 or abs(m123) > l123:
+                continue
+            c = ((-1) ** (l1 + l2 + l3 + l4 + l5) * np.sqrt((2 * l12 + 1) * (2 * l123 + 1)) * (-1) ** (l12 - m12 + l123 - m123)
+                 * float(wigner_3j(l1, l2, l12, m1, m2, -m12)) * float(wigner_3j(l12, l3, l123, m12, m3, -m123))
+                 * float(wigner_3j(l123, l4, l5, m123, m4, m5)))
+            if c != 0.0:
+                terms.append(((m1, m2, m3, m4, m5), c))
     else:
         raise ValueError(order)
 
