@@ -7,7 +7,8 @@
  *   a^b_lm(s_i) = (1/v_b) sum_{j != i} w_j Y_lm( (r_j - s_i)^ ) Theta^b(|r_j - s_i|)        eq. 35
  *   zeta^B_Lam  = (1/V) sum_i w_i sum_M E(Lam) C^Lam_M prod_k a^{b_k}_{l_k m_k}(s_i)          eq. 34
  *
- * for N = 3, 4, 5 (Lam = {l}, {l1 l2 l3}, {l1 l2 (l12) l3 l4}; eqs. 16, 18, 5/20 — PAPER.md:135, :145, :69, :157),
+ * for N = 3, 4, 5, 6 (Lam = {l}, {l1 l2 l3}, {l1 l2 (l12) l3 l4}, {l1 l2 (l12) l3 (l123) l4 l5}; eqs. 16, 18, 5/20 —
+ * PAPER.md:135, :145, :69, :157),
  * even-parity multiplets only (real zeta), ordered distinct bins b_1 < .. < b_{N-1},
  * using the half-sum m_{N-1} >= 0 of eq. 44.  Steps:
  *   a1 cell assignment, a2 counting sort by cell, a3 neighbour sweep + radial binning, a4 a_lm accumulation,
@@ -55,11 +56,12 @@ enum {
 /* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
  * S(0) = 1/2, else 1), bin edges, 1/v_b, Y_lm normalisations.  Host work only; device tables are uploaded by the
  * first encore_compute on the then-current device.
- *   npcf_order  N in {3,4,5}
+ *   npcf_order  N in {3,4,5,6}  (N = 6: Lam = {l1 l2 (l12) l3 (l123) l4 l5}, eq. 5 with two intermediates, PAPER.md:69, :161;
+ *               contracted by the literal eq. 44 kernel, one warp per (Lam, B))
  *   r_min,r_max 0 <= r_min < r_max
  *   nbins       N_r >= N-1 and <= 32
- *   lmax        0..10 for N=3; 0..6 for N=4,5 (ENCORE_EUNSUPPORTED above: the a_lm tile of 32 primaries must
- *               fit the contraction kernel's shared memory)
+ *   lmax        0..10 (ENCORE_EUNSUPPORTED above).  The factorised contraction kernels cover N=3, nbins <= 10;
+ *               N=4, nbins <= 10; N=5, nbins <= 10 and lmax <= 5; other shapes run the literal eq. 44 kernel
  *   box_size    > 0: periodic cube [0,L)^3 (PERIODIC mode), needs r_max <= L/2;  0: open geometry
  */
 int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,

@@ -83,8 +83,8 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
     const HostTables &T = P->T;
     std::vector<DevTerm> dt(T.terms.size());
     for (size_t i = 0; i < dt.size(); ++i) {
-        for (int k = 0; k < 4; ++k) { dt[i].re[k] = T.terms[i].re[k]; dt[i].im[k] = T.terms[i].im[k]; dt[i].tau[k] = T.terms[i].tau[k]; }
-        dt[i].pad = 0;
+        for (int k = 0; k < 5; ++k) { dt[i].re[k] = T.terms[i].re[k]; dt[i].im[k] = T.terms[i].im[k]; dt[i].tau[k] = T.terms[i].tau[k]; }
+        for (int k = 0; k < 7; ++k) dt[i].pad[k] = 0;
         dt[i].W = T.terms[i].W;
     }
     CU(P->d_terms.ensure(sizeof(DevTerm) * std::max<size_t>(1, dt.size())));
@@ -100,9 +100,10 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
     {   // factorised-contraction tables
         const int nm = T.order - 1, nb = T.nbins;
         size_t cells = 1;
-        for (int k = 0; k < nm; ++k) cells *= (size_t)nb;
+        if (contraction_is_factorised(T.order, nb, T.lmax)) // (tuple -> output index) is only read by the factorised kernels
+            for (int k = 0; k < nm; ++k) cells *= (size_t)nb;
         std::vector<int> tix(cells, -1);
-        for (int iB = 0; iB < T.nB(); ++iB) {
+        for (int iB = 0; cells > 1 && iB < T.nB(); ++iB) {
             size_t key = 0;
             for (int k = 0; k < nm; ++k) key = key * nb + (size_t)T.bin_tuples[(size_t)iB * nm + k];
             tix[key] = iB;
@@ -643,7 +644,7 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
         }
     }
     if (executed) *executed = ex;
-    if (canonical) *canonical = evals * (N == 3 ? 5.0 : N == 4 ? 11.0 : 17.0);
+    if (canonical) *canonical = evals * (6.0 * (N - 3) + 5.0);   // 5 / 11 / 17 / 23 flop per term evaluation for N = 3..6
     return ENCORE_OK;
 }
 

@@ -4,7 +4,7 @@
 #include <cstdint>
 #include <vector>
 
-#define ENCORE_MAX_ORDER 5
+#define ENCORE_MAX_ORDER 6
 #define ENCORE_MAX_BINS 32
 #define ENCORE_MAX_LMAX 10
 #define ENCORE_GROUP 32              // primaries per group = lanes of a warp
@@ -18,9 +18,9 @@ static inline int comp_im(int l, int m) { return m == 0 ? -1 : l * l + 2 * m; }
 // factor k = a_{l_k |m_k|} for m_k >= 0, (-1)^{m_k} conj(a_{l_k |m_k|}) for m_k < 0:
 // re[k]/im[k] are component indices (im = -1: imaginary part is zero), tau[k] = -1 conjugates.
 struct HostTerm {
-    int16_t re[4];
-    int16_t im[4];
-    int8_t tau[4];
+    int16_t re[5];
+    int16_t im[5];
+    int8_t tau[5];
     double W;
 };
 

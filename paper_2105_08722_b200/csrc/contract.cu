@@ -20,7 +20,7 @@ namespace {
 constexpr int kWarps = 8;
 constexpr unsigned kFull = 0xffffffffu;
 
-// Generic kernel, any N in {3,4,5}: one warp per output (Lam,B), terms looped, complex products in registers.
+// Generic kernel, any N in {3,..,6}: one warp per output (Lam,B), terms looped (literal eq. 44), complex products in registers.
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
     const int g = a.g_begin + blockIdx.x;
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a
 
     for (int o = warp; o < nout; o += kWarps) {
         const int iL = o / a.nB, iB = o - iL * a.nB;
-        int boff[4];
+        int boff[5];
         for (int k = 0; k < nm; ++k) boff[k] = a.bin_tuples[iB * nm + k] * 32;
         double acc = 0.0;
         const bool odd = a.lam_parity[iL] != 0; // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)

@@ -17,11 +17,11 @@ struct GridGeom {
     int ncell, npencil;
 };
 
-struct DevTerm {        // device image of HostTerm (32 bytes)
-    short re[4];
-    short im[4];
-    signed char tau[4];
-    int pad;
+struct DevTerm {        // device image of HostTerm (40 bytes)
+    short re[5];
+    short im[5];
+    signed char tau[5];
+    signed char pad[7];
     double W;
 };
 

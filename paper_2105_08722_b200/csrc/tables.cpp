@@ -64,6 +64,17 @@ double coupling(int order, const int *lam, const int *m)
     if (order == 4) { // eq. 18: C = (-1)^{l1+l2+l3} (3j); times E = same sign -> plain 3j
         return encore_host_wigner3j(lam[0], lam[1], lam[2], m[0], m[1], m[2]);
     }
+    if (order == 6) {
+        // eq. 5 for N=6: two intermediates, kappa = l12 - m12 + l123 - m123; only m12 = m1+m2 and
+        // m123 = m12+m3 survive; E*E = 1.
+        const int l1 = lam[0], l2 = lam[1], l12 = lam[2], l3 = lam[3], l123 = lam[4], l4 = lam[5], l5 = lam[6];
+        const int m12 = m[0] + m[1], m123 = m12 + m[2];
+        if (std::abs(m12) > l12 || std::abs(m123) > l123) return 0.0;
+        double v = encore_host_wigner3j(l1, l2, l12, m[0], m[1], -m12) * encore_host_wigner3j(l12, l3, l123, m12, m[2], -m123) *
+                   encore_host_wigner3j(l123, l4, l5, m123, m[3], m[4]);
+        if ((l12 - m12 + l123 - m123) & 1) v = -v;
+        return std::sqrt((2.0 * l12 + 1.0) * (2.0 * l123 + 1.0)) * v;
+    }
     // eq. 5 for N=5: C = E sqrt(2 l12+1) sum_{m12} (-1)^{l12-m12} (l1 l2 l12; m1 m2 -m12)(l12 l3 l4; m12 m3 m4);
     // only m12 = m1+m2 survives; E*E = 1.
     const int l1 = lam[0], l2 = lam[1], l12 = lam[2], l3 = lam[3], l4 = lam[4];
@@ -86,7 +97,7 @@ void enumerate_multiplets(HostTables &t)
                     if (t.allparity || ((l1 + l2 + l3) & 1) == 0) { // even parity unless ALLPARITY
                         t.multiplets.push_back(l1); t.multiplets.push_back(l2); t.multiplets.push_back(l3);
                     }
-    } else {
+    } else if (t.order == 5) {
         for (int l1 = 0; l1 <= L; ++l1)
             for (int l2 = 0; l2 <= L; ++l2)
                 for (int l12 = std::abs(l1 - l2); l12 <= l1 + l2; ++l12)
@@ -96,6 +107,18 @@ void enumerate_multiplets(HostTables &t)
                                 const int row[5] = {l1, l2, l12, l3, l4};
                                 t.multiplets.insert(t.multiplets.end(), row, row + 5);
                             }
+    } else { // N = 6: {l1, l2, (l12), l3, (l123), l4, l5}, intermediates over their whole triangle range (R5)
+        for (int l1 = 0; l1 <= L; ++l1)
+            for (int l2 = 0; l2 <= L; ++l2)
+                for (int l12 = std::abs(l1 - l2); l12 <= l1 + l2; ++l12)
+                    for (int l3 = 0; l3 <= L; ++l3)
+                        for (int l123 = std::abs(l12 - l3); l123 <= l12 + l3; ++l123)
+                            for (int l4 = 0; l4 <= L; ++l4)
+                                for (int l5 = std::abs(l123 - l4); l5 <= std::min(l123 + l4, L); ++l5)
+                                    if (t.allparity || ((l1 + l2 + l3 + l4 + l5) & 1) == 0) {
+                                        const int row[7] = {l1, l2, l12, l3, l123, l4, l5};
+                                        t.multiplets.insert(t.multiplets.end(), row, row + 7);
+                                    }
     }
 }
 
@@ -109,6 +132,7 @@ void fill_parity(HostTables &t)
         int s = 0;
         if (t.order == 4) s = lam[0] + lam[1] + lam[2];
         else if (t.order == 5) s = lam[0] + lam[1] + lam[3] + lam[4];
+        else if (t.order == 6) s = lam[0] + lam[1] + lam[3] + lam[5] + lam[6];
         t.parity[iL] = s & 1;
     }
 }
@@ -116,7 +140,7 @@ void fill_parity(HostTables &t)
 void enumerate_bins(HostTables &t)
 {
     const int k = t.order - 1;
-    int b[4];
+    int b[5];
     for (int i = 0; i < k; ++i) b[i] = i;
     for (;;) {
         t.bin_tuples.insert(t.bin_tuples.end(), b, b + k);
@@ -135,11 +159,12 @@ void enumerate_terms(HostTables &t)
     t.term_start.assign(1, 0);
     for (int iL = 0; iL < nL; ++iL) {
         const int *lam = &t.multiplets[(size_t)iL * t.width];
-        int l[4];
+        int l[5];
         if (t.order == 3) { l[0] = l[1] = lam[0]; }
         else if (t.order == 4) { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[2]; }
-        else { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[3]; l[3] = lam[4]; }
-        int m[4];
+        else if (t.order == 5) { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[3]; l[3] = lam[4]; }
+        else { l[0] = lam[0]; l[1] = lam[1]; l[2] = lam[3]; l[3] = lam[5]; l[4] = lam[6]; }
+        int m[5];
         for (int k = 0; k < nm - 1; ++k) m[k] = -l[k];
         for (;;) {
             int s = 0;
@@ -160,7 +185,7 @@ void enumerate_terms(HostTables &t)
                             if (am & 1) W = -W;
                         }
                     }
-                    for (int k = nm; k < 4; ++k) { ht.re[k] = 0; ht.im[k] = -1; ht.tau[k] = 1; }
+                    for (int k = nm; k < 5; ++k) { ht.re[k] = 0; ht.im[k] = -1; ht.tau[k] = 1; }
                     ht.W = W;
                     t.terms.push_back(ht);
                 }

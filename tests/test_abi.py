@@ -42,7 +42,7 @@ def test_plan_argument_validation():
     lib = E.lib()
     h = C.c_void_p()
     bad = [
-        (2, 0.0, 100.0, 5, 2, 0.0), (6, 0.0, 100.0, 5, 2, 0.0),      # order
+        (2, 0.0, 100.0, 5, 2, 0.0), (7, 0.0, 100.0, 6, 2, 0.0),      # order
         (3, -1.0, 100.0, 5, 2, 0.0), (3, 50.0, 50.0, 5, 2, 0.0),       # radii
         (4, 0.0, 100.0, 2, 2, 0.0), (3, 0.0, 100.0, 33, 2, 0.0),       # nbins < N-1, > 32
         (3, 0.0, 100.0, 5, -1, 0.0),                                   # lmax
@@ -91,7 +91,7 @@ def test_plan_tables_match_paper_counts(order, nbins, lmax, nlam, nb, nterms):
 
 
 def test_plan_tables_equal_oracle_enumeration(oracle):
-    for order, nbins, lmax in [(3, 6, 7), (4, 7, 4), (5, 6, 2)]:
+    for order, nbins, lmax in [(3, 6, 7), (4, 7, 4), (5, 6, 2), (6, 6, 2), (6, 7, 1)]:
         with E.Plan(order, 5.0, 65.0, nbins, lmax, 0.0) as p:
             assert (p.multiplets == oracle.multiplets(order, lmax)).all()
             assert (p.bin_tuples == oracle.bin_tuples(order, nbins)).all()
@@ -99,11 +99,24 @@ def test_plan_tables_equal_oracle_enumeration(oracle):
             assert np.array_equal(E.encore_get_bin_edges(p.h, nbins), oracle.bin_edges(5.0, 65.0, nbins))
 
 
+def test_6pcf_plan_tables():
+    """N = 6: 2 212 multiplets at lmax = 3 with uncapped intermediates (reading R5; PAPER.md:537 prints the capped 1 558),
+    C(N_r, 5) bin tuples, 23 flop per term evaluation in the canonical model"""
+    with E.Plan(6, 20.0, 160.0, 10, 3, 1000.0) as p:
+        assert (p.n_lambda, p.n_b) == (2212, 252)
+        assert p.multiplets.shape == (2212, 7)
+        ex, ca = E.encore_contraction_flops(p.h)
+        assert ca == E.encore_num_terms(p.h) * 252 * 23
+    lib = E.lib()
+    h = C.c_void_p()
+    assert lib.encore_plan(C.byref(h), 6, 0.0, 100.0, 4, 2, 0.0) == E.EINVAL      # nbins < N - 1
+
+
 def test_allparity_tables_on_the_host():
     """ALLPARITY plan (host tables only): the multiplet counts of PAPER.md:602 and the oracle's enumeration"""
     import oracle
     import paper_2105_08722_b200 as E
-    for order, lmax, expect in [(4, 5, 111), (4, 3, None), (5, 2, None), (3, 4, 5)]:
+    for order, lmax, expect in [(4, 5, 111), (4, 3, None), (5, 2, None), (3, 4, 5), (6, 1, None)]:
         h = E.encore_plan_flags(order, 1.0, 20.0, 6, lmax, 0.0, E.ALLPARITY)
         try:
             lam = E.encore_get_multiplets(h, order)
@@ -113,7 +126,7 @@ def test_allparity_tables_on_the_host():
                 assert len(lam) == expect
             assert E.encore_num_terms(h) == oracle.count_terms(order, lmax, allparity=True, half=True)
             par = E.encore_get_multiplet_parity(h)
-            principal = ref[:, [0, 1, 3, 4]] if order == 5 else ref
+            principal = ref[:, [0, 1, 3, 4]] if order == 5 else ref[:, [0, 1, 3, 5, 6]] if order == 6 else ref
             assert (par == principal.sum(axis=1) % 2).all() if order > 3 else not par.any()
         finally:
             E.encore_destroy(h)

@@ -159,6 +159,32 @@ def test_paper_gpu_shapes_and_largest_factorised_shapes(E, oracle, order, nbins,
     assert np.abs(z - o["zeta"]).max() <= TOL * scale
 
 
+@pytest.mark.parametrize("nbins,lmax,box,allparity,n", [(5, 2, 0.0, False, 160), (6, 1, 90.0, False, 200), (7, 1, 0.0, True, 120),
+                                                         (5, 3, 0.0, False, 70)])
+def test_6pcf_matches_the_oracle(E, oracle, nbins, lmax, box, allparity, n):
+    """N = 6, two intermediates (eq. 5; 2 212 multiplets at lmax = 3)"""
+    rng = np.random.default_rng(6000 + 10 * nbins + lmax)
+    pos = np.ascontiguousarray(rng.uniform(0, 90.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.2, 0.8])
+    o = oracle.zeta(6, pos, w, box, 4.0, 44.0, nbins, lmax, allparity=allparity, want_prim_counts=True)
+    dev = torch.device("cuda:0")
+    with E.Plan(6, 4.0, 44.0, nbins, lmax, box, allparity=allparity) as plan:
+        assert (plan.multiplets == o["multiplets"]).all() and (plan.bin_tuples == o["bins"]).all()
+        if lmax == 3:
+            assert plan.n_lambda == 2212
+        par = E.encore_get_multiplet_parity(plan.h).astype(bool)
+        z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+        assert E.encore_get_status(plan.h) == E.OK
+        counts, _ = E.encore_get_bin_counts(plan.h, nbins)
+    assert (counts == o["bin_counts"]).all()
+    expect = np.where(par[:, None], o["zeta_im"], o["zeta"])
+    scale = max(np.abs(o["zeta"]).max(), np.abs(o["zeta_im"]).max())
+    assert scale > 0
+    assert np.abs(z - expect).max() <= TOL * scale
+    if allparity:
+        assert par.any() and np.abs(expect[par]).max() > 1e-6 * scale
+
+
 def test_degenerate_inputs(E, oracle):
     # one particle: no pairs, zeta = 0
     g = gpu_run(E, 3, np.array([[1.0], [2.0], [3.0]]), np.ones(1), 0.0, 0.0, 10.0, 3, 2)
