@@ -11,8 +11,8 @@ from the CUDA package is imported, so no stored value comes from the GPU path.  
   digest      str                       workloads.digest(pos, w): sha256 of the input bytes
   seconds, threads                      oracle wall time and OpenMP threads of the run that wrote the file
 The GPU parity test regenerates the inputs, checks the digest (a stale fixture fails loudly) and compares element by
-element.  c4 (1.6e6 particles, ~2.5e10 pairs) takes the oracle ~20 minutes on 8 cores, which is why it is stored; c2,
-c3 and c5 are recomputed inside the test run.
+element.  c4 (1.6e6 particles, 2.54e10 pairs) took the oracle 3978 s on 8 threads, which is why it is stored; c2, c3
+and c5 are recomputed inside the test run.
 """
 import os
 import sys
