@@ -187,13 +187,14 @@ def workload_config(cfg, world, allparity=False):
                          "partial zeta per step" if world > 1 else "single GPU")}
 
 
-def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False, shard=None):
+def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False, shard=None, fp32_harmonics=False,
+                   keep_zeta=False):
     """shard = (rank, world): time sharded.compute_sharded (one catalogue, all-gather inside); None: the whole catalogue."""
     from paper_2105_08722_b200 import sharded
     pos, w = make_catalogue(cfg, rank if shard is None else 0)
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    plan = E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box, allparity=allparity)
+    plan = E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box, allparity=allparity, fp32_harmonics=fp32_harmonics)
     E.encore_set_timing(plan.h, True)
     out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream(dev)
@@ -228,6 +229,8 @@ def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allpa
     res = {"ms_total": ms, "kernel_ms": km, "launches": launches, "pairs": pairs, "candidates": cand,
            "flops_contraction": E.encore_contraction_flops(plan.h), "nout": plan.n_lambda * plan.n_b,
            "grid": E.encore_get_grid(plan.h), "pair_steps": E.encore_get_pair_steps(plan.h)}
+    if keep_zeta and shard is None:
+        res["zeta"] = out.cpu().numpy()
     if want_e2e:
         hp = torch.from_numpy(pos).pin_memory()
         hw = torch.from_numpy(w).pin_memory()
@@ -421,6 +424,15 @@ def main():
         # the same c3 catalogue with the parity-odd multiplets too (111 instead of 69 multiplets)
         r, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, allparity=True)
         per["c3_allparity"] = dict(config_entry(W.CONFIGS["c3"], r, 2, fp64_peak, fp32_peak), n_multiplets=r["nout"] // 120)
+        # fp32 harmonics with fp64 accumulation on the same c3 catalogue - a separate path with its own
+        # tolerance (1e-5); the difference to this run's fp64 result is reported beside its time
+        r64, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 1, 3, dev, want_e2e=False, keep_zeta=True)
+        r32, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, fp32_harmonics=True, keep_zeta=True)
+        e32 = config_entry(W.CONFIGS["c3"], r32, 2, fp64_peak, fp32_peak)
+        e32["dtype"] = "f32 harmonics, f64 accumulation / contraction"
+        e32["max_rel_diff_to_fp64_run"] = float(np.abs(r32["zeta"] - r64["zeta"]).max() / np.abs(r64["zeta"]).max())
+        e32["pairs_equal_fp64_run"] = bool(r32["pairs"] == r64["pairs"])
+        per["c3_fp32_harmonics"] = e32
         line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))

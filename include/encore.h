@@ -73,6 +73,12 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
  *   Im zeta = (1/V) sum_i w_i sum_{M, m_{N-1} >= 0} 2 S(m_{N-1}) E(Lam) C^Lam_M Im[prod_k a~]   (App. B),
  * with separations r_j - s_i as in eq. 35 (the sign of odd multiplets depends on it).  Unknown flags: ENCORE_EINVAL. */
 #define ENCORE_ALLPARITY 1u
+/* ENCORE_FP32_HARMONICS (the paper's reduced-precision modes): step a4 evaluates
+ * the unit vector, its powers and w (x+iy)^m of every pair in fp32 and adds 16-pair fp32 chunk sums to the fp64 a_lm
+ * accumulators.  Separations are formed in fp64 and rounded once; cell ids, the radial binning and therefore every pair
+ * count stay those of the fp64 path (bit-exact); contraction and reduction stay fp64.  A separate, separately reported
+ * path: zeta agrees with the fp64 result to ~1e-6 of max|zeta| (tests bound it by 1e-5), not to 1e-9. */
+#define ENCORE_FP32_HARMONICS 2u
 int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
                       double box_size, unsigned flags);
 

@@ -113,6 +113,7 @@ def encore_plan(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: i
 
 
 ALLPARITY = 1
+FP32_HARMONICS = 2
 
 
 def encore_plan_flags(npcf_order: int, r_min: float, r_max: float, nbins: int, lmax: int, box_size: float, flags: int):
@@ -280,10 +281,10 @@ def encore_measure_fp64_peak(cuda_stream: int = 0) -> float:
 class Plan:
     """RAII wrapper: Plan(order, r_min, r_max, nbins, lmax, box) -> .compute(pos, w) on CUDA tensors."""
 
-    def __init__(self, order, r_min, r_max, nbins, lmax, box=0.0, allparity=False):
+    def __init__(self, order, r_min, r_max, nbins, lmax, box=0.0, allparity=False, fp32_harmonics=False):
         self.order, self.r_min, self.r_max, self.nbins, self.lmax, self.box = order, r_min, r_max, nbins, lmax, box
-        self.h = (encore_plan_flags(order, r_min, r_max, nbins, lmax, box, ALLPARITY) if allparity
-                  else encore_plan(order, r_min, r_max, nbins, lmax, box))
+        flags = (ALLPARITY if allparity else 0) | (FP32_HARMONICS if fp32_harmonics else 0)
+        self.h = encore_plan_flags(order, r_min, r_max, nbins, lmax, box, flags) if flags else encore_plan(order, r_min, r_max, nbins, lmax, box)
         self.n_lambda = encore_num_multiplets(self.h)
         self.n_b = encore_num_bin_tuples(self.h)
 

@@ -39,6 +39,7 @@ struct encore_plan_s {
     std::vector<CtaPlan> ctas;      // factorised N = 4, 5 kernels: multiplets and staged l-blocks per CTA
     size_t cta_smem = 0;
     bool force_generic = false;
+    bool fp32_harmonics = false;    // ENCORE_FP32_HARMONICS
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
@@ -311,6 +312,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     std::sort(pa.bin_order, pa.bin_order + nb, [&](int x, int y) { return T.vinv[x] != T.vinv[y] ? T.vinv[x] < T.vinv[y] : x < y; });
     pa.rmax = T.rmax;
     pa.lmax = T.lmax; pa.ncomp = ncomp;
+    pa.fp32_harmonics = P->fp32_harmonics ? 1 : 0;
     pa.ynorm = P->d_ynorm.as<double>();
     pa.ycoef = P->d_ycoef.as<double>();
     pa.alm = P->alm.as<double>();
@@ -452,7 +454,7 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
 int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax, double box_size,
                       unsigned flags)
 {
-    if (flags & ~(unsigned)ENCORE_ALLPARITY) return plan_out ? (*plan_out = nullptr, ENCORE_EINVAL) : ENCORE_EINVAL;
+    if (flags & ~(unsigned)(ENCORE_ALLPARITY | ENCORE_FP32_HARMONICS)) return plan_out ? (*plan_out = nullptr, ENCORE_EINVAL) : ENCORE_EINVAL;
     if (!plan_out) return ENCORE_EINVAL;
     *plan_out = nullptr;
     if (npcf_order < 3 || npcf_order > ENCORE_MAX_ORDER) return ENCORE_EINVAL;
@@ -469,6 +471,7 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
         delete P;
         return ENCORE_EALLOC;
     }
+    P->fp32_harmonics = (flags & ENCORE_FP32_HARMONICS) != 0;
     if (npcf_order >= 4 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
     *plan_out = P;
     return ENCORE_OK;

@@ -58,6 +58,7 @@ struct PairArgs {
     BinTable bins;
     double rmax;
     int lmax, ncomp;
+    int fp32_harmonics;         // ENCORE_FP32_HARMONICS: k_harm evaluates the weighted harmonics in fp32 (fp64 accumulation)
     const double *ynorm;        // [ncomp] device
     const double *ycoef;        // [ncomp][lmax+1] device: Y_lm = sum_k ycoef[c][k] z^k (x+iy)^m
     double *alm;                // [ngroups][ncomp][nbins][32]

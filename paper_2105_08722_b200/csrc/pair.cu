@@ -76,22 +76,23 @@ __device__ __forceinline__ int cell_coord(double x, double org, double inv, int 
 // Same number of accumulators as the a_lm themselves ((LMAX+1)^2 reals over all m) and one FMA each per pair; the
 // Legendre polynomials p_lm(z) are applied once per (primary, bin) in the epilogue through the table ycoef
 // (tables.cpp): 4 multiplies for the powers of z replace the 2 operations per (l,m) of a recurrence in every pair.
-template <int LMAX, int MLO, int MHI>
-__device__ __forceinline__ void accumulate(double (&acc)[ncomp_range(LMAX, MLO, MHI)], double x, double y, double z,
-                                           double w)
+// T = double: the fp64 path.  T = float: the fp32-harmonics variant: same operations
+// in fp32 into fp32 chunk sums that k_harm adds to the fp64 accumulators every 16 pairs.
+template <int LMAX, int MLO, int MHI, class T>
+__device__ __forceinline__ void accumulate(T (&acc)[ncomp_range(LMAX, MLO, MHI)], T x, T y, T z, T w)
 {
-    double zp[LMAX + 1];
-    zp[0] = 1.0;
+    T zp[LMAX + 1];
+    zp[0] = T(1);
 #pragma unroll
     for (int k = 1; k <= LMAX - MLO; ++k) zp[k] = k == 1 ? z : zp[k - 1] * z;
-    double c = w, s = 0.0; // w (x + i y)^m
+    T c = w, s = T(0); // w (x + i y)^m
     int k = 0;
 #pragma unroll
     for (int m = 0; m <= MHI; ++m) {
         if (m == 1) { c = w * x; s = w * y; }
         if (m > 1) {
-            const double cn = fma(c, x, -(s * y));
-            const double sn = fma(c, y, s * x);
+            const T cn = fma(c, x, -(s * y));
+            const T sn = fma(c, y, s * x);
             c = cn; s = sn;
         }
         if (m >= MLO) {
@@ -554,7 +555,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // CAREFUL: the bin reaches outside fp32's comfortable range for r^2 (r_min = 0, or extreme units): library rsqrt.
 struct HarmStats { unsigned steps; };
 
-template <int LMAX, int MLO, int MHI, int MODE, int D, bool CAREFUL>
+template <int LMAX, int MLO, int MHI, int MODE, int D, bool CAREFUL, bool F32>
 __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ rows,
                                               const unsigned *__restrict__ rdesc, int nrows, bool active, uint2 *q,
                                               unsigned *stm, unsigned *std_, const double4 *__restrict__ pos4,
@@ -658,6 +659,18 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
         ent[d] = gen();
         r[d] = gather(pos4, ent[d] & kIdxMask);
     }
+    // F32: fp32 chunk sums, added to the fp64 accumulators every four loop trips (16 pairs)
+    constexpr int NACCF = F32 ? ncomp_range(LMAX, MLO, MHI) : 1;
+    float facc[NACCF];
+#pragma unroll
+    for (int k = 0; k < NACCF; ++k) facc[k] = 0.f;
+    int trips = 0;
+    auto flush_f32 = [&]() {
+        if constexpr (F32) {
+#pragma unroll
+            for (int k = 0; k < NACCF; ++k) { acc[k] += (double)facc[k]; facc[k] = 0.f; }
+        }
+    };
     // MODE 1: byte address of this thread's column of mtab; the image code of an axis selects one of three rows
     const char *const mcol = reinterpret_cast<const char *>(mtab);
     constexpr unsigned kRowB = kHarmWarps * 32 * 8;   // bytes per mtab row (power of two: 1024 at 4 warps)
@@ -682,13 +695,34 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
                 const double wj = r[u % D].zw.y;
                 ent[u % D] = gen();
                 r[u % D] = gather(pos4, ent[u % D] & kIdxMask); // D candidates ahead
-                const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
-                const double rinv = CAREFUL ? rsqrt(r2s) : rsqrt_pair(r2s);
-                accumulate<LMAX, MLO, MHI>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
+                if constexpr (F32) {
+                    // fp32 harmonics: the separation is formed in fp64 (positions are large, separations small) and
+                    // rounded once; unit vector, powers and (x+iy)^m in fp32.  CAREFUL bins keep the fp64 normalisation.
+                    float fx, fy, fz;
+                    if (CAREFUL) {
+                        const double rinv = rsqrt(fma(dz, dz, fma(dy, dy, dx * dx)));
+                        fx = (float)(dx * rinv); fy = (float)(dy * rinv); fz = (float)(dz * rinv);
+                    } else {
+                        fx = (float)dx; fy = (float)dy; fz = (float)dz;
+                        const float r2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+                        float y0;
+                        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(r2f));
+                        const float h = 0.5f * y0;
+                        const float rinvf = fmaf(h, fmaf(-r2f * y0, y0, 1.f), y0); // one Newton step: ~1 ulp
+                        fx *= rinvf; fy *= rinvf; fz *= rinvf;
+                    }
+                    accumulate<LMAX, MLO, MHI, float>(facc, fx, fy, fz, (float)wj);
+                } else {
+                    const double r2s = fma(dz, dz, fma(dy, dy, dx * dx));
+                    const double rinv = CAREFUL ? rsqrt(r2s) : rsqrt_pair(r2s);
+                    accumulate<LMAX, MLO, MHI, double>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
+                }
             }
+            if (F32 && ++trips == 4) { flush_f32(); trips = 0; }
         }
         S = refill();
     } while (S > 0);
+    flush_f32();
     cp_async_wait<0>();
     return npairs;
 }
@@ -701,10 +735,12 @@ constexpr size_t harm_smem_bytes(bool periodic)
            (size_t)kHarmWarps * 2 * kStageRows * 32 * 4 + (size_t)kHarmWarps * 2 * kStageRows * 4;
 }
 
-template <int LMAX, int MLO, int MHI, bool PERIODIC>
-__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3) k_harm(PairArgs a, int g0, int g1, int write_counts)
+// F32: the fp32-harmonics variant (ENCORE_FP32_HARMONICS): weighted harmonics in fp32, fp64 accumulation of 16-pair
+// chunk sums; the pair list (binning) is the fp64-exact one of k_fill either way.
+template <int LMAX, int MLO, int MHI, bool PERIODIC, bool F32>
+__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > (F32 ? 30 : ENCORE_HARM_FAT) ? 2 : 3) k_harm(PairArgs a, int g0, int g1, int write_counts)
 {
-    constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH;
+    constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = F32 ? 2 : (NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH);
     extern __shared__ __align__(16) unsigned char harm_smem[];
     double *mtab = reinterpret_cast<double *>(harm_smem);
     uint2 *s_q = reinterpret_cast<uint2 *>(harm_smem + (PERIODIC ? (size_t)12 * kHarmWarps * 32 * 8 : 0));
@@ -741,8 +777,8 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     unsigned np;
     HarmStats st{0u};
     if (!PERIODIC) {
-        if (careful) np = harm_rows<LMAX, MLO, MHI, 0, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
-        else np = harm_rows<LMAX, MLO, MHI, 0, D, false>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
+        if (careful) np = harm_rows<LMAX, MLO, MHI, 0, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
+        else np = harm_rows<LMAX, MLO, MHI, 0, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
     } else if (fast) {
         double *mt = mtab + threadIdx.x;
         const double L = a.geom.box;
@@ -751,9 +787,9 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
         mt[4 * R] = me.y - L; mt[5 * R] = me.y; mt[6 * R] = me.y + L;
         mt[8 * R] = me.z - L; mt[9 * R] = me.z; mt[10 * R] = me.z + L;
         __syncwarp();
-        if (careful) np = harm_rows<LMAX, MLO, MHI, 1, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
-        else np = harm_rows<LMAX, MLO, MHI, 1, D, false>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
-    } else np = harm_rows<LMAX, MLO, MHI, 2, D, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st);
+        if (careful) np = harm_rows<LMAX, MLO, MHI, 1, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
+        else np = harm_rows<LMAX, MLO, MHI, 1, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
+    } else np = harm_rows<LMAX, MLO, MHI, 2, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st);
     if (write_counts) {
         a.counts[col] = np;     // n_i(b); every m-range pass walks the same bits, the first one reports
 #ifdef ENCORE_HARM_STATS
@@ -789,8 +825,8 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     }
 }
 
-template <int LMAX, int MLO, int MHI>
-cudaError_t launch_harm(const PairArgs &a, int g0, int g1, int write_counts, cudaStream_t s, int *launches)
+template <int LMAX, int MLO, int MHI, bool F32>
+cudaError_t launch_harm_t(const PairArgs &a, int g0, int g1, int write_counts, cudaStream_t s, int *launches)
 {
     const int nitems = (g1 - g0) * a.bins.nbins;
     const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
@@ -798,15 +834,22 @@ cudaError_t launch_harm(const PairArgs &a, int g0, int g1, int write_counts, cud
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(true));
+        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(true));
         if (attr_err == cudaSuccess)
-            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(false));
+            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(false));
     });
     if (attr_err != cudaSuccess) return attr_err;
-    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true><<<grid, kHarmWarps * 32, harm_smem_bytes(true), s>>>(a, g0, g1, write_counts);
-    else k_harm<LMAX, MLO, MHI, false><<<grid, kHarmWarps * 32, harm_smem_bytes(false), s>>>(a, g0, g1, write_counts);
+    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(true), s>>>(a, g0, g1, write_counts);
+    else k_harm<LMAX, MLO, MHI, false, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(false), s>>>(a, g0, g1, write_counts);
     *launches += 1;
     return cudaGetLastError();
+}
+
+template <int LMAX, int MLO, int MHI>
+cudaError_t launch_harm(const PairArgs &a, int g0, int g1, int write_counts, cudaStream_t s, int *launches)
+{
+    return a.fp32_harmonics ? launch_harm_t<LMAX, MLO, MHI, true>(a, g0, g1, write_counts, s, launches)
+                            : launch_harm_t<LMAX, MLO, MHI, false>(a, g0, g1, write_counts, s, launches);
 }
 
 } // namespace
