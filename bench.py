@@ -42,8 +42,8 @@ import workloads as W  # noqa: E402
 
 SM_COUNT, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this
-# round's kernels on c3 (profiles/r2_ncu_full_c3.txt names the command); None for workloads that were not captured
-NCU_DRAM_BYTES = {"c3": {"k_fill": 1.95e9, "k_harm": 2.96e9, "k_contract": None}}
+# round's kernels (profiles/r2_ncu_full_c3.txt and r2_ncu_full_c5.txt name the commands); None where not captured
+NCU_DRAM_BYTES = {"c3": {"k_fill": 1.949e9, "k_harm": 2.954e9, "k_contract": 5.326e9}, "c5": {"k_contract": 0.341e9}}
 NCU_PROFILE = "profiles/r2_ncu_full_c3.txt"
 
 
