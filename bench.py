@@ -260,9 +260,9 @@ def kernel_rooflines(cfg, res, fp64_peak, fp32_peak):
     """one entry per real kernel of the step, the one with the largest share of the step first"""
     km = res["kernel_ms"]
     ex, ca = res["flops_contraction"]
-    hname = f"k_harm<{cfg.lmax}, 0, {cfg.lmax if cfg.lmax <= 7 else (2 if cfg.lmax == 8 else 3)}, {1 if cfg.box > 0 else 0}>"
+    hname = f"k_harm<{cfg.lmax}, 0, {cfg.lmax if cfg.lmax <= 7 else (2 if cfg.lmax == 8 else 3)}, {1 if cfg.box > 0 else 0}, 0>"
     if cfg.lmax > 7:
-        hname += f" + k_harm<{cfg.lmax}, {3 if cfg.lmax == 8 else 4}, {cfg.lmax}, {1 if cfg.box > 0 else 0}>"
+        hname += f" + k_harm<{cfg.lmax}, {3 if cfg.lmax == 8 else 4}, {cfg.lmax}, {1 if cfg.box > 0 else 0}, 0>"
     cname = {3: f"k_contract3<{cfg.nbins}>", 4: f"k_contract4<{cfg.nbins}>", 5: f"k_contract5<{cfg.nbins}>"}[cfg.order]
     traffic = NCU_DRAM_BYTES.get(cfg.name, {})
     ents = []

@@ -62,6 +62,10 @@ def _load():
                                 C.c_int, C.c_int, C.c_int, ip, C.c_int64, C.c_int64, C.c_int64,
                                 C.c_int, dp, dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), dp, dp]
     lib.oracle_num_threads.restype = C.c_int
+    lib.oracle_gaunt.restype = C.c_double
+    lib.oracle_gaunt.argtypes = [C.c_int] * 6
+    lib.oracle_generalized_gaunt.restype = C.c_double
+    lib.oracle_generalized_gaunt.argtypes = [C.c_int, ip, ip, ip]
     _lib = lib
     return lib
 
@@ -190,3 +194,53 @@ def zeta(order, pos, w, box, rmin, rmax, nbins, lmax, *, allparity=False, bins=N
         raise ValueError(f"oracle_zeta failed with status {rc}")
     return dict(zeta=z, zeta_im=zi, bin_counts=bc, prim_counts=pc, max_imag=mi.value,
                 multiplets=lam, bins=bt, stage_seconds=(float(secs[0]), float(secs[1])))
+
+
+# ---- edge correction (eqs. 39-42) ------------------------------------------
+def gaunt(l1, l2, l3, m1, m2, m3) -> float:
+    """Gaunt integral, eq. 13."""
+    return float(_load().oracle_gaunt(l1, l2, l3, m1, m2, m3))
+
+
+def generalized_gaunt(order: int, lam_a, lam_b, lam_c) -> float:
+    """G^{Lam Lam' Lam''} = int dR P_Lam P_Lam' P_Lam'' (eq. 15) from its definition (sum over M, M' of C C C prod Gaunt)."""
+    a, b, c = (np.ascontiguousarray(v, dtype=np.int32) for v in (lam_a, lam_b, lam_c))
+    return float(_load().oracle_generalized_gaunt(order, _ip(a), _ip(b), _ip(c)))
+
+
+def principal_sum(order: int, lam) -> int:
+    lam = [int(v) for v in lam]
+    return {3: lambda x: 2 * x[0], 4: sum, 5: lambda x: x[0] + x[1] + x[3] + x[4], 6: lambda x: x[0] + x[1] + x[3] + x[5] + x[6]}[order](lam)
+
+
+def gaunt_tensor(order: int, lams) -> np.ndarray:
+    """T[Lam, Lam', Lam''] = E(Lam'') G^{Lam Lam' Lam''} over the given multiplet list (the bracket of eq. 41 before
+    the f_Lam' weights)."""
+    lams = np.ascontiguousarray(lams, dtype=np.int32)
+    n = len(lams)
+    T = np.zeros((n, n, n))
+    for i in range(n):
+        for j in range(n):
+            for k in range(n):
+                e = -1.0 if principal_sum(order, lams[k]) % 2 else 1.0
+                T[i, j, k] = e * generalized_gaunt(order, lams[i], lams[j], lams[k])
+    return T
+
+
+def edge_correct(order: int, lams, N, R, T=None) -> np.ndarray:
+    """Edge-corrected multiplets, eq. 42, one linear system per bin tuple B:
+        f_Lam'(B) = R_Lam'^B / R_0^B;   M_{Lam Lam''}(B) = sum_Lam' f_Lam'(B) E(Lam'') G^{Lam Lam' Lam''}   (eq. 41)
+        sum_Lam zeta_Lam(B) M_{Lam Lam''}(B) = N_Lam''^B / R_0^B                                       (eq. 41) -> solve
+    N, R: [nLam, nB] raw multiplets of the data-minus-random and the random field on the multiplet list `lams`, whose
+    first row is the all-zero multiplet.  The basis is truncated to `lams` (as the paper truncates at lmax)."""
+    lams = np.ascontiguousarray(lams, dtype=np.int32)
+    assert not lams[0].any(), "the first multiplet must be Lambda = 0"
+    N, R = np.asarray(N, dtype=np.float64), np.asarray(R, dtype=np.float64)
+    if T is None:
+        T = gaunt_tensor(order, lams)
+    out = np.empty_like(N)
+    for iB in range(N.shape[1]):
+        f = R[:, iB] / R[0, iB]
+        M = np.einsum("j,ijk->ik", f, T)              # M[Lam, Lam'']
+        out[:, iB] = np.linalg.solve(M.T, N[:, iB] / R[0, iB])
+    return out

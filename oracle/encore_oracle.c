@@ -695,6 +695,73 @@ int oracle_zeta(int order, const double *pos, const double *w, int64_t n, double
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Edge correction (eqs. 37-42).
+ * Gaunt integral, eq. 13:
+ *   G^{l1 l2 l3}_{m1 m2 m3} = sqrt((2l1+1)(2l2+1)(2l3+1)/(4 pi)) (l1 l2 l3; m1 m2 m3)(l1 l2 l3; 0 0 0)
+ *                           = int d r^ Y_{l1 m1} Y_{l2 m2} Y_{l3 m3}.
+ * Generalised Gaunt integral, eq. 15, written out from its definition with eq. 4:
+ *   G^{Lam Lam' Lam''} = int dR^ P_Lam P_Lam' P_Lam''
+ *                      = sum_{M, M'} C^Lam_M C^Lam'_M' C^Lam''_M'' prod_k G^{l_k l'_k l''_k}_{m_k m'_k m''_k},  m''_k = -m_k - m'_k
+ * (the Gaunt integral vanishes unless its m's sum to zero).  No 9-j symbols: App. A's closed forms (A1-A3, whose 9-j
+ * rows are misprinted, reading R18) are what the TESTS compare this against.
+ * ------------------------------------------------------------------------------------------ */
+double oracle_gaunt(int l1, int l2, int l3, int m1, int m2, int m3)
+{
+    return (double)sqrtl((2 * l1 + 1) * (2 * l2 + 1) * (2 * l3 + 1) / (4.0L * PI_L)) *
+           oracle_wigner3j(l1, l2, l3, m1, m2, m3) * oracle_wigner3j(l1, l2, l3, 0, 0, 0);
+}
+
+double oracle_generalized_gaunt(int order, const int *LamA, const int *LamB, const int *LamC)
+{
+    if (order < 3 || order > ORACLE_MAX_ORDER) return 0.0;
+    const int nm = order - 1;
+    int la[5], lb[5], lc[5], ma[5], mb[5], mc[5];
+    principal_ls(order, LamA, la);
+    principal_ls(order, LamB, lb);
+    principal_ls(order, LamC, lc);
+    for (int k = 0; k < nm; ++k) /* (l l' l''; 0 0 0) = 0 unless triangle and even sum */
+        if (lc[k] < abs(la[k] - lb[k]) || lc[k] > la[k] + lb[k] || ((la[k] + lb[k] + lc[k]) & 1)) return 0.0;
+    long double tot = 0.0L;
+    for (int k = 0; k < nm - 1; ++k) ma[k] = -la[k];
+    for (;;) { /* odometer over M (last m fixed by the sum rule) */
+        int sa = 0;
+        for (int k = 0; k < nm - 1; ++k) sa += ma[k];
+        ma[nm - 1] = -sa;
+        if (abs(ma[nm - 1]) <= la[nm - 1]) {
+            const double ca = oracle_coupling(order, LamA, ma);
+            if (ca != 0.0) {
+                for (int k = 0; k < nm - 1; ++k) mb[k] = -lb[k];
+                for (;;) { /* odometer over M' */
+                    int sb = 0;
+                    for (int k = 0; k < nm - 1; ++k) sb += mb[k];
+                    mb[nm - 1] = -sb;
+                    if (abs(mb[nm - 1]) <= lb[nm - 1]) {
+                        int ok = 1;
+                        for (int k = 0; k < nm; ++k) { mc[k] = -ma[k] - mb[k]; if (abs(mc[k]) > lc[k]) ok = 0; }
+                        if (ok) {
+                            const double cb = oracle_coupling(order, LamB, mb);
+                            const double cc = cb != 0.0 ? oracle_coupling(order, LamC, mc) : 0.0;
+                            if (cc != 0.0) {
+                                long double pr = (long double)ca * cb * cc;
+                                for (int k = 0; k < nm && pr != 0.0L; ++k) pr *= oracle_gaunt(la[k], lb[k], lc[k], ma[k], mb[k], mc[k]);
+                                tot += pr;
+                            }
+                        }
+                    }
+                    int k = nm - 2;
+                    while (k >= 0 && ++mb[k] > lb[k]) { mb[k] = -lb[k]; --k; }
+                    if (k < 0) break;
+                }
+            }
+        }
+        int k = nm - 2;
+        while (k >= 0 && ++ma[k] > la[k]) { ma[k] = -la[k]; --k; }
+        if (k < 0) break;
+    }
+    return (double)tot;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP
