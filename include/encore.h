@@ -109,6 +109,19 @@ int encore_compute_host(encore_plan_t *plan, const double *positions, const doub
  * nshards = 1 is encore_compute.  Errors as encore_compute, plus ENCORE_EINVAL for shard outside [0, nshards). */
 int encore_compute_shard(encore_plan_t *plan, const double *positions, const double *weights, int64_t n, int shard,
                          int nshards, double *zeta_partial_out, void *cuda_stream);
+/* Edge correction of raw multiplets (eqs. 38-42).  n_raw = the plan's multiplets of the
+ * data-minus-random field (an encore_compute on D - R), r_raw = those of the random field (an encore_compute on R with
+ * positive weights), both DEVICE [n_Lambda][n_B] as encore_compute writes them.  Per bin tuple B:
+ *   f_Lam' = R_Lam' / R_0,  M_{Lam Lam''} = sum_Lam' f_Lam' E(Lam'') G^{Lam Lam' Lam''}  (generalised Gaunt integrals, eq. 15,
+ *   from App. A's closed forms with 3-j and 9-j symbols),  solve  sum_Lam zeta_Lam M_{Lam Lam''} = N_Lam'' / R_0   (eq. 41/42)
+ * by LU with partial pivoting, one CTA per B; zeta_out DEVICE [n_Lambda][n_B] (may not alias the inputs).  The basis is
+ * truncated to the plan's multiplet list, as the paper truncates at lmax.  Enqueued on cuda_stream; the first call builds
+ * the E G tensor on the host (n_Lambda^3 doubles) and synchronises once.  N = 3, 4, 5 and n_Lambda <= 256
+ * (ENCORE_EUNSUPPORTED otherwise: N = 6 has no closed form in the paper).  R_0 = 0 or a singular M give non-finite output. */
+int encore_edge_correct(encore_plan_t *plan, const double *n_raw, const double *r_raw, double *zeta_out, void *cuda_stream);
+/* host query (no GPU needed): the tensor encore_edge_correct uses, out[(i n + j) n + k] = E(Lam_k) G^{Lam_i Lam_j Lam_k}, n = n_Lambda */
+int encore_get_gaunt_tensor(const encore_plan_t *plan, double *out /* HOST n_Lambda^3 */);
+
 /* Plan options (host call, takes effect at the next encore_compute).  No behaviour is read from the environment.
  *   "list_mb"          byte budget, in MiB, of the pair stage's acceptance-mask rows per super-step (0 = default:
  *                      32 GiB, or half of the free device memory within 4-96 GiB when the rows need more)

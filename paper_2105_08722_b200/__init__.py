@@ -24,7 +24,7 @@ OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL = 0, -1, -2,
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -59,6 +59,8 @@ def lib():
     L.encore_get_pair_steps.argtypes = [vp]
     L.encore_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
     L.encore_get_status.argtypes = [vp]
+    L.encore_edge_correct.argtypes = [vp, vp, vp, vp, vp]
+    L.encore_get_gaunt_tensor.argtypes = [vp, dp]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
     L.encore_zeta_len.restype = C.c_int64
@@ -153,6 +155,18 @@ def encore_get_pair_steps(plan) -> int:
 
 def encore_set_option(plan, key: str, value: int):
     _check(lib().encore_set_option(plan, key.encode(), int(value)))
+
+
+def encore_edge_correct(plan, n_raw, r_raw, zeta_out, cuda_stream: int = 0):
+    """n_raw, r_raw, zeta_out: CUDA fp64 tensors [n_lambda, n_b] (or raw device pointers)."""
+    _check(lib().encore_edge_correct(plan, _ptr(n_raw), _ptr(r_raw), _ptr(zeta_out), C.c_void_p(cuda_stream)))
+
+
+def encore_get_gaunt_tensor(plan) -> np.ndarray:
+    n = encore_num_multiplets(plan)
+    out = np.empty((n, n, n))
+    _check(lib().encore_get_gaunt_tensor(plan, out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
 
 
 def encore_get_status(plan) -> int:
@@ -339,6 +353,17 @@ class Plan:
             out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
         st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
         encore_compute_shard(self.h, positions, weights, n, shard, nshards, out, st)
+        return out
+
+    def edge_correct(self, n_raw, r_raw, out=None, stream=None):
+        """Edge-corrected zeta [n_lambda, n_b] from the raw multiplets of the D-R field and of the random field (eq. 42)."""
+        import torch
+        for t in (n_raw, r_raw):
+            assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (self.n_lambda, self.n_b)
+        if out is None:
+            out = torch.empty_like(n_raw)
+        st = torch.cuda.current_stream(n_raw.device).cuda_stream if stream is None else stream
+        encore_edge_correct(self.h, n_raw, r_raw, out, st)
         return out
 
     def compute_host(self, positions: np.ndarray, weights=None) -> np.ndarray:

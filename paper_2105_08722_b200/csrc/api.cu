@@ -45,6 +45,8 @@ struct encore_plan_s {
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
     DevBuf io_pos, io_w, io_zeta;
     DevBuf gbound, gprefix, gwide, rows, rowdesc, rowcnt, errflag;
+    DevBuf d_gaunt, edge_A, edge_rhs;   // edge correction: E G tensor, per-tuple matrices and right-hand sides
+    bool gaunt_ready = false;
     int *h_gprefix = nullptr;   // pinned
     size_t h_gprefix_cap = 0;
     size_t list_budget_bytes = (size_t)32 << 30;
@@ -522,6 +524,46 @@ int encore_get_status(const encore_plan_t *P)
     return f ? ENCORE_EINTERNAL : ENCORE_OK;
 }
 
+int encore_edge_correct(encore_plan_t *P, const double *n_raw, const double *r_raw, double *zeta_out, void *cuda_stream)
+{
+    if (!P || !n_raw || !r_raw || !zeta_out) return ENCORE_EINVAL;
+    const HostTables &T = P->T;
+    const size_t n = (size_t)T.nLam(), nB = (size_t)T.nB();
+    if (T.order > 5 || n > 256) return ENCORE_EUNSUPPORTED;   // App. A gives N = 3, 4, 5; the dense E G tensor holds n^3 doubles
+    for (int k = 0; k < T.width; ++k) if (T.multiplets[k] != 0) return ENCORE_EUNSUPPORTED; // row 0 must be Lambda = 0
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (!P->gaunt_ready) {
+        std::vector<double> G;
+        try {
+            if (encore_build_gaunt_tensor(T, G) != 0) return ENCORE_EUNSUPPORTED;
+        } catch (...) {
+            return ENCORE_EALLOC;
+        }
+        CU(P->d_gaunt.ensure(sizeof(double) * G.size()));
+        CU(cudaMemcpyAsync(P->d_gaunt.p, G.data(), sizeof(double) * G.size(), cudaMemcpyHostToDevice, s));
+        CU(cudaStreamSynchronize(s)); // the staging vector dies at return
+        P->gaunt_ready = true;
+    }
+    CU(P->edge_A.ensure(sizeof(double) * nB * n * n));
+    CU(P->edge_rhs.ensure(sizeof(double) * nB * n));
+    CU(launch_edge_correct(P->d_gaunt.as<double>(), n_raw, r_raw, (int)n, (int)nB, P->edge_A.as<double>(), P->edge_rhs.as<double>(), zeta_out, s));
+    return ENCORE_OK;
+}
+
+int encore_get_gaunt_tensor(const encore_plan_t *P, double *out)
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    if (P->T.order > 5 || P->T.nLam() > 256) return ENCORE_EUNSUPPORTED;
+    std::vector<double> G;
+    try {
+        if (encore_build_gaunt_tensor(P->T, G) != 0) return ENCORE_EUNSUPPORTED;
+    } catch (...) {
+        return ENCORE_EALLOC;
+    }
+    std::memcpy(out, G.data(), sizeof(double) * G.size());
+    return ENCORE_OK;
+}
+
 int encore_get_pair_steps(const encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
@@ -568,7 +610,7 @@ int encore_destroy(encore_plan_t *P)
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
                       &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->gwide,
-                      &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag};
+                      &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag, &P->d_gaunt, &P->edge_A, &P->edge_rhs};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);

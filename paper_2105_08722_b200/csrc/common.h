@@ -91,4 +91,6 @@ struct HostTables {
 
 // Host side (tables.cpp)
 double encore_host_wigner3j(int j1, int j2, int j3, int m1, int m2, int m3);
+double encore_host_wigner9j(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9);
+int encore_build_gaunt_tensor(const HostTables &t, std::vector<double> &T); // edge correction: E(Lam'') G^{Lam Lam' Lam''}
 int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int nbins, int lmax, double box, int allparity = 0);

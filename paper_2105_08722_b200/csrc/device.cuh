@@ -129,6 +129,11 @@ size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas);
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
 
+// ---- edge.cu -------------------------------------------------------------------------------------------
+// T: [n][n][n] E G tensor; Nraw, Rraw: [n][nB] raw multiplets; A: [nB][n][n], rhs: [nB][n] scratch; zeta: [n][nB]
+cudaError_t launch_edge_correct(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *A, double *rhs,
+                                double *zeta, cudaStream_t s);
+
 // ---- diag.cu --------------------------------------------------------------------------------------------
 cudaError_t launch_sum_bin_counts(const uint32_t *counts, const int *group_start, int npencil, int nbins,
                                   unsigned long long *out, int ngroups_max, cudaStream_t s);

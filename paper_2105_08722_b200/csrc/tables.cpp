@@ -14,11 +14,11 @@ namespace {
 const long double kPi = 3.14159265358979323846264338327950288L;
 
 struct FactTable {
-    long double v[64];
+    long double v[256];
     FactTable()
     {
         v[0] = 1.0L;
-        for (int i = 1; i < 64; ++i) v[i] = v[i - 1] * (long double)i;
+        for (int i = 1; i < 256; ++i) v[i] = v[i - 1] * (long double)i;
     }
 };
 
@@ -349,5 +349,94 @@ int encore_build_tables(HostTables &t, int order, double rmin, double rmax, int 
         }
     }
     build_factorised(t);
+    return 0;
+}
+
+
+// ---- edge correction (App. A :676-691) -------------------------------------
+// Wigner 6-j by Racah's formula and 9-j as a sum over products of three 6-j symbols (NIST DLMF 34.4.2, 34.6.1);
+// integer arguments only.  The generalised Gaunt integrals then follow from App. A's closed forms (A1-A3) with the 9-j
+// rows read as (l_k l'_k l''_k) (R18; the oracle evaluates the defining sum over M instead).
+namespace {
+
+bool tri(int a, int b, int c) { return c >= std::abs(a - b) && c <= a + b; }
+
+long double delta_tri(int a, int b, int c)
+{
+    return std::sqrt(fact(a + b - c) * fact(a - b + c) * fact(-a + b + c) / fact(a + b + c + 1));
+}
+
+long double wigner6j(int a, int b, int c, int d, int e, int f)
+{
+    if (!tri(a, b, c) || !tri(a, e, f) || !tri(d, b, f) || !tri(d, e, c)) return 0.0L;
+    const int t0 = std::max(std::max(a + b + c, a + e + f), std::max(d + b + f, d + e + c));
+    const int t1 = std::min(std::min(a + b + d + e, b + c + e + f), c + a + f + d);
+    long double s = 0.0L;
+    for (int t = t0; t <= t1; ++t) {
+        const long double den = fact(t - a - b - c) * fact(t - a - e - f) * fact(t - d - b - f) * fact(t - d - e - c) *
+                                fact(a + b + d + e - t) * fact(b + c + e + f - t) * fact(c + a + f + d - t);
+        s += ((t & 1) ? -1.0L : 1.0L) * fact(t + 1) / den;
+    }
+    return delta_tri(a, b, c) * delta_tri(a, e, f) * delta_tri(d, b, f) * delta_tri(d, e, c) * s;
+}
+
+long double wigner9j(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9)
+{
+    if (!tri(j1, j2, j3) || !tri(j4, j5, j6) || !tri(j7, j8, j9) || !tri(j1, j4, j7) || !tri(j2, j5, j8) || !tri(j3, j6, j9)) return 0.0L;
+    const int x0 = std::max(std::max(std::abs(j1 - j9), std::abs(j4 - j8)), std::abs(j2 - j6));
+    const int x1 = std::min(std::min(j1 + j9, j4 + j8), j2 + j6);
+    long double s = 0.0L;
+    for (int x = x0; x <= x1; ++x)
+        s += (long double)(2 * x + 1) * wigner6j(j1, j4, j7, j8, j9, x) * wigner6j(j2, j5, j8, j4, x, j6) * wigner6j(j3, j6, j9, x, j1, j2);
+    return s;
+}
+
+// sqrt((2a+1)(2b+1)(2c+1)) (a b c; 0 0 0), zero unless triangle and even sum
+long double w000(int a, int b, int c)
+{
+    if (!tri(a, b, c) || ((a + b + c) & 1)) return 0.0L;
+    return std::sqrt((long double)((2 * a + 1) * (2 * b + 1) * (2 * c + 1))) * (long double)encore_host_wigner3j(a, b, c, 0, 0, 0);
+}
+
+} // namespace
+
+double encore_host_wigner9j(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9)
+{
+    return (double)wigner9j(j1, j2, j3, j4, j5, j6, j7, j8, j9);
+}
+
+// T[(i*n + j)*n + k] = E(Lam_k) G^{Lam_i Lam_j Lam_k} over the plan's multiplet list (N = 3, 4, 5)
+int encore_build_gaunt_tensor(const HostTables &t, std::vector<double> &T)
+{
+    const int n = t.nLam(), N = t.order;
+    if (N < 3 || N > 5) return -1;
+    T.assign((size_t)n * n * n, 0.0);
+    const long double fourpi = 4.0L * kPi;
+    for (int i = 0; i < n; ++i)
+        for (int j = i; j < n; ++j)       // G is symmetric under Lam <-> Lam'
+            for (int k = 0; k < n; ++k) {
+                const int *a = &t.multiplets[(size_t)i * t.width], *b = &t.multiplets[(size_t)j * t.width], *c = &t.multiplets[(size_t)k * t.width];
+                long double g = 0.0L;
+                if (N == 3) {             // A1
+                    const long double w = w000(a[0], b[0], c[0]);
+                    g = w == 0.0L ? 0.0L : w * w / std::sqrt((long double)((2 * a[0] + 1) * (2 * b[0] + 1) * (2 * c[0] + 1))) / fourpi;
+                } else if (N == 4) {      // A2
+                    g = w000(a[0], b[0], c[0]);
+                    if (g != 0.0L) g *= w000(a[1], b[1], c[1]);
+                    if (g != 0.0L) g *= w000(a[2], b[2], c[2]);
+                    if (g != 0.0L) g *= wigner9j(a[0], b[0], c[0], a[1], b[1], c[1], a[2], b[2], c[2]) / std::pow(fourpi, 1.5L);
+                } else {                  // A3
+                    g = w000(a[0], b[0], c[0]);
+                    if (g != 0.0L) g *= w000(a[1], b[1], c[1]);
+                    if (g != 0.0L) g *= w000(a[3], b[3], c[3]);
+                    if (g != 0.0L) g *= w000(a[4], b[4], c[4]);
+                    if (g != 0.0L) g *= std::sqrt((long double)((2 * a[2] + 1) * (2 * b[2] + 1) * (2 * c[2] + 1)));
+                    if (g != 0.0L) g *= wigner9j(a[0], a[1], a[2], b[0], b[1], b[2], c[0], c[1], c[2]);
+                    if (g != 0.0L) g *= wigner9j(a[2], a[3], a[4], b[2], b[3], b[4], c[2], c[3], c[4]) / (fourpi * fourpi);
+                }
+                const double v = (double)(t.parity[k] ? -g : g);
+                T[((size_t)i * n + j) * n + k] = v;
+                T[((size_t)j * n + i) * n + k] = v;
+            }
     return 0;
 }

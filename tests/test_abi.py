@@ -132,4 +132,24 @@ def test_allparity_tables_on_the_host():
             E.encore_destroy(h)
     import pytest
     with pytest.raises(E.EncoreError):
-        E.encore_plan_flags(4, 1.0, 20.0, 6, 2, 0.0, 2)      # unknown flag
+        E.encore_plan_flags(4, 1.0, 20.0, 6, 2, 0.0, 4)      # unknown flag
+
+
+@pytest.mark.parametrize("order,lmax,allparity", [(3, 6, False), (4, 3, False), (4, 2, True), (5, 1, False), (5, 1, True)])
+def test_gaunt_tensor_equals_the_oracle_definition(oracle, order, lmax, allparity):
+    """edge correction tables: the library builds E(Lam'') G^{Lam Lam' Lam''} from App. A's closed forms
+    (own 6-j / 9-j symbols); the oracle evaluates eq. 15's defining sum over M - two routes, one tensor"""
+    h = E.encore_plan_flags(order, 1.0, 20.0, 6, lmax, 0.0, E.ALLPARITY if allparity else 0)
+    try:
+        T = E.encore_get_gaunt_tensor(h)
+        lams = E.encore_get_multiplets(h, order)
+    finally:
+        E.encore_destroy(h)
+    ref = oracle.gaunt_tensor(order, lams)
+    assert np.abs(ref).max() > 0
+    assert np.abs(T - ref).max() <= 1e-14
+    from sympy.physics.wigner import wigner_9j
+    lib = E.lib()
+    lib.encore_get_gaunt_tensor.restype = C.c_int
+    with E.Plan(6, 1.0, 20.0, 6, 1, 0.0) as p6:
+        assert lib.encore_get_gaunt_tensor(p6.h, (C.c_double * 1)()) == E.EUNSUPPORTED

@@ -215,6 +215,42 @@ def test_fp32_harmonics_variant(E, oracle, name):
     assert np.abs(a_g - ref).max() <= (2e-6 if cfg.lmax <= 5 else 1e-3) * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("order,nbins,lmax", [(3, 6, 6), (4, 6, 3), (5, 6, 1)])
+def test_edge_correction_matches_the_oracle(E, oracle, order, nbins, lmax):
+    """SURVEY.md §8(f2), eqs. 38-42: raw multiplets of a data-minus-random field and of its randoms on
+    a cut-sky footprint (both through encore_compute), then encore_edge_correct against the oracle's eq. 41/42 on the
+    same N and R; and on synthetic N, R with strong geometry terms."""
+    cfg = W.scaled(W.CONFIGS["c4"], n=6000)
+    pos, w = W.make(cfg)
+    rand = w < 0
+    dev = torch.device("cuda:0")
+    with E.Plan(order, 20.0, 160.0, nbins, lmax, 0.0) as plan:
+        lams = plan.multiplets
+        n_raw = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).clone()
+        r_raw = plan.compute(torch.from_numpy(np.ascontiguousarray(pos[:, rand])).to(dev), torch.from_numpy(-w[rand]).to(dev)).clone()
+        z = plan.edge_correct(n_raw, r_raw)
+        torch.cuda.synchronize()
+        T = oracle.gaunt_tensor(order, lams)
+        ref = oracle.edge_correct(order, lams, n_raw.cpu().numpy(), r_raw.cpu().numpy(), T)
+        assert np.abs(z.cpu().numpy() - ref).max() <= TOL * np.abs(ref).max()
+        # the correction is not trivial on this footprint: geometry multiplets are a sizeable fraction of R_0
+        f = (r_raw / r_raw[0]).cpu().numpy()
+        assert np.abs(f[1:]).max() > 1e-2
+        rng = np.random.default_rng(order)
+        R = rng.standard_normal((plan.n_lambda, plan.n_b)) * 0.3
+        R[0] = rng.uniform(1.0, 2.0, plan.n_b)
+        R[1:] *= R[0]
+        N = rng.standard_normal((plan.n_lambda, plan.n_b))
+        z2 = plan.edge_correct(torch.from_numpy(N).to(dev), torch.from_numpy(R).to(dev)).cpu().numpy()
+        ref2 = oracle.edge_correct(order, lams, N, R, T)
+        assert np.abs(z2 - ref2).max() <= 1e-9 * np.abs(ref2).max()
+    with E.Plan(6, 20.0, 160.0, 6, 1, 0.0) as p6:
+        t = torch.zeros((p6.n_lambda, p6.n_b), dtype=torch.float64, device=dev)
+        with pytest.raises(E.EncoreError) as ei:
+            p6.edge_correct(t, t)
+        assert ei.value.status == E.EUNSUPPORTED
+
+
 def test_degenerate_inputs(E, oracle):
     # one particle: no pairs, zeta = 0
     g = gpu_run(E, 3, np.array([[1.0], [2.0], [3.0]]), np.ones(1), 0.0, 0.0, 10.0, 3, 2)
