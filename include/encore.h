@@ -109,6 +109,17 @@ int encore_compute_host(encore_plan_t *plan, const double *positions, const doub
  * nshards = 1 is encore_compute.  Errors as encore_compute, plus ENCORE_EINVAL for shard outside [0, nshards). */
 int encore_compute_shard(encore_plan_t *plan, const double *positions, const double *weights, int64_t n, int shard,
                          int nshards, double *zeta_partial_out, void *cuda_stream);
+/* Gridded estimator (eq. 36): the multiplets of a density field given on a periodic
+ * mesh.  The plan must be periodic (box_size > 0); delta DEVICE, G^3 doubles, delta[(ix G + iy) G + iz] = value at the cell
+ * centre ((ix,iy,iz) + 1/2) h, h = box_size / G.  Discretised on the mesh (int dr -> h^3 sum over cells)
+ *   a^b_lm(s) = (1/v_b) sum_{cells x != s} delta(x) h^3 Y_lm((x - s)^) Theta^b(|x - s|)        (eq. 36 evaluated with FFTs)
+ *   zeta^B_Lam = (1/V) sum_{cells s} delta(s) h^3 sum_M E(Lam) C^Lam_M prod_k a^{b_k}_{l_k m_k}(s)  (steps i-iii)
+ * i.e. eq. 34/35 for particles at the cell centres with weights delta h^3; separations are (integer offset) h, minimal
+ * image, binned on r^2 like the particle path.  zeta_out DEVICE as for encore_compute.  Scratch: two complex G^3 fields and
+ * the a_lm array of all cells, (lmax+1)^2 nbins G^3 doubles (the memory cost the paper warns of, PAPER.md fn. 5).  Uses cuFFT.
+ * Enqueued on cuda_stream without host synchronisation once the scratch exists.  2 <= G <= 1024. */
+int encore_compute_grid(encore_plan_t *plan, const double *delta, int G, double *zeta_out, void *cuda_stream);
+
 /* Edge correction of raw multiplets (eqs. 38-42).  n_raw = the plan's multiplets of the
  * data-minus-random field (an encore_compute on D - R), r_raw = those of the random field (an encore_compute on R with
  * positive weights), both DEVICE [n_Lambda][n_B] as encore_compute writes them.  Per bin tuple B:

@@ -24,7 +24,7 @@ OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL = 0, -1, -2,
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor", "encore_compute_grid",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -61,6 +61,7 @@ def lib():
     L.encore_get_status.argtypes = [vp]
     L.encore_edge_correct.argtypes = [vp, vp, vp, vp, vp]
     L.encore_get_gaunt_tensor.argtypes = [vp, dp]
+    L.encore_compute_grid.argtypes = [vp, vp, C.c_int, vp, vp]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
     L.encore_zeta_len.restype = C.c_int64
@@ -160,6 +161,10 @@ def encore_set_option(plan, key: str, value: int):
 def encore_edge_correct(plan, n_raw, r_raw, zeta_out, cuda_stream: int = 0):
     """n_raw, r_raw, zeta_out: CUDA fp64 tensors [n_lambda, n_b] (or raw device pointers)."""
     _check(lib().encore_edge_correct(plan, _ptr(n_raw), _ptr(r_raw), _ptr(zeta_out), C.c_void_p(cuda_stream)))
+
+
+def encore_compute_grid(plan, delta, G: int, zeta_out, cuda_stream: int = 0):
+    _check(lib().encore_compute_grid(plan, _ptr(delta), G, _ptr(zeta_out), C.c_void_p(cuda_stream)))
 
 
 def encore_get_gaunt_tensor(plan) -> np.ndarray:
@@ -353,6 +358,18 @@ class Plan:
             out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
         st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
         encore_compute_shard(self.h, positions, weights, n, shard, nshards, out, st)
+        return out
+
+    def compute_grid(self, delta, out=None, stream=None):
+        """zeta of a density field on a periodic mesh: delta CUDA fp64 tensor (G, G, G) (encore_compute_grid, eq. 36)."""
+        import torch
+        assert delta.is_cuda and delta.dtype == torch.float64 and delta.is_contiguous() and delta.dim() == 3
+        G = delta.shape[0]
+        assert tuple(delta.shape) == (G, G, G)
+        if out is None:
+            out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=delta.device)
+        st = torch.cuda.current_stream(delta.device).cuda_stream if stream is None else stream
+        encore_compute_grid(self.h, delta, G, out, st)
         return out
 
     def edge_correct(self, n_raw, r_raw, out=None, stream=None):

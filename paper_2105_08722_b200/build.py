@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libencore_b200.so")
-SOURCES = ["tables.cpp", "grid.cu", "pair.cu", "contract.cu", "edge.cu", "diag.cu", "api.cu"]
+SOURCES = ["tables.cpp", "grid.cu", "pair.cu", "contract.cu", "edge.cu", "mesh.cu", "diag.cu", "api.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", INCLUDE] + os.environ.get("ENCORE_NVCC_FLAGS", "").split()
@@ -62,7 +62,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
         objs = list(ex.map(lambda s: _compile(s, verbose), SOURCES))
     tmp = LIB + f".{os.getpid()}.tmp"
-    r = subprocess.run([NVCC, "-shared", "-o", tmp, *objs, "-lcudart"], capture_output=True, text=True)
+    r = subprocess.run([NVCC, "-shared", "-o", tmp, *objs, "-lcudart", "-lcufft"], capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, LIB)

@@ -45,6 +45,8 @@ struct encore_plan_s {
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
     DevBuf io_pos, io_w, io_zeta;
     DevBuf gbound, gprefix, gwide, rows, rowdesc, rowcnt, errflag;
+    DevBuf mesh_fd, mesh_kern;          // gridded estimator: F[delta h^3] and the kernel / a_lm field being transformed
+    int mesh_fft = -1, mesh_G = 0;      // cuFFT plan for G^3
     DevBuf d_gaunt, edge_A, edge_rhs;   // edge correction: E G tensor, per-tuple matrices and right-hand sides
     bool gaunt_ready = false;
     int *h_gprefix = nullptr;   // pinned
@@ -199,6 +201,64 @@ int mark(encore_plan_s *P, int kind, cudaStream_t s)
 
 #define TRY(call) do { int r__ = (call); if (r__ != ENCORE_OK) return r__; } while (0)
 
+// steps a5 + a6 on a_lm tiles [group][component][bin][lane] with primary weights gweights[group][lane]
+int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweights, int g_begin, int g_end, int ngmax, bool factorised,
+                        int nchunk, double *zeta_out, cudaStream_t s)
+{
+    const HostTables &T = P->T;
+    ContractArgs ca{};
+    ca.order = T.order; ca.nbins = T.nbins; ca.ncomp = T.ncomp; ca.nLam = T.nLam(); ca.nB = T.nB();
+    ca.terms = P->d_terms.as<DevTerm>();
+    ca.term_start = P->d_term_start.as<int>();
+    ca.bin_tuples = P->d_bin_tuples.as<int>();
+    ca.alm = alm; ca.gweights = gweights;
+    ca.partial = P->partial.as<double>();
+    ca.partial2 = P->partial2.as<double>();
+    ca.nseg = 64;
+    ca.vinv_total = T.box > 0.0 ? 1.0 / (T.box * T.box * T.box) : 1.0; // DESIGN.md R12
+    ca.zeta_out = zeta_out;
+    ca.ngroups_max = ngmax;
+    ca.g_begin = g_begin; ca.g_end = g_end;
+    ca.pair_terms = P->d_pair_terms.as<PairTerm>();
+    ca.lam4 = P->d_lam4.as<Lam4>();
+    ca.lam5 = P->d_lam5.as<Lam5>();
+    ca.lam_order = P->d_lam_order.as<int>();
+    ca.lam_parity = P->d_lam_parity.as<int>();
+    ca.tuple_index = P->d_tuple_index.as<int>();
+    ca.lmax = T.lmax;
+    ca.max_terms = 1;
+    for (const Lam4 &q : T.lam4) ca.max_terms = std::max(ca.max_terms, q.nterms);
+    for (const Lam5 &q : T.lam5) ca.max_terms = std::max(ca.max_terms, q.nterms);
+    ca.ctas = P->d_ctas.as<CtaPlan>();
+    ca.ncta = (int)P->ctas.size();
+    ca.cta_smem = P->cta_smem;
+    ca.nchunk = nchunk;
+    ca.factorised = factorised ? 1 : 0;
+    CU(launch_contraction(ca, s, &P->launches));
+    TRY(mark(P, K_CONTRACT, s));
+    CU(launch_reduction(ca, s, &P->launches));
+    TRY(mark(P, K_REDUCE, s));
+    return ENCORE_OK;
+}
+
+// chunks of groups per multiplet slot of the factorised kernels: the grid (slots x chunks CTAs, one per SM) should fill whole waves
+int choose_nchunk(const encore_plan_s *P, bool factorised)
+{
+    int nchunk = 32;
+    if (factorised) {
+        int sms = 148, dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const int slots = P->T.order == 3 ? P->T.nLam() : (int)P->ctas.size();
+        double best = 0.0;
+        for (int c = 28; c <= 40; ++c) {
+            const int ctas = slots * c, waves = (ctas + sms - 1) / sms;
+            const double eff = (double)ctas / ((double)waves * sms) - 1e-4 * std::abs(c - 32);
+            if (eff > best) { best = eff; nchunk = c; }
+        }
+    }
+    return nchunk;
+}
+
 // shard/nshards: the primaries are cut into nshards contiguous ranges of cell-sorted groups with equal pair-stage
 // work bounds; this call evaluates the sums over the primaries of range `shard` only (1 of 1 = everything).
 int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t n, double *zeta_out, cudaStream_t s,
@@ -235,7 +295,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     const int ngmax = (int)(n / ENCORE_GROUP) + G.npencil + 1;
     const int nb = T.nbins, ncomp = T.ncomp;
     const size_t nout = (size_t)T.nLam() * T.nB();
-    const int nseg = 64;
+    const int nseg = 64;   // (contract_and_reduce uses the same count)
 
     // ---- scratch ----------------------------------------------------------------------------------------------
     CU(P->cid.ensure(sizeof(int32_t) * n));
@@ -251,19 +311,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
     CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
     const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax) && (T.order == 3 || P->cta_smem > 0);
-    // chunks of groups per multiplet slot: the grid (slots x chunks CTAs, one per SM) should fill whole waves
-    int nchunk = 32;
-    if (factorised) {
-        int sms = 148, dev = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        const int slots = T.order == 3 ? T.nLam() : (int)P->ctas.size();
-        double best = 0.0;
-        for (int c = 28; c <= 40; ++c) {
-            const int ctas = slots * c, waves = (ctas + sms - 1) / sms;
-            const double eff = (double)ctas / ((double)waves * sms) - 1e-4 * std::abs(c - 32);
-            if (eff > best) { best = eff; nchunk = c; }
-        }
-    }
+    const int nchunk = choose_nchunk(P, factorised);
     CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout));
     CU(P->gweights.ensure(sizeof(double) * (size_t)ngmax * 32));
     CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
@@ -403,41 +451,8 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     }
     // internal-consistency flag of the pair stage, read by whoever synchronises next (encore_get_status, the getters)
     CU(cudaMemcpyAsync(reinterpret_cast<int *>(P->pinned + 7), P->errflag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
-    // ---- a5: contraction ---------------------------------------------------------------------------------------
-    ContractArgs ca{};
-    ca.order = T.order; ca.nbins = nb; ca.ncomp = ncomp; ca.nLam = T.nLam(); ca.nB = T.nB();
-    ca.terms = P->d_terms.as<DevTerm>();
-    ca.term_start = P->d_term_start.as<int>();
-    ca.bin_tuples = P->d_bin_tuples.as<int>();
-    ca.alm = pa.alm; ca.gweights = pa.gweights; ca.pos4 = pa.pos4; ca.cell_start = pa.cell_start; ca.group_start = pa.group_start;
-    ca.geom = G;
-    ca.partial = P->partial.as<double>();
-    ca.partial2 = P->partial2.as<double>();
-    ca.nseg = nseg;
-    ca.vinv_total = T.box > 0.0 ? 1.0 / (T.box * T.box * T.box) : 1.0; // DESIGN.md R12
-    ca.zeta_out = zeta_out;
-    ca.ngroups_max = ngmax;
-    ca.g_begin = g_begin; ca.g_end = g_end;
-    ca.pair_terms = P->d_pair_terms.as<PairTerm>();
-    ca.lam4 = P->d_lam4.as<Lam4>();
-    ca.lam5 = P->d_lam5.as<Lam5>();
-    ca.lam_order = P->d_lam_order.as<int>();
-    ca.lam_parity = P->d_lam_parity.as<int>();
-    ca.tuple_index = P->d_tuple_index.as<int>();
-    ca.lmax = T.lmax;
-    ca.max_terms = 1;
-    for (const Lam4 &q : T.lam4) ca.max_terms = std::max(ca.max_terms, q.nterms);
-    for (const Lam5 &q : T.lam5) ca.max_terms = std::max(ca.max_terms, q.nterms);
-    ca.ctas = P->d_ctas.as<CtaPlan>();
-    ca.ncta = (int)P->ctas.size();
-    ca.cta_smem = P->cta_smem;
-    ca.nchunk = nchunk;
-    ca.factorised = factorised ? 1 : 0;
-    CU(launch_contraction(ca, s, &P->launches));
-    TRY(mark(P, K_CONTRACT, s));
-    // ---- a6: reduction -----------------------------------------------------------------------------------------
-    CU(launch_reduction(ca, s, &P->launches));
-    TRY(mark(P, K_REDUCE, s));
+    // ---- a5: contraction, a6: reduction ------------------------------------------------------------------------
+    TRY(contract_and_reduce(P, pa.alm, pa.gweights, g_begin, g_end, ngmax, factorised, nchunk, zeta_out, s));
 
     P->have = true; P->n = n; P->geom = G; P->ngroups_max = ngmax; P->stream = s;
     P->g_begin = g_begin; P->g_end = g_end; P->ngroups = ngroups_total;
@@ -522,6 +537,42 @@ int encore_get_status(const encore_plan_t *P)
     int f = 0;
     std::memcpy(&f, P->pinned + 7, sizeof(int));
     return f ? ENCORE_EINTERNAL : ENCORE_OK;
+}
+
+int encore_compute_grid(encore_plan_t *P, const double *delta, int G, double *zeta_out, void *cuda_stream)
+{
+    if (!P || !delta || !zeta_out || G < 2 || G > 1024) return ENCORE_EINVAL;
+    const HostTables &T = P->T;
+    if (!(T.box > 0.0)) return ENCORE_EINVAL;     // the mesh is periodic
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    P->have = false;
+    P->launches = 0;
+    TRY(upload_tables(P, s));
+    const size_t ncell = (size_t)G * G * G, npad = (ncell + 31) / 32 * 32;
+    const int ngroups = (int)(npad / 32), nb = T.nbins, ncomp = T.ncomp;
+    const size_t nout = (size_t)T.nLam() * T.nB();
+    const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax) && (T.order == 3 || P->cta_smem > 0);
+    const int nchunk = choose_nchunk(P, factorised);
+    CU(P->mesh_fd.ensure(sizeof(double) * 2 * ncell));
+    CU(P->mesh_kern.ensure(sizeof(double) * 2 * ncell));
+    CU(P->alm.ensure(sizeof(double) * (size_t)ngroups * ncomp * nb * 32));
+    CU(P->gweights.ensure(sizeof(double) * npad));
+    CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngroups) * nout));
+    CU(P->partial2.ensure(sizeof(double) * (size_t)64 * nout));
+    if (P->mesh_fft < 0 || P->mesh_G != G) {
+        if (P->mesh_fft >= 0) mesh_fft_plan_destroy(P->mesh_fft);
+        P->mesh_fft = -1;
+        if (mesh_fft_plan_create(G, s, &P->mesh_fft) != 0) return ENCORE_EALLOC;
+        P->mesh_G = G;
+    } else if (mesh_fft_plan_set_stream(P->mesh_fft, s) != 0) return ENCORE_ECUDA;
+    TRY(mark(P, K_START, s));
+    int fft_error = 0;
+    CU(launch_mesh_alm(delta, G, T.box, T.lmax, nb, T.edges2.data(), T.vinv.data(), P->d_ycoef.as<double>(), P->mesh_fd.p, P->mesh_kern.p,
+                       P->alm.as<double>(), P->gweights.as<double>(), P->mesh_fft, s, &P->launches, &fft_error));
+    if (fft_error) return ENCORE_ECUDA;
+    TRY(mark(P, K_HARM, s));
+    TRY(contract_and_reduce(P, P->alm.as<double>(), P->gweights.as<double>(), 0, ngroups, ngroups, factorised, nchunk, zeta_out, s));
+    return ENCORE_OK;
 }
 
 int encore_edge_correct(encore_plan_t *P, const double *n_raw, const double *r_raw, double *zeta_out, void *cuda_stream)
@@ -610,11 +661,12 @@ int encore_destroy(encore_plan_t *P)
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
                       &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->gwide,
-                      &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag, &P->d_gaunt, &P->edge_A, &P->edge_rhs};
+                      &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag, &P->d_gaunt, &P->edge_A, &P->edge_rhs, &P->mesh_fd, &P->mesh_kern};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
     for (cudaEvent_t e : P->ev) cudaEventDestroy(e);
+    if (P->mesh_fft >= 0) mesh_fft_plan_destroy(P->mesh_fft);
     delete P;
     return ENCORE_OK;
 }

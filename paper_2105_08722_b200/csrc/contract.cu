@@ -24,15 +24,10 @@ constexpr unsigned kFull = 0xffffffffu;
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
     const int g = a.g_begin + blockIdx.x;
-    const GridGeom &G = a.geom;
     if (g >= a.g_end) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nb = a.nbins, nm = a.order - 1;
-    const int p = find_pencil_of_group(a.group_start, G.npencil, g);
-    const int pstart = a.cell_start[p * G.nc[0]], pend = a.cell_start[(p + 1) * G.nc[0]];
-    const int first = pstart + ENCORE_GROUP * (g - a.group_start[p]);
-    const int cnt = min(ENCORE_GROUP, pend - first);
-    const double wi = lane < cnt ? a.pos4[first + lane].w : 0.0;
+    const double wi = a.gweights[(size_t)g * 32 + lane];
     const double *tile = a.alm + (size_t)g * a.ncomp * nb * 32 + lane;
     const int nout = a.nLam * a.nB;
     double *out = a.partial + (size_t)g * nout;

@@ -93,11 +93,7 @@ struct ContractArgs {
     const int *term_start;      // device [nLam+1]
     const int *bin_tuples;      // device [nB][order-1]
     const double *alm;
-    const double *gweights;     // [ngroups][32]
-    const double4 *pos4;
-    const int *cell_start;
-    const int *group_start;
-    GridGeom geom;
+    const double *gweights;     // [ngroups][32] weight of the primary (group, lane), 0 for empty lanes
     double *partial;            // [ngroups_max][nout]
     double *partial2;           // [nseg][nout]
     int nseg;
@@ -133,6 +129,14 @@ cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launche
 // T: [n][n][n] E G tensor; Nraw, Rraw: [n][nB] raw multiplets; A: [nB][n][n], rhs: [nB][n] scratch; zeta: [n][nB]
 cudaError_t launch_edge_correct(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *A, double *rhs,
                                 double *zeta, cudaStream_t s);
+
+// ---- mesh.cu (gridded estimator, eq. 36) ------------------------------------------------------------------
+cudaError_t launch_mesh_alm(const double *delta, int G, double box, int lmax, int nb, const double *e2, const double *vinv,
+                            const double *ycoef_dev, void *fd, void *kern, double *alm, double *gweights, int fft_plan,
+                            cudaStream_t s, int *launches, int *fft_error);
+int mesh_fft_plan_create(int G, cudaStream_t s, int *plan_out);
+int mesh_fft_plan_set_stream(int plan, cudaStream_t s);
+void mesh_fft_plan_destroy(int plan);
 
 // ---- diag.cu --------------------------------------------------------------------------------------------
 cudaError_t launch_sum_bin_counts(const uint32_t *counts, const int *group_start, int npencil, int nbins,

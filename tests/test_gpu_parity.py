@@ -251,6 +251,36 @@ def test_edge_correction_matches_the_oracle(E, oracle, order, nbins, lmax):
         assert ei.value.status == E.EUNSUPPORTED
 
 
+@pytest.mark.parametrize("order,G,nbins,lmax,allparity", [(3, 16, 4, 5, False), (4, 12, 5, 3, False), (4, 10, 4, 2, True), (5, 10, 5, 2, False),
+                                                          (3, 9, 3, 2, False)])
+def test_gridded_estimator_matches_the_oracle(E, oracle, order, G, nbins, lmax, allparity):
+    """SURVEY.md §8(f3), eq. 36: a_lm on a periodic mesh by FFTs + the per-cell contraction against the
+    oracle's direct lattice sums.  Bin edges are chosen off the lattice distances (a distance equal to an edge to rounding
+    would be binned by (offset) h here and by the difference of rounded cell centres in the oracle)."""
+    rng = np.random.default_rng(3600 + 10 * order + G)
+    box = 60.0
+    delta = rng.standard_normal((G, G, G)) + 0.3
+    delta[rng.random((G, G, G)) < 0.3] = 0.0
+    rmin, rmax = 1.3, 0.49 * box - 0.77
+    o = oracle.zeta_grid(order, delta, box, rmin, rmax, nbins, lmax, allparity=allparity)
+    dev = torch.device("cuda:0")
+    with E.Plan(order, rmin, rmax, nbins, lmax, box, allparity=allparity) as plan:
+        z = plan.compute_grid(torch.from_numpy(delta).to(dev))
+        torch.cuda.synchronize()
+        z = z.cpu().numpy()
+        par = E.encore_get_multiplet_parity(plan.h).astype(bool)
+        z2 = plan.compute_grid(torch.from_numpy(delta).to(dev)).cpu().numpy()
+    expect = np.where(par[:, None], o["zeta_im"], o["zeta"])
+    scale = np.abs(expect).max()
+    assert scale > 0 and np.isfinite(z).all()
+    assert np.abs(z - expect).max() <= TOL * scale
+    assert np.array_equal(z, z2)
+    with E.Plan(3, 1.0, 10.0, 3, 2, 0.0) as open_plan:      # the mesh is periodic: an open-geometry plan is refused
+        with pytest.raises(E.EncoreError) as ei:
+            open_plan.compute_grid(torch.zeros((4, 4, 4), dtype=torch.float64, device=dev))
+        assert ei.value.status == E.EINVAL
+
+
 def test_degenerate_inputs(E, oracle):
     # one particle: no pairs, zeta = 0
     g = gpu_run(E, 3, np.array([[1.0], [2.0], [3.0]]), np.ones(1), 0.0, 0.0, 10.0, 3, 2)
