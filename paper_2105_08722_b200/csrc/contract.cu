@@ -359,17 +359,17 @@ struct TilePipe {
     int nbuf;
 };
 
-// Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.y, + gridDim.y, ... < g_end.  Only the l-blocks the
+// Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.x, + gridDim.x, ... < g_end (the chunk of this CTA).  Only the l-blocks the
 // CTA's multiplets need (CtaPlan) are copied: one bulk copy per block, all completing on the buffer's mbarrier.
 template <class Body>
 __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, Body body)
 {
     const int ngroups = a.g_end;
     const size_t tile = (size_t)a.ncomp * a.nbins * 32;
-    const int stride = gridDim.y;
+    const int stride = gridDim.x;
     const bool issuer = threadIdx.x == 0;
     const int rs = a.nbins * 32;
-    int g = a.g_begin + blockIdx.y;
+    int g = a.g_begin + blockIdx.x;
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
     auto load = [&](int buf, int gg) {
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bar[buf])), "r"(tp.bytes) : "memory");
@@ -435,7 +435,7 @@ __device__ __forceinline__ void warp4(const ContractArgs &a, const CtaPlan &C, c
         task4<NB, NW, W>(acc, L, toff, t + o1, t + o2, t + o3, wi);
     });
     if (!have) return;
-    double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
+    double *out = a.partial + ((size_t)blockIdx.x * a.nLam + iL) * a.nB;
     flush4<NB, NW, W>(acc, a.tuple_index, out, lane);
 }
 
@@ -454,7 +454,7 @@ __global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(Contra
 {
     constexpr int NW = nw4(NB);
     __shared__ CtaPlan C;
-    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.x)[threadIdx.x];
+    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.y)[threadIdx.x];
     __syncthreads();
     const int warp = threadIdx.x >> 5;
     const int iLs = C.lam[warp / NW];
@@ -703,7 +703,7 @@ __device__ __forceinline__ void warp5(const ContractArgs &a, const CtaPlan &C, c
         task5<NB, LO, HI, NTOT>(acc, L, toff, smem_c + t + o1, smem_c + t + o2, smem_c + t + o3, smem_c + t + o4, wi);
     });
     if (!have) return;
-    double *out = a.partial + ((size_t)blockIdx.y * a.nLam + iL) * a.nB;
+    double *out = a.partial + ((size_t)blockIdx.x * a.nLam + iL) * a.nB;
     if constexpr (LO <= HI) flush5<NB, LO, HI, NTOT>(acc, a.tuple_index, out, lane);
 }
 
@@ -720,7 +720,7 @@ __global__ void __launch_bounds__(nw5(NB) * lpc5(NB) * 32, 1) k_contract5(Contra
 {
     constexpr int NW = nw5(NB);
     __shared__ CtaPlan C;
-    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.x)[threadIdx.x];
+    if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.y)[threadIdx.x];
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int iLs = C.lam[warp / NW];
@@ -746,7 +746,9 @@ cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
     if (attr_err != cudaSuccess) return attr_err;
-    k_contract4<NB><<<dim3(a.ncta, a.nchunk), nw4(NB) * lpc4(NB) * 32, a.cta_smem, s>>>(a);
+    // x = chunk (dispatched fastest), y = CTA plan: the CTAs of the heaviest multiplets all start first and the light ones
+    // fill the tail (with the plan index on x, a heavy CTA of the last chunk started late: 8.4 against 6.1 by the cost model)
+    k_contract4<NB><<<dim3(a.nchunk, a.ncta), nw4(NB) * lpc4(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -757,7 +759,7 @@ cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
     if (attr_err != cudaSuccess) return attr_err;
-    k_contract5<NB><<<dim3(a.ncta, a.nchunk), nw5(NB) * lpc5(NB) * 32, a.cta_smem, s>>>(a);
+    k_contract5<NB><<<dim3(a.nchunk, a.ncta), nw5(NB) * lpc5(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();
 }
 
