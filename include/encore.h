@@ -138,6 +138,8 @@ int encore_get_gaunt_tensor(const encore_plan_t *plan, double *out /* HOST n_Lam
  *                      32 GiB, or half of the free device memory within 4-96 GiB when the rows need more)
  *   "sub_yz", "sub_x"  grid subdivisions S_y = S_z and S_x of reading R11 (cell size r_max / S; 0 = automatic:
  *                      S_y = clamp(round(r_max / (32 / density)^(1/3)), 1, 8), S_x = 4 S_y halved until <= 4e6 cells)
+ *   "nchunk"           chunks of primaries per multiplet group in the factorised contraction kernels (grid = nchunk x CTA
+ *                      columns; 0 = automatic)
  *   "generic_contract" 1: contract with the literal eq. 44 kernel (one warp per (Lambda, B)) instead of the
  *                      factorised kernels
  * Unknown key or value out of range: ENCORE_EINVAL. */

@@ -40,6 +40,7 @@ struct encore_plan_s {
     size_t cta_smem = 0;
     bool force_generic = false;
     bool fp32_harmonics = false;    // ENCORE_FP32_HARMONICS
+    int nchunk_override = 0;        // option "nchunk"
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
@@ -245,6 +246,7 @@ int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweig
 int choose_nchunk(const encore_plan_s *P, bool factorised)
 {
     int nchunk = 32;
+    if (P->nchunk_override > 0) return P->nchunk_override;
     if (factorised) {
         int sms = 148, dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -522,6 +524,9 @@ int encore_set_option(encore_plan_t *P, const char *key, long long value)
     } else if (k == "sub_x") {      // grid subdivision S_x; 0: 4 S_y
         if (value < 0 || value > 32) return ENCORE_EINVAL;
         P->sub_x_override = (int)value;
+    } else if (k == "nchunk") {     // chunks of groups per CTA column of the factorised contraction kernels; 0: automatic
+        if (value < 0 || value > 1024) return ENCORE_EINVAL;
+        P->nchunk_override = (int)value;
     } else if (k == "generic_contract") { // 1: run the literal eq. 44 kernel instead of the factorised ones
         if (value < 0 || value > 1) return ENCORE_EINVAL;
         P->force_generic = value != 0;

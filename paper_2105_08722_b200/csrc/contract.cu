@@ -380,17 +380,36 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
         }
     };
     if (issuer && g < ngroups) load(0, g);
+    if (tp.nbuf == 2) {
+        // two buffers: "full" barriers carry the copies, "empty" barriers (one arrival per warp) say that every warp is done
+        // with a buffer.  Only the issuing thread waits for the other warps (before it refills the buffer they used one
+        // tile ago); nobody else waits on anything but data, so the warps drift by up to one tile instead of meeting at a
+        // CTA barrier after every group.
+        unsigned long long *empty = bar + 2;
+        const int lane = threadIdx.x & 31;
+        for (int k = 0; g < ngroups; ++k, g += stride) {
+            const int st = k & 1;
+            if (issuer && g + stride < ngroups) {
+                const int use = (k + 1) >> 1;              // tile k+1 is the use-th tile of buffer st^1
+                if (use >= 1) mbar_wait(&empty[st ^ 1], (unsigned)((use - 1) & 1));
+                load(st ^ 1, g + stride);
+            }
+            mbar_wait(&bar[st], (unsigned)((k >> 1) & 1));
+            body(tp.buf[st], g);
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&empty[st])) : "memory");
+        }
+        return;
+    }
     for (int k = 0; g < ngroups; ++k, g += stride) {
-        const int st = tp.nbuf == 2 ? (k & 1) : 0;
-        if (tp.nbuf == 2 && issuer && g + stride < ngroups) load(st ^ 1, g + stride);
-        mbar_wait(&bar[st], tp.nbuf == 2 ? (unsigned)((k >> 1) & 1) : (unsigned)(k & 1));
-        body(tp.buf[st], g);
-        __syncthreads(); // every warp is done with buf[st] before it is refilled
-        if (tp.nbuf == 1 && issuer && g + stride < ngroups) load(0, g + stride);
+        mbar_wait(&bar[0], (unsigned)(k & 1));
+        body(tp.buf[0], g);
+        __syncthreads(); // every warp is done with the buffer before it is refilled
+        if (issuer && g + stride < ngroups) load(0, g + stride);
     }
 }
 
-// shared memory: [nbuf tile buffers][2 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
+// shared memory: [nbuf tile buffers][4 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
 __device__ __forceinline__ TilePipe make_pipe(const CtaPlan &C)
 {
     TilePipe tp;
@@ -403,6 +422,8 @@ __device__ __forceinline__ TilePipe make_pipe(const CtaPlan &C)
         unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
+        mbar_init(&bar[2], blockDim.x / 32);   // "empty" barriers: one arrival per warp
+        mbar_init(&bar[3], blockDim.x / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     return tp; // the caller's __syncthreads (after it has copied its term list) publishes the barriers
