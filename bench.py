@@ -43,7 +43,7 @@ import workloads as W  # noqa: E402
 SM_COUNT, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this
 # round's kernels (profiles/r2_ncu_full_c3.txt and r2_ncu_full_c5.txt name the commands); None where not captured
-NCU_DRAM_BYTES = {"c3": {"k_fill": 1.949e9, "k_harm": 2.954e9, "k_contract": 5.326e9}, "c5": {"k_contract": 0.341e9}}
+NCU_DRAM_BYTES = {"c3": {"k_fill": 1.948e9, "k_harm": 2.953e9, "k_contract": 9.622e9}, "c5": {"k_contract": 10.125e9}}
 NCU_PROFILE = "profiles/r2_ncu_full_c3.txt"
 
 
