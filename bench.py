@@ -188,7 +188,7 @@ def workload_config(cfg, world, allparity=False):
 
 
 def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allparity=False, shard=None, fp32_harmonics=False,
-                   keep_zeta=False):
+                   keep_zeta=False, want_graph=False):
     """shard = (rank, world): time sharded.compute_sharded (one catalogue, all-gather inside); None: the whole catalogue."""
     from paper_2105_08722_b200 import sharded
     pos, w = make_catalogue(cfg, rank if shard is None else 0)
@@ -231,6 +231,25 @@ def measure_config(E, torch, cfg, rank, steps, warmup, dev, want_e2e=True, allpa
            "grid": E.encore_get_grid(plan.h), "pair_steps": E.encore_get_pair_steps(plan.h)}
     if keep_zeta and shard is None:
         res["zeta"] = out.cpu().numpy()
+    if want_graph and shard is None:
+        # encore_compute_enqueue (no read-back, no allocation) captured once into a CUDA graph and replayed: the step without
+        # the two host read-backs and the launch latencies of encore_compute (same kernels, same flush between replays)
+        E.encore_set_timing(plan.h, False)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            flush.zero_()
+            plan.compute_enqueue(tp, tw, out, pos.min(axis=1), pos.max(axis=1))
+        g.replay()
+        torch.cuda.synchronize(dev)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(stream)
+        for _ in range(steps):
+            g.replay()
+        g1.record(stream)
+        torch.cuda.synchronize(dev)
+        assert E.encore_get_status(plan.h) == E.OK
+        res["graph_replay_ms"] = g0.elapsed_time(g1) / steps
+        del g
     if want_e2e:
         hp = torch.from_numpy(pos).pin_memory()
         hw = torch.from_numpy(w).pin_memory()
@@ -419,8 +438,9 @@ def main():
         per = {}
         for name in sorted(W.CONFIGS):
             c = W.CONFIGS[name]
-            r, _ = measure_config(E, torch, c, 0, 2, 3, dev, want_e2e=False)
+            r, _ = measure_config(E, torch, c, 0, 2, 3, dev, want_e2e=False, want_graph=True)
             per[name] = config_entry(c, r, 2, fp64_peak, fp32_peak)
+            per[name]["graph_replay_ms_per_step"] = r["graph_replay_ms"]   # encore_compute_enqueue replayed from a CUDA graph
         # the same c3 catalogue with the parity-odd multiplets too (111 instead of 69 multiplets)
         r, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, allparity=True)
         per["c3_allparity"] = dict(config_entry(W.CONFIGS["c3"], r, 2, fp64_peak, fp32_peak), n_multiplets=r["nout"] // 120)

@@ -50,7 +50,8 @@ enum {
     ENCORE_ECUDA = -4,    /* a CUDA call failed; encore_last_cuda_error() has the cudaError_t */
     ENCORE_ESTATE = -5,   /* diagnostic getter called before a successful encore_compute */
     ENCORE_EUNSUPPORTED = -6, /* valid problem outside what this build's kernels cover (see encore_plan) */
-    ENCORE_EINTERNAL = -7  /* a device-side consistency check failed; results must not be used (encore_get_status) */
+    ENCORE_EINTERNAL = -7, /* a device-side consistency check failed; results must not be used (encore_get_status) */
+    ENCORE_ECAPACITY = -8  /* encore_compute_enqueue: the plan's scratch, sized by its last encore_compute, is too small */
 };
 
 /* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
@@ -92,6 +93,23 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
  * Inputs are validated on the device (ENCORE_EDOMAIN is reported by this call). */
 int encore_compute(encore_plan_t *plan, const double *positions, const double *weights, int64_t n,
                    double *zeta_out, void *cuda_stream);
+
+/* Enqueue-only variant of encore_compute ("enqueues on cuda_stream and returns without synchronising"):
+ * no device->host read, no allocation, no host synchronisation, so the call can be captured into a CUDA graph and replayed
+ * on new catalogues of the same size.  It needs a previous successful encore_compute / encore_compute_host on this plan
+ * (tables uploaded, scratch and the pair stage's row reservation sized): ENCORE_ESTATE before that.
+ *   bbox_lo, bbox_hi  HOST, 3 doubles each: a box holding every particle (open geometry; ignored, may be NULL, when the
+ *                     plan is periodic).  The grid is built on THIS box (reading R11), so cell ids follow it; zeta, the
+ *                     pair counts and a_lm do not depend on it.
+ * What encore_compute decides on the host is decided on the device instead: kernels are launched for the upper bound
+ * n/32 + pencils + 1 of the group count and clamp to the count on the device; the pair stage runs as ONE step inside the
+ * plan's row reservation.  Returns ENCORE_ECAPACITY at once when a scratch array would have to grow (larger n, or a box
+ * with more cells); everything that can only be seen on the device is reported by the next encore_get_status:
+ * ENCORE_EDOMAIN (non-finite input, coordinate outside [0, box) or outside the given box), ENCORE_ECAPACITY (this
+ * catalogue needs more rows than the reservation holds: run encore_compute once, it re-sizes), ENCORE_EINTERNAL.
+ * After such a status zeta_out is unspecified.  Per-kernel timing (encore_set_timing) must be off while capturing. */
+int encore_compute_enqueue(encore_plan_t *plan, const double *positions, const double *weights, int64_t n,
+                           const double *bbox_lo, const double *bbox_hi, double *zeta_out, void *cuda_stream);
 
 /* Same, with HOST buffers: copies positions/weights to the device, computes, copies zeta back and
  * synchronises.  This is the end-to-end entry bench.py times as `e2e`. */
@@ -145,8 +163,8 @@ int encore_get_gaunt_tensor(const encore_plan_t *plan, double *out /* HOST n_Lam
  * Unknown key or value out of range: ENCORE_EINVAL. */
 int encore_set_option(encore_plan_t *plan, const char *key, long long value);
 /* Synchronises the last compute's stream and reports its device-side status: ENCORE_OK, or ENCORE_EINTERNAL if the
- * pair stage's consistency check (one periodic image per candidate word) failed.  encore_compute_host
- * returns this status itself. */
+ * pair stage's consistency check (one periodic image per candidate word) failed; after
+ * encore_compute_enqueue also ENCORE_EDOMAIN / ENCORE_ECAPACITY (see there).  encore_compute_host returns this status itself. */
 int encore_get_status(const encore_plan_t *plan);
 /* super-steps the pair stage of the last compute took: the acceptance-mask rows of a step stay under the byte budget
  * (option "list_mb"), whole groups per step, steps of equal size.  >= 1, or a status < 0. */
@@ -168,6 +186,11 @@ int encore_get_bin_edges(const encore_plan_t *plan, double *out /* HOST [nbins+1
 /* flop counts per primary of the contraction as executed (fused multiply-add = 2) and by the canonical
  * "Algorithm 3 literal" model of SURVEY.md §8(d) (5/11/17 flop per term evaluation for N=3/4/5) */
 int encore_contraction_flops(const encore_plan_t *plan, double *executed, double *canonical);
+
+/* The grid a compute would build for n particles in the box [bbox_lo, bbox_hi] (open geometry; ignored when the plan is
+ * periodic): cells per axis and subdivisions S_a of reading R11 / DESIGN.md §4.1.  Host arithmetic only, no GPU needed. */
+int encore_query_grid(const encore_plan_t *plan, int64_t n, const double *bbox_lo, const double *bbox_hi, int nc[3] /* HOST */,
+                      int sub[3] /* HOST */);
 
 /* ---- diagnostics of the last successful encore_compute (each synchronises the compute stream) ---- */
 /* grid geometry chosen for that input: cells per axis, subdivisions S_a with cell size r_max/S_a (reading R11) */

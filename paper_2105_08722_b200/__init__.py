@@ -20,11 +20,11 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
-OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL = 0, -1, -2, -3, -4, -5, -6, -7
+OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL, ECAPACITY = 0, -1, -2, -3, -4, -5, -6, -7, -8
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor", "encore_compute_grid",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_enqueue", "encore_query_grid", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor", "encore_compute_grid",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -54,6 +54,8 @@ def lib():
     L.encore_get_multiplet_parity.argtypes = [vp, ip]
     L.encore_compute.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
     L.encore_compute_host.argtypes = [vp, vp, vp, C.c_int64, vp]
+    L.encore_compute_enqueue.argtypes = [vp, vp, vp, C.c_int64, dp, dp, vp, vp]
+    L.encore_query_grid.argtypes = [vp, C.c_int64, dp, dp, ip, ip]
     L.encore_compute_shard.argtypes = [vp, vp, vp, C.c_int64, C.c_int, C.c_int, vp, vp]
     L.encore_get_shard_groups.argtypes = [vp, ip]
     L.encore_get_pair_steps.argtypes = [vp]
@@ -152,6 +154,22 @@ def encore_get_pair_steps(plan) -> int:
     if v < 0:
         _check(v)
     return int(v)
+
+
+def _d3(v):
+    return None if v is None else (C.c_double * 3)(*[float(x) for x in v])
+
+
+def encore_compute_enqueue(plan, positions, weights, n: int, bbox_lo, bbox_hi, zeta_out, cuda_stream: int = 0):
+    """positions / weights / zeta_out: CUDA tensors (or raw device pointers); bbox_lo / bbox_hi: 3 floats each or None."""
+    _check(lib().encore_compute_enqueue(plan, _ptr(positions), _ptr(weights), n, _d3(bbox_lo), _d3(bbox_hi), _ptr(zeta_out),
+                                        C.c_void_p(cuda_stream)))
+
+
+def encore_query_grid(plan, n: int, bbox_lo=None, bbox_hi=None):
+    nc, sub = (C.c_int * 3)(), (C.c_int * 3)()
+    _check(lib().encore_query_grid(plan, n, _d3(bbox_lo), _d3(bbox_hi), nc, sub))
+    return list(nc), list(sub)
 
 
 def encore_set_option(plan, key: str, value: int):
@@ -344,6 +362,19 @@ class Plan:
             out = torch.empty((self.n_lambda, self.n_b), dtype=torch.float64, device=positions.device)
         st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
         encore_compute(self.h, positions, weights, n, out, st)
+        return out
+
+    def compute_enqueue(self, positions, weights, out, bbox_lo=None, bbox_hi=None, stream=None):
+        """encore_compute_enqueue: enqueue only (no read-back, no allocation; CUDA-graph capturable).  `out` must exist."""
+        import torch
+        assert positions.is_cuda and positions.dtype == torch.float64 and positions.is_contiguous()
+        assert positions.dim() == 2 and positions.shape[0] == 3
+        n = positions.shape[1]
+        if weights is not None:
+            assert weights.is_cuda and weights.dtype == torch.float64 and weights.is_contiguous() and weights.numel() == n
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.n_lambda * self.n_b
+        st = torch.cuda.current_stream(positions.device).cuda_stream if stream is None else stream
+        encore_compute_enqueue(self.h, positions, weights, n, bbox_lo, bbox_hi, out, st)
         return out
 
     def compute_shard(self, positions, weights, shard: int, nshards: int, out=None, stream=None):

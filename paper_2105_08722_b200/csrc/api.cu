@@ -204,7 +204,7 @@ int mark(encore_plan_s *P, int kind, cudaStream_t s)
 
 // steps a5 + a6 on a_lm tiles [group][component][bin][lane] with primary weights gweights[group][lane]
 int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweights, int g_begin, int g_end, int ngmax, bool factorised,
-                        int nchunk, double *zeta_out, cudaStream_t s)
+                        int nchunk, double *zeta_out, cudaStream_t s, const int *ngroups_dev = nullptr)
 {
     const HostTables &T = P->T;
     ContractArgs ca{};
@@ -220,6 +220,7 @@ int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweig
     ca.zeta_out = zeta_out;
     ca.ngroups_max = ngmax;
     ca.g_begin = g_begin; ca.g_end = g_end;
+    ca.ngroups_dev = ngroups_dev;
     ca.pair_terms = P->d_pair_terms.as<PairTerm>();
     ca.lam4 = P->d_lam4.as<Lam4>();
     ca.lam5 = P->d_lam5.as<Lam5>();
@@ -263,27 +264,46 @@ int choose_nchunk(const encore_plan_s *P, bool factorised)
 
 // shard/nshards: the primaries are cut into nshards contiguous ranges of cell-sorted groups with equal pair-stage
 // work bounds; this call evaluates the sums over the primaries of range `shard` only (1 of 1 = everything).
+//
+// enqueue = true (encore_compute_enqueue): nothing is read back and nothing is allocated, so the call can be captured into
+// a CUDA graph.  The grid geometry comes from the caller's bounding box `ubox` (open geometry; lo[3], hi[3]), the group
+// count stays on the device (kernels are launched for the upper bound ngmax and clamp), the row reservation of the
+// plan is used as it is (k_fill flags a group whose rows would not fit), validation flags travel with the status word.
 int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t n, double *zeta_out, cudaStream_t s,
-                   int shard = 0, int nshards = 1)
+                   int shard = 0, int nshards = 1, const double *ubox = nullptr, bool enqueue = false)
 {
     const HostTables &T = P->T;
     P->have = false;
     P->launches = 0;
+    if (enqueue && !P->uploaded) return ENCORE_ESTATE;
     TRY(upload_tables(P, s));
+// scratch: grown on demand, or (enqueue) only checked against what the plan already owns
+#define ENS(buf, bytes)                                                      \
+    do {                                                                     \
+        if (enqueue) { if ((size_t)(bytes) > (buf).cap) return ENCORE_ECAPACITY; } \
+        else CU((buf).ensure(bytes));                                        \
+    } while (0)
 
     // ---- validation + bounding box (one small device->host read) ------------------------------------------
-    CU(P->bbox_tmp.ensure(sizeof(double) * 6 * 592));
-    CU(P->bbox.ensure(sizeof(double) * 8));
-    CU(P->flags.ensure(sizeof(int) * 2));
+    ENS(P->bbox_tmp, sizeof(double) * 6 * 592);
+    ENS(P->bbox, sizeof(double) * 8);
+    ENS(P->flags, sizeof(int) * 2);
     CU(launch_bbox_validate(pos, w, n, T.box, P->bbox_tmp.as<double>(), P->bbox.as<double>(), P->flags.as<int>(), s, &P->launches));
-    CU(cudaMemcpyAsync(P->pinned, P->bbox.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, s));
-    CU(cudaMemcpyAsync(P->pinned + 6, P->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
-    CU(cudaStreamSynchronize(s));
-    int fl[2];
-    std::memcpy(fl, P->pinned + 6, sizeof(fl));
-    if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
+    double bb[6] = {0, 0, 0, 0, 0, 0};  // bounding box the grid is built on (open geometry)
+    if (!enqueue) {
+        CU(cudaMemcpyAsync(P->pinned, P->bbox.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(P->pinned + 6, P->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        int fl[2];
+        std::memcpy(fl, P->pinned + 6, sizeof(fl));
+        if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
+        std::memcpy(bb, P->pinned, sizeof(bb));
+    } else if (!(T.box > 0.0)) {
+        std::memcpy(bb, ubox, sizeof(bb));
+        CU(launch_bbox_check(P->bbox.as<double>(), bb, bb + 3, P->flags.as<int>(), s, &P->launches));
+    }
     GridGeom G;
-    if (!choose_geometry(P, n, P->pinned, P->pinned + 3, G)) return ENCORE_EUNSUPPORTED;
+    if (!choose_geometry(P, n, bb, bb + 3, G)) return ENCORE_EUNSUPPORTED;
     int nr_cap;
     {
         // inv <= sub / r_max (choose_geometry), so these are at most sub + 1 cells
@@ -295,29 +315,30 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         if (pair_fill_smem_bytes(T.nbins, nr_cap) > 200 * 1024) return ENCORE_EUNSUPPORTED;
     }
     const int ngmax = (int)(n / ENCORE_GROUP) + G.npencil + 1;
+    if (ngmax > 2048 * 2048) return ENCORE_EUNSUPPORTED;   // (the three-kernel scan of the per-group word counts)
     const int nb = T.nbins, ncomp = T.ncomp;
     const size_t nout = (size_t)T.nLam() * T.nB();
     const int nseg = 64;   // (contract_and_reduce uses the same count)
 
     // ---- scratch ----------------------------------------------------------------------------------------------
-    CU(P->cid.ensure(sizeof(int32_t) * n));
-    CU(P->cell_count.ensure(sizeof(int) * (size_t)G.ncell));
-    CU(P->cell_fill.ensure(sizeof(int) * (size_t)G.ncell));
-    CU(P->cell_start.ensure(sizeof(int) * ((size_t)G.ncell + 1)));
-    CU(P->scan_tmp.ensure(sizeof(int) * (std::max<size_t>(std::max<size_t>((size_t)G.ncell, (size_t)ngmax), 4000000) / 2048 + 8)));
-    CU(P->tmp_idx.ensure(sizeof(int) * n));
-    CU(P->sorted_idx.ensure(sizeof(int) * n));
-    CU(P->pos4.ensure(sizeof(double4) * ((size_t)n + 1)));   // + the padding particle
-    CU(P->groups.ensure(sizeof(int) * (size_t)G.npencil));
-    CU(P->group_start.ensure(sizeof(int) * ((size_t)G.npencil + 1)));
-    CU(P->alm.ensure(sizeof(double) * (size_t)ngmax * ncomp * nb * 32));
-    CU(P->counts.ensure(sizeof(uint32_t) * (size_t)ngmax * nb * 32));
+    ENS(P->cid, sizeof(int32_t) * n);
+    ENS(P->cell_count, sizeof(int) * (size_t)G.ncell);
+    ENS(P->cell_fill, sizeof(int) * (size_t)G.ncell);
+    ENS(P->cell_start, sizeof(int) * ((size_t)G.ncell + 1));
+    ENS(P->scan_tmp, sizeof(int) * (std::max<size_t>(std::max<size_t>((size_t)G.ncell, (size_t)ngmax), 4000000) / 2048 + 8));
+    ENS(P->tmp_idx, sizeof(int) * n);
+    ENS(P->sorted_idx, sizeof(int) * n);
+    ENS(P->pos4, sizeof(double4) * ((size_t)n + 1));   // + the padding particle
+    ENS(P->groups, sizeof(int) * (size_t)G.npencil);
+    ENS(P->group_start, sizeof(int) * ((size_t)G.npencil + 1));
+    ENS(P->alm, sizeof(double) * (size_t)ngmax * ncomp * nb * 32);
+    ENS(P->counts, sizeof(uint32_t) * (size_t)ngmax * nb * 32);
     const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax) && (T.order == 3 || P->cta_smem > 0);
     const int nchunk = choose_nchunk(P, factorised);
-    CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout));
-    CU(P->gweights.ensure(sizeof(double) * (size_t)ngmax * 32));
-    CU(P->partial2.ensure(sizeof(double) * (size_t)nseg * nout));
-    CU(P->cand.ensure(3 * sizeof(unsigned long long)));   // candidate pairs, k_harm steps, k_harm ideal steps
+    ENS(P->partial, sizeof(double) * (size_t)(factorised ? nchunk : ngmax) * nout);
+    ENS(P->gweights, sizeof(double) * (size_t)ngmax * 32);
+    ENS(P->partial2, sizeof(double) * (size_t)nseg * nout);
+    ENS(P->cand, 3 * sizeof(unsigned long long));   // candidate pairs, k_harm steps, k_harm ideal steps
 
     TRY(mark(P, K_START, s));
     // ---- a1: cell ids + histogram -----------------------------------------------------------------------------
@@ -340,17 +361,15 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         for (int a = 0; a < 3; ++a) {
             if (G.periodic) { far[a] = 3.0 * T.box; r2 += 9.0 * T.box * T.box; }
             else {
-                const double ext = P->pinned[3 + a] - P->pinned[a];
-                const double emax = std::max(std::max(P->pinned[3] - P->pinned[0], P->pinned[4] - P->pinned[1]), P->pinned[5] - P->pinned[2]);
+                const double ext = bb[3 + a] - bb[a];
+                const double emax = std::max(std::max(bb[3] - bb[0], bb[4] - bb[1]), bb[5] - bb[2]);
                 const double off = 2.0 * (emax + T.rmax);
-                far[a] = P->pinned[3 + a] + off;
+                far[a] = bb[3 + a] + off;
                 r2 += (ext + off) * (ext + off);
             }
         }
-        // (the bounding box in pinned[0..5] was read above; the slots 8..11 are only written here, after that synchronise)
-        P->pinned[8] = far[0]; P->pinned[9] = far[1]; P->pinned[10] = far[2]; P->pinned[11] = 0.0;
         pa.pad_r2max = r2;
-        CU(cudaMemcpyAsync(P->pos4.as<double4>() + n, P->pinned + 8, sizeof(double4), cudaMemcpyHostToDevice, s));
+        CU(launch_set_particle(P->pos4.as<double4>() + n, far[0], far[1], far[2], 0.0, s, &P->launches));
     }
     pa.cell_start = P->cell_start.as<int>();
     pa.group_start = P->group_start.as<int>();
@@ -372,18 +391,18 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     pa.cand_pairs = P->cand.as<unsigned long long>();
     pa.gweights = P->gweights.as<double>();
     pa.ngroups = ngmax;
-    CU(P->gbound.ensure(sizeof(int) * (size_t)ngmax));
-    CU(P->gprefix.ensure(sizeof(int) * ((size_t)ngmax + 2)));
-    CU(P->gwide.ensure(sizeof(int) * (size_t)ngmax));
-    CU(P->rowcnt.ensure(sizeof(int) * (size_t)ngmax * nb));
-    CU(P->errflag.ensure(sizeof(int)));
+    ENS(P->gbound, sizeof(int) * (size_t)ngmax);
+    ENS(P->gprefix, sizeof(int) * ((size_t)ngmax + 2));
+    ENS(P->gwide, sizeof(int) * (size_t)ngmax);
+    ENS(P->rowcnt, sizeof(int) * (size_t)ngmax * nb);
+    ENS(P->errflag, sizeof(int));
     pa.gbound = P->gbound.as<int>();
     pa.gprefix = P->gprefix.as<int>();
     pa.gwide = P->gwide.as<int>();
     pa.scan_tmp = P->scan_tmp.as<int>();
     pa.rowcnt = P->rowcnt.as<int>();
     pa.err_flag = P->errflag.as<int>();
-    if (P->h_gprefix_cap < (size_t)ngmax + 2) {
+    if (!enqueue && P->h_gprefix_cap < (size_t)ngmax + 2) {
         if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
         P->h_gprefix = nullptr; P->h_gprefix_cap = 0;
         CU(cudaMallocHost((void **)&P->h_gprefix, sizeof(int) * ((size_t)ngmax + 2)));
@@ -393,6 +412,21 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     CU(cudaMemsetAsync(P->cand.p, 0, 3 * sizeof(unsigned long long), s));
     CU(cudaMemsetAsync(P->errflag.p, 0, sizeof(int), s));
     CU(launch_pair_bounds(pa, s, &P->launches));
+    if (enqueue) {
+        // no read-back: one step over the upper bound of the group count with the rows the plan already owns
+        const size_t cap_words = std::min(P->rows.cap / ((size_t)nb * 32 * sizeof(unsigned)), P->rowdesc.cap / ((size_t)nb * sizeof(unsigned)));
+        if (cap_words == 0) return ENCORE_ECAPACITY;
+        TRY(mark(P, K_BOUNDS, s));
+        pa.rows = P->rows.as<unsigned>();
+        pa.rowdesc = P->rowdesc.as<unsigned>();
+        pa.rows_cap_words = cap_words;
+        g_begin = 0; g_end = ngmax; ngroups_total = ngmax;
+        P->pair_steps = 1;
+        CU(launch_pair_fill(pa, 0, ngmax, nr_cap, s, &P->launches));
+        TRY(mark(P, K_FILL, s));
+        CU(launch_pair_harmonics(pa, 0, ngmax, s, &P->launches));
+        TRY(mark(P, K_HARM, s));
+    } else {
     // second small device->host read: candidate words per group (prefix) and the number of groups -> super-steps
     CU(cudaMemcpyAsync(P->h_gprefix, P->gprefix.p, sizeof(int) * ((size_t)ngmax + 1), cudaMemcpyDeviceToHost, s));
     CU(cudaMemcpyAsync(P->h_gprefix + ngmax + 1, P->group_start.as<int>() + G.npencil, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -419,8 +453,13 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         size_t max_group_words = 0;
         for (int g = 0; g < ngroups; ++g) max_group_words = std::max(max_group_words, (size_t)(gp[g + 1] - gp[g]));
         const size_t cap_words = std::max(std::min(total_words, budget_words), std::max<size_t>(max_group_words, 1));
-        CU(P->rows.ensure(cap_words * nb * 32 * sizeof(unsigned)));
-        CU(P->rowdesc.ensure(cap_words * nb * sizeof(unsigned)));
+        // reserved: an eighth more than this catalogue needs when the budget allows, so that encore_compute_enqueue can
+        // replay the plan on other catalogues of the same size and clustering (a reservation is never shrunk)
+        const size_t reserve_words = std::max(cap_words, std::min(budget_words, total_words + total_words / 8));
+        if (P->rows.cap < cap_words * nb * 32 * sizeof(unsigned) || P->rowdesc.cap < cap_words * nb * sizeof(unsigned)) {
+            CU(P->rows.ensure(reserve_words * nb * 32 * sizeof(unsigned)));
+            CU(P->rowdesc.ensure(reserve_words * nb * sizeof(unsigned)));
+        }
         pa.rows = P->rows.as<unsigned>();
         pa.rowdesc = P->rowdesc.as<unsigned>();
         pa.ngroups = ngroups;
@@ -451,10 +490,14 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
             g0 = g1;
         }
     }
+    }
+    if (enqueue) CU(cudaMemcpyAsync(P->pinned + 6, P->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, s)); // validation flags
     // internal-consistency flag of the pair stage, read by whoever synchronises next (encore_get_status, the getters)
     CU(cudaMemcpyAsync(reinterpret_cast<int *>(P->pinned + 7), P->errflag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
     // ---- a5: contraction, a6: reduction ------------------------------------------------------------------------
-    TRY(contract_and_reduce(P, pa.alm, pa.gweights, g_begin, g_end, ngmax, factorised, nchunk, zeta_out, s));
+    TRY(contract_and_reduce(P, pa.alm, pa.gweights, g_begin, g_end, ngmax, factorised, nchunk, zeta_out, s,
+                            enqueue ? P->group_start.as<int>() + G.npencil : nullptr));
+#undef ENS
 
     P->have = true; P->n = n; P->geom = G; P->ngroups_max = ngmax; P->stream = s;
     P->g_begin = g_begin; P->g_end = g_end; P->ngroups = ngroups_total;
@@ -510,6 +553,35 @@ int encore_compute_shard(encore_plan_t *P, const double *positions, const double
     return compute_device(P, positions, weights, n, zeta_partial_out, static_cast<cudaStream_t>(cuda_stream), shard, nshards);
 }
 
+int encore_compute_enqueue(encore_plan_t *P, const double *positions, const double *weights, int64_t n, const double *bbox_lo,
+                           const double *bbox_hi, double *zeta_out, void *cuda_stream)
+{
+    if (!P || !positions || !zeta_out || n < 1 || n >= (int64_t(1) << 26)) return ENCORE_EINVAL;
+    double ub[6] = {0, 0, 0, 0, 0, 0};
+    if (!(P->T.box > 0.0)) {
+        if (!bbox_lo || !bbox_hi) return ENCORE_EINVAL;
+        for (int a = 0; a < 3; ++a) {
+            if (!std::isfinite(bbox_lo[a]) || !std::isfinite(bbox_hi[a]) || bbox_hi[a] < bbox_lo[a]) return ENCORE_EINVAL;
+            ub[a] = bbox_lo[a]; ub[3 + a] = bbox_hi[a];
+        }
+    }
+    return compute_device(P, positions, weights, n, zeta_out, static_cast<cudaStream_t>(cuda_stream), 0, 1, ub, true);
+}
+
+int encore_query_grid(const encore_plan_t *P, int64_t n, const double *bbox_lo, const double *bbox_hi, int nc[3], int sub[3])
+{
+    if (!P || !nc || !sub || n < 1) return ENCORE_EINVAL;
+    double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    if (!(P->T.box > 0.0)) {
+        if (!bbox_lo || !bbox_hi) return ENCORE_EINVAL;
+        for (int a = 0; a < 3; ++a) { lo[a] = bbox_lo[a]; hi[a] = bbox_hi[a]; }
+    }
+    GridGeom G;
+    if (!choose_geometry(P, n, lo, hi, G)) return ENCORE_EUNSUPPORTED;
+    for (int a = 0; a < 3; ++a) { nc[a] = G.nc[a]; sub[a] = G.sub[a]; }
+    return ENCORE_OK;
+}
+
 int encore_set_option(encore_plan_t *P, const char *key, long long value)
 {
     if (!P || !key) return ENCORE_EINVAL;
@@ -539,8 +611,11 @@ int encore_get_status(const encore_plan_t *P)
     if (!P) return ENCORE_EINVAL;
     if (!P->have) return ENCORE_ESTATE;
     CU(cudaStreamSynchronize(P->stream));
-    int f = 0;
+    int f = 0, fl[2];
     std::memcpy(&f, P->pinned + 7, sizeof(int));
+    std::memcpy(fl, P->pinned + 6, sizeof(fl));   // validation flags (encore_compute reports them itself; encore_compute_enqueue cannot)
+    if (fl[0] || fl[1]) return ENCORE_EDOMAIN;
+    if (f & 2) return ENCORE_ECAPACITY;
     return f ? ENCORE_EINTERNAL : ENCORE_OK;
 }
 
@@ -908,6 +983,7 @@ const char *encore_strerror(int status)
     case ENCORE_ESTATE: return "no successful encore_compute to report on (or timing disabled)";
     case ENCORE_EUNSUPPORTED: return "configuration not covered by this build's kernels";
     case ENCORE_EINTERNAL: return "internal consistency check of the pair stage failed (please report)";
+    case ENCORE_ECAPACITY: return "encore_compute_enqueue: the plan's scratch (sized by its last encore_compute) is too small for this input";
     default: return "unknown status";
     }
 }

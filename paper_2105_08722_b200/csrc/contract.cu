@@ -20,11 +20,17 @@ namespace {
 constexpr int kWarps = 8;
 constexpr unsigned kFull = 0xffffffffu;
 
+// one past the last group of this call: a.g_end, or (encore_compute_enqueue) the device-side group count it bounds
+__device__ __forceinline__ int group_end(const ContractArgs &a)
+{
+    return a.ngroups_dev ? min(a.g_end, *a.ngroups_dev) : a.g_end;
+}
+
 // Generic kernel, any N in {3,..,6}: one warp per output (Lam,B), terms looped (literal eq. 44), complex products in registers.
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
     const int g = a.g_begin + blockIdx.x;
-    if (g >= a.g_end) return;
+    if (g >= group_end(a)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nb = a.nbins, nm = a.order - 1;
     const double wi = a.gweights[(size_t)g * 32 + lane];
@@ -65,7 +71,7 @@ __global__ void k_reduce_groups(ContractArgs a)
     const int o = blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= nout) return;
     // rows of `partial`: one per chunk (factorised kernels) or one per group of this call's range
-    const int r0 = a.factorised ? 0 : a.g_begin, r1 = a.factorised ? a.nchunk : a.g_end;
+    const int r0 = a.factorised ? 0 : a.g_begin, r1 = a.factorised ? a.nchunk : group_end(a);
     const int s = blockIdx.y;
     const int per = (r1 - r0 + a.nseg - 1) / a.nseg;
     const int g0 = r0 + s * per, g1 = min(r1, g0 + per);
@@ -119,7 +125,8 @@ __global__ void __launch_bounds__(128) k_contract3(ContractArgs a)
     double acc[NP];
 #pragma unroll
     for (int p = 0; p < NP; ++p) acc[p] = 0.0;
-    for (int g = a.g_begin + chunk * 4 + warp; g < a.g_end; g += 4 * (int)gridDim.y) {
+    const int g_end = group_end(a);
+    for (int g = a.g_begin + chunk * 4 + warp; g < g_end; g += 4 * (int)gridDim.y) {
         const double wi = a.gweights[(size_t)g * 32 + lane];
         const double *tile = a.alm + ((size_t)g * a.ncomp + (size_t)l * l) * NB * 32 + lane;
         for (int c = 0; c <= 2 * l; ++c) {
@@ -364,7 +371,7 @@ struct TilePipe {
 template <class Body>
 __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, Body body)
 {
-    const int ngroups = a.g_end;
+    const int ngroups = group_end(a);
     const size_t tile = (size_t)a.ncomp * a.nbins * 32;
     const int stride = gridDim.x;
     const bool issuer = threadIdx.x == 0;

@@ -37,6 +37,8 @@ struct BinTable {       // passed by value (kernel parameter space -> constant b
 // periodic coordinate is outside [0, box)
 cudaError_t launch_bbox_validate(const double *pos, const double *w, int64_t n, double box, double *bbox_tmp,
                                  double *bbox_out, int *flags, cudaStream_t s, int *launches);
+cudaError_t launch_set_particle(double4 *dst, double x, double y, double z, double w, cudaStream_t s, int *launches);
+cudaError_t launch_bbox_check(const double *bbox_dev, const double lo[3], const double hi[3], int *flags, cudaStream_t s, int *launches);
 cudaError_t launch_cell_ids(const double *pos, int64_t n, GridGeom g, int32_t *cid, int *cell_count,
                             cudaStream_t s, int *launches);
 // exclusive scan of `in[0..m)` into `out[0..m]` (out[m] = total); tmp needs (m/2048+2) ints; m <= 2048*2048
@@ -75,7 +77,9 @@ struct PairArgs {
     unsigned *rows;             // [(gprefix[g]-gprefix[g0]) * nbins + bin * words(g) + k][32] masks, lane = primary
     unsigned *rowdesc;          // same index: first sorted index of the word | image codes << 26
     int *rowcnt;                // [ngroups][nbins] rows written
-    int *err_flag;              // set if a word's candidates disagreed on the periodic image (excluded by DESIGN.md §5.3)
+    int *err_flag;              // bit 0: a word's candidates disagreed on the periodic image (excluded by DESIGN.md §5.3);
+                                // bit 1: the row reservation is too small for this input (encore_compute_enqueue only)
+    size_t rows_cap_words;      // candidate words the row buffers hold; 0: sized from the word counts on the host (not checked)
     int bin_order[ENCORE_MAX_BINS]; // bins by decreasing shell volume (work per item)
 };
 // per-group word counts -> gbound, gprefix, gwide (device).  The caller reads gprefix back, sizes the row buffer, and
@@ -101,6 +105,7 @@ struct ContractArgs {
     double *zeta_out;
     int ngroups_max;
     int g_begin, g_end;         // groups of this call (all of them, or one shard's contiguous range)
+    const int *ngroups_dev;     // encore_compute_enqueue: the group count lives on the device and g_end is an upper bound; else NULL
     // factorised kernels (N = 4, 5)
     const PairTerm *pair_terms; // device
     const Lam4 *lam4;           // device [nLam]

@@ -64,7 +64,8 @@ __global__ void k_bbox_final(const double *__restrict__ part, int nblocks, doubl
 __device__ __forceinline__ int cell_coord(double x, double org, double inv, int nc)
 {
     int v = (int)((x - org) * inv);
-    return v > nc - 1 ? nc - 1 : v;
+    v = v > nc - 1 ? nc - 1 : v;
+    return v < 0 ? 0 : v;       // only below a caller-supplied bounding box (encore_compute_enqueue; flagged as a domain error)
 }
 
 __global__ void k_cell_ids(const double *__restrict__ pos, int64_t n, GridGeom g, int32_t *__restrict__ cid,
@@ -185,7 +186,36 @@ __global__ void k_pencil_groups(const int *__restrict__ cell_start, GridGeom g, 
     groups[p] = (cnt + ENCORE_GROUP - 1) / ENCORE_GROUP;
 }
 
+// encore_compute_enqueue: the caller's bounding box must hold every particle (flags[1] otherwise)
+__global__ void k_bbox_check(const double *__restrict__ bbox, double lx, double ly, double lz, double hx, double hy, double hz,
+                             int *__restrict__ flags)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const bool ok = bbox[0] >= lx && bbox[1] >= ly && bbox[2] >= lz && bbox[3] <= hx && bbox[4] <= hy && bbox[5] <= hz;
+        if (!ok) flags[1] = 1;
+    }
+}
+
+__global__ void k_set_particle(double4 *dst, double x, double y, double z, double w)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) *dst = make_double4(x, y, z, w);
+}
+
 } // namespace
+
+cudaError_t launch_set_particle(double4 *dst, double x, double y, double z, double w, cudaStream_t s, int *launches)
+{
+    k_set_particle<<<1, 32, 0, s>>>(dst, x, y, z, w);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bbox_check(const double *bbox_dev, const double lo[3], const double hi[3], int *flags, cudaStream_t s, int *launches)
+{
+    k_bbox_check<<<1, 32, 0, s>>>(bbox_dev, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], flags);
+    *launches += 1;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_bbox_validate(const double *pos, const double *w, int64_t n, double box, double *bbox_tmp,
                                  double *bbox_out, int *flags, cudaStream_t s, int *launches)

@@ -69,7 +69,8 @@ __host__ __device__ constexpr int ncomp_range(int lmax, int mlo, int mhi)
 __device__ __forceinline__ int cell_coord(double x, double org, double inv, int nc)
 {
     int v = (int)((x - org) * inv);
-    return v > nc - 1 ? nc - 1 : v;
+    v = v > nc - 1 ? nc - 1 : v;
+    return v < 0 ? 0 : v;
 }
 
 // acc[] order: m ascending, k ascending, (re, im): S_{m,k} = sum w z^k (x+iy)^m, k = 0..LMAX-m.
@@ -311,6 +312,12 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     int *rng_len = rng_start + nr_cap;
     int *rng_woff = rng_len + nr_cap;
 
+    if (a.rows_cap_words && (size_t)(a.gprefix[g + 1] - a.gprefix[g0]) > a.rows_cap_words) {
+        // encore_compute_enqueue: the rows of this group would not fit the reservation of the last encore_compute
+        if (lane < nb) a.rowcnt[(size_t)g * nb + lane] = 0;
+        if (lane == 0) atomicOr(a.err_flag, 2);
+        return;
+    }
     const Group gr = locate_group<PERIODIC>(a, g);
     const int first = gr.first, cnt = gr.cnt;
     const double4 ctr = a.pos4[first];
@@ -412,7 +419,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
         if (km == 0u) continue;         // no candidate of the word is within reach of the group
         const unsigned wcode = __shfl_sync(kFull, code, 0); // lane 0 of a word is always a candidate
         if (PERIODIC && fast && __any_sync(kFull, keep && code != wcode)) { // excluded by DESIGN.md §5.3
-            if (lane == 0) *a.err_flag = 1;
+            if (lane == 0) atomicOr(a.err_flag, 1);
         }
         // survivors compacted to the front of cand[], two per 32-byte slot as {x0,x1,y0,y1 | z0,z1,pos0,pos1} (pos =
         // position in the word) so that a pair of candidates feeds the packed fp32x2 instructions of sm_100; padded
@@ -751,6 +758,7 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     const int item = blockIdx.x * kHarmWarps + warp;
     if (item >= ng * nb) return;
     const int bin = a.bin_order[item / ng], g = g0 + item % ng;
+    if (g >= a.group_start[a.geom.npencil]) return;    // (g1 is an upper bound when the group count was not read back)
     const Group gr = locate_group<PERIODIC>(a, g);
     const bool active = lane < gr.cnt;
     const double4 me = a.pos4[gr.first + (active ? lane : 0)];

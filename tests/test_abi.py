@@ -2,6 +2,7 @@
 arguments, and its host-built plan tables agree with the paper's printed counts and with the oracle's
 enumeration.  No compute call is made here (no GPU)."""
 import ctypes as C
+import math
 import os
 import re
 import subprocess
@@ -153,3 +154,50 @@ def test_gaunt_tensor_equals_the_oracle_definition(oracle, order, lmax, allparit
     lib.encore_get_gaunt_tensor.restype = C.c_int
     with E.Plan(6, 1.0, 20.0, 6, 1, 0.0) as p6:
         assert lib.encore_get_gaunt_tensor(p6.h, (C.c_double * 1)()) == E.EUNSUPPORTED
+
+
+def _grid_rule(n, ext, rmax):
+    """S_y = S_z = clamp(round(r_max / (32 / rho)^(1/3)), 1, 8), rho = n / prod max(ext_a, r_max); S_x = 4 S_y,
+    halved until nc_x nc_y nc_z <= 4e6; nc_a = max(1, floor(ext_a / (r_max / S_a)))."""
+    rho = n / np.prod([max(e, rmax) for e in ext])
+    syz = int(min(8, max(1, math.floor(rmax / (32.0 / rho) ** (1.0 / 3.0) + 0.5))))
+    sx = 4 * syz
+    while True:
+        sub = [sx, syz, syz]
+        nc = [max(1, int(math.floor(e / (rmax / s)))) for e, s in zip(ext, sub)]
+        if nc[0] * nc[1] * nc[2] <= 4.0e6 or sx == 1:
+            return (nc, sub) if nc[0] * nc[1] * nc[2] <= 4.0e6 else None
+        sx = max(1, sx // 2)
+
+
+@pytest.mark.parametrize("n,box,lo,hi,rmax", [
+    (2000, 1000.0, None, None, 200.0),                       # c1
+    (200000, 1000.0, None, None, 200.0),                     # c2
+    (300000, 1000.0, None, None, 160.0),                     # c3, c5
+    (1600000, 0.0, (1039.2, -900.0, -900.0), (1800.0, 900.0, 900.0), 160.0),   # c4's footprint
+    (500, 0.0, (0.0, 0.0, 5.0 - 1e-12), (80.0, 80.0, 5.0 + 1e-12), 30.0),      # an axis thinner than a cell
+    (40, 0.0, (1.0, 2.0, 3.0), (1.0, 2.0, 3.0), 10.0),                        # all points coincide
+    (3000000, 3000.0, None, None, 25.0),                     # S_x has to be halved
+])
+def test_query_grid_follows_the_rule_of_design_4_1(n, box, lo, hi, rmax):
+    """ADVICE/VERDICT r1: nothing checked that the subdivisions the library reports follow the stated rule (host only)."""
+    plan = E.encore_plan(3, 0.0, rmax, 3, 1, box)
+    ext = [box] * 3 if box > 0 else [h - l for l, h in zip(lo, hi)]
+    want = _grid_rule(n, ext, rmax)
+    assert want is not None
+    nc, sub = E.encore_query_grid(plan, n, lo, hi)
+    assert (nc, sub) == want
+    E.encore_destroy(plan)
+
+
+def test_query_grid_errors():
+    plan = E.encore_plan(3, 0.0, 20.0, 3, 1, 0.0)
+    with pytest.raises(E.EncoreError) as ei:
+        E.encore_query_grid(plan, 100, None, None)           # open geometry needs the box
+    assert ei.value.status == E.EINVAL
+    E.encore_destroy(plan)
+    plan = E.encore_plan(3, 0.0, 20.0, 3, 1, 20000.0)        # box / r_max = 1000: beyond the cell tables even at S = 1
+    with pytest.raises(E.EncoreError) as ei:
+        E.encore_query_grid(plan, 1000000000 // 16, None, None)
+    assert ei.value.status == E.EUNSUPPORTED
+    E.encore_destroy(plan)

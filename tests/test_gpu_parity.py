@@ -621,3 +621,116 @@ def test_options_and_thin_axis(E, oracle):
             counts, _ = E.encore_get_bin_counts(plan.h, cfg.nbins)
         assert (counts == o["bin_counts"]).all()
         assert np.abs(z - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+
+
+def test_enqueue_variant_matches_compute(E, oracle):
+    """encore_compute_enqueue (no read-back, no allocation) gives the bits of encore_compute when the grid
+    is the same, the oracle's zeta and counts when the caller's box is larger, and reports what only the device can see
+    (domain errors, a row reservation that is too small) through encore_get_status."""
+    dev = torch.device("cuda:0")
+    for name, kw in [("c3", dict(box=360.0, n=6000, grid=64)), ("c4", dict(n=6000, grid=64)), ("c5", dict(box=330.0, n=3000, grid=32))]:
+        cfg = W.scaled(W.CONFIGS[name], **kw)
+        pos, w = W.make(cfg)
+        tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+        o = oracle.zeta(cfg.order, pos, w, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+        scale = np.abs(o["zeta"]).max()
+        with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+            out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+            with pytest.raises(E.EncoreError) as ei:             # nothing sized yet
+                plan.compute_enqueue(tp, tw, out, pos.min(axis=1), pos.max(axis=1))
+            assert ei.value.status == E.ESTATE
+            z0 = plan.compute(tp, tw).cpu().numpy()
+            assert E.encore_get_status(plan.h) == E.OK
+            lo, hi = pos.min(axis=1), pos.max(axis=1)
+            out.zero_()
+            plan.compute_enqueue(tp, tw, out, lo, hi)
+            assert E.encore_get_status(plan.h) == E.OK
+            assert out.cpu().numpy().tobytes() == z0.tobytes()   # same grid, same order of every sum
+            counts, _ = E.encore_get_bin_counts(plan.h, cfg.nbins)
+            assert (counts == o["bin_counts"]).all()
+            if cfg.box == 0.0:
+                # a larger box (fewer or as many cells per axis would need no new scratch; more cells may: accept ECAPACITY)
+                pad = 0.01 * (hi - lo)
+                out.zero_()
+                try:
+                    plan.compute_enqueue(tp, tw, out, lo - pad, hi + pad)
+                    assert E.encore_get_status(plan.h) == E.OK
+                    assert np.abs(out.cpu().numpy() - o["zeta"]).max() <= TOL * scale
+                    counts, _ = E.encore_get_bin_counts(plan.h, cfg.nbins)
+                    assert (counts == o["bin_counts"]).all()
+                except E.EncoreError as e:
+                    assert e.status == E.ECAPACITY
+                # a particle outside the caller's box: flagged, not a crash
+                bad_hi = hi.copy()
+                bad_hi[1] = 0.5 * (lo[1] + hi[1])
+                plan.compute_enqueue(tp, tw, out, lo, bad_hi)
+                assert E.encore_get_status(plan.h) == E.EDOMAIN
+                with pytest.raises(E.EncoreError) as ei:
+                    plan.compute_enqueue(tp, tw, out, None, None)
+                assert ei.value.status == E.EINVAL
+            # a non-finite coordinate
+            tq = tp.clone()
+            tq[1, 17] = float("nan")
+            plan.compute_enqueue(tq, tw, out, lo, hi)
+            assert E.encore_get_status(plan.h) == E.EDOMAIN
+            # and the plan still works
+            plan.compute_enqueue(tp, tw, out, lo, hi)
+            assert E.encore_get_status(plan.h) == E.OK
+            assert out.cpu().numpy().tobytes() == z0.tobytes()
+            # more particles than the scratch was sized for
+            big = torch.cat([tp, tp + 0.25], dim=1).contiguous() if cfg.box == 0.0 else torch.cat([tp, (tp + 0.25) % cfg.box], dim=1).contiguous()
+            with pytest.raises(E.EncoreError) as ei:
+                plan.compute_enqueue(big, None, out, lo, hi + 0.25)
+            assert ei.value.status == E.ECAPACITY
+
+
+def test_enqueue_row_reservation_overflow_is_reported(E, oracle):
+    """a catalogue of the same size but far denser needs more acceptance-mask rows than the plan reserved: status
+    ENCORE_ECAPACITY from the device, and one encore_compute re-sizes the plan"""
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(5)
+    n, box = 6000, 300.0
+    a = np.ascontiguousarray(rng.uniform(0, box, (3, n)))
+    b = np.ascontiguousarray(rng.uniform(0, box / 3, (3, n)))        # 27 times the density
+    ta, tb = torch.from_numpy(a).to(dev), torch.from_numpy(b).to(dev)
+    with E.Plan(3, 5.0, 60.0, 4, 2, box) as plan:
+        out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+        plan.compute(ta, None)
+        plan.compute_enqueue(tb, None, out)
+        assert E.encore_get_status(plan.h) == E.ECAPACITY
+        zb = plan.compute(tb, None).cpu().numpy()
+        assert E.encore_get_status(plan.h) == E.OK
+        plan.compute_enqueue(tb, None, out)
+        assert E.encore_get_status(plan.h) == E.OK
+        assert out.cpu().numpy().tobytes() == zb.tobytes()
+        o = oracle.zeta(3, b, np.ones(n), box, 5.0, 60.0, 4, 2)
+        assert np.abs(zb - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+
+
+def test_enqueue_variant_in_a_cuda_graph(E, oracle):
+    """capture one encore_compute_enqueue into a CUDA graph, replay it on a second catalogue of the same size written into
+    the same buffers: the oracle's zeta for that catalogue"""
+    dev = torch.device("cuda:0")
+    cfg = W.scaled(W.CONFIGS["c3"], box=360.0, n=6000, grid=64)
+    pos, w = W.make(cfg)
+    cfg2 = W.scaled(W.CONFIGS["c3"], box=360.0, n=6000, grid=64)
+    import dataclasses
+    pos2, w2 = W.make(dataclasses.replace(cfg2, seed=cfg2.seed + 11))
+    assert pos2.shape == pos.shape and not np.array_equal(pos, pos2)
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+        out = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+        plan.compute(tp, tw, out=out)                       # sizes the plan
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            plan.compute_enqueue(tp, tw, out)               # on the capture stream (torch's current stream)
+        for p_, w_ in [(pos2, w2), (pos, w)]:
+            tp.copy_(torch.from_numpy(p_))
+            tw.copy_(torch.from_numpy(w_))
+            out.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            o = oracle.zeta(cfg.order, p_, w_, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
+            assert np.abs(out.cpu().numpy() - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
+        del g
