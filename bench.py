@@ -326,6 +326,67 @@ def config_entry(cfg, res, steps, fp64_peak, fp32_peak):
             "contraction_frac_fp64_executed": cfg.n * ex / (st["contraction"] * 1e-3) / fp64_peak}
 
 
+def measure_next_rows(E, torch, dev, fp64_peak):
+    """SURVEY.md §8(f1)-(f3) beside the five configs: 6PCF (literal eq. 44 kernel), edge correction, gridded estimator.
+    CUDA events on torch's current stream (the stream the calls are enqueued on), 3 warm-up + 3 timed calls each."""
+    import dataclasses
+    out = {}
+    stream = torch.cuda.current_stream(dev)
+
+    def timed(fn, reps=3):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        return e0.elapsed_time(e1) / reps
+
+    # (f1) 6PCF: the lognormal recipe of c5 at the same density in a smaller box, 8 bins in [20,160], lmax = 2
+    c6 = W.scaled(dataclasses.replace(W.CONFIGS["c5"], order=6, lmax=2), box=400.0, grid=128, name="x6")
+    pos, w = W.make(c6)
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(6, c6.rmin, c6.rmax, c6.nbins, c6.lmax, c6.box) as plan:
+        E.encore_set_timing(plan.h, True)
+        z = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+        ms = timed(lambda: plan.compute(tp, tw, out=z))
+        km = E.encore_get_kernel_ms(plan.h)
+        ex, ca = E.encore_contraction_flops(plan.h)
+        out["f1_6pcf"] = {"workload": f"6PCF, n={c6.n} lognormal points, periodic L={c6.box:g}, {c6.nbins} bins in [20,160], lmax={c6.lmax}: "
+                                      f"{plan.n_lambda} multiplets x {plan.n_b} bin tuples, {E.encore_num_terms(plan.h)} terms",
+                          "ms_per_step": ms, "primaries_per_s": c6.n / (ms * 1e-3), "kernel_ms": km, "kernel": "k_contract_generic (literal eq. 44)",
+                          "contraction_frac_fp64_executed": c6.n * ex / (km["k_contract"] * 1e-3) / fp64_peak}
+    # (f2) edge correction at the shape of c3 / c4: 69 multiplets, 120 bin tuples (120 LU solves of 69 unknowns)
+    c3 = W.CONFIGS["c3"]
+    with E.Plan(c3.order, c3.rmin, c3.rmax, c3.nbins, c3.lmax, 0.0) as plan:
+        g = torch.Generator(device="cpu").manual_seed(42)
+        R = torch.randn((plan.n_lambda, plan.n_b), generator=g, dtype=torch.float64) * 0.1
+        R[0] = 1.0 + torch.rand(plan.n_b, generator=g, dtype=torch.float64)
+        R[1:] *= R[0]
+        N = torch.randn((plan.n_lambda, plan.n_b), generator=g, dtype=torch.float64)
+        tn, tr = N.to(dev), R.to(dev)
+        z = torch.empty_like(tn)
+        plan.edge_correct(tn, tr, out=z)          # builds the E G tensor on the host once
+        ms = timed(lambda: plan.edge_correct(tn, tr, out=z), reps=10)
+        out["f2_edge_correction"] = {"workload": f"eq. 41/42 for {plan.n_lambda} multiplets x {plan.n_b} bin tuples (the shape of c3 / c4)",
+                                     "ms_per_call": ms, "kernels": "k_edge_assemble + k_edge_solve (one CTA per bin tuple)"}
+    # (f3) gridded estimator: a 64^3 mesh in the box of c3, 4PCF with the bins and lmax of c3
+    G = 64
+    rng = np.random.default_rng(64)
+    delta = torch.from_numpy(rng.standard_normal((G, G, G)) * 0.5).to(dev)
+    with E.Plan(c3.order, c3.rmin, c3.rmax, c3.nbins, c3.lmax, c3.box) as plan:
+        E.encore_set_timing(plan.h, True)
+        z = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+        ms = timed(lambda: plan.compute_grid(delta, out=z))
+        out["f3_gridded"] = {"workload": f"4PCF of a {G}^3 mesh, periodic L={c3.box:g}, {c3.nbins} bins in [20,160], lmax={c3.lmax} "
+                                         f"({c3.nbins * (c3.lmax + 1) * (c3.lmax + 2) // 2} FFT cross-correlations, then {G ** 3} cells through a5)",
+                             "ms_per_step": ms, "cells_per_s": G ** 3 / (ms * 1e-3), "kernel_ms": E.encore_get_kernel_ms(plan.h)}
+    return out
+
+
 _DIST = {"on": False}
 
 
@@ -454,6 +515,7 @@ def main():
         e32["pairs_equal_fp64_run"] = bool(r32["pairs"] == r64["pairs"])
         per["c3_fp32_harmonics"] = e32
         line["per_config"] = per
+        line["next_rows"] = measure_next_rows(E, torch, dev, fp64_peak)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -890,7 +890,7 @@ int encore_get_kernel_ms(const encore_plan_t *Pc, float ms[7])
 {
     encore_plan_t *P = const_cast<encore_plan_t *>(Pc);
     if (!P || !ms) return ENCORE_EINVAL;
-    if (!P->have || !P->timing || P->ev_used < 2) return ENCORE_ESTATE;
+    if (!P->timing || P->ev_used < 2) return ENCORE_ESTATE;   // (also valid after encore_compute_grid: [4] = the FFT stage)
     CU(cudaEventSynchronize(P->ev[P->ev_used - 1]));
     for (int k = 0; k < K_COUNT; ++k) ms[k] = 0.f;
     for (size_t i = 1; i < P->ev_used; ++i) {
