@@ -812,10 +812,12 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
                 double tup = 0;
                 for (int b2 = lo; b2 <= hi; ++b2) tup += (double)b2 * c2(nb - 1 - b2);
                 for (const Lam5 &q : T.lam5) {
-                    const double nl = q.lbeg[q.l12 + 1] - q.lbeg[0], nr = q.rbeg[q.l12 + 1] - q.rbeg[0], nM = q.l12 + 1;
+                    const double nl = q.lbeg[q.l12 + 1] - q.lbeg[1], nr = q.rbeg[q.l12 + 1] - q.rbeg[1], nM = q.l12; // M >= 1
                     ex += nl * (4.0 * (hi - lo + 1) + 8.0 * nyh) + nM * 2.0 * nyh;   // Y block, times w_i
                     ex += nr * (4.0 * (nb - 2 - lo) + 8.0 * nrh);                    // R block
                     ex += nM * 4.0 * tup;                                            // Re[Y R]
+                    const double hl = q.lbeg[1] - q.lbeg[0], hr = q.rbeg[1] - q.rbeg[0];   // M = 0: half terms, real pairs
+                    ex += hl * (2.0 * (hi - lo + 1) + 4.0 * nyh) + nyh + hr * (2.0 * (nb - 2 - lo) + 4.0 * nrh) + 2.0 * tup;
                 }
             }
         }

@@ -620,6 +620,33 @@ __device__ __forceinline__ void pairs_block(double (&zr)[NZ], double (&zi)[NZ], 
     }
 }
 
+// M = 0 ("half terms", tables.cpp): the coupled pair is one real number,  Z(x,y) += wrr A[ia_re](x) B[ib_re](y) + wii A[ia_im](x) B[ib_im](y)
+template <int NB, int KIND, int X0, int X1, int Y0, int Y1, int NZ>
+__device__ __forceinline__ void pairs_block_half(double (&z)[NZ], const PairTerm *terms, int t0, int t1, const double *pa, const double *pb)
+{
+    constexpr int rs = NB * 32, NY = Y1 - Y0 + 1;
+#pragma unroll 1
+    for (int t = t0; t < t1; ++t) {
+        const PairTerm T = terms[t];
+        double u[NY], v[NY];
+        const double *br = pb + T.ib_re * rs, *bi = pb + T.ib_im * rs;
+        static_for<Y0, Y1 + 1>([&](auto Yc) {
+            constexpr int y = decltype(Yc)::value;
+            u[y - Y0] = T.wrr * br[y * 32]; v[y - Y0] = T.wii * bi[y * 32];
+        });
+        const double *ar = pa + T.ia_re * rs, *ai = pa + T.ia_im * rs;
+        static_for<X0, X1 + 1>([&](auto Xc) {
+            constexpr int x = decltype(Xc)::value;
+            const double rx = ar[x * 32], ix = ai[x * 32];
+            static_for<(x + 1 > Y0 ? x + 1 : Y0), Y1 + 1>([&](auto Yc) {
+                constexpr int y = decltype(Yc)::value;
+                constexpr int k = slot5<NB, KIND, X0, Y0>(x, y);
+                z[k] = fma(u[y - Y0], rx, fma(v[y - Y0], ix, z[k]));
+            });
+        });
+    }
+}
+
 // ---- how the second bins 1 .. NB-3 of a multiplet are dealt to its warps -----------------------------------
 // Up to 8 bins: two warps, b2 <= T and b2 > T (T = t5(NB), measured on c5).  9 and 10 bins: consecutive ranges grown
 // greedily while partial sums + held coupled pairs stay under 105 doubles (3 and 5 warps).
@@ -661,7 +688,34 @@ __device__ __forceinline__ void task5(double (&acc)[NTOT], const Lam5 &L, int to
         constexpr int NYH = c2(HI + 1) - c2(LO);   // pairs b1 < b2, LO <= b2 <= HI
         constexpr int NRH = c2(NB - 1 - LO);       // pairs LO+1 <= b3 < b4 <= NB-1
         const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.lbeg[0];
-        for (int M = 0; M <= L.l12; ++M) {
+        {   // M = 0: Y12_0 and R34_0 are one real number each (half terms), H_0 = Ys Rs: one FMA per quadruple
+            double ys[NYH];
+#pragma unroll
+            for (int k = 0; k < NYH; ++k) ys[k] = 0.0;
+            pairs_block_half<NB, 0, 0, HI - 1, LO, HI, NYH>(ys, terms, L.lbeg[0], L.lbeg[1], p1, p2);
+#pragma unroll
+            for (int k = 0; k < NYH; ++k) ys[k] *= wi;
+            double rs0[NRH];
+#pragma unroll
+            for (int k = 0; k < NRH; ++k) rs0[k] = 0.0;
+            pairs_block_half<NB, 1, LO + 1, NB - 2, LO + 2, NB - 1, NRH>(rs0, terms, L.rbeg[0], L.rbeg[1], p3, p4);
+            static_for<LO, HI + 1>([&](auto B2) {
+                constexpr int b2 = decltype(B2)::value;
+                static_for<b2 + 1, NB - 1>([&](auto B3) {
+                    constexpr int b3 = decltype(B3)::value;
+                    static_for<b3 + 1, NB>([&](auto B4) {
+                        constexpr int b4 = decltype(B4)::value;
+                        constexpr int k = slot5<NB, 1, LO + 1, LO + 2>(b3, b4);
+                        static_for<0, b2>([&](auto B1) {
+                            constexpr int b1 = decltype(B1)::value;
+                            constexpr int o = aidx5(NB, LO, b1, b2, b3, b4), q = slot5<NB, 0, 0, LO>(b1, b2);
+                            acc[o] = fma(ys[q], rs0[k], acc[o]);
+                        });
+                    });
+                });
+            });
+        }
+        for (int M = 1; M <= L.l12; ++M) {
             double yr[NYH], yi[NYH];
 #pragma unroll
             for (int k = 0; k < NYH; ++k) { yr[k] = 0.0; yi[k] = 0.0; }

@@ -264,21 +264,45 @@ void build_factorised(HostTables &t)
             const int *lam = &t.multiplets[(size_t)iL * 5];
             Lam5 q{};
             q.l1 = lam[0]; q.l2 = lam[1]; q.l12 = lam[2]; q.l3 = lam[3]; q.l4 = lam[4]; q.odd = t.parity[iL];
+            // M = 0: the terms (m, -m) and (-m, m) of a coupled pair are complex conjugates up to sigma = (-1)^{la+lb+l12}
+            // (3-j column symmetry, a_{l,-m} = (-1)^m a*_lm), so Y12_0 and R34_0 are real (sigma = +1) or imaginary
+            // (sigma = -1): one real number per bin pair from "half terms" m >= 0 (as for N = 4, m3 = 0),
+            //   T(m) = c_m (-1)^m a_m conj(b_m),  c_m = (la lb l12; m -m 0)
+            //   sigma = +1: Re Y_0 = c_0 r r' + sum_{m>0} 2 c_m (-1)^m (r r' + i i');   sigma = -1: Im Y_0 = sum_{m>0} 2 c_m (-1)^m (i r' - r i')
+            // and H_0 = s Ys Rs with s = -1 iff both are imaginary (even multiplet, (i Yi)(i Ri)); s is folded into the left weights.
+            auto half_terms = [&](int la, int lb, int L, double factor) {
+                const int sig_odd = (la + lb + L) & 1;
+                for (int m = 0; m <= std::min(la, lb); ++m) {
+                    const double c = encore_host_wigner3j(la, lb, L, m, -m, 0);
+                    if (std::fabs(c) < 1e-15) continue;
+                    const double w = factor * (m == 0 ? 1.0 : 2.0) * ((m & 1) ? -c : c);
+                    const int re = m == 0 ? 0 : 2 * m - 1, im = m == 0 ? 0 : 2 * m;
+                    PairTerm pt{};
+                    if (!sig_odd) { pt.ia_re = re; pt.ib_re = re; pt.ia_im = im; pt.ib_im = im; pt.wrr = w; pt.wii = m ? w : 0.0; }
+                    else if (m > 0) { pt.ia_re = im; pt.ib_re = re; pt.ia_im = re; pt.ib_im = im; pt.wrr = w; pt.wii = -w; }
+                    else continue;
+                    t.pair_terms.push_back(pt);
+                }
+            };
+            const bool both_imag = ((q.l1 + q.l2 + q.l12) & 1) && ((q.l3 + q.l4 + q.l12) & 1);
             for (int M = 0; M <= q.l12; ++M) {
                 const double f = std::sqrt(2.0 * q.l12 + 1.0) * (((q.l12 - M) & 1) ? -1.0 : 1.0) * (M == 0 ? 1.0 : 2.0);
                 q.lbeg[M] = (int)t.pair_terms.size();
-                coupled_pair_terms(q.l1, q.l2, q.l12, M, f, t.pair_terms);   // (l1 l2 l12; m1 m2 -M)
+                if (M == 0) half_terms(q.l1, q.l2, q.l12, both_imag ? -f : f);
+                else coupled_pair_terms(q.l1, q.l2, q.l12, M, f, t.pair_terms);   // (l1 l2 l12; m1 m2 -M)
                 q.lbeg[M + 1] = (int)t.pair_terms.size();
             }
             for (int M = q.l12 + 1; M < 13; ++M) q.lbeg[M + 1] = q.lbeg[q.l12 + 1];
             for (int M = 0; M <= q.l12; ++M) {
                 q.rbeg[M] = (int)t.pair_terms.size();
-                coupled_pair_terms(q.l3, q.l4, q.l12, -M, 1.0, t.pair_terms); // (l3 l4 l12; m3 m4 M) = (l12 l3 l4; M m3 m4)
+                if (M == 0) half_terms(q.l3, q.l4, q.l12, 1.0);
+                else coupled_pair_terms(q.l3, q.l4, q.l12, -M, 1.0, t.pair_terms); // (l3 l4 l12; m3 m4 M) = (l12 l3 l4; M m3 m4)
                 q.rbeg[M + 1] = (int)t.pair_terms.size();
             }
             for (int M = q.l12 + 1; M < 13; ++M) q.rbeg[M + 1] = q.rbeg[q.l12 + 1];
             q.nterms = (q.lbeg[q.l12 + 1] - q.lbeg[0]) + (q.rbeg[q.l12 + 1] - q.rbeg[0]);
-            cost[iL] = (q.lbeg[q.l12 + 1] - q.lbeg[0]) + 3.0 * (q.rbeg[q.l12 + 1] - q.rbeg[0]) + (q.l12 + 1);
+            cost[iL] = (q.lbeg[q.l12 + 1] - q.lbeg[1]) + 0.5 * (q.lbeg[1] - q.lbeg[0]) + 3.0 * (q.rbeg[q.l12 + 1] - q.rbeg[1]) +
+                       1.5 * (q.rbeg[1] - q.rbeg[0]) + (q.l12 + 1);
             t.lam5.push_back(q);
         }
     }
