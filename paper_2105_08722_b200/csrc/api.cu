@@ -89,8 +89,12 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
     const HostTables &T = P->T;
     std::vector<DevTerm> dt(T.terms.size());
     for (size_t i = 0; i < dt.size(); ++i) {
-        for (int k = 0; k < 5; ++k) { dt[i].re[k] = T.terms[i].re[k]; dt[i].im[k] = T.terms[i].im[k]; dt[i].tau[k] = T.terms[i].tau[k]; }
-        for (int k = 0; k < 7; ++k) dt[i].pad[k] = 0;
+        for (int k = 0; k < 5; ++k) {
+            const int rs = T.nbins * 32;
+            dt[i].off_re[k] = T.terms[i].re[k] * rs;
+            dt[i].off_im[k] = (T.terms[i].im[k] >= 0 ? T.terms[i].im[k] : T.terms[i].re[k]) * rs;
+            dt[i].tau[k] = T.terms[i].im[k] >= 0 ? (double)T.terms[i].tau[k] : 0.0;
+        }
         dt[i].W = T.terms[i].W;
     }
     CU(P->d_terms.ensure(sizeof(DevTerm) * std::max<size_t>(1, dt.size())));

@@ -27,41 +27,71 @@ __device__ __forceinline__ int group_end(const ContractArgs &a)
 }
 
 // Generic kernel, any N in {3,..,6}: one warp per output (Lam,B), terms looped (literal eq. 44), complex products in registers.
+// One CTA per group of 32 primaries; its a_lm tile ([component][bin][lane], contiguous) is first copied to shared memory
+// when it fits (STAGED), otherwise read through the caches.  The term records carry row offsets and the conjugation sign
+// as a multiplier (DevTerm), the number of factors NM = N - 1 is a template parameter: the inner loop is two loads, one
+// multiply and a complex product per factor (6PCF, lmax = 2, 8 bins, 20 000 primaries: 151 -> 80 ms).
+extern __shared__ __align__(128) double smem_generic[];
+template <bool STAGED, int NM>
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
     const int g = a.g_begin + blockIdx.x;
     if (g >= group_end(a)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nb = a.nbins, nm = a.order - 1;
+    const int nb = a.nbins;
     const double wi = a.gweights[(size_t)g * 32 + lane];
-    const double *tile = a.alm + (size_t)g * a.ncomp * nb * 32 + lane;
+    const size_t tile_len = (size_t)a.ncomp * nb * 32;
+    const double *tile = a.alm + (size_t)g * tile_len + lane;
+    if (STAGED) {
+        const double2 *src = reinterpret_cast<const double2 *>(a.alm + (size_t)g * tile_len);
+        double2 *dst = reinterpret_cast<double2 *>(smem_generic);
+        for (int i = threadIdx.x; i < (int)(tile_len / 2); i += kWarps * 32) dst[i] = src[i];
+        __syncthreads();
+        tile = smem_generic + lane;
+    }
     const int nout = a.nLam * a.nB;
     double *out = a.partial + (size_t)g * nout;
 
     for (int o = warp; o < nout; o += kWarps) {
         const int iL = o / a.nB, iB = o - iL * a.nB;
-        int boff[5];
-        for (int k = 0; k < nm; ++k) boff[k] = a.bin_tuples[iB * nm + k] * 32;
-        double acc = 0.0;
-        const bool odd = a.lam_parity[iL] != 0; // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)
+        const double *fac[NM];      // row 0 of the tile at the bin of factor k (this lane's primary)
+#pragma unroll
+        for (int k = 0; k < NM; ++k) fac[k] = tile + a.bin_tuples[iB * NM + k] * 32;
+        double accr = 0.0, acci = 0.0;
         const int t1 = a.term_start[iL + 1];
         for (int t = a.term_start[iL]; t < t1; ++t) {
-            const DevTerm tm = a.terms[t];
-            double pr = tm.W, pi = 0.0;
-            for (int k = 0; k < nm; ++k) {
-                const double re = tile[(size_t)tm.re[k] * nb * 32 + boff[k]];
-                const double im = tm.im[k] >= 0 ? (double)tm.tau[k] * tile[(size_t)tm.im[k] * nb * 32 + boff[k]] : 0.0;
-                const double nr = pr * re - pi * im;
-                const double ni = pr * im + pi * re;
+            const DevTerm &tm = a.terms[t];
+            double pr = tm.W * fac[0][tm.off_re[0]], pi = tm.W * (tm.tau[0] * fac[0][tm.off_im[0]]);
+#pragma unroll
+            for (int k = 1; k < NM; ++k) {
+                const double re = fac[k][tm.off_re[k]];
+                const double im = tm.tau[k] * fac[k][tm.off_im[k]];
+                const double nr = fma(pr, re, -(pi * im));
+                const double ni = fma(pr, im, pi * re);
                 pr = nr; pi = ni;
             }
-            acc += odd ? pi : pr;
+            accr += pr; acci += pi;
         }
-        acc *= wi;
+        // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)
+        double acc = (a.lam_parity[iL] != 0 ? acci : accr) * wi;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(kFull, acc, d);
         if (lane == 0) out[o] = acc;
     }
+}
+
+template <int NM>
+cudaError_t launch_generic(const ContractArgs &a, cudaStream_t s)
+{
+    const size_t tile_bytes = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
+    if (tile_bytes <= 96 * 1024) {   // at least two CTAs per SM
+        static std::once_flag once;
+        static cudaError_t attr_err = cudaSuccess;
+        std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract_generic<true, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024); });
+        if (attr_err != cudaSuccess) return attr_err;
+        k_contract_generic<true, NM><<<a.g_end - a.g_begin, kWarps * 32, tile_bytes, s>>>(a);
+    } else k_contract_generic<false, NM><<<a.g_end - a.g_begin, kWarps * 32, 0, s>>>(a);
+    return cudaGetLastError();
 }
 
 // a6, level 1: segment s sums its groups in index order.  level 2: sums the segments in index order, times 1/V.
@@ -924,8 +954,13 @@ cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launc
     *launches += 1;
     if (!a.factorised) {
         if (a.g_end <= a.g_begin) return cudaSuccess;
-        k_contract_generic<<<a.g_end - a.g_begin, kWarps * 32, 0, s>>>(a);
-        return cudaGetLastError();
+        switch (a.order) {
+        case 3: return launch_generic<2>(a, s);
+        case 4: return launch_generic<3>(a, s);
+        case 5: return launch_generic<4>(a, s);
+        case 6: return launch_generic<5>(a, s);
+        }
+        return cudaErrorInvalidValue;
     }
     // every (multiplet, tuple) of a chunk row is written by exactly one warp; no initialisation needed
     if (a.order == 3) {

@@ -17,11 +17,10 @@ struct GridGeom {
     int ncell, npencil;
 };
 
-struct DevTerm {        // device image of HostTerm (40 bytes)
-    short re[5];
-    short im[5];
-    signed char tau[5];
-    signed char pad[7];
+struct DevTerm {        // device image of HostTerm for the literal eq. 44 kernel (88 bytes)
+    int off_re[5];      // offset (doubles) of the real-part row of factor k inside a tile: component * nbins * 32
+    int off_im[5];      // same for the imaginary part (m = 0: the real-part row, with tau = 0)
+    double tau[5];      // +1, -1 (conjugated factor) or 0 (m = 0: no imaginary part)
     double W;
 };
 
