@@ -96,7 +96,15 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
             dt[i].tau[k] = T.terms[i].im[k] >= 0 ? (double)T.terms[i].tau[k] : 0.0;
         }
         dt[i].W = T.terms[i].W;
+        dt[i].start = 0; dt[i].pad = 0;
     }
+    for (int iL = 0; iL < T.nLam(); ++iL)
+        for (int t = T.term_start[iL] + 1; t < T.term_start[iL + 1]; ++t) {
+            int k = 0;
+            while (k < T.order - 2 && dt[t].off_re[k] == dt[t - 1].off_re[k] && dt[t].off_im[k] == dt[t - 1].off_im[k] &&
+                   dt[t].tau[k] == dt[t - 1].tau[k]) ++k;
+            dt[t].start = k;   // (the last factor always changes with any other: m_{N-1} = -sum of the others)
+        }
     CU(P->d_terms.ensure(sizeof(DevTerm) * std::max<size_t>(1, dt.size())));
     CU(P->d_term_start.ensure(sizeof(int) * T.term_start.size()));
     CU(P->d_bin_tuples.ensure(sizeof(int) * T.bin_tuples.size()));

@@ -26,12 +26,15 @@ __device__ __forceinline__ int group_end(const ContractArgs &a)
     return a.ngroups_dev ? min(a.g_end, *a.ngroups_dev) : a.g_end;
 }
 
-// Generic kernel, any N in {3,..,6}: one warp per output (Lam,B), terms looped (literal eq. 44), complex products in registers.
+// Generic kernel, any N in {3,..,6}: one warp per output (Lam,B) at a time, terms looped (literal eq. 44), complex products in registers.
 // One CTA per group of 32 primaries; its a_lm tile ([component][bin][lane], contiguous) is first copied to shared memory
 // when it fits (STAGED), otherwise read through the caches.  The term records carry row offsets and the conjugation sign
 // as a multiplier (DevTerm), the number of factors NM = N - 1 is a template parameter: the inner loop is two loads, one
-// multiply and a complex product per factor (6PCF, lmax = 2, 8 bins, 20 000 primaries: 151 -> 80 ms).
+// multiply and a complex product per factor, and the partial products of the leading factors a term shares with its
+// predecessor (terms are in lexicographic order of their m's) are kept.
 extern __shared__ __align__(128) double smem_generic[];
+constexpr int kTermChunk = 128;     // terms of a multiplet staged in shared memory at a time (12 kB)
+
 template <bool STAGED, int NM>
 __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a)
 {
@@ -41,56 +44,88 @@ __global__ void __launch_bounds__(kWarps * 32) k_contract_generic(ContractArgs a
     const int nb = a.nbins;
     const double wi = a.gweights[(size_t)g * 32 + lane];
     const size_t tile_len = (size_t)a.ncomp * nb * 32;
-    const double *tile = a.alm + (size_t)g * tile_len + lane;
+    const double *tbase = a.alm + (size_t)g * tile_len;
+    // dynamic shared memory: [term chunk][tile, if staged]
+    DevTerm *s_terms = reinterpret_cast<DevTerm *>(smem_generic);
+    double *s_tile = smem_generic + kTermChunk * sizeof(DevTerm) / sizeof(double);
     if (STAGED) {
         const double2 *src = reinterpret_cast<const double2 *>(a.alm + (size_t)g * tile_len);
-        double2 *dst = reinterpret_cast<double2 *>(smem_generic);
+        double2 *dst = reinterpret_cast<double2 *>(s_tile);
         for (int i = threadIdx.x; i < (int)(tile_len / 2); i += kWarps * 32) dst[i] = src[i];
-        __syncthreads();
-        tile = smem_generic + lane;
     }
     const int nout = a.nLam * a.nB;
     double *out = a.partial + (size_t)g * nout;
 
-    for (int o = warp; o < nout; o += kWarps) {
-        const int iL = o / a.nB, iB = o - iL * a.nB;
-        const double *fac[NM];      // row 0 of the tile at the bin of factor k (this lane's primary)
-#pragma unroll
-        for (int k = 0; k < NM; ++k) fac[k] = tile + a.bin_tuples[iB * NM + k] * 32;
-        double accr = 0.0, acci = 0.0;
-        const int t1 = a.term_start[iL + 1];
-        for (int t = a.term_start[iL]; t < t1; ++t) {
-            const DevTerm &tm = a.terms[t];
-            double pr = tm.W * fac[0][tm.off_re[0]], pi = tm.W * (tm.tau[0] * fac[0][tm.off_im[0]]);
-#pragma unroll
-            for (int k = 1; k < NM; ++k) {
-                const double re = fac[k][tm.off_re[k]];
-                const double im = tm.tau[k] * fac[k][tm.off_im[k]];
-                const double nr = fma(pr, re, -(pi * im));
-                const double ni = fma(pr, im, pi * re);
-                pr = nr; pi = ni;
+    // the CTA walks the multiplets; the terms of the current one sit in shared memory (a chunk at a time), the warps
+    // share out its bin tuples.  out[o] is owned by one warp: a later chunk adds to what the first one wrote.
+    for (int iL = blockIdx.y; iL < a.nLam; iL += gridDim.y) {    // (interleaved: heavy and light multiplets mix)
+        const int t0 = a.term_start[iL], t1 = a.term_start[iL + 1];
+        const bool odd = a.lam_parity[iL] != 0;   // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)
+        for (int c0 = t0; c0 < t1 || c0 == t0; c0 += kTermChunk) {
+            const int nt = min(t1, c0 + kTermChunk) - c0;
+            __syncthreads();        // the previous chunk has been consumed (and, the first time, the tile is complete)
+            {
+                const double *src = reinterpret_cast<const double *>(a.terms + c0);
+                double *dst = reinterpret_cast<double *>(s_terms);
+                for (int i = threadIdx.x; i < nt * (int)(sizeof(DevTerm) / sizeof(double)); i += kWarps * 32) dst[i] = src[i];
             }
-            accr += pr; acci += pi;
-        }
-        // parity-odd multiplet: zeta = i * sum W Im[prod] (App. B)
-        double acc = (a.lam_parity[iL] != 0 ? acci : accr) * wi;
+            __syncthreads();
+            for (int iB = warp; iB < a.nB; iB += kWarps) {
+                int fo[NM];                 // offset of row 0 of the tile at the bin of factor k (this lane's primary)
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(kFull, acc, d);
-        if (lane == 0) out[o] = acc;
+                for (int k = 0; k < NM; ++k) fo[k] = a.bin_tuples[iB * NM + k] * 32 + lane;
+                double accr = 0.0, acci = 0.0;
+                double pr[NM], pi[NM];      // partial products a~_0 .. a~_k of the current term
+#pragma unroll
+                for (int k = 0; k < NM; ++k) { pr[k] = 0.0; pi[k] = 0.0; }
+                auto factor = [&](auto K, const DevTerm &tm) {
+                    constexpr int k = decltype(K)::value;
+                    const double re = STAGED ? s_tile[fo[k] + tm.off_re[k]] : tbase[fo[k] + tm.off_re[k]];
+                    const double im = tm.tau[k] * (STAGED ? s_tile[fo[k] + tm.off_im[k]] : tbase[fo[k] + tm.off_im[k]]);
+                    if constexpr (k == 0) { pr[0] = re; pi[0] = im; }
+                    else {
+                        pr[k] = fma(pr[k - 1], re, -(pi[k - 1] * im));
+                        pi[k] = fma(pr[k - 1], im, pi[k - 1] * re);
+                    }
+                };
+                for (int t = 0; t < nt; ++t) {
+                    const DevTerm &tm = s_terms[t];
+                    // the factors from tm.start on are new (warp-uniform); the first term of a chunk starts from scratch
+                    switch (t == 0 ? 0 : tm.start) {
+                    case 0: factor(std::integral_constant<int, 0>{}, tm); [[fallthrough]];
+                    case 1: if constexpr (NM > 1) factor(std::integral_constant<int, 1>{}, tm); [[fallthrough]];
+                    case 2: if constexpr (NM > 2) factor(std::integral_constant<int, 2>{}, tm); [[fallthrough]];
+                    case 3: if constexpr (NM > 3) factor(std::integral_constant<int, 3>{}, tm); [[fallthrough]];
+                    default: if constexpr (NM > 4) factor(std::integral_constant<int, 4>{}, tm);
+                    }
+                    accr = fma(tm.W, pr[NM - 1], accr); acci = fma(tm.W, pi[NM - 1], acci);
+                }
+                double acc = (odd ? acci : accr) * wi;
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(kFull, acc, d);
+                const int o = iL * a.nB + iB;
+                if (lane == 0) out[o] = c0 == t0 ? acc : out[o] + acc;
+            }
+        }
     }
 }
 
 template <int NM>
 cudaError_t launch_generic(const ContractArgs &a, cudaStream_t s)
 {
-    const size_t tile_bytes = (size_t)a.ncomp * a.nbins * 32 * sizeof(double);
+    const size_t tile_bytes = (size_t)a.ncomp * a.nbins * 32 * sizeof(double), term_bytes = kTermChunk * sizeof(DevTerm);
+    static_assert(sizeof(DevTerm) % sizeof(double) == 0, "DevTerm is copied by doubles");
+    // grid: (group, slice of the multiplet list); enough CTAs for ~8 waves of 148 SMs x 4 CTAs, so that the last wave is short
+    const int ng = a.g_end - a.g_begin;
+    const int slices = std::max(1, std::min(a.nLam, (8 * 148 * 4 + ng - 1) / ng));
+    const dim3 grid(ng, slices);
     if (tile_bytes <= 96 * 1024) {   // at least two CTAs per SM
         static std::once_flag once;
         static cudaError_t attr_err = cudaSuccess;
-        std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract_generic<true, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024); });
+        std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract_generic<true, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024); });
         if (attr_err != cudaSuccess) return attr_err;
-        k_contract_generic<true, NM><<<a.g_end - a.g_begin, kWarps * 32, tile_bytes, s>>>(a);
-    } else k_contract_generic<false, NM><<<a.g_end - a.g_begin, kWarps * 32, 0, s>>>(a);
+        k_contract_generic<true, NM><<<grid, kWarps * 32, tile_bytes + term_bytes, s>>>(a);
+    } else k_contract_generic<false, NM><<<grid, kWarps * 32, term_bytes, s>>>(a);
     return cudaGetLastError();
 }
 

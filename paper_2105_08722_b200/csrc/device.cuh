@@ -17,11 +17,13 @@ struct GridGeom {
     int ncell, npencil;
 };
 
-struct DevTerm {        // device image of HostTerm for the literal eq. 44 kernel (88 bytes)
+struct DevTerm {        // device image of HostTerm for the literal eq. 44 kernel (96 bytes)
     int off_re[5];      // offset (doubles) of the real-part row of factor k inside a tile: component * nbins * 32
     int off_im[5];      // same for the imaginary part (m = 0: the real-part row, with tau = 0)
     double tau[5];      // +1, -1 (conjugated factor) or 0 (m = 0: no imaginary part)
     double W;
+    int start;          // first factor that differs from the previous term of the multiplet (terms are in lexicographic
+    int pad;            // order of m_1 .. m_{N-2}): the partial products of the factors before it are reused
 };
 
 struct BinTable {       // passed by value (kernel parameter space -> constant bank)
