@@ -83,6 +83,17 @@ namespace {
         }                                            \
     } while (0)
 
+// literal eq. 44 kernel: first factor of term t that differs from term t-1 of the same multiplet (the terms are in
+// lexicographic order of m_1 .. m_{N-2}; the partial products of the factors before it are reused).  The last factor
+// always differs: m_{N-1} = -(m_1 + .. + m_{N-2}).
+int term_prefix_start(const HostTables &T, int t)
+{
+    int k = 0;
+    while (k < T.order - 2 && T.terms[t].re[k] == T.terms[t - 1].re[k] && T.terms[t].im[k] == T.terms[t - 1].im[k] &&
+           T.terms[t].tau[k] == T.terms[t - 1].tau[k]) ++k;
+    return k;
+}
+
 int upload_tables(encore_plan_s *P, cudaStream_t s)
 {
     if (P->uploaded) return ENCORE_OK;
@@ -99,12 +110,7 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
         dt[i].start = 0; dt[i].pad = 0;
     }
     for (int iL = 0; iL < T.nLam(); ++iL)
-        for (int t = T.term_start[iL] + 1; t < T.term_start[iL + 1]; ++t) {
-            int k = 0;
-            while (k < T.order - 2 && dt[t].off_re[k] == dt[t - 1].off_re[k] && dt[t].off_im[k] == dt[t - 1].off_im[k] &&
-                   dt[t].tau[k] == dt[t - 1].tau[k]) ++k;
-            dt[t].start = k;   // (the last factor always changes with any other: m_{N-1} = -sum of the others)
-        }
+        for (int t = T.term_start[iL] + 1; t < T.term_start[iL + 1]; ++t) dt[t].start = term_prefix_start(T, t);
     CU(P->d_terms.ensure(sizeof(DevTerm) * std::max<size_t>(1, dt.size())));
     CU(P->d_term_start.ensure(sizeof(int) * T.term_start.size()));
     CU(P->d_bin_tuples.ensure(sizeof(int) * T.bin_tuples.size()));
@@ -795,7 +801,15 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
     const HostTables &T = P->T;
     const double evals = (double)T.terms.size() * (double)T.nB();
     const int N = T.order, nb = T.nbins;
-    double ex = evals * (6.0 * (N - 1) + 1.0); // generic kernel: N-1 complex multiplies + 1 add per term
+    // literal eq. 44 kernel: per term and bin tuple, one multiply (conjugation sign) + one complex multiply (2 mul + 2 FMA)
+    // for every factor that differs from the previous term's (the first factor: the sign multiply only), 2 FMA for W
+    double ex = 0.0;
+    for (int iL = 0; iL < T.nLam(); ++iL)
+        for (int t = T.term_start[iL]; t < T.term_start[iL + 1]; ++t) {
+            const int start = t == T.term_start[iL] ? 0 : term_prefix_start(T, t);
+            ex += (start == 0 ? 1.0 + 7.0 * (N - 2) : 7.0 * (N - 1 - start)) + 4.0;
+        }
+    ex *= (double)T.nB();
     if (!P->force_generic && contraction_is_factorised(N, nb, T.lmax) && (N == 3 || P->cta_smem > 0)) {
         // executed by the factorised kernels, fused multiply-add = 2
         ex = 0.0;
