@@ -345,8 +345,9 @@ def measure_next_rows(E, torch, dev, fp64_peak):
         torch.cuda.synchronize(dev)
         return e0.elapsed_time(e1) / reps
 
-    # (f1) 6PCF: the lognormal recipe of c5 at the same density in a smaller box, 8 bins in [20,160], lmax = 2
-    c6 = W.scaled(dataclasses.replace(W.CONFIGS["c5"], order=6, lmax=2), box=400.0, grid=128, name="x6")
+    # (f1) 6PCF on the catalogue of c5 (300 000 lognormal points, 8 bins in [20,160]) at lmax = 2: 327 multiplets x 56 bin
+    # quintuples, factorised kernel k_contract6<8>; the literal eq. 44 kernel on a 20 000-point sub-box beside it
+    c6 = dataclasses.replace(W.CONFIGS["c5"], order=6, lmax=2, name="c5 catalogue")
     pos, w = W.make(c6)
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     with E.Plan(6, c6.rmin, c6.rmax, c6.nbins, c6.lmax, c6.box) as plan:
@@ -355,10 +356,24 @@ def measure_next_rows(E, torch, dev, fp64_peak):
         ms = timed(lambda: plan.compute(tp, tw, out=z))
         km = E.encore_get_kernel_ms(plan.h)
         ex, ca = E.encore_contraction_flops(plan.h)
-        out["f1_6pcf"] = {"workload": f"6PCF, n={c6.n} lognormal points, periodic L={c6.box:g}, {c6.nbins} bins in [20,160], lmax={c6.lmax}: "
-                                      f"{plan.n_lambda} multiplets x {plan.n_b} bin tuples, {E.encore_num_terms(plan.h)} terms",
-                          "ms_per_step": ms, "primaries_per_s": c6.n / (ms * 1e-3), "kernel_ms": km, "kernel": "k_contract_generic (literal eq. 44)",
+        out["f1_6pcf"] = {"workload": f"6PCF, n={c6.n} lognormal points (the catalogue of c5), periodic L={c6.box:g}, {c6.nbins} bins in [20,160], "
+                                      f"lmax={c6.lmax}: {plan.n_lambda} multiplets x {plan.n_b} bin tuples, {E.encore_num_terms(plan.h)} terms",
+                          "ms_per_step": ms, "primaries_per_s": c6.n / (ms * 1e-3), "kernel_ms": km, "kernel": "k_contract6<8> (factorised, contract6.cu)",
+                          "contraction_flops_per_primary_executed": ex, "contraction_flops_per_primary_canonical": ca,
                           "contraction_frac_fp64_executed": c6.n * ex / (km["k_contract"] * 1e-3) / fp64_peak}
+        sel = (pos[0] < 406.0) & (pos[1] < 406.0) & (pos[2] < 406.0)
+        ps, ws = np.ascontiguousarray(pos[:, sel]), np.ascontiguousarray(w[sel])
+    with E.Plan(6, c6.rmin, c6.rmax, c6.nbins, c6.lmax, 0.0) as plan:
+        tps, tws = torch.from_numpy(ps).to(dev), torch.from_numpy(ws).to(dev)
+        E.encore_set_timing(plan.h, True)
+        z = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+        res = {}
+        for tag, lit in (("factorised", 0), ("literal_eq44", 1)):
+            E.encore_set_option(plan.h, "generic_contract", lit)
+            timed(lambda: plan.compute(tps, tws, out=z), reps=2)
+            res[tag + "_contraction_ms"] = E.encore_get_kernel_ms(plan.h)["k_contract"]
+            res[tag + "_flops_per_primary"] = E.encore_contraction_flops(plan.h)[0]
+        out["f1_6pcf"]["sub_box"] = dict(res, n=int(ps.shape[1]), note="open-geometry sub-box of the same catalogue, both contraction kernels")
     # (f2) edge correction at the shape of c3 / c4: 69 multiplets, 120 bin tuples (120 LU solves of 69 unknowns)
     c3 = W.CONFIGS["c3"]
     with E.Plan(c3.order, c3.rmin, c3.rmax, c3.nbins, c3.lmax, 0.0) as plan:

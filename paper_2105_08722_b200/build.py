@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libencore_b200.so")
-SOURCES = ["tables.cpp", "grid.cu", "pair.cu", "contract.cu", "edge.cu", "mesh.cu", "diag.cu", "api.cu"]
+SOURCES = ["tables.cpp", "grid.cu", "pair.cu", "contract.cu", "contract6.cu", "edge.cu", "mesh.cu", "diag.cu", "api.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", INCLUDE] + os.environ.get("ENCORE_NVCC_FLAGS", "").split()

@@ -35,7 +35,7 @@ struct DevBuf {
 struct encore_plan_s {
     HostTables T;
     bool uploaded = false;
-    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam_order, d_lam_parity, d_tuple_index, d_ctas, gweights;
+    DevBuf d_terms, d_term_start, d_bin_tuples, d_ynorm, d_ycoef, d_pair_terms, d_lam4, d_lam5, d_lam6, d_lam_order, d_lam_parity, d_tuple_index, d_ctas, gweights;
     std::vector<CtaPlan> ctas;      // factorised N = 4, 5 kernels: multiplets and staged l-blocks per CTA
     size_t cta_smem = 0;
     bool force_generic = false;
@@ -135,6 +135,8 @@ int upload_tables(encore_plan_s *P, cudaStream_t s)
         CU(P->d_pair_terms.ensure(sizeof(PairTerm) * std::max<size_t>(1, T.pair_terms.size())));
         CU(P->d_lam4.ensure(sizeof(Lam4) * std::max<size_t>(1, T.lam4.size())));
         CU(P->d_lam5.ensure(sizeof(Lam5) * std::max<size_t>(1, T.lam5.size())));
+        CU(P->d_lam6.ensure(sizeof(Lam6) * std::max<size_t>(1, T.lam6.size())));
+        CU(cudaMemcpyAsync(P->d_lam6.p, T.lam6.data(), sizeof(Lam6) * T.lam6.size(), cudaMemcpyHostToDevice, s));
         CU(P->d_lam_order.ensure(sizeof(int) * std::max<size_t>(1, T.lam_order.size())));
         CU(P->d_lam_parity.ensure(sizeof(int) * std::max<size_t>(1, T.parity.size())));
         CU(cudaMemcpyAsync(P->d_lam_parity.p, T.parity.data(), sizeof(int) * T.parity.size(), cudaMemcpyHostToDevice, s));
@@ -242,6 +244,7 @@ int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweig
     ca.pair_terms = P->d_pair_terms.as<PairTerm>();
     ca.lam4 = P->d_lam4.as<Lam4>();
     ca.lam5 = P->d_lam5.as<Lam5>();
+    ca.lam6 = P->d_lam6.as<Lam6>();
     ca.lam_order = P->d_lam_order.as<int>();
     ca.lam_parity = P->d_lam_parity.as<int>();
     ca.tuple_index = P->d_tuple_index.as<int>();
@@ -249,6 +252,7 @@ int contract_and_reduce(encore_plan_s *P, const double *alm, const double *gweig
     ca.max_terms = 1;
     for (const Lam4 &q : T.lam4) ca.max_terms = std::max(ca.max_terms, q.nterms);
     for (const Lam5 &q : T.lam5) ca.max_terms = std::max(ca.max_terms, q.nterms);
+    for (const Lam6 &q : T.lam6) ca.max_terms = std::max(ca.max_terms, q.nterms);
     ca.ctas = P->d_ctas.as<CtaPlan>();
     ca.ncta = (int)P->ctas.size();
     ca.cta_smem = P->cta_smem;
@@ -552,7 +556,8 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
         return ENCORE_EALLOC;
     }
     P->fp32_harmonics = (flags & ENCORE_FP32_HARMONICS) != 0;
-    if (npcf_order >= 4 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
+    if (npcf_order >= 4 && npcf_order <= 5 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
+    if (npcf_order == 6 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas6(P->T, P->ctas);
     *plan_out = P;
     return ENCORE_OK;
 }
@@ -754,7 +759,7 @@ int encore_compute_host(encore_plan_t *P, const double *positions, const double 
 int encore_destroy(encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
-    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_ycoef, &P->d_pair_terms, &P->d_lam4, &P->d_lam5,
+    DevBuf *bufs[] = {&P->d_terms, &P->d_term_start, &P->d_bin_tuples, &P->d_ynorm, &P->d_ycoef, &P->d_pair_terms, &P->d_lam4, &P->d_lam5, &P->d_lam6,
                       &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->d_ctas, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
@@ -816,6 +821,8 @@ int encore_contraction_flops(const encore_plan_t *P, double *executed, double *c
         auto c2 = [](int n) { return n * (n - 1) / 2; };
         if (N == 3) { // per real component: nb scalings + one FMA per bin pair
             ex = (double)T.ncomp * (nb + 2.0 * (nb * (nb - 1) / 2));
+        } else if (N == 6) {
+            ex = contraction6_flops(T);
         } else if (N == 4) {
             for (const Lam4 &q : T.lam4)
                 for (int b1 = 0; b1 + 2 < nb; ++b1) {

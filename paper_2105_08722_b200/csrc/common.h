@@ -56,6 +56,21 @@ struct Lam5 {
     int nterms;
 };
 
+// N=6 multiplet for the factorised contraction (contract6.cu):  H_i = sum_{m123>=0} Re[ T_{m123}(b1,b2,b3) R45_{m123}(b4,b5) ],
+//   U_m(b1,b2)   = sum_{m1+m2=m} (l1 l2 l12; m1 m2 -m) a~1 a~2,  m = 0..l12   (U_{-m} = (-1)^{l1+l2+l12+m} conj U_m)
+//   T_M(b1,b2,b3) = f_M sum_{m12+m3=M} (-1)^{l12-m12} (l12 l3 l123; m12 m3 -M) U~_{m12} a~3,
+//                   f_M = sqrt((2 l12+1)(2 l123+1)) (-1)^{l123-M} (2 - delta_M0)                      (eq. 5 with two intermediates)
+//   R45_M(b4,b5) = sum_{m4+m5=-M} (l123 l4 l5; M m4 m5) a~4 a~5
+// All three are PairTerm lists; the first factor of a T term is a component of U (2|m12| real part, 2|m12|+1 imaginary part).
+struct Lam6 {
+    int l1, l2, l12, l3, l123, l4, l5;
+    int odd;
+    int ubeg[14];       // U terms of m12: [ubeg[m], ubeg[m+1])     (l12 <= 12)
+    int tbeg[14];       // T terms of M                              (l123 <= 12)
+    int rbeg[14];       // R terms of M
+    int nterms;         // all of them, contiguous from ubeg[0]
+};
+
 // One CTA of the factorised N = 4, 5 kernels: its multiplets and the l-blocks of the a_lm tile they need (only those
 // are brought into shared memory; a block l is the (2l+1) x nbins x 32 doubles starting at component l^2).
 struct CtaPlan {
@@ -65,6 +80,7 @@ struct CtaPlan {
     int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged
     int tile;                       // doubles per tile buffer
     int nbuf;                       // 2: double-buffered, 1: single
+    int aux;                        // N = 6: largest l12 of the CTA's multiplets (sizes the per-warp U scratch)
 };
 
 struct HostTables {
@@ -84,6 +100,7 @@ struct HostTables {
     std::vector<PairTerm> pair_terms; // factorised contraction (N=4,5)
     std::vector<Lam4> lam4;
     std::vector<Lam5> lam5;
+    std::vector<Lam6> lam6;          // N = 6, only when every intermediate is <= 12 (empty otherwise: literal kernel)
     std::vector<int> lam_order;      // multiplets by decreasing work (launch order)
     int nLam() const { return width ? (int)multiplets.size() / width : 0; }
     int nB() const { return order > 1 ? (int)bin_tuples.size() / (order - 1) : 0; }

@@ -111,6 +111,7 @@ struct ContractArgs {
     const PairTerm *pair_terms; // device
     const Lam4 *lam4;           // device [nLam]
     const Lam5 *lam5;           // device [nLam]
+    const Lam6 *lam6;           // device [nLam] (factorised N = 6 only)
     const int *lam_order;       // device [nLam], heaviest first
     const int *lam_parity;      // device [nLam]: 1 = parity-odd multiplet (the stored value is Im zeta)
     const int *tuple_index;     // device [nbins^(N-1)]: index of the ordered tuple in bin_tuples, -1 if not ordered
@@ -129,6 +130,11 @@ void contraction_range5(int nbins, int w, int *lo, int *hi); // N = 5: second bi
 // multiplets -> CTAs of the factorised N = 4, 5 kernels; returns the dynamic shared memory of the launch (0: does not fit)
 size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas);
 cudaError_t launch_contraction(const ContractArgs &a, cudaStream_t s, int *launches);
+// factorised N = 6 (contract6.cu): shapes covered, host plan (dynamic shared memory, 0: not covered), executed flops, launch
+int contraction6_supported(int nbins, int lmax);
+size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas);
+double contraction6_flops(const HostTables &T);
+cudaError_t launch_contract6(const ContractArgs &a, cudaStream_t s);
 cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launches);
 
 // ---- edge.cu -------------------------------------------------------------------------------------------

@@ -224,6 +224,32 @@ void coupled_pair_terms(int la, int lb, int L, int msum, double factor, std::vec
     }
 }
 
+// Terms of f sum_{m12+m3=M} (-1)^{l12-m12} (l12 l3 l123; m12 m3 -M) U~_{m12} a~_{l3 m3}: the first factor is a coupled pair
+// U of (l1,l2,l12) stored for m12 >= 0 as components 2 m12 (real part), 2 m12 + 1 (imaginary part);
+// U~_{-m} = sigma (-1)^m conj(U_m), sigma = (-1)^{l1+l2+l12}.
+void coupled_triple_terms(int l12, int l3, int l123, int M, double f, int sigma_odd, std::vector<PairTerm> &out)
+{
+    for (int m12 = -l12; m12 <= l12; ++m12) {
+        const int m3 = M - m12;
+        if (std::abs(m3) > l3) continue;
+        double w = f * (((l12 - m12) & 1) ? -1.0 : 1.0) * encore_host_wigner3j(l12, l3, l123, m12, m3, -M);
+        if (std::fabs(w) < 1e-15) continue;
+        const int aa = std::abs(m12), ab = std::abs(m3);
+        const double ta = m12 < 0 ? -1.0 : 1.0, tb = m3 < 0 ? -1.0 : 1.0;
+        if (m12 < 0) { if (sigma_odd) w = -w; if (aa & 1) w = -w; }
+        if (m3 < 0 && (ab & 1)) w = -w;
+        PairTerm t{};
+        t.ia_re = 2 * aa; t.ia_im = 2 * aa + 1;
+        t.ib_re = ab == 0 ? 0 : 2 * ab - 1;
+        t.ib_im = ab == 0 ? t.ib_re : 2 * ab;
+        t.wrr = w;
+        t.wii = ab ? -w * ta * tb : 0.0;
+        t.wri = ab ? w * tb : 0.0;
+        t.wir = w * ta;
+        out.push_back(t);
+    }
+}
+
 void build_factorised(HostTables &t)
 {
     const int nL = t.nLam();
@@ -304,6 +330,37 @@ void build_factorised(HostTables &t)
             cost[iL] = (q.lbeg[q.l12 + 1] - q.lbeg[1]) + 0.5 * (q.lbeg[1] - q.lbeg[0]) + 3.0 * (q.rbeg[q.l12 + 1] - q.rbeg[1]) +
                        1.5 * (q.rbeg[1] - q.rbeg[0]) + (q.l12 + 1);
             t.lam5.push_back(q);
+        }
+    }
+    else if (t.order == 6) {
+        bool ok = true;
+        for (int iL = 0; iL < nL && ok; ++iL) ok = t.multiplets[(size_t)iL * 7 + 2] <= 12 && t.multiplets[(size_t)iL * 7 + 4] <= 12;
+        for (int iL = 0; iL < nL && ok; ++iL) {
+            const int *lam = &t.multiplets[(size_t)iL * 7];
+            Lam6 q{};
+            q.l1 = lam[0]; q.l2 = lam[1]; q.l12 = lam[2]; q.l3 = lam[3]; q.l123 = lam[4]; q.l4 = lam[5]; q.l5 = lam[6]; q.odd = t.parity[iL];
+            for (int m = 0; m <= q.l12; ++m) {
+                q.ubeg[m] = (int)t.pair_terms.size();
+                coupled_pair_terms(q.l1, q.l2, q.l12, m, 1.0, t.pair_terms);        // (l1 l2 l12; m1 m2 -m)
+                q.ubeg[m + 1] = (int)t.pair_terms.size();
+            }
+            for (int m = q.l12 + 1; m < 13; ++m) q.ubeg[m + 1] = q.ubeg[q.l12 + 1];
+            for (int M = 0; M <= q.l123; ++M) {
+                const double f = std::sqrt((2.0 * q.l12 + 1.0) * (2.0 * q.l123 + 1.0)) * (((q.l123 - M) & 1) ? -1.0 : 1.0) * (M == 0 ? 1.0 : 2.0);
+                q.tbeg[M] = (int)t.pair_terms.size();
+                coupled_triple_terms(q.l12, q.l3, q.l123, M, f, (q.l1 + q.l2 + q.l12) & 1, t.pair_terms);
+                q.tbeg[M + 1] = (int)t.pair_terms.size();
+            }
+            for (int M = q.l123 + 1; M < 13; ++M) q.tbeg[M + 1] = q.tbeg[q.l123 + 1];
+            for (int M = 0; M <= q.l123; ++M) {
+                q.rbeg[M] = (int)t.pair_terms.size();
+                coupled_pair_terms(q.l4, q.l5, q.l123, -M, 1.0, t.pair_terms);      // (l4 l5 l123; m4 m5 M) = (l123 l4 l5; M m4 m5)
+                q.rbeg[M + 1] = (int)t.pair_terms.size();
+            }
+            for (int M = q.l123 + 1; M < 13; ++M) q.rbeg[M + 1] = q.rbeg[q.l123 + 1];
+            q.nterms = q.rbeg[q.l123 + 1] - q.ubeg[0];
+            cost[iL] = (q.ubeg[q.l12 + 1] - q.ubeg[0]) + 2.0 * (q.tbeg[q.l123 + 1] - q.tbeg[0]) + (q.rbeg[q.l123 + 1] - q.rbeg[0]) + 2.0 * (q.l123 + 1);
+            t.lam6.push_back(q);
         }
     }
     t.lam_order.resize(nL);

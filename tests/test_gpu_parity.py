@@ -160,9 +160,11 @@ def test_paper_gpu_shapes_and_largest_factorised_shapes(E, oracle, order, nbins,
 
 
 @pytest.mark.parametrize("nbins,lmax,box,allparity,n", [(5, 2, 0.0, False, 160), (6, 1, 90.0, False, 200), (7, 1, 0.0, True, 120),
-                                                         (5, 3, 0.0, False, 70)])
+                                                         (5, 3, 0.0, False, 70), (8, 2, 0.0, False, 80), (8, 1, 90.0, True, 100),
+                                                         (6, 4, 0.0, False, 24), (9, 1, 0.0, False, 100)])
 def test_6pcf_matches_the_oracle(E, oracle, nbins, lmax, box, allparity, n):
-    """N = 6, two intermediates (eq. 5; 2 212 multiplets at lmax = 3)"""
+    """N = 6, two intermediates (eq. 5; 2 212 multiplets at lmax = 3).  5-8 bins and
+    lmax <= 4 run the factorised kernel (contract6.cu), 9 bins the literal eq. 44 kernel; the two are also compared directly."""
     rng = np.random.default_rng(6000 + 10 * nbins + lmax)
     pos = np.ascontiguousarray(rng.uniform(0, 90.0, (3, n)))
     w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.2, 0.8])
@@ -176,11 +178,20 @@ def test_6pcf_matches_the_oracle(E, oracle, nbins, lmax, box, allparity, n):
         z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
         assert E.encore_get_status(plan.h) == E.OK
         counts, _ = E.encore_get_bin_counts(plan.h, nbins)
+        ex_fact = E.encore_contraction_flops(plan.h)[0]
+        E.encore_set_option(plan.h, "generic_contract", 1)
+        z_lit = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+        ex_lit = E.encore_contraction_flops(plan.h)[0]
     assert (counts == o["bin_counts"]).all()
     expect = np.where(par[:, None], o["zeta_im"], o["zeta"])
     scale = max(np.abs(o["zeta"]).max(), np.abs(o["zeta_im"]).max())
     assert scale > 0
     assert np.abs(z - expect).max() <= TOL * scale
+    assert np.abs(z_lit - expect).max() <= TOL * scale
+    if 5 <= nbins <= 8 and lmax <= 4:
+        assert ex_fact < ex_lit         # the factorised kernel ran the first time (fewer executed flops by its own count)
+    else:
+        assert ex_fact == ex_lit
     if allparity:
         assert par.any() and np.abs(expect[par]).max() > 1e-6 * scale
 
