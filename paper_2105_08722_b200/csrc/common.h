@@ -80,7 +80,7 @@ struct CtaPlan {
     int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged
     int tile;                       // doubles per tile buffer
     int nbuf;                       // 2: double-buffered, 1: single
-    int aux;                        // N = 6: largest l12 of the CTA's multiplets (sizes the per-warp U scratch)
+    int scr[8];                     // N = 6: lam[w] = 2 * multiplet + warp role; offset (doubles) of warp w's U scratch
 };
 
 struct HostTables {

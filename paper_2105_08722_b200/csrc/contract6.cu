@@ -23,7 +23,7 @@
 
 namespace {
 
-constexpr int kWarps6 = 8, kSlots6 = 4;     // 4 multiplets x 2 warps per CTA (255 registers)
+constexpr int kWarps6 = 8;      // work units (multiplet, warp role) per CTA (255 registers)
 
 __host__ __device__ constexpr int tup6(int nb, int b3) { return c2(b3) * c2(nb - 1 - b3); }   // quintuples with third bin b3
 // third bins 2 .. T go to warp 0, T+1 .. NB-3 to warp 1
@@ -60,8 +60,8 @@ __host__ __device__ constexpr int ai6(int nb, int lo, int b1, int b2, int b3, in
     for (int b = lo; b < b3; ++b) s += tup6(nb, b);
     return s + pr6(nb, b3, b4, b5) * c2(b3) + c2(b2) + b1;
 }
-// doubles of U scratch of warp role w for intermediates up to l12max: [component 2m, 2m+1][pair][lane]
-__host__ __device__ constexpr int scratch6(int nb, int w, int l12max) { return (l12max + 1) * 2 * npu6(hi6(nb, w)) * 32; }
+// doubles of U scratch of warp role w of a multiplet with intermediate l12: [component 2m, 2m+1][pair][lane]
+__host__ __device__ constexpr int scratch6(int nb, int w, int l12) { return (l12 + 1) * 2 * npu6(hi6(nb, w)) * 32; }
 
 struct SlotU6 { __host__ __device__ constexpr int operator()(int x, int y) const { return pu6(x, y); } };
 template <int NB, int LO>
@@ -101,12 +101,11 @@ __device__ __forceinline__ void pair_sums6(double (&zr)[NZ], double (&zi)[NZ], c
 }
 
 template <int NB, int LO, int HI, int NACC>
-__device__ __forceinline__ void task6(double (&acc)[NACC], const Lam6 &L, int toff, double *scr, const double *p1, const double *p2,
+__device__ __forceinline__ void task6(double (&acc)[NACC], const Lam6 &L, const PairTerm *terms, double *scr, const double *p1, const double *p2,
                                       const double *p3, const double *p4, const double *p5, double wi)
 {
     if constexpr (LO <= HI && HI <= NB - 3) {
         constexpr int NPU = npu6(HI), NT = nt6(LO, HI), NPR = npr6(NB, LO), NB3 = HI - LO + 1, rs = NB * 32;
-        const PairTerm *terms = reinterpret_cast<const PairTerm *>(smem_c + toff) - L.ubeg[0];
         // (i) U_m(b1,b2), b1 < b2 <= HI-1, m = 0 .. l12 -> scratch [2m | 2m+1][pair][lane]
         for (int m = 0; m <= L.l12; ++m) {
             double zr[NPU], zi[NPU];
@@ -216,7 +215,7 @@ __device__ __forceinline__ void warp6(const ContractArgs &a, const CtaPlan &C, c
     for_each_group_tile(a, C, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
-        task6<NB, LO, HI, NACC>(acc, L, toff, smem_c + soff + lane, smem_c + t + o1, smem_c + t + o2, smem_c + t + o3, smem_c + t + o4,
+        task6<NB, LO, HI, NACC>(acc, L, reinterpret_cast<const PairTerm *>(smem_c + toff) - L.ubeg[0], smem_c + soff + lane, smem_c + t + o1, smem_c + t + o2, smem_c + t + o3, smem_c + t + o4,
                                 smem_c + t + o5, wi);
     });
     if (!have) return;
@@ -224,25 +223,25 @@ __device__ __forceinline__ void warp6(const ContractArgs &a, const CtaPlan &C, c
     if constexpr (LO <= HI) flush6<NB, LO, HI, NACC>(acc, a.tuple_index, out, lane);
 }
 
-// shared memory: [nbuf tile buffers][4 mbarriers (+pad to 8 doubles)][term lists of the 4 slots][U scratch of the 8 warps]
+// A CTA holds 8 work units (multiplet, warp role), dealt by decreasing cost so that the warps of a CTA - which advance tile
+// by tile together - carry about the same work.  shared memory: [nbuf tile buffers][4 mbarriers (+pad)][term lists of the 8 warps][U scratch of the 8 warps]
 template <int NB>
 __global__ void __launch_bounds__(kWarps6 * 32, 1) k_contract6(ContractArgs a)
 {
     __shared__ CtaPlan C;
     if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.y)[threadIdx.x];
     __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, slot = warp >> 1, w = warp & 1;
-    const int iLs = C.lam[slot];
-    const bool have = iLs >= 0;
-    const int iL = have ? iLs : 0;
+    const int warp = threadIdx.x >> 5;
+    const int unit = C.lam[warp];
+    const bool have = unit >= 0;
+    const int iL = have ? unit >> 1 : 0, role = have ? unit & 1 : 0;
     const Lam6 L = a.lam6[iL];
     const TilePipe tp = make_pipe(C);
-    const int toff = tp.bar + 8 + slot * 6 * a.max_terms;
-    const int s0 = scratch6(NB, 0, C.aux), s1 = scratch6(NB, 1, C.aux);
-    const int soff = tp.bar + 8 + kSlots6 * 6 * a.max_terms + slot * (s0 + s1) + (w ? s0 : 0);
-    if (have && w == 0) stage_terms(toff, a.pair_terms + L.ubeg[0], L.nterms, lane);
+    const int toff = tp.bar + 8 + warp * 6 * a.max_terms;           // every warp stages the term lists of its multiplet
+    const int soff = tp.bar + 8 + kWarps6 * 6 * a.max_terms + C.scr[warp];
+    if (have) stage_terms(toff, a.pair_terms + L.ubeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
-    if (w == 0) warp6<NB, 0>(a, C, tp, have, L, iL, toff, soff);
+    if (role == 0) warp6<NB, 0>(a, C, tp, have, L, iL, toff, soff);
     else warp6<NB, 1>(a, C, tp, have, L, iL, toff, soff);
 }
 
@@ -263,52 +262,71 @@ cudaError_t launch6(const ContractArgs &a, cudaStream_t s)
 
 int contraction6_supported(int nbins, int lmax) { return nbins >= 5 && nbins <= 8 && lmax >= 0 && lmax <= 4; }
 
-// Deal the multiplets (heaviest first) to CTAs of 4 slots while the l-blocks of all of them, their term lists and the U
-// scratch of the 8 warps (sized by the largest l12 in the CTA) fit the shared memory; returns the dynamic shared memory of
-// the launch (0: the factorised kernel does not cover this plan).
+// fp64 instructions of one group of unit (multiplet q, warp role w), the cost the units are sorted and packed by
+static double unit_cost6(int nb, const Lam6 &q, int w)
+{
+    const int lo = lo6(nb, w), hi = hi6(nb, w);
+    if (lo > hi || hi > nb - 3) return 0.0;
+    const double npu = npu6(hi), nt = nt6(lo, hi), npr = npr6(nb, lo), nb3 = hi - lo + 1;
+    double tup = 0;
+    for (int b = lo; b <= hi; ++b) tup += tup6(nb, b);
+    const double nu = q.ubeg[q.l12 + 1] - q.ubeg[0], ntt = q.tbeg[q.l123 + 1] - q.tbeg[0], nr = q.rbeg[q.l123 + 1] - q.rbeg[0], nM = q.l123 + 1;
+    return nu * (4.0 * (hi - 1) + 4.0 * npu + 6.0) + ntt * (4.0 * nb3 + 4.0 * nt + 2.0 * npu + 6.0) + nr * (4.0 * (nb - 2 - lo) + 4.0 * npr + 6.0) +
+           nM * (2.0 * tup + 2.0 * nt + 30.0) + 2.0 * npu * (q.l12 + 1);
+}
+
+// Deal the work units (multiplet, warp role), heaviest first, to CTAs of 8 warps while the l-blocks of all their multiplets
+// and the U scratch of the warps fit the shared memory; returns the dynamic shared memory of the launch (0: the factorised
+// kernel does not cover this plan).
 size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
 {
     ctas.clear();
     if (T.order != 6 || !contraction6_supported(T.nbins, T.lmax) || T.lam6.empty()) return 0;
     const int nb = T.nbins, nL = T.nLam();
-    size_t max_terms = 1;
-    for (const Lam6 &q : T.lam6) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
     const size_t blk = (size_t)nb * 32 * sizeof(double);
-    auto scratch_bytes = [&](int l12max) {
-        size_t s = 0;
+    auto scratch_doubles = [&](int w, int l12) {
         switch (nb) {
-        case 5: s = scratch6(5, 0, l12max) + scratch6(5, 1, l12max); break;
-        case 6: s = scratch6(6, 0, l12max) + scratch6(6, 1, l12max); break;
-        case 7: s = scratch6(7, 0, l12max) + scratch6(7, 1, l12max); break;
-        default: s = scratch6(8, 0, l12max) + scratch6(8, 1, l12max); break;
+        case 5: return scratch6(5, w, l12);
+        case 6: return scratch6(6, w, l12);
+        case 7: return scratch6(7, w, l12);
+        default: return scratch6(8, w, l12);
         }
-        return s * kSlots6 * sizeof(double);
     };
     auto tile_bytes = [&](unsigned mask) {
         size_t b = 0;
         for (int l = 0; l <= T.lmax; ++l) if (mask >> l & 1u) b += (size_t)(2 * l + 1) * blk;
         return b;
     };
-    const size_t fixed = 64 + (size_t)kSlots6 * max_terms * sizeof(PairTerm);
+    size_t max_terms = 1;
+    for (const Lam6 &q : T.lam6) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
+    const size_t fixed = 64 + (size_t)kWarps6 * max_terms * sizeof(PairTerm);
+    std::vector<std::pair<double, int>> units;
+    for (int iL = 0; iL < nL; ++iL)
+        for (int w = 0; w < 2; ++w) {
+            const double c = unit_cost6(nb, T.lam6[iL], w);
+            if (c > 0.0) units.push_back({c, 2 * iL + w});
+        }
+    std::stable_sort(units.begin(), units.end(), [](const std::pair<double, int> &x, const std::pair<double, int> &y) { return x.first > y.first; });
     std::vector<unsigned> masks;
-    std::vector<int> l12max;
-    int fill = kSlots6;
-    for (int k = 0; k < nL; ++k) {
-        const int iL = T.lam_order[k];
-        const Lam6 &q = T.lam6[iL];
+    std::vector<size_t> scr;
+    int fill = kWarps6;
+    for (const auto &u : units) {
+        const Lam6 &q = T.lam6[u.second >> 1];
         const unsigned m = (1u << q.l1) | (1u << q.l2) | (1u << q.l3) | (1u << q.l4) | (1u << q.l5);
-        if (tile_bytes(m) + fixed + scratch_bytes(q.l12) > kSmemLimit6) return 0;
-        if (fill == kSlots6 || tile_bytes(masks.back() | m) + fixed + scratch_bytes(std::max(l12max.back(), q.l12)) > kSmemLimit6) {
+        const size_t s = (size_t)scratch_doubles(u.second & 1, q.l12) * sizeof(double);
+        if (tile_bytes(m) + fixed + s > kSmemLimit6) { ctas.clear(); return 0; }
+        if (fill == kWarps6 || tile_bytes(masks.back() | m) + fixed + scr.back() + s > kSmemLimit6) {
             CtaPlan c{};
             for (int j = 0; j < 12; ++j) c.lam[j] = -1;
             ctas.push_back(c);
             masks.push_back(0u);
-            l12max.push_back(0);
+            scr.push_back(0);
             fill = 0;
         }
-        ctas.back().lam[fill++] = iL;
+        ctas.back().scr[fill] = (int)(scr.back() / sizeof(double));
+        ctas.back().lam[fill++] = u.second;
         masks.back() |= m;
-        l12max.back() = std::max(l12max.back(), q.l12);
+        scr.back() += s;
     }
     size_t smem = 0;
     for (size_t i = 0; i < ctas.size(); ++i) {
@@ -320,8 +338,7 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
             if (l <= T.lmax && (masks[i] >> l & 1u)) { c.bl[c.nblk++] = l; c.off[l] = off; off += (2 * l + 1) * nb * 32; }
         }
         c.tile = off;
-        c.aux = l12max[i];
-        const size_t tb = (size_t)off * sizeof(double), extra = fixed + scratch_bytes(l12max[i]);
+        const size_t tb = (size_t)off * sizeof(double), extra = fixed + scr[i];
         c.nbuf = 2 * tb + extra <= kSmemLimit6 ? 2 : 1;
         smem = std::max(smem, c.nbuf * tb + extra);
     }
