@@ -212,7 +212,7 @@ __device__ __forceinline__ void warp6(const ContractArgs &a, const CtaPlan &C, c
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    for_each_group_tile(a, C, tp, [&](int t, int g) {
+    for_each_group_tile<true>(a, C, tp, [&](int t, int g) {
         if (!have) return;
         const double wi = a.gweights[(size_t)g * 32 + lane];
         task6<NB, LO, HI, NACC>(acc, L, reinterpret_cast<const PairTerm *>(smem_c + toff) - L.ubeg[0], smem_c + soff + lane, smem_c + t + o1, smem_c + t + o2, smem_c + t + o3, smem_c + t + o4,
@@ -339,7 +339,8 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
         }
         c.tile = off;
         const size_t tb = (size_t)off * sizeof(double), extra = fixed + scr[i];
-        c.nbuf = 2 * tb + extra <= kSmemLimit6 ? 2 : 1;
+        c.nbuf = 1;     // as many tile buffers as fit, up to 4 (contract_tile.cuh)
+        for (int nbf = 2; nbf <= 4; ++nbf) if (nbf * tb + extra <= kSmemLimit6) c.nbuf = nbf;
         smem = std::max(smem, c.nbuf * tb + extra);
     }
     return smem;

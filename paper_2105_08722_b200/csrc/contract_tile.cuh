@@ -71,15 +71,17 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
 }
 
 struct TilePipe {
-    int buf[2];              // offsets into smem_c (doubles)
-    int bar;                 // offset of the two mbarriers
+    int buf[4];              // offsets into smem_c (doubles)
+    int bar;                 // offset of the mbarriers: full[4], empty[4]
     unsigned bytes;          // bytes of the staged l-blocks of one group
     int nbuf;
 };
 
 // Calls body(tile_in_smem, g) for the groups g = g_begin + blockIdx.x, + gridDim.x, ... < g_end (the chunk of this CTA).  Only the l-blocks the
 // CTA's multiplets need (CtaPlan) are copied: one bulk copy per block, all completing on the buffer's mbarrier.
-template <class Body>
+// RING: the plan may ask for 3-4 buffers (k_contract6; the N = 4, 5 plans stay at two: their heavy tiles leave no room and a
+// third copy of their fully unrolled bodies costs more than the light CTAs gain).
+template <bool RING = false, class Body>
 __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, Body body)
 {
     const int ngroups = group_end(a);
@@ -97,13 +99,37 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
             bulk_copy(smem_c + tp.buf[buf] + C.off[l], src + (size_t)l * l * rs, (unsigned)((2 * l + 1) * rs * sizeof(double)), &bar[buf]);
         }
     };
+    if (RING && tp.nbuf > 2) {
+        // a ring of 3-4 buffers: "full" barriers carry the copies, "empty" barriers (one arrival per warp) say that every warp
+        // is done with a buffer.  Tile k + nbuf - 1 is requested while tile k is contracted (light CTAs finish a tile faster
+        // than a copy takes to arrive: one tile of look-ahead left them waiting for data).  Only the issuing thread waits for
+        // the other warps (before it refills the buffer they used one tile ago); nobody else waits on anything but data, so
+        // the warps drift by up to a tile instead of meeting at a CTA barrier after every group.
+        const int nbuf = tp.nbuf;
+        unsigned long long *empty = bar + 4;
+        const int lane = threadIdx.x & 31;
+        if (issuer)
+            for (int j = 0; j < nbuf - 1 && g + j * stride < ngroups; ++j) load(j, g + j * stride);
+        int st = 0, use = 0;                            // tile k sits in buffer st = k % nbuf, as that buffer's use-th tile
+        for (int k = 0; g < ngroups; ++k, g += stride) {
+            if (issuer && g + (nbuf - 1) * stride < ngroups) {
+                const int sb = st == 0 ? nbuf - 1 : st - 1;     // (k + nbuf - 1) % nbuf: the buffer of tile k - 1
+                const int ub = st == 0 ? use : use + 1;         // (k + nbuf - 1) / nbuf
+                if (ub >= 1) mbar_wait(&empty[sb], (unsigned)((ub - 1) & 1));
+                load(sb, g + (nbuf - 1) * stride);
+            }
+            mbar_wait(&bar[st], (unsigned)(use & 1));
+            body(tp.buf[st], g);
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&empty[st])) : "memory");
+            if (++st == nbuf) { st = 0; ++use; }
+        }
+        return;
+    }
     if (issuer && g < ngroups) load(0, g);
     if (tp.nbuf == 2) {
-        // two buffers: "full" barriers carry the copies, "empty" barriers (one arrival per warp) say that every warp is done
-        // with a buffer.  Only the issuing thread waits for the other warps (before it refills the buffer they used one
-        // tile ago); nobody else waits on anything but data, so the warps drift by up to one tile instead of meeting at a
-        // CTA barrier after every group.
-        unsigned long long *empty = bar + 2;
+        // two buffers (the tiles of the heavy CTAs are too large for more): the same scheme with one tile of look-ahead
+        unsigned long long *empty = bar + 4;
         const int lane = threadIdx.x & 31;
         for (int k = 0; g < ngroups; ++k, g += stride) {
             const int st = k & 1;
@@ -127,21 +153,20 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
     }
 }
 
-// shared memory: [nbuf tile buffers][4 mbarriers (+pad to 8 doubles)][term lists of the CTA's multiplets]
+// shared memory: [nbuf tile buffers][8 mbarriers = 8 doubles][term lists of the CTA's multiplets]
 __device__ __forceinline__ TilePipe make_pipe(const CtaPlan &C)
 {
     TilePipe tp;
-    tp.buf[0] = 0;
-    tp.buf[1] = C.nbuf == 2 ? C.tile : 0;
+    for (int i = 0; i < 4; ++i) tp.buf[i] = i < C.nbuf ? i * C.tile : 0;
     tp.bar = C.nbuf * C.tile;
     tp.bytes = (unsigned)(C.tile * sizeof(double));
     tp.nbuf = C.nbuf;
     if (threadIdx.x == 0) {
         unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
-        mbar_init(&bar[0], 1);
-        mbar_init(&bar[1], 1);
-        mbar_init(&bar[2], blockDim.x / 32);   // "empty" barriers: one arrival per warp
-        mbar_init(&bar[3], blockDim.x / 32);
+        for (int i = 0; i < 4; ++i) {
+            mbar_init(&bar[i], 1);                      // "full": the issuing thread's expect_tx arrival
+            mbar_init(&bar[4 + i], blockDim.x / 32);    // "empty": one arrival per warp
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     return tp; // the caller's __syncthreads (after it has copied its term list) publishes the barriers
