@@ -57,12 +57,12 @@ enum {
 /* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
  * S(0) = 1/2, else 1), bin edges, 1/v_b, Y_lm normalisations.  Host work only; device tables are uploaded by the
  * first encore_compute on the then-current device.
- *   npcf_order  N in {3,4,5,6}  (N = 6: Lam = {l1 l2 (l12) l3 (l123) l4 l5}, eq. 5 with two intermediates, PAPER.md:69, :161;
- *               contracted by the literal eq. 44 kernel, one warp per (Lam, B))
+ *   npcf_order  N in {3,4,5,6}  (N = 6: Lam = {l1 l2 (l12) l3 (l123) l4 l5}, eq. 5 with two intermediates)
  *   r_min,r_max 0 <= r_min < r_max
  *   nbins       N_r >= N-1 and <= 32
  *   lmax        0..10 (ENCORE_EUNSUPPORTED above).  The factorised contraction kernels cover N=3, nbins <= 10;
- *               N=4, nbins <= 10; N=5, nbins <= 10 and lmax <= 5; other shapes run the literal eq. 44 kernel
+ *               N=4, nbins <= 10; N=5, nbins <= 10 and lmax <= 5; N=6, 5 <= nbins <= 8 and lmax <= 4; other shapes run the
+ *               literal eq. 44 kernel (one warp per (Lam, B) at a time)
  *   box_size    > 0: periodic cube [0,L)^3 (PERIODIC mode), needs r_max <= L/2;  0: open geometry
  */
 int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
