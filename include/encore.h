@@ -61,7 +61,7 @@ enum {
  *   r_min,r_max 0 <= r_min < r_max
  *   nbins       N_r >= N-1 and <= 32
  *   lmax        0..10 (ENCORE_EUNSUPPORTED above).  The factorised contraction kernels cover N=3, nbins <= 10;
- *               N=4, nbins <= 10; N=5, nbins <= 10 and lmax <= 5; N=6, 5 <= nbins <= 8 and lmax <= 4; other shapes run the
+ *               N=4, nbins <= 10; N=5, nbins <= 10 and lmax <= 5; N=6, 5 <= nbins <= 10 and lmax <= 4; other shapes run the
  *               literal eq. 44 kernel (one warp per (Lam, B) at a time)
  *   box_size    > 0: periodic cube [0,L)^3 (PERIODIC mode), needs r_max <= L/2;  0: open geometry
  */

@@ -80,7 +80,7 @@ struct CtaPlan {
     int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged
     int tile;                       // doubles per tile buffer
     int nbuf;                       // tile buffers of the ring: 1 (single) .. 4
-    int scr[8];                     // N = 6: lam[w] = 2 * multiplet + warp role; offset (doubles) of warp w's U scratch
+    int scr[8];                     // N = 6: lam[w] = 8 * multiplet + warp role; offset (doubles) of warp w's U scratch
 };
 
 struct HostTables {

@@ -38,8 +38,42 @@ __host__ __device__ constexpr int t6(int nb)
     }
     return best;
 }
-__host__ __device__ constexpr int lo6(int nb, int w) { return w == 0 ? 2 : t6(nb) + 1; }
-__host__ __device__ constexpr int hi6(int nb, int w) { return w == 0 ? t6(nb) : nb - 3; }
+// Up to 8 bins: two warp roles per multiplet, third bins 2..T and T+1..NB-3.  9 and 10 bins (126 / 252 quintuples): contiguous
+// ranges grown greedily while partial sums + T + R45 + the pre-weighted operands of a term stay under 110 doubles
+// (4 and 6 roles).
+__host__ __device__ constexpr int regs6(int nb, int lo, int hi)
+{
+    int acc = 0, nt = 0;
+    for (int b = lo; b <= hi; ++b) { acc += tup6(nb, b); nt += c2(b); }
+    int ny = nb - 2 - lo;
+    if (hi - lo + 1 > ny) ny = hi - lo + 1;
+    if (hi - 1 > ny) ny = hi - 1;
+    return acc + 2 * nt + 2 * c2(nb - 1 - lo) + 4 * ny;
+}
+constexpr int kMaxRoles6 = 8;
+struct Part6 { int n; int lo[kMaxRoles6], hi[kMaxRoles6]; };
+__host__ __device__ constexpr Part6 make_part6(int nb)
+{
+    Part6 p{};
+    for (int w = 0; w < kMaxRoles6; ++w) { p.lo[w] = 3; p.hi[w] = 2; }
+    if (nb <= 8) {
+        p.n = 2;
+        p.lo[0] = 2; p.hi[0] = t6(nb); p.lo[1] = t6(nb) + 1; p.hi[1] = nb - 3;
+        return p;
+    }
+    int lo = 2, w = 0;
+    while (lo <= nb - 3 && w < kMaxRoles6) {
+        int hi = lo;
+        while (hi + 1 <= nb - 3 && regs6(nb, lo, hi + 1) <= 110) ++hi;
+        p.lo[w] = lo; p.hi[w] = hi;
+        lo = hi + 1; ++w;
+    }
+    p.n = w;
+    return p;
+}
+__host__ __device__ constexpr int nw6(int nb) { return make_part6(nb).n; }
+__host__ __device__ constexpr int lo6(int nb, int w) { return make_part6(nb).lo[w]; }
+__host__ __device__ constexpr int hi6(int nb, int w) { return make_part6(nb).hi[w]; }
 
 // index spaces of a warp whose third bins are LO..HI
 __host__ __device__ constexpr int npu6(int hi) { return hi >= 2 ? c2(hi) : 0; }                       // pairs b1 < b2 <= HI-1
@@ -223,6 +257,13 @@ __device__ __forceinline__ void warp6(const ContractArgs &a, const CtaPlan &C, c
     if constexpr (LO <= HI) flush6<NB, LO, HI, NACC>(acc, a.tuple_index, out, lane);
 }
 
+template <int NB, int W>
+__device__ __forceinline__ void dispatch6(int role, const ContractArgs &a, const CtaPlan &C, const TilePipe &tp, bool have, const Lam6 &L, int iL, int toff, int soff)
+{
+    if (role == W) warp6<NB, W>(a, C, tp, have, L, iL, toff, soff);
+    else if constexpr (W + 1 < nw6(NB)) dispatch6<NB, W + 1>(role, a, C, tp, have, L, iL, toff, soff);
+}
+
 // A CTA holds 8 work units (multiplet, warp role), dealt by decreasing cost so that the warps of a CTA - which advance tile
 // by tile together - carry about the same work.  shared memory: [nbuf tile buffers][4 mbarriers (+pad)][term lists of the 8 warps][U scratch of the 8 warps]
 template <int NB>
@@ -234,15 +275,14 @@ __global__ void __launch_bounds__(kWarps6 * 32, 1) k_contract6(ContractArgs a)
     const int warp = threadIdx.x >> 5;
     const int unit = C.lam[warp];
     const bool have = unit >= 0;
-    const int iL = have ? unit >> 1 : 0, role = have ? unit & 1 : 0;
+    const int iL = have ? unit >> 3 : 0, role = have ? unit & 7 : 0;
     const Lam6 L = a.lam6[iL];
     const TilePipe tp = make_pipe(C);
     const int toff = tp.bar + 8 + warp * 6 * a.max_terms;           // every warp stages the term lists of its multiplet
     const int soff = tp.bar + 8 + kWarps6 * 6 * a.max_terms + C.scr[warp];
     if (have) stage_terms(toff, a.pair_terms + L.ubeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
-    if (role == 0) warp6<NB, 0>(a, C, tp, have, L, iL, toff, soff);
-    else warp6<NB, 1>(a, C, tp, have, L, iL, toff, soff);
+    dispatch6<NB, 0>(role, a, C, tp, have, L, iL, toff, soff);
 }
 
 constexpr size_t kSmemLimit6 = 224 * 1024;
@@ -260,7 +300,7 @@ cudaError_t launch6(const ContractArgs &a, cudaStream_t s)
 
 } // namespace
 
-int contraction6_supported(int nbins, int lmax) { return nbins >= 5 && nbins <= 8 && lmax >= 0 && lmax <= 4; }
+int contraction6_supported(int nbins, int lmax) { return nbins >= 5 && nbins <= 10 && lmax >= 0 && lmax <= 4; }
 
 // fp64 instructions of one group of unit (multiplet q, warp role w), the cost the units are sorted and packed by
 static double unit_cost6(int nb, const Lam6 &q, int w)
@@ -289,7 +329,9 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
         case 5: return scratch6(5, w, l12);
         case 6: return scratch6(6, w, l12);
         case 7: return scratch6(7, w, l12);
-        default: return scratch6(8, w, l12);
+        case 8: return scratch6(8, w, l12);
+        case 9: return scratch6(9, w, l12);
+        default: return scratch6(10, w, l12);
         }
     };
     auto tile_bytes = [&](unsigned mask) {
@@ -302,18 +344,18 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
     const size_t fixed = 64 + (size_t)kWarps6 * max_terms * sizeof(PairTerm);
     std::vector<std::pair<double, int>> units;
     for (int iL = 0; iL < nL; ++iL)
-        for (int w = 0; w < 2; ++w) {
+        for (int w = 0; w < nw6(nb); ++w) {
             const double c = unit_cost6(nb, T.lam6[iL], w);
-            if (c > 0.0) units.push_back({c, 2 * iL + w});
+            if (c > 0.0) units.push_back({c, 8 * iL + w});
         }
     std::stable_sort(units.begin(), units.end(), [](const std::pair<double, int> &x, const std::pair<double, int> &y) { return x.first > y.first; });
     std::vector<unsigned> masks;
     std::vector<size_t> scr;
     int fill = kWarps6;
     for (const auto &u : units) {
-        const Lam6 &q = T.lam6[u.second >> 1];
+        const Lam6 &q = T.lam6[u.second >> 3];
         const unsigned m = (1u << q.l1) | (1u << q.l2) | (1u << q.l3) | (1u << q.l4) | (1u << q.l5);
-        const size_t s = (size_t)scratch_doubles(u.second & 1, q.l12) * sizeof(double);
+        const size_t s = (size_t)scratch_doubles(u.second & 7, q.l12) * sizeof(double);
         if (tile_bytes(m) + fixed + s > kSmemLimit6) { ctas.clear(); return 0; }
         if (fill == kWarps6 || tile_bytes(masks.back() | m) + fixed + scr.back() + s > kSmemLimit6) {
             CtaPlan c{};
@@ -351,7 +393,7 @@ double contraction6_flops(const HostTables &T)
 {
     const int nb = T.nbins;
     double ex = 0.0;
-    for (int w = 0; w < 2; ++w) {
+    for (int w = 0; w < nw6(nb); ++w) {
         const int lo = lo6(nb, w), hi = hi6(nb, w);
         if (lo > hi || hi > nb - 3) continue;
         const double npu = npu6(hi), nt = nt6(lo, hi), npr = npr6(nb, lo), nb3 = hi - lo + 1;
@@ -375,6 +417,8 @@ cudaError_t launch_contract6(const ContractArgs &a, cudaStream_t s)
     case 6: return launch6<6>(a, s);
     case 7: return launch6<7>(a, s);
     case 8: return launch6<8>(a, s);
+    case 9: return launch6<9>(a, s);
+    case 10: return launch6<10>(a, s);
     }
     return cudaErrorInvalidValue;
 }
