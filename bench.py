@@ -43,7 +43,7 @@ import workloads as W  # noqa: E402
 SM_COUNT, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this
 # round's kernels (profiles/r2_ncu_full_c3.txt and r2_ncu_full_c5.txt name the commands); None where not captured
-NCU_DRAM_BYTES = {"c3": {"k_fill": 1.948e9, "k_harm": 2.953e9, "k_contract": 9.622e9}, "c5": {"k_contract": 10.125e9}}
+NCU_DRAM_BYTES = {"c3": {"k_fill": 1.947e9, "k_harm": 2.958e9, "k_contract": 9.587e9}, "c5": {"k_contract": 9.243e9}}
 NCU_PROFILE = "profiles/r2_ncu_full_c3.txt"
 
 
@@ -431,6 +431,7 @@ def main():
     ap.add_argument("--all-configs", action="store_true", help="(default now) kept for compatibility")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--allparity", action="store_true", help="ALLPARITY plan: parity-odd multiplets too (not the headline config)")
+    ap.add_argument("--only-next-rows", action="store_true", help="measure and print only `next_rows` (6PCF, edge correction, gridded estimator)")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]
     if args.impl == "reference":
@@ -454,6 +455,10 @@ def main():
     steps, warmup = args.steps, max(3, args.warmup)
     fp64_peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6
     fp32_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6
+    if args.only_next_rows:
+        if rank == 0:
+            print(json.dumps({"next_rows": measure_next_rows(E, torch, dev, fp64_peak)}))
+        return
 
     with ClockSampler(local) as clocks:
         res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev, allparity=args.allparity,
