@@ -44,7 +44,7 @@ struct encore_plan_s {
     // scratch
     DevBuf cid, cell_count, cell_fill, cell_start, scan_tmp, tmp_idx, sorted_idx, pos4, groups, group_start;
     DevBuf alm, counts, partial, partial2, bbox_tmp, bbox, flags, cand, bincounts, alm_export;
-    DevBuf io_pos, io_w, io_zeta;
+    DevBuf io_pos, io_w, io_zeta, pos4f;
     DevBuf gbound, gprefix, gwide, rows, rowdesc, rowcnt, errflag;
     DevBuf mesh_fd, mesh_kern;          // gridded estimator: F[delta h^3] and the kernel / a_lm field being transformed
     int mesh_fft = -1, mesh_G = 0;      // cuFFT plan for G^3
@@ -392,6 +392,19 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
         }
         pa.pad_r2max = r2;
         CU(launch_set_particle(P->pos4.as<double4>() + n, far[0], far[1], far[2], 0.0, s, &P->launches));
+        if (P->fp32_harmonics) {
+            // 16-byte candidate records relative to the centre of the box / bounding box; used for the bins whose lower edge
+            // is at least 2^-10 of the largest such coordinate (fp32 then resolves every accepted separation to < 2^-13)
+            double cmax = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                pa.ctr[a] = G.periodic ? 0.5 * T.box : 0.5 * (bb[a] + bb[3 + a]);
+                cmax = std::max(cmax, G.periodic ? 0.5 * T.box : 0.5 * (bb[3 + a] - bb[a]));
+            }
+            pa.gf_min_r2 = (cmax / 1024.0) * (cmax / 1024.0);
+            ENS(P->pos4f, sizeof(float4) * ((size_t)n + 1));
+            pa.pos4f = P->pos4f.as<float4>();
+            CU(launch_make_pos4f(P->pos4.as<double4>(), n + 1, pa.ctr, P->pos4f.as<float4>(), s, &P->launches));
+        }
     }
     pa.cell_start = P->cell_start.as<int>();
     pa.group_start = P->group_start.as<int>();
@@ -763,7 +776,7 @@ int encore_destroy(encore_plan_t *P)
                       &P->d_lam_order, &P->d_lam_parity, &P->d_tuple_index, &P->d_ctas, &P->gweights, &P->cid, &P->cell_count, &P->cell_fill,
                       &P->cell_start, &P->scan_tmp, &P->tmp_idx, &P->sorted_idx, &P->pos4, &P->groups, &P->group_start,
                       &P->alm, &P->counts, &P->partial, &P->partial2, &P->bbox_tmp, &P->bbox, &P->flags, &P->cand,
-                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->gbound, &P->gprefix, &P->gwide,
+                      &P->bincounts, &P->alm_export, &P->io_pos, &P->io_w, &P->io_zeta, &P->pos4f, &P->gbound, &P->gprefix, &P->gwide,
                       &P->rows, &P->rowdesc, &P->rowcnt, &P->errflag, &P->d_gaunt, &P->edge_A, &P->edge_rhs, &P->mesh_fd, &P->mesh_kern};
     for (DevBuf *b : bufs) b->release();
     if (P->pinned) cudaFreeHost(P->pinned);

@@ -47,6 +47,7 @@ cudaError_t launch_exclusive_scan(const int *in, int *out, int m, int *tmp, cuda
 cudaError_t launch_sort_gather(const double *pos, const double *w, int64_t n, const int32_t *cid,
                                const int *cell_start, int *cell_fill, int *tmp_idx, int *sorted_idx,
                                double4 *pos4, cudaStream_t s, int *launches);
+cudaError_t launch_make_pos4f(const double4 *pos4, int64_t count, const double ctr[3], float4 *pos4f, cudaStream_t s, int *launches);
 cudaError_t launch_pencil_groups(const int *cell_start, GridGeom g, int *groups_per_pencil, cudaStream_t s,
                                  int *launches);
 
@@ -62,6 +63,9 @@ struct PairArgs {
     double rmax;
     int lmax, ncomp;
     int fp32_harmonics;         // ENCORE_FP32_HARMONICS: k_harm evaluates the weighted harmonics in fp32 (fp64 accumulation)
+    const float4 *pos4f;        // ENCORE_FP32_HARMONICS: {x - c, y - c, z - c, w} of pos4 rounded to fp32 (c = ctr: box / bounding-box centre)
+    double ctr[3];
+    double gf_min_r2;           // bins whose lower edge^2 is at least this gather pos4f (16 B per candidate) instead of pos4
     const double *ynorm;        // [ncomp] device
     const double *ycoef;        // [ncomp][lmax+1] device: Y_lm = sum_k ycoef[c][k] z^k (x+iy)^m
     double *alm;                // [ngroups][ncomp][nbins][32]

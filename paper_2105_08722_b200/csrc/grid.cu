@@ -196,12 +196,28 @@ __global__ void k_bbox_check(const double *__restrict__ bbox, double lx, double 
     }
 }
 
+// fp32-harmonics variant: candidate records of 16 instead of 32 bytes (the gather of k_harm is bound by L1 bytes)
+__global__ void k_make_pos4f(const double4 *__restrict__ pos4, int64_t count, double cx, double cy, double cz, float4 *__restrict__ out)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const double4 p = pos4[i];
+    out[i] = make_float4((float)(p.x - cx), (float)(p.y - cy), (float)(p.z - cz), (float)p.w);
+}
+
 __global__ void k_set_particle(double4 *dst, double x, double y, double z, double w)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) *dst = make_double4(x, y, z, w);
 }
 
 } // namespace
+
+cudaError_t launch_make_pos4f(const double4 *pos4, int64_t count, const double ctr[3], float4 *pos4f, cudaStream_t s, int *launches)
+{
+    k_make_pos4f<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, s>>>(pos4, count, ctr[0], ctr[1], ctr[2], pos4f);
+    *launches += 1;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_set_particle(double4 *dst, double x, double y, double z, double w, cudaStream_t s, int *launches)
 {

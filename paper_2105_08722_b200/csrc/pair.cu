@@ -32,6 +32,7 @@
 #include <algorithm>
 #include <climits>
 #include <mutex>
+#include <type_traits>
 
 namespace {
 
@@ -52,6 +53,7 @@ constexpr int kHarmWarps = ENCORE_HARM_WARPS;       // k_harm: independent warps
 #define ENCORE_HARM_QUEUE 32
 #endif
 constexpr int kQueue = ENCORE_HARM_QUEUE;           // k_harm: (mask, descriptor) records queued per lane (power of two)
+constexpr int kQueueF32 = 16;                       // fp32-harmonics variant: its fp64 accumulators take the shared memory (3 CTAs per SM)
 constexpr int kStageRows = 8;                       // k_harm: rows per cp.async chunk (two chunks in flight)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoHit = 254u;
@@ -562,13 +564,18 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // CAREFUL: the bin reaches outside fp32's comfortable range for r^2 (r_min = 0, or extreme units): library rsqrt.
 struct HarmStats { unsigned steps; };
 
-template <int LMAX, int MLO, int MHI, int MODE, int D, bool CAREFUL, bool F32>
+// GF (fp32-harmonics variant only): the candidates are gathered from pos4f, 16-byte fp32 records relative to the centre of
+// the box (half the L1 bytes of the gather, no conversions), the separation is formed in fp32; mef = this primary in the
+// same coordinates, mtab then holds floats.
+template <int LMAX, int MLO, int MHI, int MODE, int D, bool CAREFUL, bool F32, bool GF = false>
 __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, MLO, MHI)], const unsigned *__restrict__ rows,
                                               const unsigned *__restrict__ rdesc, int nrows, bool active, uint2 *q,
                                               unsigned *stm, unsigned *std_, const double4 *__restrict__ pos4,
                                               const double4 &me, const double *mtab, double box, double half, int lane,
-                                              unsigned padent, HarmStats &st)
+                                              unsigned padent, HarmStats &st, const float4 *__restrict__ pos4f = nullptr,
+                                              float3 mef = make_float3(0.f, 0.f, 0.f), double *sacc = nullptr)
 {
+    static_assert(!GF || (F32 && !CAREFUL), "fp32 candidate records belong to the fp32-harmonics variant");
     static_assert(D >= 1 && D <= 4 && 4 % D == 0, "four steps per loop trip use the D gather slots in turn");
     // ---- rows -> shared memory: a ring of 2 chunks of kStageRows rows, both in flight (every chunk slot commits one
     // cp.async group, empty or not).  A chunk is kStageRows * 128 contiguous bytes: 16 bytes per lane and copy.
@@ -591,7 +598,8 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
     issue_chunk(1);
     int rows_done = 0;
     // lane-private queue cursors as byte offsets into the lane's column of q (stride 256 bytes per record)
-    constexpr unsigned kQBytes = kQueue * 256u;
+    constexpr int QN = F32 ? kQueueF32 : kQueue;
+    constexpr unsigned kQBytes = QN * 256u;
     unsigned head = 0u, tail = 0u, level = 0u;
     char *const qcol = reinterpret_cast<char *>(q + lane);
     int avail = 0;                      // pairs queued and not yet generated (bits of cur + bits of the queued masks)
@@ -600,7 +608,7 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
     bool drained = false;
     // push rows while every lane has room for one more record; returns the number of steps to run next (0: finished)
     auto refill = [&]() -> int {
-        int room = kQueue - __reduce_max_sync(kFull, (int)level);
+        int room = QN - __reduce_max_sync(kFull, (int)level);
         while (room > 0 && rows_done < nrows) {
             const int k0 = rows_done & (kStageRows - 1);
             if (k0 == 0) { cp_async_wait<1>(); __syncwarp(); }
@@ -659,14 +667,21 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
 #endif
         return 0u;
     }
-    Raw r[D];
+    using RawT = std::conditional_t<GF, float4, Raw>;
+    RawT r[D];
     unsigned ent[D];
+    auto fetch = [&](unsigned idx) -> RawT {
+        if constexpr (GF) return __ldg(pos4f + idx);
+        else return gather(pos4, idx);
+    };
 #pragma unroll
     for (int d = 0; d < D; ++d) {
         ent[d] = gen();
-        r[d] = gather(pos4, ent[d] & kIdxMask);
+        r[d] = fetch(ent[d] & kIdxMask);
     }
-    // F32: fp32 chunk sums, added to the fp64 accumulators every four loop trips (16 pairs)
+    // F32: fp32 chunk sums, added every eight loop trips (32 pairs) to the fp64 accumulators, which sit in shared memory
+    // (sacc, this thread's column, stride = threads of the CTA): in registers they held the kernel at 219 registers and
+    // 8 warps per SM
     constexpr int NACCF = F32 ? ncomp_range(LMAX, MLO, MHI) : 1;
     float facc[NACCF];
 #pragma unroll
@@ -675,7 +690,7 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
     auto flush_f32 = [&]() {
         if constexpr (F32) {
 #pragma unroll
-            for (int k = 0; k < NACCF; ++k) { acc[k] += (double)facc[k]; facc[k] = 0.f; }
+            for (int k = 0; k < NACCF; ++k) { sacc[k * (kHarmWarps * 32)] += (double)facc[k]; facc[k] = 0.f; }
         }
     };
     // MODE 1: byte address of this thread's column of mtab; the image code of an axis selects one of three rows
@@ -687,6 +702,33 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 // everything that reads slot u first, so that the next gather can land in the same registers
+                if constexpr (GF) {
+                    float fx, fy, fz;
+                    constexpr unsigned kRowF = kRowB / 2;       // bytes per row of the float table
+                    if (MODE == 1) {
+                        const unsigned c0 = ent[u % D];
+                        fx = r[u % D].x - *reinterpret_cast<const float *>(mcol + (((c0 >> 26) & 3u) * kRowF));
+                        fy = r[u % D].y - *reinterpret_cast<const float *>(mcol + 4 * kRowF + (((c0 >> 28) & 3u) * kRowF));
+                        fz = r[u % D].z - *reinterpret_cast<const float *>(mcol + 8 * kRowF + ((c0 >> 30) * kRowF));
+                    } else {
+                        fx = r[u % D].x - mef.x; fy = r[u % D].y - mef.y; fz = r[u % D].z - mef.z;
+                        if (MODE == 2) {
+                            const float bf = (float)box, hf = (float)half;
+                            if (fx > hf) fx -= bf; else if (fx < -hf) fx += bf;
+                            if (fy > hf) fy -= bf; else if (fy < -hf) fy += bf;
+                            if (fz > hf) fz -= bf; else if (fz < -hf) fz += bf;
+                        }
+                    }
+                    const float wf = r[u % D].w;
+                    ent[u % D] = gen();
+                    r[u % D] = fetch(ent[u % D] & kIdxMask);
+                    const float r2f = fmaxf(fmaf(fz, fz, fmaf(fy, fy, fx * fx)), 1e-30f);
+                    float y0;
+                    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(r2f));
+                    const float h = 0.5f * y0;
+                    const float rinvf = fmaf(h, fmaf(-r2f * y0, y0, 1.f), y0); // one Newton step: ~1 ulp
+                    accumulate<LMAX, MLO, MHI, float>(facc, fx * rinvf, fy * rinvf, fz * rinvf, wf);
+                } else {
                 double dx, dy, dz;
                 if (MODE == 1) {
                     const unsigned c0 = ent[u % D];
@@ -701,7 +743,7 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
                 }
                 const double wj = r[u % D].zw.y;
                 ent[u % D] = gen();
-                r[u % D] = gather(pos4, ent[u % D] & kIdxMask); // D candidates ahead
+                r[u % D] = fetch(ent[u % D] & kIdxMask); // D candidates ahead
                 if constexpr (F32) {
                     // fp32 harmonics: the separation is formed in fp64 (positions are large, separations small) and
                     // rounded once; unit vector, powers and (x+iy)^m in fp32.  CAREFUL bins keep the fp64 normalisation.
@@ -724,8 +766,9 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
                     const double rinv = CAREFUL ? rsqrt(r2s) : rsqrt_pair(r2s);
                     accumulate<LMAX, MLO, MHI, double>(acc, dx * rinv, dy * rinv, dz * rinv, wj);
                 }
+                }
             }
-            if (F32 && ++trips == 4) { flush_f32(); trips = 0; }
+            if (F32 && ++trips == 8) { flush_f32(); trips = 0; }
         }
         S = refill();
     } while (S > 0);
@@ -736,22 +779,23 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
 
 // dynamic shared memory of k_harm per CTA: mtab[12][threads] double | queue[warps][kQueue][32] uint2 |
 //                                          stage[warps][2][kStageRows][32] u32 | stage descriptors[warps][2][kStageRows] u32
-constexpr size_t harm_smem_bytes(bool periodic)
+__host__ __device__ constexpr size_t harm_smem_bytes(bool periodic, bool f32 = false)
 {
-    return (periodic ? (size_t)12 * kHarmWarps * 32 * 8 : 0) + (size_t)kHarmWarps * kQueue * 32 * 8 +
+    return (periodic ? (size_t)12 * kHarmWarps * 32 * 8 : 0) + (size_t)kHarmWarps * (f32 ? kQueueF32 : kQueue) * 32 * 8 +
            (size_t)kHarmWarps * 2 * kStageRows * 32 * 4 + (size_t)kHarmWarps * 2 * kStageRows * 4;
 }
 
-// F32: the fp32-harmonics variant (ENCORE_FP32_HARMONICS): weighted harmonics in fp32, fp64 accumulation of 16-pair
+// F32: the fp32-harmonics variant (ENCORE_FP32_HARMONICS): weighted harmonics in fp32, fp64 accumulation of 32-pair
 // chunk sums; the pair list (binning) is the fp64-exact one of k_fill either way.
 template <int LMAX, int MLO, int MHI, bool PERIODIC, bool F32>
-__global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) > (F32 ? 30 : ENCORE_HARM_FAT) ? 2 : 3) k_harm(PairArgs a, int g0, int g1, int write_counts)
+__global__ void __launch_bounds__(kHarmWarps * 32, F32 ? 3 : (ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3)) k_harm(PairArgs a, int g0, int g1, int write_counts)
 {
     constexpr int NACC = ncomp_range(LMAX, MLO, MHI), D = F32 ? 2 : (NACC > ENCORE_HARM_FAT ? ENCORE_HARM_DEPTH_FAT : ENCORE_HARM_DEPTH);
     extern __shared__ __align__(16) unsigned char harm_smem[];
     double *mtab = reinterpret_cast<double *>(harm_smem);
     uint2 *s_q = reinterpret_cast<uint2 *>(harm_smem + (PERIODIC ? (size_t)12 * kHarmWarps * 32 * 8 : 0));
-    unsigned *s_stm = reinterpret_cast<unsigned *>(s_q + kHarmWarps * kQueue * 32);
+    constexpr int QN = F32 ? kQueueF32 : kQueue;
+    unsigned *s_stm = reinterpret_cast<unsigned *>(s_q + kHarmWarps * QN * 32);
     unsigned *s_std = s_stm + kHarmWarps * 2 * kStageRows * 32;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ng = g1 - g0, nb = a.bins.nbins;
@@ -776,7 +820,7 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     const unsigned padent = (unsigned)a.npart | (0x15u << 26);
     // r^2 of every pair of this item lies in [e2[bin], e2[bin+1]) up to rounding; the padding particle is a few box sizes away
     const bool careful = !(a.bins.e2[bin] > 1e-290 && a.bins.e2[bin + 1] < 1e290 && a.pad_r2max < 1e290);
-    uint2 *q = s_q + warp * kQueue * 32;
+    uint2 *q = s_q + warp * QN * 32;
     unsigned *stm = s_stm + warp * 2 * kStageRows * 32, *std_ = s_std + warp * 2 * kStageRows;
 
     double acc[NACC];
@@ -784,20 +828,54 @@ __global__ void __launch_bounds__(kHarmWarps * 32, ncomp_range(LMAX, MLO, MHI) >
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned np;
     HarmStats st{0u};
+    // F32: the fp64 accumulators of this thread are a column of shared memory behind the other regions
+    double *sacc = reinterpret_cast<double *>(harm_smem + harm_smem_bytes(PERIODIC, F32)) + threadIdx.x;
+    if constexpr (F32) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) sacc[k * (kHarmWarps * 32)] = 0.0;
+    }
+    // fp32-harmonics variant: 16-byte fp32 candidate records for the bins fp32 coordinates resolve (api.cu: gf_min_r2)
+    const bool gf = F32 && !careful && a.pos4f != nullptr && a.bins.e2[bin] >= a.gf_min_r2;
+    const float3 mef = make_float3((float)(me.x - a.ctr[0]), (float)(me.y - a.ctr[1]), (float)(me.z - a.ctr[2]));
     if (!PERIODIC) {
-        if (careful) np = harm_rows<LMAX, MLO, MHI, 0, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
-        else np = harm_rows<LMAX, MLO, MHI, 0, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st);
+        if constexpr (F32) {
+            if (gf) np = harm_rows<LMAX, MLO, MHI, 0, D, false, true, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st, a.pos4f, mef, sacc);
+        }
+        if (!gf) {
+            if (careful) np = harm_rows<LMAX, MLO, MHI, 0, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st, nullptr, mef, sacc);
+            else np = harm_rows<LMAX, MLO, MHI, 0, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, 0.0, 0.0, lane, padent, st, nullptr, mef, sacc);
+        }
     } else if (fast) {
-        double *mt = mtab + threadIdx.x;
         const double L = a.geom.box;
         constexpr int R = kHarmWarps * 32;
-        mt[0 * R] = me.x - L; mt[1 * R] = me.x; mt[2 * R] = me.x + L;
-        mt[4 * R] = me.y - L; mt[5 * R] = me.y; mt[6 * R] = me.y + L;
-        mt[8 * R] = me.z - L; mt[9 * R] = me.z; mt[10 * R] = me.z + L;
-        __syncwarp();
-        if (careful) np = harm_rows<LMAX, MLO, MHI, 1, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
-        else np = harm_rows<LMAX, MLO, MHI, 1, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st);
-    } else np = harm_rows<LMAX, MLO, MHI, 2, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st);
+        if (gf) {
+            float *mt = reinterpret_cast<float *>(mtab) + threadIdx.x;
+            const double x = me.x - a.ctr[0], y = me.y - a.ctr[1], z = me.z - a.ctr[2];
+            mt[0 * R] = (float)(x - L); mt[1 * R] = (float)x; mt[2 * R] = (float)(x + L);
+            mt[4 * R] = (float)(y - L); mt[5 * R] = (float)y; mt[6 * R] = (float)(y + L);
+            mt[8 * R] = (float)(z - L); mt[9 * R] = (float)z; mt[10 * R] = (float)(z + L);
+            __syncwarp();
+            if constexpr (F32)
+                np = harm_rows<LMAX, MLO, MHI, 1, D, false, true, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, reinterpret_cast<const double *>(mt), L, a.geom.half, lane, padent, st, a.pos4f, mef, sacc);
+        } else {
+            double *mt = mtab + threadIdx.x;
+            mt[0 * R] = me.x - L; mt[1 * R] = me.x; mt[2 * R] = me.x + L;
+            mt[4 * R] = me.y - L; mt[5 * R] = me.y; mt[6 * R] = me.y + L;
+            mt[8 * R] = me.z - L; mt[9 * R] = me.z; mt[10 * R] = me.z + L;
+            __syncwarp();
+            if (careful) np = harm_rows<LMAX, MLO, MHI, 1, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st, nullptr, mef, sacc);
+            else np = harm_rows<LMAX, MLO, MHI, 1, D, false, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, mt, L, a.geom.half, lane, padent, st, nullptr, mef, sacc);
+        }
+    } else {
+        if constexpr (F32) {
+            if (gf) np = harm_rows<LMAX, MLO, MHI, 2, D, false, true, true>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st, a.pos4f, mef, sacc);
+        }
+        if (!gf) np = harm_rows<LMAX, MLO, MHI, 2, D, true, F32>(acc, rows, rdesc, nrows, active, q, stm, std_, a.pos4, me, nullptr, a.geom.box, a.geom.half, lane, padent, st, nullptr, mef, sacc);
+    }
+    if constexpr (F32) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) acc[k] = sacc[k * (kHarmWarps * 32)];
+    }
     if (write_counts) {
         a.counts[col] = np;     // n_i(b); every m-range pass walks the same bits, the first one reports
 #ifdef ENCORE_HARM_STATS
@@ -838,17 +916,19 @@ cudaError_t launch_harm_t(const PairArgs &a, int g0, int g1, int write_counts, c
 {
     const int nitems = (g1 - g0) * a.bins.nbins;
     const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
+    // F32: the fp64 accumulators live in shared memory, one column per thread
+    constexpr size_t kAccBytes = F32 ? (size_t)ncomp_range(LMAX, MLO, MHI) * kHarmWarps * 32 * sizeof(double) : 0;
     // the opt-in shared-memory limit is a per-kernel, process-wide attribute: set once per instantiation
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(true));
+        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(true, F32) + kAccBytes));
         if (attr_err == cudaSuccess)
-            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)harm_smem_bytes(false));
+            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(false, F32) + kAccBytes));
     });
     if (attr_err != cudaSuccess) return attr_err;
-    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(true), s>>>(a, g0, g1, write_counts);
-    else k_harm<LMAX, MLO, MHI, false, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(false), s>>>(a, g0, g1, write_counts);
+    if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(true, F32) + kAccBytes, s>>>(a, g0, g1, write_counts);
+    else k_harm<LMAX, MLO, MHI, false, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(false, F32) + kAccBytes, s>>>(a, g0, g1, write_counts);
     *launches += 1;
     return cudaGetLastError();
 }
