@@ -516,24 +516,26 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline_entry(oracle_sample(cfg, pos, w, target_s=15.0))
     if world == 1 and not args.no_per_config:
-        per = {}
+        per, z64, pairs64 = {}, {}, {}
         for name in sorted(W.CONFIGS):
             c = W.CONFIGS[name]
-            r, _ = measure_config(E, torch, c, 0, 2, 3, dev, want_e2e=False, want_graph=True)
+            r, _ = measure_config(E, torch, c, 0, 2, 3, dev, want_e2e=False, want_graph=True, keep_zeta=name in ("c3", "c4"))
             per[name] = config_entry(c, r, 2, fp64_peak, fp32_peak)
             per[name]["graph_replay_ms_per_step"] = r["graph_replay_ms"]   # encore_compute_enqueue replayed from a CUDA graph
+            if "zeta" in r:
+                z64[name], pairs64[name] = r["zeta"], r["pairs"]
         # the same c3 catalogue with the parity-odd multiplets too (111 instead of 69 multiplets)
         r, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, allparity=True)
         per["c3_allparity"] = dict(config_entry(W.CONFIGS["c3"], r, 2, fp64_peak, fp32_peak), n_multiplets=r["nout"] // 120)
-        # fp32 harmonics with fp64 accumulation on the same c3 catalogue - a separate path with its own
+        # fp32 harmonics with fp64 accumulation on the c3 and c4 catalogues - a separate path with its own
         # tolerance (1e-5); the difference to this run's fp64 result is reported beside its time
-        r64, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 1, 3, dev, want_e2e=False, keep_zeta=True)
-        r32, _ = measure_config(E, torch, W.CONFIGS["c3"], 0, 2, 3, dev, want_e2e=False, fp32_harmonics=True, keep_zeta=True)
-        e32 = config_entry(W.CONFIGS["c3"], r32, 2, fp64_peak, fp32_peak)
-        e32["dtype"] = "f32 harmonics, f64 accumulation / contraction"
-        e32["max_rel_diff_to_fp64_run"] = float(np.abs(r32["zeta"] - r64["zeta"]).max() / np.abs(r64["zeta"]).max())
-        e32["pairs_equal_fp64_run"] = bool(r32["pairs"] == r64["pairs"])
-        per["c3_fp32_harmonics"] = e32
+        for name in ("c3", "c4"):
+            r32, _ = measure_config(E, torch, W.CONFIGS[name], 0, 2, 3, dev, want_e2e=False, fp32_harmonics=True, keep_zeta=True)
+            e32 = config_entry(W.CONFIGS[name], r32, 2, fp64_peak, fp32_peak)
+            e32["dtype"] = "f32 harmonics, f64 accumulation / contraction"
+            e32["max_rel_diff_to_fp64_run"] = float(np.abs(r32["zeta"] - z64[name]).max() / np.abs(z64[name]).max())
+            e32["pairs_equal_fp64_run"] = bool(r32["pairs"] == pairs64[name])
+            per[name + "_fp32_harmonics"] = e32
         line["per_config"] = per
         line["next_rows"] = measure_next_rows(E, torch, dev, fp64_peak)
     if rank == 0:
