@@ -746,3 +746,29 @@ def test_enqueue_variant_in_a_cuda_graph(E, oracle):
             o = oracle.zeta(cfg.order, p_, w_, cfg.box, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax)
             assert np.abs(out.cpu().numpy() - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
         del g
+
+
+def test_enqueue_and_shards_on_the_other_plan_kinds(E, oracle):
+    """encore_compute_enqueue and encore_compute_shard on a 6PCF plan (factorised kernel), an fp32-harmonics plan and an
+    ALLPARITY plan: enqueue gives the bits of encore_compute, the shards add up to it"""
+    import dataclasses
+    dev = torch.device("cuda:0")
+    base = W.scaled(W.CONFIGS["c5"], box=330.0, n=1500, grid=32)
+    pos, w = W.make(base)
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    for order, nbins, lmax, kw in [(6, 6, 2, {}), (4, 7, 3, {"fp32_harmonics": True}), (5, 6, 2, {"allparity": True})]:
+        with E.Plan(order, 20.0, 160.0, nbins, lmax, base.box, **kw) as plan:
+            z0 = plan.compute(tp, tw).clone()
+            assert E.encore_get_status(plan.h) == E.OK
+            out = torch.zeros_like(z0)
+            plan.compute_enqueue(tp, tw, out)
+            assert E.encore_get_status(plan.h) == E.OK
+            assert torch.equal(out, z0)
+            parts = [plan.compute_shard(tp, tw, k, 3).clone() for k in range(3)]
+            tot = parts[0] + parts[1] + parts[2]
+            scale = float(z0.abs().max())
+            assert float((tot - z0).abs().max()) <= 1e-12 * scale
+    o = oracle.zeta(6, pos, w, base.box, 20.0, 160.0, 6, 2)
+    with E.Plan(6, 20.0, 160.0, 6, 2, base.box) as plan:
+        z = plan.compute(tp, tw).cpu().numpy()
+    assert np.abs(z - o["zeta"]).max() <= TOL * np.abs(o["zeta"]).max()
