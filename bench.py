@@ -431,6 +431,7 @@ def main():
     ap.add_argument("--all-configs", action="store_true", help="(default now) kept for compatibility")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--allparity", action="store_true", help="ALLPARITY plan: parity-odd multiplets too (not the headline config)")
+    ap.add_argument("--fp32-harmonics", action="store_true", help="ENCORE_FP32_HARMONICS plan (a separately reported path, tolerance 1e-5; not the headline)")
     ap.add_argument("--only-next-rows", action="store_true", help="measure and print only `next_rows` (6PCF, edge correction, gridded estimator)")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]
@@ -462,7 +463,7 @@ def main():
 
     with ClockSampler(local) as clocks:
         res, (pos, w) = measure_config(E, torch, cfg, rank, steps, warmup, dev, allparity=args.allparity,
-                                       shard=(rank, world) if world > 1 else None)
+                                       shard=(rank, world) if world > 1 else None, fp32_harmonics=args.fp32_harmonics)
     ms_total = max_over_ranks(torch, res["ms_total"], dev)
     e2e_ms = max_over_ranks(torch, res["e2e_ms_total"], dev)
     ms_per_step = ms_total / steps
@@ -480,7 +481,8 @@ def main():
     line = {
         "metric": "primaries_per_s", "value": value, "unit": "primaries/s", "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, args.allparity),
+        "dtype": "f32 harmonics, f64 accumulation / contraction" if args.fp32_harmonics else "f64", "data": "synthetic",
+        "config": workload_config(cfg, world, args.allparity),
         "pairs_per_s": res["pairs"] / (ms_per_step * 1e-3) if world == 1 else None,   # (a shard only counts its own pairs)
         "accepted_pairs": res["pairs"], "candidate_pairs": res["candidates"],
         "contraction_gflops_canonical": cfg.n * ca_flops / (st["contraction"] * 1e-3) / 1e9 if world == 1 else None,

@@ -711,7 +711,7 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
         ent[d] = gen();
         r[d] = fetch(ent[d] & kIdxMask);
     }
-    // F32: fp32 chunk sums, added every eight loop trips (32 pairs) to the fp64 accumulators, which sit in shared memory
+    // F32: fp32 chunk sums, added every sixteen loop trips (64 pairs) to the fp64 accumulators, which sit in shared memory
     // (sacc, this thread's column, stride = threads of the CTA): in registers they held the kernel at 219 registers and
     // 8 warps per SM
     constexpr int NACCF = F32 ? ncomp_range(LMAX, MLO, MHI) : 1;
@@ -800,7 +800,7 @@ __device__ __forceinline__ unsigned harm_rows(double (&acc)[ncomp_range(LMAX, ML
                 }
                 }
             }
-            if (F32 && ++trips == 8) { flush_f32(); trips = 0; }
+            if (F32 && ++trips == 16) { flush_f32(); trips = 0; }
         }
         S = refill();
     } while (S > 0);
@@ -817,7 +817,7 @@ __host__ __device__ constexpr size_t harm_smem_bytes(bool periodic, bool f32 = f
            (size_t)kHarmWarps * 2 * kStageRows * 32 * 4 + (size_t)kHarmWarps * 2 * kStageRows * 4;
 }
 
-// F32: the fp32-harmonics variant (ENCORE_FP32_HARMONICS): weighted harmonics in fp32, fp64 accumulation of 32-pair
+// F32: the fp32-harmonics variant (ENCORE_FP32_HARMONICS): weighted harmonics in fp32, fp64 accumulation of 64-pair
 // chunk sums; the pair list (binning) is the fp64-exact one of k_fill either way.
 template <int LMAX, int MLO, int MHI, bool PERIODIC, bool F32>
 __global__ void __launch_bounds__(kHarmWarps * 32, F32 ? 3 : (ncomp_range(LMAX, MLO, MHI) > ENCORE_HARM_FAT ? 2 : 3)) k_harm(PairArgs a, int g0, int g1, int write_counts)
