@@ -44,7 +44,7 @@ SM_COUNT, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this
 # round's kernels (profiles/r2_ncu_full_c3.txt and r2_ncu_full_c5.txt name the commands); None where not captured
 NCU_DRAM_BYTES = {"c3": {"k_fill": 1.947e9, "k_harm": 2.958e9, "k_contract": 9.587e9}, "c5": {"k_contract": 9.243e9}}
-NCU_PROFILE = "profiles/r2_ncu_full_c3.txt"
+NCU_PROFILE = {"c3": "profiles/r2_ncu_full_c3.txt", "c5": "profiles/r2_ncu_full_c5.txt"}   # where NCU_DRAM_BYTES comes from
 
 
 def peaks():
@@ -496,7 +496,7 @@ def main():
             "contraction_frac_fp64_executed": cfg.n * ex_flops / (st["contraction"] * 1e-3) / fp64_peak,
         },
         "roofline": {"bound": top["bound"], "kernel": top["kernel"], "achieved": top["achieved"], "peak": top["peak"],
-                     "unit": "TFLOP/s", "frac": top["frac"], "traffic": top.get("traffic"), "traffic_source": NCU_PROFILE,
+                     "unit": "TFLOP/s", "frac": top["frac"], "traffic": top.get("traffic"), "traffic_source": NCU_PROFILE.get(cfg.name) if top.get("traffic") is not None else None,
                      "ms": top["ms"], "share_of_step": top["share_of_step"], "model": top["model"],
                      "peak_source": f"derived: {SM_COUNT} SM x {FP64_LANES_PER_SM} fp64 (x {FP32_LANES_PER_SM} fp32) FMA lanes x 2 x "
                                     f"{sm_max_mhz:g} MHz ({peak_src} clock); MEASURED_PEAKS.json has no fp64 entry",
