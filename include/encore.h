@@ -133,7 +133,7 @@ int encore_compute_shard(encore_plan_t *plan, const double *positions, const dou
  *   a^b_lm(s) = (1/v_b) sum_{cells x != s} delta(x) h^3 Y_lm((x - s)^) Theta^b(|x - s|)        (eq. 36 evaluated with FFTs)
  *   zeta^B_Lam = (1/V) sum_{cells s} delta(s) h^3 sum_M E(Lam) C^Lam_M prod_k a^{b_k}_{l_k m_k}(s)  (steps i-iii)
  * i.e. eq. 34/35 for particles at the cell centres with weights delta h^3; separations are (integer offset) h, minimal
- * image, binned on r^2 like the particle path.  zeta_out DEVICE as for encore_compute.  Scratch: two complex G^3 fields and
+ * image, binned on r^2 like the particle path.  zeta_out DEVICE as for encore_compute.  Scratch: one complex G^3 field, one per (l, m >= 0) of a batch (all of them when they fit 2 GiB) and
  * the a_lm array of all cells, (lmax+1)^2 nbins G^3 doubles (the memory cost the paper warns of, PAPER.md fn. 5).  Uses cuFFT.
  * Enqueued on cuda_stream without host synchronisation once the scratch exists.  2 <= G <= 1024. */
 int encore_compute_grid(encore_plan_t *plan, const double *delta, int G, double *zeta_out, void *cuda_stream);

@@ -47,7 +47,7 @@ struct encore_plan_s {
     DevBuf io_pos, io_w, io_zeta, pos4f;
     DevBuf gbound, gprefix, gwide, rows, rowdesc, rowcnt, errflag;
     DevBuf mesh_fd, mesh_kern;          // gridded estimator: F[delta h^3] and the kernel / a_lm field being transformed
-    int mesh_fft = -1, mesh_G = 0;      // cuFFT plan for G^3
+    int mesh_fft = -1, mesh_fftb = -1, mesh_G = 0, mesh_batch = 0;   // cuFFT plans for one and for mesh_batch G^3 fields
     DevBuf d_gaunt, edge_A, edge_rhs;   // edge correction: E G tensor, per-tuple matrices and right-hand sides
     bool gaunt_ready = false;
     int *h_gprefix = nullptr;   // pinned
@@ -669,22 +669,27 @@ int encore_compute_grid(encore_plan_t *P, const double *delta, int G, double *ze
     const size_t nout = (size_t)T.nLam() * T.nB();
     const bool factorised = !P->force_generic && contraction_is_factorised(T.order, nb, T.lmax) && (T.order == 3 || P->cta_smem > 0);
     const int nchunk = choose_nchunk(P, factorised);
+    // (l, m >= 0) fields per FFT batch: all of them if they fit 2 GiB of scratch
+    const int nlm = (T.lmax + 1) * (T.lmax + 2) / 2;
+    const int batch = (int)std::max<size_t>(1, std::min<size_t>((size_t)nlm, ((size_t)2 << 30) / (ncell * 2 * sizeof(double))));
     CU(P->mesh_fd.ensure(sizeof(double) * 2 * ncell));
-    CU(P->mesh_kern.ensure(sizeof(double) * 2 * ncell));
+    CU(P->mesh_kern.ensure(sizeof(double) * 2 * ncell * (size_t)batch));
     CU(P->alm.ensure(sizeof(double) * (size_t)ngroups * ncomp * nb * 32));
     CU(P->gweights.ensure(sizeof(double) * npad));
     CU(P->partial.ensure(sizeof(double) * (size_t)(factorised ? nchunk : ngroups) * nout));
     CU(P->partial2.ensure(sizeof(double) * (size_t)64 * nout));
-    if (P->mesh_fft < 0 || P->mesh_G != G) {
+    if (P->mesh_fft < 0 || P->mesh_G != G || P->mesh_batch != batch) {
         if (P->mesh_fft >= 0) mesh_fft_plan_destroy(P->mesh_fft);
-        P->mesh_fft = -1;
-        if (mesh_fft_plan_create(G, s, &P->mesh_fft) != 0) return ENCORE_EALLOC;
-        P->mesh_G = G;
-    } else if (mesh_fft_plan_set_stream(P->mesh_fft, s) != 0) return ENCORE_ECUDA;
+        if (P->mesh_fftb >= 0) mesh_fft_plan_destroy(P->mesh_fftb);
+        P->mesh_fft = P->mesh_fftb = -1;
+        if (mesh_fft_plan_create(G, 1, s, &P->mesh_fft) != 0) return ENCORE_EALLOC;
+        if (mesh_fft_plan_create(G, batch, s, &P->mesh_fftb) != 0) return ENCORE_EALLOC;
+        P->mesh_G = G; P->mesh_batch = batch;
+    } else if (mesh_fft_plan_set_stream(P->mesh_fft, s) != 0 || mesh_fft_plan_set_stream(P->mesh_fftb, s) != 0) return ENCORE_ECUDA;
     TRY(mark(P, K_START, s));
     int fft_error = 0;
     CU(launch_mesh_alm(delta, G, T.box, T.lmax, nb, T.edges2.data(), T.vinv.data(), P->d_ycoef.as<double>(), P->mesh_fd.p, P->mesh_kern.p,
-                       P->alm.as<double>(), P->gweights.as<double>(), P->mesh_fft, s, &P->launches, &fft_error));
+                       P->alm.as<double>(), P->gweights.as<double>(), P->mesh_fft, P->mesh_fftb, batch, s, &P->launches, &fft_error));
     if (fft_error) return ENCORE_ECUDA;
     TRY(mark(P, K_HARM, s));
     TRY(contract_and_reduce(P, P->alm.as<double>(), P->gweights.as<double>(), 0, ngroups, ngroups, factorised, nchunk, zeta_out, s));
@@ -783,6 +788,7 @@ int encore_destroy(encore_plan_t *P)
     if (P->h_gprefix) cudaFreeHost(P->h_gprefix);
     for (cudaEvent_t e : P->ev) cudaEventDestroy(e);
     if (P->mesh_fft >= 0) mesh_fft_plan_destroy(P->mesh_fft);
+    if (P->mesh_fftb >= 0) mesh_fft_plan_destroy(P->mesh_fftb);
     delete P;
     return ENCORE_OK;
 }

@@ -148,9 +148,9 @@ cudaError_t launch_edge_correct(const double *T, const double *Nraw, const doubl
 
 // ---- mesh.cu (gridded estimator, eq. 36) ------------------------------------------------------------------
 cudaError_t launch_mesh_alm(const double *delta, int G, double box, int lmax, int nb, const double *e2, const double *vinv,
-                            const double *ycoef_dev, void *fd, void *kern, double *alm, double *gweights, int fft_plan,
-                            cudaStream_t s, int *launches, int *fft_error);
-int mesh_fft_plan_create(int G, cudaStream_t s, int *plan_out);
+                            const double *ycoef_dev, void *fd, void *kern, double *alm, double *gweights, int fft_plan1, int fft_planb,
+                            int batch, cudaStream_t s, int *launches, int *fft_error);
+int mesh_fft_plan_create(int G, int batch, cudaStream_t s, int *plan_out);
 int mesh_fft_plan_set_stream(int plan, cudaStream_t s);
 void mesh_fft_plan_destroy(int plan);
 

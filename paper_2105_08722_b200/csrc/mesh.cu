@@ -30,10 +30,17 @@ __global__ void k_mesh_weights(const double *__restrict__ delta, size_t ncell, d
 
 // kern[c] = conj(Y_lm(r^)) Theta^b(r) at the minimal-image offset of cell c from cell 0, r = h |offset|;
 // Y_lm = sum_k ycoef[comp][k] z^k (x+iy)^m (tables.cpp), bins decided on r^2 against e_b^2 (R8, R9)
-__global__ void k_mesh_kernel(int G, double h, int l, int m, int lmax, const double *__restrict__ ycoef, double e2lo, double e2hi,
+// blockIdx.y = field of the batch: (l, m >= 0) number j0 + blockIdx.y in the order l ascending, m ascending
+__global__ void k_mesh_kernel(int G, double h, int j0, int nlm, int lmax, const double *__restrict__ ycoef, double e2lo, double e2hi,
                               cufftDoubleComplex *__restrict__ kern)
 {
+    const int j = j0 + (int)blockIdx.y;
+    if (j >= nlm) return;
+    int l = 0;
+    while ((l + 1) * (l + 2) / 2 <= j) ++l;
+    const int m = j - l * (l + 1) / 2;
     const size_t ncell = (size_t)G * G * G;
+    kern += (size_t)blockIdx.y * ncell;
     const size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
     if (c >= ncell) return;
     const int iz = (int)(c % G), iy = (int)((c / G) % G), ix = (int)(c / ((size_t)G * G));
@@ -61,16 +68,23 @@ __global__ void k_mesh_mul(const cufftDoubleComplex *__restrict__ fd, cufftDoubl
 {
     const size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
     if (c >= ncell) return;
+    kern += (size_t)blockIdx.y * ncell;
     const cufftDoubleComplex a = fd[c], b = kern[c];
     kern[c] = make_cuDoubleComplex(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
 }
 
 // a_lm tile layout: alm[((g * ncomp + comp) * nb + b) * 32 + lane], cell = 32 g + lane
 __global__ void k_mesh_scatter(const cufftDoubleComplex *__restrict__ field, size_t ncell, size_t npad, double scale, int ncomp, int nb,
-                               int b, int cre, int cim, double *__restrict__ alm)
+                               int b, int j0, int nlm, double *__restrict__ alm)
 {
     const size_t c = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-    if (c >= npad) return;
+    const int j = j0 + (int)blockIdx.y;
+    if (c >= npad || j >= nlm) return;
+    int l = 0;
+    while ((l + 1) * (l + 2) / 2 <= j) ++l;
+    const int m = j - l * (l + 1) / 2;
+    const int cre = m == 0 ? l * l : l * l + 2 * m - 1, cim = m == 0 ? -1 : l * l + 2 * m;
+    field += (size_t)blockIdx.y * ncell;
     const size_t g = c >> 5, lane = c & 31;
     const double re = c < ncell ? field[c].x * scale : 0.0, im = c < ncell ? field[c].y * scale : 0.0;
     alm[((g * ncomp + cre) * nb + b) * 32 + lane] = re;
@@ -79,39 +93,43 @@ __global__ void k_mesh_scatter(const cufftDoubleComplex *__restrict__ field, siz
 
 } // namespace
 
-// fd, kern: G^3 complex scratch; alm: [npad/32][ncomp][nb][32]; gweights: [npad]; plan: a cufftHandle for G^3 Z2Z on stream s
+// fd: G^3 complex scratch; kern: batch x G^3 complex scratch; alm: [npad/32][ncomp][nb][32]; gweights: [npad];
+// plan1: cufftHandle for one G^3 Z2Z, planb: for `batch` of them (contiguous fields), both on stream s.  Per bin the
+// (l, m >= 0) fields go through the FFTs `batch` at a time: 5 launches per batch instead of per field (a 64^3 mesh is
+// launch-bound otherwise: 1050 launches for 10 bins, lmax = 5).
 cudaError_t launch_mesh_alm(const double *delta, int G, double box, int lmax, int nb, const double *e2, const double *vinv,
-                            const double *ycoef_dev, void *fd_, void *kern_, double *alm, double *gweights, int fft_plan,
-                            cudaStream_t s, int *launches, int *fft_error)
+                            const double *ycoef_dev, void *fd_, void *kern_, double *alm, double *gweights, int fft_plan1, int fft_planb,
+                            int batch, cudaStream_t s, int *launches, int *fft_error)
 {
     cufftDoubleComplex *fd = static_cast<cufftDoubleComplex *>(fd_), *kern = static_cast<cufftDoubleComplex *>(kern_);
     const size_t ncell = (size_t)G * G * G, npad = (ncell + 31) / 32 * 32;
     const double h = box / G, h3 = h * h * h;
-    const int ncomp = (lmax + 1) * (lmax + 1);
+    const int ncomp = (lmax + 1) * (lmax + 1), nlm = (lmax + 1) * (lmax + 2) / 2;
     const unsigned blocks = (unsigned)((npad + kT - 1) / kT);
     *fft_error = 0;
     k_mesh_weights<<<blocks, kT, 0, s>>>(delta, ncell, h3, fd, gweights, npad);
     *launches += 1;
-    cufftHandle plan = (cufftHandle)fft_plan;
-    if (cufftExecZ2Z(plan, fd, fd, CUFFT_FORWARD) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
+    if (cufftExecZ2Z((cufftHandle)fft_plan1, fd, fd, CUFFT_FORWARD) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
+    cufftHandle planb = (cufftHandle)fft_planb;
     for (int b = 0; b < nb; ++b)
-        for (int l = 0; l <= lmax; ++l)
-            for (int m = 0; m <= l; ++m) {
-                k_mesh_kernel<<<blocks, kT, 0, s>>>(G, h, l, m, lmax, ycoef_dev, e2[b], e2[b + 1], kern);
-                if (cufftExecZ2Z(plan, kern, kern, CUFFT_FORWARD) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
-                k_mesh_mul<<<blocks, kT, 0, s>>>(fd, kern, ncell);
-                if (cufftExecZ2Z(plan, kern, kern, CUFFT_INVERSE) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
-                const int cre = m == 0 ? l * l : l * l + 2 * m - 1, cim = m == 0 ? -1 : l * l + 2 * m;
-                k_mesh_scatter<<<blocks, kT, 0, s>>>(kern, ncell, npad, vinv[b] / (double)ncell, ncomp, nb, b, cre, cim, alm);
-                *launches += 3;
-            }
+        for (int j0 = 0; j0 < nlm; j0 += batch) {
+            // (a last, partial batch transforms the stale fields behind it as well; they are not read)
+            const dim3 grid(blocks, (unsigned)batch);
+            k_mesh_kernel<<<grid, kT, 0, s>>>(G, h, j0, nlm, lmax, ycoef_dev, e2[b], e2[b + 1], kern);
+            if (cufftExecZ2Z(planb, kern, kern, CUFFT_FORWARD) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
+            k_mesh_mul<<<grid, kT, 0, s>>>(fd, kern, ncell);
+            if (cufftExecZ2Z(planb, kern, kern, CUFFT_INVERSE) != CUFFT_SUCCESS) { *fft_error = 1; return cudaSuccess; }
+            k_mesh_scatter<<<grid, kT, 0, s>>>(kern, ncell, npad, vinv[b] / (double)ncell, ncomp, nb, b, j0, nlm, alm);
+            *launches += 3;
+        }
     return cudaGetLastError();
 }
 
-int mesh_fft_plan_create(int G, cudaStream_t s, int *plan_out)
+int mesh_fft_plan_create(int G, int batch, cudaStream_t s, int *plan_out)
 {
     cufftHandle p;
-    if (cufftPlan3d(&p, G, G, G, CUFFT_Z2Z) != CUFFT_SUCCESS) return 1;
+    int n[3] = {G, G, G};
+    if (cufftPlanMany(&p, 3, n, nullptr, 1, G * G * G, nullptr, 1, G * G * G, CUFFT_Z2Z, batch) != CUFFT_SUCCESS) return 1;
     if (cufftSetStream(p, s) != CUFFT_SUCCESS) { cufftDestroy(p); return 1; }
     *plan_out = (int)p;
     return 0;
