@@ -410,7 +410,7 @@ __global__ void __launch_bounds__(nw4(NB) * lpc4(NB) * 32, 1) k_contract4(Contra
     const int iL = have ? iLs : 0;
     const Lam4 L = a.lam4[iL];
     const TilePipe tp = make_pipe(C);
-    const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // this multiplet's term list in shared memory
+    const int toff = tp.bar + kBarDoubles + (warp / NW) * 6 * a.max_terms; // this multiplet's term list in shared memory
     if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.tbeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
     dispatch4<NB, NW, 0>(warp % NW, a, C, tp, have, L, iL, toff);
@@ -730,7 +730,7 @@ __global__ void __launch_bounds__(nw5(NB) * lpc5(NB) * 32, 1) k_contract5(Contra
     const int iL = have ? iLs : 0;
     const Lam5 L = a.lam5[iL];
     const TilePipe tp = make_pipe(C);
-    const int toff = tp.bar + 8 + (warp / NW) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
+    const int toff = tp.bar + kBarDoubles + (warp / NW) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
     if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
     __syncthreads();
     dispatch5<NB, 0>(warp % NW, a, C, tp, have, L, iL, toff);
@@ -793,7 +793,7 @@ size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas)
     size_t max_terms = 1;
     for (const Lam4 &q : T.lam4) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
     for (const Lam5 &q : T.lam5) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
-    const size_t extra = 64 + sizeof(CtaPlan) + (size_t)lpc * max_terms * sizeof(PairTerm);
+    const size_t extra = kBarDoubles * sizeof(double) + sizeof(CtaPlan) + (size_t)lpc * max_terms * sizeof(PairTerm);
     const size_t blk = (size_t)T.nbins * 32 * sizeof(double); // bytes of one component of a tile
     auto ls_of = [&](int iL, int *l) {
         if (T.order == 4) { const Lam4 &q = T.lam4[iL]; l[0] = q.l1; l[1] = q.l2; l[2] = q.l3; return 3; }

@@ -278,8 +278,8 @@ __global__ void __launch_bounds__(kWarps6 * 32, 1) k_contract6(ContractArgs a)
     const int iL = have ? unit >> 3 : 0, role = have ? unit & 7 : 0;
     const Lam6 L = a.lam6[iL];
     const TilePipe tp = make_pipe(C);
-    const int toff = tp.bar + 8 + warp * 6 * a.max_terms;           // every warp stages the term lists of its multiplet
-    const int soff = tp.bar + 8 + kWarps6 * 6 * a.max_terms + C.scr[warp];
+    const int toff = tp.bar + kBarDoubles + warp * 6 * a.max_terms;           // every warp stages the term lists of its multiplet
+    const int soff = tp.bar + kBarDoubles + kWarps6 * 6 * a.max_terms + C.scr[warp];
     if (have) stage_terms(toff, a.pair_terms + L.ubeg[0], L.nterms, threadIdx.x & 31);
     __syncthreads();
     dispatch6<NB, 0>(role, a, C, tp, have, L, iL, toff, soff);
@@ -341,7 +341,7 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
     };
     size_t max_terms = 1;
     for (const Lam6 &q : T.lam6) max_terms = std::max<size_t>(max_terms, (size_t)q.nterms);
-    const size_t fixed = 64 + (size_t)kWarps6 * max_terms * sizeof(PairTerm);
+    const size_t fixed = kBarDoubles * sizeof(double) + (size_t)kWarps6 * max_terms * sizeof(PairTerm);
     std::vector<std::pair<double, int>> units;
     for (int iL = 0; iL < nL; ++iL)
         for (int w = 0; w < nw6(nb); ++w) {
@@ -382,7 +382,7 @@ size_t contraction_plan_ctas6(const HostTables &T, std::vector<CtaPlan> &ctas)
         c.tile = off;
         const size_t tb = (size_t)off * sizeof(double), extra = fixed + scr[i];
         c.nbuf = 1;     // as many tile buffers as fit, up to 4 (contract_tile.cuh)
-        for (int nbf = 2; nbf <= 4; ++nbf) if (nbf * tb + extra <= kSmemLimit6) c.nbuf = nbf;
+        for (int nbf = 2; nbf <= kMaxTileBufs; ++nbf) if (nbf * tb + extra <= kSmemLimit6) c.nbuf = nbf;
         smem = std::max(smem, c.nbuf * tb + extra);
     }
     return smem;

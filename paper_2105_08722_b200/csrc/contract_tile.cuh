@@ -70,9 +70,12 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
         : "memory");
 }
 
+constexpr int kMaxTileBufs = 8;                 // tile buffers of the ring (k_contract6: as many as fit; N = 4, 5: two)
+constexpr int kBarDoubles = 2 * kMaxTileBufs;   // shared memory of the mbarriers, in doubles
+
 struct TilePipe {
-    int buf[4];              // offsets into smem_c (doubles)
-    int bar;                 // offset of the mbarriers: full[4], empty[4]
+    int buf[kMaxTileBufs];   // offsets into smem_c (doubles)
+    int bar;                 // offset of the mbarriers: full[kMaxTileBufs], empty[kMaxTileBufs]
     unsigned bytes;          // bytes of the staged l-blocks of one group
     int nbuf;
 };
@@ -100,13 +103,13 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
         }
     };
     if (RING && tp.nbuf > 2) {
-        // a ring of 3-4 buffers: "full" barriers carry the copies, "empty" barriers (one arrival per warp) say that every warp
+        // a ring of 3-8 buffers: "full" barriers carry the copies, "empty" barriers (one arrival per warp) say that every warp
         // is done with a buffer.  Tile k + nbuf - 1 is requested while tile k is contracted (light CTAs finish a tile faster
         // than a copy takes to arrive: one tile of look-ahead left them waiting for data).  Only the issuing thread waits for
         // the other warps (before it refills the buffer they used one tile ago); nobody else waits on anything but data, so
         // the warps drift by up to a tile instead of meeting at a CTA barrier after every group.
         const int nbuf = tp.nbuf;
-        unsigned long long *empty = bar + 4;
+        unsigned long long *empty = bar + kMaxTileBufs;
         const int lane = threadIdx.x & 31;
         if (issuer)
             for (int j = 0; j < nbuf - 1 && g + j * stride < ngroups; ++j) load(j, g + j * stride);
@@ -129,7 +132,7 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
     if (issuer && g < ngroups) load(0, g);
     if (tp.nbuf == 2) {
         // two buffers (the tiles of the heavy CTAs are too large for more): the same scheme with one tile of look-ahead
-        unsigned long long *empty = bar + 4;
+        unsigned long long *empty = bar + kMaxTileBufs;
         const int lane = threadIdx.x & 31;
         for (int k = 0; g < ngroups; ++k, g += stride) {
             const int st = k & 1;
@@ -153,19 +156,19 @@ __device__ __forceinline__ void for_each_group_tile(const ContractArgs &a, const
     }
 }
 
-// shared memory: [nbuf tile buffers][8 mbarriers = 8 doubles][term lists of the CTA's multiplets]
+// shared memory: [nbuf tile buffers][2 x 8 mbarriers = kBarDoubles doubles][term lists of the CTA's multiplets]
 __device__ __forceinline__ TilePipe make_pipe(const CtaPlan &C)
 {
     TilePipe tp;
-    for (int i = 0; i < 4; ++i) tp.buf[i] = i < C.nbuf ? i * C.tile : 0;
+    for (int i = 0; i < kMaxTileBufs; ++i) tp.buf[i] = i < C.nbuf ? i * C.tile : 0;
     tp.bar = C.nbuf * C.tile;
     tp.bytes = (unsigned)(C.tile * sizeof(double));
     tp.nbuf = C.nbuf;
     if (threadIdx.x == 0) {
         unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_c + tp.bar);
-        for (int i = 0; i < 4; ++i) {
-            mbar_init(&bar[i], 1);                      // "full": the issuing thread's expect_tx arrival
-            mbar_init(&bar[4 + i], blockDim.x / 32);    // "empty": one arrival per warp
+        for (int i = 0; i < kMaxTileBufs; ++i) {
+            mbar_init(&bar[i], 1);                                  // "full": the issuing thread's expect_tx arrival
+            mbar_init(&bar[kMaxTileBufs + i], blockDim.x / 32);     // "empty": one arrival per warp
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
