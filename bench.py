@@ -374,6 +374,24 @@ def measure_next_rows(E, torch, dev, fp64_peak):
             res[tag + "_contraction_ms"] = E.encore_get_kernel_ms(plan.h)["k_contract"]
             res[tag + "_flops_per_primary"] = E.encore_contraction_flops(plan.h)[0]
         out["f1_6pcf"]["sub_box"] = dict(res, n=int(ps.shape[1]), note="open-geometry sub-box of the same catalogue, both contraction kernels")
+    # the shapes of the paper's Table 2: ~5e4 uniform points in a periodic box L = 1500, N_r = 10 bins up to
+    # r_max = 200, 4PCF at lmax = 5 and 10, 5PCF at lmax = 5.  The paper's seconds (16-core Skylake / best P100 row, a_lm on one
+    # CPU core) are context from other hardware, quoted beside this run's time; they are not a target and not a ratio.
+    t2 = W.Config("table2", 4, 10, 0.0, 200.0, 5, 1500.0, 50625, 578, "uniform", "unit")
+    pos, w = W.make(t2)
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    rows = {}
+    for tag, order, lmax, cpu_s, gpu_s in (("4pcf_lmax5", 4, 5, 4.8, 21.9), ("4pcf_lmax10", 4, 10, 58.8, 38.4), ("5pcf_lmax5", 5, 5, 741.8, 74.3)):
+        with E.Plan(order, t2.rmin, t2.rmax, t2.nbins, lmax, t2.box) as plan:
+            E.encore_set_timing(plan.h, True)
+            z = torch.empty((plan.n_lambda, plan.n_b), dtype=torch.float64, device=dev)
+            ms = timed(lambda: plan.compute(tp, tw, out=z))
+            km = E.encore_get_kernel_ms(plan.h)
+            ex, ca = E.encore_contraction_flops(plan.h)
+            rows[tag] = {"outputs": plan.n_lambda * plan.n_b, "ms_per_catalogue": ms, "primaries_per_s": t2.n / (ms * 1e-3), "kernel_ms": km,
+                         "contraction_frac_fp64_executed": t2.n * ex / (km["k_contract"] * 1e-3) / fp64_peak,
+                         "paper_seconds_16core_cpu": cpu_s, "paper_seconds_best_p100_row": gpu_s}
+    out["paper_table2_shapes"] = dict(rows, workload=f"n={t2.n} uniform points, periodic L={t2.box:g}, {t2.nbins} bins in [0,200] (PAPER.md:578)")
     # (f2) edge correction at the shape of c3 / c4: 69 multiplets, 120 bin tuples (120 LU solves of 69 unknowns)
     c3 = W.CONFIGS["c3"]
     with E.Plan(c3.order, c3.rmin, c3.rmax, c3.nbins, c3.lmax, 0.0) as plan:
