@@ -74,13 +74,14 @@ struct Lam6 {
 // One CTA of the factorised N = 4, 5 kernels: its multiplets and the l-blocks of the a_lm tile they need (only those
 // are brought into shared memory; a block l is the (2l+1) x nbins x 32 doubles starting at component l^2).
 struct CtaPlan {
-    int lam[12];                    // multiplet per slot (at most 12: one warp per multiplet), -1: empty
+    int lam[12];                    // multiplet per slot (at most 12: one warp per multiplet), -1: empty; N = 5 at 9-10 bins and N = 6:
+                                    // lam[w] = 8 * multiplet + warp role for w < 8 (N = 5: lam[8 + s] = multiplet staged in term slot s)
     int nblk;
     int bl[ENCORE_MAX_LMAX + 1];    // l of block j
     int off[ENCORE_MAX_LMAX + 1];   // offset (doubles) of block l inside a tile buffer, -1: not staged
     int tile;                       // doubles per tile buffer
     int nbuf;                       // tile buffers of the ring: 1 (single) .. 4
-    int scr[8];                     // N = 6: lam[w] = 8 * multiplet + warp role; offset (doubles) of warp w's U scratch
+    int scr[8];                     // N = 6: offset (doubles) of warp w's U scratch;  N = 5 at 9-10 bins: term slot of warp w's multiplet
 };
 
 struct HostTables {

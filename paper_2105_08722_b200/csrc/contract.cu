@@ -716,24 +716,42 @@ __device__ __forceinline__ void dispatch5(int w, const ContractArgs &a, const Ct
     else if constexpr (W + 1 < nw5(NB)) dispatch5<NB, W + 1>(w, a, C, tp, have, L, iL, toff);
 }
 
-// lpc5 multiplets per CTA on nw5 warps each (8 warps at up to 8 bins: 255 registers)
+// Up to 8 bins: lpc5 = 4 multiplets per CTA on two warps each.  9 and 10 bins (3 / 5 warp roles per multiplet): the 8 warps of
+// a CTA take (multiplet, role) units of up to four consecutive multiplets, so that no warp slot stays empty
+// (C.lam[w] = 8 * multiplet + role, C.scr[w] = the term slot of that multiplet, C.lam[8 + s] = multiplet staged in slot s).
+__host__ __device__ constexpr int cta_warps5(int nb) { return nb >= 9 ? 8 : nw5(nb) * lpc5(nb); }
 template <int NB>
-__global__ void __launch_bounds__(nw5(NB) * lpc5(NB) * 32, 1) k_contract5(ContractArgs a)
+__global__ void __launch_bounds__(cta_warps5(NB) * 32, 1) k_contract5(ContractArgs a)
 {
     constexpr int NW = nw5(NB);
     __shared__ CtaPlan C;
     if (threadIdx.x < sizeof(CtaPlan) / sizeof(int)) reinterpret_cast<int *>(&C)[threadIdx.x] = reinterpret_cast<const int *>(a.ctas + blockIdx.y)[threadIdx.x];
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int iLs = C.lam[warp / NW];
-    const bool have = iLs >= 0;
-    const int iL = have ? iLs : 0;
-    const Lam5 L = a.lam5[iL];
-    const TilePipe tp = make_pipe(C);
-    const int toff = tp.bar + kBarDoubles + (warp / NW) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
-    if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
-    __syncthreads();
-    dispatch5<NB, 0>(warp % NW, a, C, tp, have, L, iL, toff);
+    if constexpr (NB >= 9) {
+        const int unit = C.lam[warp];
+        const bool have = unit >= 0;
+        const int iL = have ? unit >> 3 : 0, role = have ? unit & 7 : 0;
+        const Lam5 L = a.lam5[iL];
+        const TilePipe tp = make_pipe(C);
+        const int tbase = tp.bar + kBarDoubles;
+        if (warp < 4 && C.lam[8 + warp] >= 0) {
+            const Lam5 &S = a.lam5[C.lam[8 + warp]];
+            stage_terms(tbase + warp * 6 * a.max_terms, a.pair_terms + S.lbeg[0], S.nterms, lane);
+        }
+        __syncthreads();
+        dispatch5<NB, 0>(role, a, C, tp, have, L, iL, tbase + C.scr[warp] * 6 * a.max_terms);
+    } else {
+        const int iLs = C.lam[warp / NW];
+        const bool have = iLs >= 0;
+        const int iL = have ? iLs : 0;
+        const Lam5 L = a.lam5[iL];
+        const TilePipe tp = make_pipe(C);
+        const int toff = tp.bar + kBarDoubles + (warp / NW) * 6 * a.max_terms; // left terms first, right terms behind them (host order)
+        if (have && warp % NW == 0) stage_terms(toff, a.pair_terms + L.lbeg[0], L.nterms, lane);
+        __syncthreads();
+        dispatch5<NB, 0>(warp % NW, a, C, tp, have, L, iL, toff);
+    }
 }
 
 // ---- host side: multiplets -> CTAs, l-blocks per CTA, shared memory ----------------------------------------------
@@ -761,7 +779,7 @@ cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
     if (attr_err != cudaSuccess) return attr_err;
-    k_contract5<NB><<<dim3(a.nchunk, a.ncta), nw5(NB) * lpc5(NB) * 32, a.cta_smem, s>>>(a);
+    k_contract5<NB><<<dim3(a.nchunk, a.ncta), cta_warps5(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -805,6 +823,54 @@ size_t contraction_plan_ctas(const HostTables &T, std::vector<CtaPlan> &ctas)
         return b;
     };
     std::vector<unsigned> masks;
+    if (T.order == 5 && T.nbins >= 9) {
+        // (multiplet, role) units of consecutive multiplets fill the 8 warps of a CTA; at most four multiplets (term slots)
+        const int nw = nw5(T.nbins);
+        const size_t extra5 = kBarDoubles * sizeof(double) + sizeof(CtaPlan) + (size_t)4 * max_terms * sizeof(PairTerm);
+        int fillw = 8, nslots = 0;
+        for (int k = 0; k < nL; ++k) {
+            const int iL = T.lam_order[k];
+            int l[4];
+            const int nl = ls_of(iL, l);
+            unsigned m = 0;
+            for (int j = 0; j < nl; ++j) m |= 1u << l[j];
+            if (tile_bytes(m) + extra5 > kSmemLimit) return 0;
+            for (int role = 0; role < nw; ++role) {
+                bool fresh = ctas.empty() || fillw == 8;
+                if (!fresh) {
+                    const bool staged = nslots > 0 && ctas.back().lam[8 + nslots - 1] == iL;
+                    if ((!staged && nslots == 4) || tile_bytes(masks.back() | m) + extra5 > kSmemLimit) fresh = true;
+                }
+                if (fresh) {
+                    CtaPlan c{};
+                    for (int j = 0; j < 12; ++j) c.lam[j] = -1;
+                    ctas.push_back(c);
+                    masks.push_back(0u);
+                    fillw = 0; nslots = 0;
+                }
+                CtaPlan &c = ctas.back();
+                if (nslots == 0 || c.lam[8 + nslots - 1] != iL) c.lam[8 + nslots++] = iL;
+                c.scr[fillw] = nslots - 1;
+                c.lam[fillw++] = 8 * iL + role;
+                masks.back() |= m;
+            }
+        }
+        size_t smem5 = 0;
+        for (size_t i = 0; i < ctas.size(); ++i) {
+            CtaPlan &c = ctas[i];
+            int off = 0;
+            c.nblk = 0;
+            for (int l = 0; l <= ENCORE_MAX_LMAX; ++l) {
+                c.off[l] = -1;
+                if (l <= T.lmax && (masks[i] >> l & 1u)) { c.bl[c.nblk++] = l; c.off[l] = off; off += (2 * l + 1) * T.nbins * 32; }
+            }
+            c.tile = off;
+            const size_t tb = (size_t)off * sizeof(double);
+            c.nbuf = 2 * tb + extra5 <= kSmemLimit ? 2 : 1;
+            smem5 = std::max(smem5, c.nbuf * tb + extra5);
+        }
+        return smem5;
+    }
     int fill = lpc;
     for (int k = 0; k < nL; ++k) {
         const int iL = T.lam_order[k];
