@@ -570,6 +570,10 @@ __device__ __forceinline__ void pairs_block_half(double (&z)[NZ], const PairTerm
 // ---- how the second bins 1 .. NB-3 of a multiplet are dealt to its warps -----------------------------------
 // Up to 8 bins: two warps, b2 <= T and b2 > T (T = t5(NB), measured on c5).  9 and 10 bins: consecutive ranges grown
 // greedily while partial sums + held coupled pairs stay under 105 doubles (3 and 5 warps).
+#ifndef ENCORE_REGS5
+#define ENCORE_REGS5 105
+#endif
+constexpr int kRegs5 = ENCORE_REGS5;    // doubles a warp role of the N = 5 kernel may hold at 9-10 bins
 __host__ __device__ constexpr int regs5(int nb, int lo, int hi)
 {
     return ntot5(nb, lo, hi) + 2 * c2(nb - 1 - lo) + 2 * (c2(hi + 1) - c2(lo));
@@ -585,7 +589,7 @@ __host__ __device__ constexpr int hi5(int nb, int w)
     if (nb <= 8) return w == 0 ? t5(nb) : nb - 3;
     const int lo = lo5(nb, w);
     int hi = lo;
-    while (hi + 1 <= nb - 3 && regs5(nb, lo, hi + 1) <= 105) ++hi;
+    while (hi + 1 <= nb - 3 && regs5(nb, lo, hi + 1) <= kRegs5) ++hi;
     return hi;
 }
 __host__ __device__ constexpr int nw5(int nb)
