@@ -51,7 +51,8 @@ enum {
     ENCORE_ESTATE = -5,   /* diagnostic getter called before a successful encore_compute */
     ENCORE_EUNSUPPORTED = -6, /* valid problem outside what this build's kernels cover (see encore_plan) */
     ENCORE_EINTERNAL = -7, /* a device-side consistency check failed; results must not be used (encore_get_status) */
-    ENCORE_ECAPACITY = -8  /* encore_compute_enqueue: the plan's scratch, sized by its last encore_compute, is too small */
+    ENCORE_ECAPACITY = -8, /* encore_compute_enqueue: the plan's scratch, sized by its last encore_compute, is too small */
+    ENCORE_ETOOBIG = -9    /* encore_edge_correct_noalloc: the problem needs more than the library's fixed scratch array holds */
 };
 
 /* Build a plan: the Lambda / B / M tables with weights 2 S(m_{N-1}) E(Lam) C^Lam_M (eq. 44, PAPER.md:428-430;
@@ -150,6 +151,37 @@ int encore_compute_grid(encore_plan_t *plan, const double *delta, int G, double 
 int encore_edge_correct(encore_plan_t *plan, const double *n_raw, const double *r_raw, double *zeta_out, void *cuda_stream);
 /* host query (no GPU needed): the tensor encore_edge_correct uses, out[(i n + j) n + k] = E(Lam_k) G^{Lam_i Lam_j Lam_k}, n = n_Lambda */
 int encore_get_gaunt_tensor(const encore_plan_t *plan, double *out /* HOST n_Lambda^3 */);
+
+/* Edge correction for callers that must not allocate device memory.
+ *
+ * Who this is for: encore_edge_correct keeps its per-bin-tuple matrices in plan-owned buffers that it cudaMallocs (and
+ * grows) on demand.  Some hosts cannot accept that: a serving or training process that has handed all of HBM to its own
+ * pool allocator (a cudaMalloc there fails, or breaks the pool's accounting), a job running under a fixed device-memory
+ * quota, and latency-bound loops in which cudaMalloc / cudaFree are unwelcome because they take driver-wide locks and
+ * cudaFree waits for the whole device, stalling unrelated streams.  This entry point calls no cudaMalloc, no cudaFree and
+ * no library routine that allocates; it needs no plan on the device.  The caller passes every input and the output:
+ *   gaunt     DEVICE, n_lambda^3 doubles: the tensor of encore_get_gaunt_tensor (a host query), copied to the device by the caller
+ *   n_raw     DEVICE [n_lambda][n_b], raw multiplets of the D - R field      (as for encore_edge_correct)
+ *   r_raw     DEVICE [n_lambda][n_b], raw multiplets of the random field; row 0 must be Lambda = 0
+ *   zeta_out  DEVICE [n_lambda][n_b], written; may not alias an input
+ * The result is that of encore_edge_correct on the same inputs (same kernels, same order of operations).
+ *
+ * The scratch (n_b matrices of n_lambda^2 doubles and n_b right-hand sides) lives in ONE fixed array compiled into the
+ * library, ENCORE_EDGE_NOALLOC_MAX_DOUBLES doubles (8 MiB) of device memory that every GPU which loads the library keeps
+ * until the process exits.  Limit:  n_b * n_lambda * (n_lambda + 1) <= ENCORE_EDGE_NOALLOC_MAX_DOUBLES  (the c3/c4 shape,
+ * 69 multiplets x 120 bin tuples, needs 579 600); anything larger is refused with ENCORE_ETOOBIG before any GPU work,
+ * n_lambda < 1 or n_b < 1 or a NULL pointer with ENCORE_EINVAL.
+ *
+ * First call on a device: it looks up the array's address on the current device (cudaGetSymbolAddress) and remembers it
+ * per device; make that first call, with the device current, before starting any stream capture.  Later calls only launch
+ * the two kernels on cuda_stream and return without synchronising.
+ * Sharing: every call on a device uses the same array.  The part a call uses is overwritten in full before it is read, so
+ * nothing left behind by an earlier call (of any shape) can reach the result and nothing needs clearing; but two calls
+ * whose kernels can overlap on the GPU - different streams, or two host threads - race on it and give garbage.  Keep all
+ * calls of a device on one stream, or order them with events. */
+#define ENCORE_EDGE_NOALLOC_MAX_DOUBLES 1048576
+int encore_edge_correct_noalloc(const double *gaunt, const double *n_raw, const double *r_raw, int n_lambda, int n_b,
+                                double *zeta_out, void *cuda_stream);
 
 /* Plan options (host call, takes effect at the next encore_compute).  No behaviour is read from the environment.
  *   "list_mb"          byte budget, in MiB, of the pair stage's acceptance-mask rows per super-step (0 = default:

@@ -20,11 +20,11 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
-OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL, ECAPACITY = 0, -1, -2, -3, -4, -5, -6, -7, -8
+OK, EINVAL, EDOMAIN, EALLOC, ECUDA, ESTATE, EUNSUPPORTED, EINTERNAL, ECAPACITY, ETOOBIG = 0, -1, -2, -3, -4, -5, -6, -7, -8, -9
 
 # every symbol include/encore.h declares (tests check the .so exports all of them)
 SYMBOLS = [
-    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_enqueue", "encore_query_grid", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_get_gaunt_tensor", "encore_compute_grid",
+    "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_enqueue", "encore_query_grid", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_edge_correct_noalloc", "encore_get_gaunt_tensor", "encore_compute_grid",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
@@ -62,6 +62,7 @@ def lib():
     L.encore_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
     L.encore_get_status.argtypes = [vp]
     L.encore_edge_correct.argtypes = [vp, vp, vp, vp, vp]
+    L.encore_edge_correct_noalloc.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.encore_get_gaunt_tensor.argtypes = [vp, dp]
     L.encore_compute_grid.argtypes = [vp, vp, C.c_int, vp, vp]
     L.encore_destroy.argtypes = [vp]
@@ -179,6 +180,17 @@ def encore_set_option(plan, key: str, value: int):
 def encore_edge_correct(plan, n_raw, r_raw, zeta_out, cuda_stream: int = 0):
     """n_raw, r_raw, zeta_out: CUDA fp64 tensors [n_lambda, n_b] (or raw device pointers)."""
     _check(lib().encore_edge_correct(plan, _ptr(n_raw), _ptr(r_raw), _ptr(zeta_out), C.c_void_p(cuda_stream)))
+
+
+def encore_edge_correct_noalloc(gaunt, n_raw, r_raw, n_lambda: int, n_b: int, zeta_out, cuda_stream: int = 0):
+    """Edge correction for callers that must not allocate device memory (a process whose HBM belongs to its own pool
+    allocator, a fixed memory quota, a loop that cannot take the device-wide stalls of cudaMalloc / cudaFree).
+    gaunt: CUDA fp64 tensor [n_lambda]^3, the caller's device copy of encore_get_gaunt_tensor; n_raw, r_raw, zeta_out:
+    CUDA fp64 [n_lambda, n_b].  The library allocates nothing: its scratch is a fixed 8 MiB device array, which limits
+    n_b * n_lambda * (n_lambda + 1) to ENCORE_EDGE_NOALLOC_MAX_DOUBLES = 2^20 (ETOOBIG beyond).  Calls on one device
+    share that array: keep them on one stream.  The first call on a device should come before any stream capture."""
+    _check(lib().encore_edge_correct_noalloc(_ptr(gaunt), _ptr(n_raw), _ptr(r_raw), int(n_lambda), int(n_b), _ptr(zeta_out),
+                                             C.c_void_p(cuda_stream)))
 
 
 def encore_compute_grid(plan, delta, G: int, zeta_out, cuda_stream: int = 0):

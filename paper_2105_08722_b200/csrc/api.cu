@@ -722,6 +722,18 @@ int encore_edge_correct(encore_plan_t *P, const double *n_raw, const double *r_r
     return ENCORE_OK;
 }
 
+// Edge correction for callers that may not allocate device memory (see include/encore.h): no plan, no cudaMalloc / cudaFree;
+// the scratch is the fixed device array in edge.cu.  Sizes beyond it are refused here, before anything touches the GPU.
+int encore_edge_correct_noalloc(const double *gaunt, const double *n_raw, const double *r_raw, int n_lambda, int n_b,
+                                double *zeta_out, void *cuda_stream)
+{
+    if (!gaunt || !n_raw || !r_raw || !zeta_out || n_lambda < 1 || n_b < 1) return ENCORE_EINVAL;
+    const unsigned long long need = (unsigned long long)n_b * (unsigned long long)n_lambda * ((unsigned long long)n_lambda + 1ull);
+    if (need > (unsigned long long)ENCORE_EDGE_NOALLOC_MAX_DOUBLES) return ENCORE_ETOOBIG;
+    CU(launch_edge_correct_noalloc(gaunt, n_raw, r_raw, n_lambda, n_b, zeta_out, static_cast<cudaStream_t>(cuda_stream)));
+    return ENCORE_OK;
+}
+
 int encore_get_gaunt_tensor(const encore_plan_t *P, double *out)
 {
     if (!P || !out) return ENCORE_EINVAL;
@@ -1038,6 +1050,7 @@ const char *encore_strerror(int status)
     case ENCORE_EUNSUPPORTED: return "configuration not covered by this build's kernels";
     case ENCORE_EINTERNAL: return "internal consistency check of the pair stage failed (please report)";
     case ENCORE_ECAPACITY: return "encore_compute_enqueue: the plan's scratch (sized by its last encore_compute) is too small for this input";
+    case ENCORE_ETOOBIG: return "encore_edge_correct_noalloc: n_b * n_lambda * (n_lambda + 1) exceeds ENCORE_EDGE_NOALLOC_MAX_DOUBLES, the library's fixed scratch array";
     default: return "unknown status";
     }
 }

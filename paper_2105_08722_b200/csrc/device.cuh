@@ -145,6 +145,9 @@ cudaError_t launch_reduction(const ContractArgs &a, cudaStream_t s, int *launche
 // T: [n][n][n] E G tensor; Nraw, Rraw: [n][nB] raw multiplets; A: [nB][n][n], rhs: [nB][n] scratch; zeta: [n][nB]
 cudaError_t launch_edge_correct(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *A, double *rhs,
                                 double *zeta, cudaStream_t s);
+// same kernels with A and rhs in the library's fixed file-scope device array (no allocation; sizes checked by the caller)
+cudaError_t launch_edge_correct_noalloc(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *zeta,
+                                        cudaStream_t s);
 
 // ---- mesh.cu (gridded estimator, eq. 36) ------------------------------------------------------------------
 cudaError_t launch_mesh_alm(const double *delta, int G, double box, int lmax, int nb, const double *e2, const double *vinv,

@@ -7,7 +7,10 @@
 // tensor T = E G (host tables from App. A's closed forms) sits in HBM; one CTA per bin tuple assembles A = M^T and solves
 // A zeta = rhs by LU with partial pivoting (fixed order of operations: deterministic).  Tiny next to the pair stage:
 // 120 systems of 69 unknowns at c3/c4.
+#include "../../include/encore.h"
 #include "device.cuh"
+
+#include <mutex>
 
 namespace {
 
@@ -108,6 +111,58 @@ __global__ void __launch_bounds__(kEdgeThreads) k_edge_solve(double *__restrict_
 cudaError_t launch_edge_correct(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *A, double *rhs,
                                 double *zeta, cudaStream_t s)
 {
+    k_edge_assemble<<<nB, kEdgeThreads, sizeof(double) * n, s>>>(T, Nraw, Rraw, n, nB, A, rhs);
+    k_edge_solve<<<nB, kEdgeThreads, 0, s>>>(A, rhs, n, nB, zeta);
+    return cudaGetLastError();
+}
+
+// ---- edge correction without allocating (encore_edge_correct_noalloc, include/encore.h) ---------------------------------
+// For callers that may not cudaMalloc (all of HBM handed to a pool allocator, a fixed memory quota, a loop that cannot
+// afford the device-wide stalls of cudaMalloc / cudaFree).  The A and rhs scratch of the two kernels above sits in one
+// file-scope device array of fixed size; every GPU that loads this library holds its 8 MiB until the process exits.
+// NOTE for host code in this file: `g_edge_scratch` below is the HOST-side handle of the symbol, not a device address.
+// Only cudaGetSymbolAddress turns it into a pointer a kernel may be given; that pointer differs from device to device.
+namespace {
+
+static __device__ __align__(256) double g_edge_scratch[ENCORE_EDGE_NOALLOC_MAX_DOUBLES];
+
+constexpr int kCachedDevices = 64;
+std::mutex g_edge_scratch_mu;
+double *g_edge_scratch_addr[kCachedDevices]; // device address of g_edge_scratch on device d; nullptr: not looked up yet
+
+// address of the scratch array on the CURRENT device; looked up once per device (devices >= 64: every call)
+cudaError_t edge_scratch_address(double **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cache = dev >= 0 && dev < kCachedDevices;
+    std::lock_guard<std::mutex> lock(g_edge_scratch_mu);
+    if (cache && g_edge_scratch_addr[dev]) {
+        *out = g_edge_scratch_addr[dev];
+        return cudaSuccess;
+    }
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_edge_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if (cache) g_edge_scratch_addr[dev] = static_cast<double *>(p);
+    *out = static_cast<double *>(p);
+    return cudaSuccess;
+}
+
+} // namespace
+
+// The caller (api.cu) has checked nB * n * (n + 1) <= ENCORE_EDGE_NOALLOC_MAX_DOUBLES.  No allocation on any path.
+// A[b] and rhs[b] are written in full by k_edge_assemble before k_edge_solve reads them: stale contents of the shared
+// array never matter, and nothing has to be cleared.  Calls that overlap on the GPU would race on the array.
+cudaError_t launch_edge_correct_noalloc(const double *T, const double *Nraw, const double *Rraw, int n, int nB, double *zeta,
+                                        cudaStream_t s)
+{
+    double *scratch = nullptr;
+    const cudaError_t e = edge_scratch_address(&scratch);
+    if (e != cudaSuccess) return e;
+    double *A = scratch, *rhs = scratch + (size_t)nB * n * n;
     k_edge_assemble<<<nB, kEdgeThreads, sizeof(double) * n, s>>>(T, Nraw, Rraw, n, nB, A, rhs);
     k_edge_solve<<<nB, kEdgeThreads, 0, s>>>(A, rhs, n, nB, zeta);
     return cudaGetLastError();
