@@ -9,7 +9,8 @@
  *
  * for N = 3, 4, 5, 6 (Lam = {l}, {l1 l2 l3}, {l1 l2 (l12) l3 l4}, {l1 l2 (l12) l3 (l123) l4 l5}; eqs. 16, 18, 5/20 —
  * PAPER.md:135, :145, :69, :157),
- * even-parity multiplets only (real zeta), ordered distinct bins b_1 < .. < b_{N-1},
+ * even-parity multiplets (real zeta) and, with ENCORE_ALLPARITY, the parity-odd ones too (imaginary zeta,
+ * stored as Im zeta), ordered distinct bins b_1 < .. < b_{N-1},
  * using the half-sum m_{N-1} >= 0 of eq. 44.  Steps:
  *   a1 cell assignment, a2 counting sort by cell, a3 neighbour sweep + radial binning, a4 a_lm accumulation,
  *   a5 per-primary coupling contraction, a6 deterministic fp64 reduction over primaries.
@@ -76,10 +77,15 @@ int encore_plan(encore_plan_t **plan_out, int npcf_order, double r_min, double r
  * with separations r_j - s_i as in eq. 35 (the sign of odd multiplets depends on it).  Unknown flags: ENCORE_EINVAL. */
 #define ENCORE_ALLPARITY 1u
 /* ENCORE_FP32_HARMONICS (the paper's reduced-precision modes): step a4 evaluates
- * the unit vector, its powers and w (x+iy)^m of every pair in fp32 and adds 16-pair fp32 chunk sums to the fp64 a_lm
- * accumulators.  Separations are formed in fp64 and rounded once; cell ids, the radial binning and therefore every pair
- * count stay those of the fp64 path (bit-exact); contraction and reduction stay fp64.  A separate, separately reported
- * path: zeta agrees with the fp64 result to ~1e-6 of max|zeta| (tests bound it by 1e-5), not to 1e-9. */
+ * the unit vector, its powers and w (x+iy)^m of every pair in fp32 and adds fp32 chunk sums of 64 pairs to the fp64 a_lm
+ * accumulators.  For the bins fp32 resolves (lower edge >= 2^-10 of the largest coordinate measured from the centre of
+ * the box / bounding box) candidates are gathered as 16-byte fp32 records {x, y, z, w} relative to that centre and the
+ * separation is an fp32 subtraction: its components are off by <= 2^-24 of that largest coordinate, i.e. < 2^-13 r.  For the
+ * inner bins the separation is formed in fp64 and rounded once (2^-24 r).  These errors are independent from pair to pair
+ * and average down over the thousands of pairs of a bin; with the <= 64 x 2^-24 of a chunk sum they give the ~1e-6 below.  Cell ids,
+ * the radial binning and therefore every pair count stay those of the fp64 path (bit-exact); contraction and reduction
+ * stay fp64.  A separate, separately reported path: zeta agrees with the fp64 result to ~1e-6 of max|zeta| (tests bound
+ * it by 1e-5), not to 1e-9. */
 #define ENCORE_FP32_HARMONICS 2u
 int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, double r_max, int nbins, int lmax,
                       double box_size, unsigned flags);
@@ -149,7 +155,10 @@ int encore_compute_grid(encore_plan_t *plan, const double *delta, int G, double 
  * the E G tensor on the host (n_Lambda^3 doubles) and synchronises once.  N = 3, 4, 5 and n_Lambda <= 256
  * (ENCORE_EUNSUPPORTED otherwise: N = 6 has no closed form in the paper).  R_0 = 0 or a singular M give non-finite output. */
 int encore_edge_correct(encore_plan_t *plan, const double *n_raw, const double *r_raw, double *zeta_out, void *cuda_stream);
-/* host query (no GPU needed): the tensor encore_edge_correct uses, out[(i n + j) n + k] = E(Lam_k) G^{Lam_i Lam_j Lam_k}, n = n_Lambda */
+/* host query (no GPU needed): the tensor encore_edge_correct uses, out[(i n + j) n + k] = E(Lam_k) G^{Lam_i Lam_j Lam_k}, n = n_Lambda.
+ * ENCORE_ALLPARITY plans: rows of parity-odd multiplets hold imaginary parts (coefficient = i x stored value) in n_raw, r_raw
+ * and zeta_out alike; eqs. 40-42 relate the complex coefficients, so the entries with Lam_i and Lam_j BOTH odd (they feed an
+ * even Lam_k) carry the extra factor i x i = -1 in this tensor.  With it the real system on stored values is eq. 41 exactly. */
 int encore_get_gaunt_tensor(const encore_plan_t *plan, double *out /* HOST n_Lambda^3 */);
 
 /* Edge correction for callers that must not allocate device memory.
@@ -196,7 +205,11 @@ int encore_edge_correct_noalloc(const double *gaunt, const double *n_raw, const 
 int encore_set_option(encore_plan_t *plan, const char *key, long long value);
 /* Synchronises the last compute's stream and reports its device-side status: ENCORE_OK, or ENCORE_EINTERNAL if the
  * pair stage's consistency check (one periodic image per candidate word) failed; after
- * encore_compute_enqueue also ENCORE_EDOMAIN / ENCORE_ECAPACITY (see there).  encore_compute_host returns this status itself. */
+ * encore_compute_enqueue also ENCORE_EDOMAIN / ENCORE_ECAPACITY (see there).  encore_compute_host returns this status itself.
+ * After encore_compute_grid it synchronises that call's stream and returns ENCORE_OK (the gridded path has no device-side
+ * checks); encore_get_launch_count and the timers are valid then, the particle diagnostics return ENCORE_ESTATE.
+ * The stream it waits on is the one the compute was ENQUEUED on: after replaying a CUDA graph captured around
+ * encore_compute_enqueue, synchronise the replay stream yourself before calling this. */
 int encore_get_status(const encore_plan_t *plan);
 /* super-steps the pair stage of the last compute took: the acceptance-mask rows of a step stay under the byte budget
  * (option "list_mb"), whole groups per step, steps of equal size.  >= 1, or a status < 0. */
@@ -218,6 +231,12 @@ int encore_get_bin_edges(const encore_plan_t *plan, double *out /* HOST [nbins+1
 /* flop counts per primary of the contraction as executed (fused multiply-add = 2) and by the canonical
  * "Algorithm 3 literal" model of SURVEY.md §8(d) (5/11/17 flop per term evaluation for N=3/4/5) */
 int encore_contraction_flops(const encore_plan_t *plan, double *executed, double *canonical);
+
+/* How the contraction (step a5) of this plan is laid out - a host query for tests and benchmarks, so that they can tell
+ * which kernel and which tile pipeline a shape runs on.  out = { order of the factorised kernel (3, 4, 5, 6) or 0 when the
+ * literal eq. 44 kernel is used,  number of CTA work plans (0 for N = 3 and the literal kernel),  smallest and largest
+ * number of a_lm tile buffers over those CTAs: 1 = one buffer refilled between tiles, 2 = double buffer, 3..8 = ring }. */
+int encore_get_contraction_layout(const encore_plan_t *plan, int out[4] /* HOST */);
 
 /* The grid a compute would build for n particles in the box [bbox_lo, bbox_hi] (open geometry; ignored when the plan is
  * periodic): cells per axis and subdivisions S_a of reading R11 / DESIGN.md §4.1.  Host arithmetic only, no GPU needed. */

@@ -232,17 +232,29 @@ def edge_correct(order: int, lams, N, R, T=None) -> np.ndarray:
         f_Lam'(B) = R_Lam'^B / R_0^B;   M_{Lam Lam''}(B) = sum_Lam' f_Lam'(B) E(Lam'') G^{Lam Lam' Lam''}   (eq. 41)
         sum_Lam zeta_Lam(B) M_{Lam Lam''}(B) = N_Lam''^B / R_0^B                                       (eq. 41) -> solve
     N, R: [nLam, nB] raw multiplets of the data-minus-random and the random field on the multiplet list `lams`, whose
-    first row is the all-zero multiplet.  The basis is truncated to `lams` (as the paper truncates at lmax)."""
+    first row is the all-zero multiplet.  The basis is truncated to `lams` (as the paper truncates at lmax).
+
+    Parity-odd multiplets (ALLPARITY lists): their coefficients are purely imaginary (eq. 8) and the rows of
+    N, R and of the result hold the IMAGINARY part for them (the real part for even multiplets), as `zeta` stores them.
+    Eqs. 40-42 are relations between the complex coefficients, so they are evaluated here in complex arithmetic:
+    coefficient = stored value for even, i * stored value for odd multiplets; the solution is real for even and
+    imaginary for odd multiplets (checked) and is returned in the stored form."""
     lams = np.ascontiguousarray(lams, dtype=np.int32)
     assert not lams[0].any(), "the first multiplet must be Lambda = 0"
     N, R = np.asarray(N, dtype=np.float64), np.asarray(R, dtype=np.float64)
     if T is None:
         T = gaunt_tensor(order, lams)
+    odd = np.array([principal_sum(order, lam) % 2 == 1 for lam in lams])
+    unit = np.where(odd, 1j, 1.0)                       # stored value -> complex coefficient
     out = np.empty_like(N)
     for iB in range(N.shape[1]):
-        f = R[:, iB] / R[0, iB]
-        M = np.einsum("j,ijk->ik", f, T)              # M[Lam, Lam'']
-        out[:, iB] = np.linalg.solve(M.T, N[:, iB] / R[0, iB])
+        f = unit * R[:, iB] / R[0, iB]
+        M = np.einsum("j,ijk->ik", f, T.astype(np.complex128))   # M[Lam, Lam'']
+        z = np.linalg.solve(M.T, unit * N[:, iB] / R[0, iB])
+        stored = np.where(odd, z.imag, z.real)
+        other = np.where(odd, z.real, z.imag)
+        assert np.abs(other).max() <= 1e-9 * max(np.abs(stored).max(), 1e-300), "solution has the wrong reality"
+        out[:, iB] = stored
     return out
 
 

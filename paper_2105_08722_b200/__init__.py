@@ -27,7 +27,7 @@ SYMBOLS = [
     "encore_plan", "encore_plan_flags", "encore_get_multiplet_parity", "encore_compute", "encore_compute_enqueue", "encore_query_grid", "encore_compute_host", "encore_compute_shard", "encore_get_shard_groups", "encore_get_pair_steps", "encore_set_option", "encore_get_status", "encore_edge_correct", "encore_edge_correct_noalloc", "encore_get_gaunt_tensor", "encore_compute_grid",
     "encore_destroy", "encore_zeta_len",
     "encore_num_multiplets", "encore_num_bin_tuples", "encore_num_terms", "encore_get_multiplets",
-    "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_grid",
+    "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_contraction_layout", "encore_get_grid",
     "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
     "encore_get_stage_ms", "encore_get_kernel_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs", "encore_get_harm_steps",
     "encore_measure_fp64_peak", "encore_strerror", "encore_last_cuda_error",
@@ -64,6 +64,7 @@ def lib():
     L.encore_edge_correct.argtypes = [vp, vp, vp, vp, vp]
     L.encore_edge_correct_noalloc.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.encore_get_gaunt_tensor.argtypes = [vp, dp]
+    L.encore_get_contraction_layout.argtypes = [vp, ip]
     L.encore_compute_grid.argtypes = [vp, vp, C.c_int, vp, vp]
     L.encore_destroy.argtypes = [vp]
     L.encore_zeta_len.argtypes = [vp]
@@ -202,6 +203,13 @@ def encore_get_gaunt_tensor(plan) -> np.ndarray:
     out = np.empty((n, n, n))
     _check(lib().encore_get_gaunt_tensor(plan, out.ctypes.data_as(C.POINTER(C.c_double))))
     return out
+
+
+def encore_get_contraction_layout(plan) -> dict:
+    """{'kernel': 3..6 (factorised) or 0 (literal eq. 44), 'ctas': CTA work plans, 'nbuf_min', 'nbuf_max': a_lm tile buffers per CTA}"""
+    out = (C.c_int * 4)()
+    _check(lib().encore_get_contraction_layout(plan, out))
+    return {"kernel": out[0], "ctas": out[1], "nbuf_min": out[2], "nbuf_max": out[3]}
 
 
 def encore_get_status(plan) -> int:

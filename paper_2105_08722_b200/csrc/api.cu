@@ -58,6 +58,7 @@ struct encore_plan_s {
     double *pinned = nullptr; // 16 doubles: bbox[6], flags as 2 ints in [6], internal-error flag as int in [7], padding particle [8..11]
     // state of the last compute
     bool have = false;
+    bool have_grid = false;   // the last compute was encore_compute_grid: stream / launch count / timers are valid, particle diagnostics are not
     int64_t n = 0;
     GridGeom geom{};
     int ngroups_max = 0;
@@ -296,6 +297,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
 {
     const HostTables &T = P->T;
     P->have = false;
+    P->have_grid = false;
     P->launches = 0;
     if (enqueue && !P->uploaded) return ENCORE_ESTATE;
     TRY(upload_tables(P, s));
@@ -562,15 +564,15 @@ int encore_plan_flags(encore_plan_t **plan_out, int npcf_order, double r_min, do
     if (lmax > ENCORE_MAX_LMAX) return ENCORE_EUNSUPPORTED;
     encore_plan_s *P = new (std::nothrow) encore_plan_s();
     if (!P) return ENCORE_EALLOC;
-    try {
+    try {   // everything that grows a std::vector stays inside: nothing may throw across the C ABI
         encore_build_tables(P->T, npcf_order, r_min, r_max, nbins, lmax, box_size, (flags & ENCORE_ALLPARITY) ? 1 : 0);
+        if (npcf_order >= 4 && npcf_order <= 5 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
+        if (npcf_order == 6 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas6(P->T, P->ctas);
     } catch (...) {
         delete P;
         return ENCORE_EALLOC;
     }
     P->fp32_harmonics = (flags & ENCORE_FP32_HARMONICS) != 0;
-    if (npcf_order >= 4 && npcf_order <= 5 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas(P->T, P->ctas);
-    if (npcf_order == 6 && contraction_is_factorised(npcf_order, nbins, lmax)) P->cta_smem = contraction_plan_ctas6(P->T, P->ctas);
     *plan_out = P;
     return ENCORE_OK;
 }
@@ -645,6 +647,10 @@ int encore_set_option(encore_plan_t *P, const char *key, long long value)
 int encore_get_status(const encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
+    if (P->have_grid) {           // gridded estimator: no device-side checks to report, the call is the synchronisation point
+        CU(cudaStreamSynchronize(P->stream));
+        return ENCORE_OK;
+    }
     if (!P->have) return ENCORE_ESTATE;
     CU(cudaStreamSynchronize(P->stream));
     int f = 0, fl[2];
@@ -662,6 +668,7 @@ int encore_compute_grid(encore_plan_t *P, const double *delta, int G, double *ze
     if (!(T.box > 0.0)) return ENCORE_EINVAL;     // the mesh is periodic
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     P->have = false;
+    P->have_grid = false;
     P->launches = 0;
     TRY(upload_tables(P, s));
     const size_t ncell = (size_t)G * G * G, npad = (ncell + 31) / 32 * 32;
@@ -693,6 +700,8 @@ int encore_compute_grid(encore_plan_t *P, const double *delta, int G, double *ze
     if (fft_error) return ENCORE_ECUDA;
     TRY(mark(P, K_HARM, s));
     TRY(contract_and_reduce(P, P->alm.as<double>(), P->gweights.as<double>(), 0, ngroups, ngroups, factorised, nchunk, zeta_out, s));
+    P->stream = s;
+    P->have_grid = true;
     return ENCORE_OK;
 }
 
@@ -731,6 +740,21 @@ int encore_edge_correct_noalloc(const double *gaunt, const double *n_raw, const 
     const unsigned long long need = (unsigned long long)n_b * (unsigned long long)n_lambda * ((unsigned long long)n_lambda + 1ull);
     if (need > (unsigned long long)ENCORE_EDGE_NOALLOC_MAX_DOUBLES) return ENCORE_ETOOBIG;
     CU(launch_edge_correct_noalloc(gaunt, n_raw, r_raw, n_lambda, n_b, zeta_out, static_cast<cudaStream_t>(cuda_stream)));
+    return ENCORE_OK;
+}
+
+int encore_get_contraction_layout(const encore_plan_t *P, int out[4])
+{
+    if (!P || !out) return ENCORE_EINVAL;
+    const HostTables &T = P->T;
+    const bool factorised = !P->force_generic && contraction_is_factorised(T.order, T.nbins, T.lmax) && (T.order == 3 || P->cta_smem > 0);
+    out[0] = factorised ? T.order : 0;
+    out[1] = factorised ? (int)P->ctas.size() : 0;
+    out[2] = out[3] = 0;
+    if (factorised && !P->ctas.empty()) {
+        out[2] = out[3] = P->ctas[0].nbuf;
+        for (const CtaPlan &c : P->ctas) { out[2] = std::min(out[2], c.nbuf); out[3] = std::max(out[3], c.nbuf); }
+    }
     return ENCORE_OK;
 }
 
@@ -986,7 +1010,7 @@ int encore_set_timing(encore_plan_t *P, int enabled)
 int encore_get_launch_count(const encore_plan_t *P)
 {
     if (!P) return ENCORE_EINVAL;
-    return P->have ? P->launches : ENCORE_ESTATE;
+    return (P->have || P->have_grid) ? P->launches : ENCORE_ESTATE;
 }
 
 int encore_get_candidate_pairs(const encore_plan_t *P, uint64_t *out)

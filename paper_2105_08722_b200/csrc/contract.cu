@@ -112,9 +112,8 @@ cudaError_t launch_generic(const ContractArgs &a, cudaStream_t s)
     const int slices = std::max(1, std::min(a.nLam, (8 * 148 * 4 + ng - 1) / ng));
     const dim3 grid(ng, slices);
     if (tile_bytes <= 96 * 1024) {   // at least two CTAs per SM
-        static std::once_flag once;
-        static cudaError_t attr_err = cudaSuccess;
-        std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract_generic<true, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024); });
+        static PerDeviceOnce once;
+        const cudaError_t attr_err = once.run([] { return cudaFuncSetAttribute(k_contract_generic<true, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024); });
         if (attr_err != cudaSuccess) return attr_err;
         k_contract_generic<true, NM><<<grid, kWarps * 32, tile_bytes + term_bytes, s>>>(a);
     } else k_contract_generic<false, NM><<<grid, kWarps * 32, term_bytes, s>>>(a);
@@ -766,9 +765,8 @@ static constexpr size_t kSmemLimit = 224 * 1024;
 template <int NB>
 cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 {
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
+    static PerDeviceOnce once;
+    const cudaError_t attr_err = once.run([] { return cudaFuncSetAttribute(k_contract4<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
     if (attr_err != cudaSuccess) return attr_err;
     // x = chunk (dispatched fastest), y = CTA plan: the CTAs of the heaviest multiplets all start first and the light ones
     // fill the tail (with the plan index on x, a heavy CTA of the last chunk started late: 8.4 against 6.1 by the cost model)
@@ -779,9 +777,8 @@ cudaError_t launch4(const ContractArgs &a, cudaStream_t s)
 template <int NB>
 cudaError_t launch5(const ContractArgs &a, cudaStream_t s)
 {
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
+    static PerDeviceOnce once;
+    const cudaError_t attr_err = once.run([] { return cudaFuncSetAttribute(k_contract5<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit); });
     if (attr_err != cudaSuccess) return attr_err;
     k_contract5<NB><<<dim3(a.nchunk, a.ncta), cta_warps5(NB) * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();

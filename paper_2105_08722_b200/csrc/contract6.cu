@@ -290,9 +290,8 @@ constexpr size_t kSmemLimit6 = 224 * 1024;
 template <int NB>
 cudaError_t launch6(const ContractArgs &a, cudaStream_t s)
 {
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] { attr_err = cudaFuncSetAttribute(k_contract6<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit6); });
+    static PerDeviceOnce once;
+    const cudaError_t attr_err = once.run([] { return cudaFuncSetAttribute(k_contract6<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit6); });
     if (attr_err != cudaSuccess) return attr_err;
     k_contract6<NB><<<dim3(a.nchunk, a.ncta), kWarps6 * 32, a.cta_smem, s>>>(a);
     return cudaGetLastError();

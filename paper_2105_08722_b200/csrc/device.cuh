@@ -2,8 +2,30 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <mutex>
 
 #include "common.h"
+
+// Set-up that CUDA keeps per DEVICE (cudaFuncSetAttribute acts on the current device only): run f once on every device
+// a kernel is launched on, not once per process - a process may hold plans on several GPUs (encore.h binds a plan to the
+// device current at its first compute).  Costs one cudaGetDevice and an uncontended lock per launch.  A failure is not
+// remembered: the next launch tries again.
+struct PerDeviceOnce {
+    std::mutex mu;
+    unsigned long long done[4] = {0, 0, 0, 0};   // bit d: device d is set up (devices >= 256: set up at every launch)
+    template <class F> cudaError_t run(F f)
+    {
+        int dev = -1;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        const bool tracked = dev >= 0 && dev < 256;
+        std::lock_guard<std::mutex> lock(mu);
+        if (tracked && (done[dev >> 6] >> (dev & 63) & 1ull)) return cudaSuccess;
+        e = f();
+        if (e == cudaSuccess && tracked) done[dev >> 6] |= 1ull << (dev & 63);
+        return e;
+    }
+};
 
 // Uniform grid (R11): per axis a, cell size ~ r_max / sub[a]; x is the fast (fine) axis so that a
 // "pencil" (iy,iz) is one contiguous run of the cell-sorted particle array.

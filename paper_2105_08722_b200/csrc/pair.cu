@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(32) k_fill(PairArgs a, int g0, int g1, int nr_
     const double4 mine = a.pos4[first + (lane < cnt ? lane : 0)];
     sp[lane] = mine.x; sp[32 + lane] = mine.y; sp[64 + lane] = mine.z;
     a.gweights[(size_t)g * 32 + lane] = lane < cnt ? mine.w : 0.0;
-    if (lane <= nb) e2[lane] = a.bins.e2[lane];
+    for (int b = lane; b <= nb; b += 32) e2[b] = a.bins.e2[b];   // nb + 1 edges: 33 at ENCORE_MAX_BINS
     for (int b = 0; b < nb; ++b) masks[b * 32 + lane] = 0u;
     // this lane's primary, relative to primary 0, fp32 (lanes beyond the group sit far away: never a hit)
     const float pxf = lane < cnt ? (float)(mine.x - ctr.x) : -1e18f, pyf = (float)(mine.y - ctr.y), pzf = (float)(mine.z - ctr.z);
@@ -950,13 +950,13 @@ cudaError_t launch_harm_t(const PairArgs &a, int g0, int g1, int write_counts, c
     const int grid = (nitems + kHarmWarps - 1) / kHarmWarps;
     // F32: the fp64 accumulators live in shared memory, one column per thread
     constexpr size_t kAccBytes = F32 ? (size_t)ncomp_range(LMAX, MLO, MHI) * kHarmWarps * 32 * sizeof(double) : 0;
-    // the opt-in shared-memory limit is a per-kernel, process-wide attribute: set once per instantiation
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(true, F32) + kAccBytes));
-        if (attr_err == cudaSuccess)
-            attr_err = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(false, F32) + kAccBytes));
+    // the opt-in shared-memory limit is a per-kernel, per-DEVICE attribute: set once per instantiation and device
+    static PerDeviceOnce once;
+    const cudaError_t attr_err = once.run([] {
+        cudaError_t e = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, true, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(true, F32) + kAccBytes));
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_harm<LMAX, MLO, MHI, false, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(harm_smem_bytes(false, F32) + kAccBytes));
+        return e;
     });
     if (attr_err != cudaSuccess) return attr_err;
     if (a.geom.periodic) k_harm<LMAX, MLO, MHI, true, F32><<<grid, kHarmWarps * 32, harm_smem_bytes(true, F32) + kAccBytes, s>>>(a, g0, g1, write_counts);
@@ -1005,12 +1005,12 @@ cudaError_t launch_pair_fill(const PairArgs &a, int g0, int g1, int nr_cap, cuda
 {
     const int ng = g1 - g0, nb = a.bins.nbins;
     if (ng <= 0) return cudaSuccess;
-    // the opt-in shared-memory limit is a per-kernel, process-wide attribute: set it once, to the most any plan asks for
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(k_fill<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (attr_err == cudaSuccess) attr_err = cudaFuncSetAttribute(k_fill<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    // the opt-in shared-memory limit is a per-kernel, per-DEVICE attribute: set it once per device, to the most any plan asks for
+    static PerDeviceOnce once;
+    const cudaError_t attr_err = once.run([] {
+        cudaError_t e = cudaFuncSetAttribute(k_fill<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fill<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        return e;
     });
     if (attr_err != cudaSuccess) return attr_err;
     const size_t smem = fill_smem_bytes(nb, nr_cap);

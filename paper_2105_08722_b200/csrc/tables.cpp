@@ -515,7 +515,12 @@ int encore_build_gaunt_tensor(const HostTables &t, std::vector<double> &T)
                     if (g != 0.0L) g *= wigner9j(a[0], a[1], a[2], b[0], b[1], b[2], c[0], c[1], c[2]);
                     if (g != 0.0L) g *= wigner9j(a[2], a[3], a[4], b[2], b[3], b[4], c[2], c[3], c[4]) / (fourpi * fourpi);
                 }
-                const double v = (double)(t.parity[k] ? -g : g);
+                // E(Lam'') = (-1)^{parity of Lam''}.  ALLPARITY lists: zeta, N, R rows of odd multiplets hold the imaginary parts
+                // (coefficient = i * stored value), so an (odd Lam, odd Lam') pair feeding an even Lam'' carries i * i = -1 in
+                // eq. 40; (odd, even) -> odd and (even, odd) -> odd keep their sign (i on both sides).
+                long double sgn = t.parity[k] ? -1.0L : 1.0L;
+                if (t.parity[i] && t.parity[j]) sgn = -sgn;
+                const double v = (double)(sgn * g);
                 T[((size_t)i * n + j) * n + k] = v;
                 T[((size_t)j * n + i) * n + k] = v;
             }

@@ -122,6 +122,19 @@ def test_small_clouds_open_and_periodic(E, oracle, order, nbins, lmax):
     check_full(E, oracle, order, pos, w, 90.0, 4.0, 44.0, nbins, lmax)
 
 
+@pytest.mark.parametrize("order,lmax", [(3, 2), (4, 1)])
+def test_maximum_bin_count_open_and_small_periodic_box(E, oracle, order, lmax):
+    """nbins = 32 = ENCORE_MAX_BINS has 33 bin edges, one more than a warp has lanes: every edge must reach k_fill's
+    shared copy (pairs near a bin edge and all pairs of 'wide' periodic groups are decided on it).  Open geometry and a
+    periodic box small enough that groups span more than half of it."""
+    rng = np.random.default_rng(3200 + order)
+    n = 200
+    pos = np.ascontiguousarray(rng.uniform(0, 50.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.3, 0.7])
+    check_full(E, oracle, order, pos, w, 0.0, 1.0, 24.5, 32, lmax)
+    check_full(E, oracle, order, pos, w, 50.0, 1.0, 24.5, 32, lmax)
+
+
 @pytest.mark.parametrize("order,nbins", [(3, 6), (3, 7), (3, 8), (3, 9), (3, 12), (4, 4), (4, 5), (4, 6), (4, 7), (4, 8), (4, 9), (4, 11),
                                          (5, 6), (5, 7), (5, 9), (5, 10), (5, 11)])
 def test_every_bin_count_of_the_factorised_contraction(E, oracle, order, nbins):
@@ -157,6 +170,58 @@ def test_paper_gpu_shapes_and_largest_factorised_shapes(E, oracle, order, nbins,
     assert (counts == o["bin_counts"]).all()
     scale = np.abs(o["zeta"]).max()
     assert np.abs(z - o["zeta"]).max() <= TOL * scale
+
+
+# (order, nbins, lmax, allparity, n, nchunk, expected (nbuf_min, nbuf_max) of the CTA plans)
+DEEP = [
+    # (a) N = 4, lmax 6 at 9-10 bins: the heaviest CTAs hold ONE tile buffer that is refilled between tiles
+    (4, 9, 6, False, 2000, 1, (1, 2)), (4, 10, 6, False, 2000, 1, (1, 2)), (4, 9, 6, True, 2000, 1, (1, 2)),
+    (4, 10, 6, True, 2000, 2, (1, 2)), (4, 10, 10, False, 1300, 1, (1, 2)),
+    # (b) N = 6: ring of 3-8 buffers (6 bins: every CTA has 8; 7 bins: 7-8; 8-10 bins: everything from 1 to 8)
+    (6, 6, 2, False, 2000, 1, (8, 8)), (6, 7, 2, False, 2000, 1, (7, 8)), (6, 8, 2, False, 2000, 1, (1, 8)),
+    (6, 8, 2, True, 1300, 2, (1, 8)), (6, 10, 2, False, 2000, 1, (1, 8)), (6, 6, 3, False, 1100, 1, (5, 8)),
+    # (c) N = 5 at 9-10 bins: (multiplet, warp role) units, two buffers
+    (5, 9, 3, False, 2000, 1, (2, 2)), (5, 10, 3, False, 2000, 1, (2, 2)), (5, 10, 4, False, 1300, 1, (2, 2)),
+    (5, 10, 5, False, 640, 1, (2, 2)), (5, 9, 3, True, 1300, 2, (2, 2)),
+]
+
+
+@pytest.mark.parametrize("order,nbins,lmax,allparity,n,nchunk,nbuf", DEEP)
+def test_tile_pipeline_steady_state(E, oracle, order, nbins, lmax, allparity, n, nchunk, nbuf):
+    """The factorised contraction kernels stream one a_lm tile per group of 32 primaries through shared memory; CTA x of a
+    multiplet column takes the groups x, x + nchunk, ...  With the automatic nchunk (28-40) a cloud the oracle can afford
+    gives a CTA one or two tiles, so the refill of a single buffer (N = 4, lmax 6, 9-10 bins), the wrap-around of the
+    3-8-buffer ring (N = 6) and the unit loop of N = 5 at 9-10 bins would never reach their steady state.  Here nchunk is
+    forced to 1 or 2: every CTA streams >= 20 tiles, all compared with the oracle element by element
+    (agreement for all Lambda, N in {3,4,5,6}); the buffer counts are asserted so that the case cannot
+    silently land on another pipeline."""
+    rng = np.random.default_rng(11000 + 100 * order + 10 * nbins + lmax + int(allparity))
+    pos = np.ascontiguousarray(rng.uniform(0, 100.0, (3, n)))
+    w = rng.uniform(0.5, 1.5, n) * rng.choice([-1.0, 1.0], n, p=[0.2, 0.8])
+    o = oracle.zeta(order, pos, w, 0.0, 3.0, 45.0, nbins, lmax, allparity=allparity)
+    dev = torch.device("cuda:0")
+    with E.Plan(order, 3.0, 45.0, nbins, lmax, 0.0, allparity=allparity) as plan:
+        lay = E.encore_get_contraction_layout(plan.h)
+        assert lay["kernel"] == order and lay["ctas"] > 0
+        assert (lay["nbuf_min"], lay["nbuf_max"]) == nbuf
+        E.encore_set_option(plan.h, "nchunk", nchunk)
+        tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+        z = plan.compute(tp, tw).cpu().numpy()
+        assert E.encore_get_status(plan.h) == E.OK
+        ngroups = E.encore_get_shard_groups(plan.h)[2]
+        assert ngroups // nchunk >= 20                      # tiles per CTA
+        counts, _ = E.encore_get_bin_counts(plan.h, nbins)
+        par = E.encore_get_multiplet_parity(plan.h).astype(bool)
+        z_again = plan.compute(tp, tw).cpu().numpy()
+        E.encore_set_option(plan.h, "nchunk", 0)            # the automatic grid on the same cloud
+        z_auto = plan.compute(tp, tw).cpu().numpy()
+    assert (counts == o["bin_counts"]).all()
+    expect = np.where(par[:, None], o["zeta_im"], o["zeta"]) if allparity else o["zeta"]
+    scale = np.abs(expect).max()
+    assert scale > 0
+    assert np.abs(z - expect).max() <= TOL * scale
+    assert np.array_equal(z, z_again)                       # deterministic
+    assert np.abs(z_auto - expect).max() <= TOL * scale
 
 
 @pytest.mark.parametrize("nbins,lmax,box,allparity,n", [(5, 2, 0.0, False, 160), (6, 1, 90.0, False, 200), (7, 1, 0.0, True, 120),
@@ -256,6 +321,19 @@ def test_edge_correction_matches_the_oracle(E, oracle, order, nbins, lmax):
         z2 = plan.edge_correct(torch.from_numpy(N).to(dev), torch.from_numpy(R).to(dev)).cpu().numpy()
         ref2 = oracle.edge_correct(order, lams, N, R, T)
         assert np.abs(z2 - ref2).max() <= 1e-9 * np.abs(ref2).max()
+    # ALLPARITY plan: odd multiplets hold imaginary parts; the oracle solves eq. 41/42 in complex arithmetic
+    if order in (4, 5):
+        with E.Plan(order, 20.0, 160.0, nbins, min(lmax, 2), 0.0, allparity=True) as pa:
+            la = pa.multiplets
+            odd = np.array([oracle.principal_sum(order, x) % 2 == 1 for x in la])
+            assert odd.any()
+            R = rng.standard_normal((pa.n_lambda, pa.n_b)) * 0.3        # odd geometry multiplets well away from zero
+            R[0] = rng.uniform(1.0, 2.0, pa.n_b)
+            R[1:] *= R[0]
+            N = rng.standard_normal((pa.n_lambda, pa.n_b))
+            z3 = pa.edge_correct(torch.from_numpy(N).to(dev), torch.from_numpy(R).to(dev)).cpu().numpy()
+            ref3 = oracle.edge_correct(order, la, N, R)
+            assert np.abs(z3 - ref3).max() <= 1e-9 * np.abs(ref3).max()
     with E.Plan(6, 20.0, 160.0, 6, 1, 0.0) as p6:
         t = torch.zeros((p6.n_lambda, p6.n_b), dtype=torch.float64, device=dev)
         with pytest.raises(E.EncoreError) as ei:
@@ -277,9 +355,14 @@ def test_gridded_estimator_matches_the_oracle(E, oracle, order, G, nbins, lmax, 
     o = oracle.zeta_grid(order, delta, box, rmin, rmax, nbins, lmax, allparity=allparity)
     dev = torch.device("cuda:0")
     with E.Plan(order, rmin, rmax, nbins, lmax, box, allparity=allparity) as plan:
+        assert E.encore_get_status(plan.h) == E.ESTATE                # nothing computed yet
         z = plan.compute_grid(torch.from_numpy(delta).to(dev))
-        torch.cuda.synchronize()
+        assert E.encore_get_status(plan.h) == E.OK                    # the gridded compute's synchronisation point
         z = z.cpu().numpy()
+        assert E.lib().encore_get_launch_count(plan.h) > 0
+        with pytest.raises(E.EncoreError) as est:                     # particle diagnostics do not exist after a mesh run
+            E.encore_get_bin_counts(plan.h, nbins)
+        assert est.value.status == E.ESTATE
         par = E.encore_get_multiplet_parity(plan.h).astype(bool)
         z2 = plan.compute_grid(torch.from_numpy(delta).to(dev)).cpu().numpy()
     expect = np.where(par[:, None], o["zeta_im"], o["zeta"])

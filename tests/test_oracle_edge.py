@@ -124,3 +124,57 @@ def test_uniform_geometry_limit_and_round_trip(oracle):
         R[1:] = 0.2 * rng.standard_normal((n - 1, nB)) * R[0]                                     # a survey-like f_Lam
         N = np.stack([np.einsum("i,j,ijk->k", zeta[:, b], R[:, b] / R[0, b], T) * R[0, b] for b in range(nB)], axis=1)   # eq. 41
         assert np.abs(oracle.edge_correct(order, lams, N, R, T) - zeta).max() < 1e-10
+
+
+@pytest.mark.parametrize("order,lmax", [(4, 1), (5, 1)])
+def test_parity_odd_multiplets_in_the_edge_correction(oracle, order, lmax):
+    """ALLPARITY lists: odd multiplets have imaginary coefficients and odd basis functions are imaginary.
+    (i) eqs. 39-40 in complex arithmetic at a random set of directions: with zeta_Lam = i z_Lam and
+    R_Lam' = i phi_Lam' for odd multiplets, zeta(R^) and R(R^) are real, and the coefficients N_Lam'' = sum zeta_Lam R_Lam'
+    E(Lam'') G^{Lam Lam' Lam''}, summed over ALL Lam'' the product reaches, rebuild the function zeta(R^) R(R^); they are
+    real for even and imaginary for odd Lam''.  (ii) the stored (Re / Im) rows of that N and R, on a list closed under the
+    product, go through oracle.edge_correct and return the stored zeta - which fails if the factor i * i = -1 of an
+    (odd, odd) -> even coupling, e.g. G^{111,111,000} = -(4 pi)^{-3/2}, is dropped."""
+    rng = np.random.default_rng(4100 + order)
+    lams = oracle.multiplets(order, lmax, allparity=True)
+    odd = np.array([oracle.principal_sum(order, lam) % 2 == 1 for lam in lams])
+    assert odd.any() and not odd[0]
+    n = len(lams)
+    z = rng.standard_normal(n)                       # stored values
+    phi = 0.3 * rng.standard_normal(n)
+    phi[0] = 1.5
+    unit = np.where(odd, 1j, 1.0)
+    zc, rc = unit * z, unit * phi
+    # every multiplet the products P_Lam P_Lam' reach: principal l'' <= 2 lmax, intermediates free
+    big = oracle.multiplets(order, 2 * lmax, allparity=True)
+    if order == 5:   # the intermediate l12'' of a product is not capped by 2 lmax in `multiplets`; list them all
+        big = np.array([[a, b, c, d, e] for a in range(2 * lmax + 1) for b in range(2 * lmax + 1) for c in range(abs(a - b), a + b + 1)
+                        for d in range(2 * lmax + 1) for e in range(abs(c - d), c + d + 1) if e <= 2 * lmax], dtype=np.int32)
+    big_odd = np.array([oracle.principal_sum(order, lam) % 2 == 1 for lam in big])
+    Nc = np.zeros(len(big), dtype=complex)
+    for k, c in enumerate(big):
+        e = -1.0 if big_odd[k] else 1.0
+        for i in range(n):
+            for j in range(n):
+                g = oracle.generalized_gaunt(order, lams[i], lams[j], c)
+                if g != 0.0:
+                    Nc[k] += zc[i] * rc[j] * e * g
+    assert np.abs(np.where(big_odd, Nc.real, Nc.imag)).max() < 1e-14
+    assert np.abs(Nc[big_odd]).max() > 1e-3 and np.abs(Nc[~big_odd]).max() > 1e-3
+    u = rng.standard_normal((order - 1, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    Y = [oracle.ylm(2 * lmax, v) for v in u]
+    zeta_fn = sum(zc[i] * _P(oracle, order, lams[i], Y) for i in range(n))
+    rand_fn = sum(rc[i] * _P(oracle, order, lams[i], Y) for i in range(n))
+    n_fn = sum(Nc[k] * _P(oracle, order, big[k], Y) for k in range(len(big)) if Nc[k] != 0)
+    assert abs(zeta_fn.imag) < 1e-13 and abs(rand_fn.imag) < 1e-13          # real functions (eq. 8)
+    assert abs(n_fn - zeta_fn * rand_fn) < 1e-12 * max(1.0, abs(zeta_fn * rand_fn))
+    # (ii) truncated to `lams`, as the estimator does: eq. 41 forward in complex arithmetic, eq. 42 back through the oracle
+    T = oracle.gaunt_tensor(order, lams)
+    Nl = np.einsum("i,j,ijk->k", zc, rc, T.astype(complex))
+    N_stored = np.where(odd, Nl.imag, Nl.real)
+    back = oracle.edge_correct(order, lams, N_stored[:, None], phi[:, None], T)[:, 0]
+    assert np.abs(back - z).max() < 1e-11
+    # the (odd, odd) -> even couplings are there and carry weight: dropping their sign changes N
+    oo = np.einsum("i,j,ijk->k", np.where(odd, z, 0.0), np.where(odd, phi, 0.0), T)
+    assert np.abs(oo[~odd]).max() > 1e-3
