@@ -274,6 +274,9 @@ int encore_get_harm_steps(const encore_plan_t *plan, uint64_t *executed /* HOST 
 /* Dependent-DFMA-chain micro-benchmark on the current device: achieved fp64 FLOP/s (FMA = 2) with every SM busy.
  * The ALU roofline denominator reported by bench.py beside the derived 148 SM x 64 lanes x 2 x f_clk. */
 int encore_measure_fp64_peak(double *flops_per_s /* HOST */, void *cuda_stream);
+/* The same for the fp64 tensor-core path, mma.sync.m8n8k4.f64 in independent accumulator chains on every SM (FLOP/s, FMA = 2):
+ * the number that decides whether recasting a contraction as fp64 MMAs could pay. */
+int encore_measure_dmma_peak(double *flops_per_s /* HOST */, void *cuda_stream);
 
 const char *encore_strerror(int status);
 int encore_last_cuda_error(void); /* cudaError_t of the most recent ENCORE_ECUDA on this thread */

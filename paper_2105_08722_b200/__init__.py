@@ -30,7 +30,7 @@ SYMBOLS = [
     "encore_get_bin_tuples", "encore_get_bin_edges", "encore_contraction_flops", "encore_get_contraction_layout", "encore_get_grid",
     "encore_get_cell_ids", "encore_get_bin_counts", "encore_get_primary_counts", "encore_get_alm",
     "encore_get_stage_ms", "encore_get_kernel_ms", "encore_set_timing", "encore_get_launch_count", "encore_get_candidate_pairs", "encore_get_harm_steps",
-    "encore_measure_fp64_peak", "encore_strerror", "encore_last_cuda_error",
+    "encore_measure_fp64_peak", "encore_measure_dmma_peak", "encore_strerror", "encore_last_cuda_error",
 ]
 
 
@@ -88,6 +88,7 @@ def lib():
     L.encore_get_launch_count.argtypes = [vp]
     L.encore_get_candidate_pairs.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.encore_measure_fp64_peak.argtypes = [dp, vp]
+    L.encore_measure_dmma_peak.argtypes = [dp, vp]
     L.encore_get_harm_steps.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.encore_strerror.argtypes = [C.c_int]
     L.encore_strerror.restype = C.c_char_p
@@ -332,6 +333,12 @@ def encore_get_harm_steps(plan):
 def encore_measure_fp64_peak(cuda_stream: int = 0) -> float:
     v = C.c_double()
     _check(lib().encore_measure_fp64_peak(C.byref(v), C.c_void_p(cuda_stream)))
+    return v.value
+
+
+def encore_measure_dmma_peak(cuda_stream: int = 0) -> float:
+    v = C.c_double()
+    _check(lib().encore_measure_dmma_peak(C.byref(v), C.c_void_p(cuda_stream)))
     return v.value
 
 

@@ -1062,6 +1062,33 @@ int encore_measure_fp64_peak(double *flops_per_s, void *cuda_stream)
     return ENCORE_OK;
 }
 
+int encore_measure_dmma_peak(double *flops_per_s, void *cuda_stream)
+{
+    if (!flops_per_s) return ENCORE_EINVAL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    double *sink = nullptr;
+    CU(cudaMalloc((void **)&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int iters = 1024;
+    CU(launch_dmma_peak(sink, 64, s)); // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        CU(cudaEventRecord(e0, s));
+        CU(launch_dmma_peak(sink, iters, s));
+        CU(cudaEventRecord(e1, s));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    const double fmas = 148.0 * 8 * 8 * (double)iters * 32 * 256;   // CTAs x warps x iterations x MMAs per iteration x FMA per MMA
+    *flops_per_s = 2.0 * fmas / (best * 1e-3);
+    return ENCORE_OK;
+}
+
 const char *encore_strerror(int status)
 {
     switch (status) {

@@ -189,6 +189,7 @@ cudaError_t launch_export_alm(const double *alm, const int32_t *cid, const int *
                               const int *group_start, GridGeom g, int nbins, int lmax, int64_t n, int64_t i,
                               double *out_dev, cudaStream_t s);
 cudaError_t launch_fp64_peak(double *sink, int iters, cudaStream_t s);
+cudaError_t launch_dmma_peak(double *sink, int iters, cudaStream_t s);   // 148 * 8 CTAs x 8 warps x iters x 32 MMAs (m8n8k4, 256 FMA each)
 
 // locate the group of cell-sorted slot `s` (shared by diag and contraction kernels)
 __device__ __forceinline__ int find_pencil_of_group(const int *group_start, int npencil, int g)

@@ -85,7 +85,36 @@ __global__ void __launch_bounds__(512) k_fp64_peak(double *sink, int iters)
     if (r == 123.456) sink[0] = r; // never true; keeps the chains alive
 }
 
+// FP64 tensor-core rate ("measure it"): mma.sync.m8n8k4.f64 - the only fp64 MMA sm_100a has (tcgen05 has
+// no fp64 kind) - in 8 independent accumulator chains per warp; one MMA = 8 x 8 x 4 = 256 FMA per warp.
+__global__ void __launch_bounds__(256) k_dmma_peak(double *sink, int iters)
+{
+    double c[8][2];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { c[k][0] = threadIdx.x * 1e-9 + k; c[k][1] = c[k][0] + 0.5; }
+    const double a = 1.0000001, b = 1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                             : "+d"(c[k][0]), "+d"(c[k][1]) : "d"(a), "d"(b));
+        }
+    }
+    double r = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) r += c[k][0] + c[k][1];
+    if (r == 123.456) sink[0] = r; // never true; keeps the chains alive
+}
+
 } // namespace
+
+cudaError_t launch_dmma_peak(double *sink, int iters, cudaStream_t s)
+{
+    k_dmma_peak<<<148 * 8, 256, 0, s>>>(sink, iters);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_sum_bin_counts(const uint32_t *counts, const int *group_start, int npencil, int nbins,
                                   unsigned long long *out, int ngroups_max, cudaStream_t s)
