@@ -392,7 +392,7 @@ def measure_next_rows(E, torch, dev, fp64_peak):
     # the shapes of the paper's Table 2: ~5e4 uniform points in a periodic box L = 1500, N_r = 10 bins up to
     # r_max = 200, 4PCF at lmax = 5 and 10, 5PCF at lmax = 5.  The paper's seconds (16-core Skylake / best P100 row, a_lm on one
     # CPU core) are context from other hardware, quoted beside this run's time; they are not a target and not a ratio.
-    t2 = W.Config("table2", 4, 10, 0.0, 200.0, 5, 1500.0, 50625, 578, "uniform", "unit")
+    t2 = W.TABLE2
     pos, w = W.make(t2)
     tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
     rows = {}

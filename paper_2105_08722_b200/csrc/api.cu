@@ -371,7 +371,7 @@ int compute_device(encore_plan_s *P, const double *pos, const double *w, int64_t
     // ---- a2: counting sort by cell, gather to AoS, groups of 32 per pencil ----------------------------------
     CU(launch_exclusive_scan(P->cell_count.as<int>(), P->cell_start.as<int>(), G.ncell, P->scan_tmp.as<int>(), s, &P->launches));
     CU(cudaMemsetAsync(P->cell_fill.p, 0, sizeof(int) * (size_t)G.ncell, s));
-    CU(launch_sort_gather(pos, w, n, P->cid.as<int32_t>(), P->cell_start.as<int>(), P->cell_fill.as<int>(), P->tmp_idx.as<int>(),
+    CU(launch_sort_gather(pos, w, n, P->cid.as<int32_t>(), P->cell_start.as<int>(), G.ncell, P->cell_fill.as<int>(), P->tmp_idx.as<int>(),
                           P->sorted_idx.as<int>(), P->pos4.as<double4>(), s, &P->launches));
     CU(launch_pencil_groups(P->cell_start.as<int>(), G, P->groups.as<int>(), s, &P->launches));
     CU(launch_exclusive_scan(P->groups.as<int>(), P->group_start.as<int>(), G.npencil, P->scan_tmp.as<int>(), s, &P->launches));

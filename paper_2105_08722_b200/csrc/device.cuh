@@ -67,7 +67,7 @@ cudaError_t launch_cell_ids(const double *pos, int64_t n, GridGeom g, int32_t *c
 // exclusive scan of `in[0..m)` into `out[0..m]` (out[m] = total); tmp needs (m/2048+2) ints; m <= 2048*2048
 cudaError_t launch_exclusive_scan(const int *in, int *out, int m, int *tmp, cudaStream_t s, int *launches);
 cudaError_t launch_sort_gather(const double *pos, const double *w, int64_t n, const int32_t *cid,
-                               const int *cell_start, int *cell_fill, int *tmp_idx, int *sorted_idx,
+                               const int *cell_start, int ncell, int *cell_fill, int *tmp_idx, int *sorted_idx,
                                double4 *pos4, cudaStream_t s, int *launches);
 cudaError_t launch_make_pos4f(const double4 *pos4, int64_t count, const double ctr[3], float4 *pos4f, cudaStream_t s, int *launches);
 cudaError_t launch_pencil_groups(const int *cell_start, GridGeom g, int *groups_per_pencil, cudaStream_t s,

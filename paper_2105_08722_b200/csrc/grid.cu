@@ -6,6 +6,8 @@
 // All HBM-bound, a few tens of bytes per particle.
 #include "device.cuh"
 
+#include <algorithm>
+
 namespace {
 
 constexpr int kThreads = 256;
@@ -159,8 +161,69 @@ __global__ void k_scatter(int64_t n, const int32_t *__restrict__ cid, const int 
     tmp_idx[slot] = (int)i;
 }
 
+// Cells with more particles than this are put in order by k_sort_big_cells; smaller ones by the counting loop of k_rank_gather.
+constexpr int kRankLoopMax = 64;
+constexpr int kBigSortThreads = 1024;
+
+// Sorts a[0..len) ascending with the CTA's threads: a bitonic network whose merges all run in the same direction (the first
+// step of each stage compares mirror images, i with block_end - 1 - i, the others i with i + j), so that elements beyond len
+// act as +infinity without being stored - a compare-exchange whose upper partner is >= len is simply skipped.
+// O(len log^2 len) compare-exchanges in global memory (L2-resident), __syncthreads between steps.
+__device__ void sort_segment_ascending(int *__restrict__ a, int len)
+{
+    int P = 1;
+    while (P < len) P <<= 1;
+    const int half = P >> 1;
+    for (int k = 2; k <= P; k <<= 1) {
+        const int hk = k >> 1;
+        for (int t = threadIdx.x; t < half; t += blockDim.x) {
+            const int blk = t / hk, off = t - blk * hk;
+            const int i = blk * k + off, q = blk * k + k - 1 - off;
+            if (q < len) {
+                const int x = a[i], y = a[q];
+                if (x > y) { a[i] = y; a[q] = x; }
+            }
+        }
+        __syncthreads();
+        for (int j = hk >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < half; t += blockDim.x) {
+                const int i = (t / j) * 2 * j + (t % j), q = i + j;
+                if (q < len) {
+                    const int x = a[i], y = a[q];
+                    if (x > y) { a[i] = y; a[q] = x; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// A dense clump in a coarse cell would make the counting loop of k_rank_gather quadratic in the cell's occupancy.  CTAs sweep the
+// cell table (1024 cells at a time); a cell holding more than kRankLoopMax particles has its slice of tmp_idx sorted by original
+// index, by the whole CTA.  After that a slot of such a cell IS its rank.  On ordinary inputs (c1..c5: <= 40 per cell) this
+// kernel reads cell_start once and sorts nothing.  No list of big cells, no extra buffer, nothing read back.
+__global__ void __launch_bounds__(kBigSortThreads) k_sort_big_cells(const int *__restrict__ cell_start, int ncell, int *__restrict__ tmp_idx)
+{
+    __shared__ int big[kBigSortThreads];
+    __shared__ int nbig;
+    for (int base = blockIdx.x * kBigSortThreads; base < ncell; base += gridDim.x * kBigSortThreads) {
+        if (threadIdx.x == 0) nbig = 0;
+        __syncthreads();
+        const int c = base + threadIdx.x;
+        if (c < ncell && cell_start[c + 1] - cell_start[c] > kRankLoopMax) big[atomicAdd(&nbig, 1)] = c;
+        __syncthreads();
+        const int nb = nbig;
+        for (int k = 0; k < nb; ++k) {      // the order of `big` is arbitrary; every cell is sorted on its own, the result is not
+            const int b = cell_start[big[k]];
+            sort_segment_ascending(tmp_idx + b, cell_start[big[k] + 1] - b);
+        }
+        __syncthreads();
+    }
+}
+
 // Each particle finds its rank inside its cell by counting smaller original indices: the arrival order of the
-// scatter's atomics does not survive.  Cells hold a handful of particles, so this is O(n * occupancy).
+// scatter's atomics does not survive.  Cells hold a handful of particles, so this is O(n * occupancy); cells above
+// kRankLoopMax were sorted by k_sort_big_cells and a slot there is already the rank.
 __global__ void k_rank_gather(int64_t n, const double *__restrict__ pos, const double *__restrict__ w,
                               const int32_t *__restrict__ cid, const int *__restrict__ cell_start,
                               const int *__restrict__ tmp_idx, int *__restrict__ sorted_idx,
@@ -171,8 +234,11 @@ __global__ void k_rank_gather(int64_t n, const double *__restrict__ pos, const d
     const int i = tmp_idx[s];
     const int c = cid[i];
     const int b = cell_start[c], e = cell_start[c + 1];
-    int rank = 0;
-    for (int q = b; q < e; ++q) rank += tmp_idx[q] < i;
+    int rank = (int)s - b;
+    if (e - b <= kRankLoopMax) {
+        rank = 0;
+        for (int q = b; q < e; ++q) rank += tmp_idx[q] < i;
+    }
     const int dst = b + rank;
     sorted_idx[dst] = i;
     pos4[dst] = make_double4(pos[i], pos[n + i], pos[2 * n + i], w ? w[i] : 1.0);
@@ -268,13 +334,15 @@ cudaError_t launch_exclusive_scan(const int *in, int *out, int m, int *tmp, cuda
 }
 
 cudaError_t launch_sort_gather(const double *pos, const double *w, int64_t n, const int32_t *cid,
-                               const int *cell_start, int *cell_fill, int *tmp_idx, int *sorted_idx,
+                               const int *cell_start, int ncell, int *cell_fill, int *tmp_idx, int *sorted_idx,
                                double4 *pos4, cudaStream_t s, int *launches)
 {
     const unsigned nb = (unsigned)((n + kThreads - 1) / kThreads);
     k_scatter<<<nb, kThreads, 0, s>>>(n, cid, cell_start, cell_fill, tmp_idx);
+    const int sweep = std::max(1, std::min(296, (ncell + kBigSortThreads - 1) / kBigSortThreads));   // at most 2 CTAs per SM
+    k_sort_big_cells<<<sweep, kBigSortThreads, 0, s>>>(cell_start, ncell, tmp_idx);
     k_rank_gather<<<nb, kThreads, 0, s>>>(n, pos, w, cid, cell_start, tmp_idx, sorted_idx, pos4);
-    *launches += 2;
+    *launches += 3;
     return cudaGetLastError();
 }
 

@@ -398,6 +398,30 @@ def test_degenerate_inputs(E, oracle):
     check_full(E, oracle, 4, pos, None, 12.0, 1.0, 4.0, 3, 2)
 
 
+@pytest.mark.parametrize("nclump", [700, 50000])
+def test_dense_clump_in_one_cell_is_sorted_not_ranked_quadratically(E, oracle, nclump):
+    """a2: the order inside a cell is by original index.  Cells above 64 particles are sorted by
+    k_sort_big_cells (one CTA, bitonic network) instead of the per-particle counting loop, which is quadratic in the
+    occupancy.  A clump far smaller than a cell, plus a background that gives the bins something to hold: cell ids, counts
+    and zeta against the oracle, identical bits on a second run, and the a2 time printed and bounded."""
+    rng = np.random.default_rng(77 + nclump)
+    clump = 500.0 + rng.uniform(-0.4, 0.4, (3, nclump))
+    back = 500.0 + rng.uniform(-20.0, 20.0, (3, 2000))
+    pos = np.ascontiguousarray(np.concatenate([clump, back], axis=1)[:, rng.permutation(nclump + 2000)])
+    w = rng.uniform(0.5, 1.5, nclump + 2000)
+    check_full(E, oracle, 3, pos, w, 1000.0, 2.0, 8.0, 4, 2)
+    dev = torch.device("cuda:0")
+    tp, tw = torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)
+    with E.Plan(3, 2.0, 8.0, 4, 2, 1000.0) as plan:
+        E.encore_set_timing(plan.h, True)
+        z1 = plan.compute(tp, tw).cpu().numpy()
+        z2 = plan.compute(tp, tw).cpu().numpy()
+        sort_ms = E.encore_get_kernel_ms(plan.h)["sort"]
+    assert np.array_equal(z1, z2)
+    print(f"a2 with {nclump} particles in one cell: {sort_ms:.3f} ms")
+    assert sort_ms < 20.0
+
+
 def test_domain_errors(E):
     dev = torch.device("cuda:0")
     with E.Plan(3, 0.0, 10.0, 3, 2, 100.0) as p:
@@ -493,6 +517,30 @@ def test_full_size_zeta_matches_the_oracle(E, oracle, name):
     if cfg.weights == "unit":   # l = 0 identity from the GPU's own integer counts
         _l0_identity(E, g["plan"], cfg, g["zeta"], (np.ones(cfg.n), g["prim_counts"].astype(np.float64)))
     g["plan"].close()
+
+
+def test_paper_table2_4pcf_lmax10_against_the_golden_oracle_run(E):
+    """The input of the paper's Table 2 (~5e4 uniform points, periodic L = 1500, 10 bins to 200) with the
+    paper's largest 4PCF GPU shape, lmax = 10: 381 multiplets x 120 bin triples = 45 720 outputs - the
+    launch configuration of bench.py's `next_rows.paper_table2_shapes.4pcf_lmax10`.  Every element against the oracle's run
+    stored in tests/golden/ (written by tests/golden/make_golden.py from oracle/ and workloads/ only; 278 s on 8 threads)."""
+    cfg = W.EXTRA["table2_4pcf_lmax10"]
+    pos, w = W.make(cfg)
+    gold = np.load(os.path.join(GOLDEN, "table2_4pcf_lmax10_oracle.npz"))
+    assert str(gold["digest"]) == W.digest(pos, w), "tests/golden/table2_4pcf_lmax10_oracle.npz was written for other input bytes"
+    dev = torch.device("cuda:0")
+    with E.Plan(cfg.order, cfg.rmin, cfg.rmax, cfg.nbins, cfg.lmax, cfg.box) as plan:
+        assert (plan.n_lambda, plan.n_b) == (381, 120)
+        lay = E.encore_get_contraction_layout(plan.h)
+        assert lay["kernel"] == 4 and lay["nbuf_min"] == 1          # the heaviest CTAs refill a single tile buffer
+        z = plan.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+        assert E.encore_get_status(plan.h) == E.OK
+        counts, pairs = E.encore_get_bin_counts(plan.h, cfg.nbins)
+    assert (counts == gold["bin_counts"]).all() and pairs == int(gold["bin_counts"].sum())
+    scale = np.abs(gold["zeta"]).max()
+    err = np.abs(z - gold["zeta"]).max() / scale
+    print(f"table 2, 4PCF lmax 10: zeta rel-to-max error {err:.3e} over {z.size} elements, pairs {pairs}")
+    assert err <= TOL
 
 
 @pytest.mark.slow

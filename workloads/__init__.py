@@ -49,6 +49,13 @@ CONFIGS = {
 }
 
 
+# The input of the paper's Table 2: ~5e4 uniform points in a periodic box L = 1500, N_r = 10 bins up to
+# r_max = 200.  Not a BASELINE.json config: bench.py's `next_rows.paper_table2_shapes` times it, tests/golden/ holds the
+# oracle's 4PCF lmax = 10 run of it (the paper's largest 4PCF GPU shape: 381 multiplets x 120 bin triples).
+TABLE2 = Config("table2", 4, 10, 0.0, 200.0, 5, 1500.0, 50625, 578, "uniform", "unit")
+EXTRA = {"table2_4pcf_lmax10": dataclasses.replace(TABLE2, name="table2_4pcf_lmax10", lmax=10)}
+
+
 def scaled(cfg: Config, box: float | None = None, n: int | None = None,
            grid: int | None = None, name: str | None = None) -> Config:
     """Same recipe at a reduced size (parity-test cases the oracle finishes in seconds).
